@@ -1,0 +1,191 @@
+"""Seeded synthetic workloads: lattice bond lists, couplings and T grid.
+
+This module is the ONLY code shared by the CUDA path's tests/bench and the CPU
+oracle's tests.  It holds no arithmetic of the method (no Hamiltonian action, no
+index map, no Lanczos): only graph definitions ("the N_B bonds
+<i,j> of the cluster graph"), the bond couplings J_b, and the temperature grid of
+BASELINE.json config 1.  It imports neither `oracle/` nor the CUDA binding.
+
+Site numbering conventions follow SURVEY.md section 8(d) (the paper gives lattice
+names only; any fixed numbering is the same physics, reading 30).
+Every workload is generated from its definition; nothing is read from disk.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+SEED_VECTORS = 20260526   # start-vector seed used by tests and bench
+SEED_J = 1234             # random-bond seed (config 4b)
+
+_M64 = (1 << 64) - 1
+
+
+def _mix64(x: int) -> int:
+    """Plain 64-bit integer finaliser (xor-shift-multiply); input generator only."""
+    x &= _M64
+    x = ((x ^ (x >> 30)) * 0xBF58476D1CE4E5B9) & _M64
+    x = ((x ^ (x >> 27)) * 0x94D049BB133111EB) & _M64
+    return x ^ (x >> 31)
+
+
+@dataclass
+class Workload:
+    name: str
+    N: int
+    bond_i: np.ndarray          # int32 [N_B], bond_i < bond_j
+    bond_j: np.ndarray          # int32 [N_B]
+    J: np.ndarray               # float64 [N_B]
+    h: float = 0.0
+    sectors: list = field(default_factory=list)   # N_up values computed (M_z >= 0)
+    R: int = 1
+    n_steps: int = 1
+    note: str = ""
+
+    @property
+    def n_bonds(self) -> int:
+        return int(self.bond_i.shape[0])
+
+    def dim(self, n_up: int) -> int:
+        return math.comb(self.N, n_up)
+
+
+def _mk(name, N, pairs, J=None, **kw) -> Workload:
+    pairs = [(min(a, b), max(a, b)) for a, b in pairs]
+    bi = np.array([p[0] for p in pairs], dtype=np.int32)
+    bj = np.array([p[1] for p in pairs], dtype=np.int32)
+    if J is None:
+        J = np.ones(len(pairs), dtype=np.float64)
+    return Workload(name, N, bi, bj, np.asarray(J, dtype=np.float64), **kw)
+
+
+def dimer() -> Workload:
+    return _mk("dimer", 2, [(0, 1)], sectors=[1, 2])
+
+
+def ring(N: int, J1: float = 1.0, J2: float | None = None, **kw) -> Workload:
+    """Periodic chain; bonds (i, i+1 mod N), optionally (i, i+2 mod N) with J2."""
+    if N == 2:
+        pairs, J = [(0, 1)], [J1]
+    else:
+        pairs = [(i, (i + 1) % N) for i in range(N)]
+        J = [J1] * N
+        if J2 is not None:
+            pairs += [(i, (i + 2) % N) for i in range(N)]
+            J += [J2] * N
+    kw.setdefault("sectors", list(range((N + 1) // 2, N + 1)))
+    return _mk(f"ring{N}" + ("_j1j2" if J2 is not None else ""), N, pairs, J, **kw)
+
+
+def square(Lx: int, Ly: int, **kw) -> Workload:
+    """Periodic square lattice, site x + Lx*y, bonds to (x+1, y) and (x, y+1)."""
+    s = lambda x, y: (x % Lx) + Lx * (y % Ly)
+    pairs = []
+    for y in range(Ly):
+        for x in range(Lx):
+            pairs.append((s(x, y), s(x + 1, y)))
+            pairs.append((s(x, y), s(x, y + 1)))
+    N = Lx * Ly
+    kw.setdefault("sectors", list(range((N + 1) // 2, N + 1)))
+    return _mk(f"square{Lx}x{Ly}", N, pairs, **kw)
+
+
+def triangular(Lx: int, Ly: int, **kw) -> Workload:
+    """Periodic triangular lattice, site x + Lx*y, bonds (x+1,y), (x,y+1), (x+1,y+1)."""
+    s = lambda x, y: (x % Lx) + Lx * (y % Ly)
+    pairs = []
+    for y in range(Ly):
+        for x in range(Lx):
+            pairs.append((s(x, y), s(x + 1, y)))
+            pairs.append((s(x, y), s(x, y + 1)))
+            pairs.append((s(x, y), s(x + 1, y + 1)))
+    N = Lx * Ly
+    kw.setdefault("sectors", [N // 2])
+    return _mk(f"triangular{Lx}x{Ly}", N, pairs, **kw)
+
+
+def _icosahedron_vertices():
+    phi = (1.0 + math.sqrt(5.0)) / 2.0
+    V = []
+    for perm in range(3):                 # cyclic permutations of (0, +-1, +-phi)
+        for s1 in (1.0, -1.0):
+            for s2 in (1.0, -1.0):
+                base = (0.0, s1, s2 * phi)
+                V.append(tuple(base[(k - perm) % 3] for k in range(3)))
+    return V
+
+
+def _icosahedron_edges():
+    V = _icosahedron_vertices()
+    E = []
+    for a in range(12):
+        for b in range(a + 1, 12):
+            d2 = sum((V[a][k] - V[b][k]) ** 2 for k in range(3))
+            if abs(d2 - 4.0) < 1e-9:
+                E.append((a, b))
+    assert len(E) == 30
+    return V, sorted(E)
+
+
+def icosahedron(**kw) -> Workload:
+    """N=12 icosahedron, N_B=30 (Table 1)."""
+    _, E = _icosahedron_edges()
+    kw.setdefault("sectors", list(range(6, 13)))
+    return _mk("icosahedron", 12, E, **kw)
+
+
+def icosidodecahedron(random_bonds: bool = False, seed_J: int = SEED_J, **kw) -> Workload:
+    """N=30: sites = the 30 icosahedron edges in lexicographic order; two sites are
+    bonded iff their edges lie on a common triangular face (edge midpoints at distance
+    1).  60 bonds, every site has degree 4.  random_bonds: J_b uniform in [0.5, 1.5]
+    from the counter-based generator, bond b in list order (BASELINE config 4b)."""
+    V, E = _icosahedron_edges()
+    mid = [tuple((V[a][k] + V[b][k]) / 2.0 for k in range(3)) for a, b in E]
+    pairs = []
+    for a in range(30):
+        for b in range(a + 1, 30):
+            d2 = sum((mid[a][k] - mid[b][k]) ** 2 for k in range(3))
+            if abs(d2 - 1.0) < 1e-9:
+                pairs.append((a, b))
+    assert len(pairs) == 60
+    J = None
+    if random_bonds:
+        J = [0.5 + (_mix64(_mix64(seed_J) + 0x9E3779B97F4A7C15 * (b + 1)) >> 11) * 2.0 ** -53
+             for b in range(60)]
+    kw.setdefault("sectors", [15])
+    return _mk("icosidodecahedron" + ("_randJ" if random_bonds else ""), 30, pairs, J, **kw)
+
+
+def relabel(w: Workload, perm) -> Workload:
+    """Renumber sites: old site s becomes perm[s].  Same physics (reading 30)."""
+    perm = np.asarray(perm, dtype=np.int64)
+    assert sorted(perm.tolist()) == list(range(w.N))
+    a, b = perm[w.bond_i], perm[w.bond_j]
+    return Workload(w.name + "_relabel", w.N, np.minimum(a, b).astype(np.int32),
+                    np.maximum(a, b).astype(np.int32), w.J.copy(), w.h, list(w.sectors),
+                    w.R, w.n_steps, w.note)
+
+
+def baseline_config(k: int) -> Workload:
+    """The five BASELINE.json configs, k = 1..5 (k = 40 is config 4's random-bond variant)."""
+    if k == 1:
+        return ring(16, R=20, n_steps=60, note="N=16 ring, all S^z sectors, FP64+FP32")
+    if k == 2:
+        return square(4, 6, R=50, n_steps=100, note="4x6 square PBC, all sectors, FP32 CLT")
+    if k == 3:
+        return triangular(4, 7, R=20, n_steps=100, note="4x7 triangular PBC, S^z=0")
+    if k == 4:
+        return icosidodecahedron(False, R=10, n_steps=100, note="icosidodecahedron S^z=0, D=155117520")
+    if k == 40:
+        return icosidodecahedron(True, R=10, n_steps=100, note="icosidodecahedron random J_b")
+    if k == 5:
+        return ring(34, 1.0, 0.5, sectors=[17], R=2, n_steps=80, note="N=34 J1-J2 ring S^z=0, CR only")
+    raise ValueError(k)
+
+
+def temperature_grid(n: int = 200, lo: float = 0.05, hi: float = 10.0) -> np.ndarray:
+    """T_i = lo*(hi/lo)^(i/(n-1)), both ends included (BASELINE config 1; reading 19)."""
+    i = np.arange(n, dtype=np.float64)
+    return lo * (hi / lo) ** (i / (n - 1))

@@ -1,0 +1,168 @@
+"""Pins for the oracle's Hamiltonian (O2): closed-form spectra (dimer, 4-ring), the full-space
+Kronecker-product construction for N <= 12, Table 1's N_nz, the sector-trace closed form,
+symmetry, [H, S^2] = 0, SU(2) spectrum nesting, the Zeeman shift.  CPU only."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import ftlm_oracle as fo
+from oracle import c_oracle as co
+from paper_2605_26261_b200 import workloads as W
+
+
+def _dense(w, N_up, h=0.0, J=None):
+    return fo.dense_H(w.N, w.bond_i, w.bond_j, w.J if J is None else J, h, N_up)
+
+
+def test_ladder_coefficients_spin_half_reduce_to_J_over_2():
+    # reading 6: Eqs. 13-14 at s = 1/2
+    J = 1.7
+    for mi in (-0.5, 0.5):
+        for mj in (-0.5, 0.5):
+            cp, cm = fo.ladder_coeffs(J, mi, mj)
+            if mi == mj:
+                assert cp == 0.0 and cm == 0.0
+            else:
+                assert sorted([cp, cm]) == pytest.approx([0.0, J / 2])
+
+
+def test_dimer_spectrum():
+    w = W.dimer()
+    J = np.array([1.3])
+    assert np.linalg.eigvalsh(_dense(w, 1, J=J)) == pytest.approx([-0.75 * 1.3, 0.25 * 1.3])
+    assert _dense(w, 2, J=J) == pytest.approx(np.array([[0.25 * 1.3]]))
+    assert _dense(w, 0, J=J) == pytest.approx(np.array([[0.25 * 1.3]]))
+
+
+def test_four_ring_spectrum():
+    # H = (J/2)[S^2 - S_13^2 - S_24^2]
+    w = W.ring(4)
+    assert np.linalg.eigvalsh(_dense(w, 2)) == pytest.approx([-2, -1, 0, 0, 0, 1], abs=1e-12)
+    for n_up in (1, 3):
+        assert np.linalg.eigvalsh(_dense(w, n_up)) == pytest.approx([-1, 0, 0, 1], abs=1e-12)
+    for n_up in (0, 4):
+        assert np.linalg.eigvalsh(_dense(w, n_up)) == pytest.approx([1.0])
+
+
+@pytest.mark.parametrize("wl", ["ring8", "randgraph9", "icosahedron"])
+def test_sector_blocks_equal_full_space_kronecker_hamiltonian(wl):
+    rng = np.random.default_rng(3)
+    if wl == "ring8":
+        w = W.ring(8, 1.0, 0.4)
+        h = 0.3
+    elif wl == "randgraph9":
+        N = 9
+        pairs = [(a, b) for a in range(N) for b in range(a + 1, N) if rng.random() < 0.45]
+        w = W._mk("rand9", N, pairs, rng.uniform(-1.0, 1.5, len(pairs)))
+        h = -0.7
+    else:
+        w = W.icosahedron()
+        h = 0.0
+    Hf = fo.full_space_H_kron(w.N, w.bond_i, w.bond_j, w.J, h)
+    assert np.abs(Hf - Hf.T).max() == 0.0
+    seen = 0
+    for n_up in range(w.N + 1):
+        basis = fo.sector_basis(w.N, n_up).astype(np.int64)
+        Hs = fo.dense_H(w.N, w.bond_i, w.bond_j, w.J, h, n_up)
+        assert np.abs(Hf[np.ix_(basis, basis)] - Hs).max() < 1e-13
+        seen += np.count_nonzero(Hf[np.ix_(basis, basis)])
+    assert seen == np.count_nonzero(Hf)          # S^z conserved: nothing outside the blocks
+
+
+def test_apply_H_matches_dense_and_c_oracle():
+    rng = np.random.default_rng(11)
+    w = W.ring(12, 1.0, 0.5)
+    J = rng.uniform(0.5, 1.5, w.n_bonds)
+    for n_up in (6, 7, 11, 12):
+        basis = fo.sector_basis(w.N, n_up)
+        v = rng.standard_normal(basis.shape[0])
+        Hd = fo.dense_H(w.N, w.bond_i, w.bond_j, J, 0.2, n_up)
+        y = fo.apply_H(basis, w.N, w.bond_i, w.bond_j, J, 0.2, n_up, v)
+        assert np.abs(y - Hd @ v).max() < 1e-13
+        yc = co.apply_rows(w.N, w.bond_i, w.bond_j, J, 0.2, n_up, basis, v)
+        assert np.abs(yc - Hd @ v).max() < 1e-13
+
+
+def test_table1_nnz_icosahedron(golden_paper):
+    w = W.icosahedron()
+    H = _dense(w, 6)
+    assert H.shape[0] == int(golden_paper["table1_D0"])
+    # structural count: one diagonal entry per row + one entry per antiparallel bond
+    basis = fo.sector_basis(12, 6)
+    nb = fo.neighbor_indices(basis, w.bond_i, w.bond_j, np.arange(basis.shape[0]))
+    assert basis.shape[0] + int((nb >= 0).sum()) == int(golden_paper["table1_Nnz"])
+    assert np.count_nonzero(H - np.diag(np.diag(H))) == int(golden_paper["table1_Nnz"]) - 924
+
+
+def test_sector_trace_closed_form():
+    # Tr_sector H = (sum_b J_b / 4) [C(N-2,N_up-2) + C(N-2,N_up) - 2 C(N-2,N_up-1)]
+    def c(n, k):
+        return math.comb(n, k) if 0 <= k <= n else 0
+    w = W.icosahedron()
+    assert np.trace(_dense(w, 6)) == pytest.approx(-630.0)
+    rng = np.random.default_rng(2)
+    w2 = W.ring(10, 1.0, 0.5)
+    J = rng.uniform(0.5, 1.5, w2.n_bonds)
+    for n_up in range(11):
+        expect = J.sum() / 4 * (c(8, n_up - 2) + c(8, n_up) - 2 * c(8, n_up - 1))
+        assert np.trace(_dense(w2, n_up, J=J)) == pytest.approx(expect, abs=1e-10)
+
+
+def test_max_eigenvalue_is_ferromagnetic_energy():
+    # for J_b > 0 the top of every sector's spectrum is sum_b J_b / 4 (the S = N/2 multiplet)
+    w = W.ring(10, 1.0, 0.5)
+    for n_up in range(11):
+        assert np.linalg.eigvalsh(_dense(w, n_up))[-1] == pytest.approx(w.J.sum() / 4)
+
+
+def test_commutes_with_total_spin_and_su2_nesting():
+    w = W.icosahedron()
+    N = w.N
+    # S^2 = 3N/4 + 2 sum_{i<j} s_i.s_j : the same operator code on the complete graph, J = 2
+    ci = np.array([a for a in range(N) for b in range(a + 1, N)], dtype=np.int32)
+    cj = np.array([b for a in range(N) for b in range(a + 1, N)], dtype=np.int32)
+    prev = None
+    for n_up in (6, 7, 8):
+        H = _dense(w, n_up)
+        S2 = fo.dense_H(N, ci, cj, np.full(len(ci), 2.0), 0.0, n_up) + 0.75 * N * np.eye(H.shape[0])
+        assert np.abs(H @ S2 - S2 @ H).max() < 1e-11
+        ev = np.linalg.eigvalsh(H)
+        if prev is not None:            # spectrum of sector M_z+1 is contained in sector M_z
+            for e in ev:
+                assert np.abs(prev - e).min() < 1e-9
+        prev = ev
+    # +M_z and -M_z have identical spectra (L32)
+    assert np.linalg.eigvalsh(_dense(w, 4)) == pytest.approx(np.linalg.eigvalsh(_dense(w, 8)), abs=1e-10)
+
+
+def test_zeeman_shift_is_minus_h_Mz():
+    w = W.ring(8)
+    for n_up in (3, 4, 6):
+        e0 = np.linalg.eigvalsh(_dense(w, n_up))
+        e1 = np.linalg.eigvalsh(_dense(w, n_up, h=0.37))
+        assert e1 - e0 == pytest.approx(-0.37 * (n_up - 4) * np.ones_like(e0), abs=1e-12)
+
+
+def test_matrix_free_symmetry_at_larger_N():
+    # <u, H v> = <H u, v> at a size with no dense matrix (C oracle, N = 20)
+    w = W.ring(20, 1.0, 0.5)
+    basis = co.enumerate_basis(20, 10)
+    rng = np.random.default_rng(7)
+    u, v = rng.standard_normal(basis.shape[0]), rng.standard_normal(basis.shape[0])
+    Hv = co.apply_rows(20, w.bond_i, w.bond_j, w.J, 0.0, 10, basis, v)
+    Hu = co.apply_rows(20, w.bond_i, w.bond_j, w.J, 0.0, 10, basis, u)
+    assert abs(u @ Hv - Hu @ v) < 1e-9 * abs(u @ Hv)
+
+
+def test_config1_ground_state_energy_by_lanczos_agrees_with_dense():
+    # N=16 ring S^z=0: E0 from dense eigvalsh of the 12 870-dim sector is too slow for CI;
+    # instead pin the C-oracle Lanczos extremal Ritz value at N=12 against dense ED.
+    w = W.ring(12)
+    basis = co.enumerate_basis(12, 6)
+    q1 = fo.start_vector(1, 6, 0, basis.shape[0])
+    a, b = co.lanczos(12, w.bond_i, w.bond_j, w.J, 0.0, 6, basis, q1, 80)
+    th, _ = fo.ritz(a, b)
+    ev = np.linalg.eigvalsh(_dense(w, 6))
+    assert th[0] == pytest.approx(ev[0], abs=1e-9)
+    assert th[-1] <= w.J.sum() / 4 + 1e-9
