@@ -1,0 +1,167 @@
+/* ftlm.h - C ABI of the B200-native FTLM hot path (arxiv/paper_2605_26261, PAPER.md).
+ *
+ * What the library computes: the matrix-free, row-wise gather y = H v (Eq. 12,
+ * L97-L109) of the spin-1/2 Heisenberg Hamiltonian H = sum_b J_b s_i.s_j - h sum_i s^z_i
+ * (Eq. 1; per-bond J_b and the Zeeman term are DESIGN.md readings 4-5) restricted to
+ * one S^z sector, the state-to-index map it needs in two forms - the compressed lookup table
+ * "CLT" (L148-L183, Alg. 2) and combinatorial ranking "CR" (L121-L146, Alg. 1) - fused with
+ * the Lanczos recursion it drives (L45), plus the host-side tridiagonal eigensolve and FTLM
+ * trace assembly (Eqs. 4-9).
+ *
+ * Conventions
+ *  - Bit k of a label = 1 <=> site k up (Eq. 11); N_up = N/2 + M_z (Eq. 17).
+ *  - Sector basis = labels with popcount N_up in ascending order; indices are 0-based
+ *    int64_t, labels uint64_t; "not in the sector" = -1 (Alg. 2 step 2).
+ *  - Every function returns FTLM_OK (0) or a positive error code; nothing throws across the
+ *    ABI; ftlm_last_error() gives the thread-local message of the last failure.
+ *  - "d_" arguments are DEVICE pointers, "h_" arguments (and all plain arrays of
+ *    ftlm_create / ftlm_thermo / ftlm_tridiag_eig) are HOST pointers.  The library never
+ *    takes ownership of a caller buffer.  Vectors hold ftlm_dim() elements of the handle's
+ *    precision (float or double), densely packed.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls
+ *    documented "asynchronous" only enqueue work on it.
+ *  - One GPU per handle.  There is no CPU fallback: without a CUDA device every device call
+ *    fails with FTLM_ECUDA.
+ */
+#ifndef FTLM_H
+#define FTLM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ftlm_ctx ftlm_ctx;
+
+enum { FTLM_OK = 0, FTLM_EINVAL = 1, FTLM_ENOMEM = 2, FTLM_ECUDA = 3, FTLM_EUNSUPPORTED = 4 };
+enum { FTLM_INDEX_CLT = 0, FTLM_INDEX_CR = 1 };
+enum { FTLM_FP32 = 0, FTLM_FP64 = 1 };
+
+/* Kernel variants selectable with ftlm_set_option("kernel", ...).
+ * ROW  = one thread per row, every row unranked, per-bond loop (the paper's launch shape, L105,
+ *        L136, L203), kept as the plain in-library baseline.
+ * TILE = B200 design: one CTA per run of rows sharing the high label bits. */
+enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_TILE = 2 };
+
+/* ---- handle ------------------------------------------------------------------------------ */
+
+/* Build the sector tables on `device` (A0/A1 of SURVEY 8(a)): binomials C(n,k) (= D_c of
+ * Eq. 16 at d = 2), bond masks and couplings, and in CLT mode the table of (M_b, C_b) pairs of
+ * L150-L154 / Eq. 18.  All array arguments are host pointers and are copied.
+ *   N in [1, 62]; 0 <= bond_i[b] != bond_j[b] < N (duplicates are legal and add); N_up in
+ *   [0, N]; n_bonds in [0, 4096].  CLT needs N <= 32.
+ * Errors: FTLM_EINVAL (bad argument), FTLM_EUNSUPPORTED (CLT with N > 32),
+ *         FTLM_ENOMEM (table does not fit), FTLM_ECUDA (no device / CUDA failure). */
+int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bond_i, const int32_t* bond_j,
+                const double* J, double h, int N_up, int index_mode, int precision, int device);
+
+/* Free the handle and everything it owns (tables, chain workspace).  NULL is accepted. */
+int ftlm_destroy(ftlm_ctx* ctx);
+
+/* Sector dimension C(N, N_up). */
+int64_t ftlm_dim(const ftlm_ctx* ctx);
+
+/* Options: "kernel" (FTLM_KERNEL_*), "low_bits" (w of the TILE kernels, 0 = auto),
+ * "graph" (1 = replay Lanczos steps from a CUDA graph).  FTLM_EINVAL on unknown key/value. */
+int ftlm_set_option(ftlm_ctx* ctx, const char* key, int64_t value);
+int64_t ftlm_get_option(const ftlm_ctx* ctx, const char* key);
+
+/* Bytes of index-table memory on the device (CLT: 8*ceil(2^N/32), Eq. 21; CR: the small tables). */
+int64_t ftlm_table_bytes(const ftlm_ctx* ctx);
+
+/* Copy CLT blocks [b0, b0+nb) to host arrays (test hook for A1).  FTLM_EINVAL in CR mode. */
+int ftlm_clt_read(ftlm_ctx* ctx, int64_t b0, int64_t nb, uint32_t* h_mask, uint32_t* h_count);
+
+/* ---- index maps (L0) --------------------------------------------------------------------- */
+
+/* d_idx[k] = sector index of d_labels[k] with the handle's index mode, -1 if the label is not
+ * in the sector (CLT: Alg. 2; CR: Alg. 1).  Asynchronous. */
+int ftlm_index_of(ftlm_ctx* ctx, const uint64_t* d_labels, int64_t n, int64_t* d_idx, void* stream);
+
+/* d_labels[k] = label of sector index d_idx[k] (the inverse map, L136); indices outside
+ * [0, dim) give UINT64_MAX.  Asynchronous. */
+int ftlm_state_of(ftlm_ctx* ctx, const int64_t* d_idx, int64_t n, uint64_t* d_labels, void* stream);
+
+/* d_idx[(r*n_bonds + b)] for rows row0 <= row0+r < row0+nrows: index of the source state that
+ * bond b couples row row0+r to (the "lookup[n_ij]" of Eq. 12), or -1 if the bond's spins are
+ * parallel.  Computed by the SAME device code path as the H.v kernel selected by "kernel".
+ * Asynchronous. */
+int ftlm_neighbors(ftlm_ctx* ctx, int64_t row0, int64_t nrows, int64_t* d_idx, void* stream);
+
+/* ---- Hamiltonian action (L1) ------------------------------------------------------------- */
+
+/* y = H v (Eq. 12).  d_v, d_y: dim elements of the handle's precision, d_y != d_v and
+ * non-overlapping.  Asynchronous on `stream`. */
+int ftlm_apply_H(ftlm_ctx* ctx, const void* d_v, void* d_y, void* stream);
+
+/* Host-buffer variant: copies h_v to the device, applies H, copies y back; synchronous. */
+int ftlm_apply_H_host(ftlm_ctx* ctx, const void* h_v, void* h_y);
+
+/* ---- start vectors ----------------------------------------------------------------------- */
+
+/* d_v = normalised Gaussian start vector r of this sector under `seed`: the counter-based
+ * generator specified in DESIGN.md section 4 (element t depends only on seed, N_up, r, t);
+ * generated and normalised in FP64, rounded once to the handle's precision.  Asynchronous. */
+int ftlm_fill_random(ftlm_ctx* ctx, uint64_t seed, int r, void* d_v, void* stream);
+
+/* ---- fused Lanczos chain (L2) ------------------------------------------------------------ */
+
+/* Begin a chain: q_1 = d_q1 (copied; need not be normalised) or, if d_q1 == NULL, the seeded
+ * vector ftlm_fill_random(seed, r).  Allocates the handle's three work vectors on first use.
+ * Asynchronous. */
+int ftlm_chain_begin(ftlm_ctx* ctx, const void* d_q1, uint64_t seed, int r, void* stream);
+
+/* Enqueue `nsteps` more fused Lanczos steps (L45): per step one fused
+ * H.v pass  y = H q_j - beta_{j-1} q_{j-1}  with FP64-accumulated <q,y>, <y,y>, <q,q>, and one
+ * pass q_{j+1} = (y - alpha_j q_j)/beta_j.  alpha, beta stay on the device; after a breakdown
+ * (beta_j <= tol*max(|alpha_k|, beta_k), tol = 1e-5 FP32 / 1e-12 FP64) or once min(n, dim)
+ * steps are done the remaining launches are no-ops.  At most FTLM_MAX_STEPS per chain.
+ * Asynchronous. */
+int ftlm_chain_steps(ftlm_ctx* ctx, int nsteps, void* stream);
+
+/* Synchronise `stream` and copy out the coefficients: alpha[0..m_eff), beta[0..m_eff-1).
+ * `cap` = capacity of h_alpha (and of h_beta).  h_m_eff receives the number of steps done. */
+int ftlm_chain_end(ftlm_ctx* ctx, double* h_alpha, double* h_beta, int cap, int* h_m_eff, void* stream);
+
+/* Run `nsteps` steps with CUDA events around every kernel and return the average device time
+ * (ms) of the fused H.v kernel and of the normalisation kernel.  Synchronous; for bench.py. */
+int ftlm_chain_profile(ftlm_ctx* ctx, int nsteps, void* stream, double* ms_hv, double* ms_norm);
+
+#define FTLM_MAX_STEPS 1024
+
+/* Whole sector: R chains from seeded starts r = 0..R-1, n_steps each, then the Ritz pairs.
+ * Host outputs (caller-owned): alpha[R][n_steps], beta[R][n_steps], m_eff[R],
+ * theta[R][n_steps], weight[R][n_steps] (weight = s_{k,1}^2, L45); entries beyond m_eff[r] are
+ * zero.  theta/weight may be NULL.  Synchronous. */
+int ftlm_lanczos(ftlm_ctx* ctx, uint64_t seed, int R, int n_steps, double* h_alpha, double* h_beta,
+                 int* h_m_eff, double* h_theta, double* h_weight, void* stream);
+
+/* Same with caller-provided HOST start vectors h_q1[R][dim] (handle precision): each is copied
+ * host->device inside the call (end-to-end path of bench.py). */
+int ftlm_lanczos_host(ftlm_ctx* ctx, const void* h_q1, int R, int n_steps, double* h_alpha,
+                      double* h_beta, int* h_m_eff, double* h_theta, double* h_weight, void* stream);
+
+/* ---- host-only parts (A8, A9) ------------------------------------------------------------ */
+
+/* Eigenvalues theta[m] (ascending) of the symmetric tridiagonal T(alpha[m], beta[m-1]) and
+ * weights weight[k] = (first component of the normalised eigenvector k)^2 (L45).  FP64. */
+int ftlm_tridiag_eig(int m, const double* alpha, const double* beta, double* theta, double* weight);
+
+/* FTLM trace assembly, Eqs. 7-9 (L61-L74).  Sector s has dim[s], magnetisation Mz[s],
+ * multiplicity mult[s] (2 for M_z > 0, reading 15), R[s] chains; chain c of sector s has
+ * m_eff[off+c] Ritz pairs stored at theta/weight[(off+c)*stride ...], off = sum of R over
+ * earlier sectors.  Outputs per temperature T[i]: E_ref (scalar, = min theta),
+ * Zs = Z*exp(E_ref/T), E = <H>, C = (<H^2>-<H>^2)/T^2, chi = g^2 sum Mz^2 Z_M/(T sum Z_M). */
+int ftlm_thermo(int n_sec, const int64_t* dim, const double* Mz, const double* mult, const int* R,
+                int stride, const int* m_eff, const double* theta, const double* weight, int nT,
+                const double* T, double g, double* E_ref, double* Zs, double* E, double* C,
+                double* chi);
+
+const char* ftlm_last_error(void);
+const char* ftlm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FTLM_H */

@@ -1,0 +1,173 @@
+// Internal definitions shared by the CUDA translation units of libftlm (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/ftlm.h"
+
+#define FTLM_MAX_BONDS 4096
+
+void ftlm_set_error(const char* fmt, ...);
+int ftlm_cuda_fail(cudaError_t e, const char* what);
+
+#define CK(call)                                                   \
+  do {                                                             \
+    cudaError_t e__ = (call);                                      \
+    if (e__ != cudaSuccess) return ftlm_cuda_fail(e__, #call);     \
+  } while (0)
+
+// Device-resident scalars of one Lanczos chain (never read by the host between steps).
+struct ChainState {
+  double alpha[FTLM_MAX_STEPS];
+  double beta[FTLM_MAX_STEPS];
+  double scale;      // max_k(|alpha_k|, beta_k) so far (breakdown rule, reading 10)
+  double beta_prev;  // beta_{j-1} used by the next fused H.v pass
+  double a;          // alpha_j for the normalisation pass
+  double inv_b;      // 1/beta_j for the normalisation pass
+  double tol;
+  double norm2;      // scratch: sum of squares (start-vector normalisation)
+  int step;          // completed steps (= number of alphas stored)
+  int limit;         // m = min(requested, dim)  (reading 9)
+  int done;          // 1 after breakdown or once `limit` steps are done
+  int pad;
+};
+
+struct BondDev {          // one bond as the kernels see it
+  uint64_t mask;          // (1<<i) | (1<<j)
+  double Jh;              // J_b / 2   (off-diagonal element on an antiparallel bond)
+  double Jq;              // J_b / 4
+  int i, j;               // i < j
+};
+
+// Run-tiled ("TILE") kernel plan, built on the host in ftlm_create.
+struct TilePlan;
+
+struct ftlm_ctx {
+  int N = 0, nb = 0, N_up = 0, mode = 0, prec = 0, device = 0;
+  double h = 0.0;
+  int64_t dim = 0;
+  bool idx64 = false;     // indices need 64 bits (dim >= 2^32)
+  bool lab64 = false;     // labels need 64 bits (N > 32)
+  double diag0 = 0.0;     // sum_b J_b/4 - h*M_z : diagonal if every bond were parallel
+  int sm_count = 148;
+
+  // device tables
+  uint64_t* d_binom64 = nullptr;   // [(N+1)][(N_up+1)] : C(p, a), exact
+  uint32_t* d_binom32 = nullptr;   // same, saturated at 2^32-1 (used when !idx64)
+  BondDev* d_bonds = nullptr;
+  uint2* d_clt = nullptr;          // {M_b, C_b}
+  int64_t n_clt = 0;
+  std::vector<BondDev> bonds;
+  std::vector<uint64_t> binom64;   // host copy
+
+  // options
+  int kernel = FTLM_KERNEL_AUTO;
+  int low_bits = 0;
+  int use_graph = 0;
+
+  // tile plan (ftlm_tile.cu)
+  TilePlan* tile = nullptr;
+
+  // chain workspace
+  void* q[3] = {nullptr, nullptr, nullptr};
+  int cur = 0;                     // q[cur] = q_j, q[(cur+2)%3] = q_{j-1}, q[(cur+1)%3] = y
+  ChainState* d_state = nullptr;
+  double* d_partials = nullptr;    // [3][max_blocks]
+  unsigned int* d_ticket = nullptr;
+  int max_blocks = 0;
+  int steps_enqueued = 0;
+  int chain_limit = 0;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+};
+
+size_t ftlm_elem_size(const ftlm_ctx* c);
+int ftlm_effective_kernel(const ftlm_ctx* c);
+
+// ---- launches implemented in the kernel translation units -------------------------------
+// fused == 0: y = H v.   fused == 1: y = H q - beta_prev q_prev with the three FP64 sums and
+// the in-kernel finalisation of alpha_j, beta_j into ctx->d_state.
+int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
+int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
+
+int ftlm_tile_plan_create(ftlm_ctx* c);
+void ftlm_tile_plan_destroy(ftlm_ctx* c);
+int ftlm_launch_hv_tile(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
+int ftlm_launch_neighbors_tile(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
+
+// ---- device helpers ---------------------------------------------------------------------
+#ifdef __CUDACC__
+
+__device__ __forceinline__ int popc_(uint32_t x) { return __popc(x); }
+__device__ __forceinline__ int popc_(uint64_t x) { return __popcll(x); }
+__device__ __forceinline__ int ffs_(uint32_t x) { return __ffs((int)x); }
+__device__ __forceinline__ int ffs_(uint64_t x) { return __ffsll((long long)x); }
+
+__device__ __forceinline__ double warp_sum(double x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+  return x;
+}
+
+// Deterministic block sum of three doubles (fixed tree). Result valid in thread 0.
+// `sh` must hold 3*32 doubles.
+__device__ __forceinline__ void block_sum3(double& a, double& b, double& c, double* sh) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+  __syncthreads();
+  if (lane == 0) { sh[w] = a; sh[32 + w] = b; sh[64 + w] = c; }
+  __syncthreads();
+  if (w == 0) {
+    a = lane < nw ? sh[lane] : 0.0;
+    b = lane < nw ? sh[32 + lane] : 0.0;
+    c = lane < nw ? sh[64 + lane] : 0.0;
+    a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+  }
+}
+
+// Grid-wide deterministic finish of the fused Lanczos reductions (H9): every block stores its
+// three partial sums, the last block to arrive (ticket) adds them in block order with a fixed
+// tree and advances the chain state: alpha_j = <q,y>/<q,q>, beta_j^2 = <y,y> - <q,y>^2/<q,q>
+// (H5(i): never assumes ||q|| = 1), breakdown rule of reading 10.
+__device__ __forceinline__ void lanczos_finish(double s_qy, double s_yy, double s_qq, double* partials,
+                                               int stride, unsigned int* ticket, ChainState* st,
+                                               double* sh) {
+  block_sum3(s_qy, s_yy, s_qq, sh);
+  __shared__ bool last;
+  if (threadIdx.x == 0) {
+    partials[blockIdx.x] = s_qy;
+    partials[stride + blockIdx.x] = s_yy;
+    partials[2 * stride + blockIdx.x] = s_qq;
+    __threadfence();
+    last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  double a = 0.0, b = 0.0, c = 0.0;
+  for (int k = threadIdx.x; k < (int)gridDim.x; k += blockDim.x) {   // fixed assignment + order
+    a += partials[k]; b += partials[stride + k]; c += partials[2 * stride + k];
+  }
+  block_sum3(a, b, c, sh);
+  if (threadIdx.x == 0) {
+    *ticket = 0;
+    const int j = st->step;
+    const double alpha = c > 0.0 ? a / c : 0.0;
+    double b2 = c > 0.0 ? b - a * a / c : 0.0;
+    if (!(b2 > 0.0)) b2 = 0.0;
+    const double beta = sqrt(b2);
+    st->alpha[j] = alpha;
+    st->beta[j] = beta;
+    double sc = st->scale;
+    sc = fmax(sc, fmax(fabs(alpha), beta));
+    st->scale = sc;
+    st->step = j + 1;
+    st->a = alpha;
+    st->inv_b = beta > 0.0 ? 1.0 / beta : 0.0;
+    st->beta_prev = beta;
+    if (j + 1 >= st->limit || beta <= st->tol * sc) st->done = 1;
+  }
+}
+
+#endif  // __CUDACC__

@@ -1,0 +1,555 @@
+// libftlm core: handle, sector tables (A0/A1), start vectors, the fused Lanczos chain driver
+// and the C-ABI entry points that dispatch to the ROW / TILE kernels.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "ftlm_common.cuh"
+
+// ---- errors --------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+void ftlm_set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+int ftlm_cuda_fail(cudaError_t e, const char* what) {
+  ftlm_set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+  return FTLM_ECUDA;
+}
+extern "C" const char* ftlm_last_error(void) { return g_err; }
+extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.1 (sm_100a)"; }
+
+size_t ftlm_elem_size(const ftlm_ctx* c) { return c->prec == FTLM_FP64 ? 8 : 4; }
+
+// ---- CLT construction (A1; L150-L154, Eq. 18) --------------------------------------------
+// For d = 2 the occupancy mask of block b depends only on N_up - popc(b) and C_b is the number
+// of sector labels below 32 b, so every block is built independently (no scan):
+//   M_b bit j = [popc(j) == N_up - popc(b)],  C_b = sum over set bits p of 32b (from the top) of
+//   C(p, N_up - ones_above).  Equals the paper's "set bits, then cumulative sum" construction.
+__global__ void clt_build_kernel(uint2* __restrict__ clt, int64_t nblk, int N, int K,
+                                 const uint64_t* __restrict__ binom) {
+  const int K1 = K + 1;
+  for (int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; b < nblk;
+       b += (int64_t)gridDim.x * blockDim.x) {
+    const int want = K - __popcll((unsigned long long)b);
+    uint32_t mask = 0;
+    if (want >= 0 && want <= 5) {
+      for (int j = 0; j < 32; ++j)
+        if (__popc(j) == want && (N >= 5 || j < (1 << N))) mask |= 1u << j;
+    }
+    const uint64_t base = (uint64_t)b << 5;
+    uint64_t cnt = 0;
+    int above = 0;
+    for (int p = N - 1; p >= 5; --p) {
+      if ((base >> p) & 1ull) {
+        const int need = K - above;
+        if (need >= 0 && need <= p) cnt += binom[p * K1 + need];
+        ++above;
+      }
+    }
+    clt[b] = make_uint2(mask, (uint32_t)cnt);
+  }
+}
+
+// ---- start vectors (readings 12-14) ---------------------------------------
+__device__ __forceinline__ uint64_t mix64(uint64_t x) {
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+  return x ^ (x >> 31);
+}
+static uint64_t mix64_host(uint64_t x) {
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+  return x ^ (x >> 31);
+}
+#define FTLM_GOLD 0x9E3779B97F4A7C15ull
+
+__device__ __forceinline__ double gauss_elem(uint64_t key, uint64_t t) {
+  const uint64_t a = mix64(key + FTLM_GOLD * (2ull * t + 1ull));
+  const uint64_t b = mix64(key + FTLM_GOLD * (2ull * t + 2ull));
+  const double u1 = ((double)(a >> 11) + 1.0) * 0x1.0p-53;
+  const double u2 = (double)(b >> 11) * 0x1.0p-53;
+  return sqrt(-2.0 * log(u1)) * cos(6.283185307179586 * u2);
+}
+
+__global__ void __launch_bounds__(256)
+gauss_norm_kernel(uint64_t key, int64_t dim, double* __restrict__ partials) {
+  __shared__ double sh[96];
+  double s = 0.0, z1 = 0.0, z2 = 0.0;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
+       t += (int64_t)gridDim.x * blockDim.x) {
+    const double g = gauss_elem(key, (uint64_t)t);
+    s += g * g;
+  }
+  block_sum3(s, z1, z2, sh);
+  if (threadIdx.x == 0) partials[blockIdx.x] = s;
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256)
+sumsq_kernel(const R* __restrict__ v, int64_t dim, double* __restrict__ partials) {
+  __shared__ double sh[96];
+  double s = 0.0, z1 = 0.0, z2 = 0.0;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
+       t += (int64_t)gridDim.x * blockDim.x) {
+    const double g = (double)v[t];
+    s += g * g;
+  }
+  block_sum3(s, z1, z2, sh);
+  if (threadIdx.x == 0) partials[blockIdx.x] = s;
+}
+
+__global__ void reduce_partials_kernel(const double* __restrict__ partials, int n, double* out) {
+  __shared__ double sh[96];
+  double s = 0.0, z1 = 0.0, z2 = 0.0;
+  for (int k = threadIdx.x; k < n; k += blockDim.x) s += partials[k];
+  block_sum3(s, z1, z2, sh);
+  if (threadIdx.x == 0) *out = s;
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256)
+gauss_write_kernel(uint64_t key, int64_t dim, const double* __restrict__ norm2, R* __restrict__ v) {
+  const double nrm = sqrt(*norm2);
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
+       t += (int64_t)gridDim.x * blockDim.x)
+    v[t] = (R)(gauss_elem(key, (uint64_t)t) / nrm);
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256)
+scale_copy_kernel(const R* __restrict__ src, int64_t dim, const double* __restrict__ norm2, R* __restrict__ dst) {
+  const double nrm = sqrt(*norm2);
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
+       t += (int64_t)gridDim.x * blockDim.x)
+    dst[t] = (R)((double)src[t] / nrm);
+}
+
+// ---- Lanczos normalisation pass (A7): q_{j+1} = (y - alpha_j q_j) / beta_j ----------------------
+template <typename R, typename V4>
+__global__ void __launch_bounds__(256)
+lanczos_next_kernel(const R* __restrict__ y, const R* __restrict__ q, R* __restrict__ qnext,
+                    int64_t dim, const ChainState* __restrict__ st) {
+  if (st->done) return;
+  const R a = (R)st->a, ib = (R)st->inv_b;
+  constexpr int W = sizeof(V4) / sizeof(R);
+  const int64_t nvec = dim / W;
+  const V4* y4 = (const V4*)y;
+  const V4* q4 = (const V4*)q;
+  V4* o4 = (V4*)qnext;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvec; k += stride) {
+    V4 yy = __ldcs(&y4[k]);
+    V4 qq = q4[k];
+    R* yp = (R*)&yy;
+    const R* qp = (const R*)&qq;
+#pragma unroll
+    for (int e = 0; e < W; ++e) yp[e] = (yp[e] - a * qp[e]) * ib;
+    o4[k] = yy;
+  }
+  for (int64_t t = nvec * W + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim; t += stride)
+    qnext[t] = (y[t] - a * q[t]) * ib;
+}
+
+__global__ void chain_reset_kernel(ChainState* st, int limit, double tol) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    st->scale = 0.0; st->beta_prev = 0.0; st->a = 0.0; st->inv_b = 0.0; st->tol = tol;
+    st->step = 0; st->limit = limit; st->done = (limit <= 0);
+  }
+}
+
+// ---- handle ------------------------------------------------------------------------------------
+static uint64_t binom_u64(int n, int k) {
+  if (k < 0 || k > n) return 0;
+  if (k > n - k) k = n - k;
+  unsigned __int128 r = 1;
+  for (int i = 1; i <= k; ++i) r = r * (unsigned)(n - k + i) / (unsigned)i;
+  return (uint64_t)r;
+}
+
+extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bond_i, const int32_t* bond_j,
+                           const double* J, double h, int N_up, int index_mode, int precision, int device) {
+  if (!out) { ftlm_set_error("ftlm_create: out is NULL"); return FTLM_EINVAL; }
+  *out = nullptr;
+  if (N < 1 || N > 62) { ftlm_set_error("ftlm_create: N=%d outside [1,62]", N); return FTLM_EINVAL; }
+  if (N_up < 0 || N_up > N) { ftlm_set_error("ftlm_create: N_up=%d outside [0,%d]", N_up, N); return FTLM_EINVAL; }
+  if (n_bonds < 0 || n_bonds > FTLM_MAX_BONDS || (n_bonds > 0 && (!bond_i || !bond_j || !J))) {
+    ftlm_set_error("ftlm_create: bad bond list (n_bonds=%d)", n_bonds); return FTLM_EINVAL;
+  }
+  if (index_mode != FTLM_INDEX_CLT && index_mode != FTLM_INDEX_CR) { ftlm_set_error("ftlm_create: bad index_mode %d", index_mode); return FTLM_EINVAL; }
+  if (precision != FTLM_FP32 && precision != FTLM_FP64) { ftlm_set_error("ftlm_create: bad precision %d", precision); return FTLM_EINVAL; }
+  for (int b = 0; b < n_bonds; ++b) {
+    if (bond_i[b] < 0 || bond_i[b] >= N || bond_j[b] < 0 || bond_j[b] >= N || bond_i[b] == bond_j[b]) {
+      ftlm_set_error("ftlm_create: bond %d = (%d,%d) invalid for N=%d", b, bond_i[b], bond_j[b], N);
+      return FTLM_EINVAL;
+    }
+  }
+  if (index_mode == FTLM_INDEX_CLT && N > 32) { ftlm_set_error("ftlm_create: CLT needs N <= 32 (got %d); use CR", N); return FTLM_EUNSUPPORTED; }
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev <= 0) {
+    ftlm_set_error("ftlm_create: no CUDA device (%s); this library has no CPU path", cudaGetErrorString(e));
+    return FTLM_ECUDA;
+  }
+  if (device < 0 || device >= ndev) { ftlm_set_error("ftlm_create: device %d of %d", device, ndev); return FTLM_EINVAL; }
+  CK(cudaSetDevice(device));
+
+  ftlm_ctx* c = new ftlm_ctx();
+  c->N = N; c->nb = n_bonds; c->N_up = N_up; c->mode = index_mode; c->prec = precision; c->device = device; c->h = h;
+  c->dim = (int64_t)binom_u64(N, N_up);
+  c->idx64 = (uint64_t)c->dim >= (1ull << 32);
+  c->lab64 = N > 32;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->sm_count = prop.multiProcessorCount;
+
+  double sumJq = 0.0;
+  c->bonds.resize(n_bonds);
+  for (int b = 0; b < n_bonds; ++b) {
+    BondDev& d = c->bonds[b];
+    d.i = bond_i[b] < bond_j[b] ? bond_i[b] : bond_j[b];
+    d.j = bond_i[b] < bond_j[b] ? bond_j[b] : bond_i[b];
+    d.mask = (1ull << d.i) | (1ull << d.j);
+    d.Jh = 0.5 * J[b]; d.Jq = 0.25 * J[b];
+    sumJq += d.Jq;
+  }
+  c->diag0 = sumJq - h * ((double)N_up - 0.5 * (double)N);
+
+  const int K1 = N_up + 1;
+  c->binom64.assign((size_t)(N + 1) * K1, 0);
+  std::vector<uint32_t> b32((size_t)(N + 1) * K1, 0);
+  for (int p = 0; p <= N; ++p)
+    for (int a = 0; a <= N_up; ++a) {
+      const uint64_t v = binom_u64(p, a);
+      c->binom64[(size_t)p * K1 + a] = v;
+      b32[(size_t)p * K1 + a] = v > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)v;
+    }
+  int rc = FTLM_OK;
+  auto fail = [&](int code) { ftlm_destroy(c); return code; };
+#define CKF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { rc = ftlm_cuda_fail(e__, #call); return fail(e__ == cudaErrorMemoryAllocation ? FTLM_ENOMEM : rc); } } while (0)
+  CKF(cudaMalloc(&c->d_binom64, c->binom64.size() * 8));
+  CKF(cudaMalloc(&c->d_binom32, b32.size() * 4));
+  CKF(cudaMemcpy(c->d_binom64, c->binom64.data(), c->binom64.size() * 8, cudaMemcpyHostToDevice));
+  CKF(cudaMemcpy(c->d_binom32, b32.data(), b32.size() * 4, cudaMemcpyHostToDevice));
+  CKF(cudaMalloc(&c->d_bonds, sizeof(BondDev) * (size_t)(n_bonds > 0 ? n_bonds : 1)));
+  if (n_bonds > 0) CKF(cudaMemcpy(c->d_bonds, c->bonds.data(), sizeof(BondDev) * n_bonds, cudaMemcpyHostToDevice));
+  c->max_blocks = c->sm_count * 32;
+  CKF(cudaMalloc(&c->d_state, sizeof(ChainState)));
+  CKF(cudaMemset(c->d_state, 0, sizeof(ChainState)));
+  CKF(cudaMalloc(&c->d_partials, sizeof(double) * 3 * (size_t)c->max_blocks));
+  CKF(cudaMalloc(&c->d_ticket, sizeof(unsigned int)));
+  CKF(cudaMemset(c->d_ticket, 0, sizeof(unsigned int)));
+  if (index_mode == FTLM_INDEX_CLT) {
+    c->n_clt = (int64_t)(((1ull << N) + 31ull) / 32ull);
+    CKF(cudaMalloc(&c->d_clt, sizeof(uint2) * (size_t)c->n_clt));
+    int grid = (int)((c->n_clt + 255) / 256);
+    if (grid > c->sm_count * 16) grid = c->sm_count * 16;
+    clt_build_kernel<<<grid, 256>>>(c->d_clt, c->n_clt, N, N_up, c->d_binom64);
+    CKF(cudaGetLastError());
+  }
+  for (int k = 0; k < 4; ++k) CKF(cudaEventCreate(&c->ev[k]));
+  rc = ftlm_tile_plan_create(c);
+  if (rc != FTLM_OK) return fail(rc);
+  CKF(cudaDeviceSynchronize());
+#undef CKF
+  *out = c;
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_destroy(ftlm_ctx* c) {
+  if (!c) return FTLM_OK;
+  cudaSetDevice(c->device);
+  ftlm_tile_plan_destroy(c);
+  cudaFree(c->d_binom64); cudaFree(c->d_binom32); cudaFree(c->d_bonds); cudaFree(c->d_clt);
+  cudaFree(c->d_state); cudaFree(c->d_partials); cudaFree(c->d_ticket);
+  for (int k = 0; k < 3; ++k) cudaFree(c->q[k]);
+  for (int k = 0; k < 4; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+  delete c;
+  return FTLM_OK;
+}
+
+extern "C" int64_t ftlm_dim(const ftlm_ctx* c) { return c ? c->dim : -1; }
+
+extern "C" int64_t ftlm_table_bytes(const ftlm_ctx* c) {
+  if (!c) return -1;
+  int64_t b = (int64_t)c->binom64.size() * 12 + (int64_t)c->nb * (int64_t)sizeof(BondDev);
+  if (c->mode == FTLM_INDEX_CLT) b += c->n_clt * 8;
+  return b;
+}
+
+int ftlm_effective_kernel(const ftlm_ctx* c) {
+  if (c->kernel == FTLM_KERNEL_ROW) return FTLM_KERNEL_ROW;
+  if (c->tile) return FTLM_KERNEL_TILE;
+  return FTLM_KERNEL_ROW;
+}
+
+extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
+  if (!c || !key) { ftlm_set_error("ftlm_set_option: NULL"); return FTLM_EINVAL; }
+  if (!strcmp(key, "kernel")) {
+    if (value < 0 || value > 2) { ftlm_set_error("kernel must be 0..2"); return FTLM_EINVAL; }
+    if (value == FTLM_KERNEL_TILE && !c->tile) { ftlm_set_error("TILE kernel unavailable for this sector"); return FTLM_EUNSUPPORTED; }
+    c->kernel = (int)value; return FTLM_OK;
+  }
+  if (!strcmp(key, "low_bits")) {
+    if (value < 0 || value > 20) { ftlm_set_error("low_bits must be 0..20"); return FTLM_EINVAL; }
+    const int old = c->low_bits;
+    c->low_bits = (int)value;
+    ftlm_tile_plan_destroy(c);
+    int rc = ftlm_tile_plan_create(c);
+    if (rc != FTLM_OK) { c->low_bits = old; ftlm_tile_plan_destroy(c); ftlm_tile_plan_create(c); }
+    return rc;
+  }
+  if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
+  ftlm_set_error("ftlm_set_option: unknown key '%s'", key);
+  return FTLM_EINVAL;
+}
+
+extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
+  if (!c || !key) return -1;
+  if (!strcmp(key, "kernel")) return ftlm_effective_kernel(c);
+  if (!strcmp(key, "low_bits")) return c->low_bits;
+  if (!strcmp(key, "graph")) return c->use_graph;
+  if (!strcmp(key, "sm_count")) return c->sm_count;
+  return -1;
+}
+
+extern "C" int ftlm_clt_read(ftlm_ctx* c, int64_t b0, int64_t nb, uint32_t* h_mask, uint32_t* h_count) {
+  if (!c || c->mode != FTLM_INDEX_CLT || b0 < 0 || nb < 0 || b0 + nb > c->n_clt || !h_mask || !h_count) {
+    ftlm_set_error("ftlm_clt_read: bad argument or not a CLT handle"); return FTLM_EINVAL;
+  }
+  CK(cudaSetDevice(c->device));
+  std::vector<uint2> tmp((size_t)nb);
+  CK(cudaMemcpy(tmp.data(), c->d_clt + b0, sizeof(uint2) * (size_t)nb, cudaMemcpyDeviceToHost));
+  for (int64_t k = 0; k < nb; ++k) { h_mask[k] = tmp[(size_t)k].x; h_count[k] = tmp[(size_t)k].y; }
+  return FTLM_OK;
+}
+
+// ---- H.v ---------------------------------------------------------------------------------------
+static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
+  if (ftlm_effective_kernel(c) == FTLM_KERNEL_TILE) return ftlm_launch_hv_tile(c, v, qp, y, fused, s);
+  return ftlm_launch_hv_row(c, v, qp, y, fused, s);
+}
+
+extern "C" int ftlm_apply_H(ftlm_ctx* c, const void* d_v, void* d_y, void* stream) {
+  if (!c || !d_v || !d_y || d_v == d_y) { ftlm_set_error("ftlm_apply_H: bad argument (NULL or d_y == d_v)"); return FTLM_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  return launch_hv(c, d_v, nullptr, d_y, 0, (cudaStream_t)stream);
+}
+
+extern "C" int ftlm_apply_H_host(ftlm_ctx* c, const void* h_v, void* h_y) {
+  if (!c || !h_v || !h_y) { ftlm_set_error("ftlm_apply_H_host: NULL"); return FTLM_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
+  void *dv = nullptr, *dy = nullptr;
+  if (cudaMalloc(&dv, bytes) != cudaSuccess || cudaMalloc(&dy, bytes) != cudaSuccess) {
+    cudaFree(dv); ftlm_set_error("ftlm_apply_H_host: out of device memory"); return FTLM_ENOMEM;
+  }
+  int rc = FTLM_OK;
+  cudaError_t e = cudaMemcpy(dv, h_v, bytes, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) rc = launch_hv(c, dv, nullptr, dy, 0, 0);
+  if (e == cudaSuccess && rc == FTLM_OK) e = cudaMemcpy(h_y, dy, bytes, cudaMemcpyDeviceToHost);
+  cudaFree(dv); cudaFree(dy);
+  if (e != cudaSuccess) return ftlm_cuda_fail(e, "ftlm_apply_H_host");
+  return rc;
+}
+
+extern "C" int ftlm_neighbors(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, void* stream) {
+  if (!c || row0 < 0 || nrows < 0 || row0 + nrows > c->dim || (nrows > 0 && !d_idx)) {
+    ftlm_set_error("ftlm_neighbors: bad row range"); return FTLM_EINVAL;
+  }
+  if (nrows == 0 || c->nb == 0) return FTLM_OK;
+  CK(cudaSetDevice(c->device));
+  if (ftlm_effective_kernel(c) == FTLM_KERNEL_TILE) return ftlm_launch_neighbors_tile(c, row0, nrows, d_idx, (cudaStream_t)stream);
+  return ftlm_launch_neighbors_row(c, row0, nrows, d_idx, (cudaStream_t)stream);
+}
+
+// ---- start vectors -----------------------------------------------------------------------------
+static uint64_t chain_key(uint64_t seed, int N_up, int r) {
+  uint64_t k = mix64_host(seed);
+  k = mix64_host(k + FTLM_GOLD * (uint64_t)(N_up + 1));
+  k = mix64_host(k + FTLM_GOLD * (uint64_t)(r + 1));
+  return k;
+}
+
+static int stream_grid(const ftlm_ctx* c, int64_t n, int per_sm) {
+  int64_t blocks = (n + 255) / 256;
+  int64_t cap = (int64_t)c->sm_count * per_sm;
+  if (blocks > cap) blocks = cap;
+  if (blocks > c->max_blocks) blocks = c->max_blocks;
+  return (int)(blocks < 1 ? 1 : blocks);
+}
+
+extern "C" int ftlm_fill_random(ftlm_ctx* c, uint64_t seed, int r, void* d_v, void* stream) {
+  if (!c || !d_v || r < 0) { ftlm_set_error("ftlm_fill_random: bad argument"); return FTLM_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  cudaStream_t s = (cudaStream_t)stream;
+  const uint64_t key = chain_key(seed, c->N_up, r);
+  const int grid = stream_grid(c, c->dim, 8);
+  gauss_norm_kernel<<<grid, 256, 0, s>>>(key, c->dim, c->d_partials);
+  reduce_partials_kernel<<<1, 256, 0, s>>>(c->d_partials, grid, &c->d_state->norm2);
+  if (c->prec == FTLM_FP32) gauss_write_kernel<float><<<grid, 256, 0, s>>>(key, c->dim, &c->d_state->norm2, (float*)d_v);
+  else gauss_write_kernel<double><<<grid, 256, 0, s>>>(key, c->dim, &c->d_state->norm2, (double*)d_v);
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+
+// ---- chain -------------------------------------------------------------------------------------
+static int ensure_workspace(ftlm_ctx* c) {
+  const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
+  for (int k = 0; k < 3; ++k)
+    if (!c->q[k]) {
+      cudaError_t e = cudaMalloc(&c->q[k], bytes);
+      if (e != cudaSuccess) { ftlm_set_error("chain workspace: cannot allocate 3 x %zu bytes (%s)", bytes, cudaGetErrorString(e)); cudaGetLastError(); return FTLM_ENOMEM; }
+    }
+  return FTLM_OK;
+}
+
+static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64_t seed, int r, cudaStream_t s) {
+  CK(cudaSetDevice(c->device));
+  int rc = ensure_workspace(c);
+  if (rc != FTLM_OK) return rc;
+  const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
+  c->cur = 0;
+  c->steps_enqueued = 0;
+  c->chain_limit = (int)(c->dim < FTLM_MAX_STEPS ? c->dim : FTLM_MAX_STEPS);
+  if (!q1) {
+    rc = ftlm_fill_random(c, seed, r, c->q[0], s);
+    if (rc != FTLM_OK) return rc;
+  } else {
+    // copy into q[1] (scratch), then normalise in FP64 into q[0]
+    CK(cudaMemcpyAsync(c->q[1], q1, bytes, q1_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
+    const int grid = stream_grid(c, c->dim, 8);
+    if (c->prec == FTLM_FP32) sumsq_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[1], c->dim, c->d_partials);
+    else sumsq_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[1], c->dim, c->d_partials);
+    reduce_partials_kernel<<<1, 256, 0, s>>>(c->d_partials, grid, &c->d_state->norm2);
+    if (c->prec == FTLM_FP32) scale_copy_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[1], c->dim, &c->d_state->norm2, (float*)c->q[0]);
+    else scale_copy_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[1], c->dim, &c->d_state->norm2, (double*)c->q[0]);
+  }
+  CK(cudaMemsetAsync(c->q[2], 0, bytes, s));          // q_0 = 0
+  chain_reset_kernel<<<1, 32, 0, s>>>(c->d_state, c->chain_limit, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_chain_begin(ftlm_ctx* c, const void* d_q1, uint64_t seed, int r, void* stream) {
+  if (!c || r < 0) { ftlm_set_error("ftlm_chain_begin: bad argument"); return FTLM_EINVAL; }
+  return chain_begin_impl(c, d_q1, false, seed, r, (cudaStream_t)stream);
+}
+
+static int launch_next(ftlm_ctx* c, cudaStream_t s) {
+  const void* y = c->q[(c->cur + 1) % 3];
+  const void* q = c->q[c->cur];
+  void* qn = c->q[(c->cur + 2) % 3];
+  const int grid = stream_grid(c, c->dim / 4 + 1, 8);
+  if (c->prec == FTLM_FP32) lanczos_next_kernel<float, float4><<<grid, 256, 0, s>>>((const float*)y, (const float*)q, (float*)qn, c->dim, c->d_state);
+  else lanczos_next_kernel<double, double2><<<grid, 256, 0, s>>>((const double*)y, (const double*)q, (double*)qn, c->dim, c->d_state);
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+
+static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv, float* ms_norm) {
+  // y = H q_j - beta_{j-1} q_{j-1}   (+ reductions, alpha_j, beta_j on the device)
+  if (timed) CK(cudaEventRecord(c->ev[0], s));
+  int rc = launch_hv(c, c->q[c->cur], c->q[(c->cur + 2) % 3], c->q[(c->cur + 1) % 3], 1, s);
+  if (rc != FTLM_OK) return rc;
+  if (timed) CK(cudaEventRecord(c->ev[1], s));
+  // q_{j+1} = (y - alpha_j q_j)/beta_j, written over q_{j-1}
+  rc = launch_next(c, s);
+  if (rc != FTLM_OK) return rc;
+  if (timed) {
+    CK(cudaEventRecord(c->ev[2], s));
+    CK(cudaEventSynchronize(c->ev[2]));
+    CK(cudaEventElapsedTime(ms_hv, c->ev[0], c->ev[1]));
+    CK(cudaEventElapsedTime(ms_norm, c->ev[1], c->ev[2]));
+  }
+  // rotate: q_{j+1} lives in old q_{j-1}; old q_j becomes q_{j-1}; old y becomes scratch
+  c->cur = (c->cur + 2) % 3;
+  c->steps_enqueued++;
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_chain_steps(ftlm_ctx* c, int nsteps, void* stream) {
+  if (!c || nsteps < 0 || !c->q[0]) { ftlm_set_error("ftlm_chain_steps: no chain begun or nsteps < 0"); return FTLM_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  for (int k = 0; k < nsteps; ++k) {
+    if (c->steps_enqueued >= c->chain_limit) break;      // the device would no-op anyway
+    int rc = chain_one_step(c, (cudaStream_t)stream, false, nullptr, nullptr);
+    if (rc != FTLM_OK) return rc;
+  }
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_chain_profile(ftlm_ctx* c, int nsteps, void* stream, double* ms_hv, double* ms_norm) {
+  if (!c || nsteps <= 0 || !c->q[0] || !ms_hv || !ms_norm) { ftlm_set_error("ftlm_chain_profile: bad argument"); return FTLM_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  double a = 0.0, b = 0.0;
+  int n = 0;
+  for (int k = 0; k < nsteps; ++k) {
+    if (c->steps_enqueued >= c->chain_limit) break;
+    float x = 0.f, y = 0.f;
+    int rc = chain_one_step(c, (cudaStream_t)stream, true, &x, &y);
+    if (rc != FTLM_OK) return rc;
+    a += x; b += y; ++n;
+  }
+  *ms_hv = n ? a / n : 0.0;
+  *ms_norm = n ? b / n : 0.0;
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_chain_end(ftlm_ctx* c, double* h_alpha, double* h_beta, int cap, int* h_m_eff, void* stream) {
+  if (!c || !h_m_eff || cap < 0) { ftlm_set_error("ftlm_chain_end: bad argument"); return FTLM_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize((cudaStream_t)stream));
+  static thread_local ChainState hs;
+  CK(cudaMemcpy(&hs, c->d_state, sizeof(ChainState), cudaMemcpyDeviceToHost));
+  int m = hs.step;
+  *h_m_eff = m;
+  if (m > cap) m = cap;
+  if (h_alpha) for (int k = 0; k < m; ++k) h_alpha[k] = hs.alpha[k];
+  if (h_beta) for (int k = 0; k + 1 < m; ++k) h_beta[k] = hs.beta[k];
+  return FTLM_OK;
+}
+
+static int lanczos_impl(ftlm_ctx* c, const void* h_q1, uint64_t seed, int R, int n_steps, double* h_alpha,
+                        double* h_beta, int* h_m_eff, double* h_theta, double* h_weight, cudaStream_t s) {
+  if (!c || R < 0 || n_steps < 1 || n_steps > FTLM_MAX_STEPS || !h_alpha || !h_beta || !h_m_eff) {
+    ftlm_set_error("ftlm_lanczos: bad argument (n_steps must be in [1,%d])", FTLM_MAX_STEPS); return FTLM_EINVAL;
+  }
+  const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
+  for (int r = 0; r < R; ++r) {
+    double* a = h_alpha + (size_t)r * n_steps;
+    double* b = h_beta + (size_t)r * n_steps;
+    for (int k = 0; k < n_steps; ++k) { a[k] = 0.0; b[k] = 0.0; }
+    int rc = chain_begin_impl(c, h_q1 ? (const char*)h_q1 + (size_t)r * bytes : nullptr, h_q1 != nullptr, seed, r, s);
+    if (rc != FTLM_OK) return rc;
+    if (c->chain_limit > n_steps) {           // m = min(n_steps, dim)
+      c->chain_limit = n_steps;
+      chain_reset_kernel<<<1, 32, 0, s>>>(c->d_state, n_steps, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
+    }
+    rc = ftlm_chain_steps(c, n_steps, s);
+    if (rc != FTLM_OK) return rc;
+    rc = ftlm_chain_end(c, a, b, n_steps, &h_m_eff[r], s);
+    if (rc != FTLM_OK) return rc;
+    if (h_theta && h_weight) {
+      double* th = h_theta + (size_t)r * n_steps;
+      double* w = h_weight + (size_t)r * n_steps;
+      for (int k = 0; k < n_steps; ++k) { th[k] = 0.0; w[k] = 0.0; }
+      rc = ftlm_tridiag_eig(h_m_eff[r], a, b, th, w);
+      if (rc != FTLM_OK) return rc;
+    }
+  }
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_lanczos(ftlm_ctx* c, uint64_t seed, int R, int n_steps, double* h_alpha, double* h_beta,
+                            int* h_m_eff, double* h_theta, double* h_weight, void* stream) {
+  return lanczos_impl(c, nullptr, seed, R, n_steps, h_alpha, h_beta, h_m_eff, h_theta, h_weight, (cudaStream_t)stream);
+}
+
+extern "C" int ftlm_lanczos_host(ftlm_ctx* c, const void* h_q1, int R, int n_steps, double* h_alpha, double* h_beta,
+                                 int* h_m_eff, double* h_theta, double* h_weight, void* stream) {
+  if (!h_q1) { ftlm_set_error("ftlm_lanczos_host: h_q1 is NULL"); return FTLM_EINVAL; }
+  return lanczos_impl(c, h_q1, 0, R, n_steps, h_alpha, h_beta, h_m_eff, h_theta, h_weight, (cudaStream_t)stream);
+}

@@ -1,0 +1,317 @@
+// ROW kernels: one thread per sector row, every row unranked, per-bond loop.  This is the
+// paper's launch shape ("assigning one GPU thread to each
+// sector-basis state") written for sm_100a; it is the plain in-library baseline and the path
+// used for index-map queries.  The B200 design proper is in ftlm_tile.cu.
+#include "ftlm_common.cuh"
+
+namespace {
+
+// Inverse map (L136; reading 26): at bit p with A ones left, bit p = 1 iff r >= C(p, A).
+// binom is the (saturated) table [p*(K+1) + a] in shared memory.
+template <typename L, typename I>
+__device__ __forceinline__ L unrank(I r, int N, int K1, int K, const I* __restrict__ binom) {
+  L n = 0;
+  int A = K;
+  for (int p = N - 1; p >= 0 && A > 0; --p) {
+    const I c = binom[p * K1 + A];
+    if (r >= c) { n |= (L)1 << p; r -= c; --A; }
+  }
+  return n;
+}
+
+// Algorithm 1 (L138-L144) at d = 2: rank += D_c(p, A, a_p) = a_p ? C(p, A) : 0; A -= a_p.
+template <typename L, typename I>
+__device__ __forceinline__ I rank_alg1(L x, int N, int K1, int K, const I* __restrict__ binom) {
+  I rank = 0;
+  int A = K;
+  for (int p = N - 1; p >= 0; --p) {
+    if ((x >> p) & 1) { rank += binom[p * K1 + A]; --A; }
+  }
+  return rank;
+}
+
+// Incremental CR: index change when the one of an antiparallel bond (i < j) moves.
+// Only the binomial terms of positions i..j change.  Unsigned wrap-around is harmless.
+template <typename L, typename I>
+__device__ __forceinline__ I cr_delta(L x, int i, int j, int K1, const I* __restrict__ binom) {
+  const int ci = popc_((L)(x & ((((L)2) << i) - 1)));         // ones at positions <= i
+  const int cj = popc_((L)(x & ((((L)2) << j) - 1)));         // ones at positions <= j
+  L between = x & ((((L)1) << j) - 1) & ~((((L)2) << i) - 1);
+  I d;
+  int c = ci;
+  if ((x >> j) & 1) {                                          // the one moves down j -> i
+    d = binom[i * K1 + ci + 1] - binom[j * K1 + cj];
+    while (between) {
+      const int p = ffs_(between) - 1;
+      between &= between - 1;
+      ++c;
+      d += binom[p * K1 + c + 1] - binom[p * K1 + c];
+    }
+  } else {                                                     // the one moves up i -> j
+    d = binom[j * K1 + cj] - binom[i * K1 + ci];
+    while (between) {
+      const int p = ffs_(between) - 1;
+      between &= between - 1;
+      ++c;
+      d += binom[p * K1 + c - 1] - binom[p * K1 + c];
+    }
+  }
+  return d;
+}
+
+// Algorithm 2 (L167-L173): b = n >> 5, j = n & 31, index = C_b + popc(M_b & (2^j - 1)).
+__device__ __forceinline__ int64_t clt_lookup_checked(uint64_t n, int N, const uint2* __restrict__ clt) {
+  if (N < 64 && (n >> N)) return -1;
+  const uint2 e = clt[n >> 5];
+  const uint32_t j = (uint32_t)n & 31u;
+  if (!((e.x >> j) & 1u)) return -1;
+  return (int64_t)e.y + __popc(e.x & ((1u << j) - 1u));
+}
+__device__ __forceinline__ uint32_t clt_lookup(uint32_t n, const uint2* __restrict__ clt) {
+  const uint2 e = __ldg(&clt[n >> 5]);
+  return e.y + __popc(e.x & ((1u << (n & 31u)) - 1u));
+}
+
+struct RowParams {
+  int N, K, nb, mode;
+  int64_t dim;
+  const void* binom;       // I[(N+1)*(K+1)]
+  const BondDev* bonds;
+  const uint2* clt;
+  double diag0;
+  // fused part
+  ChainState* st;
+  double* partials;
+  unsigned int* ticket;
+  int stride;
+};
+
+template <typename R> struct BondS { uint64_t mask; R Jh, Jq; int i, j; };
+
+template <typename R, typename L, typename I>
+__device__ __forceinline__ void load_tables(const RowParams& p, I* s_binom, BondS<R>* s_bonds) {
+  const int nbin = (p.N + 1) * (p.K + 1);
+  const I* g = (const I*)p.binom;
+  for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = g[k];
+  for (int k = threadIdx.x; k < p.nb; k += blockDim.x) {
+    BondDev b = p.bonds[k];
+    s_bonds[k].mask = b.mask; s_bonds[k].Jh = (R)b.Jh; s_bonds[k].Jq = (R)b.Jq;
+    s_bonds[k].i = b.i; s_bonds[k].j = b.j;
+  }
+  __syncthreads();
+}
+
+template <typename R, typename L, typename I, int MODE, bool FUSED>
+__global__ void __launch_bounds__(256)
+hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev, R* __restrict__ y) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ double sh_red[96];
+  if (FUSED) { if (p.st->done) return; }
+  I* s_binom = (I*)smem;
+  const int nbin = (p.N + 1) * (p.K + 1);
+  BondS<R>* s_bonds = (BondS<R>*)(smem + (((size_t)nbin * sizeof(I) + 15) & ~(size_t)15));
+  load_tables<R, L, I>(p, s_binom, s_bonds);
+  const int K1 = p.K + 1;
+  const R bprev = FUSED ? (R)p.st->beta_prev : (R)0;
+  double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < p.dim; t += stride) {
+    const L n = unrank<L, I>((I)t, p.N, K1, p.K, s_binom);
+    R acc = 0, danti = 0;
+    for (int b = 0; b < p.nb; ++b) {
+      const L m = (L)s_bonds[b].mask;
+      const L x = n & m;
+      if (x != 0 && x != m) {                                   // antiparallel spins
+        I idx;
+        if (MODE == FTLM_INDEX_CLT) idx = (I)clt_lookup((uint32_t)(n ^ m), p.clt);
+        else idx = (I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom);
+        acc += s_bonds[b].Jh * __ldg(&v[idx]);
+        danti += s_bonds[b].Jq;
+      }
+    }
+    const R vt = v[t];
+    R out = ((R)p.diag0 - 2 * danti) * vt + acc;
+    if (FUSED) {
+      out -= bprev * qprev[t];
+      s_qy += (double)vt * (double)out;
+      s_yy += (double)out * (double)out;
+      s_qq += (double)vt * (double)vt;
+    }
+    y[t] = out;
+  }
+  if (FUSED) lanczos_finish(s_qy, s_yy, s_qq, p.partials, p.stride, p.ticket, p.st, sh_red);
+}
+
+template <typename L, typename I, int MODE>
+__global__ void __launch_bounds__(256)
+neighbors_row_kernel(RowParams p, int64_t row0, int64_t nrows, int64_t* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  I* s_binom = (I*)smem;
+  const int nbin = (p.N + 1) * (p.K + 1);
+  BondS<float>* s_bonds = (BondS<float>*)(smem + (((size_t)nbin * sizeof(I) + 15) & ~(size_t)15));
+  load_tables<float, L, I>(p, s_binom, s_bonds);
+  const int K1 = p.K + 1;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < nrows; r += stride) {
+    const int64_t t = row0 + r;
+    const L n = unrank<L, I>((I)t, p.N, K1, p.K, s_binom);
+    for (int b = 0; b < p.nb; ++b) {
+      const L m = (L)s_bonds[b].mask;
+      const L x = n & m;
+      int64_t idx = -1;
+      if (x != 0 && x != m) {
+        if (MODE == FTLM_INDEX_CLT) idx = (int64_t)clt_lookup((uint32_t)(n ^ m), p.clt);
+        else idx = (int64_t)(I)((I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom));
+      }
+      out[r * p.nb + b] = idx;
+    }
+  }
+}
+
+template <typename L, typename I>
+__global__ void index_of_kernel(RowParams p, const uint64_t* __restrict__ labels, int64_t n,
+                                int64_t* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  I* s_binom = (I*)smem;
+  const int nbin = (p.N + 1) * (p.K + 1);
+  for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = ((const I*)p.binom)[k];
+  __syncthreads();
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
+    const uint64_t lab = labels[k];
+    int64_t idx;
+    if (p.mode == FTLM_INDEX_CLT) {
+      idx = clt_lookup_checked(lab, p.N, p.clt);
+    } else {
+      const bool in = (p.N >= 64 || (lab >> p.N) == 0) && __popcll(lab) == p.K;
+      idx = in ? (int64_t)rank_alg1<L, I>((L)lab, p.N, p.K + 1, p.K, s_binom) : -1;
+    }
+    out[k] = idx;
+  }
+}
+
+template <typename L, typename I>
+__global__ void state_of_kernel(RowParams p, const int64_t* __restrict__ idx, int64_t n,
+                                uint64_t* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  I* s_binom = (I*)smem;
+  const int nbin = (p.N + 1) * (p.K + 1);
+  for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = ((const I*)p.binom)[k];
+  __syncthreads();
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
+    const int64_t t = idx[k];
+    out[k] = (t < 0 || t >= p.dim) ? ~0ull : (uint64_t)unrank<L, I>((I)t, p.N, p.K + 1, p.K, s_binom);
+  }
+}
+
+RowParams make_params(ftlm_ctx* c) {
+  RowParams p;
+  p.N = c->N; p.K = c->N_up; p.nb = c->nb; p.mode = c->mode; p.dim = c->dim;
+  p.binom = c->idx64 ? (const void*)c->d_binom64 : (const void*)c->d_binom32;
+  p.bonds = c->d_bonds; p.clt = c->d_clt; p.diag0 = c->diag0;
+  p.st = c->d_state; p.partials = c->d_partials; p.ticket = c->d_ticket; p.stride = c->max_blocks;
+  return p;
+}
+
+size_t table_smem(const ftlm_ctx* c, size_t bond_sz) {
+  const size_t isz = c->idx64 ? 8 : 4;
+  size_t b = ((size_t)(c->N + 1) * (c->N_up + 1) * isz + 15) & ~(size_t)15;
+  return b + (size_t)c->nb * bond_sz;
+}
+
+int grid_for(const ftlm_ctx* c, int64_t work, int per_sm) {
+  int64_t blocks = (work + 255) / 256;
+  int64_t cap = (int64_t)c->sm_count * per_sm;
+  if (blocks > cap) blocks = cap;
+  if (blocks < 1) blocks = 1;
+  return (int)blocks;
+}
+
+template <typename R, typename L, typename I>
+int launch_hv(ftlm_ctx* c, const RowParams& p, const void* v, const void* qp, void* y, int fused,
+              cudaStream_t s) {
+  const size_t sm = table_smem(c, sizeof(BondS<R>));
+  const int grid = grid_for(c, c->dim, 8);
+  if (fused && grid > c->max_blocks) { ftlm_set_error("internal: grid > max_blocks"); return FTLM_EINVAL; }
+#define LAUNCH(MODE, FUSED)                                                                      \
+  do {                                                                                           \
+    auto k = hv_row_kernel<R, L, I, MODE, FUSED>;                                                \
+    if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
+    k<<<grid, 256, sm, s>>>(p, (const R*)v, (const R*)qp, (R*)y);                                \
+  } while (0)
+  if (c->mode == FTLM_INDEX_CLT) { if (fused) LAUNCH(FTLM_INDEX_CLT, true); else LAUNCH(FTLM_INDEX_CLT, false); }
+  else { if (fused) LAUNCH(FTLM_INDEX_CR, true); else LAUNCH(FTLM_INDEX_CR, false); }
+#undef LAUNCH
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+
+}  // namespace
+
+int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s) {
+  RowParams p = make_params(c);
+  if (c->prec == FTLM_FP32) {
+    if (!c->lab64) return launch_hv<float, uint32_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    if (!c->idx64) return launch_hv<float, uint64_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    return launch_hv<float, uint64_t, uint64_t>(c, p, v, qprev, y, fused, s);
+  } else {
+    if (!c->lab64) return launch_hv<double, uint32_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    if (!c->idx64) return launch_hv<double, uint64_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    return launch_hv<double, uint64_t, uint64_t>(c, p, v, qprev, y, fused, s);
+  }
+}
+
+int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s) {
+  RowParams p = make_params(c);
+  const size_t sm = table_smem(c, sizeof(BondS<float>));
+  const int grid = grid_for(c, nrows, 8);
+#define LAUNCHN(L, I)                                                                                 \
+  do {                                                                                                \
+    if (c->mode == FTLM_INDEX_CLT) {                                                                  \
+      auto k = neighbors_row_kernel<L, I, FTLM_INDEX_CLT>;                                            \
+      if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
+      k<<<grid, 256, sm, s>>>(p, row0, nrows, d_idx);                                                 \
+    } else {                                                                                          \
+      auto k = neighbors_row_kernel<L, I, FTLM_INDEX_CR>;                                             \
+      if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
+      k<<<grid, 256, sm, s>>>(p, row0, nrows, d_idx);                                                 \
+    }                                                                                                 \
+  } while (0)
+  if (!c->lab64) LAUNCHN(uint32_t, uint32_t);
+  else if (!c->idx64) LAUNCHN(uint64_t, uint32_t);
+  else LAUNCHN(uint64_t, uint64_t);
+#undef LAUNCHN
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_index_of(ftlm_ctx* c, const uint64_t* d_labels, int64_t n, int64_t* d_idx, void* stream) {
+  if (!c || (n > 0 && (!d_labels || !d_idx)) || n < 0) { ftlm_set_error("ftlm_index_of: bad argument"); return FTLM_EINVAL; }
+  if (n == 0) return FTLM_OK;
+  CK(cudaSetDevice(c->device));
+  RowParams p = make_params(c);
+  const size_t sm = table_smem(c, 0);
+  const int grid = grid_for(c, n, 8);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (!c->lab64) index_of_kernel<uint32_t, uint32_t><<<grid, 256, sm, s>>>(p, d_labels, n, d_idx);
+  else if (!c->idx64) index_of_kernel<uint64_t, uint32_t><<<grid, 256, sm, s>>>(p, d_labels, n, d_idx);
+  else index_of_kernel<uint64_t, uint64_t><<<grid, 256, sm, s>>>(p, d_labels, n, d_idx);
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+
+extern "C" int ftlm_state_of(ftlm_ctx* c, const int64_t* d_idx, int64_t n, uint64_t* d_labels, void* stream) {
+  if (!c || (n > 0 && (!d_labels || !d_idx)) || n < 0) { ftlm_set_error("ftlm_state_of: bad argument"); return FTLM_EINVAL; }
+  if (n == 0) return FTLM_OK;
+  CK(cudaSetDevice(c->device));
+  RowParams p = make_params(c);
+  const size_t sm = table_smem(c, 0);
+  const int grid = grid_for(c, n, 8);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (!c->lab64) state_of_kernel<uint32_t, uint32_t><<<grid, 256, sm, s>>>(p, d_idx, n, d_labels);
+  else if (!c->idx64) state_of_kernel<uint64_t, uint32_t><<<grid, 256, sm, s>>>(p, d_idx, n, d_labels);
+  else state_of_kernel<uint64_t, uint64_t><<<grid, 256, sm, s>>>(p, d_idx, n, d_labels);
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
