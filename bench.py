@@ -1,0 +1,284 @@
+#!/usr/bin/env python
+"""bench.py - FTLM hot path on B200: fused Lanczos steps/s at D = 1.55e8 (BASELINE config 4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 4] [--mode clt|cr] [--kernel auto|row|tile] [--no-cpu-baseline]
+
+A "step" is one fused Lanczos step (row states, diagonal, gather with
+CLT or CR indexing, fused recurrence + FP64 reductions, normalisation pass) on the S^z = 0
+sector of the N = 30 icosidodecahedron in FP32; the one-time tables (A0/A1) are built before
+the timed region and the host parts (A8/A9) run once per chain inside the e2e measurement.
+Prints ONE JSON line (rank 0).  N > 1: one independent chain (replica) per GPU, no data-path
+collective ("scaling": "weak"); timing = max over ranks of the device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "lanczos_steps_per_s"
+UNIT = "steps/s"
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def recorded_traffic(kernel_key):
+    """dram bytes/launch of the dominant kernel from the committed ncu --set full capture."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(kernel_key)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in out.strip().split(",")]
+                if len(f) >= 6:
+                    self.rows.append(f)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[2 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+def oracle_hv_rate(w, n_up, budget_s=15.0):
+    """Time the C oracle's H.v (as it stands) on a bounded sample of rows of the same sector."""
+    from oracle import c_oracle as co
+    t0 = time.time()
+    basis = co.enumerate_basis(w.N, n_up)
+    t_enum = time.time() - t0
+    D = basis.shape[0]
+    rng = np.random.default_rng(0)
+    v = rng.standard_normal(D)
+    rows = min(D, 1 << 18)
+    t0 = time.time()
+    co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, v, 0, rows)
+    dt = max(time.time() - t0, 1e-6)
+    rows2 = int(min(D, max(rows, rows * budget_s / dt)))
+    row0 = (D - rows2) // 2                       # middle of the sector: typical rows
+    t0 = time.time()
+    co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, v, row0, rows2)
+    dt = time.time() - t0
+    return dict(rows_per_s=rows2 / dt, rows=rows2, row0=row0, seconds=dt, enum_seconds=t_enum,
+                cores=co.threads(), D=D)
+
+
+def run_reference(args, w, n_up):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import c_oracle as co
+    basis = co.enumerate_basis(w.N, n_up)
+    D = basis.shape[0]
+    rng = np.random.default_rng(0)
+    v = rng.standard_normal(D)
+    # size one "step" = a bounded slice of rows so that K + W steps finish within ~2 minutes
+    t0 = time.time()
+    co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, v, D // 2, 1 << 18)
+    per_row = (time.time() - t0) / (1 << 18)
+    rows = int(min(D, max(1 << 16, 100.0 / max(args.steps + args.warmup, 1) / per_row)))
+    row0 = (D - rows) // 2
+    for _ in range(args.warmup):
+        co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, v, row0, rows)
+    t0 = time.time()
+    for _ in range(args.steps):
+        co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, v, row0, rows)
+    dt = time.time() - t0
+    value = (rows * args.steps / dt) / D
+    sample = (f"FP64 C/OpenMP oracle H.v on rows [{row0}, {row0 + rows}) of the D={D} sector per step; "
+              f"steps/s = rows/s / D (vector updates of the recurrence not included)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": w.name, "N": w.N, "N_up": n_up, "dim": D,
+                                            "n_bonds": w.n_bonds, "sample_rows_per_step": rows},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": co.threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--mode", default="clt", choices=["clt", "cr"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "row", "tile"])
+    ap.add_argument("--low-bits", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    from paper_2605_26261_b200 import workloads as W
+    w = W.baseline_config(args.config)
+    n_up = w.sectors[0]
+    if args.impl == "reference":
+        run_reference(args, w, n_up)
+        return
+
+    import torch
+    from paper_2605_26261_b200 import ftlm
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    mode = ftlm.INDEX_CLT if args.mode == "clt" else ftlm.INDEX_CR
+    if w.N > 32:
+        mode, args.mode = ftlm.INDEX_CR, "cr"
+    ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, local)
+    if args.low_bits:
+        ftlm.ftlm_set_option(ctx, "low_bits", args.low_bits)
+    ftlm.ftlm_set_option(ctx, "kernel", {"auto": 0, "row": 1, "tile": 2}[args.kernel])
+    kernel_used = {1: "row", 2: "tile"}[ftlm.ftlm_get_option(ctx, "kernel")]
+    D = ftlm.ftlm_dim(ctx)
+    K, Wm = args.steps, args.warmup
+    assert 1 <= K and K + Wm <= ftlm.MAX_STEPS, "steps + warmup must be <= 1024 (one chain)"
+
+    # ---- device-resident timing: `value` ---------------------------------------------------
+    ftlm.ftlm_chain_begin(ctx, None, W.SEED_VECTORS, rank)       # one replica chain per rank
+    ftlm.ftlm_chain_steps(ctx, Wm)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    ftlm.ftlm_chain_steps(ctx, K)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    sampler.stop_flag = True
+    a, b, m_eff = ftlm.ftlm_chain_end(ctx)
+    assert m_eff == K + Wm and np.isfinite(a).all() and np.isfinite(b).all(), (m_eff, K + Wm)
+    t_ms = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms = float(t_ms.item())
+    value = world * K / (ms * 1e-3)
+
+    # ---- per-kernel timing for the roofline of the dominant kernel --------------------------
+    ftlm.ftlm_chain_begin(ctx, None, W.SEED_VECTORS, rank)
+    ftlm.ftlm_chain_steps(ctx, 3)
+    ms_hv, ms_norm = ftlm.ftlm_chain_profile(ctx, min(K, 30))
+    table_bytes = (8 * ((1 << w.N) // 32)) if mode == ftlm.INDEX_CLT else 0
+    alg_bytes = 12 * D + table_bytes             # floor A of SURVEY 8(d): v, v_prev, y + table
+    peak, peak_src = measured_peak()
+    achieved = alg_bytes / (ms_hv * 1e-3) / 1e9
+    kname = f"hv_{kernel_used}_{args.mode}_fp32_fused"
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": recorded_traffic(kname), "kernel": kname, "ms_per_launch": ms_hv,
+                "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
+                "norm_kernel_ms": ms_norm, "norm_kernel_GBps": 12 * D / (ms_norm * 1e-3) / 1e9 if ms_norm > 0 else None}
+
+    # ---- end-to-end through the host-buffer ABI call ---------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hq = torch.empty((1, D), dtype=torch.float32).pin_memory()
+        hq.normal_(generator=torch.Generator().manual_seed(1234 + rank))
+        hq_np = hq.numpy()
+        ke = min(K, 100)
+        ftlm.ftlm_lanczos_host(ctx, hq_np, 2)                     # warm-up of the path
+        barrier()
+        t0 = time.perf_counter()
+        out = ftlm.ftlm_lanczos_host(ctx, hq_np, ke)              # H2D start vector, ke steps, D2H alpha/beta, T eig
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        t_e = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        assert int(out["m_eff"][0]) == ke
+        e2e = {"value": world * ke / float(t_e.item()), "unit": UNIT, "h2d_bytes_per_step": 4 * D / ke,
+               "d2h_bytes_per_step": 16.0 + 8.0 / ke, "steps": ke,
+               "call": "ftlm_lanczos_host(pinned host start vector -> alpha, beta, theta, weight)"}
+
+    ftlm.ftlm_destroy(ctx)
+    if dist is not None:
+        dist.barrier()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        o = oracle_hv_rate(w, n_up)
+        cpu = {"value": o["rows_per_s"] / D, "unit": UNIT, "cores": o["cores"], "kind": "oracle",
+               "sample": (f"FP64 C/OpenMP oracle H.v on rows [{o['row0']}, {o['row0'] + o['rows']}) of the D={D} "
+                          f"sector ({o['seconds']:.1f} s); steps/s = rows/s / D; basis enumeration "
+                          f"({o['enum_seconds']:.1f} s) excluded"),
+               "rows_per_s": o["rows_per_s"]}
+
+    nnz = D + 2 * w.n_bonds * __import__("math").comb(w.N - 2, n_up - 1)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"config{args.config}:{w.name}", "N": w.N, "N_up": n_up, "dim": D,
+                       "n_bonds": w.n_bonds, "index_mode": args.mode, "kernel": kernel_used,
+                       "precision": "fp32 vectors, fp64 reductions", "l2": "inputs_exceed_l2 (3 x 620 MB vectors)",
+                       "parallelism": f"replicas x{world}"},
+            "hv_rows_per_s": world * D / (ms_hv * 1e-3), "hv_gelem_per_s": world * nnz / (ms_hv * 1e-3) / 1e9,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": 2 * K,
+            "clocks": sampler.summary()}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

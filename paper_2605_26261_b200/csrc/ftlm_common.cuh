@@ -72,7 +72,7 @@ struct ftlm_ctx {
 
   // chain workspace
   void* q[3] = {nullptr, nullptr, nullptr};
-  int cur = 0;                     // q[cur] = q_j, q[(cur+2)%3] = q_{j-1}, q[(cur+1)%3] = y
+  int cur = 0;                     // q[cur] = q_j, q[1-cur] = q_{j-1}, q[2] = y
   ChainState* d_state = nullptr;
   double* d_partials = nullptr;    // [3][max_blocks]
   unsigned int* d_ticket = nullptr;

@@ -418,16 +418,16 @@ static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64
     rc = ftlm_fill_random(c, seed, r, c->q[0], s);
     if (rc != FTLM_OK) return rc;
   } else {
-    // copy into q[1] (scratch), then normalise in FP64 into q[0]
-    CK(cudaMemcpyAsync(c->q[1], q1, bytes, q1_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
+    // copy into q[2] (scratch), then normalise in FP64 into q[0]
+    CK(cudaMemcpyAsync(c->q[2], q1, bytes, q1_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
     const int grid = stream_grid(c, c->dim, 8);
-    if (c->prec == FTLM_FP32) sumsq_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[1], c->dim, c->d_partials);
-    else sumsq_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[1], c->dim, c->d_partials);
+    if (c->prec == FTLM_FP32) sumsq_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[2], c->dim, c->d_partials);
+    else sumsq_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[2], c->dim, c->d_partials);
     reduce_partials_kernel<<<1, 256, 0, s>>>(c->d_partials, grid, &c->d_state->norm2);
-    if (c->prec == FTLM_FP32) scale_copy_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[1], c->dim, &c->d_state->norm2, (float*)c->q[0]);
-    else scale_copy_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[1], c->dim, &c->d_state->norm2, (double*)c->q[0]);
+    if (c->prec == FTLM_FP32) scale_copy_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[2], c->dim, &c->d_state->norm2, (float*)c->q[0]);
+    else scale_copy_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[2], c->dim, &c->d_state->norm2, (double*)c->q[0]);
   }
-  CK(cudaMemsetAsync(c->q[2], 0, bytes, s));          // q_0 = 0
+  CK(cudaMemsetAsync(c->q[1], 0, bytes, s));          // q_0 = 0
   chain_reset_kernel<<<1, 32, 0, s>>>(c->d_state, c->chain_limit, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
   CK(cudaGetLastError());
   return FTLM_OK;
@@ -439,9 +439,9 @@ extern "C" int ftlm_chain_begin(ftlm_ctx* c, const void* d_q1, uint64_t seed, in
 }
 
 static int launch_next(ftlm_ctx* c, cudaStream_t s) {
-  const void* y = c->q[(c->cur + 1) % 3];
+  const void* y = c->q[2];
   const void* q = c->q[c->cur];
-  void* qn = c->q[(c->cur + 2) % 3];
+  void* qn = c->q[1 - c->cur];
   const int grid = stream_grid(c, c->dim / 4 + 1, 8);
   if (c->prec == FTLM_FP32) lanczos_next_kernel<float, float4><<<grid, 256, 0, s>>>((const float*)y, (const float*)q, (float*)qn, c->dim, c->d_state);
   else lanczos_next_kernel<double, double2><<<grid, 256, 0, s>>>((const double*)y, (const double*)q, (double*)qn, c->dim, c->d_state);
@@ -452,7 +452,7 @@ static int launch_next(ftlm_ctx* c, cudaStream_t s) {
 static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv, float* ms_norm) {
   // y = H q_j - beta_{j-1} q_{j-1}   (+ reductions, alpha_j, beta_j on the device)
   if (timed) CK(cudaEventRecord(c->ev[0], s));
-  int rc = launch_hv(c, c->q[c->cur], c->q[(c->cur + 2) % 3], c->q[(c->cur + 1) % 3], 1, s);
+  int rc = launch_hv(c, c->q[c->cur], c->q[1 - c->cur], c->q[2], 1, s);
   if (rc != FTLM_OK) return rc;
   if (timed) CK(cudaEventRecord(c->ev[1], s));
   // q_{j+1} = (y - alpha_j q_j)/beta_j, written over q_{j-1}
@@ -464,8 +464,8 @@ static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv,
     CK(cudaEventElapsedTime(ms_hv, c->ev[0], c->ev[1]));
     CK(cudaEventElapsedTime(ms_norm, c->ev[1], c->ev[2]));
   }
-  // rotate: q_{j+1} lives in old q_{j-1}; old q_j becomes q_{j-1}; old y becomes scratch
-  c->cur = (c->cur + 2) % 3;
+  // swap roles: q_{j+1} lives in the old q_{j-1} buffer, the old q_j becomes q_{j-1}; y stays q[2]
+  c->cur = 1 - c->cur;
   c->steps_enqueued++;
   return FTLM_OK;
 }
