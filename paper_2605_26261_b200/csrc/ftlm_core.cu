@@ -281,8 +281,8 @@ extern "C" int64_t ftlm_table_bytes(const ftlm_ctx* c) {
 
 int ftlm_effective_kernel(const ftlm_ctx* c) {
   if (c->kernel == FTLM_KERNEL_ROW) return FTLM_KERNEL_ROW;
-  if (c->tile) return FTLM_KERNEL_TILE;
-  return FTLM_KERNEL_ROW;
+  if (c->tile && (c->kernel == FTLM_KERNEL_TILE || c->dim >= (1 << 20))) return FTLM_KERNEL_TILE;
+  return FTLM_KERNEL_ROW;                    // AUTO: small sectors are launch-bound, ROW is simpler
 }
 
 extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {

@@ -311,3 +311,58 @@ def test_thermodynamics_ring12_all_sectors_vs_oracle(mode, prec):
     assert _max_rel(got["C"], ref["C"]) <= tol
     assert _max_rel(got["chi"], ref["chi"]) <= tol
     assert _max_rel(got["E"], ref["E"]) <= tol
+
+
+# ---------------------------------------------------------------- TILE kernel: low-bit splits
+
+@pytest.mark.parametrize("prec", ["fp32", "fp64"])
+@pytest.mark.parametrize("mode", ["clt", "cr"])
+@pytest.mark.parametrize("w_bits", [6, 9, 12, 14, 15])
+def test_tile_kernel_low_bit_splits(prec, mode, w_bits):
+    # every ll / hh / mixed classification of the same bonds must give the same H.v and indices
+    rng = np.random.default_rng(w_bits)
+    w = W.triangular(4, 5)                       # N = 20, 60 bonds
+    J = rng.uniform(0.5, 1.5, w.n_bonds)
+    n_up = 9
+    basis = co.enumerate_basis(w.N, n_up)
+    v = rng.standard_normal(basis.shape[0]).astype(NDT[prec])
+    ref = co.apply_rows(w.N, w.bond_i, w.bond_j, J, 0.21, n_up, basis, v.astype(np.float64))
+    with Ctx(w, n_up, mode, prec, h=0.21, J=J) as c:
+        try:
+            ftlm.ftlm_set_option(c.ctx, "low_bits", w_bits)
+        except ftlm.FtlmError as e:
+            if e.code == ftlm.EUNSUPPORTED:
+                pytest.skip("split does not fit shared memory")
+            raise
+        ftlm.ftlm_set_option(c.ctx, "kernel", ftlm.KERNEL_TILE)
+        assert relerr(c.apply(v), ref) <= HV_TOL[prec]
+        got = c.neighbors(1000, 3000)
+        exp = co.neighbors_rows(w.N, w.bond_i, w.bond_j, basis, np.arange(1000, 4000))
+        assert (got == exp).all()
+
+
+def test_tile_and_row_kernels_agree_on_config3_slice_fp32():
+    # 4x7 triangular lattice (N = 28, D = 40 116 600): ROW vs TILE on the whole vector, and both
+    # against the oracle on a slice of rows
+    w = W.baseline_config(3)
+    n_up = 14
+    basis = co.enumerate_basis(w.N, n_up)
+    outs = {}
+    for mode in ("clt", "cr"):
+        with Ctx(w, n_up, mode, "fp32") as c:
+            v = c.fill_random(W.SEED_VECTORS, 0)
+            for kern in (ftlm.KERNEL_ROW, ftlm.KERNEL_TILE):
+                ftlm.ftlm_set_option(c.ctx, "kernel", kern)
+                y = torch.empty_like(v)
+                ftlm.ftlm_apply_H(c.ctx, v, y)
+                torch.cuda.synchronize()
+                outs[(mode, kern)] = y.cpu().numpy()
+            vh = v.cpu().numpy().astype(np.float64)
+    D = basis.shape[0]
+    for row0 in (0, D // 2 - 50000, D - 100000):
+        ref = co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, vh, row0, 100000)
+        for key, y in outs.items():
+            assert relerr(y[row0:row0 + 100000], ref) <= HV_TOL["fp32"], key
+    base = outs[("clt", ftlm.KERNEL_ROW)].astype(np.float64)
+    for key, y in outs.items():
+        assert relerr(y, base) <= 1e-6, key
