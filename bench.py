@@ -147,8 +147,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--mode", default="clt", choices=["clt", "cr"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "row", "tile"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "row", "tile", "tml"])
     ap.add_argument("--low-bits", type=int, default=0)
+    ap.add_argument("--tml-low-bits", type=int, default=0)
+    ap.add_argument("--tml-mid-bits", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -185,8 +187,12 @@ def main():
     ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, local)
     if args.low_bits:
         ftlm.ftlm_set_option(ctx, "low_bits", args.low_bits)
-    ftlm.ftlm_set_option(ctx, "kernel", {"auto": 0, "row": 1, "tile": 2}[args.kernel])
-    kernel_used = {1: "row", 2: "tile"}[ftlm.ftlm_get_option(ctx, "kernel")]
+    if args.tml_low_bits:
+        ftlm.ftlm_set_option(ctx, "tml_low_bits", args.tml_low_bits)
+    if args.tml_mid_bits:
+        ftlm.ftlm_set_option(ctx, "tml_mid_bits", args.tml_mid_bits)
+    ftlm.ftlm_set_option(ctx, "kernel", {"auto": 0, "row": 1, "tile": 2, "tml": 3}[args.kernel])
+    kernel_used = {1: "row", 2: "tile", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
     D = ftlm.ftlm_dim(ctx)
     K, Wm = args.steps, args.warmup
     assert 1 <= K and K + Wm <= ftlm.MAX_STEPS, "steps + warmup must be <= 1024 (one chain)"

@@ -41,8 +41,10 @@ enum { FTLM_FP32 = 0, FTLM_FP64 = 1 };
 /* Kernel variants selectable with ftlm_set_option("kernel", ...).
  * ROW  = one thread per row, every row unranked, per-bond loop (the paper's launch shape, L105,
  *        L136, L203), kept as the plain in-library baseline.
- * TILE = B200 design: one CTA per run of rows sharing the high label bits. */
-enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_TILE = 2 };
+ * TILE = one CTA per run of rows sharing the high label bits.
+ * TML  = B200 design: label split into top/middle/low parts, one CTA per top part with the tile
+ *        staged in shared memory and per-class neighbour tables. */
+enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_TILE = 2, FTLM_KERNEL_TML = 3 };
 
 /* ---- handle ------------------------------------------------------------------------------ */
 
@@ -63,7 +65,11 @@ int ftlm_destroy(ftlm_ctx* ctx);
 int64_t ftlm_dim(const ftlm_ctx* ctx);
 
 /* Options: "kernel" (FTLM_KERNEL_*), "low_bits" (w of the TILE kernels, 0 = auto),
- * "graph" (1 = replay Lanczos steps from a CUDA graph).  FTLM_EINVAL on unknown key/value. */
+ * "tml_low_bits" / "tml_mid_bits" (w, m of the TML kernels, 0 = auto), "graph" (1 = replay
+ * Lanczos steps from a CUDA graph).  FTLM_EINVAL on unknown key/value, FTLM_EUNSUPPORTED when
+ * the requested kernel / split cannot be built for this sector.  ftlm_get_option also answers
+ * the read-only keys "sm_count", "tml_w", "tml_m", "tml_smem", "tml_ctas_per_sm",
+ * "tml_threads", "tml_n_ll", "tml_n_mm", "tml_n_ml", "tml_n_tt", "tml_n_tm", "tml_n_tl". */
 int ftlm_set_option(ftlm_ctx* ctx, const char* key, int64_t value);
 int64_t ftlm_get_option(const ftlm_ctx* ctx, const char* key);
 

@@ -41,8 +41,10 @@ struct BondDev {          // one bond as the kernels see it
   int i, j;               // i < j
 };
 
-// Run-tiled ("TILE") kernel plan, built on the host in ftlm_create.
+// Run-tiled ("TILE") and three-level ("TML") kernel plans, built on the host in ftlm_create
+// (DESIGN.md section 6).
 struct TilePlan;
+struct TmlPlan;
 
 struct ftlm_ctx {
   int N = 0, nb = 0, N_up = 0, mode = 0, prec = 0, device = 0;
@@ -65,10 +67,13 @@ struct ftlm_ctx {
   // options
   int kernel = FTLM_KERNEL_AUTO;
   int low_bits = 0;
+  int tml_low_bits = 0, tml_mid_bits = 0;
   int use_graph = 0;
 
   // tile plan (ftlm_tile.cu)
   TilePlan* tile = nullptr;
+  // three-level tile plan (ftlm_tml.cu)
+  TmlPlan* tml = nullptr;
 
   // chain workspace
   void* q[3] = {nullptr, nullptr, nullptr};
@@ -95,6 +100,12 @@ int ftlm_tile_plan_create(ftlm_ctx* c);
 void ftlm_tile_plan_destroy(ftlm_ctx* c);
 int ftlm_launch_hv_tile(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
 int ftlm_launch_neighbors_tile(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
+
+int ftlm_tml_plan_create(ftlm_ctx* c);
+void ftlm_tml_plan_destroy(ftlm_ctx* c);
+int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key);
+int ftlm_launch_hv_tml(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
+int ftlm_launch_neighbors_tml(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
 
 // ---- device helpers ---------------------------------------------------------------------
 #ifdef __CUDACC__

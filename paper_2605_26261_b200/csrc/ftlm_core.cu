@@ -252,6 +252,8 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
   for (int k = 0; k < 4; ++k) CKF(cudaEventCreate(&c->ev[k]));
   rc = ftlm_tile_plan_create(c);
   if (rc != FTLM_OK) return fail(rc);
+  rc = ftlm_tml_plan_create(c);
+  if (rc != FTLM_OK) return fail(rc);
   CKF(cudaDeviceSynchronize());
 #undef CKF
   *out = c;
@@ -262,6 +264,7 @@ extern "C" int ftlm_destroy(ftlm_ctx* c) {
   if (!c) return FTLM_OK;
   cudaSetDevice(c->device);
   ftlm_tile_plan_destroy(c);
+  ftlm_tml_plan_destroy(c);
   cudaFree(c->d_binom64); cudaFree(c->d_binom32); cudaFree(c->d_bonds); cudaFree(c->d_clt);
   cudaFree(c->d_state); cudaFree(c->d_partials); cudaFree(c->d_ticket);
   for (int k = 0; k < 3; ++k) cudaFree(c->q[k]);
@@ -281,6 +284,7 @@ extern "C" int64_t ftlm_table_bytes(const ftlm_ctx* c) {
 
 int ftlm_effective_kernel(const ftlm_ctx* c) {
   if (c->kernel == FTLM_KERNEL_ROW) return FTLM_KERNEL_ROW;
+  if (c->kernel == FTLM_KERNEL_TML && c->tml) return FTLM_KERNEL_TML;
   if (c->tile && (c->kernel == FTLM_KERNEL_TILE || c->dim >= (1 << 20))) return FTLM_KERNEL_TILE;
   return FTLM_KERNEL_ROW;                    // AUTO: small sectors are launch-bound, ROW is simpler
 }
@@ -288,8 +292,9 @@ int ftlm_effective_kernel(const ftlm_ctx* c) {
 extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   if (!c || !key) { ftlm_set_error("ftlm_set_option: NULL"); return FTLM_EINVAL; }
   if (!strcmp(key, "kernel")) {
-    if (value < 0 || value > 2) { ftlm_set_error("kernel must be 0..2"); return FTLM_EINVAL; }
+    if (value < 0 || value > 3) { ftlm_set_error("kernel must be 0..3"); return FTLM_EINVAL; }
     if (value == FTLM_KERNEL_TILE && !c->tile) { ftlm_set_error("TILE kernel unavailable for this sector"); return FTLM_EUNSUPPORTED; }
+    if (value == FTLM_KERNEL_TML && !c->tml) { ftlm_set_error("TML kernel unavailable for this sector"); return FTLM_EUNSUPPORTED; }
     c->kernel = (int)value; return FTLM_OK;
   }
   if (!strcmp(key, "low_bits")) {
@@ -299,6 +304,17 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     ftlm_tile_plan_destroy(c);
     int rc = ftlm_tile_plan_create(c);
     if (rc != FTLM_OK) { c->low_bits = old; ftlm_tile_plan_destroy(c); ftlm_tile_plan_create(c); }
+    return rc;
+  }
+  if (!strcmp(key, "tml_low_bits") || !strcmp(key, "tml_mid_bits")) {
+    if (value < 0 || value > 16) { ftlm_set_error("%s must be 0..16", key); return FTLM_EINVAL; }
+    int* slot = !strcmp(key, "tml_low_bits") ? &c->tml_low_bits : &c->tml_mid_bits;
+    const int old = *slot;
+    *slot = (int)value;
+    CK(cudaSetDevice(c->device));
+    ftlm_tml_plan_destroy(c);
+    int rc = ftlm_tml_plan_create(c);
+    if (rc != FTLM_OK) { *slot = old; ftlm_tml_plan_destroy(c); ftlm_tml_plan_create(c); }
     return rc;
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
@@ -312,6 +328,7 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "low_bits")) return c->low_bits;
   if (!strcmp(key, "graph")) return c->use_graph;
   if (!strcmp(key, "sm_count")) return c->sm_count;
+  if (!strncmp(key, "tml_", 4)) return ftlm_tml_info(c, key);
   return -1;
 }
 
@@ -328,7 +345,9 @@ extern "C" int ftlm_clt_read(ftlm_ctx* c, int64_t b0, int64_t nb, uint32_t* h_ma
 
 // ---- H.v ---------------------------------------------------------------------------------------
 static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
-  if (ftlm_effective_kernel(c) == FTLM_KERNEL_TILE) return ftlm_launch_hv_tile(c, v, qp, y, fused, s);
+  const int k = ftlm_effective_kernel(c);
+  if (k == FTLM_KERNEL_TML) return ftlm_launch_hv_tml(c, v, qp, y, fused, s);
+  if (k == FTLM_KERNEL_TILE) return ftlm_launch_hv_tile(c, v, qp, y, fused, s);
   return ftlm_launch_hv_row(c, v, qp, y, fused, s);
 }
 
@@ -361,6 +380,7 @@ extern "C" int ftlm_neighbors(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
   }
   if (nrows == 0 || c->nb == 0) return FTLM_OK;
   CK(cudaSetDevice(c->device));
+  if (ftlm_effective_kernel(c) == FTLM_KERNEL_TML) return ftlm_launch_neighbors_tml(c, row0, nrows, d_idx, (cudaStream_t)stream);
   if (ftlm_effective_kernel(c) == FTLM_KERNEL_TILE) return ftlm_launch_neighbors_tile(c, row0, nrows, d_idx, (cudaStream_t)stream);
   return ftlm_launch_neighbors_row(c, row0, nrows, d_idx, (cudaStream_t)stream);
 }

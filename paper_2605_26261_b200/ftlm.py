@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libftlm.so")
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
 INDEX_CLT, INDEX_CR = 0, 1
 FP32, FP64 = 0, 1
-KERNEL_AUTO, KERNEL_ROW, KERNEL_TILE = 0, 1, 2
+KERNEL_AUTO, KERNEL_ROW, KERNEL_TILE, KERNEL_TML = 0, 1, 2, 3
 MAX_STEPS = 1024
 
 EXPORTS = [

@@ -15,7 +15,7 @@ from paper_2605_26261_b200 import ftlm         # noqa: E402
 from paper_2605_26261_b200 import workloads as W   # noqa: E402
 from gpu_util import Ctx, HV_TOL, NDT, relerr  # noqa: E402
 
-KERNELS = [ftlm.KERNEL_ROW, ftlm.KERNEL_TILE]
+KERNELS = [ftlm.KERNEL_ROW, ftlm.KERNEL_TILE, ftlm.KERNEL_TML]
 
 
 def _kernel_ok(c, kernel):
@@ -341,6 +341,53 @@ def test_tile_kernel_low_bit_splits(prec, mode, w_bits):
         assert (got == exp).all()
 
 
+@pytest.mark.parametrize("prec", ["fp32", "fp64"])
+@pytest.mark.parametrize("mode", ["clt", "cr"])
+@pytest.mark.parametrize("w_bits,m_bits", [(5, 1), (6, 4), (8, 7), (9, 7), (10, 6), (12, 3), (7, 9), (5, 9)])
+def test_tml_kernel_splits(prec, mode, w_bits, m_bits):
+    # every LL/MM/ML/TT/TM/TL classification of the same bonds must give the same H.v and indices
+    rng = np.random.default_rng(100 * w_bits + m_bits)
+    w = W.triangular(4, 5)                       # N = 20, 60 bonds
+    J = rng.uniform(0.5, 1.5, w.n_bonds)
+    n_up = 9
+    basis = co.enumerate_basis(w.N, n_up)
+    v = rng.standard_normal(basis.shape[0]).astype(NDT[prec])
+    ref = co.apply_rows(w.N, w.bond_i, w.bond_j, J, 0.21, n_up, basis, v.astype(np.float64))
+    with Ctx(w, n_up, mode, prec, h=0.21, J=J) as c:
+        try:
+            ftlm.ftlm_set_option(c.ctx, "tml_low_bits", w_bits)
+            ftlm.ftlm_set_option(c.ctx, "tml_mid_bits", m_bits)
+        except ftlm.FtlmError as e:
+            if e.code == ftlm.EUNSUPPORTED:
+                pytest.skip("split does not fit shared memory / class caps")
+            raise
+        assert ftlm.ftlm_get_option(c.ctx, "tml_w") == w_bits and ftlm.ftlm_get_option(c.ctx, "tml_m") == m_bits
+        ftlm.ftlm_set_option(c.ctx, "kernel", ftlm.KERNEL_TML)
+        assert ftlm.ftlm_get_option(c.ctx, "kernel") == ftlm.KERNEL_TML
+        assert relerr(c.apply(v), ref) <= HV_TOL[prec]
+        assert relerr(c.apply(v), ref) <= HV_TOL[prec]          # second launch: counters were reset
+        D = c.dim
+        for row0, nrows in ((0, 3000), (D // 2, 3000), (D - 2000, 2000)):
+            got = c.neighbors(row0, nrows)
+            exp = co.neighbors_rows(w.N, w.bond_i, w.bond_j, basis, np.arange(row0, row0 + nrows))
+            assert (got == exp).all()
+
+
+def test_tml_lanczos_is_bit_reproducible_and_matches_row():
+    # dynamic tile scheduling must not change alpha, beta run to run (per-tile partial sums added in
+    # fixed order); TML and ROW agree to FP64 round-off in FP64 mode
+    w = W.ring(22, 1.0, 0.5)
+    n_up = 11
+    outs = []
+    with Ctx(w, n_up, "cr", "fp64") as c:
+        for kern in (ftlm.KERNEL_TML, ftlm.KERNEL_TML, ftlm.KERNEL_ROW):
+            ftlm.ftlm_set_option(c.ctx, "kernel", kern)
+            outs.append(ftlm.ftlm_lanczos(c.ctx, W.SEED_VECTORS, 1, 40))
+    assert (outs[0]["alpha"] == outs[1]["alpha"]).all() and (outs[0]["beta"] == outs[1]["beta"]).all()
+    assert np.abs(outs[0]["alpha"][0, :10] - outs[2]["alpha"][0, :10]).max() < 1e-10
+    assert abs(outs[0]["theta"][0, 0] - outs[2]["theta"][0, 0]) < 1e-9
+
+
 def test_tile_and_row_kernels_agree_on_config3_slice_fp32():
     # 4x7 triangular lattice (N = 28, D = 40 116 600): ROW vs TILE on the whole vector, and both
     # against the oracle on a slice of rows
@@ -351,7 +398,7 @@ def test_tile_and_row_kernels_agree_on_config3_slice_fp32():
     for mode in ("clt", "cr"):
         with Ctx(w, n_up, mode, "fp32") as c:
             v = c.fill_random(W.SEED_VECTORS, 0)
-            for kern in (ftlm.KERNEL_ROW, ftlm.KERNEL_TILE):
+            for kern in (ftlm.KERNEL_ROW, ftlm.KERNEL_TILE, ftlm.KERNEL_TML):
                 ftlm.ftlm_set_option(c.ctx, "kernel", kern)
                 y = torch.empty_like(v)
                 ftlm.ftlm_apply_H(c.ctx, v, y)
