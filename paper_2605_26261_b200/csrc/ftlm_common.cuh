@@ -104,7 +104,7 @@ int ftlm_launch_neighbors_tile(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t
 int ftlm_tml_plan_create(ftlm_ctx* c);
 void ftlm_tml_plan_destroy(ftlm_ctx* c);
 int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key);
-int ftlm_launch_hv_tml(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
+int ftlm_launch_hv_tml(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, int batch, cudaStream_t s);
 int ftlm_launch_neighbors_tml(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
 
 // ---- device helpers ---------------------------------------------------------------------

@@ -346,7 +346,7 @@ extern "C" int ftlm_clt_read(ftlm_ctx* c, int64_t b0, int64_t nb, uint32_t* h_ma
 // ---- H.v ---------------------------------------------------------------------------------------
 static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
   const int k = ftlm_effective_kernel(c);
-  if (k == FTLM_KERNEL_TML) return ftlm_launch_hv_tml(c, v, qp, y, fused, s);
+  if (k == FTLM_KERNEL_TML) return ftlm_launch_hv_tml(c, v, qp, y, fused, 1, s);
   if (k == FTLM_KERNEL_TILE) return ftlm_launch_hv_tile(c, v, qp, y, fused, s);
   return ftlm_launch_hv_row(c, v, qp, y, fused, s);
 }

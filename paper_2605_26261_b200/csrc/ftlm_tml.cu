@@ -5,18 +5,22 @@
 // popc(T)); inside it the rows sharing M are one contiguous "column" (C(w, kL) rows, kL = kT -
 // popc(M)), ordered by lr(L) = rank of L among the w-bit words of equal popcount:
 //     index(n) = base(T) + coloff[kT][M] + lr(L).
-// One CTA stages one tile in shared memory; one warp owns 32 consecutive rows of one column, so
-// everything that depends on (T, M) alone is warp-uniform.  The 6 bond classes (by where the two
-// sites sit) cost, per row:
-//   LL  in-column permutation      -> shared-memory table LLtab[bond][L] (self if parallel)
-//   MM  column -> column, same lr  -> conflict-free shared-memory read, warp-uniform test
-//   ML  column change + flip of L_i-> shared-memory read at FLtab[i][L], per-lane test
-//   TT  tile -> tile, same offset  -> coalesced global stream (L2), tile-uniform test
-//   TM  tile and column change     -> coalesced global read, warp-uniform test
-//   TL  tile change + flip of L_i  -> global gather at FLtab[i][L], per-lane test
-// Every bond contributes (J_b/2) (v[swap_b n] - v[n]) on top of diag0 * v[n] (Eq. 12 with the
-// s=1/2 coefficients of Eqs. 13-14: an antiparallel bond has the off-diagonal element J/2 and
-// lowers the diagonal from +J/4 to -J/4).
+// One CTA stages one tile in shared memory; one warp owns up to 4 x 32 consecutive rows of one
+// column, so everything that depends on (T, M) alone is warp-uniform.  Per column the warp first
+// builds, cooperatively (lane e handles list entry e), compact descriptor lists in its own
+// shared-memory scratch; the row loop then only walks those lists.  The 6 bond classes:
+//   LL  in-column permutation       -> table LLtab[bond][L] in shared memory (self if parallel)
+//   MM  column -> column, same lr   -> S list {column offset, J}: conflict-free smem read
+//   ML  column change + flip of L_i -> FS list {column offset, J, i, M_j}: smem read at FLtab[i][L]
+//   TT  tile -> tile, same offset   -> U list {row offset, J}: coalesced global read (L2)
+//   TM  tile and column change      -> U list, coalesced global read
+//   TL  tile change + flip of L_i   -> FG list: global gather at FLtab[i][L]
+// S and U lists hold only the bonds that are antiparallel for this (T, M); the FS/FG tests
+// (L_i != partner bit) are per lane.  Every bond contributes (J_b/2) (v[swap_b n] - v[n]) on top
+// of diag0 * v[n] (Eq. 12 with the s=1/2 coefficients of Eqs. 13-14: an antiparallel bond has the
+// off-diagonal element J/2 and lowers the diagonal from +J/4 to -J/4).
+// B interleaved vectors (v[t][B]) share all of the index work (the paper's batched Lanczos,
+// L207, L309).
 // Index strategies (bit-exact with ROW and the oracle): CR ranks T' with the binomial table in
 // shared memory (Eq. 15-16 at d=2) - the rank is updated only across the flipped positions
 // because coloff/FLtab/LLtab hold the low-part ranks; CLT reads base(T') = C_b of block
@@ -26,65 +30,108 @@
 // buffer indexed by T and added in fixed order by the last CTA (bit-reproducible alpha, beta).
 #include <algorithm>
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 #include "ftlm_common.cuh"
 
 #define TML_MAX_LL 32
-#define TML_MAX_MM 32
-#define TML_MAX_ML 32
 #define TML_MAX_TT 64
 #define TML_MAX_TS 32
-#define TML_MAX_TX 64
-#define TML_MAX_THREADS 1024
+#define TML_MAX_LIST 64            // entries per static list (MM, ML, TM, TL)
+#define TML_MAX_CHUNKS 8           // 32-row chunks per work item
+
+struct TmlSEnt { uint32_t a, b; double J; };   // static list entry (see the plan builder)
 
 template <typename R>
 struct TmlParams {
   int N, K, w, m, t, mw, mode;
   uint32_t nT;
-  int n_ll4, n_mm, n_ml, n_tt, n_ts;
-  int max_tile;
+  int n_ll4, n_mm, n_ml, n_tt, n_ts, n_tm, n_tl;
+  int max_tile, scratch_bytes;
   int64_t dim;
   const uint64_t* binom;              // [(N+1)*(K+1)] global
   const uint2* clt;                   // CLT mode: base(T') = clt[T' << (mw-5)].y
   const unsigned char* blob;          // tables staged into shared memory
-  int blob_bytes, off_koff, off_lstate, off_coloff, off_ll, off_fl, off_tlen;
-  const uint32_t* items;              // (M | chunk << 16), grouped by kT
+  int blob_bytes, off_koff, off_tlen, off_coloff, off_ll, off_fl, off_mm, off_ml, off_tm, off_tl;
+  const uint32_t* items;              // M | chunk0 << 16 | nchunks << 24, grouped by kT
   const int* item_off;                // [mw + 2]
-  double* partials;                   // [3][nT]
+  double* partials;                   // [3*B][nT]
   unsigned int* counter;              // [0] tile counter, [1] ticket
-  ChainState* st;
+  ChainState* st;                     // [B]
   R diag_coef;                        // diag0 - sum_{LL} J_b/2  (LL bonds are in swap form)
   R ll_J[TML_MAX_LL];
-  uint32_t mm_mask[TML_MAX_MM]; R mm_J[TML_MAX_MM];
-  uint8_t ml_i[TML_MAX_ML], ml_j[TML_MAX_ML]; R ml_J[TML_MAX_ML];
-  uint32_t tt_mask[TML_MAX_TT]; R tt_J[TML_MAX_TT];
-  uint8_t ts_site[TML_MAX_TS], ts_first[TML_MAX_TS + 1];
-  uint8_t tx_kind[TML_MAX_TX], tx_i[TML_MAX_TX]; R tx_J[TML_MAX_TX];
+  uint32_t tt_mask[TML_MAX_TT]; double tt_J[TML_MAX_TT];
+  uint8_t ts_site[TML_MAX_TS];
 };
 
 struct TmlPlan {
   int w = 0, m = 0, t = 0;
-  int n_ll = 0, n_ll4 = 0, n_mm = 0, n_ml = 0, n_tt = 0, n_ts = 0, n_tx = 0;
-  int threads = 512, ctas_per_sm = 1, max_tile = 0;
+  int n_ll = 0, n_ll4 = 0, n_mm = 0, n_ml = 0, n_tt = 0, n_ts = 0, n_tm = 0, n_tl = 0;
+  int max_tile = 0;
   uint32_t nT = 0;
-  size_t smem_bytes = 0;
   unsigned char* d_blob = nullptr;
-  int blob_bytes = 0, off_koff = 0, off_lstate = 0, off_coloff = 0, off_ll = 0, off_fl = 0, off_tlen = 0;
+  int blob_bytes = 0, off_koff = 0, off_tlen = 0, off_coloff = 0, off_ll = 0, off_fl = 0, off_mm = 0, off_ml = 0,
+      off_tm = 0, off_tl = 0;
   uint32_t* d_items = nullptr;
   int* d_item_off = nullptr;
-  double* d_partials = nullptr;
+  double* d_partials = nullptr;       // [3 * max_batch][nT]
+  int partials_batch = 0;
   unsigned int* d_counter = nullptr;
   int* d_bond_class = nullptr;        // per original bond: class 0..5 (LL, MM, ML, TT, TM, TL)
-  int* d_bond_entry = nullptr;        // index in the class list (TM/TL: index in tx list)
-  int* d_bond_ts = nullptr;           // TM/TL: index of the T-site entry
+  int* d_bond_entry = nullptr;        // index in the class list
   double diag_coef = 0.0;
-  std::vector<double> ll_J, mm_J, ml_J, tt_J, tx_J;
-  std::vector<uint32_t> mm_mask, tt_mask;
-  std::vector<uint8_t> ml_i, ml_j, ts_site, ts_first, tx_kind, tx_i;
+  std::vector<double> ll_J, tt_J;
+  std::vector<uint32_t> tt_mask;
+  std::vector<uint8_t> ts_site;
+  std::vector<TmlSEnt> mm, ml, tm, tl;
 };
 
 namespace {
+
+// ---- B interleaved values of R --------------------------------------------------------------
+template <typename R, int B>
+struct __align__((sizeof(R) * B) > 16 ? 16 : (sizeof(R) * B)) Vec { R x[B]; };
+
+template <typename V> __device__ __forceinline__ V vec_ldg(const V* p) {
+  V r;
+  if constexpr (sizeof(V) == 4) *(float*)&r = __ldg((const float*)p);
+  else if constexpr (sizeof(V) == 8) *(float2*)&r = __ldg((const float2*)p);
+  else {
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(V) / 16); ++k) ((float4*)&r)[k] = __ldg((const float4*)p + k);
+  }
+  return r;
+}
+template <typename V> __device__ __forceinline__ V vec_ldcs(const V* p) {
+  V r;
+  if constexpr (sizeof(V) == 4) *(float*)&r = __ldcs((const float*)p);
+  else if constexpr (sizeof(V) == 8) *(float2*)&r = __ldcs((const float2*)p);
+  else {
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(V) / 16); ++k) ((float4*)&r)[k] = __ldcs((const float4*)p + k);
+  }
+  return r;
+}
+template <typename V> __device__ __forceinline__ void vec_stcs(V* p, const V& r) {
+  if constexpr (sizeof(V) == 4) __stcs((float*)p, *(const float*)&r);
+  else if constexpr (sizeof(V) == 8) __stcs((float2*)p, *(const float2*)&r);
+  else {
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(V) / 16); ++k) __stcs((float4*)p + k, ((const float4*)&r)[k]);
+  }
+}
+
+// descriptor entries of the per-warp scratch lists
+template <typename R> struct UEnt;      // uniform gather: {offset, J}
+template <> struct __align__(8) UEnt<float> { uint32_t off; float J; };
+template <> struct __align__(16) UEnt<double> { uint32_t off, pad; double J; };
+// flip gather: {row offset of the target column minus (!u << 15), J, FLtab row offset (bytes), u << 15}:
+// an active lane (L_i != u) reads FLtab = row | (!u << 15), so target row = off + FLtab entry.
+template <typename R> struct FEnt;
+template <> struct __align__(16) FEnt<float> { uint32_t off; float J; uint32_t fl, uw; };
+template <> struct __align__(16) FEnt<double> { uint32_t off, fl; double J; uint32_t uw, pad0, pad1, pad2; };
+struct TmlTx { uint32_t off; int cofs; uint32_t u; int valid; };   // per-tile data of one TM / TL entry
 
 // base(T): number of sector labels below T << mw (same combinatorial sum as Eq. 15-16 at d=2).
 __device__ __forceinline__ uint64_t tml_base_cr(uint32_t T, int mw, int K, const uint64_t* __restrict__ binom) {
@@ -111,43 +158,72 @@ __device__ __forceinline__ uint64_t tml_base(uint32_t T, int mw, int K, const ui
 struct TmlSmem {
   uint64_t* binom;
   unsigned char* blob;
-  unsigned char* vs;          // tile buffer (R[max_tile])
-  long long* tt_base;         // [TML_MAX_TT] active TT bonds of the current tile (compacted)
-  double* tt_J;               // [TML_MAX_TT] (stored as double, converted on use)
-  long long* ts_base;         // [TML_MAX_TS]
-  int* ts_kT;                 // [TML_MAX_TS]  (-1 = neighbour tile does not exist)
-  double* red;                // [96]
+  unsigned char* vs;          // tile buffer (B * R [max_tile])
+  uint32_t* tt_off;           // [TML_MAX_TT] base of the neighbour tile of each ACTIVE TT bond (compacted)
+  double* tt_J;               // [TML_MAX_TT]
+  TmlTx* txm;                 // [TML_MAX_LIST] per-tile data of the TM entries
+  TmlTx* txl;                 // [TML_MAX_LIST] per-tile data of the TL entries
+  double* red;                // [32 warps][3 * B]
   int* misc;                  // [0] tile index, [1] n active TT
-  long long* base;            // [0] base of the current tile
+  unsigned char* scratch;     // [warps][scratch_bytes]
 };
 
 __host__ __device__ inline size_t tml_layout(TmlSmem& s, unsigned char* p0, int N, int K, int blob_bytes,
-                                             int max_tile, int esz) {
+                                             int max_tile, int row_bytes, int batch, int warps, int scratch_bytes) {
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return p0 + at; };
   s.binom = (uint64_t*)take((size_t)(N + 1) * (K + 1) * 8);
   s.blob = take((size_t)blob_bytes);
-  s.vs = take((size_t)max_tile * esz + 16);
-  s.tt_base = (long long*)take(TML_MAX_TT * 8);
+  s.vs = take((size_t)max_tile * row_bytes + 32);
+  s.tt_off = (uint32_t*)take(TML_MAX_TT * 4);
   s.tt_J = (double*)take(TML_MAX_TT * 8);
-  s.ts_base = (long long*)take(TML_MAX_TS * 8);
-  s.ts_kT = (int*)take(TML_MAX_TS * 4);
-  s.red = (double*)take(96 * 8);
+  s.txm = (TmlTx*)take(TML_MAX_LIST * sizeof(TmlTx));
+  s.txl = (TmlTx*)take(TML_MAX_LIST * sizeof(TmlTx));
+  s.red = (double*)take((size_t)32 * 3 * batch * 8);
   s.misc = (int*)take(16);
-  s.base = (long long*)take(16);
+  s.scratch = take((size_t)warps * scratch_bytes);
   return o;
 }
 
-template <typename R, int MODE, bool FUSED>
-__global__ void __launch_bounds__(TML_MAX_THREADS, 1)
-hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v, const R* __restrict__ qprev,
-              R* __restrict__ y) {
+__host__ __device__ inline int tml_scratch_bytes(int esz, int n_tt, int n_tm, int n_mm, int n_ml, int n_tl) {
+  const int ue = esz == 4 ? 8 : 16, fe = esz == 4 ? 16 : 32;
+  auto r16 = [](int x) { return (x + 15) & ~15; };
+  return r16((n_tt + n_tm + 4) * ue) + r16((n_mm + 4) * ue) + r16((n_ml + 4) * fe) + r16((n_tl + 4) * fe);
+}
+
+__device__ __forceinline__ void load_fent(const FEnt<float>* e, uint32_t& off, float& J, uint32_t& fl, uint32_t& uw) {
+  const uint4 q = *(const uint4*)e;
+  off = q.x; J = __uint_as_float(q.y); fl = q.z; uw = q.w;
+}
+__device__ __forceinline__ void load_fent(const FEnt<double>* e, uint32_t& off, double& J, uint32_t& fl, uint32_t& uw) {
+  off = e->off; fl = e->fl; J = e->J; uw = e->uw;
+}
+__device__ __forceinline__ const void* addr_u32(const void* base, uint32_t idx, uint32_t scale) {
+  unsigned long long a;
+  asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(a) : "r"(idx), "r"(scale), "l"((unsigned long long)base));
+  return (const void*)a;
+}
+
+template <typename R, int B, int MODE, bool FUSED>
+__global__ void __launch_bounds__(B >= 4 ? 512 : 1024, 1)
+hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, const R* __restrict__ qprev_,
+              R* __restrict__ y_) {
+  typedef Vec<R, B> V;
+  constexpr int RB = (int)sizeof(V);                    // bytes per row
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ bool s_last;
-  if (FUSED) { if (p.st->done) return; }
-  TmlSmem S;
-  tml_layout(S, smem, p.N, p.K, p.blob_bytes, p.max_tile, (int)sizeof(R));
+  if (FUSED) {
+    bool all_done = true;
+#pragma unroll
+    for (int b = 0; b < B; ++b) all_done = all_done && p.st[b].done;
+    if (all_done) return;
+  }
+  const V* __restrict__ v = (const V*)v_;
+  const V* __restrict__ qprev = (const V*)qprev_;
+  V* __restrict__ y = (V*)y_;
   const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
+  TmlSmem S;
+  tml_layout(S, smem, p.N, p.K, p.blob_bytes, p.max_tile, RB, B, NW, p.scratch_bytes);
   // ---- one-time staging of the tables --------------------------------------------------------
   for (int k = tid; k < (p.N + 1) * (p.K + 1); k += NT) S.binom[k] = p.binom[k];
   {
@@ -156,14 +232,26 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v, c
     for (int k = tid; k < (p.blob_bytes >> 4); k += NT) dst[k] = __ldg(&src[k]);
   }
   const int* s_koff = (const int*)(S.blob + p.off_koff);
-  const uint16_t* s_lstate = (const uint16_t*)(S.blob + p.off_lstate);
+  const int* s_tlen = (const int*)(S.blob + p.off_tlen);
   const uint16_t* s_coloff = (const uint16_t*)(S.blob + p.off_coloff);       // [kT][M]
-  const uint2* s_ll = (const uint2*)(S.blob + p.off_ll);                     // [group][Lidx] 4 x u16 byte offsets
-  const uint16_t* s_fl = (const uint16_t*)(S.blob + p.off_fl);               // [i][Lidx] byte offset
-  const int* s_tlen = (const int*)(S.blob + p.off_tlen);                     // [kT]
+  const uint2* s_ll = (const uint2*)(S.blob + p.off_ll);                     // [group][Lidx] 4 x u16 rows
+  const unsigned char* s_fl = S.blob + p.off_fl;                             // u16 [i][Lidx]: row | L_i << 15
+  const TmlSEnt* s_mm = (const TmlSEnt*)(S.blob + p.off_mm);
+  const TmlSEnt* s_ml = (const TmlSEnt*)(S.blob + p.off_ml);
+  const TmlSEnt* s_tm = (const TmlSEnt*)(S.blob + p.off_tm);
+  const TmlSEnt* s_tl = (const TmlSEnt*)(S.blob + p.off_tl);
   const int nL = 1 << p.w, nM = 1 << p.m;
-  const R bprev = FUSED ? (R)p.st->beta_prev : (R)0;
-  const unsigned char* vsb0 = S.vs;
+  // per-warp scratch lists
+  auto r16 = [](int x) { return (x + 15) & ~15; };
+  unsigned char* sc = S.scratch + (size_t)warp * p.scratch_bytes;
+  UEnt<R>* const Ul = (UEnt<R>*)sc;
+  UEnt<R>* const Sl = (UEnt<R>*)(sc + r16((p.n_tt + p.n_tm + 4) * (int)sizeof(UEnt<R>)));
+  FEnt<R>* const FSl = (FEnt<R>*)((unsigned char*)Sl + r16((p.n_mm + 4) * (int)sizeof(UEnt<R>)));
+  FEnt<R>* const FGl = (FEnt<R>*)((unsigned char*)FSl + r16((p.n_ml + 4) * (int)sizeof(FEnt<R>)));
+  V bprev;
+#pragma unroll
+  for (int b = 0; b < B; ++b) bprev.x[b] = FUSED ? (R)p.st[b].beta_prev : (R)0;
+  const unsigned ltmask = (1u << lane) - 1u;
 
   for (;;) {
     __syncthreads();                                   // previous tile done: smem reusable
@@ -174,7 +262,6 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v, c
     const int kT = p.K - __popc(T);
     if (kT < 0 || kT > p.mw) continue;                  // no rows with this top part
     // ---- per-tile uniform data ----------------------------------------------------------------
-    if (tid == 0) S.base[0] = (long long)tml_base<MODE>(T, p.mw, p.K, S.binom, p.clt);
     if (warp == 1) {                                    // compact the active TT bonds
       int count = 0;
       for (int b0 = 0; b0 < p.n_tt; b0 += 32) {
@@ -184,119 +271,264 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v, c
         if (b < p.n_tt) { mk = p.tt_mask[b]; const uint32_t x = T & mk; act = (x != 0 && x != mk); }
         const unsigned bal = __ballot_sync(0xffffffffu, act);
         if (act) {
-          const int pos = count + __popc(bal & ((1u << lane) - 1u));
-          S.tt_base[pos] = (long long)tml_base<MODE>(T ^ mk, p.mw, p.K, S.binom, p.clt);
-          S.tt_J[pos] = (double)p.tt_J[b];
+          const int pos = count + __popc(bal & ltmask);
+          S.tt_off[pos] = (uint32_t)tml_base<MODE>(T ^ mk, p.mw, p.K, S.binom, p.clt);
+          S.tt_J[pos] = p.tt_J[b];
         }
         count += __popc(bal);
       }
       if (lane == 0) S.misc[1] = count;
     }
-    if (warp == 2 && lane < p.n_ts) {                   // neighbour tiles of the mixed T sites
-      const uint32_t bit = 1u << p.ts_site[lane];
-      const int kTp = (T & bit) ? kT + 1 : kT - 1;
-      const bool ok = (kTp >= 0 && kTp <= p.mw);
-      S.ts_kT[lane] = ok ? kTp : -1;
-      S.ts_base[lane] = ok ? (long long)tml_base<MODE>(T ^ bit, p.mw, p.K, S.binom, p.clt) : 0;
+    if (warp == 2 || warp == 3) {                       // neighbour tile of every TM (warp 2) / TL (warp 3) entry
+      const int n = warp == 2 ? p.n_tm : p.n_tl;
+      const TmlSEnt* src = warp == 2 ? s_tm : s_tl;
+      TmlTx* dst = warp == 2 ? S.txm : S.txl;
+      for (int e = lane; e < n; e += 32) {
+        const TmlSEnt d = src[e];
+        const uint32_t site = p.ts_site[d.b], bit = 1u << site;
+        const int kTp = (T & bit) ? kT + 1 : kT - 1;
+        const bool ok = (kTp >= 0 && kTp <= p.mw);
+        TmlTx x;
+        x.off = ok ? (uint32_t)tml_base<MODE>(T ^ bit, p.mw, p.K, S.binom, p.clt) : 0u;
+        x.cofs = ok ? kTp * nM : 0;
+        x.u = (T >> site) & 1u;
+        x.valid = ok ? 1 : 0;
+        dst[e] = x;
+      }
     }
-    __syncthreads();
-    const long long base = S.base[0];
+    const uint32_t base = (uint32_t)tml_base<MODE>(T, p.mw, p.K, S.binom, p.clt);
     const int tlen = s_tlen[kT];
-    // ---- stage the tile --------------------------------------------------------------------------
+    // ---- stage the tile (16-byte loads on the aligned interior; smem keeps the global misalignment) ----
+    const int mis = (RB >= 16) ? 0 : (int)(base & (uint32_t)(16 / RB - 1));   // rows past a 16-byte boundary
+    const unsigned char* vsb0 = S.vs + (size_t)mis * RB;                        // row 0 of the tile
     {
-      R* vs = (R*)S.vs;
-      const R* src = v + base;
-      for (int x = tid; x < tlen; x += NT) vs[x] = src[x];
+      constexpr int RPV = RB >= 16 ? 1 : 16 / RB;                                // rows per 16 bytes
+      const V* src = v + base;
+      V* vs = (V*)vsb0;
+      if (RPV == 1) {
+        for (int x = tid; x < tlen; x += NT) vs[x] = src[x];
+      } else {
+        const int head = mis ? (RPV - mis) : 0;                                  // rows before the first boundary
+        const int h = head < tlen ? head : tlen;
+        const int nvec = (tlen - h) / RPV;
+        if (tid < h) vs[tid] = src[tid];
+        const uint4* s4 = (const uint4*)(src + h);
+        uint4* d4 = (uint4*)(vs + h);
+#pragma unroll 4
+        for (int x = tid; x < nvec; x += NT) d4[x] = s4[x];
+        const int done = h + nvec * RPV;
+        if (tid < tlen - done) vs[done + tid] = src[done + tid];
+      }
     }
     __syncthreads();
-    // ---- rows: one warp per (column, 32-row chunk) -------------------------------------------------
+    // ---- rows: one warp per column (up to 8 chunks of 32 rows) ---------------------------------------
     const int it0 = p.item_off[kT], it1 = p.item_off[kT + 1];
     const int ntt = S.misc[1];
     const uint16_t* co = s_coloff + kT * nM;
-    double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
+    double s_qy[B], s_yy[B], s_qq[B];
+#pragma unroll
+    for (int b = 0; b < B; ++b) { s_qy[b] = 0.0; s_yy[b] = 0.0; s_qq[b] = 0.0; }
     for (int it = it0 + warp; it < it1; it += NW) {
       const uint32_t item = __ldg(&p.items[it]);
       const uint32_t M = item & 0xffffu;
+      const int chunk0 = (int)((item >> 16) & 0xffu), nch = (int)(item >> 24);
       const int kL = kT - __popc(M);
       const int k0 = s_koff[kL];
       const int len = s_koff[kL + 1] - k0;
-      const int lr = (int)(item >> 16) * 32 + lane;
-      const bool valid = lr < len;
-      const int lrc = valid ? lr : 0;
-      const int Lidx = k0 + lrc;
-      const int cb = co[M];
-      const unsigned char* vsb = vsb0 + (size_t)cb * sizeof(R);            // column base (bytes)
-      const R own = *(const R*)(vsb + (size_t)lrc * sizeof(R));
-      const uint32_t Lw = s_lstate[Lidx];
-      R acc = 0;
-      // LL: swap form, 4 bonds per 8-byte table entry
-      for (int g = 0; g < (p.n_ll4 >> 2); ++g) {
-        const uint2 q = s_ll[g * nL + Lidx];
-        acc += p.ll_J[4 * g + 0] * *(const R*)(vsb + (q.x & 0xffffu));
-        acc += p.ll_J[4 * g + 1] * *(const R*)(vsb + (q.x >> 16));
-        acc += p.ll_J[4 * g + 2] * *(const R*)(vsb + (q.y & 0xffffu));
-        acc += p.ll_J[4 * g + 3] * *(const R*)(vsb + (q.y >> 16));
+      const uint32_t cb = co[M];
+      // ---- build the descriptor lists of this column (lane e <-> list entry e) ---------------------
+      __syncwarp();
+      int nU = ntt, nS = 0, nFG = 0;
+      const int nFS = p.n_ml;
+      R sumJ = 0;                                       // J of the uniform (U, S) entries: folded into the diagonal
+      for (int a = lane; a < ntt; a += 32) {             // TT: same offset in tile T ^ mask
+        const R J = (R)S.tt_J[a];
+        Ul[a].off = S.tt_off[a] + cb; Ul[a].J = J; sumJ += J;
       }
-      // MM: other column of this tile, same lr (warp-uniform test)
-      for (int b = 0; b < p.n_mm; ++b) {
-        const uint32_t mk = p.mm_mask[b];
-        if (__popc(M & mk) == 1) {
-          const R* col = (const R*)(vsb0 + (size_t)co[M ^ mk] * sizeof(R));
-          acc += p.mm_J[b] * (col[lrc] - own);
+      for (int e0 = 0; e0 < p.n_tm; e0 += 32) {          // TM: tile T ^ bit_s, column M ^ bit_i, same lr
+        const int e = e0 + lane;
+        bool act = false;
+        uint32_t off = 0;
+        R J = 0;
+        if (e < p.n_tm) {
+          const TmlTx x = S.txm[e];
+          const uint32_t i = s_tm[e].a;
+          act = x.valid && ((M >> i) & 1u) != x.u;
+          if (act) { off = x.off + s_coloff[x.cofs + (int)(M ^ (1u << i))]; J = (R)s_tm[e].J; }
         }
+        const unsigned bal = __ballot_sync(0xffffffffu, act);
+        if (act) { const int pos = nU + __popc(bal & ltmask); Ul[pos].off = off; Ul[pos].J = J; sumJ += J; }
+        nU += __popc(bal);
       }
-      // ML: column M ^ bit_j, row = L with bit i flipped (per-lane test L_i != M_j)
-      for (int b = 0; b < p.n_ml; ++b) {
-        const int i = p.ml_i[b], j = p.ml_j[b];
-        const uint32_t u = (M >> j) & 1u;
-        const unsigned char* col = vsb0 + (size_t)co[M ^ (1u << j)] * sizeof(R);
-        const uint32_t nb = s_fl[i * nL + Lidx];
-        if (((Lw >> i) & 1u) != u) acc += p.ml_J[b] * (*(const R*)(col + nb) - own);
+      for (int e0 = 0; e0 < p.n_mm; e0 += 32) {          // MM: column M ^ mask of this tile, same lr
+        const int e = e0 + lane;
+        bool act = false;
+        uint32_t off = 0;
+        R J = 0;
+        if (e < p.n_mm) {
+          const TmlSEnt d = s_mm[e];
+          act = __popc(M & d.a) == 1;
+          if (act) { off = (uint32_t)co[M ^ d.a] * RB; J = (R)d.J; }
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, act);
+        if (act) { const int pos = nS + __popc(bal & ltmask); Sl[pos].off = off; Sl[pos].J = J; sumJ += J; }
+        nS += __popc(bal);
       }
-      // TT: same offset in another tile (tile-uniform list of active bonds)
-      const long long off = (long long)cb + lrc;
-      for (int a = 0; a < ntt; ++a) acc += (R)S.tt_J[a] * (__ldg(&v[S.tt_base[a] + off]) - own);
-      // TM / TL: neighbour tile T ^ bit_s
-      for (int s = 0; s < p.n_ts; ++s) {
-        const int kTp = S.ts_kT[s];
-        if (kTp < 0) continue;
-        const uint32_t u = (T >> p.ts_site[s]) & 1u;
-        const uint16_t* cop = s_coloff + kTp * nM;
-        const R* tb = v + S.ts_base[s];
-        for (int e = p.ts_first[s]; e < p.ts_first[s + 1]; ++e) {
-          const int i = p.tx_i[e];
-          if (p.tx_kind[e] == 0) {                       // TM: column M ^ bit_i, same lr
-            if (((M >> i) & 1u) != u) acc += p.tx_J[e] * (__ldg(&tb[(int)cop[M ^ (1u << i)] + lrc]) - own);
-          } else {                                       // TL: column M, row flipped at L_i
-            const uint32_t nb = s_fl[i * nL + Lidx];
-            const unsigned char* colg = (const unsigned char*)(tb + cop[M]);
-            if (((Lw >> i) & 1u) != u) acc += p.tx_J[e] * (__ldg((const R*)(colg + nb)) - own);
+      for (int e = lane; e < nFS; e += 32) {             // ML: column M ^ bit_j, row flipped at L_i
+        const TmlSEnt d = s_ml[e];
+        const uint32_t u = (M >> d.b) & 1u;
+        FSl[e].off = (uint32_t)co[M ^ (1u << d.b)] - ((u ^ 1u) << 15);
+        FSl[e].J = (R)d.J;
+        FSl[e].fl = d.a * (uint32_t)nL * 2u;
+        FSl[e].uw = u << 15;
+      }
+      for (int e0 = 0; e0 < p.n_tl; e0 += 32) {          // TL: tile T ^ bit_s, column M, row flipped at L_i
+        const int e = e0 + lane;
+        bool act = false;
+        TmlTx x;
+        if (e < p.n_tl) { x = S.txl[e]; act = x.valid != 0; }
+        const unsigned bal = __ballot_sync(0xffffffffu, act);
+        if (act) {
+          const int pos = nFG + __popc(bal & ltmask);
+          FGl[pos].off = x.off + s_coloff[x.cofs + (int)M] - ((x.u ^ 1u) << 15);
+          FGl[pos].J = (R)s_tl[e].J;
+          FGl[pos].fl = s_tl[e].a * (uint32_t)nL * 2u;
+          FGl[pos].uw = x.u << 15;
+        }
+        nFG += __popc(bal);
+      }
+      // pad the flip lists to a multiple of 4 with entries that are never active: row w of FLtab is
+      // all zero, so (entry ^ 0) & 0x8000 == 0 for every lane
+      if (lane < 4) {
+        FEnt<R> z; z.off = cb; z.J = 0; z.fl = (uint32_t)p.w * (uint32_t)nL * 2u; z.uw = 0;
+        { const uint32_t q = (nFS + lane); if (q < (uint32_t)((nFS + 3) & ~3)) FSl[q] = z; }
+        z.off = base + cb;
+        { const uint32_t q = (nFG + lane); if (q < (uint32_t)((nFG + 3) & ~3)) FGl[q] = z; }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) sumJ += __shfl_xor_sync(0xffffffffu, sumJ, o);
+      const R dcoef = p.diag_coef - sumJ;
+      __syncwarp();
+      const int nFS4 = (nFS + 3) & ~3, nFG4 = (nFG + 3) & ~3;
+      // ---- rows ------------------------------------------------------------------------------------
+      const unsigned char* vsb = vsb0 + (size_t)cb * RB;                  // column base (bytes)
+      for (int c = 0; c < nch; ++c) {
+        const int lr = (chunk0 + c) * 32 + lane;
+        const bool valid = lr < len;
+        const int lrc = valid ? lr : 0;
+        const int Lidx = k0 + lrc;
+        const unsigned char* pl = vsb0 + (size_t)lrc * RB;               // lane pointer: row lrc of column 0
+        const unsigned char* flp = s_fl + Lidx * 2;
+        const V own = *(const V*)(vsb + (size_t)lrc * RB);
+        V acc;
+#pragma unroll
+        for (int b = 0; b < B; ++b) acc.x[b] = dcoef * own.x[b];
+        // U: same lr in another tile (TT) / another tile and column (TM): coalesced global reads (issued first)
+        {
+          const V* vl = v + lrc;
+          int e = 0;
+          for (; e + 4 <= nU; e += 4) {
+            const UEnt<R> d0 = Ul[e], d1 = Ul[e + 1], d2 = Ul[e + 2], d3 = Ul[e + 3];
+            const V a0 = vec_ldg((const V*)addr_u32(vl, d0.off, RB));
+            const V a1 = vec_ldg((const V*)addr_u32(vl, d1.off, RB));
+            const V a2 = vec_ldg((const V*)addr_u32(vl, d2.off, RB));
+            const V a3 = vec_ldg((const V*)addr_u32(vl, d3.off, RB));
+#pragma unroll
+            for (int b = 0; b < B; ++b) acc.x[b] += d0.J * a0.x[b] + d1.J * a1.x[b] + d2.J * a2.x[b] + d3.J * a3.x[b];
+          }
+          for (; e < nU; ++e) {
+            const UEnt<R> d = Ul[e];
+            const V a = vec_ldg((const V*)addr_u32(vl, d.off, RB));
+#pragma unroll
+            for (int b = 0; b < B; ++b) acc.x[b] += d.J * a.x[b];
           }
         }
-      }
-      // epilogue: diagonal, Lanczos recurrence, reductions
-      R out = p.diag_coef * own + acc;
-      if (valid) {
-        const long long g = base + off;
-        if (FUSED) {
-          out -= bprev * __ldcs(&qprev[g]);
-          s_qy += (double)own * (double)out;
-          s_yy += (double)out * (double)out;
-          s_qq += (double)own * (double)own;
+        // FG: another tile, row flipped at L_i (per-lane test L_i != T_s); inactive lanes re-read nothing
+        for (int e = 0; e < nFG4; e += 4) {
+          uint32_t o0, o1, o2, o3, f0, f1, f2, f3, u0, u1, u2, u3;
+          R j0, j1, j2, j3;
+          load_fent(FGl + e, o0, j0, f0, u0); load_fent(FGl + e + 1, o1, j1, f1, u1);
+          load_fent(FGl + e + 2, o2, j2, f2, u2); load_fent(FGl + e + 3, o3, j3, f3, u3);
+          const uint32_t x0 = *(const uint16_t*)(flp + f0), x1 = *(const uint16_t*)(flp + f1);
+          const uint32_t x2 = *(const uint16_t*)(flp + f2), x3 = *(const uint16_t*)(flp + f3);
+          V a0 = own, a1 = own, a2 = own, a3 = own;
+          if ((x0 ^ u0) & 0x8000u) a0 = vec_ldg((const V*)addr_u32(v, o0 + x0, RB));
+          if ((x1 ^ u1) & 0x8000u) a1 = vec_ldg((const V*)addr_u32(v, o1 + x1, RB));
+          if ((x2 ^ u2) & 0x8000u) a2 = vec_ldg((const V*)addr_u32(v, o2 + x2, RB));
+          if ((x3 ^ u3) & 0x8000u) a3 = vec_ldg((const V*)addr_u32(v, o3 + x3, RB));
+#pragma unroll
+          for (int b = 0; b < B; ++b)
+            acc.x[b] += j0 * (a0.x[b] - own.x[b]) + j1 * (a1.x[b] - own.x[b]) + j2 * (a2.x[b] - own.x[b]) + j3 * (a3.x[b] - own.x[b]);
         }
-        __stcs(&y[g], out);
+        // LL: swap form, 4 bonds per 8-byte table entry
+        for (int g = 0; g < (p.n_ll4 >> 2); ++g) {
+          const uint2 q = s_ll[g * nL + Lidx];
+          const V a0 = *(const V*)(vsb + (q.x & 0xffffu) * RB);
+          const V a1 = *(const V*)(vsb + (q.x >> 16) * RB);
+          const V a2 = *(const V*)(vsb + (q.y & 0xffffu) * RB);
+          const V a3 = *(const V*)(vsb + (q.y >> 16) * RB);
+          const R j0 = p.ll_J[4 * g + 0], j1 = p.ll_J[4 * g + 1], j2 = p.ll_J[4 * g + 2], j3 = p.ll_J[4 * g + 3];
+#pragma unroll
+          for (int b = 0; b < B; ++b) acc.x[b] += j0 * a0.x[b] + j1 * a1.x[b] + j2 * a2.x[b] + j3 * a3.x[b];
+        }
+        // S: other column of this tile, same lr
+#pragma unroll 4
+        for (int e = 0; e < nS; ++e) {
+          const UEnt<R> d = Sl[e];
+          const V a = *(const V*)(pl + d.off);
+#pragma unroll
+          for (int b = 0; b < B; ++b) acc.x[b] += d.J * a.x[b];
+        }
+        // FS: other column of this tile, row = L with bit i flipped (per-lane test L_i != M_j)
+        for (int e = 0; e < nFS4; e += 4) {
+          uint32_t o0, o1, o2, o3, f0, f1, f2, f3, u0, u1, u2, u3;
+          R j0, j1, j2, j3;
+          load_fent(FSl + e, o0, j0, f0, u0); load_fent(FSl + e + 1, o1, j1, f1, u1);
+          load_fent(FSl + e + 2, o2, j2, f2, u2); load_fent(FSl + e + 3, o3, j3, f3, u3);
+          const uint32_t x0 = *(const uint16_t*)(flp + f0), x1 = *(const uint16_t*)(flp + f1);
+          const uint32_t x2 = *(const uint16_t*)(flp + f2), x3 = *(const uint16_t*)(flp + f3);
+          V a0 = own, a1 = own, a2 = own, a3 = own;
+          if ((x0 ^ u0) & 0x8000u) a0 = *(const V*)(vsb0 + (size_t)(o0 + x0) * RB);
+          if ((x1 ^ u1) & 0x8000u) a1 = *(const V*)(vsb0 + (size_t)(o1 + x1) * RB);
+          if ((x2 ^ u2) & 0x8000u) a2 = *(const V*)(vsb0 + (size_t)(o2 + x2) * RB);
+          if ((x3 ^ u3) & 0x8000u) a3 = *(const V*)(vsb0 + (size_t)(o3 + x3) * RB);
+#pragma unroll
+          for (int b = 0; b < B; ++b)
+            acc.x[b] += j0 * (a0.x[b] - own.x[b]) + j1 * (a1.x[b] - own.x[b]) + j2 * (a2.x[b] - own.x[b]) + j3 * (a3.x[b] - own.x[b]);
+        }
+        // epilogue: Lanczos recurrence, reductions
+        if (valid) {
+          const size_t g = (size_t)base + cb + lrc;
+          if (FUSED) {
+            const V qp = vec_ldcs(qprev + g);
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+              acc.x[b] -= bprev.x[b] * qp.x[b];
+              s_qy[b] += (double)own.x[b] * (double)acc.x[b];
+              s_yy[b] += (double)acc.x[b] * (double)acc.x[b];
+              s_qq[b] += (double)own.x[b] * (double)own.x[b];
+            }
+          }
+          vec_stcs(y + g, acc);
+        }
       }
     }
     if (FUSED) {                                        // deterministic per-tile partial sums
-      block_sum3(s_qy, s_yy, s_qq, S.red);
-      if (tid == 0) {
-        p.partials[T] = s_qy;
-        p.partials[(size_t)p.nT + T] = s_yy;
-        p.partials[2 * (size_t)p.nT + T] = s_qq;
+#pragma unroll
+      for (int b = 0; b < B; ++b) {
+        const double a = warp_sum(s_qy[b]), bb = warp_sum(s_yy[b]), c = warp_sum(s_qq[b]);
+        if (lane == 0) { S.red[warp * 3 * B + 3 * b] = a; S.red[warp * 3 * B + 3 * b + 1] = bb; S.red[warp * 3 * B + 3 * b + 2] = c; }
+      }
+      __syncthreads();
+      if (tid < 3 * B) {
+        double s = 0.0;
+        for (int wv = 0; wv < NW; ++wv) s += S.red[wv * 3 * B + tid];
+        p.partials[(size_t)tid * p.nT + T] = s;
       }
     }
   }
-  // ---- grid-wide finish: the last CTA resets the counters and (fused) advances the chain ---------
+  // ---- grid-wide finish: the last CTA resets the counters and (fused) advances the chains --------
+  __syncthreads();
   if (tid == 0) {
     __threadfence();
     s_last = (atomicAdd(&p.counter[1], 1u) == gridDim.x - 1);
@@ -306,28 +538,40 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v, c
   __threadfence();
   if (tid == 0) { p.counter[0] = 0; p.counter[1] = 0; }
   if (!FUSED) return;
-  double a = 0.0, b = 0.0, c = 0.0;
-  for (uint32_t k = tid; k < p.nT; k += NT) {            // fixed assignment and order
-    a += p.partials[k]; b += p.partials[(size_t)p.nT + k]; c += p.partials[2 * (size_t)p.nT + k];
+  for (int q = 0; q < 3 * B; ++q) {                       // fixed assignment and order
+    double a = 0.0;
+    for (uint32_t k = tid; k < p.nT; k += NT) a += p.partials[(size_t)q * p.nT + k];
+    a = warp_sum(a);
+    __syncthreads();
+    if (lane == 0) S.red[warp] = a;
+    __syncthreads();
+    if (tid == 0) {
+      double s = 0.0;
+      for (int wv = 0; wv < NW; ++wv) s += S.red[wv];
+      S.red[64 + q] = s;
+    }
   }
-  block_sum3(a, b, c, S.red);
-  if (tid == 0) {
-    ChainState* st = p.st;
-    const int j = st->step;
-    const double alpha = c > 0.0 ? a / c : 0.0;
-    double b2 = c > 0.0 ? b - a * a / c : 0.0;
-    if (!(b2 > 0.0)) b2 = 0.0;
-    const double beta = sqrt(b2);
-    st->alpha[j] = alpha;
-    st->beta[j] = beta;
-    double sc = st->scale;
-    sc = fmax(sc, fmax(fabs(alpha), beta));
-    st->scale = sc;
-    st->step = j + 1;
-    st->a = alpha;
-    st->inv_b = beta > 0.0 ? 1.0 / beta : 0.0;
-    st->beta_prev = beta;
-    if (j + 1 >= st->limit || beta <= st->tol * sc) st->done = 1;
+  __syncthreads();
+  if (tid < B) {
+    ChainState* st = p.st + tid;
+    if (!st->done) {
+      const double a = S.red[64 + 3 * tid], b = S.red[64 + 3 * tid + 1], c = S.red[64 + 3 * tid + 2];
+      const int j = st->step;
+      const double alpha = c > 0.0 ? a / c : 0.0;
+      double b2 = c > 0.0 ? b - a * a / c : 0.0;
+      if (!(b2 > 0.0)) b2 = 0.0;
+      const double beta = sqrt(b2);
+      st->alpha[j] = alpha;
+      st->beta[j] = beta;
+      double sc = st->scale;
+      sc = fmax(sc, fmax(fabs(alpha), beta));
+      st->scale = sc;
+      st->step = j + 1;
+      st->a = alpha;
+      st->inv_b = beta > 0.0 ? 1.0 / beta : 0.0;
+      st->beta_prev = beta;
+      if (j + 1 >= st->limit || beta <= st->tol * sc) { st->done = 1; st->inv_b = 0.0; }
+    }
   }
 }
 
@@ -337,14 +581,17 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v, c
 template <typename R, int MODE>
 __global__ void __launch_bounds__(256)
 neighbors_tml_kernel(const __grid_constant__ TmlParams<R> p, const BondDev* __restrict__ bonds, int nb,
-                     const int* __restrict__ bclass, const int* __restrict__ bentry, const int* __restrict__ bts,
+                     const int* __restrict__ bclass, const int* __restrict__ bentry,
                      int64_t row0, int64_t nrows, int64_t* __restrict__ out) {
   const int K1 = p.K + 1;
   const int* koff = (const int*)(p.blob + p.off_koff);
-  const uint16_t* lstate = (const uint16_t*)(p.blob + p.off_lstate);
   const uint16_t* coloff = (const uint16_t*)(p.blob + p.off_coloff);
   const uint2* ll = (const uint2*)(p.blob + p.off_ll);
   const uint16_t* fl = (const uint16_t*)(p.blob + p.off_fl);
+  const TmlSEnt* mm = (const TmlSEnt*)(p.blob + p.off_mm);
+  const TmlSEnt* ml = (const TmlSEnt*)(p.blob + p.off_ml);
+  const TmlSEnt* tm = (const TmlSEnt*)(p.blob + p.off_tm);
+  const TmlSEnt* tl = (const TmlSEnt*)(p.blob + p.off_tl);
   const int nL = 1 << p.w, nM = 1 << p.m;
   for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < nrows; r += (int64_t)gridDim.x * blockDim.x) {
     const uint64_t tr = (uint64_t)(row0 + r);
@@ -359,8 +606,9 @@ neighbors_tml_kernel(const __grid_constant__ TmlParams<R> p, const BondDev* __re
     const uint64_t base = tml_base<MODE>(T, p.mw, p.K, p.binom, p.clt);
     const int cb = coloff[kT * nM + M];
     const int lr = (int)(tr - base) - cb;
-    const bool ok = lr >= 0 && lr < koff[kL + 1] - koff[kL] && lstate[koff[kL] + lr] == L;
+    bool ok = lr >= 0 && lr < koff[kL + 1] - koff[kL];
     const int Lidx = ok ? koff[kL] + lr : 0;
+    for (int i = 0; ok && i < p.w; ++i) ok = ((fl[i * nL + Lidx] >> 15) == ((L >> i) & 1u));   // FLtab knows L
     for (int b = 0; b < nb; ++b) {
       const uint64_t mk = bonds[b].mask, x = n & mk;
       int64_t idx = -1;
@@ -370,30 +618,27 @@ neighbors_tml_kernel(const __grid_constant__ TmlParams<R> p, const BondDev* __re
           case 0: {                                      // LL
             const uint2 q = ll[(e >> 2) * nL + Lidx];
             const uint32_t h = (e & 2) ? q.y : q.x;
-            const uint32_t nbB = (e & 1) ? (h >> 16) : (h & 0xffffu);
-            idx = (int64_t)base + cb + (int)(nbB / sizeof(R));
+            idx = (int64_t)base + cb + (int)((e & 1) ? (h >> 16) : (h & 0xffffu));
             break;
           }
-          case 1: idx = (int64_t)base + coloff[kT * nM + (M ^ p.mm_mask[e])] + lr; break;          // MM
-          case 2: idx = (int64_t)base + coloff[kT * nM + (M ^ (1u << p.ml_j[e]))] +               // ML
-                        (int)(fl[p.ml_i[e] * nL + Lidx] / sizeof(R)); break;
+          case 1: idx = (int64_t)base + coloff[kT * nM + (M ^ mm[e].a)] + lr; break;                 // MM
+          case 2: idx = (int64_t)base + coloff[kT * nM + (M ^ (1u << ml[e].b))] +                    // ML
+                        (int)(fl[ml[e].a * nL + Lidx] & 0x7fffu); break;
           case 3: idx = (int64_t)tml_base<MODE>(T ^ p.tt_mask[e], p.mw, p.K, p.binom, p.clt) + cb + lr; break;  // TT
           default: {                                     // TM / TL
-            const int s = bts[b];
-            const uint32_t bit = 1u << p.ts_site[s];
+            const TmlSEnt d = bclass[b] == 4 ? tm[e] : tl[e];
+            const uint32_t bit = 1u << p.ts_site[d.b];
             const int kTp = (T & bit) ? kT + 1 : kT - 1;
             const uint64_t tb = tml_base<MODE>(T ^ bit, p.mw, p.K, p.binom, p.clt);
-            const int i = p.tx_i[e];
-            if (p.tx_kind[e] == 0) idx = (int64_t)tb + coloff[kTp * nM + (M ^ (1u << i))] + lr;
-            else idx = (int64_t)tb + coloff[kTp * nM + M] + (int)(fl[i * nL + Lidx] / sizeof(R));
+            if (bclass[b] == 4) idx = (int64_t)tb + coloff[kTp * nM + (M ^ (1u << d.a))] + lr;
+            else idx = (int64_t)tb + coloff[kTp * nM + M] + (int)(fl[d.a * nL + Lidx] & 0x7fffu);
           }
         }
         if (!ok) idx = -2;
       } else if (bclass[b] == 0 && ok) {                 // parallel LL bond: the table must say "self"
         const uint2 q = ll[(e >> 2) * nL + Lidx];
         const uint32_t h = (e & 2) ? q.y : q.x;
-        const uint32_t nbB = (e & 1) ? (h >> 16) : (h & 0xffffu);
-        if ((int)(nbB / sizeof(R)) != lr) idx = -3;
+        if ((int)((e & 1) ? (h >> 16) : (h & 0xffffu)) != lr) idx = -3;
       }
       out[r * nb + b] = idx;
     }
@@ -409,46 +654,74 @@ uint64_t binom_t(int n, int k) {
 }
 
 template <typename R>
-void fill_params(const ftlm_ctx* c, const TmlPlan* t, TmlParams<R>& p) {
+void fill_params(const ftlm_ctx* c, const TmlPlan* t, TmlParams<R>& p, int batch) {
   memset(&p, 0, sizeof(p));
   p.N = c->N; p.K = c->N_up; p.w = t->w; p.m = t->m; p.t = t->t; p.mw = t->w + t->m; p.mode = c->mode;
   p.nT = t->nT; p.n_ll4 = t->n_ll4; p.n_mm = t->n_mm; p.n_ml = t->n_ml; p.n_tt = t->n_tt; p.n_ts = t->n_ts;
-  p.max_tile = t->max_tile; p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.blob = t->d_blob;
-  p.blob_bytes = t->blob_bytes; p.off_koff = t->off_koff; p.off_lstate = t->off_lstate; p.off_coloff = t->off_coloff;
-  p.off_ll = t->off_ll; p.off_fl = t->off_fl; p.off_tlen = t->off_tlen; p.items = t->d_items; p.item_off = t->d_item_off;
+  p.n_tm = t->n_tm; p.n_tl = t->n_tl;
+  p.max_tile = t->max_tile;
+  p.scratch_bytes = tml_scratch_bytes((int)sizeof(R), t->n_tt, t->n_tm, t->n_mm, t->n_ml, t->n_tl);
+  p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.blob = t->d_blob;
+  p.blob_bytes = t->blob_bytes; p.off_koff = t->off_koff; p.off_tlen = t->off_tlen; p.off_coloff = t->off_coloff;
+  p.off_ll = t->off_ll; p.off_fl = t->off_fl; p.off_mm = t->off_mm; p.off_ml = t->off_ml; p.off_tm = t->off_tm;
+  p.off_tl = t->off_tl; p.items = t->d_items; p.item_off = t->d_item_off;
   p.partials = t->d_partials; p.counter = t->d_counter; p.st = c->d_state; p.diag_coef = (R)t->diag_coef;
   for (int k = 0; k < t->n_ll4; ++k) p.ll_J[k] = (R)t->ll_J[(size_t)k];
-  for (int k = 0; k < t->n_mm; ++k) { p.mm_mask[k] = t->mm_mask[(size_t)k]; p.mm_J[k] = (R)t->mm_J[(size_t)k]; }
-  for (int k = 0; k < t->n_ml; ++k) { p.ml_i[k] = t->ml_i[(size_t)k]; p.ml_j[k] = t->ml_j[(size_t)k]; p.ml_J[k] = (R)t->ml_J[(size_t)k]; }
-  for (int k = 0; k < t->n_tt; ++k) { p.tt_mask[k] = t->tt_mask[(size_t)k]; p.tt_J[k] = (R)t->tt_J[(size_t)k]; }
+  for (int k = 0; k < t->n_tt; ++k) { p.tt_mask[k] = t->tt_mask[(size_t)k]; p.tt_J[k] = t->tt_J[(size_t)k]; }
   for (int k = 0; k < t->n_ts; ++k) p.ts_site[k] = t->ts_site[(size_t)k];
-  for (int k = 0; k <= t->n_ts; ++k) p.ts_first[k] = t->ts_first[(size_t)k];
-  for (int k = 0; k < t->n_tx; ++k) { p.tx_kind[k] = t->tx_kind[(size_t)k]; p.tx_i[k] = t->tx_i[(size_t)k]; p.tx_J[k] = (R)t->tx_J[(size_t)k]; }
+  (void)batch;
 }
 
-size_t tml_smem_bytes(const ftlm_ctx* c, int blob_bytes, int max_tile) {
+struct TmlLaunchCfg { int threads, ctas; size_t smem; };
+
+// threads / CTAs per SM / dynamic shared memory for a batch of B vectors; smem == 0 if it does not fit
+TmlLaunchCfg tml_config(const ftlm_ctx* c, const TmlPlan* t, int batch) {
+  const int esz = (int)ftlm_elem_size(c);
+  const int sb = tml_scratch_bytes(esz, t->n_tt, t->n_tm, t->n_mm, t->n_ml, t->n_tl);
+  const size_t cap = 227 * 1024 - 1024;
   TmlSmem S;
-  return tml_layout(S, nullptr, c->N, c->N_up, blob_bytes, max_tile, (int)ftlm_elem_size(c));
+  TmlLaunchCfg best{0, 0, 0};
+  const size_t s512 = tml_layout(S, nullptr, c->N, c->N_up, t->blob_bytes, t->max_tile, esz * batch, batch, 16, sb);
+  if (batch < 4) {
+    if (2 * (s512 + 1024) <= 228 * 1024) return TmlLaunchCfg{512, 2, s512};
+    const size_t s1024 = tml_layout(S, nullptr, c->N, c->N_up, t->blob_bytes, t->max_tile, esz * batch, batch, 32, sb);
+    if (s1024 <= cap) return TmlLaunchCfg{1024, 1, s1024};
+  }
+  if (s512 <= cap) return TmlLaunchCfg{512, (2 * (s512 + 1024) <= 228 * 1024) ? 2 : 1, s512};
+  return best;
 }
 
-template <typename R, int MODE>
+template <typename R, int B, int MODE>
 int launch_tml(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
   TmlPlan* t = c->tml;
+  const TmlLaunchCfg cfg = tml_config(c, t, B);
+  if (cfg.smem == 0) { ftlm_set_error("TML: batch %d does not fit shared memory with this split", B); return FTLM_EUNSUPPORTED; }
+  if (fused && B > t->partials_batch) { ftlm_set_error("TML: internal: partials sized for batch %d", t->partials_batch); return FTLM_EINVAL; }
   TmlParams<R> p;
-  fill_params<R>(c, t, p);
-  int grid = c->sm_count * t->ctas_per_sm;
+  fill_params<R>(c, t, p, B);
+  int grid = c->sm_count * cfg.ctas;
   if ((uint32_t)grid > t->nT) grid = (int)t->nT;
   if (fused) {
-    auto k = hv_tml_kernel<R, MODE, true>;
-    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem_bytes));
-    k<<<grid, t->threads, t->smem_bytes, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
+    auto k = hv_tml_kernel<R, B, MODE, true>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
+    k<<<grid, cfg.threads, cfg.smem, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
   } else {
-    auto k = hv_tml_kernel<R, MODE, false>;
-    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem_bytes));
-    k<<<grid, t->threads, t->smem_bytes, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
+    auto k = hv_tml_kernel<R, B, MODE, false>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
+    k<<<grid, cfg.threads, cfg.smem, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
   }
   CK(cudaGetLastError());
   return FTLM_OK;
+}
+
+template <typename R, int MODE>
+int launch_tml_b(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, int batch, cudaStream_t s) {
+  switch (batch) {
+    case 1: return launch_tml<R, 1, MODE>(c, v, qp, y, fused, s);
+    case 2: return launch_tml<R, 2, MODE>(c, v, qp, y, fused, s);
+    case 4: return launch_tml<R, 4, MODE>(c, v, qp, y, fused, s);
+    default: ftlm_set_error("TML: batch must be 1, 2 or 4 (got %d)", batch); return FTLM_EINVAL;
+  }
 }
 
 }  // namespace
@@ -457,16 +730,16 @@ void ftlm_tml_plan_destroy(ftlm_ctx* c) {
   TmlPlan* t = c->tml;
   if (!t) return;
   cudaFree(t->d_blob); cudaFree(t->d_items); cudaFree(t->d_item_off); cudaFree(t->d_partials);
-  cudaFree(t->d_counter); cudaFree(t->d_bond_class); cudaFree(t->d_bond_entry); cudaFree(t->d_bond_ts);
+  cudaFree(t->d_counter); cudaFree(t->d_bond_class); cudaFree(t->d_bond_entry);
   delete t;
   c->tml = nullptr;
 }
 
 // Build the plan.  FTLM_OK with c->tml == nullptr when no split is possible for this sector (the
-// dispatcher then uses the TILE / ROW kernels).  c->low_bits / c->mid_bits (0 = auto) choose w, m.
+// dispatcher then uses the TILE / ROW kernels).  c->tml_low_bits / c->tml_mid_bits (0 = auto) choose w, m.
 int ftlm_tml_plan_create(ftlm_ctx* c) {
   c->tml = nullptr;
-  const int N = c->N, K = c->N_up, esz = (int)ftlm_elem_size(c);
+  const int N = c->N, esz = (int)ftlm_elem_size(c);
   const bool forced = c->tml_low_bits != 0 || c->tml_mid_bits != 0;
   int w = c->tml_low_bits, m = c->tml_mid_bits;
   if (!forced) {
@@ -484,44 +757,35 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
   };
   if (w < 5 || w > 12 || m < 1 || m > 9 || w + m > 18 || t < 1 || t > 31) return unusable("need 5<=w<=12, 1<=m<=9, w+m<=18, 1<=t<=31");
   if (c->dim < 64) return unusable("sector too small");
+  if ((uint64_t)c->dim >= (1ull << 32)) return unusable("dim >= 2^32 (row offsets are 32-bit)");
   const int mw = w + m;
   TmlPlan* P = new TmlPlan();
   P->w = w; P->m = m; P->t = t; P->nT = 1u << t;
-  std::vector<int> bclass((size_t)c->nb, 0), bentry((size_t)c->nb, 0), bts((size_t)c->nb, 0);
+  std::vector<int> bclass((size_t)c->nb, 0), bentry((size_t)c->nb, 0);
   struct LLb { uint32_t mask; double Jh; };
   std::vector<LLb> ll;
-  std::vector<std::vector<std::pair<int, int>>> per_site((size_t)t);   // (bond, kind) per T site
+  std::vector<int> ts_index((size_t)t, -1);
+  auto ts_of = [&](int site) {
+    const int s = site - mw;
+    if (ts_index[(size_t)s] < 0) { ts_index[(size_t)s] = (int)P->ts_site.size(); P->ts_site.push_back((uint8_t)s); }
+    return (uint32_t)ts_index[(size_t)s];
+  };
   double sumJ_ll = 0.0;
   for (int b = 0; b < c->nb; ++b) {
     const BondDev& d = c->bonds[(size_t)b];
     const int i = d.i, j = d.j;                                          // i < j
     if (j < w) { bclass[(size_t)b] = 0; bentry[(size_t)b] = (int)ll.size(); ll.push_back({(uint32_t)d.mask, d.Jh}); sumJ_ll += d.Jh; }
-    else if (i >= w && j < mw) { bclass[(size_t)b] = 1; bentry[(size_t)b] = (int)P->mm_mask.size(); P->mm_mask.push_back((uint32_t)(d.mask >> w)); P->mm_J.push_back(d.Jh); }
-    else if (i < w && j < mw) { bclass[(size_t)b] = 2; bentry[(size_t)b] = (int)P->ml_i.size(); P->ml_i.push_back((uint8_t)i); P->ml_j.push_back((uint8_t)(j - w)); P->ml_J.push_back(d.Jh); }
+    else if (i >= w && j < mw) { bclass[(size_t)b] = 1; bentry[(size_t)b] = (int)P->mm.size(); P->mm.push_back({(uint32_t)(d.mask >> w), 0u, d.Jh}); }
+    else if (i < w && j < mw) { bclass[(size_t)b] = 2; bentry[(size_t)b] = (int)P->ml.size(); P->ml.push_back({(uint32_t)i, (uint32_t)(j - w), d.Jh}); }
     else if (i >= mw) { bclass[(size_t)b] = 3; bentry[(size_t)b] = (int)P->tt_mask.size(); P->tt_mask.push_back((uint32_t)(d.mask >> mw)); P->tt_J.push_back(d.Jh); }
-    else { bclass[(size_t)b] = i >= w ? 4 : 5; per_site[(size_t)(j - mw)].push_back({b, i >= w ? 0 : 1}); }
-  }
-  P->ts_first.push_back(0);
-  for (int s = 0; s < t; ++s) {
-    if (per_site[(size_t)s].empty()) continue;
-    for (int kind = 0; kind < 2; ++kind)
-      for (auto& e : per_site[(size_t)s]) {
-        if (e.second != kind) continue;
-        const BondDev& d = c->bonds[(size_t)e.first];
-        bentry[(size_t)e.first] = (int)P->tx_kind.size();
-        bts[(size_t)e.first] = (int)P->ts_site.size();
-        P->tx_kind.push_back((uint8_t)kind);
-        P->tx_i.push_back((uint8_t)(kind == 0 ? d.i - w : d.i));
-        P->tx_J.push_back(d.Jh);
-      }
-    P->ts_site.push_back((uint8_t)s);
-    P->ts_first.push_back((uint8_t)P->tx_kind.size());
+    else if (i >= w) { bclass[(size_t)b] = 4; bentry[(size_t)b] = (int)P->tm.size(); P->tm.push_back({(uint32_t)(i - w), ts_of(j), d.Jh}); }
+    else { bclass[(size_t)b] = 5; bentry[(size_t)b] = (int)P->tl.size(); P->tl.push_back({(uint32_t)i, ts_of(j), d.Jh}); }
   }
   P->n_ll = (int)ll.size(); P->n_ll4 = (P->n_ll + 3) & ~3;
-  P->n_mm = (int)P->mm_mask.size(); P->n_ml = (int)P->ml_i.size(); P->n_tt = (int)P->tt_mask.size();
-  P->n_ts = (int)P->ts_site.size(); P->n_tx = (int)P->tx_kind.size();
-  if (P->n_ll4 > TML_MAX_LL || P->n_mm > TML_MAX_MM || P->n_ml > TML_MAX_ML || P->n_tt > TML_MAX_TT ||
-      P->n_ts > TML_MAX_TS || P->n_tx > TML_MAX_TX) { delete P; return unusable("too many bonds in one class"); }
+  P->n_mm = (int)P->mm.size(); P->n_ml = (int)P->ml.size(); P->n_tt = (int)P->tt_mask.size();
+  P->n_ts = (int)P->ts_site.size(); P->n_tm = (int)P->tm.size(); P->n_tl = (int)P->tl.size();
+  if (P->n_ll4 > TML_MAX_LL || P->n_mm > TML_MAX_LIST || P->n_ml > TML_MAX_LIST || P->n_tt > TML_MAX_TT ||
+      P->n_ts > TML_MAX_TS || P->n_tm > TML_MAX_LIST || P->n_tl > TML_MAX_LIST) { delete P; return unusable("too many bonds in one class"); }
   for (int k = 0; k < P->n_ll4; ++k) P->ll_J.push_back(k < P->n_ll ? ll[(size_t)k].Jh : 0.0);
   P->diag_coef = c->diag0 - sumJ_ll;
   // ---- tables (blob) ---------------------------------------------------------------------------
@@ -538,7 +802,7 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
     lstate[(size_t)(koff[(size_t)cnt] + (int)r)] = (uint16_t)L;
   }
   P->max_tile = (int)binom_t(mw, mw / 2);
-  if (P->max_tile > 65535 || (size_t)binom_t(w, w / 2) * (size_t)esz > 65535) { delete P; return unusable("tile too large for 16-bit offsets"); }
+  if (P->max_tile > 65535 || binom_t(w, w / 2) > 32767) { delete P; return unusable("tile too large for 16-bit offsets"); }
   std::vector<int> tlen((size_t)mw + 1);
   std::vector<uint16_t> coloff((size_t)(mw + 1) * nM, 0);
   std::vector<uint32_t> items;
@@ -551,12 +815,19 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
       const int kL = kT - __builtin_popcount((unsigned)M);
       if (kL < 0 || kL > w) continue;
       const int len = (int)binom_t(w, kL);
-      for (int ch = 0; ch * 32 < len; ++ch) items.push_back((uint32_t)M | ((uint32_t)ch << 16));
+      const int nchunks = (len + 31) / 32;
+      for (int ch = 0; ch < nchunks; ch += TML_MAX_CHUNKS) {
+        const int nc = std::min(TML_MAX_CHUNKS, nchunks - ch);
+        items.push_back((uint32_t)M | ((uint32_t)ch << 16) | ((uint32_t)nc << 24));
+      }
       off += len;
     }
+    // longest columns first: the strided assignment item -> warp then balances the warps
+    std::stable_sort(items.begin() + item_off[(size_t)kT], items.end(),
+                     [](uint32_t a, uint32_t b) { return (a >> 24) > (b >> 24); });
     item_off[(size_t)kT + 1] = (int)items.size();
   }
-  std::vector<uint16_t> lltab((size_t)(P->n_ll4 / 4) * nL * 4, 0), fltab((size_t)w * nL, 0);
+  std::vector<uint16_t> lltab((size_t)(P->n_ll4 / 4) * nL * 4, 0), fltab((size_t)(w + 1) * nL, 0);   // row w stays zero (padding entries)
   for (int k = 0; k <= w; ++k)
     for (int r = 0; r < koff[(size_t)k + 1] - koff[(size_t)k]; ++r) {
       const int Lidx = koff[(size_t)k] + r;
@@ -567,9 +838,10 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
           const uint32_t mk = ll[(size_t)b].mask, x = L & mk;
           if (x != 0 && x != mk) nb = lr[(size_t)(L ^ mk)];
         }
-        lltab[((size_t)(b >> 2) * nL + Lidx) * 4 + (b & 3)] = (uint16_t)(nb * (uint32_t)esz);
+        lltab[((size_t)(b >> 2) * nL + Lidx) * 4 + (b & 3)] = (uint16_t)nb;
       }
-      for (int i = 0; i < w; ++i) fltab[(size_t)i * nL + Lidx] = (uint16_t)((uint32_t)lr[(size_t)(L ^ (1u << i))] * (uint32_t)esz);
+      for (int i = 0; i < w; ++i)
+        fltab[(size_t)i * nL + Lidx] = (uint16_t)((uint32_t)lr[(size_t)(L ^ (1u << i))] | (((L >> i) & 1u) << 15));
     }
   std::vector<unsigned char> blob;
   auto put = [&](const void* src, size_t bytes) {
@@ -580,29 +852,30 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
   };
   P->off_koff = put(koff.data(), koff.size() * 4);
   P->off_tlen = put(tlen.data(), tlen.size() * 4);
-  P->off_lstate = put(lstate.data(), lstate.size() * 2);
   P->off_coloff = put(coloff.data(), coloff.size() * 2);
   P->off_ll = put(lltab.data(), lltab.size() * 2);
   P->off_fl = put(fltab.data(), fltab.size() * 2);
+  P->off_mm = put(P->mm.data(), P->mm.size() * sizeof(TmlSEnt));
+  P->off_ml = put(P->ml.data(), P->ml.size() * sizeof(TmlSEnt));
+  P->off_tm = put(P->tm.data(), P->tm.size() * sizeof(TmlSEnt));
+  P->off_tl = put(P->tl.data(), P->tl.size() * sizeof(TmlSEnt));
   P->blob_bytes = (int)blob.size();
-  P->smem_bytes = tml_smem_bytes(c, P->blob_bytes, P->max_tile);
-  const size_t cap = 227 * 1024 - 1024;
-  if (P->smem_bytes > cap) { delete P; return unusable("tables + tile exceed shared memory"); }
-  if (P->smem_bytes + 1024 <= (228 * 1024) / 2) { P->ctas_per_sm = 2; P->threads = 512; }
-  else { P->ctas_per_sm = 1; P->threads = 1024; }
-  // ---- upload ----------------------------------------------------------------------------------
   c->tml = P;
+  if (tml_config(c, P, 1).smem == 0) { c->tml = nullptr; delete P; return unusable("tables + tile exceed shared memory"); }
+  // ---- upload ----------------------------------------------------------------------------------
+  P->partials_batch = 4;
   auto up = [&](void** d, const void* h, size_t bytes) -> bool {
     if (cudaMalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
     if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
     return true;
   };
+  const size_t pbytes = (size_t)P->nT * 24 * (size_t)P->partials_batch;
   bool ok = up((void**)&P->d_blob, blob.data(), blob.size()) && up((void**)&P->d_items, items.data(), items.size() * 4) &&
             up((void**)&P->d_item_off, item_off.data(), item_off.size() * 4) &&
             up((void**)&P->d_bond_class, bclass.data(), bclass.size() * 4) &&
-            up((void**)&P->d_bond_entry, bentry.data(), bentry.size() * 4) && up((void**)&P->d_bond_ts, bts.data(), bts.size() * 4) &&
-            up((void**)&P->d_partials, nullptr, (size_t)P->nT * 24) && up((void**)&P->d_counter, nullptr, 16);
-  if (ok) ok = cudaMemset(P->d_partials, 0, (size_t)P->nT * 24) == cudaSuccess && cudaMemset(P->d_counter, 0, 16) == cudaSuccess;
+            up((void**)&P->d_bond_entry, bentry.data(), bentry.size() * 4) &&
+            up((void**)&P->d_partials, nullptr, pbytes) && up((void**)&P->d_counter, nullptr, 16);
+  if (ok) ok = cudaMemset(P->d_partials, 0, pbytes) == cudaSuccess && cudaMemset(P->d_counter, 0, 16) == cudaSuccess;
   if (!ok) { cudaGetLastError(); ftlm_tml_plan_destroy(c); ftlm_set_error("TML: table upload failed"); return FTLM_ENOMEM; }
   return FTLM_OK;
 }
@@ -612,26 +885,27 @@ int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key) {
   if (!t) return -1;
   if (!strcmp(key, "tml_w")) return t->w;
   if (!strcmp(key, "tml_m")) return t->m;
-  if (!strcmp(key, "tml_smem")) return (int64_t)t->smem_bytes;
-  if (!strcmp(key, "tml_ctas_per_sm")) return t->ctas_per_sm;
-  if (!strcmp(key, "tml_threads")) return t->threads;
+  if (!strcmp(key, "tml_smem")) return (int64_t)tml_config(c, t, 1).smem;
+  if (!strcmp(key, "tml_ctas_per_sm")) return tml_config(c, t, 1).ctas;
+  if (!strcmp(key, "tml_threads")) return tml_config(c, t, 1).threads;
+  if (!strcmp(key, "tml_max_batch")) { int b = 4; while (b > 1 && tml_config(c, t, b).smem == 0) b >>= 1; return b; }
   if (!strcmp(key, "tml_n_ll")) return t->n_ll;
   if (!strcmp(key, "tml_n_mm")) return t->n_mm;
   if (!strcmp(key, "tml_n_ml")) return t->n_ml;
   if (!strcmp(key, "tml_n_tt")) return t->n_tt;
-  if (!strcmp(key, "tml_n_tm")) { int n = 0; for (auto k : t->tx_kind) n += (k == 0); return n; }
-  if (!strcmp(key, "tml_n_tl")) { int n = 0; for (auto k : t->tx_kind) n += (k == 1); return n; }
+  if (!strcmp(key, "tml_n_tm")) return t->n_tm;
+  if (!strcmp(key, "tml_n_tl")) return t->n_tl;
   return -1;
 }
 
-int ftlm_launch_hv_tml(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s) {
+int ftlm_launch_hv_tml(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, int batch, cudaStream_t s) {
   if (!c->tml) { ftlm_set_error("TML kernel unavailable"); return FTLM_EUNSUPPORTED; }
   if (c->prec == FTLM_FP32) {
-    if (c->mode == FTLM_INDEX_CLT) return launch_tml<float, FTLM_INDEX_CLT>(c, v, qprev, y, fused, s);
-    return launch_tml<float, FTLM_INDEX_CR>(c, v, qprev, y, fused, s);
+    if (c->mode == FTLM_INDEX_CLT) return launch_tml_b<float, FTLM_INDEX_CLT>(c, v, qprev, y, fused, batch, s);
+    return launch_tml_b<float, FTLM_INDEX_CR>(c, v, qprev, y, fused, batch, s);
   }
-  if (c->mode == FTLM_INDEX_CLT) return launch_tml<double, FTLM_INDEX_CLT>(c, v, qprev, y, fused, s);
-  return launch_tml<double, FTLM_INDEX_CR>(c, v, qprev, y, fused, s);
+  if (c->mode == FTLM_INDEX_CLT) return launch_tml_b<double, FTLM_INDEX_CLT>(c, v, qprev, y, fused, batch, s);
+  return launch_tml_b<double, FTLM_INDEX_CR>(c, v, qprev, y, fused, batch, s);
 }
 
 int ftlm_launch_neighbors_tml(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s) {
@@ -642,9 +916,9 @@ int ftlm_launch_neighbors_tml(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
 #define LAUNCHN(R, MODE)                                                                                   \
   do {                                                                                                     \
     TmlParams<R> p;                                                                                        \
-    fill_params<R>(c, t, p);                                                                               \
+    fill_params<R>(c, t, p, 1);                                                                            \
     neighbors_tml_kernel<R, MODE><<<(int)blocks, 256, 0, s>>>(p, c->d_bonds, c->nb, t->d_bond_class,        \
-                                                               t->d_bond_entry, t->d_bond_ts, row0, nrows, d_idx); \
+                                                               t->d_bond_entry, row0, nrows, d_idx);       \
   } while (0)
   if (c->prec == FTLM_FP32) { if (c->mode == FTLM_INDEX_CLT) LAUNCHN(float, FTLM_INDEX_CLT); else LAUNCHN(float, FTLM_INDEX_CR); }
   else { if (c->mode == FTLM_INDEX_CLT) LAUNCHN(double, FTLM_INDEX_CLT); else LAUNCHN(double, FTLM_INDEX_CR); }
