@@ -1,6 +1,13 @@
 // Internal definitions shared by the CUDA translation units of libftlm (not part of the ABI).
 #pragma once
+#ifdef FTLM_EMU
+// host SIMT emulation used by the -m "not gpu" tests (tests/emu/); never part of libftlm.so
+#include "cuda_emu.h"
+#else
 #include <cuda_runtime.h>
+#define FTLM_LAUNCH(kernel, grid, block, smem, stream, ...) kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__)
+#define FTLM_DYN_SMEM(name) extern __shared__ __align__(16) unsigned char name[]
+#endif
 #include <stdint.h>
 #include <string>
 #include <vector>

@@ -246,7 +246,7 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
     CKF(cudaMalloc(&c->d_clt, sizeof(uint2) * (size_t)c->n_clt));
     int grid = (int)((c->n_clt + 255) / 256);
     if (grid > c->sm_count * 16) grid = c->sm_count * 16;
-    clt_build_kernel<<<grid, 256>>>(c->d_clt, c->n_clt, N, N_up, c->d_binom64);
+    FTLM_LAUNCH(clt_build_kernel, grid, 256, 0, 0, c->d_clt, c->n_clt, N, N_up, c->d_binom64);
     CKF(cudaGetLastError());
   }
   for (int k = 0; k < 4; ++k) CKF(cudaEventCreate(&c->ev[k]));
@@ -407,10 +407,10 @@ extern "C" int ftlm_fill_random(ftlm_ctx* c, uint64_t seed, int r, void* d_v, vo
   cudaStream_t s = (cudaStream_t)stream;
   const uint64_t key = chain_key(seed, c->N_up, r);
   const int grid = stream_grid(c, c->dim, 8);
-  gauss_norm_kernel<<<grid, 256, 0, s>>>(key, c->dim, c->d_partials);
-  reduce_partials_kernel<<<1, 256, 0, s>>>(c->d_partials, grid, &c->d_state->norm2);
-  if (c->prec == FTLM_FP32) gauss_write_kernel<float><<<grid, 256, 0, s>>>(key, c->dim, &c->d_state->norm2, (float*)d_v);
-  else gauss_write_kernel<double><<<grid, 256, 0, s>>>(key, c->dim, &c->d_state->norm2, (double*)d_v);
+  FTLM_LAUNCH(gauss_norm_kernel, grid, 256, 0, s, key, c->dim, c->d_partials);
+  FTLM_LAUNCH(reduce_partials_kernel, 1, 256, 0, s, c->d_partials, grid, &c->d_state->norm2);
+  if (c->prec == FTLM_FP32) { auto k__ = gauss_write_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, &c->d_state->norm2, (float*)d_v); }
+  else { auto k__ = gauss_write_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, &c->d_state->norm2, (double*)d_v); }
   CK(cudaGetLastError());
   return FTLM_OK;
 }
@@ -441,14 +441,14 @@ static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64
     // copy into q[2] (scratch), then normalise in FP64 into q[0]
     CK(cudaMemcpyAsync(c->q[2], q1, bytes, q1_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
     const int grid = stream_grid(c, c->dim, 8);
-    if (c->prec == FTLM_FP32) sumsq_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[2], c->dim, c->d_partials);
-    else sumsq_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[2], c->dim, c->d_partials);
-    reduce_partials_kernel<<<1, 256, 0, s>>>(c->d_partials, grid, &c->d_state->norm2);
-    if (c->prec == FTLM_FP32) scale_copy_kernel<float><<<grid, 256, 0, s>>>((const float*)c->q[2], c->dim, &c->d_state->norm2, (float*)c->q[0]);
-    else scale_copy_kernel<double><<<grid, 256, 0, s>>>((const double*)c->q[2], c->dim, &c->d_state->norm2, (double*)c->q[0]);
+    if (c->prec == FTLM_FP32) { auto k__ = sumsq_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)c->q[2], c->dim, c->d_partials); }
+    else { auto k__ = sumsq_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)c->q[2], c->dim, c->d_partials); }
+    FTLM_LAUNCH(reduce_partials_kernel, 1, 256, 0, s, c->d_partials, grid, &c->d_state->norm2);
+    if (c->prec == FTLM_FP32) { auto k__ = scale_copy_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)c->q[2], c->dim, &c->d_state->norm2, (float*)c->q[0]); }
+    else { auto k__ = scale_copy_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)c->q[2], c->dim, &c->d_state->norm2, (double*)c->q[0]); }
   }
   CK(cudaMemsetAsync(c->q[1], 0, bytes, s));          // q_0 = 0
-  chain_reset_kernel<<<1, 32, 0, s>>>(c->d_state, c->chain_limit, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
+  FTLM_LAUNCH(chain_reset_kernel, 1, 32, 0, s, c->d_state, c->chain_limit, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
   CK(cudaGetLastError());
   return FTLM_OK;
 }
@@ -463,8 +463,8 @@ static int launch_next(ftlm_ctx* c, cudaStream_t s) {
   const void* q = c->q[c->cur];
   void* qn = c->q[1 - c->cur];
   const int grid = stream_grid(c, c->dim / 4 + 1, 8);
-  if (c->prec == FTLM_FP32) lanczos_next_kernel<float, float4><<<grid, 256, 0, s>>>((const float*)y, (const float*)q, (float*)qn, c->dim, c->d_state);
-  else lanczos_next_kernel<double, double2><<<grid, 256, 0, s>>>((const double*)y, (const double*)q, (double*)qn, c->dim, c->d_state);
+  if (c->prec == FTLM_FP32) { auto k__ = lanczos_next_kernel<float, float4>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)y, (const float*)q, (float*)qn, c->dim, c->d_state); }
+  else { auto k__ = lanczos_next_kernel<double, double2>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)y, (const double*)q, (double*)qn, c->dim, c->d_state); }
   CK(cudaGetLastError());
   return FTLM_OK;
 }
@@ -546,7 +546,7 @@ static int lanczos_impl(ftlm_ctx* c, const void* h_q1, uint64_t seed, int R, int
     if (rc != FTLM_OK) return rc;
     if (c->chain_limit > n_steps) {           // m = min(n_steps, dim)
       c->chain_limit = n_steps;
-      chain_reset_kernel<<<1, 32, 0, s>>>(c->d_state, n_steps, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
+      FTLM_LAUNCH(chain_reset_kernel, 1, 32, 0, s, c->d_state, n_steps, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
     }
     rc = ftlm_chain_steps(c, n_steps, s);
     if (rc != FTLM_OK) return rc;

@@ -104,7 +104,7 @@ __device__ __forceinline__ void load_tables(const RowParams& p, I* s_binom, Bond
 template <typename R, typename L, typename I, int MODE, bool FUSED>
 __global__ void __launch_bounds__(256)
 hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev, R* __restrict__ y) {
-  extern __shared__ __align__(16) unsigned char smem[];
+  FTLM_DYN_SMEM(smem);
   __shared__ double sh_red[96];
   if (FUSED) { if (p.st->done) return; }
   I* s_binom = (I*)smem;
@@ -145,7 +145,7 @@ hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev,
 template <typename L, typename I, int MODE>
 __global__ void __launch_bounds__(256)
 neighbors_row_kernel(RowParams p, int64_t row0, int64_t nrows, int64_t* __restrict__ out) {
-  extern __shared__ __align__(16) unsigned char smem[];
+  FTLM_DYN_SMEM(smem);
   I* s_binom = (I*)smem;
   const int nbin = (p.N + 1) * (p.K + 1);
   BondS<float>* s_bonds = (BondS<float>*)(smem + (((size_t)nbin * sizeof(I) + 15) & ~(size_t)15));
@@ -171,7 +171,7 @@ neighbors_row_kernel(RowParams p, int64_t row0, int64_t nrows, int64_t* __restri
 template <typename L, typename I>
 __global__ void index_of_kernel(RowParams p, const uint64_t* __restrict__ labels, int64_t n,
                                 int64_t* __restrict__ out) {
-  extern __shared__ __align__(16) unsigned char smem[];
+  FTLM_DYN_SMEM(smem);
   I* s_binom = (I*)smem;
   const int nbin = (p.N + 1) * (p.K + 1);
   for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = ((const I*)p.binom)[k];
@@ -193,7 +193,7 @@ __global__ void index_of_kernel(RowParams p, const uint64_t* __restrict__ labels
 template <typename L, typename I>
 __global__ void state_of_kernel(RowParams p, const int64_t* __restrict__ idx, int64_t n,
                                 uint64_t* __restrict__ out) {
-  extern __shared__ __align__(16) unsigned char smem[];
+  FTLM_DYN_SMEM(smem);
   I* s_binom = (I*)smem;
   const int nbin = (p.N + 1) * (p.K + 1);
   for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = ((const I*)p.binom)[k];
@@ -238,7 +238,7 @@ int launch_hv(ftlm_ctx* c, const RowParams& p, const void* v, const void* qp, vo
   do {                                                                                           \
     auto k = hv_row_kernel<R, L, I, MODE, FUSED>;                                                \
     if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
-    k<<<grid, 256, sm, s>>>(p, (const R*)v, (const R*)qp, (R*)y);                                \
+    FTLM_LAUNCH(k, grid, 256, sm, s, p, (const R*)v, (const R*)qp, (R*)y);                                \
   } while (0)
   if (c->mode == FTLM_INDEX_CLT) { if (fused) LAUNCH(FTLM_INDEX_CLT, true); else LAUNCH(FTLM_INDEX_CLT, false); }
   else { if (fused) LAUNCH(FTLM_INDEX_CR, true); else LAUNCH(FTLM_INDEX_CR, false); }
@@ -271,11 +271,11 @@ int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
     if (c->mode == FTLM_INDEX_CLT) {                                                                  \
       auto k = neighbors_row_kernel<L, I, FTLM_INDEX_CLT>;                                            \
       if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
-      k<<<grid, 256, sm, s>>>(p, row0, nrows, d_idx);                                                 \
+      FTLM_LAUNCH(k, grid, 256, sm, s, p, row0, nrows, d_idx);                                                 \
     } else {                                                                                          \
       auto k = neighbors_row_kernel<L, I, FTLM_INDEX_CR>;                                             \
       if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
-      k<<<grid, 256, sm, s>>>(p, row0, nrows, d_idx);                                                 \
+      FTLM_LAUNCH(k, grid, 256, sm, s, p, row0, nrows, d_idx);                                                 \
     }                                                                                                 \
   } while (0)
   if (!c->lab64) LAUNCHN(uint32_t, uint32_t);
@@ -294,9 +294,9 @@ extern "C" int ftlm_index_of(ftlm_ctx* c, const uint64_t* d_labels, int64_t n, i
   const size_t sm = table_smem(c, 0);
   const int grid = grid_for(c, n, 8);
   cudaStream_t s = (cudaStream_t)stream;
-  if (!c->lab64) index_of_kernel<uint32_t, uint32_t><<<grid, 256, sm, s>>>(p, d_labels, n, d_idx);
-  else if (!c->idx64) index_of_kernel<uint64_t, uint32_t><<<grid, 256, sm, s>>>(p, d_labels, n, d_idx);
-  else index_of_kernel<uint64_t, uint64_t><<<grid, 256, sm, s>>>(p, d_labels, n, d_idx);
+  if (!c->lab64) { auto k__ = index_of_kernel<uint32_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_labels, n, d_idx); }
+  else if (!c->idx64) { auto k__ = index_of_kernel<uint64_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_labels, n, d_idx); }
+  else { auto k__ = index_of_kernel<uint64_t, uint64_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_labels, n, d_idx); }
   CK(cudaGetLastError());
   return FTLM_OK;
 }
@@ -309,9 +309,9 @@ extern "C" int ftlm_state_of(ftlm_ctx* c, const int64_t* d_idx, int64_t n, uint6
   const size_t sm = table_smem(c, 0);
   const int grid = grid_for(c, n, 8);
   cudaStream_t s = (cudaStream_t)stream;
-  if (!c->lab64) state_of_kernel<uint32_t, uint32_t><<<grid, 256, sm, s>>>(p, d_idx, n, d_labels);
-  else if (!c->idx64) state_of_kernel<uint64_t, uint32_t><<<grid, 256, sm, s>>>(p, d_idx, n, d_labels);
-  else state_of_kernel<uint64_t, uint64_t><<<grid, 256, sm, s>>>(p, d_idx, n, d_labels);
+  if (!c->lab64) { auto k__ = state_of_kernel<uint32_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_idx, n, d_labels); }
+  else if (!c->idx64) { auto k__ = state_of_kernel<uint64_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_idx, n, d_labels); }
+  else { auto k__ = state_of_kernel<uint64_t, uint64_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_idx, n, d_labels); }
   CK(cudaGetLastError());
   return FTLM_OK;
 }

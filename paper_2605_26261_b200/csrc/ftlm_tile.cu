@@ -148,7 +148,7 @@ __device__ __forceinline__ uint32_t local_index(uint32_t Lp, const uint16_t* __r
 template <typename R, int MODE, bool FUSED>
 __global__ void __launch_bounds__(TILE_THREADS)
 hv_tile_kernel(TileParams p, const R* __restrict__ v, const R* __restrict__ qprev, R* __restrict__ y) {
-  extern __shared__ __align__(16) unsigned char smem[];
+  FTLM_DYN_SMEM(smem);
   __shared__ double sh_red[96];
   __shared__ int s_nhh_active;
   __shared__ uint64_t s_base;
@@ -360,13 +360,13 @@ int launch_tile(ftlm_ctx* c, const TileParams& p, const void* v, const void* qp,
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem_bytes));
     int occ = 1;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, TILE_THREADS, t->smem_bytes));
-    k<<<grid_of(occ < 1 ? 1 : occ), TILE_THREADS, t->smem_bytes, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
+    FTLM_LAUNCH(k, grid_of(occ < 1 ? 1 : occ), TILE_THREADS, t->smem_bytes, s, p, (const R*)v, (const R*)qp, (R*)y);
   } else {
     auto k = hv_tile_kernel<R, MODE, false>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem_bytes));
     int occ = 1;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, TILE_THREADS, t->smem_bytes));
-    k<<<grid_of(occ < 1 ? 1 : occ), TILE_THREADS, t->smem_bytes, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
+    FTLM_LAUNCH(k, grid_of(occ < 1 ? 1 : occ), TILE_THREADS, t->smem_bytes, s, p, (const R*)v, (const R*)qp, (R*)y);
   }
   CK(cudaGetLastError());
   return FTLM_OK;
@@ -480,8 +480,8 @@ int ftlm_launch_neighbors_tile(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t
   TileParams p = make_tile_params(c);
   int64_t blocks = (nrows + 255) / 256;
   if (blocks > c->sm_count * 8) blocks = c->sm_count * 8;
-  if (c->mode == FTLM_INDEX_CLT) neighbors_tile_kernel<FTLM_INDEX_CLT><<<(int)blocks, 256, 0, s>>>(p, c->d_bonds, c->nb, row0, nrows, d_idx);
-  else neighbors_tile_kernel<FTLM_INDEX_CR><<<(int)blocks, 256, 0, s>>>(p, c->d_bonds, c->nb, row0, nrows, d_idx);
+  if (c->mode == FTLM_INDEX_CLT) { auto k__ = neighbors_tile_kernel<FTLM_INDEX_CLT>; FTLM_LAUNCH(k__, (int)blocks, 256, 0, s, p, c->d_bonds, c->nb, row0, nrows, d_idx); }
+  else { auto k__ = neighbors_tile_kernel<FTLM_INDEX_CR>; FTLM_LAUNCH(k__, (int)blocks, 256, 0, s, p, c->d_bonds, c->nb, row0, nrows, d_idx); }
   CK(cudaGetLastError());
   return FTLM_OK;
 }

@@ -199,9 +199,13 @@ __device__ __forceinline__ void load_fent(const FEnt<double>* e, uint32_t& off, 
   off = e->off; fl = e->fl; J = e->J; uw = e->uw;
 }
 __device__ __forceinline__ const void* addr_u32(const void* base, uint32_t idx, uint32_t scale) {
+#ifdef FTLM_EMU
+  return (const void*)((const unsigned char*)base + (unsigned long long)idx * scale);
+#else
   unsigned long long a;
   asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(a) : "r"(idx), "r"(scale), "l"((unsigned long long)base));
   return (const void*)a;
+#endif
 }
 
 template <typename R, int B, int MODE, bool FUSED>
@@ -210,7 +214,7 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
               R* __restrict__ y_) {
   typedef Vec<R, B> V;
   constexpr int RB = (int)sizeof(V);                    // bytes per row
-  extern __shared__ __align__(16) unsigned char smem[];
+  FTLM_DYN_SMEM(smem);
   __shared__ bool s_last;
   if (FUSED) {
     bool all_done = true;
@@ -704,11 +708,11 @@ int launch_tml(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, c
   if (fused) {
     auto k = hv_tml_kernel<R, B, MODE, true>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
-    k<<<grid, cfg.threads, cfg.smem, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
+    FTLM_LAUNCH(k, grid, cfg.threads, cfg.smem, s, p, (const R*)v, (const R*)qp, (R*)y);
   } else {
     auto k = hv_tml_kernel<R, B, MODE, false>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
-    k<<<grid, cfg.threads, cfg.smem, s>>>(p, (const R*)v, (const R*)qp, (R*)y);
+    FTLM_LAUNCH(k, grid, cfg.threads, cfg.smem, s, p, (const R*)v, (const R*)qp, (R*)y);
   }
   CK(cudaGetLastError());
   return FTLM_OK;
@@ -917,8 +921,8 @@ int ftlm_launch_neighbors_tml(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
   do {                                                                                                     \
     TmlParams<R> p;                                                                                        \
     fill_params<R>(c, t, p, 1);                                                                            \
-    neighbors_tml_kernel<R, MODE><<<(int)blocks, 256, 0, s>>>(p, c->d_bonds, c->nb, t->d_bond_class,        \
-                                                               t->d_bond_entry, row0, nrows, d_idx);       \
+    { auto k__ = neighbors_tml_kernel<R, MODE>; FTLM_LAUNCH(k__, (int)blocks, 256, 0, s, p, c->d_bonds, c->nb, t->d_bond_class,        \
+                                                               t->d_bond_entry, row0, nrows, d_idx); }       \
   } while (0)
   if (c->prec == FTLM_FP32) { if (c->mode == FTLM_INDEX_CLT) LAUNCHN(float, FTLM_INDEX_CLT); else LAUNCHN(float, FTLM_INDEX_CR); }
   else { if (c->mode == FTLM_INDEX_CLT) LAUNCHN(double, FTLM_INDEX_CLT); else LAUNCHN(double, FTLM_INDEX_CR); }

@@ -1,0 +1,240 @@
+// cuda_emu.cpp - TEST INFRASTRUCTURE: fiber scheduler and guarded "device" memory behind cuda_emu.h.
+#include "cuda_emu.h"
+
+#include <sys/mman.h>
+#include <time.h>
+#include <ucontext.h>
+#include <unistd.h>
+
+#include <map>
+#include <vector>
+
+uint3 threadIdx, blockIdx;
+dim3 blockDim, gridDim;
+
+namespace {
+
+[[noreturn]] void die(const char* msg) {
+  fprintf(stderr, "cuda_emu: %s (block %u thread %u)\n", msg, blockIdx.x, threadIdx.x);
+  fflush(stderr);
+  abort();
+}
+
+// ---- guarded allocations: [PROT_NONE page][slack ... data (16-byte aligned, ends at page end)][PROT_NONE page]
+struct Alloc { void* map; size_t map_bytes; };
+std::map<void*, Alloc> g_allocs;
+const size_t PAGE = 4096;
+
+void* guarded_alloc(size_t bytes) {
+  const size_t data = (bytes + 15) & ~(size_t)15;
+  const size_t body = ((data + PAGE - 1) / PAGE) * PAGE;
+  const size_t total = body + 2 * PAGE;
+  char* m = (char*)mmap(nullptr, total, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
+  if (m == MAP_FAILED) return nullptr;
+  mprotect(m, PAGE, PROT_NONE);
+  mprotect(m + PAGE + body, PAGE, PROT_NONE);
+  char* p = m + PAGE + body - data;        // the data ends exactly at the trailing guard page
+  memset(m + PAGE, 0xCD, body - data);      // slack in front: poison
+  memset(p, 0xA5, data);                    // uninitialised device memory is not zero
+  g_allocs[p] = Alloc{m, total};
+  return p;
+}
+void guarded_free(void* p) {
+  auto it = g_allocs.find(p);
+  if (it == g_allocs.end()) die("cudaFree of an unknown pointer");
+  munmap(it->second.map, it->second.map_bytes);
+  g_allocs.erase(it);
+}
+
+// ---- fibers ------------------------------------------------------------------------------------
+struct Fiber { ucontext_t ctx; char* stack = nullptr; bool done = false; bool started = false; };
+const size_t STACK = 64 * 1024;
+std::vector<Fiber> g_fib;
+std::vector<char*> g_stack_pool;
+ucontext_t g_main;
+int g_cur = -1;
+unsigned g_nthreads = 0;
+unsigned long long g_progress = 0;
+const std::function<void()>* g_body = nullptr;
+unsigned char* g_dyn = nullptr;
+
+// CTA barrier
+unsigned g_bar_arrived = 0, g_bar_gen = 0, g_alive = 0;
+
+struct Warp {
+  uint64_t val[32], out[32];
+  int arg[32];
+  unsigned arrived_mask = 0, gen = 0, alive_mask = 0, want_mask = 0;
+  int op = -1;
+};
+std::vector<Warp> g_warps;
+
+void yield_to_scheduler() { swapcontext(&g_fib[(size_t)g_cur].ctx, &g_main); }
+
+void complete_collective(Warp& w) {
+  const unsigned part = w.arrived_mask;
+  switch (w.op) {
+    case cuda_emu::OP_SYNCWARP: break;
+    case cuda_emu::OP_BALLOT: {
+      unsigned b = 0;
+      for (int l = 0; l < 32; ++l) if ((part >> l) & 1u) b |= (w.val[l] ? 1u : 0u) << l;
+      for (int l = 0; l < 32; ++l) w.out[l] = b;
+      break;
+    }
+    case cuda_emu::OP_SHFL_DOWN:
+      for (int l = 0; l < 32; ++l) { const int s = l + w.arg[l]; w.out[l] = (s < 32 && ((part >> s) & 1u)) ? w.val[s] : w.val[l]; }
+      break;
+    case cuda_emu::OP_SHFL_UP:
+      for (int l = 0; l < 32; ++l) { const int s = l - w.arg[l]; w.out[l] = (s >= 0 && ((part >> s) & 1u)) ? w.val[s] : w.val[l]; }
+      break;
+    case cuda_emu::OP_SHFL_XOR:
+      for (int l = 0; l < 32; ++l) { const int s = l ^ w.arg[l]; w.out[l] = (s < 32 && ((part >> s) & 1u)) ? w.val[s] : w.val[l]; }
+      break;
+    case cuda_emu::OP_SHFL_IDX:
+      for (int l = 0; l < 32; ++l) { const int s = w.arg[l] & 31; w.out[l] = ((part >> s) & 1u) ? w.val[s] : w.val[l]; }
+      break;
+    default: die("unknown collective");
+  }
+  w.arrived_mask = 0;
+  w.op = -1;
+  w.gen++;
+  g_progress++;
+}
+
+void fiber_entry() {
+  (*g_body)();
+  Fiber& f = g_fib[(size_t)g_cur];
+  f.done = true;
+  g_progress++;
+  g_alive--;
+  Warp& w = g_warps[(size_t)g_cur >> 5];
+  w.alive_mask &= ~(1u << (g_cur & 31));
+  // an exit may complete a rendezvous the others are waiting in
+  if (g_bar_arrived > 0 && g_bar_arrived == g_alive) { g_bar_arrived = 0; g_bar_gen++; g_progress++; }
+  if (w.arrived_mask && w.arrived_mask == (w.want_mask & w.alive_mask)) complete_collective(w);
+  swapcontext(&f.ctx, &g_main);
+  die("resumed a finished fiber");
+}
+
+void run_block() {
+  const unsigned nt = g_nthreads;
+  if (g_fib.size() < nt) g_fib.resize(nt);
+  while (g_stack_pool.size() < nt) g_stack_pool.push_back((char*)malloc(STACK));
+  g_warps.assign((nt + 31) / 32, Warp());
+  for (unsigned i = 0; i < nt; ++i) {
+    Fiber& f = g_fib[i];
+    f.done = false; f.started = false; f.stack = g_stack_pool[i];
+    getcontext(&f.ctx);
+    f.ctx.uc_stack.ss_sp = f.stack;
+    f.ctx.uc_stack.ss_size = STACK;
+    f.ctx.uc_link = &g_main;
+    makecontext(&f.ctx, (void (*)())fiber_entry, 0);
+    g_warps[i >> 5].alive_mask |= 1u << (i & 31);
+  }
+  g_alive = nt; g_bar_arrived = 0; g_bar_gen = 0;
+  for (;;) {
+    const unsigned long long before = g_progress;
+    bool any = false;
+    for (unsigned i = 0; i < nt; ++i) {
+      Fiber& f = g_fib[i];
+      if (f.done) continue;
+      any = true;
+      g_cur = (int)i;
+      threadIdx.x = i; threadIdx.y = 0; threadIdx.z = 0;
+      if (!f.started) { f.started = true; g_progress++; }
+      swapcontext(&g_main, &f.ctx);
+    }
+    if (!any) break;
+    if (g_progress == before) die("deadlock: no thread of the CTA can make progress (mismatched barrier / collective)");
+  }
+  g_cur = -1;
+}
+
+cudaError_t g_last = cudaSuccess;
+
+}  // namespace
+
+namespace cuda_emu {
+
+unsigned char* dyn_smem() { return g_dyn; }
+
+void sync_threads() {
+  if (g_cur < 0) die("__syncthreads outside a kernel");
+  const unsigned my = g_bar_gen;
+  g_bar_arrived++;
+  if (g_bar_arrived == g_alive) { g_bar_arrived = 0; g_bar_gen++; g_progress++; return; }
+  while (g_bar_gen == my) yield_to_scheduler();
+  threadIdx.x = (unsigned)g_cur;
+}
+
+uint64_t collective(int op, unsigned mask, uint64_t v, int arg) {
+  if (g_cur < 0) die("warp collective outside a kernel");
+  Warp& w = g_warps[(size_t)g_cur >> 5];
+  const int lane = g_cur & 31;
+  if (!((mask >> lane) & 1u)) die("warp collective: calling lane not in its own mask");
+  if (w.arrived_mask == 0) { w.op = op; w.want_mask = mask; }
+  else if (w.op != op || w.want_mask != mask) die("warp collective mismatch: lanes of one warp are in different collectives");
+  w.val[lane] = v; w.arg[lane] = arg;
+  w.arrived_mask |= 1u << lane;
+  const unsigned my = w.gen;
+  if (w.arrived_mask == (w.want_mask & w.alive_mask)) complete_collective(w);
+  else while (w.gen == my) yield_to_scheduler();
+  threadIdx.x = (unsigned)g_cur;
+  return w.out[lane];
+}
+
+void launch(unsigned grid, unsigned block, size_t dyn_bytes, const std::function<void()>& body) {
+  if (g_cur >= 0) die("nested launch");
+  if (grid == 0 || block == 0 || block > 1024) { g_last = cudaErrorInvalidValue; return; }
+  if (dyn_bytes > 227 * 1024) { g_last = cudaErrorInvalidValue; return; }
+  g_body = &body;
+  g_nthreads = block;
+  gridDim = dim3(grid); blockDim = dim3(block);
+  for (unsigned b = 0; b < grid; ++b) {
+    blockIdx.x = b; blockIdx.y = 0; blockIdx.z = 0;
+    g_dyn = dyn_bytes ? (unsigned char*)guarded_alloc(dyn_bytes) : nullptr;
+    run_block();
+    if (g_dyn) guarded_free(g_dyn);
+    g_dyn = nullptr;
+  }
+  g_body = nullptr;
+}
+
+}  // namespace cuda_emu
+
+// ---- runtime API ---------------------------------------------------------------------------------
+struct cuda_emu_event { double t_ms; };
+
+cudaError_t cudaGetDeviceCount(int* n) { *n = getenv("FTLM_EMU_NO_DEVICE") ? 0 : 1; return *n ? cudaSuccess : cudaErrorNoDevice; }
+cudaError_t cudaSetDevice(int) { return cudaSuccess; }
+cudaError_t cudaGetDeviceProperties(cudaDeviceProp* p, int) {
+  memset(p, 0, sizeof(*p));
+  snprintf(p->name, sizeof(p->name), "cuda_emu (host SIMT emulation)");
+  const char* s = getenv("FTLM_EMU_SMS");
+  p->multiProcessorCount = s ? atoi(s) : 3;
+  p->sharedMemPerBlockOptin = 227 * 1024;
+  p->major = 10; p->minor = 0;
+  p->l2CacheSize = 126u << 20;
+  return cudaSuccess;
+}
+cudaError_t cudaMalloc(void** p, size_t bytes) {
+  *p = guarded_alloc(bytes ? bytes : 16);
+  if (!*p) { g_last = cudaErrorMemoryAllocation; return cudaErrorMemoryAllocation; }
+  return cudaSuccess;
+}
+cudaError_t cudaFree(void* p) { if (p) guarded_free(p); return cudaSuccess; }
+cudaError_t cudaMemcpy(void* d, const void* s, size_t n, cudaMemcpyKind) { if (n) memmove(d, s, n); return cudaSuccess; }
+cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind k, cudaStream_t) { return cudaMemcpy(d, s, n, k); }
+cudaError_t cudaMemset(void* p, int v, size_t n) { if (n) memset(p, v, n); return cudaSuccess; }
+cudaError_t cudaMemsetAsync(void* p, int v, size_t n, cudaStream_t) { return cudaMemset(p, v, n); }
+cudaError_t cudaGetLastError() { cudaError_t e = g_last; g_last = cudaSuccess; return e; }
+cudaError_t cudaPeekAtLastError() { return g_last; }
+const char* cudaGetErrorString(cudaError_t e) { return e == cudaSuccess ? "no error" : e == cudaErrorMemoryAllocation ? "out of memory" : "cuda_emu error"; }
+cudaError_t cudaDeviceSynchronize() { return cudaSuccess; }
+cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSuccess; }
+static double now_ms() { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6; }
+cudaError_t cudaEventCreate(cudaEvent_t* e) { *e = new cuda_emu_event{0.0}; return cudaSuccess; }
+cudaError_t cudaEventDestroy(cudaEvent_t e) { delete e; return cudaSuccess; }
+cudaError_t cudaEventRecord(cudaEvent_t e, cudaStream_t) { e->t_ms = now_ms(); return cudaSuccess; }
+cudaError_t cudaEventSynchronize(cudaEvent_t) { return cudaSuccess; }
+cudaError_t cudaEventElapsedTime(float* ms, cudaEvent_t a, cudaEvent_t b) { *ms = (float)(b->t_ms - a->t_ms); return cudaSuccess; }

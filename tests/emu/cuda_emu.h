@@ -1,0 +1,127 @@
+// cuda_emu.h - TEST INFRASTRUCTURE: a minimal SIMT emulation of the CUDA constructs that libftlm's
+// kernels use, so that the SAME kernel sources (paper_2605_26261_b200/csrc/*.cu, compiled as C++
+// with -DFTLM_EMU) can be executed on the host by `-m "not gpu"` tests: every CUDA thread of a CTA is
+// a fiber (ucontext), __syncthreads / __syncwarp / __ballot_sync / __shfl_*_sync are real rendezvous
+// points, "device" memory is guarded host memory (a PROT_NONE page directly behind every allocation
+// and behind the dynamic shared memory, so reads or writes past the end fault instead of passing).
+// CTAs of a grid run one after another.  This is a checker for index arithmetic, table construction,
+// barrier placement and bounds - it is never loaded by the product binding and has no performance
+// meaning.
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <functional>
+
+#define __host__
+#define __device__
+#define __global__
+#define __forceinline__ inline
+#define __launch_bounds__(...)
+#define __grid_constant__
+#define __align__(n) __attribute__((aligned(n)))
+#define __shared__ static
+#ifndef __CUDACC__
+#define __CUDACC__ 1          // ftlm_common.cuh guards its device helpers with this
+#endif
+
+struct uint3 { unsigned x, y, z; };
+struct dim3 { unsigned x = 1, y = 1, z = 1; dim3() {} dim3(unsigned a, unsigned b = 1, unsigned c = 1) : x(a), y(b), z(c) {} };
+struct __attribute__((aligned(8))) float2 { float x, y; };
+struct __attribute__((aligned(16))) float4 { float x, y, z, w; };
+struct __attribute__((aligned(16))) double2 { double x, y; };
+struct __attribute__((aligned(8))) uint2 { unsigned x, y; };
+struct __attribute__((aligned(16))) uint4 { unsigned x, y, z, w; };
+struct __attribute__((aligned(8))) int2 { int x, y; };
+static inline uint2 make_uint2(unsigned a, unsigned b) { return uint2{a, b}; }
+static inline uint4 make_uint4(unsigned a, unsigned b, unsigned c, unsigned d) { return uint4{a, b, c, d}; }
+static inline float2 make_float2(float a, float b) { return float2{a, b}; }
+static inline float4 make_float4(float a, float b, float c, float d) { return float4{a, b, c, d}; }
+static inline double2 make_double2(double a, double b) { return double2{a, b}; }
+static inline int2 make_int2(int a, int b) { return int2{a, b}; }
+
+extern uint3 threadIdx, blockIdx;
+extern dim3 blockDim, gridDim;
+
+// ---- runtime API subset ------------------------------------------------------------------------
+typedef int cudaError_t;
+enum { cudaSuccess = 0, cudaErrorInvalidValue = 1, cudaErrorMemoryAllocation = 2, cudaErrorNoDevice = 100 };
+typedef struct cuda_emu_stream* cudaStream_t;
+typedef struct cuda_emu_event* cudaEvent_t;
+enum cudaMemcpyKind { cudaMemcpyHostToHost = 0, cudaMemcpyHostToDevice = 1, cudaMemcpyDeviceToHost = 2, cudaMemcpyDeviceToDevice = 3 };
+enum cudaFuncAttribute { cudaFuncAttributeMaxDynamicSharedMemorySize = 8 };
+struct cudaDeviceProp { char name[256]; int multiProcessorCount; size_t sharedMemPerBlockOptin; int major, minor; size_t l2CacheSize; };
+
+cudaError_t cudaGetDeviceCount(int* n);
+cudaError_t cudaSetDevice(int d);
+cudaError_t cudaGetDeviceProperties(cudaDeviceProp* p, int d);
+cudaError_t cudaMalloc(void** p, size_t bytes);
+template <typename T> static inline cudaError_t cudaMalloc(T** p, size_t bytes) { return cudaMalloc((void**)p, bytes); }
+cudaError_t cudaFree(void* p);
+cudaError_t cudaMemcpy(void* dst, const void* src, size_t bytes, cudaMemcpyKind k);
+cudaError_t cudaMemcpyAsync(void* dst, const void* src, size_t bytes, cudaMemcpyKind k, cudaStream_t s = nullptr);
+cudaError_t cudaMemset(void* p, int v, size_t bytes);
+cudaError_t cudaMemsetAsync(void* p, int v, size_t bytes, cudaStream_t s = nullptr);
+cudaError_t cudaGetLastError();
+cudaError_t cudaPeekAtLastError();
+const char* cudaGetErrorString(cudaError_t e);
+cudaError_t cudaDeviceSynchronize();
+cudaError_t cudaStreamSynchronize(cudaStream_t s);
+cudaError_t cudaEventCreate(cudaEvent_t* e);
+cudaError_t cudaEventDestroy(cudaEvent_t e);
+cudaError_t cudaEventRecord(cudaEvent_t e, cudaStream_t s = nullptr);
+cudaError_t cudaEventSynchronize(cudaEvent_t e);
+cudaError_t cudaEventElapsedTime(float* ms, cudaEvent_t a, cudaEvent_t b);
+template <typename F> static inline cudaError_t cudaFuncSetAttribute(F, cudaFuncAttribute, int) { return cudaSuccess; }
+template <typename F> static inline cudaError_t cudaOccupancyMaxActiveBlocksPerMultiprocessor(int* n, F, int threads, size_t smem) {
+  size_t by_smem = smem ? (size_t)(227 * 1024) / (smem + 1024) : 32;
+  int by_thr = 2048 / (threads > 0 ? threads : 1);
+  *n = (int)std::min<size_t>(by_smem, (size_t)by_thr);
+  return cudaSuccess;
+}
+
+// ---- launch ------------------------------------------------------------------------------------
+namespace cuda_emu {
+void launch(unsigned grid, unsigned block, size_t dyn_smem, const std::function<void()>& body);
+unsigned char* dyn_smem();
+void sync_threads();
+uint64_t collective(int op, unsigned mask, uint64_t v, int arg);
+enum { OP_SYNCWARP = 0, OP_BALLOT = 1, OP_SHFL_DOWN = 2, OP_SHFL_XOR = 3, OP_SHFL_IDX = 4, OP_SHFL_UP = 5 };
+template <typename T> static inline uint64_t pack(T v) { uint64_t u = 0; static_assert(sizeof(T) <= 8, "shfl payload"); memcpy(&u, &v, sizeof(T)); return u; }
+template <typename T> static inline T unpack(uint64_t u) { T v; memcpy(&v, &u, sizeof(T)); return v; }
+}  // namespace cuda_emu
+
+#define FTLM_LAUNCH(kernel, grid, block, smem, stream, ...) \
+  cuda_emu::launch((unsigned)(grid), (unsigned)(block), (size_t)(smem), [&]() { kernel(__VA_ARGS__); })
+#define FTLM_DYN_SMEM(name) unsigned char* name = cuda_emu::dyn_smem()
+
+// ---- intrinsics --------------------------------------------------------------------------------
+static inline void __syncthreads() { cuda_emu::sync_threads(); }
+static inline void __syncwarp(unsigned mask = 0xffffffffu) { cuda_emu::collective(cuda_emu::OP_SYNCWARP, mask, 0, 0); }
+static inline unsigned __ballot_sync(unsigned mask, int pred) { return (unsigned)cuda_emu::collective(cuda_emu::OP_BALLOT, mask, pred ? 1 : 0, 0); }
+template <typename T> static inline T __shfl_down_sync(unsigned mask, T v, int d) { return cuda_emu::unpack<T>(cuda_emu::collective(cuda_emu::OP_SHFL_DOWN, mask, cuda_emu::pack(v), d)); }
+template <typename T> static inline T __shfl_up_sync(unsigned mask, T v, int d) { return cuda_emu::unpack<T>(cuda_emu::collective(cuda_emu::OP_SHFL_UP, mask, cuda_emu::pack(v), d)); }
+template <typename T> static inline T __shfl_xor_sync(unsigned mask, T v, int d) { return cuda_emu::unpack<T>(cuda_emu::collective(cuda_emu::OP_SHFL_XOR, mask, cuda_emu::pack(v), d)); }
+template <typename T> static inline T __shfl_sync(unsigned mask, T v, int src) { return cuda_emu::unpack<T>(cuda_emu::collective(cuda_emu::OP_SHFL_IDX, mask, cuda_emu::pack(v), src)); }
+static inline void __threadfence() {}
+static inline void __threadfence_block() {}
+static inline int __popc(unsigned x) { return __builtin_popcount(x); }
+static inline int __popcll(unsigned long long x) { return __builtin_popcountll(x); }
+static inline int __ffs(int x) { return __builtin_ffs(x); }
+static inline int __ffsll(long long x) { return __builtin_ffsll(x); }
+static inline int __clz(int x) { return x ? __builtin_clz((unsigned)x) : 32; }
+static inline float __uint_as_float(unsigned u) { float f; memcpy(&f, &u, 4); return f; }
+static inline unsigned __float_as_uint(float f) { unsigned u; memcpy(&u, &f, 4); return u; }
+template <typename T> static inline T __ldg(const T* p) { return *p; }
+template <typename T> static inline T __ldcs(const T* p) { return *p; }
+template <typename T> static inline T __ldcg(const T* p) { return *p; }
+template <typename T> static inline void __stcs(T* p, const T& v) { *p = v; }
+template <typename T> static inline void __stcg(T* p, const T& v) { *p = v; }
+static inline unsigned atomicAdd(unsigned* p, unsigned v) { unsigned o = *p; *p = o + v; return o; }
+static inline int atomicAdd(int* p, int v) { int o = *p; *p = o + v; return o; }
+static inline unsigned long long atomicAdd(unsigned long long* p, unsigned long long v) { unsigned long long o = *p; *p = o + v; return o; }
+static inline double atomicAdd(double* p, double v) { double o = *p; *p = o + v; return o; }
+static inline float atomicAdd(float* p, float v) { float o = *p; *p = o + v; return o; }

@@ -1,0 +1,103 @@
+"""TEST INFRASTRUCTURE: run ONE emulated parity case and print a JSON result line.
+
+    python tests/emu/run_case.py '<json spec>'
+
+spec = {"wl": "ring12j"|..., "n_up": k, "mode": "cr"|"clt", "prec": "fp32"|"fp64", "options": [[key, value], ...],
+        "what": ["neighbors", "apply", "lanczos"], "h": 0.0, "randJ": false}
+Compares the emulated CUDA path (kernel sources compiled for the host, tests/emu/cuda_emu.h) with the
+FP64 oracle on the same seeded inputs: neighbour indices bit-exactly, H.v in the norm-relative error,
+Lanczos alpha/beta (FP64) element-wise for the first steps.
+"""
+from __future__ import annotations
+
+import json
+import os
+import sys
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, HERE)
+
+from oracle import ftlm_oracle as fo  # noqa: E402
+from paper_2605_26261_b200 import workloads as W  # noqa: E402
+import emu_harness as E  # noqa: E402
+
+
+def workload(name):
+    if name.startswith("ring"):
+        j2 = name.endswith("j")
+        n = int(name[4:-1] if j2 else name[4:])
+        return W.ring(n, 1.0, 0.5 if j2 else None)
+    if name.startswith("square"):
+        a, b = name[6:].split("x")
+        return W.square(int(a), int(b))
+    if name.startswith("tri"):
+        a, b = name[3:].split("x")
+        return W.triangular(int(a), int(b))
+    if name == "icosahedron":
+        return W.icosahedron()
+    if name.startswith("rand"):                      # randN_E_seed : random graph, random J
+        n, e, s = (int(x) for x in name[4:].split("_"))
+        rng = np.random.default_rng(s)
+        pairs = set()
+        while len(pairs) < e:
+            a, b = rng.integers(0, n, 2)
+            if a != b:
+                pairs.add((min(a, b), max(a, b)))
+        pairs = sorted(pairs)
+        J = rng.uniform(0.5, 1.5, len(pairs))
+        return W._mk(name, n, pairs, J)
+    raise ValueError(name)
+
+
+def main():
+    spec = json.loads(sys.argv[1])
+    w = workload(spec["wl"])
+    n_up = spec["n_up"]
+    h = spec.get("h", 0.0)
+    mode, prec = spec.get("mode", "cr"), spec.get("prec", "fp64")
+    res = {"ok": True}
+    basis = fo.sector_basis(w.N, n_up)
+    D = basis.shape[0]
+    with E.EmuCtx(w, n_up, mode, prec, h=h, options=spec.get("options", ())) as c:
+        res["kernel"] = c.get("kernel")
+        res["dim"] = c.dim
+        assert c.dim == D
+        what = spec.get("what", ["neighbors", "apply"])
+        if "neighbors" in what:
+            nb = c.neighbors(0, D)
+            ref = fo.neighbor_indices(basis, w.bond_i, w.bond_j, np.arange(D))
+            bad = int(np.count_nonzero(nb != ref))
+            res["neighbors_bad"] = bad
+            if bad:
+                r, b = np.argwhere(nb != ref)[0]
+                res["first_bad"] = [int(r), int(b), int(nb[r, b]), int(ref[r, b])]
+                res["ok"] = False
+        if "apply" in what:
+            rng = np.random.default_rng(spec.get("seed", 1))
+            v = rng.standard_normal(D).astype(E.NDT[prec])
+            y = c.apply(v)
+            ref = fo.apply_H(basis, w.N, w.bond_i, w.bond_j, w.J, h, n_up, v.astype(np.float64))
+            den = np.linalg.norm(ref)
+            err = float(np.linalg.norm(y.astype(np.float64) - ref) / (den if den > 0 else 1.0))
+            res["hv_relerr"] = err
+            res["ok"] = res["ok"] and bool(np.isfinite(y).all()) and err <= (1e-5 if prec == "fp32" else 1e-12)
+        if "lanczos" in what:
+            m = min(spec.get("steps", 12), D)
+            out = c.lanczos(W.SEED_VECTORS, 1, m)
+            q1 = fo.start_vector(W.SEED_VECTORS, n_up, 0, D)
+            a, b = fo.lanczos(lambda x: fo.apply_H(basis, w.N, w.bond_i, w.bond_j, w.J, h, n_up, x), q1, m)[:2]
+            k = min(int(out["m_eff"][0]), len(a), 8)
+            tol = 1e-9 if prec == "fp64" else 2e-4
+            da = float(np.max(np.abs(out["alpha"][0][:k] - np.asarray(a)[:k]))) if k else 0.0
+            res["lanczos_dalpha"] = da
+            res["m_eff"] = int(out["m_eff"][0])
+            res["ok"] = res["ok"] and da <= tol
+    print(json.dumps(res))
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,81 @@
+"""Host-side execution of the CUDA kernel sources (`-m "not gpu"`).
+
+The library's .cu files are compiled as C++ against tests/emu/cuda_emu.h (every CUDA thread a fiber,
+real barrier / warp-collective rendezvous, guard pages behind every "device" allocation and behind the
+dynamic shared memory) and driven through the same C ABI as on the GPU.  Each case runs in a
+subprocess and is compared with the FP64 oracle: neighbour indices bit-exactly, H.v within the
+north_star tolerance, the first Lanczos coefficients.  This checks index arithmetic, plan tables,
+barrier placement and bounds of every kernel variant without a GPU; it says nothing about speed.
+"""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+RUN = os.path.join(ROOT, "tests", "emu", "run_case.py")
+
+K = {"row": 1, "tile": 2, "tml": 3}
+
+
+def run_case(spec, timeout=600):
+    p = subprocess.run([sys.executable, RUN, json.dumps(spec)], capture_output=True, text=True, timeout=timeout)
+    assert p.returncode == 0, f"emulated case died (rc={p.returncode}): {spec}\n{p.stderr[-2000:]}"
+    res = json.loads(p.stdout.strip().splitlines()[-1])
+    assert res["ok"], (spec, res)
+    return res
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _build():
+    sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
+    import build_emu
+    build_emu.build()
+
+
+@pytest.mark.parametrize("mode,prec", [("cr", "fp64"), ("clt", "fp32")])
+@pytest.mark.parametrize("kernel", ["row", "tile"])
+def test_emu_row_and_tile_kernels(kernel, mode, prec):
+    res = run_case({"wl": "ring12j", "n_up": 6, "mode": mode, "prec": prec, "options": [["kernel", K[kernel]]],
+                    "what": ["neighbors", "apply", "lanczos"]})
+    assert res["kernel"] == K[kernel]
+
+
+@pytest.mark.parametrize("wl,n_up,w,m,mode,prec", [
+    ("ring14j", 7, 5, 3, "cr", "fp64"),
+    ("ring16j", 8, 6, 4, "clt", "fp32"),
+    ("ring16j", 5, 7, 5, "cr", "fp32"),
+    ("rand14_30_3", 7, 5, 5, "clt", "fp64"),
+    ("tri4x4", 8, 8, 4, "cr", "fp32"),
+])
+def test_emu_tml_kernel(wl, n_up, w, m, mode, prec):
+    res = run_case({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec,
+                    "options": [["tml_low_bits", w], ["tml_mid_bits", m], ["kernel", K["tml"]]],
+                    "what": ["neighbors", "apply", "lanczos"]})
+    assert res["kernel"] == K["tml"]
+
+
+def test_emu_guard_pages_catch_overrun():
+    """The checker itself: a read past the end of an emulated device buffer must kill the process."""
+    code = ("import sys; sys.path.insert(0, %r); import numpy as np, ctypes as C, emu_harness as E; L = E.lib();"
+            "p = C.c_void_p(); L.cudaMalloc = None" % os.path.join(ROOT, "tests", "emu"))
+    # cudaMalloc is a C++ symbol of the emulation layer; exercise it through a tiny kernel instead:
+    # apply_H with a y buffer one element short must fault on the last store.
+    code = ("import sys; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+            "import numpy as np, ctypes as C, emu_harness as E\n"
+            "from paper_2605_26261_b200 import workloads as W\n"
+            "w = W.ring(10)\n"
+            "c = E.EmuCtx(w, 5, 'cr', 'fp64', options=[('kernel', 1)])\n"
+            "import mmap\n"
+            "m = mmap.mmap(-1, 8192)\n"
+            "buf = (C.c_char * 8192).from_buffer(m)\n"
+            "base = C.addressof(buf)\n"
+            "C.CDLL(None).mprotect(C.c_void_p(base + 4096), C.c_size_t(4096), C.c_int(0))\n"
+            "v = np.ones(c.dim)\n"
+            "y_addr = base + 4096 - 8 * (c.dim - 1)\n"      # one element short of the guard page
+            "E._check(E.lib().ftlm_apply_H(c.ctx, C.c_void_p(v.ctypes.data), C.c_void_p(y_addr), C.c_void_p(0)))\n"
+            "print('survived')\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=120)
+    assert p.returncode != 0 and "survived" not in p.stdout
