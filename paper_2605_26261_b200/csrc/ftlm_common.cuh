@@ -52,6 +52,7 @@ struct BondDev {          // one bond as the kernels see it
 // (DESIGN.md section 6).
 struct TilePlan;
 struct TmlPlan;
+struct PassBSet;
 
 struct ftlm_ctx {
   int N = 0, nb = 0, N_up = 0, mode = 0, prec = 0, device = 0;
@@ -81,6 +82,9 @@ struct ftlm_ctx {
   TilePlan* tile = nullptr;
   // three-level tile plan (ftlm_tml.cu)
   TmlPlan* tml = nullptr;
+  // PASS-B windows for the bonds among the top label bits (ftlm_passb.cu); owned together with `tml`
+  PassBSet* passb = nullptr;
+  int use_passb = 1;               // option "passb": 0 keeps every top-top bond in the TML kernel
 
   // chain workspace
   void* q[3] = {nullptr, nullptr, nullptr};
@@ -113,6 +117,18 @@ void ftlm_tml_plan_destroy(ftlm_ctx* c);
 int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key);
 int ftlm_launch_hv_tml(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, int batch, cudaStream_t s);
 int ftlm_launch_neighbors_tml(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
+
+// PASS-B (ftlm_passb.cu).  `tt` lists the bonds whose two sites lie at positions >= mw (candidate
+// top-top bonds) as indices into c->bonds; on return window_of[k] is the PASS-B window that took
+// tt[k] or -1 if the bond stays in the TML kernel.  FTLM_OK with c->passb == nullptr if no window pays.
+int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& tt, std::vector<int>& window_of);
+void ftlm_passb_plan_destroy(ftlm_ctx* c);
+int ftlm_passb_windows(const ftlm_ctx* c);
+void ftlm_passb_window_geometry(const ftlm_ctx* c, int window, int* lo, int* s);
+int64_t ftlm_passb_info(const ftlm_ctx* c, const char* key);
+// y += sum over the windows' bonds of (J_b/2)(P_b - 1) v.  fused: the last window also accumulates the
+// three FP64 sums over the final y and advances the chain state.
+int ftlm_launch_passb(ftlm_ctx* c, const void* v, void* y, int fused, cudaStream_t s);
 
 // ---- device helpers ---------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -285,6 +285,7 @@ extern "C" int64_t ftlm_table_bytes(const ftlm_ctx* c) {
 int ftlm_effective_kernel(const ftlm_ctx* c) {
   if (c->kernel == FTLM_KERNEL_ROW) return FTLM_KERNEL_ROW;
   if (c->kernel == FTLM_KERNEL_TML && c->tml) return FTLM_KERNEL_TML;
+  if (c->kernel == FTLM_KERNEL_AUTO && c->tml && c->dim >= (1 << 20)) return FTLM_KERNEL_TML;
   if (c->tile && (c->kernel == FTLM_KERNEL_TILE || c->dim >= (1 << 20))) return FTLM_KERNEL_TILE;
   return FTLM_KERNEL_ROW;                    // AUTO: small sectors are launch-bound, ROW is simpler
 }
@@ -318,6 +319,23 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     return rc;
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
+  if (!strcmp(key, "passb") || !strcmp(key, "tml_split")) {
+    // "passb": 0/1;  "tml_split": w | m << 8 (both at once; 0 = auto).  Rebuilds the TML / PASS-B plans.
+    const int old_pb = c->use_passb, old_w = c->tml_low_bits, old_m = c->tml_mid_bits;
+    if (!strcmp(key, "passb")) c->use_passb = value ? 1 : 0;
+    else {
+      if (value < 0 || (value & 0xff) > 16 || (value >> 8) > 16) { ftlm_set_error("tml_split must be w | m << 8"); return FTLM_EINVAL; }
+      c->tml_low_bits = (int)(value & 0xff); c->tml_mid_bits = (int)(value >> 8);
+    }
+    CK(cudaSetDevice(c->device));
+    ftlm_tml_plan_destroy(c);
+    int rc = ftlm_tml_plan_create(c);
+    if (rc != FTLM_OK) {
+      c->use_passb = old_pb; c->tml_low_bits = old_w; c->tml_mid_bits = old_m;
+      ftlm_tml_plan_destroy(c); ftlm_tml_plan_create(c);
+    }
+    return rc;
+  }
   ftlm_set_error("ftlm_set_option: unknown key '%s'", key);
   return FTLM_EINVAL;
 }
@@ -327,6 +345,8 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "kernel")) return ftlm_effective_kernel(c);
   if (!strcmp(key, "low_bits")) return c->low_bits;
   if (!strcmp(key, "graph")) return c->use_graph;
+  if (!strcmp(key, "passb")) return c->use_passb;
+  if (!strncmp(key, "passb_", 6)) return ftlm_passb_info(c, key);
   if (!strcmp(key, "sm_count")) return c->sm_count;
   if (!strncmp(key, "tml_", 4)) return ftlm_tml_info(c, key);
   return -1;
@@ -346,7 +366,13 @@ extern "C" int ftlm_clt_read(ftlm_ctx* c, int64_t b0, int64_t nb, uint32_t* h_ma
 // ---- H.v ---------------------------------------------------------------------------------------
 static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
   const int k = ftlm_effective_kernel(c);
-  if (k == FTLM_KERNEL_TML) return ftlm_launch_hv_tml(c, v, qp, y, fused, 1, s);
+  if (k == FTLM_KERNEL_TML) {
+    // two-pass step when PASS-B windows exist: the TML pass leaves the sums and the finish to PASS-B
+    const bool pb = c->passb != nullptr;
+    int rc = ftlm_launch_hv_tml(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, 1, s);
+    if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, s);
+    return rc;
+  }
   if (k == FTLM_KERNEL_TILE) return ftlm_launch_hv_tile(c, v, qp, y, fused, s);
   return ftlm_launch_hv_row(c, v, qp, y, fused, s);
 }

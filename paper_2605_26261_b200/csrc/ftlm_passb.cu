@@ -1,0 +1,458 @@
+// PASS-B kernels - bonds among the top label bits, streamed.
+//
+// For a bond whose two sites lie in a window S = [lo, lo+s) of high label positions the swap
+// P_b (Eq. 12-14 at s = 1/2: y_t += (J_b/2)(v[P_b n_t] - v[n_t])) maps the contiguous run of rows
+// (F, u, *) onto the run (F, u', *), u' = u with the two window bits exchanged, element by element
+// (same low part, same offset x inside the run).  One work item = one (F, popc(u)) class and one
+// chunk of X = 32 k run offsets:
+//   phase 1: the C(s, p_S) run chunks v[start(F,u) + x0 .. + X) are loaded into shared memory,
+//            tile[slot(u) * X + x]  (coalesced, every element of v read once per window);
+//   phase 2: one warp per u adds, for its X rows, sum_b (J_b/2) (tile[slot(u'_b)][x] - tile[slot(u)][x])
+//            to y (coalesced read-modify-write).  The antiparallel bonds of u and the slots of the
+//            u'_b come from a precomputed row of 32 entries per u (one coalesced load, then
+//            warp-broadcast), so the inner loop is one shuffle, one shared-memory read and one FMA.
+// Run starts are sector indices of the first label of a run, by CR or CLT (ftlm_passb.cuh).
+// The last window carries the fused Lanczos reductions (it writes the final y): per-item FP64
+// partial sums in a buffer indexed by item, added in fixed order by the last CTA (bit-reproducible).
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+#include "ftlm_passb.cuh"
+
+#define PASSB_MAX_BONDS 32          // one neighbour entry per lane
+#define PASSB_MAX_S 12
+#define PASSB_THREADS 1024
+#define PASSB_END 0xFFFFFFFFu
+
+template <typename R>
+struct PassBParams {
+  int N, K, lo, s, f, ngroups;
+  uint32_t nitems;
+  int64_t dim;
+  const uint64_t* binom;            // [(N+1)*(K+1)] global
+  const uint2* clt;
+  const uint16_t* ustate;           // [2^s]: window words grouped by popcount, ascending inside a group
+  const int* koff;                  // [s+2]: first slot of popcount class p in ustate
+  const uint32_t* nbr;              // [2^s][32], indexed by u: slot(u') | bond << 16, PASSB_END after the last
+  const uint32_t* grp_first;        // [ngroups+1]: first item of group g = F*(s+1) + p_S
+  double* partials;                 // [3][nitems]
+  unsigned int* counter;            // [0] item counter, [1] ticket
+  ChainState* st;
+  int xk[PASSB_MAX_S + 1];          // X/32 per popcount class
+  int max_conf;                     // largest C(s, p_S) among non-empty classes
+  R Jh[PASSB_MAX_BONDS];
+};
+
+struct PassBWindow {
+  int lo = 0, s = 0, f = 0, ngroups = 0, max_conf = 0;
+  uint32_t nitems = 0;
+  int xk[PASSB_MAX_S + 1] = {0};
+  size_t smem = 0;
+  std::vector<int> bonds;           // indices into ctx->bonds
+  std::vector<double> Jh;
+  uint16_t* d_ustate = nullptr;
+  int* d_koff = nullptr;
+  uint32_t* d_nbr = nullptr;
+  uint32_t* d_grp_first = nullptr;
+  double* d_partials = nullptr;
+  unsigned int* d_counter = nullptr;
+};
+
+struct PassBSet {
+  std::vector<PassBWindow> win;
+};
+
+namespace {
+
+__host__ __device__ inline size_t passb_smem_bytes(int N, int K, int max_conf, int max_rows, int esz) {
+  size_t o = 0;
+  o += ((size_t)(N + 1) * (K + 1) * 8 + 15) & ~(size_t)15;      // binom
+  o += ((size_t)max_conf * 8 + 15) & ~(size_t)15;               // run starts
+  o += (size_t)32 * 3 * 8;                                      // reduction scratch
+  o += (size_t)max_rows * esz;                                  // tile: max over classes of C(s,p) * X
+  return o;
+}
+
+template <typename R, int MODE, bool FUSED>
+__global__ void __launch_bounds__(PASSB_THREADS, 1)
+passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, R* __restrict__ y) {
+  FTLM_DYN_SMEM(smem);
+  __shared__ unsigned int s_item;
+  __shared__ bool s_last;
+  if (FUSED && p.st->done) return;
+  const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
+  const int K1 = p.K + 1;
+  uint64_t* s_binom = (uint64_t*)smem;
+  size_t o = ((size_t)(p.N + 1) * K1 * 8 + 15) & ~(size_t)15;
+  uint64_t* s_start = (uint64_t*)(smem + o);
+  o += ((size_t)p.max_conf * 8 + 15) & ~(size_t)15;
+  double* s_red = (double*)(smem + o);
+  o += (size_t)32 * 3 * 8;
+  R* tile = (R*)(smem + o);
+  for (int k = tid; k < (p.N + 1) * K1; k += NT) s_binom[k] = p.binom[k];
+  int cur_group = -1;
+  const int s1 = p.s + 1;
+
+  for (;;) {
+    __syncthreads();                                   // previous item done: tile, starts reusable
+    if (tid == 0) s_item = atomicAdd(&p.counter[0], 1u);
+    __syncthreads();
+    const uint32_t item = s_item;
+    if (item >= p.nitems) break;
+    // group of this item: last g with grp_first[g] <= item (uniform binary search)
+    int g0 = 0, g1 = p.ngroups;
+    while (g1 - g0 > 1) {
+      const int gm = (g0 + g1) >> 1;
+      if (__ldg(&p.grp_first[gm]) <= item) g0 = gm; else g1 = gm;
+    }
+    const int g = g0;
+    const uint32_t F = (uint32_t)(g / s1);
+    const int pS = g - (int)F * s1;
+    const int kP = p.K - __popc(F) - pS;                // in [0, lo] by construction of the groups
+    const int c0 = __ldg(&p.koff[pS]);
+    const int nconf = __ldg(&p.koff[pS + 1]) - c0;
+    const int XK = p.xk[pS];
+    const int X = 32 * XK;
+    const uint64_t RL = s_binom[p.lo * K1 + kP];        // run length C(lo, kP)
+    const uint64_t x0 = (uint64_t)(item - __ldg(&p.grp_first[g])) * (uint64_t)X;
+    if (g != cur_group) {                               // (uniform) run starts of this class
+      for (int sl = tid; sl < nconf; sl += NT) {
+        const uint64_t hi = ((uint64_t)F << p.s) | (uint64_t)__ldg(&p.ustate[c0 + sl]);
+        s_start[sl] = passb_run_start<MODE>(hi, p.lo, kP, p.K, s_binom, p.clt);
+      }
+      cur_group = g;
+      __syncthreads();
+    }
+    const uint64_t left = RL - x0;                      // rows of the run at or after x0 (> 0)
+    const int nx = left < (uint64_t)X ? (int)left : X;  // valid offsets in this chunk
+    // ---- phase 1: stage the run chunks ----------------------------------------------------------
+    for (int sl = warp; sl < nconf; sl += NW) {
+      const R* src = v + s_start[sl] + x0;
+      R* dst = tile + (size_t)sl * X;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int x = lane + 32 * k;
+        if (k < XK && x < nx) dst[x] = __ldg(&src[x]);
+      }
+    }
+    __syncthreads();
+    // ---- phase 2: one warp per window word ------------------------------------------------------
+    double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
+    for (int sl = warp; sl < nconf; sl += NW) {
+      const uint32_t u = __ldg(&p.ustate[c0 + sl]);
+      const uint32_t ent = __ldg(&p.nbr[(size_t)u * 32 + lane]);
+      const int cnt = __popc(__ballot_sync(0xffffffffu, ent != PASSB_END));
+      const R* row = tile + (size_t)sl * X;
+      R own[4], acc[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int x = lane + 32 * k;
+        own[k] = (k < XK && x < nx) ? row[x] : (R)0;
+        acc[k] = (R)0;
+      }
+      R sumJ = (R)0;
+      for (int e = 0; e < cnt; ++e) {
+        const uint32_t en = __shfl_sync(0xffffffffu, ent, e);
+        const R J = p.Jh[en >> 16];
+        const R* nrow = tile + (size_t)(en & 0xffffu) * X;
+        sumJ += J;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const int x = lane + 32 * k;
+          if (k < XK && x < nx) acc[k] += J * nrow[x];
+        }
+      }
+      R* yrow = y + s_start[sl] + x0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int x = lane + 32 * k;
+        if (k < XK && x < nx) {
+          const R yn = yrow[x] + (acc[k] - sumJ * own[k]);
+          yrow[x] = yn;
+          if (FUSED) {
+            s_qy += (double)own[k] * (double)yn;
+            s_yy += (double)yn * (double)yn;
+            s_qq += (double)own[k] * (double)own[k];
+          }
+        }
+      }
+    }
+    if (FUSED) {                                        // deterministic per-item partial sums
+      const double a = warp_sum(s_qy), b = warp_sum(s_yy), c = warp_sum(s_qq);
+      if (lane == 0) { s_red[warp * 3] = a; s_red[warp * 3 + 1] = b; s_red[warp * 3 + 2] = c; }
+      __syncthreads();
+      if (tid < 3) {
+        double s = 0.0;
+        for (int wv = 0; wv < NW; ++wv) s += s_red[wv * 3 + tid];
+        p.partials[(size_t)tid * p.nitems + item] = s;
+      }
+    }
+  }
+  // ---- grid-wide finish: the last CTA resets the counters and (fused) advances the chain ----------
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    s_last = (atomicAdd(&p.counter[1], 1u) == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (tid == 0) { p.counter[0] = 0; p.counter[1] = 0; }
+  if (!FUSED) return;
+  double tot[3];
+  for (int q = 0; q < 3; ++q) {                         // fixed assignment and order
+    double a = 0.0;
+    for (uint32_t k = tid; k < p.nitems; k += NT) a += p.partials[(size_t)q * p.nitems + k];
+    a = warp_sum(a);
+    __syncthreads();
+    if (lane == 0) s_red[warp] = a;
+    __syncthreads();
+    double s = 0.0;
+    if (tid == 0) for (int wv = 0; wv < NW; ++wv) s += s_red[wv];
+    tot[q] = s;
+  }
+  if (tid == 0) {
+    ChainState* st = p.st;
+    const double a = tot[0], b = tot[1], c = tot[2];
+    const int j = st->step;
+    const double alpha = c > 0.0 ? a / c : 0.0;
+    double b2 = c > 0.0 ? b - a * a / c : 0.0;
+    if (!(b2 > 0.0)) b2 = 0.0;
+    const double beta = sqrt(b2);
+    st->alpha[j] = alpha;
+    st->beta[j] = beta;
+    double sc = st->scale;
+    sc = fmax(sc, fmax(fabs(alpha), beta));
+    st->scale = sc;
+    st->step = j + 1;
+    st->a = alpha;
+    st->inv_b = beta > 0.0 ? 1.0 / beta : 0.0;
+    st->beta_prev = beta;
+    if (j + 1 >= st->limit || beta <= st->tol * sc) { st->done = 1; st->inv_b = 0.0; }
+  }
+}
+
+uint64_t binom_b(int n, int k) {
+  if (k < 0 || k > n) return 0;
+  if (k > n - k) k = n - k;
+  unsigned __int128 r = 1;
+  for (int i = 1; i <= k; ++i) r = r * (unsigned)(n - k + i) / (unsigned)i;
+  return (uint64_t)r;
+}
+
+}  // namespace
+
+// ---- host: window selection, tables, launch -----------------------------------------------------
+void ftlm_passb_plan_destroy(ftlm_ctx* c) {
+  PassBSet* S = c->passb;
+  if (!S) return;
+  for (PassBWindow& w : S->win) {
+    cudaFree(w.d_ustate); cudaFree(w.d_koff); cudaFree(w.d_nbr); cudaFree(w.d_grp_first);
+    cudaFree(w.d_partials); cudaFree(w.d_counter);
+  }
+  delete S;
+  c->passb = nullptr;
+}
+
+int ftlm_passb_windows(const ftlm_ctx* c) { return c->passb ? (int)c->passb->win.size() : 0; }
+
+void ftlm_passb_window_geometry(const ftlm_ctx* c, int window, int* lo, int* s) {
+  const PassBWindow& w = c->passb->win[(size_t)window];
+  *lo = w.lo; *s = w.s;
+}
+
+int64_t ftlm_passb_info(const ftlm_ctx* c, const char* key) {
+  const PassBSet* S = c->passb;
+  if (!strcmp(key, "passb_windows")) return S ? (int64_t)S->win.size() : 0;
+  if (!S || S->win.empty()) return -1;
+  if (!strcmp(key, "passb_bonds")) { int64_t n = 0; for (const PassBWindow& w : S->win) n += (int64_t)w.bonds.size(); return n; }
+  if (!strcmp(key, "passb_lo")) return S->win[0].lo;
+  if (!strcmp(key, "passb_s")) return S->win[0].s;
+  if (!strcmp(key, "passb_items")) return S->win[0].nitems;
+  if (!strcmp(key, "passb_smem")) return (int64_t)S->win[0].smem;
+  return -1;
+}
+
+// Fill the host-side geometry of a window (classes, chunk sizes, item groups).  false if it cannot run
+// (a popcount class does not fit shared memory even at X = 32, or the item count overflows 32 bits).
+static bool passb_geometry(const ftlm_ctx* c, PassBWindow& w, std::vector<uint32_t>& grp_first) {
+  const int N = c->N, K = c->N_up, esz = (int)ftlm_elem_size(c);
+  w.f = N - w.lo - w.s;
+  if (w.f < 0 || w.f > 20 || w.s < 2 || w.s > PASSB_MAX_S) return false;
+  const int s1 = w.s + 1;
+  w.ngroups = (1 << w.f) * s1;
+  // largest class that actually occurs
+  std::vector<char> used((size_t)s1, 0);
+  for (uint32_t F = 0; F < (1u << w.f); ++F)
+    for (int p = 0; p <= w.s; ++p) {
+      const int kP = K - __builtin_popcount(F) - p;
+      if (kP >= 0 && kP <= w.lo) used[(size_t)p] = 1;
+    }
+  w.max_conf = 0;
+  for (int p = 0; p <= w.s; ++p) if (used[(size_t)p]) w.max_conf = std::max(w.max_conf, (int)binom_b(w.s, p));
+  if (w.max_conf == 0) return false;
+  const size_t fixed = passb_smem_bytes(N, K, w.max_conf, 0, esz);
+  const size_t cap = 227 * 1024 - 1024;
+  if (fixed >= cap) return false;
+  const size_t budget = cap - fixed;
+  int max_rows = 0;
+  for (int p = 0; p <= w.s; ++p) {
+    w.xk[p] = 0;
+    if (!used[(size_t)p]) continue;
+    const size_t per32 = (size_t)binom_b(w.s, p) * 32 * (size_t)esz;
+    int xk = (int)std::min<size_t>(4, budget / per32);
+    if (xk < 1) return false;
+    w.xk[p] = xk;
+    max_rows = std::max(max_rows, (int)binom_b(w.s, p) * 32 * xk);
+  }
+  w.smem = passb_smem_bytes(N, K, w.max_conf, max_rows, esz);
+  grp_first.assign((size_t)w.ngroups + 1, 0);
+  uint64_t total = 0;
+  for (uint32_t F = 0; F < (1u << w.f); ++F)
+    for (int p = 0; p <= w.s; ++p) {
+      grp_first[(size_t)F * s1 + p] = (uint32_t)total;
+      const int kP = K - __builtin_popcount(F) - p;
+      if (kP < 0 || kP > w.lo) continue;
+      const uint64_t RL = binom_b(w.lo, kP), X = 32ull * (uint64_t)w.xk[p];
+      total += (RL + X - 1) / X;
+      if (total >= 0xFFFFFFF0ull) return false;
+    }
+  grp_first[(size_t)w.ngroups] = (uint32_t)total;
+  w.nitems = (uint32_t)total;
+  return total > 0;
+}
+
+int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& tt, std::vector<int>& window_of) {
+  window_of.assign(tt.size(), -1);
+  c->passb = nullptr;
+  if (!c->use_passb || tt.empty()) return FTLM_OK;
+  const int N = c->N;
+  const int smax = ftlm_elem_size(c) == 4 ? PASSB_MAX_S : PASSB_MAX_S - 1;
+  const int MIN_GAIN = 3;                          // a window costs one more stream of v and y
+  PassBSet* S = new PassBSet();
+  std::vector<std::vector<uint32_t>> groups;
+  for (;;) {
+    int best_lo = -1, best_s = 0, best_cnt = 0;
+    for (int lo = mw; lo + 2 <= N; ++lo) {
+      const int s = std::min(smax, N - lo);
+      int cnt = 0;
+      for (size_t k = 0; k < tt.size(); ++k) {
+        if (window_of[k] >= 0) continue;
+        const BondDev& d = c->bonds[(size_t)tt[k]];
+        if (d.i >= lo && d.j < lo + s) ++cnt;
+      }
+      cnt = std::min(cnt, PASSB_MAX_BONDS);
+      if (cnt > best_cnt) { best_cnt = cnt; best_lo = lo; best_s = s; }
+    }
+    if (best_cnt < MIN_GAIN) break;
+    PassBWindow w;
+    w.lo = best_lo; w.s = best_s;
+    // shrink the window to the sites its bonds use (shorter windows have smaller classes, larger X)
+    int hi_used = 0;
+    for (size_t k = 0; k < tt.size(); ++k) {
+      if (window_of[k] >= 0) continue;
+      const BondDev& d = c->bonds[(size_t)tt[k]];
+      if (d.i >= w.lo && d.j < w.lo + w.s) hi_used = std::max(hi_used, d.j);
+    }
+    if (w.lo + w.s < N) w.s = std::max(2, hi_used - w.lo + 1);   // only if something stays frozen above anyway
+    int lo_used = N;
+    for (size_t k = 0; k < tt.size(); ++k) {
+      if (window_of[k] >= 0) continue;
+      const BondDev& d = c->bonds[(size_t)tt[k]];
+      if (d.i >= w.lo && d.j < w.lo + w.s) lo_used = std::min(lo_used, d.i);
+    }
+    if (lo_used > w.lo && lo_used < N && w.s - (lo_used - w.lo) >= 2) { w.s -= lo_used - w.lo; w.lo = lo_used; }   // longer runs
+    std::vector<uint32_t> gf;
+    if (!passb_geometry(c, w, gf)) break;
+    const int widx = (int)S->win.size();
+    for (size_t k = 0; k < tt.size() && (int)w.bonds.size() < PASSB_MAX_BONDS; ++k) {
+      if (window_of[k] >= 0) continue;
+      const BondDev& d = c->bonds[(size_t)tt[k]];
+      if (d.i >= w.lo && d.j < w.lo + w.s) { window_of[k] = widx; w.bonds.push_back(tt[k]); w.Jh.push_back(d.Jh); }
+    }
+    S->win.push_back(w);
+    groups.push_back(gf);
+  }
+  if (S->win.empty()) { delete S; return FTLM_OK; }
+  c->passb = S;
+  // ---- tables + upload --------------------------------------------------------------------------
+  for (size_t wi = 0; wi < S->win.size(); ++wi) {
+    PassBWindow& w = S->win[wi];
+    const int nU = 1 << w.s;
+    std::vector<int> koff((size_t)w.s + 2, 0);
+    for (int p = 0; p <= w.s; ++p) koff[(size_t)p + 1] = koff[(size_t)p] + (int)binom_b(w.s, p);
+    std::vector<uint16_t> ustate((size_t)nU), slot((size_t)nU);
+    std::vector<int> fill(koff.begin(), koff.end() - 1);
+    for (int u = 0; u < nU; ++u) {                              // ascending u inside each popcount class
+      const int p = __builtin_popcount((unsigned)u);
+      slot[(size_t)u] = (uint16_t)(fill[(size_t)p] - koff[(size_t)p]);
+      ustate[(size_t)fill[(size_t)p]++] = (uint16_t)u;
+    }
+    std::vector<uint32_t> nbr((size_t)nU * 32, PASSB_END);
+    for (int u = 0; u < nU; ++u) {
+      int n = 0;
+      for (size_t e = 0; e < w.bonds.size(); ++e) {
+        const BondDev& d = c->bonds[(size_t)w.bonds[e]];
+        const uint32_t mk = (uint32_t)(d.mask >> w.lo), x = (uint32_t)u & mk;
+        if (x != 0 && x != mk) nbr[(size_t)u * 32 + (size_t)n++] = (uint32_t)slot[(size_t)((uint32_t)u ^ mk)] | ((uint32_t)e << 16);
+      }
+    }
+    auto up = [&](void** d, const void* h, size_t bytes) -> bool {
+      if (cudaMalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
+      if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
+      return true;
+    };
+    const size_t pbytes = (size_t)w.nitems * 24;
+    bool ok = up((void**)&w.d_ustate, ustate.data(), ustate.size() * 2) && up((void**)&w.d_koff, koff.data(), koff.size() * 4) &&
+              up((void**)&w.d_nbr, nbr.data(), nbr.size() * 4) &&
+              up((void**)&w.d_grp_first, groups[wi].data(), groups[wi].size() * 4) &&
+              up((void**)&w.d_partials, nullptr, pbytes) && up((void**)&w.d_counter, nullptr, 16);
+    if (ok) ok = cudaMemset(w.d_partials, 0, pbytes) == cudaSuccess && cudaMemset(w.d_counter, 0, 16) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); ftlm_passb_plan_destroy(c); ftlm_set_error("PASS-B: table upload failed"); return FTLM_ENOMEM; }
+  }
+  return FTLM_OK;
+}
+
+template <typename R, int MODE>
+static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, int fused, cudaStream_t s) {
+  PassBParams<R> p;
+  memset(&p, 0, sizeof(p));
+  p.N = c->N; p.K = c->N_up; p.lo = w.lo; p.s = w.s; p.f = w.f; p.ngroups = w.ngroups; p.nitems = w.nitems;
+  p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.ustate = w.d_ustate; p.koff = w.d_koff;
+  p.nbr = w.d_nbr; p.grp_first = w.d_grp_first; p.partials = w.d_partials; p.counter = w.d_counter;
+  p.st = c->d_state; p.max_conf = w.max_conf;
+  for (int k = 0; k <= PASSB_MAX_S; ++k) p.xk[k] = w.xk[k];
+  for (size_t e = 0; e < w.Jh.size(); ++e) p.Jh[e] = (R)w.Jh[e];
+  int grid = c->sm_count;
+  if ((uint32_t)grid > w.nitems) grid = (int)w.nitems;
+  if (fused) {
+    auto k = passb_kernel<R, MODE, true>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
+    FTLM_LAUNCH(k, grid, PASSB_THREADS, w.smem, s, p, (const R*)v, (R*)y);
+  } else {
+    auto k = passb_kernel<R, MODE, false>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
+    FTLM_LAUNCH(k, grid, PASSB_THREADS, w.smem, s, p, (const R*)v, (R*)y);
+  }
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+
+int ftlm_launch_passb(ftlm_ctx* c, const void* v, void* y, int fused, cudaStream_t s) {
+  PassBSet* S = c->passb;
+  if (!S) return FTLM_OK;
+  for (size_t wi = 0; wi < S->win.size(); ++wi) {
+    PassBWindow& w = S->win[wi];
+    const int fz = (fused && wi + 1 == S->win.size()) ? 1 : 0;
+    int rc;
+    if (c->prec == FTLM_FP32)
+      rc = c->mode == FTLM_INDEX_CLT ? launch_window<float, FTLM_INDEX_CLT>(c, w, v, y, fz, s)
+                                     : launch_window<float, FTLM_INDEX_CR>(c, w, v, y, fz, s);
+    else
+      rc = c->mode == FTLM_INDEX_CLT ? launch_window<double, FTLM_INDEX_CLT>(c, w, v, y, fz, s)
+                                     : launch_window<double, FTLM_INDEX_CR>(c, w, v, y, fz, s);
+    if (rc != FTLM_OK) return rc;
+  }
+  return FTLM_OK;
+}

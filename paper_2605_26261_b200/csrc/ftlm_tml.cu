@@ -33,7 +33,7 @@
 #include <type_traits>
 #include <vector>
 
-#include "ftlm_common.cuh"
+#include "ftlm_passb.cuh"
 
 #define TML_MAX_LL 32
 #define TML_MAX_TT 64
@@ -63,6 +63,7 @@ struct TmlParams {
   R ll_J[TML_MAX_LL];
   uint32_t tt_mask[TML_MAX_TT]; double tt_J[TML_MAX_TT];
   uint8_t ts_site[TML_MAX_TS];
+  int pb_lo[8];                       // low end of PASS-B window k (neighbour test hook only)
 };
 
 struct TmlPlan {
@@ -208,7 +209,10 @@ __device__ __forceinline__ const void* addr_u32(const void* base, uint32_t idx, 
 #endif
 }
 
-template <typename R, int B, int MODE, bool FUSED>
+// FUSED: 0 = y = H v;  1 = fused Lanczos pass (subtract beta q_prev, FP64 sums, finish);
+//        2 = first pass of a two-pass step: subtract beta q_prev only - PASS-B, which writes the final y,
+//            carries the sums and the finish.
+template <typename R, int B, int MODE, int FUSED>
 __global__ void __launch_bounds__(B >= 4 ? 512 : 1024, 1)
 hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, const R* __restrict__ qprev_,
               R* __restrict__ y_) {
@@ -332,6 +336,7 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
     double s_qy[B], s_yy[B], s_qq[B];
 #pragma unroll
     for (int b = 0; b < B; ++b) { s_qy[b] = 0.0; s_yy[b] = 0.0; s_qq[b] = 0.0; }
+    (void)s_qy; (void)s_yy; (void)s_qq;
     for (int it = it0 + warp; it < it1; it += NW) {
       const uint32_t item = __ldg(&p.items[it]);
       const uint32_t M = item & 0xffffu;
@@ -508,16 +513,18 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
 #pragma unroll
             for (int b = 0; b < B; ++b) {
               acc.x[b] -= bprev.x[b] * qp.x[b];
-              s_qy[b] += (double)own.x[b] * (double)acc.x[b];
-              s_yy[b] += (double)acc.x[b] * (double)acc.x[b];
-              s_qq[b] += (double)own.x[b] * (double)own.x[b];
+              if (FUSED == 1) {
+                s_qy[b] += (double)own.x[b] * (double)acc.x[b];
+                s_yy[b] += (double)acc.x[b] * (double)acc.x[b];
+                s_qq[b] += (double)own.x[b] * (double)own.x[b];
+              }
             }
           }
           vec_stcs(y + g, acc);
         }
       }
     }
-    if (FUSED) {                                        // deterministic per-tile partial sums
+    if (FUSED == 1) {                                   // deterministic per-tile partial sums
 #pragma unroll
       for (int b = 0; b < B; ++b) {
         const double a = warp_sum(s_qy[b]), bb = warp_sum(s_yy[b]), c = warp_sum(s_qq[b]);
@@ -541,7 +548,7 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
   if (!s_last) return;
   __threadfence();
   if (tid == 0) { p.counter[0] = 0; p.counter[1] = 0; }
-  if (!FUSED) return;
+  if (FUSED != 1) return;
   for (int q = 0; q < 3 * B; ++q) {                       // fixed assignment and order
     double a = 0.0;
     for (uint32_t k = tid; k < p.nT; k += NT) a += p.partials[(size_t)q * p.nT + k];
@@ -629,6 +636,16 @@ neighbors_tml_kernel(const __grid_constant__ TmlParams<R> p, const BondDev* __re
           case 2: idx = (int64_t)base + coloff[kT * nM + (M ^ (1u << ml[e].b))] +                    // ML
                         (int)(fl[ml[e].a * nL + Lidx] & 0x7fffu); break;
           case 3: idx = (int64_t)tml_base<MODE>(T ^ p.tt_mask[e], p.mw, p.K, p.binom, p.clt) + cb + lr; break;  // TT
+          case 6: {                                      // PASS-B window e: run start of the swapped window word + offset in the run
+            const int lo = p.pb_lo[e];
+            const uint64_t hi = n >> lo, low = n & ((1ull << lo) - 1ull);
+            const int kP = p.K - __popcll((unsigned long long)hi);
+            const uint64_t x = passb_low_rank(low, p.K, p.binom);
+            const uint64_t own = passb_run_start<MODE>(hi, lo, kP, p.K, p.binom, p.clt);
+            idx = (int64_t)(passb_run_start<MODE>(hi ^ (mk >> lo), lo, kP, p.K, p.binom, p.clt) + x);
+            if (own + x != tr) idx = -4;                 // the run arithmetic must reproduce the row's own index
+            break;
+          }
           default: {                                     // TM / TL
             const TmlSEnt d = bclass[b] == 4 ? tm[e] : tl[e];
             const uint32_t bit = 1u << p.ts_site[d.b];
@@ -673,6 +690,7 @@ void fill_params(const ftlm_ctx* c, const TmlPlan* t, TmlParams<R>& p, int batch
   for (int k = 0; k < t->n_ll4; ++k) p.ll_J[k] = (R)t->ll_J[(size_t)k];
   for (int k = 0; k < t->n_tt; ++k) { p.tt_mask[k] = t->tt_mask[(size_t)k]; p.tt_J[k] = t->tt_J[(size_t)k]; }
   for (int k = 0; k < t->n_ts; ++k) p.ts_site[k] = t->ts_site[(size_t)k];
+  for (int k = 0; k < 8 && k < ftlm_passb_windows(c); ++k) { int lo, sz; ftlm_passb_window_geometry(c, k, &lo, &sz); p.pb_lo[k] = lo; }
   (void)batch;
 }
 
@@ -700,17 +718,21 @@ int launch_tml(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, c
   TmlPlan* t = c->tml;
   const TmlLaunchCfg cfg = tml_config(c, t, B);
   if (cfg.smem == 0) { ftlm_set_error("TML: batch %d does not fit shared memory with this split", B); return FTLM_EUNSUPPORTED; }
-  if (fused && B > t->partials_batch) { ftlm_set_error("TML: internal: partials sized for batch %d", t->partials_batch); return FTLM_EINVAL; }
+  if (fused == 1 && B > t->partials_batch) { ftlm_set_error("TML: internal: partials sized for batch %d", t->partials_batch); return FTLM_EINVAL; }
   TmlParams<R> p;
   fill_params<R>(c, t, p, B);
   int grid = c->sm_count * cfg.ctas;
   if ((uint32_t)grid > t->nT) grid = (int)t->nT;
-  if (fused) {
-    auto k = hv_tml_kernel<R, B, MODE, true>;
+  if (fused == 1) {
+    auto k = hv_tml_kernel<R, B, MODE, 1>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
+    FTLM_LAUNCH(k, grid, cfg.threads, cfg.smem, s, p, (const R*)v, (const R*)qp, (R*)y);
+  } else if (fused == 2) {
+    auto k = hv_tml_kernel<R, B, MODE, 2>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
     FTLM_LAUNCH(k, grid, cfg.threads, cfg.smem, s, p, (const R*)v, (const R*)qp, (R*)y);
   } else {
-    auto k = hv_tml_kernel<R, B, MODE, false>;
+    auto k = hv_tml_kernel<R, B, MODE, 0>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
     FTLM_LAUNCH(k, grid, cfg.threads, cfg.smem, s, p, (const R*)v, (const R*)qp, (R*)y);
   }
@@ -731,6 +753,7 @@ int launch_tml_b(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused,
 }  // namespace
 
 void ftlm_tml_plan_destroy(ftlm_ctx* c) {
+  ftlm_passb_plan_destroy(c);
   TmlPlan* t = c->tml;
   if (!t) return;
   cudaFree(t->d_blob); cudaFree(t->d_items); cudaFree(t->d_item_off); cudaFree(t->d_partials);
@@ -741,19 +764,26 @@ void ftlm_tml_plan_destroy(ftlm_ctx* c) {
 
 // Build the plan.  FTLM_OK with c->tml == nullptr when no split is possible for this sector (the
 // dispatcher then uses the TILE / ROW kernels).  c->tml_low_bits / c->tml_mid_bits (0 = auto) choose w, m.
+static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced);
+
 int ftlm_tml_plan_create(ftlm_ctx* c) {
   c->tml = nullptr;
-  const int N = c->N, esz = (int)ftlm_elem_size(c);
+  const int N = c->N;
   const bool forced = c->tml_low_bits != 0 || c->tml_mid_bits != 0;
-  int w = c->tml_low_bits, m = c->tml_mid_bits;
-  if (!forced) {
-    int mw = N - 6 < 16 ? N - 6 : 16;
-    w = mw - 2 < 9 ? mw - 2 : 9;
-    m = mw - w;
-  } else {
-    if (w == 0) w = 9;
-    if (m == 0) m = 7;
+  if (forced) return tml_plan_try(c, c->tml_low_bits ? c->tml_low_bits : 9, c->tml_mid_bits ? c->tml_mid_bits : 7, true);
+  // auto: the largest tile that fits shared memory (fewer bonds leave the tile), w = 9 low bits
+  for (int mw = N - 6 < 17 ? N - 6 : 17; mw >= 6; --mw) {
+    const int w = mw - 2 < 9 ? mw - 2 : 9;
+    int rc = tml_plan_try(c, w, mw - w, false);
+    if (rc != FTLM_OK) return rc;
+    if (c->tml) break;
   }
+  return FTLM_OK;
+}
+
+static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
+  c->tml = nullptr;
+  const int N = c->N, esz = (int)ftlm_elem_size(c);
   const int t = N - w - m;
   auto unusable = [&](const char* why) {
     if (forced) { ftlm_set_error("TML: low_bits=%d mid_bits=%d unusable for N=%d: %s", w, m, N, why); return (int)FTLM_EUNSUPPORTED; }
@@ -775,21 +805,36 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
     return (uint32_t)ts_index[(size_t)s];
   };
   double sumJ_ll = 0.0;
+  std::vector<int> tt_cand;                                              // bonds with both sites in the top part
   for (int b = 0; b < c->nb; ++b) {
     const BondDev& d = c->bonds[(size_t)b];
     const int i = d.i, j = d.j;                                          // i < j
     if (j < w) { bclass[(size_t)b] = 0; bentry[(size_t)b] = (int)ll.size(); ll.push_back({(uint32_t)d.mask, d.Jh}); sumJ_ll += d.Jh; }
     else if (i >= w && j < mw) { bclass[(size_t)b] = 1; bentry[(size_t)b] = (int)P->mm.size(); P->mm.push_back({(uint32_t)(d.mask >> w), 0u, d.Jh}); }
     else if (i < w && j < mw) { bclass[(size_t)b] = 2; bentry[(size_t)b] = (int)P->ml.size(); P->ml.push_back({(uint32_t)i, (uint32_t)(j - w), d.Jh}); }
-    else if (i >= mw) { bclass[(size_t)b] = 3; bentry[(size_t)b] = (int)P->tt_mask.size(); P->tt_mask.push_back((uint32_t)(d.mask >> mw)); P->tt_J.push_back(d.Jh); }
+    else if (i >= mw) { bclass[(size_t)b] = 3; tt_cand.push_back(b); }
     else if (i >= w) { bclass[(size_t)b] = 4; bentry[(size_t)b] = (int)P->tm.size(); P->tm.push_back({(uint32_t)(i - w), ts_of(j), d.Jh}); }
     else { bclass[(size_t)b] = 5; bentry[(size_t)b] = (int)P->tl.size(); P->tl.push_back({(uint32_t)i, ts_of(j), d.Jh}); }
+  }
+  // top-top bonds: PASS-B windows take what pays (class 6, entry = window), the rest stays here (class 3)
+  {
+    std::vector<int> window_of;
+    ftlm_passb_plan_destroy(c);
+    int rc = ftlm_passb_plan_create(c, mw, tt_cand, window_of);
+    if (rc != FTLM_OK) { delete P; return rc; }
+    if (ftlm_passb_windows(c) > 8) { ftlm_passb_plan_destroy(c); window_of.assign(tt_cand.size(), -1); }
+    for (size_t k = 0; k < tt_cand.size(); ++k) {
+      const int b = tt_cand[k];
+      const BondDev& d = c->bonds[(size_t)b];
+      if (window_of[k] >= 0) { bclass[(size_t)b] = 6; bentry[(size_t)b] = window_of[k]; }
+      else { bclass[(size_t)b] = 3; bentry[(size_t)b] = (int)P->tt_mask.size(); P->tt_mask.push_back((uint32_t)(d.mask >> mw)); P->tt_J.push_back(d.Jh); }
+    }
   }
   P->n_ll = (int)ll.size(); P->n_ll4 = (P->n_ll + 3) & ~3;
   P->n_mm = (int)P->mm.size(); P->n_ml = (int)P->ml.size(); P->n_tt = (int)P->tt_mask.size();
   P->n_ts = (int)P->ts_site.size(); P->n_tm = (int)P->tm.size(); P->n_tl = (int)P->tl.size();
   if (P->n_ll4 > TML_MAX_LL || P->n_mm > TML_MAX_LIST || P->n_ml > TML_MAX_LIST || P->n_tt > TML_MAX_TT ||
-      P->n_ts > TML_MAX_TS || P->n_tm > TML_MAX_LIST || P->n_tl > TML_MAX_LIST) { delete P; return unusable("too many bonds in one class"); }
+      P->n_ts > TML_MAX_TS || P->n_tm > TML_MAX_LIST || P->n_tl > TML_MAX_LIST) { ftlm_passb_plan_destroy(c); delete P; return unusable("too many bonds in one class"); }
   for (int k = 0; k < P->n_ll4; ++k) P->ll_J.push_back(k < P->n_ll ? ll[(size_t)k].Jh : 0.0);
   P->diag_coef = c->diag0 - sumJ_ll;
   // ---- tables (blob) ---------------------------------------------------------------------------
@@ -806,7 +851,7 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
     lstate[(size_t)(koff[(size_t)cnt] + (int)r)] = (uint16_t)L;
   }
   P->max_tile = (int)binom_t(mw, mw / 2);
-  if (P->max_tile > 65535 || binom_t(w, w / 2) > 32767) { delete P; return unusable("tile too large for 16-bit offsets"); }
+  if (P->max_tile > 65535 || binom_t(w, w / 2) > 32767) { ftlm_passb_plan_destroy(c); delete P; return unusable("tile too large for 16-bit offsets"); }
   std::vector<int> tlen((size_t)mw + 1);
   std::vector<uint16_t> coloff((size_t)(mw + 1) * nM, 0);
   std::vector<uint32_t> items;
@@ -865,7 +910,7 @@ int ftlm_tml_plan_create(ftlm_ctx* c) {
   P->off_tl = put(P->tl.data(), P->tl.size() * sizeof(TmlSEnt));
   P->blob_bytes = (int)blob.size();
   c->tml = P;
-  if (tml_config(c, P, 1).smem == 0) { c->tml = nullptr; delete P; return unusable("tables + tile exceed shared memory"); }
+  if (tml_config(c, P, 1).smem == 0) { c->tml = nullptr; ftlm_passb_plan_destroy(c); delete P; return unusable("tables + tile exceed shared memory"); }
   // ---- upload ----------------------------------------------------------------------------------
   P->partials_batch = 4;
   auto up = [&](void** d, const void* h, size_t bytes) -> bool {

@@ -28,7 +28,7 @@ def lib():
     if _lib is None:
         sys.path.insert(0, HERE)
         import build_emu
-        L = C.CDLL(build_emu.build())
+        L = C.CDLL(os.environ.get("FTLM_EMU_LIB") or build_emu.build())   # a frozen copy, for long sweeps
         L.ftlm_dim.restype = C.c_int64
         L.ftlm_get_option.restype = C.c_int64
         L.ftlm_last_error.restype = C.c_char_p

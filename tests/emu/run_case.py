@@ -65,6 +65,8 @@ def main():
     with E.EmuCtx(w, n_up, mode, prec, h=h, options=spec.get("options", ())) as c:
         res["kernel"] = c.get("kernel")
         res["dim"] = c.dim
+        res["passb"] = [c.get("passb_windows"), c.get("passb_bonds"), c.get("passb_lo"), c.get("passb_s")]
+        res["tml"] = [c.get("tml_w"), c.get("tml_m")]
         assert c.dim == D
         what = spec.get("what", ["neighbors", "apply"])
         if "neighbors" in what:

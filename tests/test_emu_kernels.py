@@ -79,3 +79,26 @@ def test_emu_guard_pages_catch_overrun():
             "print('survived')\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
     p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=120)
     assert p.returncode != 0 and "survived" not in p.stdout
+
+
+@pytest.mark.parametrize("wl,n_up,w,m,mode,prec,what", [
+    ("ring16j", 8, 5, 3, "cr", "fp64", ["neighbors", "apply", "lanczos"]),      # one window, no frozen bits
+    ("ring16j", 8, 5, 3, "clt", "fp32", ["apply", "lanczos"]),
+    ("rand15_40_5", 7, 5, 2, "clt", "fp64", ["neighbors", "apply", "lanczos"]),  # random graph, random J
+    ("ring19j", 9, 5, 1, "cr", "fp32", ["apply"]),                               # two windows, frozen bits above the second
+])
+def test_emu_two_pass_tml_plus_passb(wl, n_up, w, m, mode, prec, what):
+    """PASS-B (bonds among the top label bits streamed by window) + the TML pass that leaves them out."""
+    res = run_case({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec,
+                    "options": [["tml_split", w | (m << 8)], ["kernel", K["tml"]]], "what": what, "steps": 6},
+                   timeout=1500)
+    assert res["kernel"] == K["tml"] and res["passb"][0] >= 1 and res["passb"][1] >= 3
+    if wl == "ring19j":
+        assert res["passb"][0] == 2
+
+
+def test_emu_passb_off_keeps_top_bonds_in_tml():
+    res = run_case({"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp64",
+                    "options": [["passb", 0], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]],
+                    "what": ["neighbors", "apply"]})
+    assert res["passb"][0] == 0
