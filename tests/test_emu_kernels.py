@@ -85,7 +85,7 @@ def test_emu_guard_pages_catch_overrun():
     ("ring16j", 8, 5, 3, "cr", "fp64", ["neighbors", "apply", "lanczos"]),      # one window, no frozen bits
     ("ring16j", 8, 5, 3, "clt", "fp32", ["apply", "lanczos"]),
     ("rand15_40_5", 7, 5, 2, "clt", "fp64", ["neighbors", "apply", "lanczos"]),  # random graph, random J
-    ("ring19j", 9, 5, 1, "cr", "fp32", ["apply"]),                               # two windows, frozen bits above the second
+    ("ring20j", 10, 5, 1, "cr", "fp32", ["apply"]),                              # two windows, frozen bits above the second
 ])
 def test_emu_two_pass_tml_plus_passb(wl, n_up, w, m, mode, prec, what):
     """PASS-B (bonds among the top label bits streamed by window) + the TML pass that leaves them out."""
@@ -93,7 +93,7 @@ def test_emu_two_pass_tml_plus_passb(wl, n_up, w, m, mode, prec, what):
                     "options": [["tml_split", w | (m << 8)], ["kernel", K["tml"]]], "what": what, "steps": 6},
                    timeout=1500)
     assert res["kernel"] == K["tml"] and res["passb"][0] >= 1 and res["passb"][1] >= 3
-    if wl == "ring19j":
+    if wl == "ring20j":
         assert res["passb"][0] == 2
 
 
