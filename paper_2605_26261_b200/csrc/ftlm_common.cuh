@@ -84,7 +84,10 @@ struct ftlm_ctx {
   TmlPlan* tml = nullptr;
   // PASS-B windows for the bonds among the top label bits (ftlm_passb.cu); owned together with `tml`
   PassBSet* passb = nullptr;
-  int use_passb = 1;               // option "passb": 0 keeps every top-top bond in the TML kernel
+  int use_passb = 1;               // option "passb": 0 keeps every bond that leaves the tile in the TML kernel
+  int passb_lo_min = 0;            // option "passb_lo_min": lowest label position a window may use (0 = auto)
+  int passb_smax = 0;              // option "passb_smax": largest window (0 = auto: 12 FP32 / 11 FP64)
+  int passb_ctas = 0;              // option "passb_ctas": CTAs per SM tried first (0 = auto: 2)
 
   // chain workspace
   void* q[3] = {nullptr, nullptr, nullptr};

@@ -336,6 +336,18 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     }
     return rc;
   }
+  if (!strcmp(key, "passb_lo_min") || !strcmp(key, "passb_smax") || !strcmp(key, "passb_ctas")) {
+    // PASS-B window planner knobs (0 = auto); rebuilds the TML / PASS-B plans
+    if (value < 0 || value > 62) { ftlm_set_error("%s out of range", key); return FTLM_EINVAL; }
+    int* slot = !strcmp(key, "passb_lo_min") ? &c->passb_lo_min : !strcmp(key, "passb_smax") ? &c->passb_smax : &c->passb_ctas;
+    const int old = *slot;
+    *slot = (int)value;
+    CK(cudaSetDevice(c->device));
+    ftlm_tml_plan_destroy(c);
+    int rc = ftlm_tml_plan_create(c);
+    if (rc != FTLM_OK) { *slot = old; ftlm_tml_plan_destroy(c); ftlm_tml_plan_create(c); }
+    return rc;
+  }
   ftlm_set_error("ftlm_set_option: unknown key '%s'", key);
   return FTLM_EINVAL;
 }

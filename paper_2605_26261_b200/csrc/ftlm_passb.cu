@@ -29,6 +29,7 @@ template <typename R>
 struct PassBParams {
   int N, K, lo, s, f, ngroups;
   uint32_t nitems;
+  uint64_t smask_hi, fmask_hi;      // active / frozen positions of the label >> lo
   int64_t dim;
   const uint64_t* binom;            // [(N+1)*(K+1)] global
   const uint2* clt;
@@ -46,6 +47,8 @@ struct PassBParams {
 
 struct PassBWindow {
   int lo = 0, s = 0, f = 0, ngroups = 0, max_conf = 0;
+  uint64_t smask = 0;               // the s active label positions (all >= lo)
+  int ctas = 1, threads = PASSB_THREADS;
   uint32_t nitems = 0;
   int xk[PASSB_MAX_S + 1] = {0};
   size_t smem = 0;
@@ -64,6 +67,16 @@ struct PassBSet {
 };
 
 namespace {
+
+__host__ __device__ inline uint64_t bits_deposit(uint64_t x, uint64_t mask) {
+  uint64_t r = 0;
+  for (int k = 0; mask; ++k) {
+    const uint64_t low = mask & (~mask + 1ull);
+    if ((x >> k) & 1ull) r |= low;
+    mask ^= low;
+  }
+  return r;
+}
 
 __host__ __device__ inline size_t passb_smem_bytes(int N, int K, int max_conf, int max_rows, int esz) {
   size_t o = 0;
@@ -118,7 +131,7 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     const uint64_t x0 = (uint64_t)(item - __ldg(&p.grp_first[g])) * (uint64_t)X;
     if (g != cur_group) {                               // (uniform) run starts of this class
       for (int sl = tid; sl < nconf; sl += NT) {
-        const uint64_t hi = ((uint64_t)F << p.s) | (uint64_t)__ldg(&p.ustate[c0 + sl]);
+        const uint64_t hi = bits_deposit((uint64_t)F, p.fmask_hi) | bits_deposit((uint64_t)__ldg(&p.ustate[c0 + sl]), p.smask_hi);
         s_start[sl] = passb_run_start<MODE>(hi, p.lo, kP, p.K, s_binom, p.clt);
       }
       cur_group = g;
@@ -144,7 +157,13 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
       const uint32_t ent = __ldg(&p.nbr[(size_t)u * 32 + lane]);
       const int cnt = __popc(__ballot_sync(0xffffffffu, ent != PASSB_END));
       const R* row = tile + (size_t)sl * X;
-      R own[4], acc[4];
+      R* yrow = y + s_start[sl] + x0;
+      R own[4], acc[4], yold[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {                      // y is read first: its latency hides behind the bond loop
+        const int x = lane + 32 * k;
+        yold[k] = (k < XK && x < nx) ? __ldcs(&yrow[x]) : (R)0;
+      }
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const int x = lane + 32 * k;
@@ -163,13 +182,12 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
           if (k < XK && x < nx) acc[k] += J * nrow[x];
         }
       }
-      R* yrow = y + s_start[sl] + x0;
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const int x = lane + 32 * k;
         if (k < XK && x < nx) {
-          const R yn = yrow[x] + (acc[k] - sumJ * own[k]);
-          yrow[x] = yn;
+          const R yn = yold[k] + (acc[k] - sumJ * own[k]);
+          __stcs(&yrow[x], yn);
           if (FUSED) {
             s_qy += (double)own[k] * (double)yn;
             s_yy += (double)yn * (double)yn;
@@ -233,6 +251,17 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
   }
 }
 
+// bit k of x goes to the position of the k-th set bit of mask / back
+__host__ __device__ inline uint64_t bits_extract(uint64_t x, uint64_t mask) {
+  uint64_t r = 0;
+  for (int k = 0; mask; ++k) {
+    const uint64_t low = mask & (~mask + 1ull);
+    if (x & low) r |= 1ull << k;
+    mask ^= low;
+  }
+  return r;
+}
+
 uint64_t binom_b(int n, int k) {
   if (k < 0 || k > n) return 0;
   if (k > n - k) k = n - k;
@@ -267,6 +296,10 @@ int64_t ftlm_passb_info(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "passb_windows")) return S ? (int64_t)S->win.size() : 0;
   if (!S || S->win.empty()) return -1;
   if (!strcmp(key, "passb_bonds")) { int64_t n = 0; for (const PassBWindow& w : S->win) n += (int64_t)w.bonds.size(); return n; }
+  if (!strncmp(key, "passb_lo", 8) && key[8] >= '0' && key[8] <= '7') { const size_t k = (size_t)(key[8] - '0'); return k < S->win.size() ? S->win[k].lo : -1; }
+  if (!strncmp(key, "passb_mask", 10) && key[10] >= '0' && key[10] <= '7') { const size_t k = (size_t)(key[10] - '0'); return k < S->win.size() ? (int64_t)S->win[k].smask : -1; }
+  if (!strncmp(key, "passb_nbonds", 12) && key[12] >= '0' && key[12] <= '7') { const size_t k = (size_t)(key[12] - '0'); return k < S->win.size() ? (int64_t)S->win[k].bonds.size() : -1; }
+  if (!strcmp(key, "passb_ctas_used")) return S->win[0].ctas;
   if (!strcmp(key, "passb_lo")) return S->win[0].lo;
   if (!strcmp(key, "passb_s")) return S->win[0].s;
   if (!strcmp(key, "passb_items")) return S->win[0].nitems;
@@ -276,10 +309,12 @@ int64_t ftlm_passb_info(const ftlm_ctx* c, const char* key) {
 
 // Fill the host-side geometry of a window (classes, chunk sizes, item groups).  false if it cannot run
 // (a popcount class does not fit shared memory even at X = 32, or the item count overflows 32 bits).
+// Two CTAs per SM when every class fits half of the shared memory at X >= 32: one CTA's staging
+// phase then overlaps the other's compute phase.
 static bool passb_geometry(const ftlm_ctx* c, PassBWindow& w, std::vector<uint32_t>& grp_first) {
   const int N = c->N, K = c->N_up, esz = (int)ftlm_elem_size(c);
   w.f = N - w.lo - w.s;
-  if (w.f < 0 || w.f > 20 || w.s < 2 || w.s > PASSB_MAX_S) return false;
+  if (w.f < 0 || w.f > 20 || w.s < 2 || w.s > PASSB_MAX_S || w.lo < 0) return false;
   const int s1 = w.s + 1;
   w.ngroups = (1 << w.f) * s1;
   // largest class that actually occurs
@@ -293,19 +328,26 @@ static bool passb_geometry(const ftlm_ctx* c, PassBWindow& w, std::vector<uint32
   for (int p = 0; p <= w.s; ++p) if (used[(size_t)p]) w.max_conf = std::max(w.max_conf, (int)binom_b(w.s, p));
   if (w.max_conf == 0) return false;
   const size_t fixed = passb_smem_bytes(N, K, w.max_conf, 0, esz);
-  const size_t cap = 227 * 1024 - 1024;
-  if (fixed >= cap) return false;
-  const size_t budget = cap - fixed;
+  bool fits = false;
   int max_rows = 0;
-  for (int p = 0; p <= w.s; ++p) {
-    w.xk[p] = 0;
-    if (!used[(size_t)p]) continue;
-    const size_t per32 = (size_t)binom_b(w.s, p) * 32 * (size_t)esz;
-    int xk = (int)std::min<size_t>(4, budget / per32);
-    if (xk < 1) return false;
-    w.xk[p] = xk;
-    max_rows = std::max(max_rows, (int)binom_b(w.s, p) * 32 * xk);
+  for (int ctas = c->passb_ctas > 0 ? c->passb_ctas : 2; ctas >= 1 && !fits; --ctas) {
+    const size_t cap = (size_t)(228 * 1024) / (size_t)ctas - 1024 - (ctas == 1 ? 1024 : 0);
+    if (fixed >= cap) continue;
+    const size_t budget = cap - fixed;
+    fits = true;
+    max_rows = 0;
+    for (int p = 0; p <= w.s && fits; ++p) {
+      w.xk[p] = 0;
+      if (!used[(size_t)p]) continue;
+      const size_t per32 = (size_t)binom_b(w.s, p) * 32 * (size_t)esz;
+      int xk = (int)std::min<size_t>(4, budget / per32);
+      if (xk < 1) { fits = false; break; }
+      w.xk[p] = xk;
+      max_rows = std::max(max_rows, (int)binom_b(w.s, p) * 32 * xk);
+    }
+    if (fits) { w.ctas = ctas; w.threads = ctas >= 2 ? 512 : PASSB_THREADS; }
   }
+  if (!fits) return false;
   w.smem = passb_smem_bytes(N, K, w.max_conf, max_rows, esz);
   grp_first.assign((size_t)w.ngroups + 1, 0);
   uint64_t total = 0;
@@ -323,56 +365,81 @@ static bool passb_geometry(const ftlm_ctx* c, PassBWindow& w, std::vector<uint32
   return total > 0;
 }
 
-int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& tt, std::vector<int>& window_of) {
-  window_of.assign(tt.size(), -1);
+// Window selection = greedy cover of the candidate bonds (those with a site at or above mw, which the
+// TML tile cannot serve from shared memory) by sets of at most smax label positions, all >= lo_min:
+// grow a set from every uncovered bond by adding the position that brings in the most uncovered
+// bonds (or, failing that, a neighbouring position), keep the best set, repeat while a window takes
+// at least MIN_GAIN bonds (a window costs one more stream of v and y).
+int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, std::vector<int>& window_of) {
+  window_of.assign(cand.size(), -1);
   c->passb = nullptr;
-  if (!c->use_passb || tt.empty()) return FTLM_OK;
+  if (!c->use_passb || cand.empty()) return FTLM_OK;
   const int N = c->N;
-  const int smax = ftlm_elem_size(c) == 4 ? PASSB_MAX_S : PASSB_MAX_S - 1;
-  const int MIN_GAIN = 3;                          // a window costs one more stream of v and y
+  int smax = ftlm_elem_size(c) == 4 ? PASSB_MAX_S : PASSB_MAX_S - 1;
+  if (c->passb_smax >= 2 && c->passb_smax < smax) smax = c->passb_smax;
+  int lo_min = c->passb_lo_min > 0 ? c->passb_lo_min : std::max(8, mw - 6);
+  if (lo_min > mw) lo_min = mw;
+  const int MIN_GAIN = 3;
   PassBSet* S = new PassBSet();
   std::vector<std::vector<uint32_t>> groups;
+  auto open_bond = [&](size_t k) {
+    if (window_of[k] >= 0) return false;
+    return c->bonds[(size_t)cand[k]].i >= lo_min;      // i < j
+  };
+  auto covered = [&](uint64_t set) {
+    int n = 0;
+    for (size_t k = 0; k < cand.size(); ++k)
+      if (open_bond(k) && (c->bonds[(size_t)cand[k]].mask & ~set) == 0) ++n;
+    return n;
+  };
   for (;;) {
-    int best_lo = -1, best_s = 0, best_cnt = 0;
-    for (int lo = mw; lo + 2 <= N; ++lo) {
-      const int s = std::min(smax, N - lo);
-      int cnt = 0;
-      for (size_t k = 0; k < tt.size(); ++k) {
-        if (window_of[k] >= 0) continue;
-        const BondDev& d = c->bonds[(size_t)tt[k]];
-        if (d.i >= lo && d.j < lo + s) ++cnt;
+    uint64_t best_set = 0;
+    int best_cnt = 0;
+    for (size_t seed = 0; seed < cand.size(); ++seed) {
+      if (!open_bond(seed)) continue;
+      uint64_t set = c->bonds[(size_t)cand[seed]].mask;
+      int cur = covered(set);
+      while (__builtin_popcountll(set) < smax) {
+        int pick = -1, pick_cnt = cur;
+        for (int v = lo_min; v < N; ++v) {
+          if ((set >> v) & 1ull) continue;
+          const int g = covered(set | (1ull << v));
+          if (g > pick_cnt) { pick_cnt = g; pick = v; }
+        }
+        if (pick < 0) {                                   // no direct gain: a position next to the set
+          for (size_t k = 0; k < cand.size() && pick < 0; ++k) {
+            if (!open_bond(k)) continue;
+            const uint64_t m = c->bonds[(size_t)cand[k]].mask;
+            if ((m & set) != 0 && (m & ~set) != 0) pick = __builtin_ctzll(m & ~set);
+          }
+          if (pick < 0) break;
+        }
+        set |= 1ull << pick;
+        cur = covered(set);
       }
-      cnt = std::min(cnt, PASSB_MAX_BONDS);
-      if (cnt > best_cnt) { best_cnt = cnt; best_lo = lo; best_s = s; }
+      if (cur > best_cnt) { best_cnt = cur; best_set = set; }
     }
     if (best_cnt < MIN_GAIN) break;
+    // keep only the positions some covered bond uses
+    uint64_t used = 0;
+    for (size_t k = 0; k < cand.size(); ++k)
+      if (open_bond(k) && (c->bonds[(size_t)cand[k]].mask & ~best_set) == 0) used |= c->bonds[(size_t)cand[k]].mask;
     PassBWindow w;
-    w.lo = best_lo; w.s = best_s;
-    // shrink the window to the sites its bonds use (shorter windows have smaller classes, larger X)
-    int hi_used = 0;
-    for (size_t k = 0; k < tt.size(); ++k) {
-      if (window_of[k] >= 0) continue;
-      const BondDev& d = c->bonds[(size_t)tt[k]];
-      if (d.i >= w.lo && d.j < w.lo + w.s) hi_used = std::max(hi_used, d.j);
-    }
-    if (w.lo + w.s < N) w.s = std::max(2, hi_used - w.lo + 1);   // only if something stays frozen above anyway
-    int lo_used = N;
-    for (size_t k = 0; k < tt.size(); ++k) {
-      if (window_of[k] >= 0) continue;
-      const BondDev& d = c->bonds[(size_t)tt[k]];
-      if (d.i >= w.lo && d.j < w.lo + w.s) lo_used = std::min(lo_used, d.i);
-    }
-    if (lo_used > w.lo && lo_used < N && w.s - (lo_used - w.lo) >= 2) { w.s -= lo_used - w.lo; w.lo = lo_used; }   // longer runs
+    w.smask = used;
+    w.s = __builtin_popcountll(used);
+    w.lo = __builtin_ctzll(used);                         // longest runs: every position below the window is passive
+    if (N - w.lo - w.s > 20) break;
     std::vector<uint32_t> gf;
     if (!passb_geometry(c, w, gf)) break;
     const int widx = (int)S->win.size();
-    for (size_t k = 0; k < tt.size() && (int)w.bonds.size() < PASSB_MAX_BONDS; ++k) {
-      if (window_of[k] >= 0) continue;
-      const BondDev& d = c->bonds[(size_t)tt[k]];
-      if (d.i >= w.lo && d.j < w.lo + w.s) { window_of[k] = widx; w.bonds.push_back(tt[k]); w.Jh.push_back(d.Jh); }
+    for (size_t k = 0; k < cand.size() && (int)w.bonds.size() < PASSB_MAX_BONDS; ++k) {
+      if (!open_bond(k)) continue;
+      const BondDev& d = c->bonds[(size_t)cand[k]];
+      if ((d.mask & ~w.smask) == 0) { window_of[k] = widx; w.bonds.push_back(cand[k]); w.Jh.push_back(d.Jh); }
     }
     S->win.push_back(w);
     groups.push_back(gf);
+    if (S->win.size() >= 8) break;
   }
   if (S->win.empty()) { delete S; return FTLM_OK; }
   c->passb = S;
@@ -394,7 +461,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& tt, std:
       int n = 0;
       for (size_t e = 0; e < w.bonds.size(); ++e) {
         const BondDev& d = c->bonds[(size_t)w.bonds[e]];
-        const uint32_t mk = (uint32_t)(d.mask >> w.lo), x = (uint32_t)u & mk;
+        const uint32_t mk = (uint32_t)bits_extract(d.mask, w.smask), x = (uint32_t)u & mk;
         if (x != 0 && x != mk) nbr[(size_t)u * 32 + (size_t)n++] = (uint32_t)slot[(size_t)((uint32_t)u ^ mk)] | ((uint32_t)e << 16);
       }
     }
@@ -422,18 +489,20 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.ustate = w.d_ustate; p.koff = w.d_koff;
   p.nbr = w.d_nbr; p.grp_first = w.d_grp_first; p.partials = w.d_partials; p.counter = w.d_counter;
   p.st = c->d_state; p.max_conf = w.max_conf;
+  p.smask_hi = w.smask >> w.lo;
+  p.fmask_hi = (c->N >= 64 ? ~0ull : ((1ull << c->N) - 1ull)) >> w.lo & ~p.smask_hi;
   for (int k = 0; k <= PASSB_MAX_S; ++k) p.xk[k] = w.xk[k];
   for (size_t e = 0; e < w.Jh.size(); ++e) p.Jh[e] = (R)w.Jh[e];
-  int grid = c->sm_count;
+  int grid = c->sm_count * w.ctas;
   if ((uint32_t)grid > w.nitems) grid = (int)w.nitems;
   if (fused) {
     auto k = passb_kernel<R, MODE, true>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
-    FTLM_LAUNCH(k, grid, PASSB_THREADS, w.smem, s, p, (const R*)v, (R*)y);
+    FTLM_LAUNCH(k, grid, w.threads, w.smem, s, p, (const R*)v, (R*)y);
   } else {
     auto k = passb_kernel<R, MODE, false>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
-    FTLM_LAUNCH(k, grid, PASSB_THREADS, w.smem, s, p, (const R*)v, (R*)y);
+    FTLM_LAUNCH(k, grid, w.threads, w.smem, s, p, (const R*)v, (R*)y);
   }
   CK(cudaGetLastError());
   return FTLM_OK;

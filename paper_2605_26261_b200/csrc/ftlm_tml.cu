@@ -805,30 +805,27 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
     return (uint32_t)ts_index[(size_t)s];
   };
   double sumJ_ll = 0.0;
-  std::vector<int> tt_cand;                                              // bonds with both sites in the top part
+  // bonds that leave the tile (a site at or above mw): PASS-B windows take what they can cover
+  // (class 6, entry = window); the rest is read from global memory here (TT / TM / TL)
+  std::vector<int> cand, window_of;
+  for (int b = 0; b < c->nb; ++b) if (c->bonds[(size_t)b].j >= mw) cand.push_back(b);
+  {
+    ftlm_passb_plan_destroy(c);
+    int rc = ftlm_passb_plan_create(c, mw, cand, window_of);
+    if (rc != FTLM_OK) { delete P; return rc; }
+  }
+  std::vector<int> win_of_bond((size_t)c->nb, -1);
+  for (size_t k = 0; k < cand.size(); ++k) win_of_bond[(size_t)cand[k]] = window_of[k];
   for (int b = 0; b < c->nb; ++b) {
     const BondDev& d = c->bonds[(size_t)b];
     const int i = d.i, j = d.j;                                          // i < j
-    if (j < w) { bclass[(size_t)b] = 0; bentry[(size_t)b] = (int)ll.size(); ll.push_back({(uint32_t)d.mask, d.Jh}); sumJ_ll += d.Jh; }
+    if (win_of_bond[(size_t)b] >= 0) { bclass[(size_t)b] = 6; bentry[(size_t)b] = win_of_bond[(size_t)b]; }
+    else if (j < w) { bclass[(size_t)b] = 0; bentry[(size_t)b] = (int)ll.size(); ll.push_back({(uint32_t)d.mask, d.Jh}); sumJ_ll += d.Jh; }
     else if (i >= w && j < mw) { bclass[(size_t)b] = 1; bentry[(size_t)b] = (int)P->mm.size(); P->mm.push_back({(uint32_t)(d.mask >> w), 0u, d.Jh}); }
     else if (i < w && j < mw) { bclass[(size_t)b] = 2; bentry[(size_t)b] = (int)P->ml.size(); P->ml.push_back({(uint32_t)i, (uint32_t)(j - w), d.Jh}); }
-    else if (i >= mw) { bclass[(size_t)b] = 3; tt_cand.push_back(b); }
+    else if (i >= mw) { bclass[(size_t)b] = 3; bentry[(size_t)b] = (int)P->tt_mask.size(); P->tt_mask.push_back((uint32_t)(d.mask >> mw)); P->tt_J.push_back(d.Jh); }
     else if (i >= w) { bclass[(size_t)b] = 4; bentry[(size_t)b] = (int)P->tm.size(); P->tm.push_back({(uint32_t)(i - w), ts_of(j), d.Jh}); }
     else { bclass[(size_t)b] = 5; bentry[(size_t)b] = (int)P->tl.size(); P->tl.push_back({(uint32_t)i, ts_of(j), d.Jh}); }
-  }
-  // top-top bonds: PASS-B windows take what pays (class 6, entry = window), the rest stays here (class 3)
-  {
-    std::vector<int> window_of;
-    ftlm_passb_plan_destroy(c);
-    int rc = ftlm_passb_plan_create(c, mw, tt_cand, window_of);
-    if (rc != FTLM_OK) { delete P; return rc; }
-    if (ftlm_passb_windows(c) > 8) { ftlm_passb_plan_destroy(c); window_of.assign(tt_cand.size(), -1); }
-    for (size_t k = 0; k < tt_cand.size(); ++k) {
-      const int b = tt_cand[k];
-      const BondDev& d = c->bonds[(size_t)b];
-      if (window_of[k] >= 0) { bclass[(size_t)b] = 6; bentry[(size_t)b] = window_of[k]; }
-      else { bclass[(size_t)b] = 3; bentry[(size_t)b] = (int)P->tt_mask.size(); P->tt_mask.push_back((uint32_t)(d.mask >> mw)); P->tt_J.push_back(d.Jh); }
-    }
   }
   P->n_ll = (int)ll.size(); P->n_ll4 = (P->n_ll + 3) & ~3;
   P->n_mm = (int)P->mm.size(); P->n_ml = (int)P->ml.size(); P->n_tt = (int)P->tt_mask.size();

@@ -97,6 +97,20 @@ def test_emu_two_pass_tml_plus_passb(wl, n_up, w, m, mode, prec, what):
         assert res["passb"][0] == 2
 
 
+@pytest.mark.parametrize("wl,n_up,split,mode,prec,opts,nwin,what", [
+    # windows reach below the tile boundary (TM / TL bonds too) and need not be contiguous
+    ("ring16j", 8, 5 | (3 << 8), "cr", "fp64", [["passb_lo_min", 4]], 1, ["neighbors", "apply", "lanczos"]),
+    ("rand15_40_5", 7, 5 | (2 << 8), "clt", "fp64", [["passb_lo_min", 3], ["passb_smax", 6]], 2, ["neighbors", "apply", "lanczos"]),
+    ("rand15_40_5", 6, 5 | (2 << 8), "cr", "fp32", [["passb_lo_min", 5], ["passb_smax", 5], ["passb_ctas", 1]], 2, ["neighbors", "apply"]),
+])
+def test_emu_generalised_windows(wl, n_up, split, mode, prec, opts, nwin, what):
+    """PASS-B windows as arbitrary sets of label positions >= lo_min chosen by the greedy cover."""
+    res = run_case({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec,
+                    "options": opts + [["tml_split", split], ["kernel", K["tml"]]], "what": what, "steps": 6},
+                   timeout=1500)
+    assert res["kernel"] == K["tml"] and res["passb"][0] >= nwin
+
+
 def test_emu_passb_off_keeps_top_bonds_in_tml():
     res = run_case({"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp64",
                     "options": [["passb", 0], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]],
