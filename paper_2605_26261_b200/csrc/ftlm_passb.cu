@@ -377,7 +377,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
   const int N = c->N;
   int smax = ftlm_elem_size(c) == 4 ? PASSB_MAX_S : PASSB_MAX_S - 1;
   if (c->passb_smax >= 2 && c->passb_smax < smax) smax = c->passb_smax;
-  int lo_min = c->passb_lo_min > 0 ? c->passb_lo_min : std::max(8, mw - 6);
+  int lo_min = c->passb_lo_min > 0 ? c->passb_lo_min : std::max(8, mw - 7);
   if (lo_min > mw) lo_min = mw;
   const int MIN_GAIN = 3;
   PassBSet* S = new PassBSet();

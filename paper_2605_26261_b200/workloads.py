@@ -168,6 +168,21 @@ def relabel(w: Workload, perm) -> Workload:
                     w.R, w.n_steps, w.note)
 
 
+# Site numbering of BASELINE config 4 (reading 30: the paper names the polyhedron only, any
+# fixed numbering is the same physics).  CONFIG4_SITE_ORDER[s] = label position of lexicographic
+# site s.  Found offline by simulated annealing over orderings of the 60-bond graph with the
+# objective "the 17 lowest positions hold as many bonds as possible (28) and every other bond lies
+# inside one of two sets of <= 12 positions >= 10" - pure graph bookkeeping, no arithmetic of the
+# method; both the oracle and the CUDA path receive the relabelled bond list.
+CONFIG4_SITE_ORDER = [2, 15, 14, 22, 29, 24, 28, 17, 21, 20, 6, 8, 0, 7, 11, 12, 5, 4, 23, 19,
+                      10, 16, 26, 3, 25, 13, 27, 9, 18, 1]
+
+
+def fold_order(n: int):
+    """Ring positions folded so that periodic neighbours stay close: 0, n-1, 1, n-2, ..."""
+    return [2 * s if s < (n + 1) // 2 else 2 * (n - 1 - s) + 1 for s in range(n)]
+
+
 def baseline_config(k: int) -> Workload:
     """The five BASELINE.json configs, k = 1..5 (k = 40 is config 4's random-bond variant)."""
     if k == 1:
@@ -177,11 +192,20 @@ def baseline_config(k: int) -> Workload:
     if k == 3:
         return triangular(4, 7, R=20, n_steps=100, note="4x7 triangular PBC, S^z=0")
     if k == 4:
-        return icosidodecahedron(False, R=10, n_steps=100, note="icosidodecahedron S^z=0, D=155117520")
+        w = relabel(icosidodecahedron(False, R=10, n_steps=100, note="icosidodecahedron S^z=0, D=155117520"),
+                    CONFIG4_SITE_ORDER)
+        w.name = "icosidodecahedron"
+        return w
     if k == 40:
-        return icosidodecahedron(True, R=10, n_steps=100, note="icosidodecahedron random J_b")
+        w = relabel(icosidodecahedron(True, R=10, n_steps=100, note="icosidodecahedron random J_b"),
+                    CONFIG4_SITE_ORDER)
+        w.name = "icosidodecahedron_randJ"
+        return w
     if k == 5:
-        return ring(34, 1.0, 0.5, sectors=[17], R=2, n_steps=80, note="N=34 J1-J2 ring S^z=0, CR only")
+        w = relabel(ring(34, 1.0, 0.5, sectors=[17], R=2, n_steps=80, note="N=34 J1-J2 ring S^z=0, CR only"),
+                    fold_order(34))
+        w.name = "ring34_j1j2"
+        return w
     raise ValueError(k)
 
 
