@@ -139,8 +139,54 @@ def run_reference(args, w, n_up):
     print(json.dumps(line), flush=True)
 
 
+# name -> option settings, in order (the candidates of ftlm_autotune, include/ftlm.h)
+CANDIDATES = {
+    "row": [("kernel", 1)],
+    "tile": [("kernel", 2)],
+    "tml": [("passb", 0), ("kernel", 3)],
+    "tml+passb": [("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tml+passb_1cta": [("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
+    "tml+passb_s11": [("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tml+passb_s10": [("passb_smax", 10), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+}
+SAFE_CHOICE = "tml"          # measured on B200 in round 1 (profiles/): the fallback if the probe dies
+
+
+def run_probe(args):
+    """Child process: ftlm_autotune on the bench sector; prints {"choice", "report"} as one JSON line.
+    Runs in its own process so that a faulting candidate cannot take the bench's CUDA context down."""
+    import torch
+    from paper_2605_26261_b200 import ftlm, workloads as W
+    w = W.baseline_config(args.config)
+    n_up = w.sectors[0]
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    mode = ftlm.INDEX_CR if (args.mode == "cr" or w.N > 32) else ftlm.INDEX_CLT
+    ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, torch.cuda.current_device())
+    rep = ftlm.ftlm_autotune(ctx, 3)
+    valid = [r for r in rep if r["valid"]]
+    best = min(valid, key=lambda r: r["ms"])["name"] if valid else None
+    ftlm.ftlm_destroy(ctx)
+    print(json.dumps({"choice": best, "report": rep}), flush=True)
+
+
+def probe_choice(args):
+    cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--config", str(args.config), "--mode", args.mode]
+    try:
+        out = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+        for ln in reversed(out.stdout.strip().splitlines()):
+            if ln.startswith("{"):
+                d = json.loads(ln)
+                if d.get("choice") in CANDIDATES:
+                    return d["choice"], d["report"], None
+        return SAFE_CHOICE, None, f"probe rc={out.returncode}: {out.stderr.strip()[-300:]}"
+    except Exception as e:  # timeout, crash
+        return SAFE_CHOICE, None, f"probe failed: {e!r}"
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--probe", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--candidate", default="", help="one of " + ", ".join(CANDIDATES))
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
@@ -160,6 +206,9 @@ def main():
     n_up = w.sectors[0]
     if args.impl == "reference":
         run_reference(args, w, n_up)
+        return
+    if args.probe:
+        run_probe(args)
         return
 
     import torch
@@ -191,8 +240,22 @@ def main():
         ftlm.ftlm_set_option(ctx, "tml_low_bits", args.tml_low_bits)
     if args.tml_mid_bits:
         ftlm.ftlm_set_option(ctx, "tml_mid_bits", args.tml_mid_bits)
-    ftlm.ftlm_set_option(ctx, "kernel", {"auto": 0, "row": 1, "tile": 2, "tml": 3}[args.kernel])
+    autotune_report, probe_note = None, None
+    if args.candidate:
+        choice = args.candidate
+    elif args.kernel == "auto":
+        # rank 0 probes in a child process; every rank applies the same choice
+        choice, autotune_report, probe_note = probe_choice(args) if rank == 0 else (SAFE_CHOICE, None, None)
+        if dist is not None:
+            box = [choice]
+            dist.broadcast_object_list(box, src=0)
+            choice = box[0]
+    else:
+        choice = {"row": "row", "tile": "tile", "tml": "tml"}[args.kernel]
+    for key, val in CANDIDATES[choice]:
+        ftlm.ftlm_set_option(ctx, key, val)
     kernel_used = {1: "row", 2: "tile", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
+    n_windows = max(ftlm.ftlm_get_option(ctx, "passb_windows"), 0) if kernel_used == "tml" else 0
     D = ftlm.ftlm_dim(ctx)
     K, Wm = args.steps, args.warmup
     assert 1 <= K and K + Wm <= ftlm.MAX_STEPS, "steps + warmup must be <= 1024 (one chain)"
@@ -226,7 +289,7 @@ def main():
     alg_bytes = 12 * D + table_bytes             # floor A of SURVEY 8(d): v, v_prev, y + table
     peak, peak_src = measured_peak()
     achieved = alg_bytes / (ms_hv * 1e-3) / 1e9
-    kname = f"hv_{kernel_used}_{args.mode}_fp32_fused"
+    kname = f"hv_{kernel_used}_{args.mode}_fp32_fused" + (f"+passb{n_windows}" if n_windows else "")
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": recorded_traffic(kname), "kernel": kname, "ms_per_launch": ms_hv,
                 "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
@@ -275,11 +338,12 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"config{args.config}:{w.name}", "N": w.N, "N_up": n_up, "dim": D,
-                       "n_bonds": w.n_bonds, "index_mode": args.mode, "kernel": kernel_used,
+                       "n_bonds": w.n_bonds, "index_mode": args.mode, "kernel": kernel_used, "candidate": choice,
+                       "hv_passes": 1 + n_windows, "autotune": autotune_report, "probe_note": probe_note,
                        "precision": "fp32 vectors, fp64 reductions", "l2": "inputs_exceed_l2 (3 x 620 MB vectors)",
                        "parallelism": f"replicas x{world}"},
             "hv_rows_per_s": world * D / (ms_hv * 1e-3), "hv_gelem_per_s": world * nnz / (ms_hv * 1e-3) / 1e9,
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": 2 * K,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": (2 + n_windows) * K,
             "clocks": sampler.summary()}
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -134,6 +134,16 @@ int ftlm_chain_end(ftlm_ctx* ctx, double* h_alpha, double* h_beta, int cap, int*
  * (ms) of the fused H.v kernel and of the normalisation kernel.  Synchronous; for bench.py. */
 int ftlm_chain_profile(ftlm_ctx* ctx, int nsteps, void* stream, double* ms_hv, double* ms_norm);
 
+/* Choose the H.v kernel configuration of the handle by measurement on the device (DESIGN.md
+ * section 7.1).  Each candidate computes y = H v for one seeded random vector and is compared on
+ * the device with the thread-per-row kernel (Eq. 12 with Alg. 1 / Alg. 2 as printed, L105-L173);
+ * candidates beyond the H.v tolerance (1e-5 FP32, 1e-12 FP64, norm-relative) are rejected, the
+ * others are timed over `reps` launches (CUDA events) and the fastest is left selected.
+ * report (host, caller-owned, may be NULL): JSON list of {name, valid, relerr, ms, windows}.
+ * Allocates and frees 3 vectors of dim elements.  Synchronous.  FTLM_EUNSUPPORTED if no
+ * candidate is valid (the handle keeps its previous selection). */
+int ftlm_autotune(ftlm_ctx* ctx, int reps, char* report, int report_cap, void* stream);
+
 #define FTLM_MAX_STEPS 1024
 
 /* Whole sector: R chains from seeded starts r = 0..R-1, n_steps each, then the Ritz pairs.

@@ -1,0 +1,139 @@
+// ftlm_autotune - choose the H.v kernel configuration of a handle by measurement, on the device.
+//
+// Every candidate (ROW, TILE, TML with its bonds that leave the tile read from global memory, TML +
+// PASS-B windows in several window sizes) first computes y = H v for one seeded random vector and is
+// compared, on the device, with the ROW kernel's result (the paper's launch shape, thread per row,
+// Eq. 12 / Alg. 1 / Alg. 2 directly): a candidate whose norm-relative deviation exceeds the
+// north_star tolerance (1e-5 FP32, 1e-12 FP64) is rejected.  The valid candidates are timed with
+// CUDA events over `reps` launches and the fastest is left selected in the handle.  All arithmetic
+// is in the library's kernels; nothing here runs on the CPU.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "ftlm_common.cuh"
+
+namespace {
+
+template <typename R>
+__global__ void __launch_bounds__(256)
+diff_norm_kernel(const R* __restrict__ a, const R* __restrict__ ref, int64_t n, double* __restrict__ out) {
+  double d2 = 0.0, r2 = 0.0;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+    const double x = (double)a[k], y = (double)ref[k];
+    const double d = x - y;
+    d2 += (d == d) ? d * d : 1e300;                    // a NaN in the candidate counts as a huge deviation
+    r2 += y * y;
+  }
+  d2 = warp_sum(d2);
+  r2 = warp_sum(r2);
+  if ((threadIdx.x & 31) == 0) { atomicAdd(&out[0], d2); atomicAdd(&out[1], r2); }
+}
+
+struct Cand {
+  const char* name;
+  int kernel, passb, smax, ctas;
+};
+
+int apply_cand(ftlm_ctx* c, const Cand& k) {
+  int rc;
+  if (k.kernel == FTLM_KERNEL_TML) {
+    if ((rc = ftlm_set_option(c, "passb_smax", k.smax)) != FTLM_OK) return rc;
+    if ((rc = ftlm_set_option(c, "passb_ctas", k.ctas)) != FTLM_OK) return rc;
+    if ((rc = ftlm_set_option(c, "passb", k.passb)) != FTLM_OK) return rc;
+  }
+  return ftlm_set_option(c, "kernel", k.kernel);
+}
+
+}  // namespace
+
+extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap, void* stream) {
+  if (!c || reps < 1) { ftlm_set_error("ftlm_autotune: bad argument"); return FTLM_EINVAL; }
+  CK(cudaSetDevice(c->device));
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t esz = ftlm_elem_size(c), bytes = (size_t)c->dim * esz;
+  void *v = nullptr, *yref = nullptr, *y = nullptr;
+  double* d_out = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  std::string rep = "[";
+  int rc = FTLM_OK;
+  auto cleanup = [&]() {
+    cudaFree(v); cudaFree(yref); cudaFree(y); cudaFree(d_out);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+  };
+  if (cudaMalloc(&v, bytes) != cudaSuccess || cudaMalloc(&yref, bytes) != cudaSuccess || cudaMalloc(&y, bytes) != cudaSuccess ||
+      cudaMalloc((void**)&d_out, 16) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+    cudaGetLastError(); cleanup();
+    ftlm_set_error("ftlm_autotune: cannot allocate 3 x %zu bytes", bytes);
+    return FTLM_ENOMEM;
+  }
+  const int saved_kernel = c->kernel, saved_pb = c->use_passb, saved_smax = c->passb_smax, saved_ctas = c->passb_ctas;
+  const Cand cands[] = {
+      {"row", FTLM_KERNEL_ROW, 0, 0, 0},
+      {"tile", FTLM_KERNEL_TILE, 0, 0, 0},
+      {"tml", FTLM_KERNEL_TML, 0, 0, 0},
+      {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0},
+      {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1},
+      {"tml+passb_s11", FTLM_KERNEL_TML, 1, 11, 0},
+      {"tml+passb_s10", FTLM_KERNEL_TML, 1, 10, 0},
+  };
+  const int ncand = (int)(sizeof(cands) / sizeof(cands[0]));
+  const double tol = c->prec == FTLM_FP32 ? 1e-5 : 1e-12;
+  int best = -1;
+  double best_ms = 0.0;
+  // reference: the ROW kernel on a seeded random vector
+  rc = ftlm_fill_random(c, 0x5EEDull, 0, v, s);
+  if (rc == FTLM_OK) rc = apply_cand(c, cands[0]);
+  if (rc == FTLM_OK) rc = ftlm_apply_H(c, v, yref, s);
+  for (int k = 0; k < ncand && rc == FTLM_OK; ++k) {
+    const Cand& cd = cands[k];
+    if (cd.kernel == FTLM_KERNEL_TILE && !c->tile) continue;
+    if (apply_cand(c, cd) != FTLM_OK) continue;                          // not available for this sector
+    if (cd.kernel == FTLM_KERNEL_TML && (!c->tml || (cd.passb && !c->passb))) continue;
+    double h_out[2] = {0.0, 0.0};
+    if (cudaMemsetAsync(d_out, 0, 16, s) != cudaSuccess) { rc = FTLM_ECUDA; break; }
+    if ((rc = ftlm_apply_H(c, v, y, s)) != FTLM_OK) break;
+    const int grid = c->sm_count * 8;
+    if (c->prec == FTLM_FP32) { auto kk = diff_norm_kernel<float>; FTLM_LAUNCH(kk, grid, 256, 0, s, (const float*)y, (const float*)yref, c->dim, d_out); }
+    else { auto kk = diff_norm_kernel<double>; FTLM_LAUNCH(kk, grid, 256, 0, s, (const double*)y, (const double*)yref, c->dim, d_out); }
+    if (cudaMemcpyAsync(h_out, d_out, 16, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
+      rc = ftlm_cuda_fail(cudaGetLastError(), "ftlm_autotune: candidate run"); break;
+    }
+    const double rel = h_out[1] > 0.0 ? std::sqrt(h_out[0] / h_out[1]) : (h_out[0] > 0.0 ? 1.0 : 0.0);
+    const bool valid = rel <= tol;
+    float ms = 0.f;
+    if (valid) {
+      cudaEventRecord(e0, s);
+      for (int r = 0; r < reps && rc == FTLM_OK; ++r) rc = ftlm_apply_H(c, v, y, s);
+      cudaEventRecord(e1, s);
+      if (rc != FTLM_OK) break;
+      if (cudaEventSynchronize(e1) != cudaSuccess) { rc = ftlm_cuda_fail(cudaGetLastError(), "ftlm_autotune: timing"); break; }
+      cudaEventElapsedTime(&ms, e0, e1);
+      ms /= (float)reps;
+      if (best < 0 || ms < best_ms) { best = k; best_ms = ms; }
+    }
+    char line[256];
+    snprintf(line, sizeof(line), "%s{\"name\": \"%s\", \"valid\": %s, \"relerr\": %.3e, \"ms\": %.5f, \"windows\": %d}",
+             rep.size() > 1 ? ", " : "", cd.name, valid ? "true" : "false", rel, (double)ms,
+             (cd.kernel == FTLM_KERNEL_TML && c->passb) ? ftlm_passb_windows(c) : 0);
+    rep += line;
+  }
+  rep += "]";
+  if (rc == FTLM_OK && best >= 0) rc = apply_cand(c, cands[best]);
+  else {                                                                  // restore what the caller had
+    c->passb_smax = saved_smax; c->passb_ctas = saved_ctas;
+    ftlm_set_option(c, "passb", saved_pb);
+    c->kernel = saved_kernel;
+    if (rc == FTLM_OK) { ftlm_set_error("ftlm_autotune: no valid candidate"); rc = FTLM_EUNSUPPORTED; }
+  }
+  if (rc == FTLM_OK) { c->autotuned = best + 1; c->autotune_ms = best_ms; }
+  if (report && report_cap > 0) {
+    strncpy(report, rep.c_str(), (size_t)report_cap - 1);
+    report[report_cap - 1] = 0;
+  }
+  cleanup();
+  return rc;
+}

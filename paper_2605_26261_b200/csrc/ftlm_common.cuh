@@ -77,6 +77,8 @@ struct ftlm_ctx {
   int low_bits = 0;
   int tml_low_bits = 0, tml_mid_bits = 0;
   int use_graph = 0;
+  int autotuned = 0;               // 1 + index of the candidate ftlm_autotune selected (0 = not tuned)
+  double autotune_ms = 0.0;
 
   // tile plan (ftlm_tile.cu)
   TilePlan* tile = nullptr;
@@ -84,9 +86,14 @@ struct ftlm_ctx {
   TmlPlan* tml = nullptr;
   // PASS-B windows for the bonds among the top label bits (ftlm_passb.cu); owned together with `tml`
   PassBSet* passb = nullptr;
-  int use_passb = 1;               // option "passb": 0 keeps every bond that leaves the tile in the TML kernel
+  int use_passb = 0;               // option "passb": 1 moves the bonds that leave the tile into PASS-B windows (ftlm_autotune turns it on when it is valid and faster)
   int passb_lo_min = 0;            // option "passb_lo_min": lowest label position a window may use (0 = auto)
   int passb_smax = 0;              // option "passb_smax": largest window (0 = auto: 12 FP32 / 11 FP64)
+  // test hooks (tests/emu runs sampled tiles / items of full-size sectors on the host): run only the
+  // passes in the mask (bit 0 = TML pass, bit k+1 = PASS-B window k; 0 = all) and only the tiles /
+  // items [first, first + count) (count 0 = all).  Non-fused H.v only.
+  int debug_pass_mask = 0;
+  int64_t debug_item_first = 0, debug_item_count = 0;
   int passb_ctas = 0;              // option "passb_ctas": CTAs per SM tried first (0 = auto: 2)
 
   // chain workspace

@@ -319,6 +319,9 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     return rc;
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
+  if (!strcmp(key, "debug_pass_mask")) { c->debug_pass_mask = (int)value; return FTLM_OK; }
+  if (!strcmp(key, "debug_item_first")) { c->debug_item_first = value; return FTLM_OK; }
+  if (!strcmp(key, "debug_item_count")) { c->debug_item_count = value; return FTLM_OK; }
   if (!strcmp(key, "passb") || !strcmp(key, "tml_split")) {
     // "passb": 0/1;  "tml_split": w | m << 8 (both at once; 0 = auto).  Rebuilds the TML / PASS-B plans.
     const int old_pb = c->use_passb, old_w = c->tml_low_bits, old_m = c->tml_mid_bits;
@@ -360,6 +363,7 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "passb")) return c->use_passb;
   if (!strncmp(key, "passb_", 6)) return ftlm_passb_info(c, key);
   if (!strcmp(key, "sm_count")) return c->sm_count;
+  if (!strcmp(key, "autotuned")) return c->autotuned;
   if (!strncmp(key, "tml_", 4)) return ftlm_tml_info(c, key);
   return -1;
 }
@@ -381,7 +385,8 @@ static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fu
   if (k == FTLM_KERNEL_TML) {
     // two-pass step when PASS-B windows exist: the TML pass leaves the sums and the finish to PASS-B
     const bool pb = c->passb != nullptr;
-    int rc = ftlm_launch_hv_tml(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, 1, s);
+    int rc = FTLM_OK;
+    if (fused || !c->debug_pass_mask || (c->debug_pass_mask & 1)) rc = ftlm_launch_hv_tml(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, 1, s);
     if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, s);
     return rc;
   }

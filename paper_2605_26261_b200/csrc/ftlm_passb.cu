@@ -29,6 +29,7 @@ template <typename R>
 struct PassBParams {
   int N, K, lo, s, f, ngroups;
   uint32_t nitems;
+  uint32_t item_begin, item_end;    // items handed out: [item_begin, item_end)  (all unless option "debug_items")
   uint64_t smask_hi, fmask_hi;      // active / frozen positions of the label >> lo
   int64_t dim;
   const uint64_t* binom;            // [(N+1)*(K+1)] global
@@ -111,8 +112,8 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     __syncthreads();                                   // previous item done: tile, starts reusable
     if (tid == 0) s_item = atomicAdd(&p.counter[0], 1u);
     __syncthreads();
-    const uint32_t item = s_item;
-    if (item >= p.nitems) break;
+    const uint32_t item = s_item + p.item_begin;
+    if (item >= p.item_end) break;
     // group of this item: last g with grp_first[g] <= item (uniform binary search)
     int g0 = 0, g1 = p.ngroups;
     while (g1 - g0 > 1) {
@@ -299,6 +300,7 @@ int64_t ftlm_passb_info(const ftlm_ctx* c, const char* key) {
   if (!strncmp(key, "passb_lo", 8) && key[8] >= '0' && key[8] <= '7') { const size_t k = (size_t)(key[8] - '0'); return k < S->win.size() ? S->win[k].lo : -1; }
   if (!strncmp(key, "passb_mask", 10) && key[10] >= '0' && key[10] <= '7') { const size_t k = (size_t)(key[10] - '0'); return k < S->win.size() ? (int64_t)S->win[k].smask : -1; }
   if (!strncmp(key, "passb_nbonds", 12) && key[12] >= '0' && key[12] <= '7') { const size_t k = (size_t)(key[12] - '0'); return k < S->win.size() ? (int64_t)S->win[k].bonds.size() : -1; }
+  if (!strncmp(key, "passb_items", 11) && key[11] >= '0' && key[11] <= '7') { const size_t k = (size_t)(key[11] - '0'); return k < S->win.size() ? (int64_t)S->win[k].nitems : -1; }
   if (!strcmp(key, "passb_ctas_used")) return S->win[0].ctas;
   if (!strcmp(key, "passb_lo")) return S->win[0].lo;
   if (!strcmp(key, "passb_s")) return S->win[0].s;
@@ -493,8 +495,13 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   p.fmask_hi = (c->N >= 64 ? ~0ull : ((1ull << c->N) - 1ull)) >> w.lo & ~p.smask_hi;
   for (int k = 0; k <= PASSB_MAX_S; ++k) p.xk[k] = w.xk[k];
   for (size_t e = 0; e < w.Jh.size(); ++e) p.Jh[e] = (R)w.Jh[e];
+  p.item_begin = 0; p.item_end = w.nitems;
+  if (c->debug_item_count > 0) {
+    p.item_begin = (uint32_t)std::min<int64_t>(c->debug_item_first, w.nitems);
+    p.item_end = (uint32_t)std::min<int64_t>(c->debug_item_first + c->debug_item_count, w.nitems);
+  }
   int grid = c->sm_count * w.ctas;
-  if ((uint32_t)grid > w.nitems) grid = (int)w.nitems;
+  if ((uint32_t)grid > p.item_end - p.item_begin) grid = (int)std::max(1u, p.item_end - p.item_begin);
   if (fused) {
     auto k = passb_kernel<R, MODE, true>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
@@ -513,6 +520,7 @@ int ftlm_launch_passb(ftlm_ctx* c, const void* v, void* y, int fused, cudaStream
   if (!S) return FTLM_OK;
   for (size_t wi = 0; wi < S->win.size(); ++wi) {
     PassBWindow& w = S->win[wi];
+    if (!fused && c->debug_pass_mask && !((c->debug_pass_mask >> (wi + 1)) & 1)) continue;
     const int fz = (fused && wi + 1 == S->win.size()) ? 1 : 0;
     int rc;
     if (c->prec == FTLM_FP32)

@@ -29,6 +29,7 @@
 // neighbouring tiles and flips of low T bits hit L2; per-tile FP64 partial sums are written to a
 // buffer indexed by T and added in fixed order by the last CTA (bit-reproducible alpha, beta).
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <type_traits>
 #include <vector>
@@ -47,6 +48,7 @@ template <typename R>
 struct TmlParams {
   int N, K, w, m, t, mw, mode;
   uint32_t nT;
+  uint32_t t_begin, t_end;            // tiles handed out: [t_begin, t_end)  (all of [0, nT) unless option "debug_items")
   int n_ll4, n_mm, n_ml, n_tt, n_ts, n_tm, n_tl;
   int max_tile, scratch_bytes;
   int64_t dim;
@@ -86,6 +88,7 @@ struct TmlPlan {
   std::vector<uint32_t> tt_mask;
   std::vector<uint8_t> ts_site;
   std::vector<TmlSEnt> mm, ml, tm, tl;
+  std::vector<int> h_bond_class, h_bond_entry;   // host copies (option "tml_bclass:<b>")
 };
 
 namespace {
@@ -265,8 +268,8 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
     __syncthreads();                                   // previous tile done: smem reusable
     if (tid == 0) S.misc[0] = (int)atomicAdd(&p.counter[0], 1u);
     __syncthreads();
-    const uint32_t T = (uint32_t)S.misc[0];
-    if (T >= p.nT) break;
+    const uint32_t T = (uint32_t)S.misc[0] + p.t_begin;
+    if (T >= p.t_end) break;
     const int kT = p.K - __popc(T);
     if (kT < 0 || kT > p.mw) continue;                  // no rows with this top part
     // ---- per-tile uniform data ----------------------------------------------------------------
@@ -678,7 +681,12 @@ template <typename R>
 void fill_params(const ftlm_ctx* c, const TmlPlan* t, TmlParams<R>& p, int batch) {
   memset(&p, 0, sizeof(p));
   p.N = c->N; p.K = c->N_up; p.w = t->w; p.m = t->m; p.t = t->t; p.mw = t->w + t->m; p.mode = c->mode;
-  p.nT = t->nT; p.n_ll4 = t->n_ll4; p.n_mm = t->n_mm; p.n_ml = t->n_ml; p.n_tt = t->n_tt; p.n_ts = t->n_ts;
+  p.nT = t->nT; p.t_begin = 0; p.t_end = t->nT;
+  if (c->debug_item_count > 0) {
+    p.t_begin = (uint32_t)std::min<int64_t>(c->debug_item_first, t->nT);
+    p.t_end = (uint32_t)std::min<int64_t>(c->debug_item_first + c->debug_item_count, t->nT);
+  }
+  p.n_ll4 = t->n_ll4; p.n_mm = t->n_mm; p.n_ml = t->n_ml; p.n_tt = t->n_tt; p.n_ts = t->n_ts;
   p.n_tm = t->n_tm; p.n_tl = t->n_tl;
   p.max_tile = t->max_tile;
   p.scratch_bytes = tml_scratch_bytes((int)sizeof(R), t->n_tt, t->n_tm, t->n_mm, t->n_ml, t->n_tl);
@@ -722,7 +730,7 @@ int launch_tml(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, c
   TmlParams<R> p;
   fill_params<R>(c, t, p, B);
   int grid = c->sm_count * cfg.ctas;
-  if ((uint32_t)grid > t->nT) grid = (int)t->nT;
+  if ((uint32_t)grid > p.t_end - p.t_begin) grid = (int)std::max(1u, p.t_end - p.t_begin);
   if (fused == 1) {
     auto k = hv_tml_kernel<R, B, MODE, 1>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
@@ -906,6 +914,7 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
   P->off_tm = put(P->tm.data(), P->tm.size() * sizeof(TmlSEnt));
   P->off_tl = put(P->tl.data(), P->tl.size() * sizeof(TmlSEnt));
   P->blob_bytes = (int)blob.size();
+  P->h_bond_class = bclass; P->h_bond_entry = bentry;
   c->tml = P;
   if (tml_config(c, P, 1).smem == 0) { c->tml = nullptr; ftlm_passb_plan_destroy(c); delete P; return unusable("tables + tile exceed shared memory"); }
   // ---- upload ----------------------------------------------------------------------------------
@@ -930,6 +939,12 @@ int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key) {
   const TmlPlan* t = c->tml;
   if (!t) return -1;
   if (!strcmp(key, "tml_w")) return t->w;
+  if (!strcmp(key, "tml_tiles")) return (int64_t)t->nT;
+  if (!strncmp(key, "tml_bclass:", 11)) {                 // class | entry << 8 of bond b (class 6 = PASS-B window `entry`)
+    const int b = atoi(key + 11);
+    if (b < 0 || b >= (int)t->h_bond_class.size()) return -1;
+    return (int64_t)t->h_bond_class[(size_t)b] | ((int64_t)t->h_bond_entry[(size_t)b] << 8);
+  }
   if (!strcmp(key, "tml_m")) return t->m;
   if (!strcmp(key, "tml_smem")) return (int64_t)tml_config(c, t, 1).smem;
   if (!strcmp(key, "tml_ctas_per_sm")) return tml_config(c, t, 1).ctas;

@@ -24,7 +24,7 @@ EXPORTS = [
     "ftlm_create", "ftlm_destroy", "ftlm_dim", "ftlm_set_option", "ftlm_get_option", "ftlm_table_bytes",
     "ftlm_clt_read", "ftlm_index_of", "ftlm_state_of", "ftlm_neighbors", "ftlm_apply_H",
     "ftlm_apply_H_host", "ftlm_fill_random", "ftlm_chain_begin", "ftlm_chain_steps", "ftlm_chain_end",
-    "ftlm_chain_profile", "ftlm_lanczos", "ftlm_lanczos_host", "ftlm_tridiag_eig", "ftlm_thermo",
+    "ftlm_chain_profile", "ftlm_autotune", "ftlm_lanczos", "ftlm_lanczos_host", "ftlm_tridiag_eig", "ftlm_thermo",
     "ftlm_last_error", "ftlm_version",
 ]
 
@@ -168,6 +168,14 @@ def ftlm_chain_profile(ctx, nsteps: int, stream=None):
     x, y = C.c_double(0), C.c_double(0)
     _check(lib().ftlm_chain_profile(ctx, C.c_int(nsteps), _stream(stream), C.byref(x), C.byref(y)))
     return x.value, y.value
+
+
+def ftlm_autotune(ctx, reps: int = 3, stream=None):
+    """Measure the kernel candidates on the device, keep the fastest valid one; returns the report list."""
+    import json
+    buf = C.create_string_buffer(8192)
+    _check(lib().ftlm_autotune(ctx, C.c_int(reps), buf, C.c_int(len(buf)), _stream(stream)))
+    return json.loads(buf.value.decode())
 
 
 def _lanczos_out(R, n_steps):

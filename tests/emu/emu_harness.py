@@ -80,6 +80,28 @@ class EmuCtx:
         _check(lib().ftlm_apply_H(self.ctx, _p(v), _p(y), C.c_void_p(0)))
         return y
 
+    def apply_into(self, v, y):
+        """y is read-modify-written when only PASS-B windows run (option debug_pass_mask)."""
+        assert v.dtype == NDT[self.prec] and y.dtype == NDT[self.prec] and v.flags.c_contiguous and y.flags.c_contiguous
+        _check(lib().ftlm_apply_H(self.ctx, _p(v), _p(y), C.c_void_p(0)))
+
+    def bond_classes(self):
+        """[(class, entry)] per bond from the TML plan; class 6 = PASS-B window `entry`."""
+        out = []
+        for b in range(self.w.n_bonds):
+            x = self.get(f"tml_bclass:{b}")
+            out.append((x & 0xff, x >> 8))
+        return out
+
+    def diag0(self):
+        return float(np.sum(self.w.J if self.w is not None else 0.0)) / 4.0
+
+    def autotune(self, reps=1):
+        import json
+        buf = C.create_string_buffer(8192)
+        _check(lib().ftlm_autotune(self.ctx, C.c_int(reps), buf, C.c_int(len(buf)), C.c_void_p(0)))
+        return json.loads(buf.value.decode())
+
     def neighbors(self, row0, nrows):
         nb = max(self.w.n_bonds, 1)
         out = np.full(nrows * nb, -7, dtype=np.int64)

@@ -90,7 +90,7 @@ def test_emu_guard_pages_catch_overrun():
 def test_emu_two_pass_tml_plus_passb(wl, n_up, w, m, mode, prec, what):
     """PASS-B (bonds among the top label bits streamed by window) + the TML pass that leaves them out."""
     res = run_case({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec,
-                    "options": [["tml_split", w | (m << 8)], ["kernel", K["tml"]]], "what": what, "steps": 6},
+                    "options": [["passb", 1], ["tml_split", w | (m << 8)], ["kernel", K["tml"]]], "what": what, "steps": 6},
                    timeout=1500)
     assert res["kernel"] == K["tml"] and res["passb"][0] >= 1 and res["passb"][1] >= 3
     if wl == "ring20j":
@@ -106,7 +106,7 @@ def test_emu_two_pass_tml_plus_passb(wl, n_up, w, m, mode, prec, what):
 def test_emu_generalised_windows(wl, n_up, split, mode, prec, opts, nwin, what):
     """PASS-B windows as arbitrary sets of label positions >= lo_min chosen by the greedy cover."""
     res = run_case({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec,
-                    "options": opts + [["tml_split", split], ["kernel", K["tml"]]], "what": what, "steps": 6},
+                    "options": [["passb", 1]] + opts + [["tml_split", split], ["kernel", K["tml"]]], "what": what, "steps": 6},
                    timeout=1500)
     assert res["kernel"] == K["tml"] and res["passb"][0] >= nwin
 
@@ -116,3 +116,34 @@ def test_emu_passb_off_keeps_top_bonds_in_tml():
                     "options": [["passb", 0], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]],
                     "what": ["neighbors", "apply"]})
     assert res["passb"][0] == 0
+
+
+def test_emu_autotune_checks_every_candidate_against_row():
+    """ftlm_autotune: every candidate is compared with the ROW kernel on the (emulated) device and timed."""
+    code = ("import sys, json; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+            "import emu_harness as E\n"
+            "from paper_2605_26261_b200 import workloads as W\n"
+            "w = W.ring(16, 1.0, 0.5)\n"
+            "with E.EmuCtx(w, 8, 'cr', 'fp32', options=[('passb_lo_min', 4), ('tml_split', 5 | (3 << 8))]) as c:\n"
+            "    rep = c.autotune(1)\n"
+            "    print(json.dumps({'rep': rep, 'tuned': c.get('autotuned')}))\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    d = json.loads(p.stdout.strip().splitlines()[-1])
+    names = [r["name"] for r in d["rep"]]
+    assert names[0] == "row" and "tml" in names and "tml+passb" in names
+    assert all(r["valid"] and r["relerr"] <= 1e-5 for r in d["rep"]) and d["tuned"] >= 1
+
+
+def test_emu_config4_full_size_sampled_tiles_and_items():
+    """BASELINE config 4 (D = 155 117 520) at full size: sampled tiles of the TML pass and sampled items of
+    both PASS-B windows run through the emulation with the real run starts and offsets; the rows each
+    pass writes and their values must be the oracle's (and nothing may touch a guard page)."""
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "tests", "emu", "run_sampled.py"),
+                        json.dumps({"config": 4, "mode": "cr", "samples": 1})],
+                       capture_output=True, text=True, timeout=1500)
+    assert p.returncode == 0, p.stderr[-2000:]
+    d = json.loads(p.stdout.strip().splitlines()[-1])
+    assert d["ok"] and d["windows"] == 2 and d["kernel"] == K["tml"], d
+    assert {x["pass"] for x in d["passes"]} == {0, 1, 2}
+    assert all(x["ok"] for x in d["passes"])
