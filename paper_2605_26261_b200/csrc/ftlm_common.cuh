@@ -148,6 +148,25 @@ __device__ __forceinline__ int popc_(uint64_t x) { return __popcll(x); }
 __device__ __forceinline__ int ffs_(uint32_t x) { return __ffs((int)x); }
 __device__ __forceinline__ int ffs_(uint64_t x) { return __ffsll((long long)x); }
 
+// asynchronous global -> shared copy of one element (LDGSTS); the emulation copies at once
+template <typename T>
+__device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc) {
+#ifdef FTLM_EMU
+  *smem_dst = *gsrc;
+#else
+  static_assert(sizeof(T) == 4 || sizeof(T) == 8 || sizeof(T) == 16, "cp.async copies 4, 8 or 16 bytes");
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if (sizeof(T) == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gsrc) : "memory");
+  else if (sizeof(T) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+  else asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+#endif
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+#ifndef FTLM_EMU
+  asm volatile("cp.async.wait_all;" ::: "memory");
+#endif
+}
+
 __device__ __forceinline__ double warp_sum(double x) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);

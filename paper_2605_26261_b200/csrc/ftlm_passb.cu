@@ -24,6 +24,8 @@
 #define PASSB_MAX_S 12
 #define PASSB_THREADS 1024
 #define PASSB_END 0xFFFFFFFFu
+#define PASSB_XK 2                  // run offsets per lane and window word (X = 32 * xk, xk <= PASSB_XK)
+#define PASSB_PF 8                  // window words whose y is in flight per warp
 
 template <typename R>
 struct PassBParams {
@@ -140,59 +142,70 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     }
     const uint64_t left = RL - x0;                      // rows of the run at or after x0 (> 0)
     const int nx = left < (uint64_t)X ? (int)left : X;  // valid offsets in this chunk
-    // ---- phase 1: stage the run chunks ----------------------------------------------------------
+    // ---- phase 1: stage the run chunks (cp.async: every copy of the item is in flight at once) ------
     for (int sl = warp; sl < nconf; sl += NW) {
       const R* src = v + s_start[sl] + x0;
       R* dst = tile + (size_t)sl * X;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
+      for (int k = 0; k < PASSB_XK; ++k) {
         const int x = lane + 32 * k;
-        if (k < XK && x < nx) dst[x] = __ldg(&src[x]);
+        if (k < XK && x < nx) cp_async_elem(&dst[x], &src[x]);
       }
     }
+    cp_async_wait_all();
     __syncthreads();
-    // ---- phase 2: one warp per window word ------------------------------------------------------
+    // ---- phase 2: one warp per window word; y of PASSB_PF words is requested before the first is used ---
     double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
-    for (int sl = warp; sl < nconf; sl += NW) {
-      const uint32_t u = __ldg(&p.ustate[c0 + sl]);
-      const uint32_t ent = __ldg(&p.nbr[(size_t)u * 32 + lane]);
-      const int cnt = __popc(__ballot_sync(0xffffffffu, ent != PASSB_END));
-      const R* row = tile + (size_t)sl * X;
-      R* yrow = y + s_start[sl] + x0;
-      R own[4], acc[4], yold[4];
+    for (int sl0 = warp; sl0 < nconf; sl0 += NW * PASSB_PF) {
+      R yold[PASSB_PF][PASSB_XK];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {                      // y is read first: its latency hides behind the bond loop
-        const int x = lane + 32 * k;
-        yold[k] = (k < XK && x < nx) ? __ldcs(&yrow[x]) : (R)0;
-      }
+      for (int j = 0; j < PASSB_PF; ++j) {
+        const int sl = sl0 + j * NW;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const int x = lane + 32 * k;
-        own[k] = (k < XK && x < nx) ? row[x] : (R)0;
-        acc[k] = (R)0;
-      }
-      R sumJ = (R)0;
-      for (int e = 0; e < cnt; ++e) {
-        const uint32_t en = __shfl_sync(0xffffffffu, ent, e);
-        const R J = p.Jh[en >> 16];
-        const R* nrow = tile + (size_t)(en & 0xffffu) * X;
-        sumJ += J;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < PASSB_XK; ++k) {
           const int x = lane + 32 * k;
-          if (k < XK && x < nx) acc[k] += J * nrow[x];
+          yold[j][k] = (sl < nconf && k < XK && x < nx) ? __ldcs(y + s_start[sl] + x0 + x) : (R)0;
         }
       }
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const int x = lane + 32 * k;
-        if (k < XK && x < nx) {
-          const R yn = yold[k] + (acc[k] - sumJ * own[k]);
-          __stcs(&yrow[x], yn);
-          if (FUSED) {
-            s_qy += (double)own[k] * (double)yn;
-            s_yy += (double)yn * (double)yn;
-            s_qq += (double)own[k] * (double)own[k];
+      for (int j = 0; j < PASSB_PF; ++j) {
+        const int sl = sl0 + j * NW;
+        if (sl >= nconf) break;
+        const uint32_t u = __ldg(&p.ustate[c0 + sl]);
+        const uint32_t ent = __ldg(&p.nbr[(size_t)u * 32 + lane]);
+        const int cnt = __popc(__ballot_sync(0xffffffffu, ent != PASSB_END));
+        const R* row = tile + (size_t)sl * X;
+        R* yrow = y + s_start[sl] + x0;
+        R own[PASSB_XK], acc[PASSB_XK];
+#pragma unroll
+        for (int k = 0; k < PASSB_XK; ++k) {
+          const int x = lane + 32 * k;
+          own[k] = (k < XK && x < nx) ? row[x] : (R)0;
+          acc[k] = (R)0;
+        }
+        R sumJ = (R)0;
+        for (int e = 0; e < cnt; ++e) {
+          const uint32_t en = __shfl_sync(0xffffffffu, ent, e);
+          const R J = p.Jh[en >> 16];
+          const R* nrow = tile + (size_t)(en & 0xffffu) * X;
+          sumJ += J;
+#pragma unroll
+          for (int k = 0; k < PASSB_XK; ++k) {
+            const int x = lane + 32 * k;
+            if (k < XK && x < nx) acc[k] += J * nrow[x];
+          }
+        }
+#pragma unroll
+        for (int k = 0; k < PASSB_XK; ++k) {
+          const int x = lane + 32 * k;
+          if (k < XK && x < nx) {
+            const R yn = yold[j][k] + (acc[k] - sumJ * own[k]);
+            __stcs(&yrow[x], yn);
+            if (FUSED) {
+              s_qy += (double)own[k] * (double)yn;
+              s_yy += (double)yn * (double)yn;
+              s_qq += (double)own[k] * (double)own[k];
+            }
           }
         }
       }
@@ -342,7 +355,7 @@ static bool passb_geometry(const ftlm_ctx* c, PassBWindow& w, std::vector<uint32
       w.xk[p] = 0;
       if (!used[(size_t)p]) continue;
       const size_t per32 = (size_t)binom_b(w.s, p) * 32 * (size_t)esz;
-      int xk = (int)std::min<size_t>(4, budget / per32);
+      int xk = (int)std::min<size_t>(PASSB_XK, budget / per32);
       if (xk < 1) { fits = false; break; }
       w.xk[p] = xk;
       max_rows = std::max(max_rows, (int)binom_b(w.s, p) * 32 * xk);

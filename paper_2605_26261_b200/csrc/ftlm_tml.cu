@@ -432,6 +432,8 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         const unsigned char* pl = vsb0 + (size_t)lrc * RB;               // lane pointer: row lrc of column 0
         const unsigned char* flp = s_fl + Lidx * 2;
         const V own = *(const V*)(vsb + (size_t)lrc * RB);
+        V qp;                                             // q_prev: issued now, consumed in the epilogue
+        if (FUSED) qp = vec_ldcs(qprev + ((size_t)base + cb + lrc));
         V acc;
 #pragma unroll
         for (int b = 0; b < B; ++b) acc.x[b] = dcoef * own.x[b];
@@ -512,7 +514,6 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         if (valid) {
           const size_t g = (size_t)base + cb + lrc;
           if (FUSED) {
-            const V qp = vec_ldcs(qprev + g);
 #pragma unroll
             for (int b = 0; b < B; ++b) {
               acc.x[b] -= bprev.x[b] * qp.x[b];
