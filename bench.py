@@ -141,13 +141,15 @@ def run_reference(args, w, n_up):
 
 # name -> option settings, in order (the candidates of ftlm_autotune, include/ftlm.h)
 CANDIDATES = {
-    "row": [("kernel", 1)],
-    "tile": [("kernel", 2)],
-    "tml": [("passb", 0), ("kernel", 3)],
-    "tml+passb": [("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
-    "tml+passb_1cta": [("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
-    "tml+passb_s11": [("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
-    "tml+passb_s10": [("passb_smax", 10), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "row": [("tmlr", 0), ("kernel", 1)],
+    "tile": [("tmlr", 0), ("kernel", 2)],
+    "tml": [("tmlr", 0), ("passb", 0), ("kernel", 3)],
+    "tml+passb": [("tmlr", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tml+passb_1cta": [("tmlr", 0), ("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
+    "tml+passb_s11": [("tmlr", 0), ("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tml+passb_s10": [("tmlr", 0), ("passb_smax", 10), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tmlr+passb": [("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
+    "tmlr+passb_s11": [("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
 }
 SAFE_CHOICE = "tml"          # measured on B200 in round 1 (profiles/): the fallback if the probe dies
 
@@ -255,7 +257,9 @@ def main():
     for key, val in CANDIDATES[choice]:
         ftlm.ftlm_set_option(ctx, key, val)
     kernel_used = {1: "row", 2: "tile", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
-    n_windows = max(ftlm.ftlm_get_option(ctx, "passb_windows"), 0) if kernel_used == "tml" else 0
+    if kernel_used == "tml" and ftlm.ftlm_get_option(ctx, "tmlr") == 1 and ftlm.ftlm_get_option(ctx, "tmlr_available") == 1:
+        kernel_used = "tmlr"
+    n_windows = max(ftlm.ftlm_get_option(ctx, "passb_windows"), 0) if kernel_used in ("tml", "tmlr") else 0
     D = ftlm.ftlm_dim(ctx)
     K, Wm = args.steps, args.warmup
     assert 1 <= K and K + Wm <= ftlm.MAX_STEPS, "steps + warmup must be <= 1024 (one chain)"

@@ -1,7 +1,7 @@
 // ftlm_autotune - choose the H.v kernel configuration of a handle by measurement, on the device.
 //
 // Every candidate (ROW, TILE, TML with its bonds that leave the tile read from global memory, TML +
-// PASS-B windows in several window sizes) first computes y = H v for one seeded random vector and is
+// PASS-B windows in several window sizes, with the TML or the TMLR in-tile pass) first computes y = H v for one seeded random vector and is
 // compared, on the device, with the ROW kernel's result (the paper's launch shape, thread per row,
 // Eq. 12 / Alg. 1 / Alg. 2 directly): a candidate whose norm-relative deviation exceeds the
 // north_star tolerance (1e-5 FP32, 1e-12 FP64) is rejected.  The valid candidates are timed with
@@ -34,7 +34,7 @@ diff_norm_kernel(const R* __restrict__ a, const R* __restrict__ ref, int64_t n, 
 
 struct Cand {
   const char* name;
-  int kernel, passb, smax, ctas;
+  int kernel, passb, smax, ctas, tmlr;
 };
 
 int apply_cand(ftlm_ctx* c, const Cand& k) {
@@ -44,6 +44,7 @@ int apply_cand(ftlm_ctx* c, const Cand& k) {
     if ((rc = ftlm_set_option(c, "passb_ctas", k.ctas)) != FTLM_OK) return rc;
     if ((rc = ftlm_set_option(c, "passb", k.passb)) != FTLM_OK) return rc;
   }
+  if ((rc = ftlm_set_option(c, "tmlr", k.tmlr)) != FTLM_OK) return rc;
   return ftlm_set_option(c, "kernel", k.kernel);
 }
 
@@ -70,15 +71,17 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
     ftlm_set_error("ftlm_autotune: cannot allocate 3 x %zu bytes", bytes);
     return FTLM_ENOMEM;
   }
-  const int saved_kernel = c->kernel, saved_pb = c->use_passb, saved_smax = c->passb_smax, saved_ctas = c->passb_ctas;
+  const int saved_kernel = c->kernel, saved_pb = c->use_passb, saved_smax = c->passb_smax, saved_ctas = c->passb_ctas, saved_tmlr = c->use_tmlr;
   const Cand cands[] = {
-      {"row", FTLM_KERNEL_ROW, 0, 0, 0},
-      {"tile", FTLM_KERNEL_TILE, 0, 0, 0},
-      {"tml", FTLM_KERNEL_TML, 0, 0, 0},
-      {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0},
-      {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1},
-      {"tml+passb_s11", FTLM_KERNEL_TML, 1, 11, 0},
-      {"tml+passb_s10", FTLM_KERNEL_TML, 1, 10, 0},
+      {"row", FTLM_KERNEL_ROW, 0, 0, 0, 0},
+      {"tile", FTLM_KERNEL_TILE, 0, 0, 0, 0},
+      {"tml", FTLM_KERNEL_TML, 0, 0, 0, 0},
+      {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0, 0},
+      {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1, 0},
+      {"tml+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 0},
+      {"tml+passb_s10", FTLM_KERNEL_TML, 1, 10, 0, 0},
+      {"tmlr+passb", FTLM_KERNEL_TML, 1, 0, 0, 1},
+      {"tmlr+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 1},
   };
   const int ncand = (int)(sizeof(cands) / sizeof(cands[0]));
   const double tol = c->prec == FTLM_FP32 ? 1e-5 : 1e-12;
@@ -92,7 +95,7 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
     const Cand& cd = cands[k];
     if (cd.kernel == FTLM_KERNEL_TILE && !c->tile) continue;
     if (apply_cand(c, cd) != FTLM_OK) continue;                          // not available for this sector
-    if (cd.kernel == FTLM_KERNEL_TML && (!c->tml || (cd.passb && !c->passb))) continue;
+    if (cd.kernel == FTLM_KERNEL_TML && (!c->tml || (cd.passb && !c->passb) || (cd.tmlr && !c->tmlr))) continue;
     double h_out[2] = {0.0, 0.0};
     if (cudaMemsetAsync(d_out, 0, 16, s) != cudaSuccess) { rc = FTLM_ECUDA; break; }
     if ((rc = ftlm_apply_H(c, v, y, s)) != FTLM_OK) break;
@@ -124,7 +127,7 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
   rep += "]";
   if (rc == FTLM_OK && best >= 0) rc = apply_cand(c, cands[best]);
   else {                                                                  // restore what the caller had
-    c->passb_smax = saved_smax; c->passb_ctas = saved_ctas;
+    c->passb_smax = saved_smax; c->passb_ctas = saved_ctas; c->use_tmlr = saved_tmlr;
     ftlm_set_option(c, "passb", saved_pb);
     c->kernel = saved_kernel;
     if (rc == FTLM_OK) { ftlm_set_error("ftlm_autotune: no valid candidate"); rc = FTLM_EUNSUPPORTED; }

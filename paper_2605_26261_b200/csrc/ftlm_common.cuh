@@ -53,6 +53,7 @@ struct BondDev {          // one bond as the kernels see it
 struct TilePlan;
 struct TmlPlan;
 struct PassBSet;
+struct TmlrPlan;
 
 struct ftlm_ctx {
   int N = 0, nb = 0, N_up = 0, mode = 0, prec = 0, device = 0;
@@ -86,6 +87,10 @@ struct ftlm_ctx {
   TmlPlan* tml = nullptr;
   // PASS-B windows for the bonds among the top label bits (ftlm_passb.cu); owned together with `tml`
   PassBSet* passb = nullptr;
+  // in-tile pass with lane tables in registers (ftlm_tmlr.cu); exists only when every bond outside the
+  // PASS-B windows stays inside the tile.  Option "tmlr": 1 = use it for the in-tile pass of kernel TML.
+  TmlrPlan* tmlr = nullptr;
+  int use_tmlr = 0;
   int use_passb = 0;               // option "passb": 1 moves the bonds that leave the tile into PASS-B windows (ftlm_autotune turns it on when it is valid and faster)
   int passb_lo_min = 0;            // option "passb_lo_min": lowest label position a window may use (0 = auto)
   int passb_smax = 0;              // option "passb_smax": largest window (0 = auto: 12 FP32 / 11 FP64)
@@ -127,6 +132,11 @@ void ftlm_tml_plan_destroy(ftlm_ctx* c);
 int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key);
 int ftlm_launch_hv_tml(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, int batch, cudaStream_t s);
 int ftlm_launch_neighbors_tml(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
+
+int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_window);
+void ftlm_tmlr_plan_destroy(ftlm_ctx* c);
+int64_t ftlm_tmlr_info(const ftlm_ctx* c, const char* key);
+int ftlm_launch_hv_tmlr(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
 
 // PASS-B (ftlm_passb.cu).  `tt` lists the bonds whose two sites lie at positions >= mw (candidate
 // top-top bonds) as indices into c->bonds; on return window_of[k] is the PASS-B window that took

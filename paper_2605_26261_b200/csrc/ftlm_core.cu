@@ -319,6 +319,7 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     return rc;
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
+  if (!strcmp(key, "tmlr")) { c->use_tmlr = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "debug_pass_mask")) { c->debug_pass_mask = (int)value; return FTLM_OK; }
   if (!strcmp(key, "debug_item_first")) { c->debug_item_first = value; return FTLM_OK; }
   if (!strcmp(key, "debug_item_count")) { c->debug_item_count = value; return FTLM_OK; }
@@ -364,6 +365,8 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strncmp(key, "passb_", 6)) return ftlm_passb_info(c, key);
   if (!strcmp(key, "sm_count")) return c->sm_count;
   if (!strcmp(key, "autotuned")) return c->autotuned;
+  if (!strcmp(key, "tmlr")) return c->use_tmlr;
+  if (!strncmp(key, "tmlr_", 5)) return ftlm_tmlr_info(c, key);
   if (!strncmp(key, "tml_", 4)) return ftlm_tml_info(c, key);
   return -1;
 }
@@ -386,7 +389,10 @@ static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fu
     // two-pass step when PASS-B windows exist: the TML pass leaves the sums and the finish to PASS-B
     const bool pb = c->passb != nullptr;
     int rc = FTLM_OK;
-    if (fused || !c->debug_pass_mask || (c->debug_pass_mask & 1)) rc = ftlm_launch_hv_tml(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, 1, s);
+    if (fused || !c->debug_pass_mask || (c->debug_pass_mask & 1)) {
+      if (c->use_tmlr && c->tmlr) rc = ftlm_launch_hv_tmlr(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, s);
+      else rc = ftlm_launch_hv_tml(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, 1, s);
+    }
     if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, s);
     return rc;
   }

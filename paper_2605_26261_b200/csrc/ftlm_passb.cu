@@ -410,9 +410,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
   for (;;) {
     uint64_t best_set = 0;
     int best_cnt = 0;
-    for (size_t seed = 0; seed < cand.size(); ++seed) {
-      if (!open_bond(seed)) continue;
-      uint64_t set = c->bonds[(size_t)cand[seed]].mask;
+    auto grow = [&](uint64_t set) {
       int cur = covered(set);
       while (__builtin_popcountll(set) < smax) {
         int pick = -1, pick_cnt = cur;
@@ -432,13 +430,27 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
         set |= 1ull << pick;
         cur = covered(set);
       }
+      return set;
+    };
+    auto prune = [&](uint64_t set) {                      // keep only the positions some covered bond uses
+      uint64_t used = 0;
+      for (size_t k = 0; k < cand.size(); ++k)
+        if (open_bond(k) && (c->bonds[(size_t)cand[k]].mask & ~set) == 0) used |= c->bonds[(size_t)cand[k]].mask;
+      return used;
+    };
+    for (size_t seed = 0; seed < cand.size(); ++seed) {
+      if (!open_bond(seed)) continue;
+      uint64_t set = c->bonds[(size_t)cand[seed]].mask;
+      for (int round = 0; round < 3; ++round) {           // positions that ended up unused are given back and re-spent
+        const uint64_t before = set;
+        set = prune(grow(set));
+        if (set == before) break;
+      }
+      const int cur = covered(set);
       if (cur > best_cnt) { best_cnt = cur; best_set = set; }
     }
     if (best_cnt < MIN_GAIN) break;
-    // keep only the positions some covered bond uses
-    uint64_t used = 0;
-    for (size_t k = 0; k < cand.size(); ++k)
-      if (open_bond(k) && (c->bonds[(size_t)cand[k]].mask & ~best_set) == 0) used |= c->bonds[(size_t)cand[k]].mask;
+    const uint64_t used = prune(best_set);
     PassBWindow w;
     w.smask = used;
     w.s = __builtin_popcountll(used);

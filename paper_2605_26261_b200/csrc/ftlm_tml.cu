@@ -763,6 +763,7 @@ int launch_tml_b(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused,
 
 void ftlm_tml_plan_destroy(ftlm_ctx* c) {
   ftlm_passb_plan_destroy(c);
+  ftlm_tmlr_plan_destroy(c);
   TmlPlan* t = c->tml;
   if (!t) return;
   cudaFree(t->d_blob); cudaFree(t->d_items); cudaFree(t->d_item_off); cudaFree(t->d_partials);
@@ -933,6 +934,12 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
             up((void**)&P->d_partials, nullptr, pbytes) && up((void**)&P->d_counter, nullptr, 16);
   if (ok) ok = cudaMemset(P->d_partials, 0, pbytes) == cudaSuccess && cudaMemset(P->d_counter, 0, 16) == cudaSuccess;
   if (!ok) { cudaGetLastError(); ftlm_tml_plan_destroy(c); ftlm_set_error("TML: table upload failed"); return FTLM_ENOMEM; }
+  {                                                       // the register-table variant of the in-tile pass, when it applies
+    std::vector<int> in_window((size_t)c->nb, 0);
+    for (int b = 0; b < c->nb; ++b) in_window[(size_t)b] = win_of_bond[(size_t)b] >= 0 ? 1 : 0;
+    int rc = ftlm_tmlr_plan_create(c, w, m, in_window);
+    if (rc != FTLM_OK) { ftlm_tml_plan_destroy(c); return rc; }
+  }
   return FTLM_OK;
 }
 

@@ -1,0 +1,511 @@
+// TMLR kernel - the in-tile pass of the gather H.v with lane tables held in registers
+// (DESIGN.md section 6.5).  Same label split as the TML kernel, n = (T | M | L), same tile in shared
+// memory, same index arithmetic (index = base(T) + coloff[kT][M] + lr(L); base(T) by CR - Alg. 1
+// restricted to the top bits - or by CLT - Alg. 2 with j = 0), but the loops are turned inside out:
+// a warp keeps one chunk of 32 low parts L (fixed popcount kL, lane <-> lr) and walks over the
+// columns M of matching popcount.  Everything that depends on L alone - the target row of every LL
+// bond, the flipped row and the spin L_i of every ML bond - is read once per unit into registers;
+// everything that depends on M alone - the diagonal coefficient, the antiparallel MM bonds and their
+// target columns, the target column and the spin M_j of every ML bond - is a descriptor built once
+// per tile in shared memory.  Per row and bond the inner loops are then
+//   LL:  one shared-memory read + one FMA             (swap form: parallel bonds read the row itself)
+//   MM:  one descriptor read (warp-uniform), one shared-memory read, one FMA, antiparallel bonds only
+//   ML:  one descriptor read (warp-uniform), a lane test L_i != M_j, one predicated read, one FMA.
+// Only bonds with both sites inside the tile are handled here (Eq. 12 with the s = 1/2 coefficients of
+// Eqs. 13-14 in swap form, y_t = d0 v_t + sum_b (J_b/2)(v[P_b n_t] - v_t)); the bonds that leave the
+// tile belong to the PASS-B windows, and the plan is refused if some are left over.
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+#include "ftlm_passb.cuh"
+
+#define TMLR_MAX_LL 16
+#define TMLR_MAX_MM 16
+#define TMLR_MAX_ML 16
+#define TMLR_THREADS 512
+
+template <typename R>
+struct TmlrParams {
+  int N, K, w, m, mw;
+  uint32_t nT, t_begin, t_end;
+  int n_ll, n_mm, n_ml, max_tile;     // n_ll, n_ml: padded to multiples of 4 (the kernel's NLL, NML)
+  int mode, fused;
+  int64_t dim;
+  const uint64_t* binom;              // [(N+1)*(K+1)] global
+  const uint2* clt;
+  const unsigned char* blob;          // static tables, staged once per CTA
+  int blob_bytes, off_koff, off_tlen, off_coloff, off_mlist, off_moff, off_ll, off_fl;
+  const uint32_t* units;              // kL | chunk << 4 | col_begin << 8 | ncols << 20, grouped by kT
+  const int* unit_off;                // [mw + 2]
+  double* partials;                   // [3][nT]
+  unsigned int* counter;              // [0] tile counter, [1] ticket
+  ChainState* st;
+  R coef0;                            // diag0 - sum of J_b/2 over the LL and ML bonds
+  R ll_J[TMLR_MAX_LL], ml_J[TMLR_MAX_ML], mm_J[TMLR_MAX_MM];
+  uint32_t mm_mask[TMLR_MAX_MM];
+  int ml_j[TMLR_MAX_ML];              // M bit of ML bond e
+};
+
+struct TmlrPlan {
+  int w = 0, m = 0, n_ll = 0, n_mm = 0, n_ml = 0, max_tile = 0;
+  uint32_t nT = 0;
+  unsigned char* d_blob = nullptr;
+  int blob_bytes = 0, off_koff = 0, off_tlen = 0, off_coloff = 0, off_mlist = 0, off_moff = 0, off_ll = 0, off_fl = 0;
+  uint32_t* d_units = nullptr;
+  int* d_unit_off = nullptr;
+  double* d_partials = nullptr;
+  unsigned int* d_counter = nullptr;
+  double coef0 = 0.0;
+  std::vector<double> ll_J, ml_J, mm_J;
+  std::vector<uint32_t> mm_mask;
+  std::vector<int> ml_j;
+  size_t smem = 0;
+};
+
+namespace {
+
+// per-column descriptor arrays in shared memory (rebuilt for every tile: they depend on kT)
+template <typename R>
+struct TmlrSmem {
+  uint64_t* binom;
+  unsigned char* blob;
+  R* vs;                // tile
+  R* dcoef;             // [nM] diagonal coefficient of column M
+  R* dmmJ;              // [nM][n_mm] J/2 of the antiparallel MM bonds (compacted)
+  uint32_t* dmm;        // [nM][n_mm] row offset of their target columns
+  uint32_t* dml;        // [nM][n_ml] byte offset of the target column | M_j (bit 0)
+  int* dnmm;            // [nM]
+  double* red;          // [warps][3] + 3
+  int* misc;            // [0] tile
+};
+
+template <typename R>
+__host__ __device__ inline size_t tmlr_layout(TmlrSmem<R>& s, unsigned char* p0, int N, int K, int blob_bytes, int max_tile,
+                                              int nM, int n_mm, int n_ml, int warps) {
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return p0 + at; };
+  s.binom = (uint64_t*)take((size_t)(N + 1) * (K + 1) * 8);
+  s.blob = take((size_t)blob_bytes);
+  s.vs = (R*)take((size_t)max_tile * sizeof(R));
+  s.dcoef = (R*)take((size_t)nM * sizeof(R));
+  s.dmmJ = (R*)take((size_t)nM * (n_mm ? n_mm : 1) * sizeof(R));
+  s.dmm = (uint32_t*)take((size_t)nM * (n_mm ? n_mm : 1) * 4);
+  s.dml = (uint32_t*)take((size_t)nM * (n_ml ? n_ml : 1) * 4);
+  s.dnmm = (int*)take((size_t)nM * 4);
+  s.red = (double*)take((size_t)(warps + 1) * 3 * 8);
+  s.misc = (int*)take(16);
+  return o;
+}
+
+}  // namespace
+
+namespace {
+
+// FUSED: 0 = y = H_A v;  1 = fused Lanczos pass (subtract beta q_prev, FP64 sums, finish);
+//        2 = first pass of a multi-pass step: subtract beta q_prev only (the last PASS-B window finishes).
+// NLL / NML: LL and ML bond slots (the plan pads the bond lists to multiples of 4 with J = 0 entries that
+// read the row itself, so the inner loops carry no predicates).  mode / fused are warp-uniform run-time values.
+template <typename R, int NLL, int NML>
+__global__ void __launch_bounds__(TMLR_THREADS, 1)
+hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v, const R* __restrict__ qprev,
+               R* __restrict__ y) {
+  FTLM_DYN_SMEM(smem);
+  __shared__ bool s_last;
+  const int FUSED = p.fused;
+  if (FUSED && p.st->done) return;
+  const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
+  const int nL = 1 << p.w, nM = 1 << p.m;
+  TmlrSmem<R> S;
+  tmlr_layout<R>(S, smem, p.N, p.K, p.blob_bytes, p.max_tile, nM, p.n_mm, p.n_ml, NW);
+  for (int k = tid; k < (p.N + 1) * (p.K + 1); k += NT) S.binom[k] = p.binom[k];
+  {
+    const uint4* src = (const uint4*)p.blob;
+    uint4* dst = (uint4*)S.blob;
+    for (int k = tid; k < (p.blob_bytes >> 4); k += NT) dst[k] = __ldg(&src[k]);
+  }
+  const int* s_koff = (const int*)(S.blob + p.off_koff);
+  const int* s_tlen = (const int*)(S.blob + p.off_tlen);
+  const uint16_t* s_coloff = (const uint16_t*)(S.blob + p.off_coloff);       // [kT][M]
+  const uint16_t* s_mlist = (const uint16_t*)(S.blob + p.off_mlist);         // M sorted by popcount
+  const int* s_moff = (const int*)(S.blob + p.off_moff);                     // [m+2]
+  const uint16_t* s_ll = (const uint16_t*)(S.blob + p.off_ll);               // [bond][Lidx]: target row in the column
+  const uint16_t* s_fl = (const uint16_t*)(S.blob + p.off_fl);               // [bond][Lidx]: flipped row | L_i << 15
+  const R bprev = FUSED ? (R)p.st->beta_prev : (R)0;
+  const unsigned char* vsm1 = (const unsigned char*)S.vs - 1;
+  const int n_mm = p.n_mm;
+  constexpr int n_ml = NML;
+
+  for (;;) {
+    __syncthreads();                                   // previous tile done: tile and descriptors reusable
+    if (tid == 0) S.misc[0] = (int)atomicAdd(&p.counter[0], 1u);
+    __syncthreads();
+    const uint32_t T = (uint32_t)S.misc[0] + p.t_begin;
+    if (T >= p.t_end) break;
+    const int kT = p.K - __popc(T);
+    if (kT < 0 || kT > p.mw) continue;                  // no rows with this top part
+    const uint64_t base = p.mode == FTLM_INDEX_CLT ? passb_run_start<FTLM_INDEX_CLT>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt)
+                                                   : passb_run_start<FTLM_INDEX_CR>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt);
+    const int tlen = s_tlen[kT];
+    {                                                   // stage the tile: every copy in flight at once
+      const R* src = v + base;
+      for (int x = tid; x < tlen; x += NT) cp_async_elem(&S.vs[x], &src[x]);
+    }
+    const uint16_t* co = s_coloff + kT * nM;
+    for (int M = tid; M < nM; M += NT) {                // column descriptors of this kT
+      R coef = p.coef0;
+      int n = 0;
+      for (int e = 0; e < n_mm; ++e) {
+        const uint32_t mk = p.mm_mask[e];
+        if (__popc((uint32_t)M & mk) == 1) {
+          S.dmm[M * n_mm + n] = (uint32_t)co[(uint32_t)M ^ mk];
+          S.dmmJ[M * n_mm + n] = p.mm_J[e];
+          coef -= p.mm_J[e];
+          ++n;
+        }
+      }
+      S.dnmm[M] = n;
+      S.dcoef[M] = coef;
+      for (int e = 0; e < n_ml; ++e) {
+        const int j = p.ml_j[e];                         // padding entries: j = -1, never active (flo = 0, bit 31 = 0)
+        S.dml[M * n_ml + e] = j < 0 ? 0u : ((uint32_t)co[(uint32_t)M ^ (1u << j)] * (uint32_t)sizeof(R) | (((uint32_t)M >> j) & 1u));
+      }
+    }
+    cp_async_wait_all();
+    __syncthreads();
+    // ---- units: one chunk of 32 low parts x a block of columns per warp ----------------------------
+    const int u0 = __ldg(&p.unit_off[kT]), u1 = __ldg(&p.unit_off[kT + 1]);
+    double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
+    (void)s_qy; (void)s_yy; (void)s_qq;
+    for (int it = u0 + warp; it < u1; it += NW) {
+      const uint32_t un = __ldg(&p.units[it]);
+      const int kL = (int)(un & 15u), chunk = (int)((un >> 4) & 15u), col0 = (int)((un >> 8) & 0xfffu), ncols = (int)(un >> 20);
+      const int k0 = s_koff[kL];
+      const int len = s_koff[kL + 1] - k0;
+      const int lr = chunk * 32 + lane;
+      const bool valid = lr < len;
+      const int lrc = valid ? lr : 0;
+      const int Lidx = k0 + lrc;
+      uint32_t llo[NLL], flo[NML];                      // lane tables (registers)
+#pragma unroll
+      for (int e = 0; e < NLL; ++e) llo[e] = (uint32_t)s_ll[e * nL + Lidx] * (uint32_t)sizeof(R);
+#pragma unroll
+      for (int e = 0; e < NML; ++e) {                    // byte offset of the flipped row | L_i
+        const uint32_t f = (uint32_t)s_fl[e * nL + Lidx];
+        flo[e] = (f & 0x7fffu) * (uint32_t)sizeof(R) | (f >> 15);
+      }
+      const uint16_t* ml = s_mlist + s_moff[kT - kL] + col0;
+      uint32_t Mn = ml[0];
+      uint32_t cbn = co[Mn];
+      R qpn = (R)0;
+      if (FUSED) qpn = __ldcs(qprev + (base + cbn + (uint32_t)lrc));
+      for (int c = 0; c < ncols; ++c) {
+        const uint32_t M = Mn, cb = cbn;
+        const R qp = qpn;
+        if (c + 1 < ncols) {                              // q_prev of the next column is requested now
+          Mn = ml[c + 1];
+          cbn = co[Mn];
+          if (FUSED) qpn = __ldcs(qprev + (base + cbn + (uint32_t)lrc));
+        }
+        const unsigned char* colb = (const unsigned char*)(S.vs + cb);
+        const R own = S.vs[cb + (uint32_t)lrc];
+        R acc = S.dcoef[M] * own;
+#pragma unroll
+        for (int e = 0; e < NLL; ++e) acc += p.ll_J[e] * *(const R*)(colb + llo[e]);
+        const int nmm = S.dnmm[M];
+        for (int a = 0; a < nmm; ++a) acc += S.dmmJ[M * n_mm + a] * S.vs[S.dmm[M * n_mm + a] + (uint32_t)lrc];
+#pragma unroll
+        for (int e = 0; e < NML; ++e) {
+          const uint32_t d = S.dml[M * n_ml + e], f = flo[e];
+          R a = own;
+          if ((d ^ f) & 1u) a = *(const R*)(vsm1 + d + f);   // active: exactly one of the two low bits is set
+          acc += p.ml_J[e] * a;
+        }
+        if (valid) {
+          const uint64_t g = base + cb + (uint32_t)lrc;
+          if (FUSED) {
+            acc -= bprev * qp;
+            if (FUSED == 1) {
+              s_qy += (double)own * (double)acc;
+              s_yy += (double)acc * (double)acc;
+              s_qq += (double)own * (double)own;
+            }
+          }
+          __stcs(y + g, acc);
+        }
+      }
+    }
+    if (FUSED == 1) {                                   // deterministic per-tile partial sums
+      const double a = warp_sum(s_qy), b = warp_sum(s_yy), c = warp_sum(s_qq);
+      if (lane == 0) { S.red[warp * 3] = a; S.red[warp * 3 + 1] = b; S.red[warp * 3 + 2] = c; }
+      __syncthreads();
+      if (tid < 3) {
+        double s = 0.0;
+        for (int wv = 0; wv < NW; ++wv) s += S.red[wv * 3 + tid];
+        p.partials[(size_t)tid * p.nT + T] = s;
+      }
+    }
+  }
+  // ---- grid-wide finish: the last CTA resets the counters and (fused) advances the chain -----------
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    s_last = (atomicAdd(&p.counter[1], 1u) == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (tid == 0) { p.counter[0] = 0; p.counter[1] = 0; }
+  if (FUSED != 1) return;
+  double tot[3];
+  for (int q = 0; q < 3; ++q) {                         // fixed assignment and order
+    double a = 0.0;
+    for (uint32_t k = tid; k < p.nT; k += NT) a += p.partials[(size_t)q * p.nT + k];
+    a = warp_sum(a);
+    __syncthreads();
+    if (lane == 0) S.red[warp] = a;
+    __syncthreads();
+    double s = 0.0;
+    if (tid == 0) for (int wv = 0; wv < NW; ++wv) s += S.red[wv];
+    tot[q] = s;
+  }
+  if (tid == 0) {
+    ChainState* st = p.st;
+    const double a = tot[0], b = tot[1], c = tot[2];
+    const int j = st->step;
+    const double alpha = c > 0.0 ? a / c : 0.0;
+    double b2 = c > 0.0 ? b - a * a / c : 0.0;
+    if (!(b2 > 0.0)) b2 = 0.0;
+    const double beta = sqrt(b2);
+    st->alpha[j] = alpha;
+    st->beta[j] = beta;
+    double sc = st->scale;
+    sc = fmax(sc, fmax(fabs(alpha), beta));
+    st->scale = sc;
+    st->step = j + 1;
+    st->a = alpha;
+    st->inv_b = beta > 0.0 ? 1.0 / beta : 0.0;
+    st->beta_prev = beta;
+    if (j + 1 >= st->limit || beta <= st->tol * sc) { st->done = 1; st->inv_b = 0.0; }
+  }
+}
+
+}  // namespace
+
+// ---- host: plan, tables, launch -------------------------------------------------------------------
+namespace {
+
+uint64_t binom_r(int n, int k) {
+  if (k < 0 || k > n) return 0;
+  if (k > n - k) k = n - k;
+  unsigned __int128 r = 1;
+  for (int i = 1; i <= k; ++i) r = r * (unsigned)(n - k + i) / (unsigned)i;
+  return (uint64_t)r;
+}
+
+template <typename R>
+size_t tmlr_smem_bytes(const ftlm_ctx* c, const TmlrPlan* t) {
+  TmlrSmem<R> S;
+  return tmlr_layout<R>(S, nullptr, c->N, c->N_up, t->blob_bytes, t->max_tile, 1 << t->m, t->n_mm, t->n_ml, TMLR_THREADS / 32);
+}
+
+template <typename R, int NLL, int NML>
+int launch_tmlr_k(ftlm_ctx* c, const TmlrParams<R>& p, int grid, size_t smem, const void* v, const void* qp, void* y, cudaStream_t s) {
+  auto k = hv_tmlr_kernel<R, NLL, NML>;
+  CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  FTLM_LAUNCH(k, grid, TMLR_THREADS, smem, s, p, (const R*)v, (const R*)qp, (R*)y);
+  CK(cudaGetLastError());
+  (void)c;
+  return FTLM_OK;
+}
+
+template <typename R, int NLL>
+int launch_tmlr_ml(ftlm_ctx* c, const TmlrParams<R>& p, int grid, size_t smem, const void* v, const void* qp, void* y, cudaStream_t s) {
+  switch (p.n_ml) {
+    case 4: return launch_tmlr_k<R, NLL, 4>(c, p, grid, smem, v, qp, y, s);
+    case 8: return launch_tmlr_k<R, NLL, 8>(c, p, grid, smem, v, qp, y, s);
+    case 12: return launch_tmlr_k<R, NLL, 12>(c, p, grid, smem, v, qp, y, s);
+    default: return launch_tmlr_k<R, NLL, 16>(c, p, grid, smem, v, qp, y, s);
+  }
+}
+
+template <typename R>
+int launch_tmlr(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
+  TmlrPlan* t = c->tmlr;
+  TmlrParams<R> p;
+  memset(&p, 0, sizeof(p));
+  p.N = c->N; p.K = c->N_up; p.w = t->w; p.m = t->m; p.mw = t->w + t->m;
+  p.nT = t->nT; p.t_begin = 0; p.t_end = t->nT;
+  if (c->debug_item_count > 0) {
+    p.t_begin = (uint32_t)std::min<int64_t>(c->debug_item_first, t->nT);
+    p.t_end = (uint32_t)std::min<int64_t>(c->debug_item_first + c->debug_item_count, t->nT);
+  }
+  p.n_ll = t->n_ll; p.n_mm = t->n_mm; p.n_ml = t->n_ml; p.max_tile = t->max_tile;
+  p.mode = c->mode; p.fused = fused;
+  p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.blob = t->d_blob; p.blob_bytes = t->blob_bytes;
+  p.off_koff = t->off_koff; p.off_tlen = t->off_tlen; p.off_coloff = t->off_coloff; p.off_mlist = t->off_mlist;
+  p.off_moff = t->off_moff; p.off_ll = t->off_ll; p.off_fl = t->off_fl;
+  p.units = t->d_units; p.unit_off = t->d_unit_off; p.partials = t->d_partials; p.counter = t->d_counter;
+  p.st = c->d_state; p.coef0 = (R)t->coef0;
+  for (int e = 0; e < t->n_ll; ++e) p.ll_J[e] = (R)t->ll_J[(size_t)e];
+  for (int e = 0; e < t->n_ml; ++e) { p.ml_J[e] = (R)t->ml_J[(size_t)e]; p.ml_j[e] = t->ml_j[(size_t)e]; }
+  for (int e = 0; e < t->n_mm; ++e) { p.mm_J[e] = (R)t->mm_J[(size_t)e]; p.mm_mask[e] = t->mm_mask[(size_t)e]; }
+  int grid = c->sm_count;
+  if ((uint32_t)grid > p.t_end - p.t_begin) grid = (int)std::max(1u, p.t_end - p.t_begin);
+  const size_t smem = tmlr_smem_bytes<R>(c, t);
+  switch (p.n_ll) {
+    case 4: return launch_tmlr_ml<R, 4>(c, p, grid, smem, v, qp, y, s);
+    case 8: return launch_tmlr_ml<R, 8>(c, p, grid, smem, v, qp, y, s);
+    case 12: return launch_tmlr_ml<R, 12>(c, p, grid, smem, v, qp, y, s);
+    default: return launch_tmlr_ml<R, 16>(c, p, grid, smem, v, qp, y, s);
+  }
+}
+
+}  // namespace
+
+void ftlm_tmlr_plan_destroy(ftlm_ctx* c) {
+  TmlrPlan* t = c->tmlr;
+  if (!t) return;
+  cudaFree(t->d_blob); cudaFree(t->d_units); cudaFree(t->d_unit_off); cudaFree(t->d_partials); cudaFree(t->d_counter);
+  delete t;
+  c->tmlr = nullptr;
+}
+
+// Build the plan for the split (w, m).  in_window[b] != 0: bond b belongs to a PASS-B window.  Leaves
+// c->tmlr == nullptr (FTLM_OK) when the kernel cannot serve this sector: a bond outside the windows
+// leaves the tile, a bond class overflows the register tables, or the tables do not fit shared memory.
+int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_window) {
+  ftlm_tmlr_plan_destroy(c);
+  const int N = c->N, mw = w + m, t = N - mw;
+  if (w < 5 || w > 11 || m < 1 || m > 12 || t < 1 || t > 31 || c->dim < 64 || (uint64_t)c->dim >= (1ull << 32)) return FTLM_OK;
+  TmlrPlan* P = new TmlrPlan();
+  P->w = w; P->m = m; P->nT = 1u << t;
+  struct LLb { uint32_t mask; };
+  struct MLb { int i, j; };
+  std::vector<LLb> ll;
+  std::vector<MLb> mlb;
+  double sumJ = 0.0;
+  for (int b = 0; b < c->nb; ++b) {
+    if (in_window[(size_t)b]) continue;
+    const BondDev& d = c->bonds[(size_t)b];
+    if (d.j >= mw) { delete P; return FTLM_OK; }                        // would need a global gather
+    if (d.j < w) { ll.push_back({(uint32_t)d.mask}); P->ll_J.push_back(d.Jh); sumJ += d.Jh; }
+    else if (d.i >= w) { P->mm_mask.push_back((uint32_t)(d.mask >> w)); P->mm_J.push_back(d.Jh); }
+    else { mlb.push_back({d.i, d.j - w}); P->ml_J.push_back(d.Jh); P->ml_j.push_back(d.j - w); sumJ += d.Jh; }
+  }
+  if (ll.size() > TMLR_MAX_LL || P->mm_mask.size() > TMLR_MAX_MM || mlb.size() > TMLR_MAX_ML) { delete P; return FTLM_OK; }
+  // pad the LL / ML lists to multiples of 4 (at least 4): J = 0, LL target = the row itself, ML never active
+  while (ll.size() < 4 || (ll.size() & 3)) { ll.push_back({0u}); P->ll_J.push_back(0.0); }
+  while (mlb.size() < 4 || (mlb.size() & 3)) { mlb.push_back({-1, -1}); P->ml_J.push_back(0.0); P->ml_j.push_back(-1); }
+  P->n_ll = (int)ll.size(); P->n_mm = (int)P->mm_mask.size(); P->n_ml = (int)mlb.size();
+  P->max_tile = (int)binom_r(mw, mw / 2);
+  if (P->max_tile > 65535) { delete P; return FTLM_OK; }
+  P->coef0 = c->diag0 - sumJ;
+  const int nL = 1 << w, nM = 1 << m;
+  std::vector<int> koff((size_t)w + 2, 0);
+  for (int k = 0; k <= w; ++k) koff[(size_t)k + 1] = koff[(size_t)k] + (int)binom_r(w, k);
+  std::vector<uint16_t> lr((size_t)nL), lstate((size_t)nL);
+  for (int L = 0; L < nL; ++L) {                                          // lr(L): rank among the w-bit words of equal popcount
+    uint64_t r = 0;
+    int cnt = 0;
+    for (int q = 0; q < w; ++q)
+      if ((L >> q) & 1) { ++cnt; r += binom_r(q, cnt); }
+    lr[(size_t)L] = (uint16_t)r;
+    lstate[(size_t)(koff[(size_t)cnt] + (int)r)] = (uint16_t)L;
+  }
+  std::vector<uint16_t> mlist((size_t)nM);
+  std::vector<int> moff((size_t)m + 2, 0);
+  for (int k = 0; k <= m; ++k) moff[(size_t)k + 1] = moff[(size_t)k] + (int)binom_r(m, k);
+  {
+    std::vector<int> fill(moff.begin(), moff.end() - 1);
+    for (int M = 0; M < nM; ++M) mlist[(size_t)fill[(size_t)__builtin_popcount((unsigned)M)]++] = (uint16_t)M;
+  }
+  std::vector<int> tlen((size_t)mw + 1);
+  std::vector<uint16_t> coloff((size_t)(mw + 1) * nM, 0);
+  std::vector<uint32_t> units;
+  std::vector<int> unit_off((size_t)mw + 2, 0);
+  for (int kT = 0; kT <= mw; ++kT) {
+    tlen[(size_t)kT] = (int)binom_r(mw, kT);
+    int off = 0;
+    for (int M = 0; M < nM; ++M) {
+      coloff[(size_t)kT * nM + M] = (uint16_t)off;
+      const int kL = kT - __builtin_popcount((unsigned)M);
+      if (kL >= 0 && kL <= w) off += (int)binom_r(w, kL);
+    }
+    // units: (kL, chunk of 32 low parts) x blocks of CB columns; CB sized so that a tile has ~6 units per warp
+    long total = 0;
+    for (int kL = std::max(0, kT - m); kL <= std::min(w, kT); ++kL) total += (long)((binom_r(w, kL) + 31) / 32) * (long)binom_r(m, kT - kL);
+    const int CB = (int)std::max<long>(4, std::min<long>(64, total / (6 * (TMLR_THREADS / 32))));
+    const size_t first = units.size();
+    for (int kL = std::max(0, kT - m); kL <= std::min(w, kT); ++kL) {
+      const int nch = (int)((binom_r(w, kL) + 31) / 32), ncol = (int)binom_r(m, kT - kL);
+      for (int ch = 0; ch < nch; ++ch)
+        for (int c0 = 0; c0 < ncol; c0 += CB)
+          units.push_back((uint32_t)kL | ((uint32_t)ch << 4) | ((uint32_t)c0 << 8) | ((uint32_t)std::min(CB, ncol - c0) << 20));
+    }
+    std::stable_sort(units.begin() + (long)first, units.end(), [](uint32_t a, uint32_t b) { return (a >> 20) > (b >> 20); });
+    unit_off[(size_t)kT + 1] = (int)units.size();
+  }
+  std::vector<uint16_t> lltab((size_t)std::max(P->n_ll, 1) * nL, 0), fltab((size_t)std::max(P->n_ml, 1) * nL, 0);
+  for (int k = 0; k <= w; ++k)
+    for (int r = 0; r < koff[(size_t)k + 1] - koff[(size_t)k]; ++r) {
+      const int Lidx = koff[(size_t)k] + r;
+      const uint32_t L = lstate[(size_t)Lidx];
+      for (int e = 0; e < P->n_ll; ++e) {
+        const uint32_t mk = ll[(size_t)e].mask, x = L & mk;
+        lltab[(size_t)e * nL + Lidx] = (uint16_t)((x != 0 && x != mk) ? lr[(size_t)(L ^ mk)] : (uint32_t)r);   // parallel: the row itself
+      }
+      for (int e = 0; e < P->n_ml; ++e) {
+        const int i = mlb[(size_t)e].i;
+        if (i < 0) continue;                                              // padding: 0 (bit 15 clear, never active)
+        fltab[(size_t)e * nL + Lidx] = (uint16_t)((uint32_t)lr[(size_t)(L ^ (1u << i))] | (((L >> i) & 1u) << 15));
+      }
+    }
+  std::vector<unsigned char> blob;
+  auto put = [&](const void* src, size_t bytes) {
+    const size_t at = blob.size();
+    blob.resize(at + ((bytes + 15) & ~(size_t)15), 0);
+    if (bytes) memcpy(blob.data() + at, src, bytes);
+    return (int)at;
+  };
+  P->off_koff = put(koff.data(), koff.size() * 4);
+  P->off_tlen = put(tlen.data(), tlen.size() * 4);
+  P->off_coloff = put(coloff.data(), coloff.size() * 2);
+  P->off_mlist = put(mlist.data(), mlist.size() * 2);
+  P->off_moff = put(moff.data(), moff.size() * 4);
+  P->off_ll = put(lltab.data(), lltab.size() * 2);
+  P->off_fl = put(fltab.data(), fltab.size() * 2);
+  P->blob_bytes = (int)blob.size();
+  c->tmlr = P;
+  P->smem = c->prec == FTLM_FP32 ? tmlr_smem_bytes<float>(c, P) : tmlr_smem_bytes<double>(c, P);
+  if (P->smem > (size_t)227 * 1024 - 1024) { c->tmlr = nullptr; delete P; return FTLM_OK; }
+  auto up = [&](void** d, const void* h, size_t bytes) -> bool {
+    if (cudaMalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
+    if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
+    return true;
+  };
+  const size_t pbytes = (size_t)P->nT * 24;
+  bool ok = up((void**)&P->d_blob, blob.data(), blob.size()) && up((void**)&P->d_units, units.data(), units.size() * 4) &&
+            up((void**)&P->d_unit_off, unit_off.data(), unit_off.size() * 4) &&
+            up((void**)&P->d_partials, nullptr, pbytes) && up((void**)&P->d_counter, nullptr, 16);
+  if (ok) ok = cudaMemset(P->d_partials, 0, pbytes) == cudaSuccess && cudaMemset(P->d_counter, 0, 16) == cudaSuccess;
+  if (!ok) { cudaGetLastError(); ftlm_tmlr_plan_destroy(c); ftlm_set_error("TMLR: table upload failed"); return FTLM_ENOMEM; }
+  return FTLM_OK;
+}
+
+int64_t ftlm_tmlr_info(const ftlm_ctx* c, const char* key) {
+  const TmlrPlan* t = c->tmlr;
+  if (!strcmp(key, "tmlr_available")) return t ? 1 : 0;
+  if (!t) return -1;
+  if (!strcmp(key, "tmlr_smem")) return (int64_t)t->smem;
+  if (!strcmp(key, "tmlr_n_ll")) return t->n_ll;
+  if (!strcmp(key, "tmlr_n_mm")) return t->n_mm;
+  if (!strcmp(key, "tmlr_n_ml")) return t->n_ml;
+  return -1;
+}
+
+int ftlm_launch_hv_tmlr(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s) {
+  if (!c->tmlr) { ftlm_set_error("TMLR kernel unavailable"); return FTLM_EUNSUPPORTED; }
+  if (c->prec == FTLM_FP32) return launch_tmlr<float>(c, v, qprev, y, fused, s);
+  return launch_tmlr<double>(c, v, qprev, y, fused, s);
+}

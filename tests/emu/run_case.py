@@ -27,6 +27,10 @@ import emu_harness as E  # noqa: E402
 
 
 def workload(name):
+    if name.startswith("fring"):                     # ring with folded site order (no long wrap bonds)
+        j2 = name.endswith("j")
+        n = int(name[5:-1] if j2 else name[5:])
+        return W.relabel(W.ring(n, 1.0, 0.5 if j2 else None), W.fold_order(n))
     if name.startswith("ring"):
         j2 = name.endswith("j")
         n = int(name[4:-1] if j2 else name[4:])
@@ -67,6 +71,7 @@ def main():
         res["dim"] = c.dim
         res["passb"] = [c.get("passb_windows"), c.get("passb_bonds"), c.get("passb_lo"), c.get("passb_s")]
         res["tml"] = [c.get("tml_w"), c.get("tml_m")]
+        res["tmlr"] = [c.get("tmlr"), c.get("tmlr_available")]
         assert c.dim == D
         what = spec.get("what", ["neighbors", "apply"])
         if "neighbors" in what:

@@ -46,7 +46,12 @@ def main():
     rng = np.random.default_rng(spec.get("seed", 1))
     basis = co.enumerate_basis(w.N, n_up)
     D = basis.shape[0]
-    v = rng.standard_normal(D).astype(E.NDT[prec])
+    if spec.get("lowmem"):                               # generated in blocks: no float64 temporary of the whole vector
+        v = np.empty(D, dtype=E.NDT[prec])
+        for a in range(0, D, 1 << 26):
+            v[a:a + (1 << 26)] = rng.standard_normal(min(1 << 26, D - a))
+    else:
+        v = rng.standard_normal(D).astype(E.NDT[prec])
     v64 = v.astype(np.float64)
     res = {"ok": True, "dim": D, "passes": []}
     tol = 1e-5 if prec == "fp32" else 1e-12
@@ -72,10 +77,14 @@ def main():
             c.set("debug_item_count", 1)
             for it in picks:
                 c.set("debug_item_first", it)
-                y0 = rng.standard_normal(D).astype(E.NDT[prec])
-                y = y0.copy()
+                if spec.get("lowmem"):                   # N = 34: y starts as (lazily allocated) zeros
+                    y0 = None
+                    y = np.zeros(D, dtype=E.NDT[prec])
+                else:
+                    y0 = rng.standard_normal(D).astype(E.NDT[prec])
+                    y = y0.copy()
                 c.apply_into(v, y)
-                rows = np.flatnonzero(y != y0)
+                rows = np.flatnonzero(y != y0) if y0 is not None else np.flatnonzero(y)
                 err2 = ref2 = 0.0
                 nrows = 0
                 for r0, n in runs_of(rows):
@@ -85,7 +94,7 @@ def main():
                         got = y[r0:r0 + n].astype(np.float64)
                     else:
                         exp = ref - shift * v64[r0:r0 + n]
-                        got = y[r0:r0 + n].astype(np.float64) - y0[r0:r0 + n].astype(np.float64)
+                        got = y[r0:r0 + n].astype(np.float64) - (y0[r0:r0 + n].astype(np.float64) if y0 is not None else 0.0)
                     err2 += float(np.sum((got - exp) ** 2))
                     ref2 += float(np.sum(exp ** 2))
                     nrows += n

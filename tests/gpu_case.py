@@ -29,6 +29,10 @@ def workload(spec):
     if "config" in spec:
         return W.baseline_config(spec["config"])
     name = spec["wl"]
+    if name.startswith("fring"):                         # ring with folded site order (no long wrap bonds)
+        j2 = name.endswith("j")
+        n = int(name[5:-1] if j2 else name[5:])
+        return W.relabel(W.ring(n, 1.0, 0.5 if j2 else None), W.fold_order(n))
     if name.startswith("ring"):
         j2 = name.endswith("j")
         return W.ring(int(name[4:-1] if j2 else name[4:]), 1.0, 0.5 if j2 else None)
@@ -70,6 +74,7 @@ def main():
     res["kernel"] = ftlm.ftlm_get_option(ctx, "kernel")
     res["windows"] = ftlm.ftlm_get_option(ctx, "passb_windows")
     res["dim"] = D
+    res["tmlr"] = [ftlm.ftlm_get_option(ctx, "tmlr"), ftlm.ftlm_get_option(ctx, "tmlr_available")]
     what = spec.get("what", ["apply"])
     basis = co.enumerate_basis(w.N, n_up)
     rng = np.random.default_rng(spec.get("seed", 1))

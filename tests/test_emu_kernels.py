@@ -111,6 +111,19 @@ def test_emu_generalised_windows(wl, n_up, split, mode, prec, opts, nwin, what):
     assert res["kernel"] == K["tml"] and res["passb"][0] >= nwin
 
 
+@pytest.mark.parametrize("wl,n_up,split,mode,prec,opts", [
+    ("fring16j", 8, 5 | (3 << 8), "cr", "fp32", [["passb_lo_min", 4]]),
+    ("fring14j", 7, 5 | (3 << 8), "clt", "fp64", [["passb_lo_min", 4]]),
+    ("fring15", 6, 6 | (3 << 8), "clt", "fp32", [["passb_lo_min", 4]]),
+])
+def test_emu_tmlr_in_tile_pass(wl, n_up, split, mode, prec, opts):
+    """TMLR (lane tables in registers, per-column descriptors) as the in-tile pass, PASS-B windows for the rest."""
+    res = run_case({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec,
+                    "options": [["passb", 1]] + opts + [["tml_split", split], ["kernel", K["tml"]], ["tmlr", 1]],
+                    "what": ["apply", "lanczos"], "steps": 6}, timeout=1500)
+    assert res["tmlr"] == [1, 1] and res["passb"][0] >= 1
+
+
 def test_emu_passb_off_keeps_top_bonds_in_tml():
     res = run_case({"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp64",
                     "options": [["passb", 0], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]],
@@ -135,12 +148,13 @@ def test_emu_autotune_checks_every_candidate_against_row():
     assert all(r["valid"] and r["relerr"] <= 1e-5 for r in d["rep"]) and d["tuned"] >= 1
 
 
-def test_emu_config4_full_size_sampled_tiles_and_items():
+@pytest.mark.parametrize("tmlr", [0, 1])
+def test_emu_config4_full_size_sampled_tiles_and_items(tmlr):
     """BASELINE config 4 (D = 155 117 520) at full size: sampled tiles of the TML pass and sampled items of
     both PASS-B windows run through the emulation with the real run starts and offsets; the rows each
     pass writes and their values must be the oracle's (and nothing may touch a guard page)."""
     p = subprocess.run([sys.executable, os.path.join(ROOT, "tests", "emu", "run_sampled.py"),
-                        json.dumps({"config": 4, "mode": "cr", "samples": 1})],
+                        json.dumps({"config": 4, "mode": "cr", "samples": 1, "options": [["tmlr", tmlr]]})],
                        capture_output=True, text=True, timeout=1500)
     assert p.returncode == 0, p.stderr[-2000:]
     d = json.loads(p.stdout.strip().splitlines()[-1])

@@ -40,6 +40,18 @@ def test_windows_match_oracle(wl, n_up, mode, prec, opts, nwin):
     assert d["kernel"] == 3 and d["windows"] >= nwin, d
 
 
+@pytest.mark.parametrize("wl,n_up,mode,prec,opts", [
+    ("fring16j", 8, "cr", "fp32", [["passb", 1], ["passb_lo_min", 4], ["tml_split", 5 | (3 << 8)]]),
+    ("fring14j", 7, "clt", "fp64", [["passb", 1], ["passb_lo_min", 4], ["tml_split", 5 | (3 << 8)]]),
+    ("fring22j", 11, "clt", "fp32", [["passb", 1]]),
+    ("fring24j", 12, "cr", "fp32", [["passb", 1]]),
+])
+def test_tmlr_in_tile_pass_matches_oracle(wl, n_up, mode, prec, opts):
+    d = run({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec, "options": opts + [["kernel", 3], ["tmlr", 1]],
+             "what": ["apply", "lanczos"], "steps": 8})
+    assert d["kernel"] == 3 and d["tmlr"] == [1, 1], d
+
+
 @pytest.mark.parametrize("cfg,mode", [(3, "clt"), (3, "cr")])
 def test_autotune_config3(cfg, mode):
     d = run({"config": cfg, "mode": mode, "autotune": True, "what": ["sampled"], "blocks": 4})
