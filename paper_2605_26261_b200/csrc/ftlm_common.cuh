@@ -91,6 +91,7 @@ struct ftlm_ctx {
   // PASS-B windows stays inside the tile.  Option "tmlr": 1 = use it for the in-tile pass of kernel TML.
   TmlrPlan* tmlr = nullptr;
   int use_tmlr = 0;
+  int unij_allowed = 1;            // option "tmlr_unij": 0 keeps the per-bond FMA form even on uniform-J lattices
   int use_passb = 0;               // option "passb": 1 moves the bonds that leave the tile into PASS-B windows (ftlm_autotune turns it on when it is valid and faster)
   int passb_lo_min = 0;            // option "passb_lo_min": lowest label position a window may use (0 = auto)
   int passb_smax = 0;              // option "passb_smax": largest window (0 = auto: 12 FP32 / 11 FP64)

@@ -320,6 +320,12 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "tmlr")) { c->use_tmlr = value ? 1 : 0; return FTLM_OK; }
+  if (!strcmp(key, "tmlr_unij")) {
+    c->unij_allowed = value ? 1 : 0;
+    CK(cudaSetDevice(c->device));
+    ftlm_tml_plan_destroy(c);
+    return ftlm_tml_plan_create(c);
+  }
   if (!strcmp(key, "debug_pass_mask")) { c->debug_pass_mask = (int)value; return FTLM_OK; }
   if (!strcmp(key, "debug_item_first")) { c->debug_item_first = value; return FTLM_OK; }
   if (!strcmp(key, "debug_item_count")) { c->debug_item_count = value; return FTLM_OK; }

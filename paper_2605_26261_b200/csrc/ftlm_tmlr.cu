@@ -61,6 +61,7 @@ struct TmlrPlan {
   std::vector<uint32_t> mm_mask;
   std::vector<int> ml_j;
   size_t smem = 0;
+  bool unij = false;                  // uniform J_b within the LL bonds and within the ML bonds
 };
 
 namespace {
@@ -106,7 +107,9 @@ namespace {
 //        2 = first pass of a multi-pass step: subtract beta q_prev only (the last PASS-B window finishes).
 // NLL / NML: LL and ML bond slots (the plan pads the bond lists to multiples of 4 with J = 0 entries that
 // read the row itself, so the inner loops carry no predicates).  mode / fused are warp-uniform run-time values.
-template <typename R, int NLL, int NML>
+// UNIJ: every LL bond has the same J_b and every ML bond has the same J_b (uniform-J lattices): the loops
+// add the gathered values and multiply once (padding entries then add J * v_t, which coef0 takes back).
+template <typename R, int NLL, int NML, bool UNIJ>
 __global__ void __launch_bounds__(TMLR_THREADS, 1)
 hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v, const R* __restrict__ qprev,
                R* __restrict__ y) {
@@ -210,17 +213,26 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         const unsigned char* colb = (const unsigned char*)(S.vs + cb);
         const R own = S.vs[cb + (uint32_t)lrc];
         R acc = S.dcoef[M] * own;
+        if (UNIJ) {
+          R sl = (R)0;
 #pragma unroll
-        for (int e = 0; e < NLL; ++e) acc += p.ll_J[e] * *(const R*)(colb + llo[e]);
+          for (int e = 0; e < NLL; ++e) sl += *(const R*)(colb + llo[e]);
+          acc += p.ll_J[0] * sl;
+        } else {
+#pragma unroll
+          for (int e = 0; e < NLL; ++e) acc += p.ll_J[e] * *(const R*)(colb + llo[e]);
+        }
         const int nmm = S.dnmm[M];
         for (int a = 0; a < nmm; ++a) acc += S.dmmJ[M * n_mm + a] * S.vs[S.dmm[M * n_mm + a] + (uint32_t)lrc];
+        R sm = (R)0;
 #pragma unroll
         for (int e = 0; e < NML; ++e) {
           const uint32_t d = S.dml[M * n_ml + e], f = flo[e];
           R a = own;
           if ((d ^ f) & 1u) a = *(const R*)(vsm1 + d + f);   // active: exactly one of the two low bits is set
-          acc += p.ml_J[e] * a;
+          if (UNIJ) sm += a; else acc += p.ml_J[e] * a;
         }
+        if (UNIJ) acc += p.ml_J[0] * sm;
         if (valid) {
           const uint64_t g = base + cb + (uint32_t)lrc;
           if (FUSED) {
@@ -311,11 +323,16 @@ size_t tmlr_smem_bytes(const ftlm_ctx* c, const TmlrPlan* t) {
 
 template <typename R, int NLL, int NML>
 int launch_tmlr_k(ftlm_ctx* c, const TmlrParams<R>& p, int grid, size_t smem, const void* v, const void* qp, void* y, cudaStream_t s) {
-  auto k = hv_tmlr_kernel<R, NLL, NML>;
-  CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  FTLM_LAUNCH(k, grid, TMLR_THREADS, smem, s, p, (const R*)v, (const R*)qp, (R*)y);
+  if (c->tmlr->unij) {
+    auto k = hv_tmlr_kernel<R, NLL, NML, true>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    FTLM_LAUNCH(k, grid, TMLR_THREADS, smem, s, p, (const R*)v, (const R*)qp, (R*)y);
+  } else {
+    auto k = hv_tmlr_kernel<R, NLL, NML, false>;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    FTLM_LAUNCH(k, grid, TMLR_THREADS, smem, s, p, (const R*)v, (const R*)qp, (R*)y);
+  }
   CK(cudaGetLastError());
-  (void)c;
   return FTLM_OK;
 }
 
@@ -394,9 +411,21 @@ int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_
     else { mlb.push_back({d.i, d.j - w}); P->ml_J.push_back(d.Jh); P->ml_j.push_back(d.j - w); sumJ += d.Jh; }
   }
   if (ll.size() > TMLR_MAX_LL || P->mm_mask.size() > TMLR_MAX_MM || mlb.size() > TMLR_MAX_ML) { delete P; return FTLM_OK; }
-  // pad the LL / ML lists to multiples of 4 (at least 4): J = 0, LL target = the row itself, ML never active
-  while (ll.size() < 4 || (ll.size() & 3)) { ll.push_back({0u}); P->ll_J.push_back(0.0); }
-  while (mlb.size() < 4 || (mlb.size() & 3)) { mlb.push_back({-1, -1}); P->ml_J.push_back(0.0); P->ml_j.push_back(-1); }
+  // uniform couplings (and at least one bond in each list): the kernel adds first and multiplies once
+  P->unij = !ll.empty() && !mlb.empty() && c->unij_allowed;
+  for (size_t e = 1; e < P->ll_J.size(); ++e) P->unij = P->unij && P->ll_J[e] == P->ll_J[0];
+  for (size_t e = 1; e < P->ml_J.size(); ++e) P->unij = P->unij && P->ml_J[e] == P->ml_J[0];
+  // pad the LL / ML lists to multiples of 4 (at least 4): LL target = the row itself, ML never active (reads the
+  // row itself); J = 0, or - uniform case - the common J with the added J * v_t taken back from the diagonal
+  while (ll.size() < 4 || (ll.size() & 3)) {
+    ll.push_back({0u});
+    if (P->unij) { P->ll_J.push_back(P->ll_J[0]); sumJ += P->ll_J[0]; } else P->ll_J.push_back(0.0);
+  }
+  while (mlb.size() < 4 || (mlb.size() & 3)) {
+    mlb.push_back({-1, -1});
+    P->ml_j.push_back(-1);
+    if (P->unij) { P->ml_J.push_back(P->ml_J[0]); sumJ += P->ml_J[0]; } else P->ml_J.push_back(0.0);
+  }
   P->n_ll = (int)ll.size(); P->n_mm = (int)P->mm_mask.size(); P->n_ml = (int)mlb.size();
   P->max_tile = (int)binom_r(mw, mw / 2);
   if (P->max_tile > 65535) { delete P; return FTLM_OK; }
@@ -498,6 +527,7 @@ int64_t ftlm_tmlr_info(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "tmlr_available")) return t ? 1 : 0;
   if (!t) return -1;
   if (!strcmp(key, "tmlr_smem")) return (int64_t)t->smem;
+  if (!strcmp(key, "tmlr_unij_used")) return t->unij ? 1 : 0;
   if (!strcmp(key, "tmlr_n_ll")) return t->n_ll;
   if (!strcmp(key, "tmlr_n_mm")) return t->n_mm;
   if (!strcmp(key, "tmlr_n_ml")) return t->n_ml;
