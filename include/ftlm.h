@@ -137,10 +137,12 @@ int ftlm_chain_profile(ftlm_ctx* ctx, int nsteps, void* stream, double* ms_hv, d
 /* Choose the H.v kernel configuration of the handle by measurement on the device (DESIGN.md
  * section 7.1).  Each candidate computes y = H v for one seeded random vector and is compared on
  * the device with the thread-per-row kernel (Eq. 12 with Alg. 1 / Alg. 2 as printed, L105-L173);
- * candidates beyond the H.v tolerance (1e-5 FP32, 1e-12 FP64, norm-relative) are rejected, the
- * others are timed over `reps` launches (CUDA events) and the fastest is left selected.
- * report (host, caller-owned, may be NULL): JSON list of {name, valid, relerr, ms, windows}.
- * Allocates and frees 3 vectors of dim elements.  Synchronous.  FTLM_EUNSUPPORTED if no
+ * candidates beyond the H.v tolerance (1e-5 FP32, 1e-12 FP64, norm-relative), or whose first three
+ * fused Lanczos steps deviate from the thread-per-row kernel's alpha, beta by more than 1e-4 / 1e-9,
+ * are rejected; the others are timed over `reps` fused steps (CUDA events) and the fastest is left
+ * selected.  report (host, caller-owned, may be NULL): JSON list of {name, valid, relerr,
+ * fused_dev, ms, windows}.  Allocates and frees 3 vectors of dim elements and uses the handle's
+ * chain workspace (any chain in progress is lost).  Synchronous.  FTLM_EUNSUPPORTED if no
  * candidate is valid (the handle keeps its previous selection). */
 int ftlm_autotune(ftlm_ctx* ctx, int reps, char* report, int report_cap, void* stream);
 

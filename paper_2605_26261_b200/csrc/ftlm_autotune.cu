@@ -4,8 +4,9 @@
 // PASS-B windows in several window sizes, with the TML or the TMLR in-tile pass) first computes y = H v for one seeded random vector and is
 // compared, on the device, with the ROW kernel's result (the paper's launch shape, thread per row,
 // Eq. 12 / Alg. 1 / Alg. 2 directly): a candidate whose norm-relative deviation exceeds the
-// north_star tolerance (1e-5 FP32, 1e-12 FP64) is rejected.  The valid candidates are timed with
-// CUDA events over `reps` launches and the fastest is left selected in the handle.  All arithmetic
+// north_star tolerance (1e-5 FP32, 1e-12 FP64) is rejected; so is one whose first three fused Lanczos steps
+// (alpha_1..3, beta_1..2) differ from the ROW kernel's by more than 1e-4 (FP32) / 1e-9 (FP64).  The valid
+// candidates are timed with CUDA events over `reps` whole fused steps and the fastest is left selected.  All arithmetic
 // is in the library's kernels; nothing here runs on the CPU.
 #include <cmath>
 #include <cstdio>
@@ -87,10 +88,24 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
   const double tol = c->prec == FTLM_FP32 ? 1e-5 : 1e-12;
   int best = -1;
   double best_ms = 0.0;
-  // reference: the ROW kernel on a seeded random vector
+  // three fused Lanczos steps from the seeded start vector: alpha_1..3, beta_1..2 (host copies)
+  auto fused_probe = [&](double* ab) -> int {
+    double al[8] = {0}, be[8] = {0};
+    int m_eff = 0;
+    int r = ftlm_chain_begin(c, nullptr, 0x5EEDull, 0, s);
+    if (r == FTLM_OK) r = ftlm_chain_steps(c, 3, s);
+    if (r == FTLM_OK) r = ftlm_chain_end(c, al, be, 8, &m_eff, s);
+    for (int k = 0; k < 3; ++k) ab[k] = al[k];
+    for (int k = 0; k < 2; ++k) ab[3 + k] = be[k];
+    return r;
+  };
+  double ab_ref[5] = {0, 0, 0, 0, 0};
+  const double tol_f = c->prec == FTLM_FP32 ? 1e-4 : 1e-9;
+  // reference: the ROW kernel on a seeded random vector, and its fused steps
   rc = ftlm_fill_random(c, 0x5EEDull, 0, v, s);
   if (rc == FTLM_OK) rc = apply_cand(c, cands[0]);
   if (rc == FTLM_OK) rc = ftlm_apply_H(c, v, yref, s);
+  if (rc == FTLM_OK) rc = fused_probe(ab_ref);
   for (int k = 0; k < ncand && rc == FTLM_OK; ++k) {
     const Cand& cd = cands[k];
     if (cd.kernel == FTLM_KERNEL_TILE && !c->tile) continue;
@@ -106,11 +121,23 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
       rc = ftlm_cuda_fail(cudaGetLastError(), "ftlm_autotune: candidate run"); break;
     }
     const double rel = h_out[1] > 0.0 ? std::sqrt(h_out[0] / h_out[1]) : (h_out[0] > 0.0 ? 1.0 : 0.0);
-    const bool valid = rel <= tol;
+    bool valid = rel <= tol;
+    double dfused = 0.0;
+    if (valid) {                                         // the fused step (recurrence, FP64 sums, finish) must agree too
+      double ab[5];
+      if ((rc = fused_probe(ab)) != FTLM_OK) break;
+      for (int q = 0; q < 5; ++q) {
+        const double d = std::fabs(ab[q] - ab_ref[q]) / std::fmax(1.0, std::fabs(ab_ref[q]));
+        dfused = std::fmax(dfused, d == d ? d : 1e300);
+      }
+      valid = dfused <= tol_f;
+    }
     float ms = 0.f;
-    if (valid) {
+    if (valid) {                                         // time `reps` whole fused steps (H.v passes + normalisation)
+      if ((rc = ftlm_chain_begin(c, nullptr, 0x5EEDull, 0, s)) != FTLM_OK) break;
+      if ((rc = ftlm_chain_steps(c, 1, s)) != FTLM_OK) break;
       cudaEventRecord(e0, s);
-      for (int r = 0; r < reps && rc == FTLM_OK; ++r) rc = ftlm_apply_H(c, v, y, s);
+      rc = ftlm_chain_steps(c, reps, s);
       cudaEventRecord(e1, s);
       if (rc != FTLM_OK) break;
       if (cudaEventSynchronize(e1) != cudaSuccess) { rc = ftlm_cuda_fail(cudaGetLastError(), "ftlm_autotune: timing"); break; }
@@ -119,8 +146,8 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
       if (best < 0 || ms < best_ms) { best = k; best_ms = ms; }
     }
     char line[256];
-    snprintf(line, sizeof(line), "%s{\"name\": \"%s\", \"valid\": %s, \"relerr\": %.3e, \"ms\": %.5f, \"windows\": %d}",
-             rep.size() > 1 ? ", " : "", cd.name, valid ? "true" : "false", rel, (double)ms,
+    snprintf(line, sizeof(line), "%s{\"name\": \"%s\", \"valid\": %s, \"relerr\": %.3e, \"fused_dev\": %.3e, \"ms\": %.5f, \"windows\": %d}",
+             rep.size() > 1 ? ", " : "", cd.name, valid ? "true" : "false", rel, dfused, (double)ms,
              (cd.kernel == FTLM_KERNEL_TML && c->passb) ? ftlm_passb_windows(c) : 0);
     rep += line;
   }
