@@ -20,7 +20,7 @@
 
 #include "ftlm_passb.cuh"
 
-#define PASSB_MAX_BONDS 32          // one neighbour entry per lane
+#define PASSB_MAX_BONDS 31          // one neighbour entry per lane; entry 31 holds the count and the sum of J
 #define PASSB_MAX_S 12
 #define PASSB_THREADS 1024
 #define PASSB_END 0xFFFFFFFFu
@@ -38,14 +38,16 @@ struct PassBParams {
   const uint2* clt;
   const uint16_t* ustate;           // [2^s]: window words grouped by popcount, ascending inside a group
   const int* koff;                  // [s+2]: first slot of popcount class p in ustate
-  const uint32_t* nbr;              // [2^s][32], indexed by u: slot(u') | bond << 16, PASSB_END after the last
+  const uint32_t* nbr_off;          // [2^s][32], row = position of u in ustate: byte offset of row slot(u') in the tile; [31] = number of entries
+  const R* nbr_J;                   // [2^s][32]: J_b/2 of the same entries; [31] = their sum
   const uint32_t* grp_first;        // [ngroups+1]: first item of group g = F*(s+1) + p_S
   double* partials;                 // [3][nitems]
   unsigned int* counter;            // [0] item counter, [1] ticket
   ChainState* st;
   int xk[PASSB_MAX_S + 1];          // X/32 per popcount class
   int max_conf;                     // largest C(s, p_S) among non-empty classes
-  R Jh[PASSB_MAX_BONDS];
+  int unij;                         // every bond of the window has the same J_b/2 (= Juni)
+  R Juni;
 };
 
 struct PassBWindow {
@@ -59,7 +61,8 @@ struct PassBWindow {
   std::vector<double> Jh;
   uint16_t* d_ustate = nullptr;
   int* d_koff = nullptr;
-  uint32_t* d_nbr = nullptr;
+  uint32_t* d_nbr = nullptr;          // byte offsets
+  void* d_nbrJ = nullptr;             // J_b/2 in the handle's precision
   uint32_t* d_grp_first = nullptr;
   double* d_partials = nullptr;
   unsigned int* d_counter = nullptr;
@@ -88,6 +91,101 @@ __host__ __device__ inline size_t passb_smem_bytes(int N, int K, int max_conf, i
   o += (size_t)32 * 3 * 8;                                      // reduction scratch
   o += (size_t)max_rows * esz;                                  // tile: max over classes of C(s,p) * X
   return o;
+}
+
+// Phase 2 of one work item, specialised on the run offsets per lane (XKC) and on uniform couplings (UNIJ) so
+// that an item executes one straight variant of the word loop (small instruction working set).
+template <typename R, bool FUSED, int XKC, bool UNIJ>
+__device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* tile, R* __restrict__ y, const uint64_t* s_start,
+                                             int c0, int nconf, int X, uint64_t x0, int nx, int lane, int warp, int NW,
+                                             double& s_qy, double& s_yy, double& s_qq) {
+  // neighbour rows are stored in window-word order (row c0 + sl); the row of the next word is requested
+  // while the current word is processed
+  uint32_t eo_n = 0;
+  R eJ_n = (R)0;
+  if (warp < nconf) {
+    eo_n = __ldg(&p.nbr_off[(size_t)(c0 + warp) * 32 + lane]);
+    eJ_n = __ldg(&p.nbr_J[(size_t)(c0 + warp) * 32 + lane]);
+  }
+  for (int sl0 = warp; sl0 < nconf; sl0 += NW * PASSB_PF) {
+    R yold[PASSB_PF][PASSB_XK];
+#pragma unroll
+    for (int j = 0; j < PASSB_PF; ++j) {
+      const int sl = sl0 + j * NW;
+#pragma unroll
+      for (int k = 0; k < PASSB_XK; ++k) {
+        const int x = lane + 32 * k;
+        yold[j][k] = (sl < nconf && k < XKC && x < nx) ? __ldcs(y + s_start[sl] + x0 + x) : (R)0;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < PASSB_PF; ++j) {
+      const int sl = sl0 + j * NW;
+      if (sl >= nconf) break;
+      const uint32_t eo = eo_n;
+      const R eJ = eJ_n;
+      if (sl + NW < nconf) {
+        eo_n = __ldg(&p.nbr_off[(size_t)(c0 + sl + NW) * 32 + lane]);
+        eJ_n = __ldg(&p.nbr_J[(size_t)(c0 + sl + NW) * 32 + lane]);
+      }
+      const int cnt = (int)__shfl_sync(0xffffffffu, eo, 31);
+      const R sumJ = __shfl_sync(0xffffffffu, eJ, 31);
+      // lanes past the end of the run (x >= nx) read stale tile words and are discarded at the store
+      const unsigned char* tl = (const unsigned char*)tile + (size_t)lane * sizeof(R);
+      R* yrow = y + s_start[sl] + x0;
+      R own[PASSB_XK], acc[PASSB_XK];
+      own[0] = *(const R*)(tl + (size_t)sl * X * sizeof(R));
+      acc[0] = (R)0;
+      if (XKC == 1) {
+        own[1] = (R)0; acc[1] = (R)0;
+        if (UNIJ) {                                  // one J_b for the whole window: add, multiply once
+#pragma unroll 4
+          for (int e = 0; e < cnt; ++e) acc[0] += *(const R*)(tl + __shfl_sync(0xffffffffu, eo, e));
+          acc[0] *= p.Juni;
+        } else {
+#pragma unroll 4
+          for (int e = 0; e < cnt; ++e) {
+            const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
+            const R J = __shfl_sync(0xffffffffu, eJ, e);
+            acc[0] += J * *(const R*)(tl + off);
+          }
+        }
+      } else {
+        own[1] = *(const R*)(tl + (size_t)sl * X * sizeof(R) + 32 * sizeof(R));
+        acc[1] = (R)0;
+        if (UNIJ) {
+#pragma unroll 4
+          for (int e = 0; e < cnt; ++e) {
+            const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
+            acc[0] += *(const R*)(tl + off);
+            acc[1] += *(const R*)(tl + off + 32 * sizeof(R));
+          }
+          acc[0] *= p.Juni; acc[1] *= p.Juni;
+        } else {
+#pragma unroll 4
+          for (int e = 0; e < cnt; ++e) {
+            const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
+            const R J = __shfl_sync(0xffffffffu, eJ, e);
+            acc[0] += J * *(const R*)(tl + off);
+            acc[1] += J * *(const R*)(tl + off + 32 * sizeof(R));
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < PASSB_XK; ++k) {
+        const int x = lane + 32 * k;
+        if (k < XKC && x < nx) {
+          const R yn = yold[j][k] + (acc[k] - sumJ * own[k]);
+          __stcs(&yrow[x], yn);
+          if (FUSED) {
+            s_qy += (double)own[k] * (double)yn;
+            s_yy += (double)yn * (double)yn;
+            s_qq += (double)own[k] * (double)own[k];
+          }
+        }
+      }
+    }
+  }
 }
 
 template <typename R, int MODE, bool FUSED>
@@ -156,59 +254,12 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     __syncthreads();
     // ---- phase 2: one warp per window word; y of PASSB_PF words is requested before the first is used ---
     double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
-    for (int sl0 = warp; sl0 < nconf; sl0 += NW * PASSB_PF) {
-      R yold[PASSB_PF][PASSB_XK];
-#pragma unroll
-      for (int j = 0; j < PASSB_PF; ++j) {
-        const int sl = sl0 + j * NW;
-#pragma unroll
-        for (int k = 0; k < PASSB_XK; ++k) {
-          const int x = lane + 32 * k;
-          yold[j][k] = (sl < nconf && k < XK && x < nx) ? __ldcs(y + s_start[sl] + x0 + x) : (R)0;
-        }
-      }
-#pragma unroll
-      for (int j = 0; j < PASSB_PF; ++j) {
-        const int sl = sl0 + j * NW;
-        if (sl >= nconf) break;
-        const uint32_t u = __ldg(&p.ustate[c0 + sl]);
-        const uint32_t ent = __ldg(&p.nbr[(size_t)u * 32 + lane]);
-        const int cnt = __popc(__ballot_sync(0xffffffffu, ent != PASSB_END));
-        const R* row = tile + (size_t)sl * X;
-        R* yrow = y + s_start[sl] + x0;
-        R own[PASSB_XK], acc[PASSB_XK];
-#pragma unroll
-        for (int k = 0; k < PASSB_XK; ++k) {
-          const int x = lane + 32 * k;
-          own[k] = (k < XK && x < nx) ? row[x] : (R)0;
-          acc[k] = (R)0;
-        }
-        R sumJ = (R)0;
-        for (int e = 0; e < cnt; ++e) {
-          const uint32_t en = __shfl_sync(0xffffffffu, ent, e);
-          const R J = p.Jh[en >> 16];
-          const R* nrow = tile + (size_t)(en & 0xffffu) * X;
-          sumJ += J;
-#pragma unroll
-          for (int k = 0; k < PASSB_XK; ++k) {
-            const int x = lane + 32 * k;
-            if (k < XK && x < nx) acc[k] += J * nrow[x];
-          }
-        }
-#pragma unroll
-        for (int k = 0; k < PASSB_XK; ++k) {
-          const int x = lane + 32 * k;
-          if (k < XK && x < nx) {
-            const R yn = yold[j][k] + (acc[k] - sumJ * own[k]);
-            __stcs(&yrow[x], yn);
-            if (FUSED) {
-              s_qy += (double)own[k] * (double)yn;
-              s_yy += (double)yn * (double)yn;
-              s_qq += (double)own[k] * (double)own[k];
-            }
-          }
-        }
-      }
+    if (XK == 1) {
+      if (p.unij) passb_phase2<R, FUSED, 1, true>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
+      else passb_phase2<R, FUSED, 1, false>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
+    } else {
+      if (p.unij) passb_phase2<R, FUSED, 2, true>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
+      else passb_phase2<R, FUSED, 2, false>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
     }
     if (FUSED) {                                        // deterministic per-item partial sums
       const double a = warp_sum(s_qy), b = warp_sum(s_yy), c = warp_sum(s_qq);
@@ -291,7 +342,7 @@ void ftlm_passb_plan_destroy(ftlm_ctx* c) {
   PassBSet* S = c->passb;
   if (!S) return;
   for (PassBWindow& w : S->win) {
-    cudaFree(w.d_ustate); cudaFree(w.d_koff); cudaFree(w.d_nbr); cudaFree(w.d_grp_first);
+    cudaFree(w.d_ustate); cudaFree(w.d_koff); cudaFree(w.d_nbr); cudaFree(w.d_nbrJ); cudaFree(w.d_grp_first);
     cudaFree(w.d_partials); cudaFree(w.d_counter);
   }
   delete S;
@@ -483,15 +534,30 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
       slot[(size_t)u] = (uint16_t)(fill[(size_t)p] - koff[(size_t)p]);
       ustate[(size_t)fill[(size_t)p]++] = (uint16_t)u;
     }
-    std::vector<uint32_t> nbr((size_t)nU * 32, PASSB_END);
+    const size_t esz = ftlm_elem_size(c);
+    std::vector<uint32_t> nbr((size_t)nU * 32, 0u);
+    std::vector<double> nbrJ((size_t)nU * 32, 0.0);
     for (int u = 0; u < nU; ++u) {
       int n = 0;
+      double sj = 0.0;
+      const int pu = __builtin_popcount((unsigned)u);
+      const int X = 32 * w.xk[pu];                                     // rows per tile row of this popcount class
+      const size_t row = (size_t)koff[(size_t)pu] + slot[(size_t)u];    // position of u in window-word order (ustate)
       for (size_t e = 0; e < w.bonds.size(); ++e) {
         const BondDev& d = c->bonds[(size_t)w.bonds[e]];
         const uint32_t mk = (uint32_t)bits_extract(d.mask, w.smask), x = (uint32_t)u & mk;
-        if (x != 0 && x != mk) nbr[(size_t)u * 32 + (size_t)n++] = (uint32_t)slot[(size_t)((uint32_t)u ^ mk)] | ((uint32_t)e << 16);
+        if (x != 0 && x != mk) {
+          nbr[row * 32 + (size_t)n] = (uint32_t)slot[(size_t)((uint32_t)u ^ mk)] * (uint32_t)X * (uint32_t)esz;
+          nbrJ[row * 32 + (size_t)n] = d.Jh;
+          sj += d.Jh;
+          ++n;
+        }
       }
+      nbr[row * 32 + 31] = (uint32_t)n;
+      nbrJ[row * 32 + 31] = sj;
     }
+    std::vector<float> nbrJf;
+    if (esz == 4) { nbrJf.resize(nbrJ.size()); for (size_t k = 0; k < nbrJ.size(); ++k) nbrJf[k] = (float)nbrJ[k]; }
     auto up = [&](void** d, const void* h, size_t bytes) -> bool {
       if (cudaMalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
       if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
@@ -500,6 +566,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
     const size_t pbytes = (size_t)w.nitems * 24;
     bool ok = up((void**)&w.d_ustate, ustate.data(), ustate.size() * 2) && up((void**)&w.d_koff, koff.data(), koff.size() * 4) &&
               up((void**)&w.d_nbr, nbr.data(), nbr.size() * 4) &&
+              up(&w.d_nbrJ, esz == 4 ? (const void*)nbrJf.data() : (const void*)nbrJ.data(), nbrJ.size() * esz) &&
               up((void**)&w.d_grp_first, groups[wi].data(), groups[wi].size() * 4) &&
               up((void**)&w.d_partials, nullptr, pbytes) && up((void**)&w.d_counter, nullptr, 16);
     if (ok) ok = cudaMemset(w.d_partials, 0, pbytes) == cudaSuccess && cudaMemset(w.d_counter, 0, 16) == cudaSuccess;
@@ -514,12 +581,14 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   memset(&p, 0, sizeof(p));
   p.N = c->N; p.K = c->N_up; p.lo = w.lo; p.s = w.s; p.f = w.f; p.ngroups = w.ngroups; p.nitems = w.nitems;
   p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.ustate = w.d_ustate; p.koff = w.d_koff;
-  p.nbr = w.d_nbr; p.grp_first = w.d_grp_first; p.partials = w.d_partials; p.counter = w.d_counter;
+  p.nbr_off = w.d_nbr; p.nbr_J = (const R*)w.d_nbrJ; p.grp_first = w.d_grp_first; p.partials = w.d_partials; p.counter = w.d_counter;
   p.st = c->d_state; p.max_conf = w.max_conf;
+  p.unij = c->unij_allowed ? 1 : 0;
+  for (size_t e = 1; e < w.Jh.size(); ++e) if (w.Jh[e] != w.Jh[0]) p.unij = 0;
+  p.Juni = w.Jh.empty() ? (R)0 : (R)w.Jh[0];
   p.smask_hi = w.smask >> w.lo;
   p.fmask_hi = (c->N >= 64 ? ~0ull : ((1ull << c->N) - 1ull)) >> w.lo & ~p.smask_hi;
   for (int k = 0; k <= PASSB_MAX_S; ++k) p.xk[k] = w.xk[k];
-  for (size_t e = 0; e < w.Jh.size(); ++e) p.Jh[e] = (R)w.Jh[e];
   p.item_begin = 0; p.item_end = w.nitems;
   if (c->debug_item_count > 0) {
     p.item_begin = (uint32_t)std::min<int64_t>(c->debug_item_first, w.nitems);
