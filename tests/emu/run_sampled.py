@@ -61,7 +61,11 @@ def main():
         res["kernel"] = c.get("kernel")
         res["windows"] = nwin
         bclass = c.bond_classes()
-        for ps in range(nwin + 1):
+        plist = list(range(nwin + 1)) + ([-1] if spec.get("tmlr_both") else [])   # -1: pass 0 again with the other in-tile kernel
+        for ps in plist:
+            if ps == -1:
+                c.set("tmlr", 0 if c.get("tmlr") else 1)
+                ps = 0
             if ps == 0:
                 nitems = c.get("tml_tiles")
                 bonds = [b for b in range(w.n_bonds) if bclass[b][0] != 6]
@@ -100,7 +104,7 @@ def main():
                     nrows += n
                 rel = (err2 / ref2) ** 0.5 if ref2 > 0 else 0.0
                 ok = rel <= (tol if ps == 0 else 20 * tol)   # windows: y0 + delta rounds in the width of y0
-                res["passes"].append({"pass": ps, "item": it, "rows": nrows, "relerr": rel, "ok": bool(ok)})
+                res["passes"].append({"pass": ps, "tmlr": c.get("tmlr") if ps == 0 else None, "item": it, "rows": nrows, "relerr": rel, "ok": bool(ok)})
                 res["ok"] = res["ok"] and bool(ok) and (nrows > 0 or ps == 0)
         c.set("debug_pass_mask", 0)
         c.set("debug_item_count", 0)
