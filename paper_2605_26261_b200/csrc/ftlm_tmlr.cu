@@ -212,27 +212,26 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         }
         const unsigned char* colb = (const unsigned char*)(S.vs + cb);
         const R own = S.vs[cb + (uint32_t)lrc];
+        // four independent partial sums (LL even/odd, ML even/odd) keep the FMA dependency chains short
         R acc = S.dcoef[M] * own;
-        if (UNIJ) {
-          R sl = (R)0;
+        R l0 = (R)0, l1 = (R)0, m0 = (R)0, m1 = (R)0;
 #pragma unroll
-          for (int e = 0; e < NLL; ++e) sl += *(const R*)(colb + llo[e]);
-          acc += p.ll_J[0] * sl;
-        } else {
-#pragma unroll
-          for (int e = 0; e < NLL; ++e) acc += p.ll_J[e] * *(const R*)(colb + llo[e]);
+        for (int e = 0; e < NLL; e += 2) {
+          const R a0 = *(const R*)(colb + llo[e]), a1 = *(const R*)(colb + llo[e + 1]);
+          if (UNIJ) { l0 += a0; l1 += a1; } else { l0 += p.ll_J[e] * a0; l1 += p.ll_J[e + 1] * a1; }
         }
         const int nmm = S.dnmm[M];
         for (int a = 0; a < nmm; ++a) acc += S.dmmJ[M * n_mm + a] * S.vs[S.dmm[M * n_mm + a] + (uint32_t)lrc];
-        R sm = (R)0;
 #pragma unroll
-        for (int e = 0; e < NML; ++e) {
-          const uint32_t d = S.dml[M * n_ml + e], f = flo[e];
-          R a = own;
-          if ((d ^ f) & 1u) a = *(const R*)(vsm1 + d + f);   // active: exactly one of the two low bits is set
-          if (UNIJ) sm += a; else acc += p.ml_J[e] * a;
+        for (int e = 0; e < NML; e += 2) {
+          const uint32_t d0 = S.dml[M * n_ml + e], f0 = flo[e], d1 = S.dml[M * n_ml + e + 1], f1 = flo[e + 1];
+          R a0 = own, a1 = own;
+          if ((d0 ^ f0) & 1u) a0 = *(const R*)(vsm1 + d0 + f0);   // active: exactly one of the two low bits is set
+          if ((d1 ^ f1) & 1u) a1 = *(const R*)(vsm1 + d1 + f1);
+          if (UNIJ) { m0 += a0; m1 += a1; } else { m0 += p.ml_J[e] * a0; m1 += p.ml_J[e + 1] * a1; }
         }
-        if (UNIJ) acc += p.ml_J[0] * sm;
+        if (UNIJ) acc += p.ll_J[0] * (l0 + l1) + p.ml_J[0] * (m0 + m1);
+        else acc += (l0 + l1) + (m0 + m1);
         if (valid) {
           const uint64_t g = base + cb + (uint32_t)lrc;
           if (FUSED) {
