@@ -65,11 +65,19 @@ int ftlm_destroy(ftlm_ctx* ctx);
 int64_t ftlm_dim(const ftlm_ctx* ctx);
 
 /* Options: "kernel" (FTLM_KERNEL_*), "low_bits" (w of the TILE kernels, 0 = auto),
- * "tml_low_bits" / "tml_mid_bits" (w, m of the TML kernels, 0 = auto), "graph" (1 = replay
- * Lanczos steps from a CUDA graph).  FTLM_EINVAL on unknown key/value, FTLM_EUNSUPPORTED when
- * the requested kernel / split cannot be built for this sector.  ftlm_get_option also answers
- * the read-only keys "sm_count", "tml_w", "tml_m", "tml_smem", "tml_ctas_per_sm",
- * "tml_threads", "tml_n_ll", "tml_n_mm", "tml_n_ml", "tml_n_tt", "tml_n_tm", "tml_n_tl". */
+ * "tml_low_bits" / "tml_mid_bits" / "tml_split" = w | m << 8 (split of the TML kernels, 0 = auto),
+ * "graph" (1 = replay Lanczos steps from a CUDA graph); multi-pass H.v of kernel TML (DESIGN.md
+ * 6.4-6.5): "passb" (1 = bonds that leave the tile go to PASS-B window passes; default 0),
+ * "passb_lo_min" / "passb_smax" / "passb_ctas" (window planner: lowest label position, largest
+ * window, CTAs per SM tried first; 0 = auto), "tmlr" (1 = in-tile pass by the TMLR kernel when its
+ * plan exists), "tmlr_unij" (0 = never use the uniform-J form).  Test hooks: "debug_pass_mask",
+ * "debug_item_first", "debug_item_count" (run only some passes / tiles / items of a non-fused
+ * H.v; used by the host emulation tests).  FTLM_EINVAL on unknown key/value, FTLM_EUNSUPPORTED
+ * when the requested kernel / split cannot be built for this sector.  ftlm_get_option also answers
+ * read-only keys: "sm_count", "autotuned", "tml_w", "tml_m", "tml_smem", "tml_ctas_per_sm",
+ * "tml_threads", "tml_tiles", "tml_n_ll|mm|ml|tt|tm|tl", "tml_bclass:<b>", "tmlr_available",
+ * "tmlr_smem", "tmlr_n_ll|mm|ml", "tmlr_unij_used", "passb_windows", "passb_bonds",
+ * "passb_lo<k>", "passb_mask<k>", "passb_nbonds<k>", "passb_items<k>", "passb_ctas_used". */
 int ftlm_set_option(ftlm_ctx* ctx, const char* key, int64_t value);
 int64_t ftlm_get_option(const ftlm_ctx* ctx, const char* key);
 
