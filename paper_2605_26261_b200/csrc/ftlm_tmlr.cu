@@ -11,9 +11,10 @@
 //   LL:  one shared-memory read + one FMA             (swap form: parallel bonds read the row itself)
 //   MM:  one descriptor read (warp-uniform), one shared-memory read, one FMA, antiparallel bonds only
 //   ML:  one descriptor read (warp-uniform), a lane test L_i != M_j, one predicated read, one FMA.
-// Only bonds with both sites inside the tile are handled here (Eq. 12 with the s = 1/2 coefficients of
-// Eqs. 13-14 in swap form, y_t = d0 v_t + sum_b (J_b/2)(v[P_b n_t] - v_t)); the bonds that leave the
-// tile belong to the PASS-B windows, and the plan is refused if some are left over.
+// (Eq. 12 with the s = 1/2 coefficients of Eqs. 13-14 in swap form, y_t = d0 v_t + sum_b (J_b/2)(v[P_b n_t] - v_t)).
+// The bonds that leave the tile belong to the PASS-B windows; a few left-over ones that are uniform per
+// column (both sites in T, or one in T and one in M) are read from global memory at the same lr (coalesced);
+// the plan is refused if a left-over bond has a site in L (that needs the TML kernel's per-lane gather).
 #include <algorithm>
 #include <cstring>
 #include <vector>
@@ -23,6 +24,7 @@
 #define TMLR_MAX_LL 16
 #define TMLR_MAX_MM 16
 #define TMLR_MAX_ML 16
+#define TMLR_MAX_G 8              // bonds that leave the tile but are uniform per column (TT, TM): coalesced global reads
 #define TMLR_THREADS 512
 
 template <typename R>
@@ -45,6 +47,10 @@ struct TmlrParams {
   R ll_J[TMLR_MAX_LL], ml_J[TMLR_MAX_ML], mm_J[TMLR_MAX_MM];
   uint32_t mm_mask[TMLR_MAX_MM];
   int ml_j[TMLR_MAX_ML];              // M bit of ML bond e
+  int n_g;                            // left-over bonds with a site in T and none in L
+  uint32_t g_tmask[TMLR_MAX_G];       // T bits the bond flips (two for TT, one for TM)
+  int g_mbit[TMLR_MAX_G];             // M bit of a TM bond, -1 for TT
+  R g_J[TMLR_MAX_G];
 };
 
 struct TmlrPlan {
@@ -60,6 +66,10 @@ struct TmlrPlan {
   std::vector<double> ll_J, ml_J, mm_J;
   std::vector<uint32_t> mm_mask;
   std::vector<int> ml_j;
+  std::vector<uint32_t> g_tmask;
+  std::vector<int> g_mbit;
+  std::vector<double> g_J;
+  int n_g = 0;
   size_t smem = 0;
   bool unij = false;                  // uniform J_b within the LL bonds and within the ML bonds
 };
@@ -77,13 +87,16 @@ struct TmlrSmem {
   uint32_t* dmm;        // [nM][n_mm] row offset of their target columns
   uint32_t* dml;        // [nM][n_ml] byte offset of the target column | M_j (bit 0)
   int* dnmm;            // [nM]
+  uint32_t* dg;         // [nM][n_g] global row (target tile base + target column offset) of the active left-over bonds
+  R* dgJ;               // [nM][n_g]
+  int* dng;             // [nM]
   double* red;          // [warps][3] + 3
   int* misc;            // [0] tile
 };
 
 template <typename R>
 __host__ __device__ inline size_t tmlr_layout(TmlrSmem<R>& s, unsigned char* p0, int N, int K, int blob_bytes, int max_tile,
-                                              int nM, int n_mm, int n_ml, int warps) {
+                                              int nM, int n_mm, int n_ml, int n_g, int warps) {
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return p0 + at; };
   s.binom = (uint64_t*)take((size_t)(N + 1) * (K + 1) * 8);
@@ -94,6 +107,9 @@ __host__ __device__ inline size_t tmlr_layout(TmlrSmem<R>& s, unsigned char* p0,
   s.dmm = (uint32_t*)take((size_t)nM * (n_mm ? n_mm : 1) * 4);
   s.dml = (uint32_t*)take((size_t)nM * (n_ml ? n_ml : 1) * 4);
   s.dnmm = (int*)take((size_t)nM * 4);
+  s.dg = (uint32_t*)take((size_t)nM * (n_g ? n_g : 1) * 4);
+  s.dgJ = (R*)take((size_t)nM * (n_g ? n_g : 1) * sizeof(R));
+  s.dng = (int*)take((size_t)nM * 4);
   s.red = (double*)take((size_t)(warps + 1) * 3 * 8);
   s.misc = (int*)take(16);
   return o;
@@ -120,7 +136,7 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
   const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
   const int nL = 1 << p.w, nM = 1 << p.m;
   TmlrSmem<R> S;
-  tmlr_layout<R>(S, smem, p.N, p.K, p.blob_bytes, p.max_tile, nM, p.n_mm, p.n_ml, NW);
+  tmlr_layout<R>(S, smem, p.N, p.K, p.blob_bytes, p.max_tile, nM, p.n_mm, p.n_ml, p.n_g, NW);
   for (int k = tid; k < (p.N + 1) * (p.K + 1); k += NT) S.binom[k] = p.binom[k];
   {
     const uint4* src = (const uint4*)p.blob;
@@ -168,6 +184,33 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         }
       }
       S.dnmm[M] = n;
+      if (p.n_g) {                                       // left-over TT / TM bonds: rows of another tile, same lr
+        int ng = 0;
+        for (int g = 0; g < p.n_g; ++g) {
+          const uint32_t tm = p.g_tmask[g];
+          const int mb = p.g_mbit[g];
+          bool act;
+          int kTn = kT;
+          uint32_t Mn = (uint32_t)M;
+          if (mb < 0) { const uint32_t x = T & tm; act = x != 0 && x != tm; }
+          else {
+            const uint32_t tj = (T & tm) ? 1u : 0u, mi = ((uint32_t)M >> mb) & 1u;
+            act = tj != mi;
+            kTn = tj ? kT + 1 : kT - 1;                  // the one moves between T and the low part
+            Mn = (uint32_t)M ^ (1u << mb);
+          }
+          if (act && kTn >= 0 && kTn <= p.mw) {
+            const uint32_t Tn = T ^ tm;
+            const uint64_t bn = p.mode == FTLM_INDEX_CLT ? passb_run_start<FTLM_INDEX_CLT>((uint64_t)Tn, p.mw, kTn, p.K, S.binom, p.clt)
+                                                         : passb_run_start<FTLM_INDEX_CR>((uint64_t)Tn, p.mw, kTn, p.K, S.binom, p.clt);
+            S.dg[M * p.n_g + ng] = (uint32_t)(bn + s_coloff[kTn * nM + (int)Mn]);
+            S.dgJ[M * p.n_g + ng] = p.g_J[g];
+            coef -= p.g_J[g];
+            ++ng;
+          }
+        }
+        S.dng[M] = ng;
+      }
       S.dcoef[M] = coef;
       for (int e = 0; e < n_ml; ++e) {
         const int j = p.ml_j[e];                         // padding entries: j = -1, never active (flo = 0, bit 31 = 0)
@@ -222,6 +265,10 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         }
         const int nmm = S.dnmm[M];
         for (int a = 0; a < nmm; ++a) acc += S.dmmJ[M * n_mm + a] * S.vs[S.dmm[M * n_mm + a] + (uint32_t)lrc];
+        if (p.n_g) {
+          const int ng = S.dng[M];
+          for (int a = 0; a < ng; ++a) acc += S.dgJ[M * p.n_g + a] * __ldg(v + ((size_t)S.dg[M * p.n_g + a] + (uint32_t)lrc));
+        }
 #pragma unroll
         for (int e = 0; e < NML; e += 2) {
           const uint32_t d0 = S.dml[M * n_ml + e], f0 = flo[e], d1 = S.dml[M * n_ml + e + 1], f1 = flo[e + 1];
@@ -317,7 +364,7 @@ uint64_t binom_r(int n, int k) {
 template <typename R>
 size_t tmlr_smem_bytes(const ftlm_ctx* c, const TmlrPlan* t) {
   TmlrSmem<R> S;
-  return tmlr_layout<R>(S, nullptr, c->N, c->N_up, t->blob_bytes, t->max_tile, 1 << t->m, t->n_mm, t->n_ml, TMLR_THREADS / 32);
+  return tmlr_layout<R>(S, nullptr, c->N, c->N_up, t->blob_bytes, t->max_tile, 1 << t->m, t->n_mm, t->n_ml, t->n_g, TMLR_THREADS / 32);
 }
 
 template <typename R, int NLL, int NML>
@@ -366,6 +413,8 @@ int launch_tmlr(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, 
   for (int e = 0; e < t->n_ll; ++e) p.ll_J[e] = (R)t->ll_J[(size_t)e];
   for (int e = 0; e < t->n_ml; ++e) { p.ml_J[e] = (R)t->ml_J[(size_t)e]; p.ml_j[e] = t->ml_j[(size_t)e]; }
   for (int e = 0; e < t->n_mm; ++e) { p.mm_J[e] = (R)t->mm_J[(size_t)e]; p.mm_mask[e] = t->mm_mask[(size_t)e]; }
+  p.n_g = t->n_g;
+  for (int g = 0; g < t->n_g; ++g) { p.g_tmask[g] = t->g_tmask[(size_t)g]; p.g_mbit[g] = t->g_mbit[(size_t)g]; p.g_J[g] = (R)t->g_J[(size_t)g]; }
   int grid = c->sm_count;
   if ((uint32_t)grid > p.t_end - p.t_begin) grid = (int)std::max(1u, p.t_end - p.t_begin);
   const size_t smem = tmlr_smem_bytes<R>(c, t);
@@ -404,7 +453,13 @@ int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_
   for (int b = 0; b < c->nb; ++b) {
     if (in_window[(size_t)b]) continue;
     const BondDev& d = c->bonds[(size_t)b];
-    if (d.j >= mw) { delete P; return FTLM_OK; }                        // would need a global gather
+    if (d.j >= mw) {                                                    // leaves the tile and no window took it
+      if (d.i < w || (int)P->g_tmask.size() >= TMLR_MAX_G) { delete P; return FTLM_OK; }   // TL: per-lane global gather, not served here
+      P->g_tmask.push_back((uint32_t)(d.mask >> mw));                   // TT: both bits; TM: the T bit (the M bit shifts out)
+      P->g_mbit.push_back(d.i >= mw ? -1 : d.i - w);
+      P->g_J.push_back(d.Jh);
+      continue;
+    }
     if (d.j < w) { ll.push_back({(uint32_t)d.mask}); P->ll_J.push_back(d.Jh); sumJ += d.Jh; }
     else if (d.i >= w) { P->mm_mask.push_back((uint32_t)(d.mask >> w)); P->mm_J.push_back(d.Jh); }
     else { mlb.push_back({d.i, d.j - w}); P->ml_J.push_back(d.Jh); P->ml_j.push_back(d.j - w); sumJ += d.Jh; }
@@ -425,7 +480,7 @@ int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_
     P->ml_j.push_back(-1);
     if (P->unij) { P->ml_J.push_back(P->ml_J[0]); sumJ += P->ml_J[0]; } else P->ml_J.push_back(0.0);
   }
-  P->n_ll = (int)ll.size(); P->n_mm = (int)P->mm_mask.size(); P->n_ml = (int)mlb.size();
+  P->n_ll = (int)ll.size(); P->n_mm = (int)P->mm_mask.size(); P->n_ml = (int)mlb.size(); P->n_g = (int)P->g_tmask.size();
   P->max_tile = (int)binom_r(mw, mw / 2);
   if (P->max_tile > 65535) { delete P; return FTLM_OK; }
   P->coef0 = c->diag0 - sumJ;
@@ -530,6 +585,7 @@ int64_t ftlm_tmlr_info(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "tmlr_n_ll")) return t->n_ll;
   if (!strcmp(key, "tmlr_n_mm")) return t->n_mm;
   if (!strcmp(key, "tmlr_n_ml")) return t->n_ml;
+  if (!strcmp(key, "tmlr_n_g")) return t->n_g;
   return -1;
 }
 

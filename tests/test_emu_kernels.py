@@ -113,6 +113,8 @@ def test_emu_generalised_windows(wl, n_up, split, mode, prec, opts, nwin, what):
     ("fring16j", 8, 5 | (3 << 8), "cr", "fp32", [["passb_lo_min", 4]]),
     ("fring14j", 7, 5 | (3 << 8), "clt", "fp64", [["passb_lo_min", 4]]),
     ("fring15", 6, 6 | (3 << 8), "clt", "fp32", [["passb_lo_min", 4]]),
+    # windows only above the tile: the bonds between M and T stay in TMLR as coalesced global reads
+    ("fring16j", 7, 5 | (4 << 8), "clt", "fp64", [["passb_lo_min", 9]]),
 ])
 def test_emu_tmlr_in_tile_pass(wl, n_up, split, mode, prec, opts):
     """TMLR (lane tables in registers, per-column descriptors) as the in-tile pass, PASS-B windows for the rest."""
