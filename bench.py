@@ -214,7 +214,7 @@ def main():
         return
 
     import torch
-    from paper_2605_26261_b200 import ftlm
+    from paper_2605_26261_b200 import ftlm, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -248,10 +248,7 @@ def main():
     elif args.kernel == "auto":
         # rank 0 probes in a child process; every rank applies the same choice
         choice, autotune_report, probe_note = probe_choice(args) if rank == 0 else (SAFE_CHOICE, None, None)
-        if dist is not None:
-            box = [choice]
-            dist.broadcast_object_list(box, src=0)
-            choice = box[0]
+        choice = replicas.broadcast_choice(choice, dist)
     else:
         choice = {"row": "row", "tile": "tile", "tml": "tml"}[args.kernel]
     for key, val in CANDIDATES[choice]:
@@ -279,10 +276,7 @@ def main():
     sampler.stop_flag = True
     a, b, m_eff = ftlm.ftlm_chain_end(ctx)
     assert m_eff == K + Wm and np.isfinite(a).all() and np.isfinite(b).all(), (m_eff, K + Wm)
-    t_ms = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    ms = float(t_ms.item())
+    ms = replicas.max_over_ranks(ms, dist, device="cuda")
     value = world * K / (ms * 1e-3)
 
     # ---- per-kernel timing for the roofline of the dominant kernel --------------------------
@@ -312,11 +306,9 @@ def main():
         out = ftlm.ftlm_lanczos_host(ctx, hq_np, ke)              # H2D start vector, ke steps, D2H alpha/beta, T eig
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        t_e = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        t_e = replicas.max_over_ranks(dt, dist, device="cuda")
         assert int(out["m_eff"][0]) == ke
-        e2e = {"value": world * ke / float(t_e.item()), "unit": UNIT, "h2d_bytes_per_step": 4 * D / ke,
+        e2e = {"value": world * ke / t_e, "unit": UNIT, "h2d_bytes_per_step": 4 * D / ke,
                "d2h_bytes_per_step": 16.0 + 8.0 / ke, "steps": ke,
                "call": "ftlm_lanczos_host(pinned host start vector -> alpha, beta, theta, weight)"}
 
