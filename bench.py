@@ -131,7 +131,7 @@ def run_reference(args, w, n_up):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": w.name, "N": w.N, "N_up": n_up, "dim": D,
+            "data": "synthetic", "config": {"workload": f"config{args.config}:{w.name}", "N": w.N, "N_up": n_up, "dim": D,
                                             "n_bonds": w.n_bonds, "sample_rows_per_step": rows},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": co.threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
