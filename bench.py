@@ -141,15 +141,17 @@ def run_reference(args, w, n_up):
 
 # name -> option settings, in order (the candidates of ftlm_autotune, include/ftlm.h)
 CANDIDATES = {
-    "row": [("tmlr", 0), ("kernel", 1)],
-    "tile": [("tmlr", 0), ("kernel", 2)],
-    "tml": [("tmlr", 0), ("passb", 0), ("kernel", 3)],
+    "row": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 1)],
+    "tile": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 2)],
+    "tml": [("lazy_norm", 0), ("tmlr", 0), ("passb", 0), ("kernel", 3)],
     "tml+passb": [("tmlr", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
     "tml+passb_1cta": [("tmlr", 0), ("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
     "tml+passb_s11": [("tmlr", 0), ("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
     "tml+passb_s10": [("tmlr", 0), ("passb_smax", 10), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
     "tmlr+passb": [("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
     "tmlr+passb_s11": [("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
+    "tmlr+passb_lazy": [("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1), ("lazy_norm", 1)],
+    "tmlr+passb_s11_lazy": [("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1), ("lazy_norm", 1)],
 }
 SAFE_CHOICE = "tml"          # measured on B200 in round 1 (profiles/): the fallback if the probe dies
 
@@ -257,6 +259,8 @@ def main():
     if kernel_used == "tml" and ftlm.ftlm_get_option(ctx, "tmlr") == 1 and ftlm.ftlm_get_option(ctx, "tmlr_available") == 1:
         kernel_used = "tmlr"
     n_windows = max(ftlm.ftlm_get_option(ctx, "passb_windows"), 0) if kernel_used in ("tml", "tmlr") else 0
+    ftlm_lazy = (kernel_used == "tmlr" and ftlm.ftlm_get_option(ctx, "lazy_norm") == 1
+                 and ftlm.ftlm_get_option(ctx, "lazy_norm_ok") == 1)
     D = ftlm.ftlm_dim(ctx)
     K, Wm = args.steps, args.warmup
     assert 1 <= K and K + Wm <= ftlm.MAX_STEPS, "steps + warmup must be <= 1024 (one chain)"
@@ -339,7 +343,7 @@ def main():
                        "precision": "fp32 vectors, fp64 reductions", "l2": "inputs_exceed_l2 (3 x 620 MB vectors)",
                        "parallelism": f"replicas x{world}"},
             "hv_rows_per_s": world * D / (ms_hv * 1e-3), "hv_gelem_per_s": world * nnz / (ms_hv * 1e-3) / 1e9,
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": (2 + n_windows) * K,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": ((1 if ftlm_lazy else 2) + n_windows) * K,
             "clocks": sampler.summary()}
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -35,7 +35,7 @@ diff_norm_kernel(const R* __restrict__ a, const R* __restrict__ ref, int64_t n, 
 
 struct Cand {
   const char* name;
-  int kernel, passb, smax, ctas, tmlr;
+  int kernel, passb, smax, ctas, tmlr, lazy;
 };
 
 int apply_cand(ftlm_ctx* c, const Cand& k) {
@@ -46,6 +46,7 @@ int apply_cand(ftlm_ctx* c, const Cand& k) {
     if ((rc = ftlm_set_option(c, "passb", k.passb)) != FTLM_OK) return rc;
   }
   if ((rc = ftlm_set_option(c, "tmlr", k.tmlr)) != FTLM_OK) return rc;
+  if ((rc = ftlm_set_option(c, "lazy_norm", k.lazy)) != FTLM_OK) return rc;
   return ftlm_set_option(c, "kernel", k.kernel);
 }
 
@@ -72,17 +73,19 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
     ftlm_set_error("ftlm_autotune: cannot allocate 3 x %zu bytes", bytes);
     return FTLM_ENOMEM;
   }
-  const int saved_kernel = c->kernel, saved_pb = c->use_passb, saved_smax = c->passb_smax, saved_ctas = c->passb_ctas, saved_tmlr = c->use_tmlr;
+  const int saved_kernel = c->kernel, saved_pb = c->use_passb, saved_smax = c->passb_smax, saved_ctas = c->passb_ctas, saved_tmlr = c->use_tmlr, saved_lazy = c->lazy_norm;
   const Cand cands[] = {
-      {"row", FTLM_KERNEL_ROW, 0, 0, 0, 0},
-      {"tile", FTLM_KERNEL_TILE, 0, 0, 0, 0},
-      {"tml", FTLM_KERNEL_TML, 0, 0, 0, 0},
-      {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0, 0},
-      {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1, 0},
-      {"tml+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 0},
-      {"tml+passb_s10", FTLM_KERNEL_TML, 1, 10, 0, 0},
-      {"tmlr+passb", FTLM_KERNEL_TML, 1, 0, 0, 1},
-      {"tmlr+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 1},
+      {"row", FTLM_KERNEL_ROW, 0, 0, 0, 0, 0},
+      {"tile", FTLM_KERNEL_TILE, 0, 0, 0, 0, 0},
+      {"tml", FTLM_KERNEL_TML, 0, 0, 0, 0, 0},
+      {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0, 0, 0},
+      {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1, 0, 0},
+      {"tml+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 0, 0},
+      {"tml+passb_s10", FTLM_KERNEL_TML, 1, 10, 0, 0, 0},
+      {"tmlr+passb", FTLM_KERNEL_TML, 1, 0, 0, 1, 0},
+      {"tmlr+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 1, 0},
+      {"tmlr+passb_lazy", FTLM_KERNEL_TML, 1, 0, 0, 1, 1},
+      {"tmlr+passb_s11_lazy", FTLM_KERNEL_TML, 1, 11, 0, 1, 1},
   };
   const int ncand = (int)(sizeof(cands) / sizeof(cands[0]));
   const double tol = c->prec == FTLM_FP32 ? 1e-5 : 1e-12;
@@ -110,7 +113,7 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
     const Cand& cd = cands[k];
     if (cd.kernel == FTLM_KERNEL_TILE && !c->tile) continue;
     if (apply_cand(c, cd) != FTLM_OK) continue;                          // not available for this sector
-    if (cd.kernel == FTLM_KERNEL_TML && (!c->tml || (cd.passb && !c->passb) || (cd.tmlr && !c->tmlr))) continue;
+    if (cd.kernel == FTLM_KERNEL_TML && (!c->tml || (cd.passb && !c->passb) || (cd.tmlr && !c->tmlr) || (cd.lazy && !ftlm_tmlr_lazy_ok(c)))) continue;
     double h_out[2] = {0.0, 0.0};
     if (cudaMemsetAsync(d_out, 0, 16, s) != cudaSuccess) { rc = FTLM_ECUDA; break; }
     if ((rc = ftlm_apply_H(c, v, y, s)) != FTLM_OK) break;
@@ -154,7 +157,7 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
   rep += "]";
   if (rc == FTLM_OK && best >= 0) rc = apply_cand(c, cands[best]);
   else {                                                                  // restore what the caller had
-    c->passb_smax = saved_smax; c->passb_ctas = saved_ctas; c->use_tmlr = saved_tmlr;
+    c->passb_smax = saved_smax; c->passb_ctas = saved_ctas; c->use_tmlr = saved_tmlr; c->lazy_norm = saved_lazy;
     ftlm_set_option(c, "passb", saved_pb);
     c->kernel = saved_kernel;
     if (rc == FTLM_OK) { ftlm_set_error("ftlm_autotune: no valid candidate"); rc = FTLM_EUNSUPPORTED; }

@@ -104,7 +104,10 @@ struct ftlm_ctx {
 
   // chain workspace
   void* q[3] = {nullptr, nullptr, nullptr};
-  int cur = 0;                     // q[cur] = q_j, q[1-cur] = q_{j-1}, q[2] = y
+  int cur = 0;                     // (unused by the chain driver; roles are ia / ib / ic below)
+  int ia = 0, ib = 1, ic = 2;      // q[ia] = q_j, q[ib] = q_{j-1}, q[ic] = y
+  bool pending_norm = false;       // lazy normalisation: q_{j+1} = (q[ic] - alpha_j q[ia]) / beta_j is not materialised yet
+  int lazy_norm = 0;               // option "lazy_norm": 1 = the TMLR pass forms q_{j+1} while staging (no normalisation pass)
   ChainState* d_state = nullptr;
   double* d_partials = nullptr;    // [3][max_blocks]
   unsigned int* d_ticket = nullptr;
@@ -138,6 +141,10 @@ int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_
 void ftlm_tmlr_plan_destroy(ftlm_ctx* c);
 int64_t ftlm_tmlr_info(const ftlm_ctx* c, const char* key);
 int ftlm_launch_hv_tmlr(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
+// Lazy-normalisation form of the fused pass: yq holds y_j on entry and q_{j+1} = (y_j - alpha_j q_j)/beta_j on
+// exit (formed while the tile is staged); q = q_j (also the q_prev of this step); y receives the pass's output.
+int ftlm_launch_hv_tmlr_lazy(ftlm_ctx* c, void* yq, const void* q, void* y, int fused, cudaStream_t s);
+bool ftlm_tmlr_lazy_ok(const ftlm_ctx* c);
 
 // PASS-B (ftlm_passb.cu).  `tt` lists the bonds whose two sites lie at positions >= mw (candidate
 // top-top bonds) as indices into c->bonds; on return window_of[k] is the PASS-B window that took

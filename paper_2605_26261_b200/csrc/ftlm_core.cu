@@ -320,6 +320,7 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "tmlr")) { c->use_tmlr = value ? 1 : 0; return FTLM_OK; }
+  if (!strcmp(key, "lazy_norm")) { c->lazy_norm = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "tmlr_unij")) {
     c->unij_allowed = value ? 1 : 0;
     CK(cudaSetDevice(c->device));
@@ -372,6 +373,8 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "sm_count")) return c->sm_count;
   if (!strcmp(key, "autotuned")) return c->autotuned;
   if (!strcmp(key, "tmlr")) return c->use_tmlr;
+  if (!strcmp(key, "lazy_norm")) return c->lazy_norm;
+  if (!strcmp(key, "lazy_norm_ok")) return ftlm_tmlr_lazy_ok(c) ? 1 : 0;
   if (!strncmp(key, "tmlr_", 5)) return ftlm_tmlr_info(c, key);
   if (!strncmp(key, "tml_", 4)) return ftlm_tml_info(c, key);
   return -1;
@@ -487,6 +490,8 @@ static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64
   if (rc != FTLM_OK) return rc;
   const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
   c->cur = 0;
+  c->ia = 0; c->ib = 1; c->ic = 2;
+  c->pending_norm = false;
   c->steps_enqueued = 0;
   c->chain_limit = (int)(c->dim < FTLM_MAX_STEPS ? c->dim : FTLM_MAX_STEPS);
   if (!q1) {
@@ -514,9 +519,9 @@ extern "C" int ftlm_chain_begin(ftlm_ctx* c, const void* d_q1, uint64_t seed, in
 }
 
 static int launch_next(ftlm_ctx* c, cudaStream_t s) {
-  const void* y = c->q[2];
-  const void* q = c->q[c->cur];
-  void* qn = c->q[1 - c->cur];
+  const void* y = c->q[c->ic];
+  const void* q = c->q[c->ia];
+  void* qn = c->q[c->ib];
   const int grid = stream_grid(c, c->dim / 4 + 1, 8);
   if (c->prec == FTLM_FP32) { auto k__ = lanczos_next_kernel<float, float4>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)y, (const float*)q, (float*)qn, c->dim, c->d_state); }
   else { auto k__ = lanczos_next_kernel<double, double2>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)y, (const double*)q, (double*)qn, c->dim, c->d_state); }
@@ -525,22 +530,42 @@ static int launch_next(ftlm_ctx* c, cudaStream_t s) {
 }
 
 static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv, float* ms_norm) {
+  // lazy normalisation (option "lazy_norm", TMLR in-tile pass only): no normalisation pass; the next step's
+  // in-tile pass forms q_{j+1} = (y_j - alpha_j q_j)/beta_j while it stages its tile and writes it over y_j
+  const bool lazy = c->lazy_norm && ftlm_effective_kernel(c) == FTLM_KERNEL_TML && ftlm_tmlr_lazy_ok(c);
   // y = H q_j - beta_{j-1} q_{j-1}   (+ reductions, alpha_j, beta_j on the device)
   if (timed) CK(cudaEventRecord(c->ev[0], s));
-  int rc = launch_hv(c, c->q[c->cur], c->q[1 - c->cur], c->q[2], 1, s);
+  int rc;
+  if (lazy && c->pending_norm) {
+    const bool pb = c->passb != nullptr;
+    rc = ftlm_launch_hv_tmlr_lazy(c, c->q[c->ic], c->q[c->ia], c->q[c->ib], pb ? 2 : 1, s);
+    if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, c->q[c->ic], c->q[c->ib], 1, s);
+    const int a = c->ia, b = c->ib, y = c->ic;             // q_{j+1} now lives in the old y, q_j becomes q_prev, y is the old q_{j-1}
+    c->ia = y; c->ib = a; c->ic = b;
+  } else {
+    if (c->pending_norm) {                                 // the option was switched off mid-chain: materialise q_{j+1} first
+      rc = launch_next(c, s);
+      if (rc != FTLM_OK) return rc;
+      const int a = c->ia; c->ia = c->ib; c->ib = a;
+      c->pending_norm = false;
+    }
+    rc = launch_hv(c, c->q[c->ia], c->q[c->ib], c->q[c->ic], 1, s);
+  }
   if (rc != FTLM_OK) return rc;
   if (timed) CK(cudaEventRecord(c->ev[1], s));
-  // q_{j+1} = (y - alpha_j q_j)/beta_j, written over q_{j-1}
-  rc = launch_next(c, s);
-  if (rc != FTLM_OK) return rc;
+  if (lazy) c->pending_norm = true;
+  else {
+    // q_{j+1} = (y - alpha_j q_j)/beta_j, written over q_{j-1}; then q_{j+1} <-> q_j roles swap, y stays
+    rc = launch_next(c, s);
+    if (rc != FTLM_OK) return rc;
+    const int a = c->ia; c->ia = c->ib; c->ib = a;
+  }
   if (timed) {
     CK(cudaEventRecord(c->ev[2], s));
     CK(cudaEventSynchronize(c->ev[2]));
     CK(cudaEventElapsedTime(ms_hv, c->ev[0], c->ev[1]));
     CK(cudaEventElapsedTime(ms_norm, c->ev[1], c->ev[2]));
   }
-  // swap roles: q_{j+1} lives in the old q_{j-1} buffer, the old q_j becomes q_{j-1}; y stays q[2]
-  c->cur = 1 - c->cur;
   c->steps_enqueued++;
   return FTLM_OK;
 }

@@ -33,6 +33,8 @@ struct TmlrParams {
   uint32_t nT, t_begin, t_end;
   int n_ll, n_mm, n_ml, max_tile;     // n_ll, n_ml: padded to multiples of 4 (the kernel's NLL, NML)
   int mode, fused;
+  int lazy;                           // 1: the tile is formed from (vio = y_j, qprev = q_j) as (y_j - alpha_j q_j) / beta_j and written back to vio
+  R* vio;
   int64_t dim;
   const uint64_t* binom;              // [(N+1)*(K+1)] global
   const uint2* clt;
@@ -166,7 +168,17 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
     const uint64_t base = p.mode == FTLM_INDEX_CLT ? passb_run_start<FTLM_INDEX_CLT>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt)
                                                    : passb_run_start<FTLM_INDEX_CR>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt);
     const int tlen = s_tlen[kT];
-    {                                                   // stage the tile: every copy in flight at once
+    if (p.lazy) {                                       // lazy normalisation: q_{j+1} formed while staging, written over y_j
+      const R a = (R)p.st->a, ib = (R)p.st->inv_b;
+      R* yq = p.vio + base;
+      const R* qs = qprev + base;
+#pragma unroll 8
+      for (int x = tid; x < tlen; x += NT) {
+        const R qn = (yq[x] - a * qs[x]) * ib;
+        S.vs[x] = qn;
+        yq[x] = qn;
+      }
+    } else {                                            // stage the tile: every copy in flight at once
       const R* src = v + base;
       for (int x = tid; x < tlen; x += NT) cp_async_elem(&S.vs[x], &src[x]);
     }
@@ -393,7 +405,7 @@ int launch_tmlr_ml(ftlm_ctx* c, const TmlrParams<R>& p, int grid, size_t smem, c
 }
 
 template <typename R>
-int launch_tmlr(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
+int launch_tmlr(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s, void* vio = nullptr) {
   TmlrPlan* t = c->tmlr;
   TmlrParams<R> p;
   memset(&p, 0, sizeof(p));
@@ -405,6 +417,7 @@ int launch_tmlr(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, 
   }
   p.n_ll = t->n_ll; p.n_mm = t->n_mm; p.n_ml = t->n_ml; p.max_tile = t->max_tile;
   p.mode = c->mode; p.fused = fused;
+  p.lazy = vio ? 1 : 0; p.vio = (R*)vio;
   p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.blob = t->d_blob; p.blob_bytes = t->blob_bytes;
   p.off_koff = t->off_koff; p.off_tlen = t->off_tlen; p.off_coloff = t->off_coloff; p.off_mlist = t->off_mlist;
   p.off_moff = t->off_moff; p.off_ll = t->off_ll; p.off_fl = t->off_fl;
@@ -593,4 +606,13 @@ int ftlm_launch_hv_tmlr(ftlm_ctx* c, const void* v, const void* qprev, void* y, 
   if (!c->tmlr) { ftlm_set_error("TMLR kernel unavailable"); return FTLM_EUNSUPPORTED; }
   if (c->prec == FTLM_FP32) return launch_tmlr<float>(c, v, qprev, y, fused, s);
   return launch_tmlr<double>(c, v, qprev, y, fused, s);
+}
+
+bool ftlm_tmlr_lazy_ok(const ftlm_ctx* c) { return c->use_tmlr && c->tmlr && c->tmlr->n_g == 0; }
+
+int ftlm_launch_hv_tmlr_lazy(ftlm_ctx* c, void* yq, const void* q, void* y, int fused, cudaStream_t s) {
+  if (!ftlm_tmlr_lazy_ok(c) || !fused) { ftlm_set_error("TMLR lazy pass unavailable"); return FTLM_EUNSUPPORTED; }
+  // v is only read through vio in this form (n_g == 0: no reads of other tiles); q is q_j = this step's q_prev
+  if (c->prec == FTLM_FP32) return launch_tmlr<float>(c, yq, q, y, fused, s, yq);
+  return launch_tmlr<double>(c, yq, q, y, fused, s, yq);
 }

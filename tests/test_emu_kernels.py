@@ -160,3 +160,27 @@ def test_emu_config4_full_size_sampled_tiles_and_items():
     assert d["ok"] and d["windows"] == 2 and d["kernel"] == K["tml"], d
     assert {x["pass"] for x in d["passes"]} == {0, 1, 2} and {x.get("tmlr") for x in d["passes"] if x["pass"] == 0} == {0, 1}
     assert all(x["ok"] for x in d["passes"])
+
+
+def test_emu_lazy_normalisation_matches_separate_pass():
+    """Option lazy_norm: the TMLR pass forms q_{j+1} = (y_j - alpha_j q_j)/beta_j while staging its tile (no
+    normalisation kernel, buffers rotate by three).  Same arithmetic, so alpha and beta must be identical."""
+    code = ("import sys, json; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+            "import numpy as np, emu_harness as E\n"
+            "from paper_2605_26261_b200 import workloads as W\n"
+            "w = W.relabel(W.ring(14, 1.0, 0.5), W.fold_order(14))\n"
+            "out = {}\n"
+            "for prec, mode in (('fp32', 'clt'), ('fp64', 'cr')):\n"
+            "    res = []\n"
+            "    for lazy in (0, 1):\n"
+            "        opts = [('passb', 1), ('passb_lo_min', 4), ('tml_split', 5 | (3 << 8)), ('kernel', 3), ('tmlr', 1), ('lazy_norm', lazy)]\n"
+            "        with E.EmuCtx(w, 7, mode, prec, options=opts) as c:\n"
+            "            assert c.get('lazy_norm_ok') == 1 and c.get('passb_windows') >= 1\n"
+            "            res.append(c.lanczos(W.SEED_VECTORS, 2, 10))\n"
+            "    out[prec] = [float(np.abs(res[0][k] - res[1][k]).max()) for k in ('alpha', 'beta')] + [int(res[1]['m_eff'].min())]\n"
+            "print(json.dumps(out))\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    d = json.loads(p.stdout.strip().splitlines()[-1])
+    for prec in ("fp32", "fp64"):
+        assert d[prec][0] <= 1e-12 and d[prec][1] <= 1e-12 and d[prec][2] == 10, d

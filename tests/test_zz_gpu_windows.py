@@ -46,8 +46,10 @@ def test_windows_match_oracle(wl, n_up, mode, prec, opts, nwin):
     ("fring22j", 11, "clt", "fp32", [["passb", 1]]),
     ("fring24j", 12, "cr", "fp32", [["passb", 1]]),
 ])
-def test_tmlr_in_tile_pass_matches_oracle(wl, n_up, mode, prec, opts):
-    d = run({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec, "options": opts + [["kernel", 3], ["tmlr", 1]],
+@pytest.mark.parametrize("lazy", [0, 1])
+def test_tmlr_in_tile_pass_matches_oracle(wl, n_up, mode, prec, opts, lazy):
+    d = run({"wl": wl, "n_up": n_up, "mode": mode, "prec": prec,
+             "options": opts + [["kernel", 3], ["tmlr", 1], ["lazy_norm", lazy]],
              "what": ["apply", "lanczos"], "steps": 8})
     assert d["kernel"] == 3 and d["tmlr"] == [1, 1], d
 
