@@ -70,13 +70,14 @@ int64_t ftlm_dim(const ftlm_ctx* ctx);
  * 6.4-6.5): "passb" (1 = bonds that leave the tile go to PASS-B window passes; default 0),
  * "passb_lo_min" / "passb_smax" / "passb_ctas" (window planner: lowest label position, largest
  * window, CTAs per SM tried first; 0 = auto), "tmlr" (1 = in-tile pass by the TMLR kernel when its
- * plan exists), "tmlr_unij" (0 = never use the uniform-J form).  Test hooks: "debug_pass_mask",
+ * plan exists), "tmlr_unij" (0 = never use the uniform-J form), "lazy_norm" (1 = no separate
+ * normalisation pass in a chain: the TMLR pass forms q_{j+1} while staging; needs "tmlr").  Test hooks: "debug_pass_mask",
  * "debug_item_first", "debug_item_count" (run only some passes / tiles / items of a non-fused
  * H.v; used by the host emulation tests).  FTLM_EINVAL on unknown key/value, FTLM_EUNSUPPORTED
  * when the requested kernel / split cannot be built for this sector.  ftlm_get_option also answers
  * read-only keys: "sm_count", "autotuned", "tml_w", "tml_m", "tml_smem", "tml_ctas_per_sm",
  * "tml_threads", "tml_tiles", "tml_n_ll|mm|ml|tt|tm|tl", "tml_bclass:<b>", "tmlr_available",
- * "tmlr_smem", "tmlr_n_ll|mm|ml", "tmlr_unij_used", "passb_windows", "passb_bonds",
+ * "tmlr_smem", "tmlr_n_ll|mm|ml|g", "tmlr_unij_used", "lazy_norm_ok", "passb_windows", "passb_bonds",
  * "passb_lo<k>", "passb_mask<k>", "passb_nbonds<k>", "passb_items<k>", "passb_ctas_used". */
 int ftlm_set_option(ftlm_ctx* ctx, const char* key, int64_t value);
 int64_t ftlm_get_option(const ftlm_ctx* ctx, const char* key);

@@ -172,11 +172,23 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
       const R a = (R)p.st->a, ib = (R)p.st->inv_b;
       R* yq = p.vio + base;
       const R* qs = qprev + base;
-#pragma unroll 8
-      for (int x = tid; x < tlen; x += NT) {
-        const R qn = (yq[x] - a * qs[x]) * ib;
-        S.vs[x] = qn;
-        yq[x] = qn;
+      for (int x0 = tid; x0 < tlen; x0 += 8 * NT) {     // 16 loads in flight per thread before the first store
+        R yv[8], qv[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int x = x0 + k * NT;
+          yv[k] = x < tlen ? __ldcs(&yq[x]) : (R)0;
+          qv[k] = x < tlen ? qs[x] : (R)0;
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int x = x0 + k * NT;
+          if (x < tlen) {
+            const R qn = (yv[k] - a * qv[k]) * ib;
+            S.vs[x] = qn;
+            yq[x] = qn;
+          }
+        }
       }
     } else {                                            // stage the tile: every copy in flight at once
       const R* src = v + base;
