@@ -143,15 +143,17 @@ def run_reference(args, w, n_up):
 CANDIDATES = {
     "row": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 1)],
     "tile": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 2)],
-    "tml": [("lazy_norm", 0), ("tmlr", 0), ("passb", 0), ("kernel", 3)],
-    "tml+passb": [("tmlr", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
-    "tml+passb_1cta": [("tmlr", 0), ("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
-    "tml+passb_s11": [("tmlr", 0), ("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
-    "tml+passb_s10": [("tmlr", 0), ("passb_smax", 10), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
-    "tmlr+passb": [("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
-    "tmlr+passb_s11": [("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
-    "tmlr+passb_lazy": [("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1), ("lazy_norm", 1)],
-    "tmlr+passb_s11_lazy": [("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1), ("lazy_norm", 1)],
+    "tml": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 0), ("passb", 0), ("kernel", 3)],
+    "tml+passb": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tml+passb_1cta": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
+    "tml+passb_s11": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tml+passb_s10": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 10), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
+    "tmlr+passb": [("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
+    "tmlr+passb_s11": [("tml_split", 0), ("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1)],
+    "tmlr+passb_lazy": [("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1), ("lazy_norm", 1)],
+    "tmlr+passb_s11_lazy": [("tml_split", 0), ("passb_smax", 11), ("passb_ctas", 0), ("passb", 1), ("kernel", 3), ("tmlr", 1), ("lazy_norm", 1)],
+    "tml_w9m7": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 9 | (7 << 8)), ("passb", 0), ("kernel", 3)],
+    "tml_w9m7+passb": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 9 | (7 << 8)), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
 }
 SAFE_CHOICE = "tml"          # measured on B200 in round 1 (profiles/): the fallback if the probe dies
 

@@ -35,12 +35,15 @@ diff_norm_kernel(const R* __restrict__ a, const R* __restrict__ ref, int64_t n, 
 
 struct Cand {
   const char* name;
-  int kernel, passb, smax, ctas, tmlr, lazy;
+  int kernel, passb, smax, ctas, tmlr, lazy, split;   // split: w | m << 8 of the TML tile (0 = auto)
 };
 
-int apply_cand(ftlm_ctx* c, const Cand& k) {
+// home_split: the split the handle had when tuning began (candidates with split == 0 keep it)
+int apply_cand(ftlm_ctx* c, const Cand& k, int home_split) {
   int rc;
   if (k.kernel == FTLM_KERNEL_TML) {
+    const int want = k.split ? k.split : home_split;
+    if ((c->tml_low_bits | (c->tml_mid_bits << 8)) != want && (rc = ftlm_set_option(c, "tml_split", want)) != FTLM_OK) return rc;
     if ((rc = ftlm_set_option(c, "passb_smax", k.smax)) != FTLM_OK) return rc;
     if ((rc = ftlm_set_option(c, "passb_ctas", k.ctas)) != FTLM_OK) return rc;
     if ((rc = ftlm_set_option(c, "passb", k.passb)) != FTLM_OK) return rc;
@@ -73,19 +76,23 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
     ftlm_set_error("ftlm_autotune: cannot allocate 3 x %zu bytes", bytes);
     return FTLM_ENOMEM;
   }
-  const int saved_kernel = c->kernel, saved_pb = c->use_passb, saved_smax = c->passb_smax, saved_ctas = c->passb_ctas, saved_tmlr = c->use_tmlr, saved_lazy = c->lazy_norm;
+  const int saved_kernel = c->kernel, saved_pb = c->use_passb, saved_smax = c->passb_smax, saved_ctas = c->passb_ctas, saved_tmlr = c->use_tmlr, saved_lazy = c->lazy_norm,
+            saved_w = c->tml_low_bits, saved_m = c->tml_mid_bits;
+  const int home_split = saved_w | (saved_m << 8);
   const Cand cands[] = {
-      {"row", FTLM_KERNEL_ROW, 0, 0, 0, 0, 0},
-      {"tile", FTLM_KERNEL_TILE, 0, 0, 0, 0, 0},
-      {"tml", FTLM_KERNEL_TML, 0, 0, 0, 0, 0},
-      {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0, 0, 0},
-      {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1, 0, 0},
-      {"tml+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 0, 0},
-      {"tml+passb_s10", FTLM_KERNEL_TML, 1, 10, 0, 0, 0},
-      {"tmlr+passb", FTLM_KERNEL_TML, 1, 0, 0, 1, 0},
-      {"tmlr+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 1, 0},
-      {"tmlr+passb_lazy", FTLM_KERNEL_TML, 1, 0, 0, 1, 1},
-      {"tmlr+passb_s11_lazy", FTLM_KERNEL_TML, 1, 11, 0, 1, 1},
+      {"row", FTLM_KERNEL_ROW, 0, 0, 0, 0, 0, 0},
+      {"tile", FTLM_KERNEL_TILE, 0, 0, 0, 0, 0, 0},
+      {"tml", FTLM_KERNEL_TML, 0, 0, 0, 0, 0, 0},
+      {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0, 0, 0, 0},
+      {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1, 0, 0, 0},
+      {"tml+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 0, 0, 0},
+      {"tml+passb_s10", FTLM_KERNEL_TML, 1, 10, 0, 0, 0, 0},
+      {"tmlr+passb", FTLM_KERNEL_TML, 1, 0, 0, 1, 0, 0},
+      {"tmlr+passb_s11", FTLM_KERNEL_TML, 1, 11, 0, 1, 0, 0},
+      {"tmlr+passb_lazy", FTLM_KERNEL_TML, 1, 0, 0, 1, 1, 0},
+      {"tmlr+passb_s11_lazy", FTLM_KERNEL_TML, 1, 11, 0, 1, 1, 0},
+      {"tml_w9m7", FTLM_KERNEL_TML, 0, 0, 0, 0, 0, 9 | (7 << 8)},              // the split measured in round 1 (2 CTAs/SM)
+      {"tml_w9m7+passb", FTLM_KERNEL_TML, 1, 0, 0, 0, 0, 9 | (7 << 8)},
   };
   const int ncand = (int)(sizeof(cands) / sizeof(cands[0]));
   const double tol = c->prec == FTLM_FP32 ? 1e-5 : 1e-12;
@@ -106,13 +113,13 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
   const double tol_f = c->prec == FTLM_FP32 ? 1e-4 : 1e-9;
   // reference: the ROW kernel on a seeded random vector, and its fused steps
   rc = ftlm_fill_random(c, 0x5EEDull, 0, v, s);
-  if (rc == FTLM_OK) rc = apply_cand(c, cands[0]);
+  if (rc == FTLM_OK) rc = apply_cand(c, cands[0], home_split);
   if (rc == FTLM_OK) rc = ftlm_apply_H(c, v, yref, s);
   if (rc == FTLM_OK) rc = fused_probe(ab_ref);
   for (int k = 0; k < ncand && rc == FTLM_OK; ++k) {
     const Cand& cd = cands[k];
     if (cd.kernel == FTLM_KERNEL_TILE && !c->tile) continue;
-    if (apply_cand(c, cd) != FTLM_OK) continue;                          // not available for this sector
+    if (apply_cand(c, cd, home_split) != FTLM_OK) continue;                          // not available for this sector
     if (cd.kernel == FTLM_KERNEL_TML && (!c->tml || (cd.passb && !c->passb) || (cd.tmlr && !c->tmlr) || (cd.lazy && !ftlm_tmlr_lazy_ok(c)))) continue;
     double h_out[2] = {0.0, 0.0};
     if (cudaMemsetAsync(d_out, 0, 16, s) != cudaSuccess) { rc = FTLM_ECUDA; break; }
@@ -155,10 +162,11 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
     rep += line;
   }
   rep += "]";
-  if (rc == FTLM_OK && best >= 0) rc = apply_cand(c, cands[best]);
+  if (rc == FTLM_OK && best >= 0) rc = apply_cand(c, cands[best], home_split);
   else {                                                                  // restore what the caller had
     c->passb_smax = saved_smax; c->passb_ctas = saved_ctas; c->use_tmlr = saved_tmlr; c->lazy_norm = saved_lazy;
-    ftlm_set_option(c, "passb", saved_pb);
+    c->use_passb = saved_pb;
+    ftlm_set_option(c, "tml_split", saved_w | (saved_m << 8));
     c->kernel = saved_kernel;
     if (rc == FTLM_OK) { ftlm_set_error("ftlm_autotune: no valid candidate"); rc = FTLM_EUNSUPPORTED; }
   }
