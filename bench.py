@@ -155,7 +155,7 @@ CANDIDATES = {
     "tml_w9m7": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 9 | (7 << 8)), ("passb", 0), ("kernel", 3)],
     "tml_w9m7+passb": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 9 | (7 << 8)), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
 }
-SAFE_CHOICE = "tml"          # measured on B200 in round 1 (profiles/): the fallback if the probe dies
+SAFE_CHOICE = "tml_w9m7"     # the kernel and launch shape measured on B200 in round 1 (profiles/): fallback if the probe dies
 
 
 def run_probe(args):
