@@ -41,6 +41,7 @@ struct PassBParams {
   const uint32_t* nbr_off;          // [2^s][32], row = position of u in ustate: byte offset of row slot(u') in the tile; [31] = number of entries
   const R* nbr_J;                   // [2^s][32]: J_b/2 of the same entries; [31] = their sum
   const uint32_t* grp_first;        // [ngroups+1]: first item of group g = F*(s+1) + p_S
+  const uint32_t* item_group;       // [nitems]: group of every item
   double* partials;                 // [3][nitems]
   unsigned int* counter;            // [0] item counter, [1] ticket
   ChainState* st;
@@ -64,6 +65,7 @@ struct PassBWindow {
   uint32_t* d_nbr = nullptr;          // byte offsets
   void* d_nbrJ = nullptr;             // J_b/2 in the handle's precision
   uint32_t* d_grp_first = nullptr;
+  uint32_t* d_item_group = nullptr;
   double* d_partials = nullptr;
   unsigned int* d_counter = nullptr;
 };
@@ -214,13 +216,7 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     __syncthreads();
     const uint32_t item = s_item + p.item_begin;
     if (item >= p.item_end) break;
-    // group of this item: last g with grp_first[g] <= item (uniform binary search)
-    int g0 = 0, g1 = p.ngroups;
-    while (g1 - g0 > 1) {
-      const int gm = (g0 + g1) >> 1;
-      if (__ldg(&p.grp_first[gm]) <= item) g0 = gm; else g1 = gm;
-    }
-    const int g = g0;
+    const int g = (int)__ldg(&p.item_group[item]);      // group g = F * (s+1) + p_S of this item
     const uint32_t F = (uint32_t)(g / s1);
     const int pS = g - (int)F * s1;
     const int kP = p.K - __popc(F) - pS;                // in [0, lo] by construction of the groups
@@ -342,7 +338,7 @@ void ftlm_passb_plan_destroy(ftlm_ctx* c) {
   PassBSet* S = c->passb;
   if (!S) return;
   for (PassBWindow& w : S->win) {
-    cudaFree(w.d_ustate); cudaFree(w.d_koff); cudaFree(w.d_nbr); cudaFree(w.d_nbrJ); cudaFree(w.d_grp_first);
+    cudaFree(w.d_ustate); cudaFree(w.d_koff); cudaFree(w.d_nbr); cudaFree(w.d_nbrJ); cudaFree(w.d_grp_first); cudaFree(w.d_item_group);
     cudaFree(w.d_partials); cudaFree(w.d_counter);
   }
   delete S;
@@ -535,6 +531,9 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
       ustate[(size_t)fill[(size_t)p]++] = (uint16_t)u;
     }
     const size_t esz = ftlm_elem_size(c);
+    std::vector<uint32_t> item_group((size_t)w.nitems);
+    for (int g = 0; g < w.ngroups; ++g)
+      for (uint32_t it = groups[wi][(size_t)g]; it < groups[wi][(size_t)g + 1]; ++it) item_group[it] = (uint32_t)g;
     std::vector<uint32_t> nbr((size_t)nU * 32, 0u);
     std::vector<double> nbrJ((size_t)nU * 32, 0.0);
     for (int u = 0; u < nU; ++u) {
@@ -568,6 +567,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
               up((void**)&w.d_nbr, nbr.data(), nbr.size() * 4) &&
               up(&w.d_nbrJ, esz == 4 ? (const void*)nbrJf.data() : (const void*)nbrJ.data(), nbrJ.size() * esz) &&
               up((void**)&w.d_grp_first, groups[wi].data(), groups[wi].size() * 4) &&
+              up((void**)&w.d_item_group, item_group.data(), item_group.size() * 4) &&
               up((void**)&w.d_partials, nullptr, pbytes) && up((void**)&w.d_counter, nullptr, 16);
     if (ok) ok = cudaMemset(w.d_partials, 0, pbytes) == cudaSuccess && cudaMemset(w.d_counter, 0, 16) == cudaSuccess;
     if (!ok) { cudaGetLastError(); ftlm_passb_plan_destroy(c); ftlm_set_error("PASS-B: table upload failed"); return FTLM_ENOMEM; }
@@ -581,7 +581,7 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   memset(&p, 0, sizeof(p));
   p.N = c->N; p.K = c->N_up; p.lo = w.lo; p.s = w.s; p.f = w.f; p.ngroups = w.ngroups; p.nitems = w.nitems;
   p.dim = c->dim; p.binom = c->d_binom64; p.clt = c->d_clt; p.ustate = w.d_ustate; p.koff = w.d_koff;
-  p.nbr_off = w.d_nbr; p.nbr_J = (const R*)w.d_nbrJ; p.grp_first = w.d_grp_first; p.partials = w.d_partials; p.counter = w.d_counter;
+  p.nbr_off = w.d_nbr; p.nbr_J = (const R*)w.d_nbrJ; p.grp_first = w.d_grp_first; p.item_group = w.d_item_group; p.partials = w.d_partials; p.counter = w.d_counter;
   p.st = c->d_state; p.max_conf = w.max_conf;
   p.unij = c->unij_allowed ? 1 : 0;
   for (size_t e = 1; e < w.Jh.size(); ++e) if (w.Jh[e] != w.Jh[0]) p.unij = 0;
