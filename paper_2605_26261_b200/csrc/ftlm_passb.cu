@@ -210,12 +210,13 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
   int cur_group = -1;
   const int s1 = p.s + 1;
 
+  if (tid == 0) s_item = atomicAdd(&p.counter[0], 1u);
   for (;;) {
-    __syncthreads();                                   // previous item done: tile, starts reusable
-    if (tid == 0) s_item = atomicAdd(&p.counter[0], 1u);
-    __syncthreads();
+    __syncthreads();                                   // previous item done (tile, starts reusable), next item id visible
     const uint32_t item = s_item + p.item_begin;
+    __syncthreads();                                   // everyone has read it
     if (item >= p.item_end) break;
+    if (tid == 0) s_item = atomicAdd(&p.counter[0], 1u);   // the following item's id travels while this item is processed
     const int g = (int)__ldg(&p.item_group[item]);      // group g = F * (s+1) + p_S of this item
     const uint32_t F = (uint32_t)(g / s1);
     const int pS = g - (int)F * s1;

@@ -157,12 +157,13 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
   const int n_mm = p.n_mm;
   constexpr int n_ml = NML;
 
+  if (tid == 0) S.misc[0] = (int)atomicAdd(&p.counter[0], 1u);
   for (;;) {
-    __syncthreads();                                   // previous tile done: tile and descriptors reusable
-    if (tid == 0) S.misc[0] = (int)atomicAdd(&p.counter[0], 1u);
-    __syncthreads();
+    __syncthreads();                                   // previous tile done (tile and descriptors reusable), next tile id visible
     const uint32_t T = (uint32_t)S.misc[0] + p.t_begin;
+    __syncthreads();                                   // everyone has read it
     if (T >= p.t_end) break;
+    if (tid == 0) S.misc[0] = (int)atomicAdd(&p.counter[0], 1u);   // the following tile's id travels while this tile is processed
     const int kT = p.K - __popc(T);
     if (kT < 0 || kT > p.mw) continue;                  // no rows with this top part
     const uint64_t base = p.mode == FTLM_INDEX_CLT ? passb_run_start<FTLM_INDEX_CLT>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt)
