@@ -242,10 +242,6 @@ def main():
     ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, local)
     if args.low_bits:
         ftlm.ftlm_set_option(ctx, "low_bits", args.low_bits)
-    if args.tml_low_bits:
-        ftlm.ftlm_set_option(ctx, "tml_low_bits", args.tml_low_bits)
-    if args.tml_mid_bits:
-        ftlm.ftlm_set_option(ctx, "tml_mid_bits", args.tml_mid_bits)
     autotune_report, probe_note = None, None
     if args.candidate:
         choice = args.candidate
@@ -257,6 +253,10 @@ def main():
         choice = {"row": "row", "tile": "tile", "tml": "tml"}[args.kernel]
     for key, val in CANDIDATES[choice]:
         ftlm.ftlm_set_option(ctx, key, val)
+    if args.tml_low_bits:                                        # explicit split flags win over the candidate's
+        ftlm.ftlm_set_option(ctx, "tml_low_bits", args.tml_low_bits)
+    if args.tml_mid_bits:
+        ftlm.ftlm_set_option(ctx, "tml_mid_bits", args.tml_mid_bits)
     kernel_used = {1: "row", 2: "tile", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
     if kernel_used == "tml" and ftlm.ftlm_get_option(ctx, "tmlr") == 1 and ftlm.ftlm_get_option(ctx, "tmlr_available") == 1:
         kernel_used = "tmlr"
