@@ -1,6 +1,7 @@
 // cuda_emu.cpp - TEST INFRASTRUCTURE: fiber scheduler and guarded "device" memory behind cuda_emu.h.
 #include "cuda_emu.h"
 
+#include <cstdlib>
 #include <sys/mman.h>
 #include <time.h>
 #include <ucontext.h>
@@ -132,10 +133,23 @@ void run_block() {
     g_warps[i >> 5].alive_mask |= 1u << (i & 31);
   }
   g_alive = nt; g_bar_arrived = 0; g_bar_gen = 0;
+  // FTLM_EMU_ORDER: order in which runnable threads are resumed in every scheduling round - 0 ascending
+  // (default), 1 descending, n >= 2 a fresh pseudo-random permutation per round (seed n).  A kernel whose
+  // result depends on this order has a race (missing __syncthreads / __syncwarp); the tests run all three.
+  static const int order_mode = getenv("FTLM_EMU_ORDER") ? atoi(getenv("FTLM_EMU_ORDER")) : 0;
+  static unsigned long long rng = 0x9E3779B97F4A7C15ull * (unsigned long long)(order_mode + 1);
+  std::vector<unsigned> order(nt);
+  for (unsigned i = 0; i < nt; ++i) order[i] = order_mode == 1 ? nt - 1 - i : i;
   for (;;) {
     const unsigned long long before = g_progress;
     bool any = false;
-    for (unsigned i = 0; i < nt; ++i) {
+    if (order_mode >= 2)
+      for (unsigned i = nt - 1; i > 0; --i) {
+        rng ^= rng << 13; rng ^= rng >> 7; rng ^= rng << 17;
+        std::swap(order[i], order[(unsigned)(rng % (i + 1))]);
+      }
+    for (unsigned oi = 0; oi < nt; ++oi) {
+      const unsigned i = order[oi];
       Fiber& f = g_fib[i];
       if (f.done) continue;
       any = true;

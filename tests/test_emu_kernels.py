@@ -20,8 +20,9 @@ RUN = os.path.join(ROOT, "tests", "emu", "run_case.py")
 K = {"row": 1, "tile": 2, "tml": 3}
 
 
-def run_case(spec, timeout=600):
-    p = subprocess.run([sys.executable, RUN, json.dumps(spec)], capture_output=True, text=True, timeout=timeout)
+def run_case(spec, timeout=600, order=None):
+    env = dict(os.environ, FTLM_EMU_ORDER=str(order)) if order is not None else None
+    p = subprocess.run([sys.executable, RUN, json.dumps(spec)], capture_output=True, text=True, timeout=timeout, env=env)
     assert p.returncode == 0, f"emulated case died (rc={p.returncode}): {spec}\n{p.stderr[-2000:]}"
     res = json.loads(p.stdout.strip().splitlines()[-1])
     assert res["ok"], (spec, res)
@@ -184,3 +185,17 @@ def test_emu_lazy_normalisation_matches_separate_pass():
     d = json.loads(p.stdout.strip().splitlines()[-1])
     for prec in ("fp32", "fp64"):
         assert d[prec][0] <= 1e-12 and d[prec][1] <= 1e-12 and d[prec][2] == 10, d
+
+
+@pytest.mark.parametrize("order", [1, 5])
+def test_emu_result_does_not_depend_on_thread_schedule(order):
+    """The emulation resumes runnable threads in ascending order by default; descending (1) and pseudo-random (>= 2)
+    orders must give the same result - a difference would be a race (missing __syncthreads / __syncwarp)."""
+    spec = {"wl": "fring14j", "n_up": 7, "mode": "clt", "prec": "fp64",
+            "options": [["passb", 1], ["passb_lo_min", 4], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]], ["tmlr", 1],
+                        ["lazy_norm", 1]], "what": ["apply", "lanczos"], "steps": 6}
+    ref = run_case(spec)
+    res = run_case(spec, order=order)
+    assert res["hv_relerr"] == ref["hv_relerr"] and res["lanczos_dalpha"] == ref["lanczos_dalpha"]
+    spec["options"] = [["passb", 1], ["passb_lo_min", 4], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]]
+    assert run_case(spec, order=order)["hv_relerr"] == run_case(spec)["hv_relerr"]
