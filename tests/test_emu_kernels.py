@@ -150,11 +150,11 @@ def test_emu_autotune_checks_every_candidate_against_row():
 
 
 def test_emu_config4_full_size_sampled_tiles_and_items():
-    """BASELINE config 4 (D = 155 117 520) at full size: sampled tiles of the TML pass and sampled items of
+    """BASELINE config 4 (D = 155 117 520) at full size, in the index mode bench.py times (CLT, 268 MB table): sampled tiles of the TML pass and sampled items of
     both PASS-B windows (in-tile pass: TMLR and TML) run through the emulation with the real run starts and offsets; the rows each
     pass writes and their values must be the oracle's (and nothing may touch a guard page)."""
     p = subprocess.run([sys.executable, os.path.join(ROOT, "tests", "emu", "run_sampled.py"),
-                        json.dumps({"config": 4, "mode": "cr", "samples": 1, "options": [["tmlr", 1]], "tmlr_both": True})],
+                        json.dumps({"config": 4, "mode": "clt", "samples": 1, "options": [["tmlr", 1]], "tmlr_both": True})],
                        capture_output=True, text=True, timeout=1500)
     assert p.returncode == 0, p.stderr[-2000:]
     d = json.loads(p.stdout.strip().splitlines()[-1])
