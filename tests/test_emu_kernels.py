@@ -147,6 +147,8 @@ def test_emu_autotune_checks_every_candidate_against_row():
     names = [r["name"] for r in d["rep"]]
     assert names[0] == "row" and "tml" in names and "tml+passb" in names and "tmlr+passb" in names
     assert all(r["valid"] and r["relerr"] <= 1e-5 for r in d["rep"]) and d["tuned"] >= 1
+    import bench
+    assert set(names) <= set(bench.CANDIDATES), set(names) - set(bench.CANDIDATES)   # bench.py can apply whatever is chosen
 
 
 def test_emu_config4_full_size_sampled_tiles_and_items():
@@ -197,3 +199,26 @@ def test_emu_result_does_not_depend_on_thread_schedule(order):
     ref = run_case(spec)
     res = run_case(spec, order=order)
     assert res["hv_relerr"] == ref["hv_relerr"] and res["lanczos_dalpha"] == ref["lanczos_dalpha"]
+
+
+def test_bench_candidates_are_valid_option_lists():
+    """Every configuration bench.py can select (its CANDIDATES table = the names ftlm_autotune reports) must be a list of
+    options the library accepts, on the bench sector itself (plans only; nothing is launched)."""
+    code = ("import sys, json; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+            "import emu_harness as E, bench\n"
+            "from paper_2605_26261_b200 import workloads as W\n"
+            "w = W.baseline_config(4)\n"
+            "out = {}\n"
+            "with E.EmuCtx(w, w.sectors[0], 'cr', 'fp32') as c:\n"
+            "    for name, opts in bench.CANDIDATES.items():\n"
+            "        for k, v in opts:\n"
+            "            c.set(k, v)\n"
+            "        out[name] = [c.get('kernel'), c.get('passb_windows'), c.get('tmlr'), c.get('tmlr_available'), c.get('lazy_norm'), c.get('tml_m')]\n"
+            "print(json.dumps(out))\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    d = json.loads(p.stdout.strip().splitlines()[-1])
+    assert d["row"][0] == K["row"] and d["tile"][0] == K["tile"] and d["tml"][:2] == [K["tml"], 0]
+    assert d["tml+passb"][:2] == [K["tml"], 2] and d["tmlr+passb"][:4] == [K["tml"], 2, 1, 1]
+    assert d["tmlr+passb_lazy"][4] == 1 and d["tml"][4] == 0
+    assert d["tml_w9m7"][5] == 7 and d["tml"][5] == 8 and d["tml_w9m7+passb"][1] >= 1
