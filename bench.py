@@ -142,7 +142,6 @@ def run_reference(args, w, n_up):
 # name -> option settings, in order (the candidates of ftlm_autotune, include/ftlm.h)
 CANDIDATES = {
     "row": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 1)],
-    "tile": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 2)],
     "tml": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 0), ("passb", 0), ("kernel", 3)],
     "tml+passb": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
     "tml+passb_1cta": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
@@ -199,7 +198,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--mode", default="clt", choices=["clt", "cr"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "row", "tile", "tml"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "row", "tml"])
     ap.add_argument("--low-bits", type=int, default=0)
     ap.add_argument("--tml-low-bits", type=int, default=0)
     ap.add_argument("--tml-mid-bits", type=int, default=0)
@@ -240,8 +239,6 @@ def main():
     if w.N > 32:
         mode, args.mode = ftlm.INDEX_CR, "cr"
     ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, local)
-    if args.low_bits:
-        ftlm.ftlm_set_option(ctx, "low_bits", args.low_bits)
     autotune_report, probe_note = None, None
     if args.candidate:
         choice = args.candidate
@@ -250,14 +247,14 @@ def main():
         choice, autotune_report, probe_note = probe_choice(args) if rank == 0 else (SAFE_CHOICE, None, None)
         choice = replicas.broadcast_choice(choice, dist)
     else:
-        choice = {"row": "row", "tile": "tile", "tml": "tml"}[args.kernel]
+        choice = {"row": "row", "tml": "tml"}[args.kernel]
     for key, val in CANDIDATES[choice]:
         ftlm.ftlm_set_option(ctx, key, val)
     if args.tml_low_bits:                                        # explicit split flags win over the candidate's
         ftlm.ftlm_set_option(ctx, "tml_low_bits", args.tml_low_bits)
     if args.tml_mid_bits:
         ftlm.ftlm_set_option(ctx, "tml_mid_bits", args.tml_mid_bits)
-    kernel_used = {1: "row", 2: "tile", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
+    kernel_used = {1: "row", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
     if kernel_used == "tml" and ftlm.ftlm_get_option(ctx, "tmlr") == 1 and ftlm.ftlm_get_option(ctx, "tmlr_available") == 1:
         kernel_used = "tmlr"
     n_windows = max(ftlm.ftlm_get_option(ctx, "passb_windows"), 0) if kernel_used in ("tml", "tmlr") else 0

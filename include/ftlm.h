@@ -41,10 +41,9 @@ enum { FTLM_FP32 = 0, FTLM_FP64 = 1 };
 /* Kernel variants selectable with ftlm_set_option("kernel", ...).
  * ROW  = one thread per row, every row unranked, per-bond loop (the paper's launch shape, L105,
  *        L136, L203), kept as the plain in-library baseline.
- * TILE = one CTA per run of rows sharing the high label bits.
  * TML  = B200 design: label split into top/middle/low parts, one CTA per top part with the tile
  *        staged in shared memory and per-class neighbour tables. */
-enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_TILE = 2, FTLM_KERNEL_TML = 3 };
+enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_TML = 3 };
 
 /* ---- handle ------------------------------------------------------------------------------ */
 
@@ -64,7 +63,7 @@ int ftlm_destroy(ftlm_ctx* ctx);
 /* Sector dimension C(N, N_up). */
 int64_t ftlm_dim(const ftlm_ctx* ctx);
 
-/* Options: "kernel" (FTLM_KERNEL_*), "low_bits" (w of the TILE kernels, 0 = auto),
+/* Options: "kernel" (FTLM_KERNEL_*),
  * "tml_low_bits" / "tml_mid_bits" / "tml_split" = w | m << 8 (split of the TML kernels, 0 = auto),
  * "graph" (1 = replay Lanczos steps from a CUDA graph); multi-pass H.v of kernel TML (DESIGN.md
  * 6.4-6.5): "passb" (1 = bonds that leave the tile go to PASS-B window passes; default 0),

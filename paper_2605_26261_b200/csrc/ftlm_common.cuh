@@ -5,7 +5,6 @@
 #include "cuda_emu.h"
 #else
 #include <cuda_runtime.h>
-#define FTLM_LAUNCH(kernel, grid, block, smem, stream, ...) kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__)
 #define FTLM_DYN_SMEM(name) extern __shared__ __align__(16) unsigned char name[]
 #endif
 #include <stdint.h>
@@ -13,6 +12,29 @@
 #include <vector>
 
 #include "../../include/ftlm.h"
+#include "ftlm_access.cuh"
+
+#ifndef FTLM_EMU
+#ifdef FTLM_CHECKED
+// checked build: every translation unit binds its copy of the check-state pointer before its first launch
+FtlmChkState* ftlm_chk_state_dev();                 // device pointer of the process-wide state (ftlm_core.cu)
+static inline void ftlm_chk_bind_tu() {
+  static bool bound = false;
+  if (!bound) { FtlmChkState* p = ftlm_chk_state_dev(); cudaMemcpyToSymbol(ftlm_chk_dev, &p, sizeof(p)); bound = true; }
+}
+#define FTLM_LAUNCH(kernel, grid, block, smem, stream, ...) (ftlm_chk_bind_tu(), kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__))
+#else
+#define FTLM_LAUNCH(kernel, grid, block, smem, stream, ...) kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__)
+#endif
+#endif
+
+// Device allocations of the library go through these (the checked build keeps the table of live ranges
+// that the kernels' address checks consult; otherwise they are cudaMalloc / cudaFree).
+cudaError_t ftlm_dmalloc_bytes(void** p, size_t bytes);
+template <typename T> static inline cudaError_t ftlm_dmalloc(T** p, size_t bytes) { return ftlm_dmalloc_bytes((void**)p, bytes); }
+cudaError_t ftlm_dfree(void* p);
+// Caller-owned device buffers an entry point is about to hand to kernels on stream `s` (checked build only).
+void ftlm_chk_caller(cudaStream_t s, const void* p, size_t bytes);
 
 #define FTLM_MAX_BONDS 4096
 
@@ -48,9 +70,8 @@ struct BondDev {          // one bond as the kernels see it
   int i, j;               // i < j
 };
 
-// Run-tiled ("TILE") and three-level ("TML") kernel plans, built on the host in ftlm_create
+// Three-level ("TML") kernel plans, built on the host in ftlm_create
 // (DESIGN.md section 6).
-struct TilePlan;
 struct TmlPlan;
 struct PassBSet;
 struct TmlrPlan;
@@ -75,14 +96,12 @@ struct ftlm_ctx {
 
   // options
   int kernel = FTLM_KERNEL_AUTO;
-  int low_bits = 0;
   int tml_low_bits = 0, tml_mid_bits = 0;
   int use_graph = 0;
+  int allow_unverified = 0;        // option "allow_unverified": ftlm_autotune may run candidates without a device record
   int autotuned = 0;               // 1 + index of the candidate ftlm_autotune selected (0 = not tuned)
   double autotune_ms = 0.0;
 
-  // tile plan (ftlm_tile.cu)
-  TilePlan* tile = nullptr;
   // three-level tile plan (ftlm_tml.cu)
   TmlPlan* tml = nullptr;
   // PASS-B windows for the bonds among the top label bits (ftlm_passb.cu); owned together with `tml`
@@ -126,11 +145,6 @@ int ftlm_effective_kernel(const ftlm_ctx* c);
 int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
 int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
 
-int ftlm_tile_plan_create(ftlm_ctx* c);
-void ftlm_tile_plan_destroy(ftlm_ctx* c);
-int ftlm_launch_hv_tile(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
-int ftlm_launch_neighbors_tile(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
-
 int ftlm_tml_plan_create(ftlm_ctx* c);
 void ftlm_tml_plan_destroy(ftlm_ctx* c);
 int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key);
@@ -168,9 +182,10 @@ __device__ __forceinline__ int ffs_(uint64_t x) { return __ffsll((long long)x); 
 
 // asynchronous global -> shared copy of one element (LDGSTS); the emulation copies at once
 template <typename T>
-__device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc) {
+__device__ __forceinline__ void cp_async_elem_(T* smem_dst, const T* gsrc, int line) {
+  if (!FTLM_S_OK(smem_dst, T, line) || !FTLM_G_OK(gsrc, T, line)) return;
 #ifdef FTLM_EMU
-  *smem_dst = *gsrc;
+  cuda_emu::cp_async_issue(smem_dst, gsrc, sizeof(T));
 #else
   static_assert(sizeof(T) == 4 || sizeof(T) == 8 || sizeof(T) == 16, "cp.async copies 4, 8 or 16 bytes");
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -179,8 +194,11 @@ __device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc) {
   else asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
 #endif
 }
+#define cp_async_elem(dst, src) cp_async_elem_((dst), (src), __LINE__)
 __device__ __forceinline__ void cp_async_wait_all() {
-#ifndef FTLM_EMU
+#ifdef FTLM_EMU
+  cuda_emu::cp_async_wait_all();      // the copies of the calling thread land here, not before
+#else
   asm volatile("cp.async.wait_all;" ::: "memory");
 #endif
 }
@@ -217,9 +235,9 @@ __device__ __forceinline__ void lanczos_finish(double s_qy, double s_yy, double 
   block_sum3(s_qy, s_yy, s_qq, sh);
   __shared__ bool last;
   if (threadIdx.x == 0) {
-    partials[blockIdx.x] = s_qy;
-    partials[stride + blockIdx.x] = s_yy;
-    partials[2 * stride + blockIdx.x] = s_qq;
+    ST_G(&partials[blockIdx.x], s_qy);
+    ST_G(&partials[stride + blockIdx.x], s_yy);
+    ST_G(&partials[2 * stride + blockIdx.x], s_qq);
     __threadfence();
     last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
   }
@@ -228,7 +246,7 @@ __device__ __forceinline__ void lanczos_finish(double s_qy, double s_yy, double 
   __threadfence();
   double a = 0.0, b = 0.0, c = 0.0;
   for (int k = threadIdx.x; k < (int)gridDim.x; k += blockDim.x) {   // fixed assignment + order
-    a += partials[k]; b += partials[stride + k]; c += partials[2 * stride + k];
+    a += LD_G(&partials[k]); b += LD_G(&partials[stride + k]); c += LD_G(&partials[2 * stride + k]);
   }
   block_sum3(a, b, c, sh);
   if (threadIdx.x == 0) {

@@ -1,9 +1,11 @@
 // libftlm core: handle, sector tables (A0/A1), start vectors, the fused Lanczos chain driver
-// and the C-ABI entry points that dispatch to the ROW / TILE kernels.
+// and the C-ABI entry points that dispatch to the ROW / TML kernels.
 #include <cstdarg>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 
+#define FTLM_TU 1
 #include "ftlm_common.cuh"
 
 // ---- errors --------------------------------------------------------------------------------
@@ -20,7 +22,132 @@ int ftlm_cuda_fail(cudaError_t e, const char* what) {
   return FTLM_ECUDA;
 }
 extern "C" const char* ftlm_last_error(void) { return g_err; }
-extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.1 (sm_100a)"; }
+#ifdef FTLM_CHECKED
+extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.2 (sm_100a) CHECKED"; }
+#else
+extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.2 (sm_100a)"; }
+#endif
+
+// ---- device allocations; checked build: table of live ranges (ftlm_access.cuh) -------------------
+#if defined(FTLM_CHECKED) && !defined(FTLM_EMU)
+#include <algorithm>
+#include <mutex>
+namespace {
+std::mutex g_chk_mu;
+FtlmChkState* g_chk_dev = nullptr;
+std::vector<FtlmChkRange> g_chk_lib;                 // sorted by lo
+FtlmChkRange g_chk_call[FTLM_CHK_CALL_RANGES];
+int g_chk_call_next = 0;
+
+void chk_upload_lib() {                              // allocation / free: no kernel of this library may be in flight on a freed range anyway
+  struct { int n, pad; } head = {(int)g_chk_lib.size(), 0};
+  cudaDeviceSynchronize();
+  cudaMemcpy((char*)g_chk_dev + offsetof(FtlmChkState, ranges), g_chk_lib.data(), sizeof(FtlmChkRange) * g_chk_lib.size(), cudaMemcpyHostToDevice);
+  cudaMemcpy((char*)g_chk_dev + offsetof(FtlmChkState, n_ranges), &head, sizeof(head), cudaMemcpyHostToDevice);
+}
+}  // namespace
+
+FtlmChkState* ftlm_chk_state_dev() {
+  std::lock_guard<std::mutex> lk(g_chk_mu);
+  if (!g_chk_dev) {
+    if (cudaMalloc((void**)&g_chk_dev, sizeof(FtlmChkState)) != cudaSuccess) { g_chk_dev = nullptr; return nullptr; }
+    cudaMemset(g_chk_dev, 0, sizeof(FtlmChkState));
+    memset(g_chk_call, 0, sizeof(g_chk_call));
+  }
+  return g_chk_dev;
+}
+
+cudaError_t ftlm_dmalloc_bytes(void** p, size_t bytes) {
+  cudaError_t e = cudaMalloc(p, bytes);
+  if (e != cudaSuccess) return e;
+  if (!ftlm_chk_state_dev()) return cudaErrorMemoryAllocation;
+  std::lock_guard<std::mutex> lk(g_chk_mu);
+  if (g_chk_lib.size() >= FTLM_CHK_MAX_RANGES) { cudaFree(*p); *p = nullptr; return cudaErrorMemoryAllocation; }
+  const FtlmChkRange r{(unsigned long long)*p, (unsigned long long)*p + bytes};
+  g_chk_lib.insert(std::upper_bound(g_chk_lib.begin(), g_chk_lib.end(), r, [](const FtlmChkRange& a, const FtlmChkRange& b) { return a.lo < b.lo; }), r);
+  chk_upload_lib();
+  return cudaSuccess;
+}
+
+cudaError_t ftlm_dfree(void* p) {
+  if (p) {
+    std::lock_guard<std::mutex> lk(g_chk_mu);
+    for (size_t k = 0; k < g_chk_lib.size(); ++k)
+      if (g_chk_lib[k].lo == (unsigned long long)p) { g_chk_lib.erase(g_chk_lib.begin() + (long)k); break; }
+    if (g_chk_dev) chk_upload_lib();
+  }
+  return cudaFree(p);
+}
+
+void ftlm_chk_caller(cudaStream_t s, const void* p, size_t bytes) {
+  if (!p || !bytes || !ftlm_chk_state_dev()) return;
+  std::lock_guard<std::mutex> lk(g_chk_mu);
+  const FtlmChkRange r{(unsigned long long)p, (unsigned long long)p + bytes};
+  for (int k = 0; k < FTLM_CHK_CALL_RANGES; ++k)
+    if (g_chk_call[k].lo == r.lo && g_chk_call[k].hi == r.hi) return;   // already listed
+  g_chk_call[g_chk_call_next] = r;
+  g_chk_call_next = (g_chk_call_next + 1) % FTLM_CHK_CALL_RANGES;
+  // stream-ordered: kernels already enqueued keep the list they were launched under (pageable source: staged at once)
+  cudaMemcpyAsync((char*)g_chk_dev + offsetof(FtlmChkState, call), g_chk_call, sizeof(g_chk_call), cudaMemcpyHostToDevice, s);
+}
+
+// Self-test of the checker ("check_selftest"): five accesses that would fault in the release build - a global load and a
+// global store outside every live range, a misaligned global load, a shared load beyond the dynamic window, an
+// asynchronous copy from a bad source - must each be suppressed and counted.  Returns how many were counted (5)
+// and puts the counter back, so that a session's "violations == 0" criterion is not disturbed.
+__global__ void chk_selftest_kernel(const float* good, float* sink) {
+  FTLM_DYN_SMEM(smem);
+  float* sm = (float*)smem;
+  if (threadIdx.x == 0) {
+    float a = LD_G(good + (1ll << 40));                       // far outside
+    ST_G((float*)(uintptr_t)64, 1.0f);                         // unmapped low address
+    a += LD_G((const float*)((const char*)good + 2));         // misaligned
+    a += LD_S(sm + (1 << 20));                                 // beyond the dynamic shared-memory window
+    cp_async_elem(sm, (const float*)(uintptr_t)128);
+    cp_async_wait_all();
+    ST_G(sink, a + LD_G(good));                                // legitimate accesses: not counted
+  }
+}
+
+static int64_t chk_selftest() {
+  if (!ftlm_chk_state_dev()) return -1;
+  float* buf = nullptr;
+  if (ftlm_dmalloc(&buf, 64) != cudaSuccess) return -1;
+  cudaMemset(buf, 0, 64);
+  unsigned long long before = 0, after = 0;
+  cudaDeviceSynchronize();
+  cudaMemcpy(&before, g_chk_dev, 8, cudaMemcpyDeviceToHost);
+  FTLM_LAUNCH(chk_selftest_kernel, 1, 32, 64, 0, buf, buf + 8);
+  const cudaError_t e = cudaDeviceSynchronize();
+  cudaMemcpy(&after, g_chk_dev, 8, cudaMemcpyDeviceToHost);
+  FtlmChkState zero;
+  memset(&zero, 0, sizeof(zero));
+  if (before == 0) cudaMemcpy(g_chk_dev, &zero, offsetof(FtlmChkState, n_ranges), cudaMemcpyHostToDevice);   // forget the deliberate ones
+  else cudaMemcpy(g_chk_dev, &before, 8, cudaMemcpyHostToDevice);
+  ftlm_dfree(buf);
+  return e == cudaSuccess ? (int64_t)(after - before) : -2;
+}
+
+static int64_t chk_read(const char* key) {
+  if (!ftlm_chk_state_dev()) return -1;
+  if (!strcmp(key, "check_selftest")) return chk_selftest();
+  FtlmChkState h;
+  cudaDeviceSynchronize();
+  if (cudaMemcpy(&h, g_chk_dev, offsetof(FtlmChkState, call), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+  if (!strcmp(key, "check_violations")) return (int64_t)h.violations;
+  if (!strcmp(key, "check_first_tu")) return h.first_tu;
+  if (!strcmp(key, "check_first_line")) return h.first_line;
+  if (!strcmp(key, "check_first_kind")) return h.first_kind;
+  if (!strcmp(key, "check_first_block")) return h.first_block;
+  if (!strcmp(key, "check_first_thread")) return h.first_thread;
+  if (!strcmp(key, "check_first_addr")) return (int64_t)h.first_addr;
+  return -1;
+}
+#else
+cudaError_t ftlm_dmalloc_bytes(void** p, size_t bytes) { return cudaMalloc(p, bytes); }
+cudaError_t ftlm_dfree(void* p) { return cudaFree(p); }
+void ftlm_chk_caller(cudaStream_t, const void*, size_t) {}
+#endif
 
 size_t ftlm_elem_size(const ftlm_ctx* c) { return c->prec == FTLM_FP64 ? 8 : 4; }
 
@@ -46,11 +173,11 @@ __global__ void clt_build_kernel(uint2* __restrict__ clt, int64_t nblk, int N, i
     for (int p = N - 1; p >= 5; --p) {
       if ((base >> p) & 1ull) {
         const int need = K - above;
-        if (need >= 0 && need <= p) cnt += binom[p * K1 + need];
+        if (need >= 0 && need <= p) cnt += LDG(&binom[p * K1 + need]);
         ++above;
       }
     }
-    clt[b] = make_uint2(mask, (uint32_t)cnt);
+    ST_G(&clt[b], make_uint2(mask, (uint32_t)cnt));
   }
 }
 
@@ -85,7 +212,7 @@ gauss_norm_kernel(uint64_t key, int64_t dim, double* __restrict__ partials) {
     s += g * g;
   }
   block_sum3(s, z1, z2, sh);
-  if (threadIdx.x == 0) partials[blockIdx.x] = s;
+  if (threadIdx.x == 0) ST_G(&partials[blockIdx.x], s);
 }
 
 template <typename R>
@@ -95,17 +222,17 @@ sumsq_kernel(const R* __restrict__ v, int64_t dim, double* __restrict__ partials
   double s = 0.0, z1 = 0.0, z2 = 0.0;
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
        t += (int64_t)gridDim.x * blockDim.x) {
-    const double g = (double)v[t];
+    const double g = (double)LD_G(&v[t]);
     s += g * g;
   }
   block_sum3(s, z1, z2, sh);
-  if (threadIdx.x == 0) partials[blockIdx.x] = s;
+  if (threadIdx.x == 0) ST_G(&partials[blockIdx.x], s);
 }
 
 __global__ void reduce_partials_kernel(const double* __restrict__ partials, int n, double* out) {
   __shared__ double sh[96];
   double s = 0.0, z1 = 0.0, z2 = 0.0;
-  for (int k = threadIdx.x; k < n; k += blockDim.x) s += partials[k];
+  for (int k = threadIdx.x; k < n; k += blockDim.x) s += LD_G(&partials[k]);
   block_sum3(s, z1, z2, sh);
   if (threadIdx.x == 0) *out = s;
 }
@@ -116,7 +243,7 @@ gauss_write_kernel(uint64_t key, int64_t dim, const double* __restrict__ norm2, 
   const double nrm = sqrt(*norm2);
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
        t += (int64_t)gridDim.x * blockDim.x)
-    v[t] = (R)(gauss_elem(key, (uint64_t)t) / nrm);
+    ST_G(&v[t], (R)(gauss_elem(key, (uint64_t)t) / nrm));
 }
 
 template <typename R>
@@ -125,7 +252,7 @@ scale_copy_kernel(const R* __restrict__ src, int64_t dim, const double* __restri
   const double nrm = sqrt(*norm2);
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
        t += (int64_t)gridDim.x * blockDim.x)
-    dst[t] = (R)((double)src[t] / nrm);
+    ST_G(&dst[t], (R)((double)LD_G(&src[t]) / nrm));
 }
 
 // ---- Lanczos normalisation pass (A7): q_{j+1} = (y - alpha_j q_j) / beta_j ----------------------
@@ -142,16 +269,16 @@ lanczos_next_kernel(const R* __restrict__ y, const R* __restrict__ q, R* __restr
   V4* o4 = (V4*)qnext;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvec; k += stride) {
-    V4 yy = __ldcs(&y4[k]);
-    V4 qq = q4[k];
+    V4 yy = LDCS(&y4[k]);
+    V4 qq = LD_G(&q4[k]);
     R* yp = (R*)&yy;
     const R* qp = (const R*)&qq;
 #pragma unroll
     for (int e = 0; e < W; ++e) yp[e] = (yp[e] - a * qp[e]) * ib;
-    o4[k] = yy;
+    ST_G(&o4[k], yy);
   }
   for (int64_t t = nvec * W + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim; t += stride)
-    qnext[t] = (y[t] - a * q[t]) * ib;
+    ST_G(&qnext[t], (LD_G(&y[t]) - a * LD_G(&q[t])) * ib);
 }
 
 __global__ void chain_reset_kernel(ChainState* st, int limit, double tol) {
@@ -229,29 +356,27 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
   int rc = FTLM_OK;
   auto fail = [&](int code) { ftlm_destroy(c); return code; };
 #define CKF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { rc = ftlm_cuda_fail(e__, #call); return fail(e__ == cudaErrorMemoryAllocation ? FTLM_ENOMEM : rc); } } while (0)
-  CKF(cudaMalloc(&c->d_binom64, c->binom64.size() * 8));
-  CKF(cudaMalloc(&c->d_binom32, b32.size() * 4));
+  CKF(ftlm_dmalloc(&c->d_binom64, c->binom64.size() * 8));
+  CKF(ftlm_dmalloc(&c->d_binom32, b32.size() * 4));
   CKF(cudaMemcpy(c->d_binom64, c->binom64.data(), c->binom64.size() * 8, cudaMemcpyHostToDevice));
   CKF(cudaMemcpy(c->d_binom32, b32.data(), b32.size() * 4, cudaMemcpyHostToDevice));
-  CKF(cudaMalloc(&c->d_bonds, sizeof(BondDev) * (size_t)(n_bonds > 0 ? n_bonds : 1)));
+  CKF(ftlm_dmalloc(&c->d_bonds, sizeof(BondDev) * (size_t)(n_bonds > 0 ? n_bonds : 1)));
   if (n_bonds > 0) CKF(cudaMemcpy(c->d_bonds, c->bonds.data(), sizeof(BondDev) * n_bonds, cudaMemcpyHostToDevice));
   c->max_blocks = c->sm_count * 32;
-  CKF(cudaMalloc(&c->d_state, sizeof(ChainState)));
+  CKF(ftlm_dmalloc(&c->d_state, sizeof(ChainState)));
   CKF(cudaMemset(c->d_state, 0, sizeof(ChainState)));
-  CKF(cudaMalloc(&c->d_partials, sizeof(double) * 3 * (size_t)c->max_blocks));
-  CKF(cudaMalloc(&c->d_ticket, sizeof(unsigned int)));
+  CKF(ftlm_dmalloc(&c->d_partials, sizeof(double) * 3 * (size_t)c->max_blocks));
+  CKF(ftlm_dmalloc(&c->d_ticket, sizeof(unsigned int)));
   CKF(cudaMemset(c->d_ticket, 0, sizeof(unsigned int)));
   if (index_mode == FTLM_INDEX_CLT) {
     c->n_clt = (int64_t)(((1ull << N) + 31ull) / 32ull);
-    CKF(cudaMalloc(&c->d_clt, sizeof(uint2) * (size_t)c->n_clt));
+    CKF(ftlm_dmalloc(&c->d_clt, sizeof(uint2) * (size_t)c->n_clt));
     int grid = (int)((c->n_clt + 255) / 256);
     if (grid > c->sm_count * 16) grid = c->sm_count * 16;
     FTLM_LAUNCH(clt_build_kernel, grid, 256, 0, 0, c->d_clt, c->n_clt, N, N_up, c->d_binom64);
     CKF(cudaGetLastError());
   }
   for (int k = 0; k < 4; ++k) CKF(cudaEventCreate(&c->ev[k]));
-  rc = ftlm_tile_plan_create(c);
-  if (rc != FTLM_OK) return fail(rc);
   rc = ftlm_tml_plan_create(c);
   if (rc != FTLM_OK) return fail(rc);
   CKF(cudaDeviceSynchronize());
@@ -263,11 +388,10 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
 extern "C" int ftlm_destroy(ftlm_ctx* c) {
   if (!c) return FTLM_OK;
   cudaSetDevice(c->device);
-  ftlm_tile_plan_destroy(c);
   ftlm_tml_plan_destroy(c);
-  cudaFree(c->d_binom64); cudaFree(c->d_binom32); cudaFree(c->d_bonds); cudaFree(c->d_clt);
-  cudaFree(c->d_state); cudaFree(c->d_partials); cudaFree(c->d_ticket);
-  for (int k = 0; k < 3; ++k) cudaFree(c->q[k]);
+  ftlm_dfree(c->d_binom64); ftlm_dfree(c->d_binom32); ftlm_dfree(c->d_bonds); ftlm_dfree(c->d_clt);
+  ftlm_dfree(c->d_state); ftlm_dfree(c->d_partials); ftlm_dfree(c->d_ticket);
+  for (int k = 0; k < 3; ++k) ftlm_dfree(c->q[k]);
   for (int k = 0; k < 4; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
   delete c;
   return FTLM_OK;
@@ -286,26 +410,15 @@ int ftlm_effective_kernel(const ftlm_ctx* c) {
   if (c->kernel == FTLM_KERNEL_ROW) return FTLM_KERNEL_ROW;
   if (c->kernel == FTLM_KERNEL_TML && c->tml) return FTLM_KERNEL_TML;
   if (c->kernel == FTLM_KERNEL_AUTO && c->tml && c->dim >= (1 << 20)) return FTLM_KERNEL_TML;
-  if (c->tile && (c->kernel == FTLM_KERNEL_TILE || c->dim >= (1 << 20))) return FTLM_KERNEL_TILE;
   return FTLM_KERNEL_ROW;                    // AUTO: small sectors are launch-bound, ROW is simpler
 }
 
 extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   if (!c || !key) { ftlm_set_error("ftlm_set_option: NULL"); return FTLM_EINVAL; }
   if (!strcmp(key, "kernel")) {
-    if (value < 0 || value > 3) { ftlm_set_error("kernel must be 0..3"); return FTLM_EINVAL; }
-    if (value == FTLM_KERNEL_TILE && !c->tile) { ftlm_set_error("TILE kernel unavailable for this sector"); return FTLM_EUNSUPPORTED; }
+    if (value != FTLM_KERNEL_AUTO && value != FTLM_KERNEL_ROW && value != FTLM_KERNEL_TML) { ftlm_set_error("kernel must be FTLM_KERNEL_AUTO, _ROW or _TML"); return FTLM_EINVAL; }
     if (value == FTLM_KERNEL_TML && !c->tml) { ftlm_set_error("TML kernel unavailable for this sector"); return FTLM_EUNSUPPORTED; }
     c->kernel = (int)value; return FTLM_OK;
-  }
-  if (!strcmp(key, "low_bits")) {
-    if (value < 0 || value > 20) { ftlm_set_error("low_bits must be 0..20"); return FTLM_EINVAL; }
-    const int old = c->low_bits;
-    c->low_bits = (int)value;
-    ftlm_tile_plan_destroy(c);
-    int rc = ftlm_tile_plan_create(c);
-    if (rc != FTLM_OK) { c->low_bits = old; ftlm_tile_plan_destroy(c); ftlm_tile_plan_create(c); }
-    return rc;
   }
   if (!strcmp(key, "tml_low_bits") || !strcmp(key, "tml_mid_bits")) {
     if (value < 0 || value > 16) { ftlm_set_error("%s must be 0..16", key); return FTLM_EINVAL; }
@@ -319,6 +432,7 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     return rc;
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
+  if (!strcmp(key, "allow_unverified")) { c->allow_unverified = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "tmlr")) { c->use_tmlr = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "lazy_norm")) { c->lazy_norm = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "tmlr_unij")) {
@@ -364,14 +478,23 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
 }
 
 extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
-  if (!c || !key) return -1;
+  if (!key) return -1;
+  if (!strncmp(key, "check_", 6)) {                      // checked build (ftlm_access.cuh): process-wide, ctx may be NULL
+#if defined(FTLM_CHECKED) && !defined(FTLM_EMU)
+    if (!strcmp(key, "check_build")) return 1;
+    return chk_read(key);
+#else
+    return !strcmp(key, "check_build") ? 0 : -1;
+#endif
+  }
+  if (!c) return -1;
   if (!strcmp(key, "kernel")) return ftlm_effective_kernel(c);
-  if (!strcmp(key, "low_bits")) return c->low_bits;
   if (!strcmp(key, "graph")) return c->use_graph;
   if (!strcmp(key, "passb")) return c->use_passb;
   if (!strncmp(key, "passb_", 6)) return ftlm_passb_info(c, key);
   if (!strcmp(key, "sm_count")) return c->sm_count;
   if (!strcmp(key, "autotuned")) return c->autotuned;
+  if (!strcmp(key, "allow_unverified")) return c->allow_unverified;
   if (!strcmp(key, "tmlr")) return c->use_tmlr;
   if (!strcmp(key, "lazy_norm")) return c->lazy_norm;
   if (!strcmp(key, "lazy_norm_ok")) return ftlm_tmlr_lazy_ok(c) ? 1 : 0;
@@ -405,13 +528,14 @@ static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fu
     if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, s);
     return rc;
   }
-  if (k == FTLM_KERNEL_TILE) return ftlm_launch_hv_tile(c, v, qp, y, fused, s);
   return ftlm_launch_hv_row(c, v, qp, y, fused, s);
 }
 
 extern "C" int ftlm_apply_H(ftlm_ctx* c, const void* d_v, void* d_y, void* stream) {
   if (!c || !d_v || !d_y || d_v == d_y) { ftlm_set_error("ftlm_apply_H: bad argument (NULL or d_y == d_v)"); return FTLM_EINVAL; }
   CK(cudaSetDevice(c->device));
+  ftlm_chk_caller((cudaStream_t)stream, d_v, (size_t)c->dim * ftlm_elem_size(c));
+  ftlm_chk_caller((cudaStream_t)stream, d_y, (size_t)c->dim * ftlm_elem_size(c));
   return launch_hv(c, d_v, nullptr, d_y, 0, (cudaStream_t)stream);
 }
 
@@ -420,14 +544,14 @@ extern "C" int ftlm_apply_H_host(ftlm_ctx* c, const void* h_v, void* h_y) {
   CK(cudaSetDevice(c->device));
   const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
   void *dv = nullptr, *dy = nullptr;
-  if (cudaMalloc(&dv, bytes) != cudaSuccess || cudaMalloc(&dy, bytes) != cudaSuccess) {
-    cudaFree(dv); ftlm_set_error("ftlm_apply_H_host: out of device memory"); return FTLM_ENOMEM;
+  if (ftlm_dmalloc(&dv, bytes) != cudaSuccess || ftlm_dmalloc(&dy, bytes) != cudaSuccess) {
+    ftlm_dfree(dv); ftlm_set_error("ftlm_apply_H_host: out of device memory"); return FTLM_ENOMEM;
   }
   int rc = FTLM_OK;
   cudaError_t e = cudaMemcpy(dv, h_v, bytes, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) rc = launch_hv(c, dv, nullptr, dy, 0, 0);
   if (e == cudaSuccess && rc == FTLM_OK) e = cudaMemcpy(h_y, dy, bytes, cudaMemcpyDeviceToHost);
-  cudaFree(dv); cudaFree(dy);
+  ftlm_dfree(dv); ftlm_dfree(dy);
   if (e != cudaSuccess) return ftlm_cuda_fail(e, "ftlm_apply_H_host");
   return rc;
 }
@@ -438,8 +562,8 @@ extern "C" int ftlm_neighbors(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
   }
   if (nrows == 0 || c->nb == 0) return FTLM_OK;
   CK(cudaSetDevice(c->device));
+  ftlm_chk_caller((cudaStream_t)stream, d_idx, (size_t)nrows * (size_t)c->nb * 8);
   if (ftlm_effective_kernel(c) == FTLM_KERNEL_TML) return ftlm_launch_neighbors_tml(c, row0, nrows, d_idx, (cudaStream_t)stream);
-  if (ftlm_effective_kernel(c) == FTLM_KERNEL_TILE) return ftlm_launch_neighbors_tile(c, row0, nrows, d_idx, (cudaStream_t)stream);
   return ftlm_launch_neighbors_row(c, row0, nrows, d_idx, (cudaStream_t)stream);
 }
 
@@ -463,6 +587,7 @@ extern "C" int ftlm_fill_random(ftlm_ctx* c, uint64_t seed, int r, void* d_v, vo
   if (!c || !d_v || r < 0) { ftlm_set_error("ftlm_fill_random: bad argument"); return FTLM_EINVAL; }
   CK(cudaSetDevice(c->device));
   cudaStream_t s = (cudaStream_t)stream;
+  ftlm_chk_caller(s, d_v, (size_t)c->dim * ftlm_elem_size(c));
   const uint64_t key = chain_key(seed, c->N_up, r);
   const int grid = stream_grid(c, c->dim, 8);
   FTLM_LAUNCH(gauss_norm_kernel, grid, 256, 0, s, key, c->dim, c->d_partials);
@@ -478,7 +603,7 @@ static int ensure_workspace(ftlm_ctx* c) {
   const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
   for (int k = 0; k < 3; ++k)
     if (!c->q[k]) {
-      cudaError_t e = cudaMalloc(&c->q[k], bytes);
+      cudaError_t e = ftlm_dmalloc(&c->q[k], bytes);
       if (e != cudaSuccess) { ftlm_set_error("chain workspace: cannot allocate 3 x %zu bytes (%s)", bytes, cudaGetErrorString(e)); cudaGetLastError(); return FTLM_ENOMEM; }
     }
   return FTLM_OK;
@@ -515,6 +640,7 @@ static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64
 
 extern "C" int ftlm_chain_begin(ftlm_ctx* c, const void* d_q1, uint64_t seed, int r, void* stream) {
   if (!c || r < 0) { ftlm_set_error("ftlm_chain_begin: bad argument"); return FTLM_EINVAL; }
+  if (d_q1) ftlm_chk_caller((cudaStream_t)stream, d_q1, (size_t)c->dim * ftlm_elem_size(c));
   return chain_begin_impl(c, d_q1, false, seed, r, (cudaStream_t)stream);
 }
 

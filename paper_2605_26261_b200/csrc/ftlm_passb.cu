@@ -18,6 +18,7 @@
 #include <cstring>
 #include <vector>
 
+#define FTLM_TU 5
 #include "ftlm_passb.cuh"
 
 #define PASSB_MAX_BONDS 31          // one neighbour entry per lane; entry 31 holds the count and the sum of J
@@ -106,8 +107,8 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* t
   uint32_t eo_n = 0;
   R eJ_n = (R)0;
   if (warp < nconf) {
-    eo_n = __ldg(&p.nbr_off[(size_t)(c0 + warp) * 32 + lane]);
-    eJ_n = __ldg(&p.nbr_J[(size_t)(c0 + warp) * 32 + lane]);
+    eo_n = LDG(&p.nbr_off[(size_t)(c0 + warp) * 32 + lane]);
+    eJ_n = LDG(&p.nbr_J[(size_t)(c0 + warp) * 32 + lane]);
   }
   for (int sl0 = warp; sl0 < nconf; sl0 += NW * PASSB_PF) {
     R yold[PASSB_PF][PASSB_XK];
@@ -117,7 +118,7 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* t
 #pragma unroll
       for (int k = 0; k < PASSB_XK; ++k) {
         const int x = lane + 32 * k;
-        yold[j][k] = (sl < nconf && k < XKC && x < nx) ? __ldcs(y + s_start[sl] + x0 + x) : (R)0;
+        yold[j][k] = (sl < nconf && k < XKC && x < nx) ? LDCS(y + LD_S(&s_start[sl]) + x0 + x) : (R)0;
       }
     }
 #pragma unroll
@@ -127,40 +128,40 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* t
       const uint32_t eo = eo_n;
       const R eJ = eJ_n;
       if (sl + NW < nconf) {
-        eo_n = __ldg(&p.nbr_off[(size_t)(c0 + sl + NW) * 32 + lane]);
-        eJ_n = __ldg(&p.nbr_J[(size_t)(c0 + sl + NW) * 32 + lane]);
+        eo_n = LDG(&p.nbr_off[(size_t)(c0 + sl + NW) * 32 + lane]);
+        eJ_n = LDG(&p.nbr_J[(size_t)(c0 + sl + NW) * 32 + lane]);
       }
       const int cnt = (int)__shfl_sync(0xffffffffu, eo, 31);
       const R sumJ = __shfl_sync(0xffffffffu, eJ, 31);
       // lanes past the end of the run (x >= nx) read stale tile words and are discarded at the store
       const unsigned char* tl = (const unsigned char*)tile + (size_t)lane * sizeof(R);
-      R* yrow = y + s_start[sl] + x0;
+      R* yrow = y + LD_S(&s_start[sl]) + x0;
       R own[PASSB_XK], acc[PASSB_XK];
-      own[0] = *(const R*)(tl + (size_t)sl * X * sizeof(R));
+      own[0] = LD_S((const R*)(tl + (size_t)sl * X * sizeof(R)));
       acc[0] = (R)0;
       if (XKC == 1) {
         own[1] = (R)0; acc[1] = (R)0;
         if (UNIJ) {                                  // one J_b for the whole window: add, multiply once
 #pragma unroll 4
-          for (int e = 0; e < cnt; ++e) acc[0] += *(const R*)(tl + __shfl_sync(0xffffffffu, eo, e));
+          for (int e = 0; e < cnt; ++e) acc[0] += LD_S((const R*)(tl + __shfl_sync(0xffffffffu, eo, e)));
           acc[0] *= p.Juni;
         } else {
 #pragma unroll 4
           for (int e = 0; e < cnt; ++e) {
             const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
             const R J = __shfl_sync(0xffffffffu, eJ, e);
-            acc[0] += J * *(const R*)(tl + off);
+            acc[0] += J * LD_S((const R*)(tl + off));
           }
         }
       } else {
-        own[1] = *(const R*)(tl + (size_t)sl * X * sizeof(R) + 32 * sizeof(R));
+        own[1] = LD_S((const R*)(tl + (size_t)sl * X * sizeof(R) + 32 * sizeof(R)));
         acc[1] = (R)0;
         if (UNIJ) {
 #pragma unroll 4
           for (int e = 0; e < cnt; ++e) {
             const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
-            acc[0] += *(const R*)(tl + off);
-            acc[1] += *(const R*)(tl + off + 32 * sizeof(R));
+            acc[0] += LD_S((const R*)(tl + off));
+            acc[1] += LD_S((const R*)(tl + off + 32 * sizeof(R)));
           }
           acc[0] *= p.Juni; acc[1] *= p.Juni;
         } else {
@@ -168,8 +169,8 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* t
           for (int e = 0; e < cnt; ++e) {
             const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
             const R J = __shfl_sync(0xffffffffu, eJ, e);
-            acc[0] += J * *(const R*)(tl + off);
-            acc[1] += J * *(const R*)(tl + off + 32 * sizeof(R));
+            acc[0] += J * LD_S((const R*)(tl + off));
+            acc[1] += J * LD_S((const R*)(tl + off + 32 * sizeof(R)));
           }
         }
       }
@@ -178,7 +179,7 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* t
         const int x = lane + 32 * k;
         if (k < XKC && x < nx) {
           const R yn = yold[j][k] + (acc[k] - sumJ * own[k]);
-          __stcs(&yrow[x], yn);
+          STCS(&yrow[x], yn);
           if (FUSED) {
             s_qy += (double)own[k] * (double)yn;
             s_yy += (double)yn * (double)yn;
@@ -206,7 +207,7 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
   double* s_red = (double*)(smem + o);
   o += (size_t)32 * 3 * 8;
   R* tile = (R*)(smem + o);
-  for (int k = tid; k < (p.N + 1) * K1; k += NT) s_binom[k] = p.binom[k];
+  for (int k = tid; k < (p.N + 1) * K1; k += NT) ST_S(&s_binom[k], LD_G(&p.binom[k]));
   int cur_group = -1;
   const int s1 = p.s + 1;
 
@@ -217,20 +218,20 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     __syncthreads();                                   // everyone has read it
     if (item >= p.item_end) break;
     if (tid == 0) s_item = atomicAdd(&p.counter[0], 1u);   // the following item's id travels while this item is processed
-    const int g = (int)__ldg(&p.item_group[item]);      // group g = F * (s+1) + p_S of this item
+    const int g = (int)LDG(&p.item_group[item]);      // group g = F * (s+1) + p_S of this item
     const uint32_t F = (uint32_t)(g / s1);
     const int pS = g - (int)F * s1;
     const int kP = p.K - __popc(F) - pS;                // in [0, lo] by construction of the groups
-    const int c0 = __ldg(&p.koff[pS]);
-    const int nconf = __ldg(&p.koff[pS + 1]) - c0;
+    const int c0 = LDG(&p.koff[pS]);
+    const int nconf = LDG(&p.koff[pS + 1]) - c0;
     const int XK = p.xk[pS];
     const int X = 32 * XK;
-    const uint64_t RL = s_binom[p.lo * K1 + kP];        // run length C(lo, kP)
-    const uint64_t x0 = (uint64_t)(item - __ldg(&p.grp_first[g])) * (uint64_t)X;
+    const uint64_t RL = LD_S(&s_binom[p.lo * K1 + kP]);        // run length C(lo, kP)
+    const uint64_t x0 = (uint64_t)(item - LDG(&p.grp_first[g])) * (uint64_t)X;
     if (g != cur_group) {                               // (uniform) run starts of this class
       for (int sl = tid; sl < nconf; sl += NT) {
-        const uint64_t hi = bits_deposit((uint64_t)F, p.fmask_hi) | bits_deposit((uint64_t)__ldg(&p.ustate[c0 + sl]), p.smask_hi);
-        s_start[sl] = passb_run_start<MODE>(hi, p.lo, kP, p.K, s_binom, p.clt);
+        const uint64_t hi = bits_deposit((uint64_t)F, p.fmask_hi) | bits_deposit((uint64_t)LDG(&p.ustate[c0 + sl]), p.smask_hi);
+        ST_S(&s_start[sl], passb_run_start<MODE>(hi, p.lo, kP, p.K, s_binom, p.clt));
       }
       cur_group = g;
       __syncthreads();
@@ -239,7 +240,7 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     const int nx = left < (uint64_t)X ? (int)left : X;  // valid offsets in this chunk
     // ---- phase 1: stage the run chunks (cp.async: every copy of the item is in flight at once) ------
     for (int sl = warp; sl < nconf; sl += NW) {
-      const R* src = v + s_start[sl] + x0;
+      const R* src = v + LD_S(&s_start[sl]) + x0;
       R* dst = tile + (size_t)sl * X;
 #pragma unroll
       for (int k = 0; k < PASSB_XK; ++k) {
@@ -260,12 +261,12 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     }
     if (FUSED) {                                        // deterministic per-item partial sums
       const double a = warp_sum(s_qy), b = warp_sum(s_yy), c = warp_sum(s_qq);
-      if (lane == 0) { s_red[warp * 3] = a; s_red[warp * 3 + 1] = b; s_red[warp * 3 + 2] = c; }
+      if (lane == 0) { ST_S(&s_red[warp * 3], a); ST_S(&s_red[warp * 3 + 1], b); ST_S(&s_red[warp * 3 + 2], c); }
       __syncthreads();
       if (tid < 3) {
         double s = 0.0;
-        for (int wv = 0; wv < NW; ++wv) s += s_red[wv * 3 + tid];
-        p.partials[(size_t)tid * p.nitems + item] = s;
+        for (int wv = 0; wv < NW; ++wv) s += LD_S(&s_red[wv * 3 + tid]);
+        ST_G(&p.partials[(size_t)tid * p.nitems + item], s);
       }
     }
   }
@@ -283,13 +284,13 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
   double tot[3];
   for (int q = 0; q < 3; ++q) {                         // fixed assignment and order
     double a = 0.0;
-    for (uint32_t k = tid; k < p.nitems; k += NT) a += p.partials[(size_t)q * p.nitems + k];
+    for (uint32_t k = tid; k < p.nitems; k += NT) a += LD_G(&p.partials[(size_t)q * p.nitems + k]);
     a = warp_sum(a);
     __syncthreads();
-    if (lane == 0) s_red[warp] = a;
+    if (lane == 0) ST_S(&s_red[warp], a);
     __syncthreads();
     double s = 0.0;
-    if (tid == 0) for (int wv = 0; wv < NW; ++wv) s += s_red[wv];
+    if (tid == 0) for (int wv = 0; wv < NW; ++wv) s += LD_S(&s_red[wv]);
     tot[q] = s;
   }
   if (tid == 0) {
@@ -339,8 +340,8 @@ void ftlm_passb_plan_destroy(ftlm_ctx* c) {
   PassBSet* S = c->passb;
   if (!S) return;
   for (PassBWindow& w : S->win) {
-    cudaFree(w.d_ustate); cudaFree(w.d_koff); cudaFree(w.d_nbr); cudaFree(w.d_nbrJ); cudaFree(w.d_grp_first); cudaFree(w.d_item_group);
-    cudaFree(w.d_partials); cudaFree(w.d_counter);
+    ftlm_dfree(w.d_ustate); ftlm_dfree(w.d_koff); ftlm_dfree(w.d_nbr); ftlm_dfree(w.d_nbrJ); ftlm_dfree(w.d_grp_first); ftlm_dfree(w.d_item_group);
+    ftlm_dfree(w.d_partials); ftlm_dfree(w.d_counter);
   }
   delete S;
   c->passb = nullptr;
@@ -559,7 +560,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
     std::vector<float> nbrJf;
     if (esz == 4) { nbrJf.resize(nbrJ.size()); for (size_t k = 0; k < nbrJ.size(); ++k) nbrJf[k] = (float)nbrJ[k]; }
     auto up = [&](void** d, const void* h, size_t bytes) -> bool {
-      if (cudaMalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
+      if (ftlm_dmalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
       if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
       return true;
     };

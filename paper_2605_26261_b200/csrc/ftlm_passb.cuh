@@ -20,7 +20,7 @@ __device__ __forceinline__ uint64_t passb_run_start(uint64_t hi, int lo, int kP,
                                                     const uint2* __restrict__ clt) {
   if (MODE == FTLM_INDEX_CLT) {
     const uint64_t n0 = (hi << lo) | ((1ull << kP) - 1ull);
-    const uint2 e = __ldg(&clt[n0 >> 5]);
+    const uint2 e = LDG(&clt[n0 >> 5]);
     const uint32_t j = (uint32_t)n0 & 31u;
     return (uint64_t)e.y + (uint64_t)__popc(e.x & ((1u << j) - 1u));
   }
@@ -31,7 +31,7 @@ __device__ __forceinline__ uint64_t passb_run_start(uint64_t hi, int lo, int kP,
     const int p = __ffsll((long long)x) - 1;
     x &= x - 1;
     ++c;
-    r += binom[(p + lo) * K1 + c];
+    r += LD_A(&binom[(p + lo) * K1 + c]);
   }
   return r;
 }
@@ -45,7 +45,7 @@ __device__ __forceinline__ uint64_t passb_low_rank(uint64_t low, int K, const ui
     const int q = __ffsll((long long)low) - 1;
     low &= low - 1;
     ++c;
-    r += binom[q * K1 + c];
+    r += LD_A(&binom[q * K1 + c]);
   }
   return r;
 }

@@ -2,6 +2,7 @@
 // paper's launch shape ("assigning one GPU thread to each
 // sector-basis state") written for sm_100a; it is the plain in-library baseline and the path
 // used for index-map queries.  The B200 design proper is in ftlm_tile.cu.
+#define FTLM_TU 2
 #include "ftlm_common.cuh"
 
 namespace {
@@ -13,7 +14,7 @@ __device__ __forceinline__ L unrank(I r, int N, int K1, int K, const I* __restri
   L n = 0;
   int A = K;
   for (int p = N - 1; p >= 0 && A > 0; --p) {
-    const I c = binom[p * K1 + A];
+    const I c = LD_S(&binom[p * K1 + A]);
     if (r >= c) { n |= (L)1 << p; r -= c; --A; }
   }
   return n;
@@ -25,7 +26,7 @@ __device__ __forceinline__ I rank_alg1(L x, int N, int K1, int K, const I* __res
   I rank = 0;
   int A = K;
   for (int p = N - 1; p >= 0; --p) {
-    if ((x >> p) & 1) { rank += binom[p * K1 + A]; --A; }
+    if ((x >> p) & 1) { rank += LD_S(&binom[p * K1 + A]); --A; }
   }
   return rank;
 }
@@ -40,20 +41,20 @@ __device__ __forceinline__ I cr_delta(L x, int i, int j, int K1, const I* __rest
   I d;
   int c = ci;
   if ((x >> j) & 1) {                                          // the one moves down j -> i
-    d = binom[i * K1 + ci + 1] - binom[j * K1 + cj];
+    d = LD_S(&binom[i * K1 + ci + 1]) - LD_S(&binom[j * K1 + cj]);
     while (between) {
       const int p = ffs_(between) - 1;
       between &= between - 1;
       ++c;
-      d += binom[p * K1 + c + 1] - binom[p * K1 + c];
+      d += LD_S(&binom[p * K1 + c + 1]) - LD_S(&binom[p * K1 + c]);
     }
   } else {                                                     // the one moves up i -> j
-    d = binom[j * K1 + cj] - binom[i * K1 + ci];
+    d = LD_S(&binom[j * K1 + cj]) - LD_S(&binom[i * K1 + ci]);
     while (between) {
       const int p = ffs_(between) - 1;
       between &= between - 1;
       ++c;
-      d += binom[p * K1 + c - 1] - binom[p * K1 + c];
+      d += LD_S(&binom[p * K1 + c - 1]) - LD_S(&binom[p * K1 + c]);
     }
   }
   return d;
@@ -62,13 +63,13 @@ __device__ __forceinline__ I cr_delta(L x, int i, int j, int K1, const I* __rest
 // Algorithm 2 (L167-L173): b = n >> 5, j = n & 31, index = C_b + popc(M_b & (2^j - 1)).
 __device__ __forceinline__ int64_t clt_lookup_checked(uint64_t n, int N, const uint2* __restrict__ clt) {
   if (N < 64 && (n >> N)) return -1;
-  const uint2 e = clt[n >> 5];
+  const uint2 e = LD_G(&clt[n >> 5]);
   const uint32_t j = (uint32_t)n & 31u;
   if (!((e.x >> j) & 1u)) return -1;
   return (int64_t)e.y + __popc(e.x & ((1u << j) - 1u));
 }
 __device__ __forceinline__ uint32_t clt_lookup(uint32_t n, const uint2* __restrict__ clt) {
-  const uint2 e = __ldg(&clt[n >> 5]);
+  const uint2 e = LDG(&clt[n >> 5]);
   return e.y + __popc(e.x & ((1u << (n & 31u)) - 1u));
 }
 
@@ -92,11 +93,12 @@ template <typename R, typename L, typename I>
 __device__ __forceinline__ void load_tables(const RowParams& p, I* s_binom, BondS<R>* s_bonds) {
   const int nbin = (p.N + 1) * (p.K + 1);
   const I* g = (const I*)p.binom;
-  for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = g[k];
+  for (int k = threadIdx.x; k < nbin; k += blockDim.x) ST_S(&s_binom[k], LD_G(&g[k]));
   for (int k = threadIdx.x; k < p.nb; k += blockDim.x) {
-    BondDev b = p.bonds[k];
-    s_bonds[k].mask = b.mask; s_bonds[k].Jh = (R)b.Jh; s_bonds[k].Jq = (R)b.Jq;
-    s_bonds[k].i = b.i; s_bonds[k].j = b.j;
+    const BondDev b = LD_G(&p.bonds[k]);
+    BondS<R> sb;
+    sb.mask = b.mask; sb.Jh = (R)b.Jh; sb.Jq = (R)b.Jq; sb.i = b.i; sb.j = b.j;
+    ST_S(&s_bonds[k], sb);
   }
   __syncthreads();
 }
@@ -125,19 +127,19 @@ hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev,
         I idx;
         if (MODE == FTLM_INDEX_CLT) idx = (I)clt_lookup((uint32_t)(n ^ m), p.clt);
         else idx = (I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom);
-        acc += s_bonds[b].Jh * __ldg(&v[idx]);
+        acc += s_bonds[b].Jh * LDG(&v[idx]);
         danti += s_bonds[b].Jq;
       }
     }
-    const R vt = v[t];
+    const R vt = LD_G(&v[t]);
     R out = ((R)p.diag0 - 2 * danti) * vt + acc;
     if (FUSED) {
-      out -= bprev * qprev[t];
+      out -= bprev * LD_G(&qprev[t]);
       s_qy += (double)vt * (double)out;
       s_yy += (double)out * (double)out;
       s_qq += (double)vt * (double)vt;
     }
-    y[t] = out;
+    ST_G(&y[t], out);
   }
   if (FUSED) lanczos_finish(s_qy, s_yy, s_qq, p.partials, p.stride, p.ticket, p.st, sh_red);
 }
@@ -163,7 +165,7 @@ neighbors_row_kernel(RowParams p, int64_t row0, int64_t nrows, int64_t* __restri
         if (MODE == FTLM_INDEX_CLT) idx = (int64_t)clt_lookup((uint32_t)(n ^ m), p.clt);
         else idx = (int64_t)(I)((I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom));
       }
-      out[r * p.nb + b] = idx;
+      ST_G(&out[r * p.nb + b], idx);
     }
   }
 }
@@ -174,11 +176,11 @@ __global__ void index_of_kernel(RowParams p, const uint64_t* __restrict__ labels
   FTLM_DYN_SMEM(smem);
   I* s_binom = (I*)smem;
   const int nbin = (p.N + 1) * (p.K + 1);
-  for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = ((const I*)p.binom)[k];
+  for (int k = threadIdx.x; k < nbin; k += blockDim.x) ST_S(&s_binom[k], LD_G(&((const I*)p.binom)[k]));
   __syncthreads();
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
-    const uint64_t lab = labels[k];
+    const uint64_t lab = LD_G(&labels[k]);
     int64_t idx;
     if (p.mode == FTLM_INDEX_CLT) {
       idx = clt_lookup_checked(lab, p.N, p.clt);
@@ -186,7 +188,7 @@ __global__ void index_of_kernel(RowParams p, const uint64_t* __restrict__ labels
       const bool in = (p.N >= 64 || (lab >> p.N) == 0) && __popcll(lab) == p.K;
       idx = in ? (int64_t)rank_alg1<L, I>((L)lab, p.N, p.K + 1, p.K, s_binom) : -1;
     }
-    out[k] = idx;
+    ST_G(&out[k], idx);
   }
 }
 
@@ -196,12 +198,12 @@ __global__ void state_of_kernel(RowParams p, const int64_t* __restrict__ idx, in
   FTLM_DYN_SMEM(smem);
   I* s_binom = (I*)smem;
   const int nbin = (p.N + 1) * (p.K + 1);
-  for (int k = threadIdx.x; k < nbin; k += blockDim.x) s_binom[k] = ((const I*)p.binom)[k];
+  for (int k = threadIdx.x; k < nbin; k += blockDim.x) ST_S(&s_binom[k], LD_G(&((const I*)p.binom)[k]));
   __syncthreads();
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
-    const int64_t t = idx[k];
-    out[k] = (t < 0 || t >= p.dim) ? ~0ull : (uint64_t)unrank<L, I>((I)t, p.N, p.K + 1, p.K, s_binom);
+    const int64_t t = LD_G(&idx[k]);
+    ST_G(&out[k], (t < 0 || t >= p.dim) ? ~0ull : (uint64_t)unrank<L, I>((I)t, p.N, p.K + 1, p.K, s_binom));
   }
 }
 
@@ -294,6 +296,7 @@ extern "C" int ftlm_index_of(ftlm_ctx* c, const uint64_t* d_labels, int64_t n, i
   const size_t sm = table_smem(c, 0);
   const int grid = grid_for(c, n, 8);
   cudaStream_t s = (cudaStream_t)stream;
+  ftlm_chk_caller(s, d_labels, (size_t)n * 8); ftlm_chk_caller(s, d_idx, (size_t)n * 8);
   if (!c->lab64) { auto k__ = index_of_kernel<uint32_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_labels, n, d_idx); }
   else if (!c->idx64) { auto k__ = index_of_kernel<uint64_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_labels, n, d_idx); }
   else { auto k__ = index_of_kernel<uint64_t, uint64_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_labels, n, d_idx); }
@@ -309,6 +312,7 @@ extern "C" int ftlm_state_of(ftlm_ctx* c, const int64_t* d_idx, int64_t n, uint6
   const size_t sm = table_smem(c, 0);
   const int grid = grid_for(c, n, 8);
   cudaStream_t s = (cudaStream_t)stream;
+  ftlm_chk_caller(s, d_labels, (size_t)n * 8); ftlm_chk_caller(s, d_idx, (size_t)n * 8);
   if (!c->lab64) { auto k__ = state_of_kernel<uint32_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_idx, n, d_labels); }
   else if (!c->idx64) { auto k__ = state_of_kernel<uint64_t, uint32_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_idx, n, d_labels); }
   else { auto k__ = state_of_kernel<uint64_t, uint64_t>; FTLM_LAUNCH(k__, grid, 256, sm, s, p, d_idx, n, d_labels); }

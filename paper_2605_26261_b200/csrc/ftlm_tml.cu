@@ -34,6 +34,7 @@
 #include <type_traits>
 #include <vector>
 
+#define FTLM_TU 3
 #include "ftlm_passb.cuh"
 
 #define TML_MAX_LL 32
@@ -97,8 +98,9 @@ namespace {
 template <typename R, int B>
 struct __align__((sizeof(R) * B) > 16 ? 16 : (sizeof(R) * B)) Vec { R x[B]; };
 
-template <typename V> __device__ __forceinline__ V vec_ldg(const V* p) {
+template <typename V> __device__ __forceinline__ V vec_ldg_(const V* p, int line) {
   V r;
+  if (!FTLM_G_OK(p, V, line)) return V{};
   if constexpr (sizeof(V) == 4) *(float*)&r = __ldg((const float*)p);
   else if constexpr (sizeof(V) == 8) *(float2*)&r = __ldg((const float2*)p);
   else {
@@ -107,8 +109,9 @@ template <typename V> __device__ __forceinline__ V vec_ldg(const V* p) {
   }
   return r;
 }
-template <typename V> __device__ __forceinline__ V vec_ldcs(const V* p) {
+template <typename V> __device__ __forceinline__ V vec_ldcs_(const V* p, int line) {
   V r;
+  if (!FTLM_G_OK(p, V, line)) return V{};
   if constexpr (sizeof(V) == 4) *(float*)&r = __ldcs((const float*)p);
   else if constexpr (sizeof(V) == 8) *(float2*)&r = __ldcs((const float2*)p);
   else {
@@ -117,7 +120,8 @@ template <typename V> __device__ __forceinline__ V vec_ldcs(const V* p) {
   }
   return r;
 }
-template <typename V> __device__ __forceinline__ void vec_stcs(V* p, const V& r) {
+template <typename V> __device__ __forceinline__ void vec_stcs_(V* p, const V& r, int line) {
+  if (!FTLM_G_OK(p, V, line)) return;
   if constexpr (sizeof(V) == 4) __stcs((float*)p, *(const float*)&r);
   else if constexpr (sizeof(V) == 8) __stcs((float2*)p, *(const float2*)&r);
   else {
@@ -125,6 +129,10 @@ template <typename V> __device__ __forceinline__ void vec_stcs(V* p, const V& r)
     for (int k = 0; k < (int)(sizeof(V) / 16); ++k) __stcs((float4*)p + k, ((const float4*)&r)[k]);
   }
 }
+
+#define vec_ldg(p) vec_ldg_((p), __LINE__)
+#define vec_ldcs(p) vec_ldcs_((p), __LINE__)
+#define vec_stcs(p, r) vec_stcs_((p), (r), __LINE__)
 
 // descriptor entries of the per-warp scratch lists
 template <typename R> struct UEnt;      // uniform gather: {offset, J}
@@ -147,7 +155,7 @@ __device__ __forceinline__ uint64_t tml_base_cr(uint32_t T, int mw, int K, const
     const int p = __ffs((int)x) - 1;
     x &= x - 1;
     ++c;
-    r += binom[(p + mw) * K1 + c];
+    r += LD_A(&binom[(p + mw) * K1 + c]);
   }
   return r;
 }
@@ -155,7 +163,7 @@ __device__ __forceinline__ uint64_t tml_base_cr(uint32_t T, int mw, int K, const
 template <int MODE>
 __device__ __forceinline__ uint64_t tml_base(uint32_t T, int mw, int K, const uint64_t* __restrict__ binom,
                                              const uint2* __restrict__ clt) {
-  if (MODE == FTLM_INDEX_CLT) return (uint64_t)__ldg(&clt[(size_t)T << (mw - 5)]).y;
+  if (MODE == FTLM_INDEX_CLT) return (uint64_t)LDG(&clt[(size_t)T << (mw - 5)]).y;
   return tml_base_cr(T, mw, K, binom);
 }
 
@@ -196,11 +204,12 @@ __host__ __device__ inline int tml_scratch_bytes(int esz, int n_tt, int n_tm, in
 }
 
 __device__ __forceinline__ void load_fent(const FEnt<float>* e, uint32_t& off, float& J, uint32_t& fl, uint32_t& uw) {
-  const uint4 q = *(const uint4*)e;
+  const uint4 q = LD_S((const uint4*)e);
   off = q.x; J = __uint_as_float(q.y); fl = q.z; uw = q.w;
 }
 __device__ __forceinline__ void load_fent(const FEnt<double>* e, uint32_t& off, double& J, uint32_t& fl, uint32_t& uw) {
-  off = e->off; fl = e->fl; J = e->J; uw = e->uw;
+  const FEnt<double> q = LD_S(e);
+  off = q.off; fl = q.fl; J = q.J; uw = q.uw;
 }
 __device__ __forceinline__ const void* addr_u32(const void* base, uint32_t idx, uint32_t scale) {
 #ifdef FTLM_EMU
@@ -236,11 +245,11 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
   TmlSmem S;
   tml_layout(S, smem, p.N, p.K, p.blob_bytes, p.max_tile, RB, B, NW, p.scratch_bytes);
   // ---- one-time staging of the tables --------------------------------------------------------
-  for (int k = tid; k < (p.N + 1) * (p.K + 1); k += NT) S.binom[k] = p.binom[k];
+  for (int k = tid; k < (p.N + 1) * (p.K + 1); k += NT) ST_S(&S.binom[k], LD_G(&p.binom[k]));
   {
     const uint4* src = (const uint4*)p.blob;
     uint4* dst = (uint4*)S.blob;
-    for (int k = tid; k < (p.blob_bytes >> 4); k += NT) dst[k] = __ldg(&src[k]);
+    for (int k = tid; k < (p.blob_bytes >> 4); k += NT) ST_S(&dst[k], LDG(&src[k]));
   }
   const int* s_koff = (const int*)(S.blob + p.off_koff);
   const int* s_tlen = (const int*)(S.blob + p.off_tlen);
@@ -283,8 +292,8 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         const unsigned bal = __ballot_sync(0xffffffffu, act);
         if (act) {
           const int pos = count + __popc(bal & ltmask);
-          S.tt_off[pos] = (uint32_t)tml_base<MODE>(T ^ mk, p.mw, p.K, S.binom, p.clt);
-          S.tt_J[pos] = p.tt_J[b];
+          ST_S(&S.tt_off[pos], (uint32_t)tml_base<MODE>(T ^ mk, p.mw, p.K, S.binom, p.clt));
+          ST_S(&S.tt_J[pos], p.tt_J[b]);
         }
         count += __popc(bal);
       }
@@ -295,8 +304,8 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
       const TmlSEnt* src = warp == 2 ? s_tm : s_tl;
       TmlTx* dst = warp == 2 ? S.txm : S.txl;
       for (int e = lane; e < n; e += 32) {
-        const TmlSEnt d = src[e];
-        const uint32_t site = p.ts_site[d.b], bit = 1u << site;
+        const TmlSEnt d = LD_S(&src[e]);
+        const uint32_t site = p.ts_site[d.b & (TML_MAX_TS - 1)], bit = 1u << site;
         const int kTp = (T & bit) ? kT + 1 : kT - 1;
         const bool ok = (kTp >= 0 && kTp <= p.mw);
         TmlTx x;
@@ -304,11 +313,11 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         x.cofs = ok ? kTp * nM : 0;
         x.u = (T >> site) & 1u;
         x.valid = ok ? 1 : 0;
-        dst[e] = x;
+        ST_S(&dst[e], x);
       }
     }
     const uint32_t base = (uint32_t)tml_base<MODE>(T, p.mw, p.K, S.binom, p.clt);
-    const int tlen = s_tlen[kT];
+    const int tlen = LD_S(&s_tlen[kT]);
     // ---- stage the tile (16-byte loads on the aligned interior; smem keeps the global misalignment) ----
     const int mis = (RB >= 16) ? 0 : (int)(base & (uint32_t)(16 / RB - 1));   // rows past a 16-byte boundary
     const unsigned char* vsb0 = S.vs + (size_t)mis * RB;                        // row 0 of the tile
@@ -317,23 +326,23 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
       const V* src = v + base;
       V* vs = (V*)vsb0;
       if (RPV == 1) {
-        for (int x = tid; x < tlen; x += NT) vs[x] = src[x];
+        for (int x = tid; x < tlen; x += NT) ST_S(&vs[x], LD_G(&src[x]));
       } else {
         const int head = mis ? (RPV - mis) : 0;                                  // rows before the first boundary
         const int h = head < tlen ? head : tlen;
         const int nvec = (tlen - h) / RPV;
-        if (tid < h) vs[tid] = src[tid];
+        if (tid < h) ST_S(&vs[tid], LD_G(&src[tid]));
         const uint4* s4 = (const uint4*)(src + h);
         uint4* d4 = (uint4*)(vs + h);
 #pragma unroll 4
-        for (int x = tid; x < nvec; x += NT) d4[x] = s4[x];
+        for (int x = tid; x < nvec; x += NT) ST_S(&d4[x], LD_G(&s4[x]));
         const int done = h + nvec * RPV;
-        if (tid < tlen - done) vs[done + tid] = src[done + tid];
+        if (tid < tlen - done) ST_S(&vs[done + tid], LD_G(&src[done + tid]));
       }
     }
     __syncthreads();
     // ---- rows: one warp per column (up to 8 chunks of 32 rows) ---------------------------------------
-    const int it0 = p.item_off[kT], it1 = p.item_off[kT + 1];
+    const int it0 = LD_G(&p.item_off[kT]), it1 = LD_G(&p.item_off[kT + 1]);
     const int ntt = S.misc[1];
     const uint16_t* co = s_coloff + kT * nM;
     double s_qy[B], s_yy[B], s_qq[B];
@@ -341,21 +350,21 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
     for (int b = 0; b < B; ++b) { s_qy[b] = 0.0; s_yy[b] = 0.0; s_qq[b] = 0.0; }
     (void)s_qy; (void)s_yy; (void)s_qq;
     for (int it = it0 + warp; it < it1; it += NW) {
-      const uint32_t item = __ldg(&p.items[it]);
+      const uint32_t item = LDG(&p.items[it]);
       const uint32_t M = item & 0xffffu;
       const int chunk0 = (int)((item >> 16) & 0xffu), nch = (int)(item >> 24);
       const int kL = kT - __popc(M);
-      const int k0 = s_koff[kL];
-      const int len = s_koff[kL + 1] - k0;
-      const uint32_t cb = co[M];
+      const int k0 = LD_S(&s_koff[kL]);
+      const int len = LD_S(&s_koff[kL + 1]) - k0;
+      const uint32_t cb = LD_S(&co[M]);
       // ---- build the descriptor lists of this column (lane e <-> list entry e) ---------------------
       __syncwarp();
       int nU = ntt, nS = 0, nFG = 0;
       const int nFS = p.n_ml;
       R sumJ = 0;                                       // J of the uniform (U, S) entries: folded into the diagonal
       for (int a = lane; a < ntt; a += 32) {             // TT: same offset in tile T ^ mask
-        const R J = (R)S.tt_J[a];
-        Ul[a].off = S.tt_off[a] + cb; Ul[a].J = J; sumJ += J;
+        const R J = (R)LD_S(&S.tt_J[a]);
+        ST_S(&Ul[a].off, LD_S(&S.tt_off[a]) + cb); ST_S(&Ul[a].J, J); sumJ += J;
       }
       for (int e0 = 0; e0 < p.n_tm; e0 += 32) {          // TM: tile T ^ bit_s, column M ^ bit_i, same lr
         const int e = e0 + lane;
@@ -363,13 +372,14 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         uint32_t off = 0;
         R J = 0;
         if (e < p.n_tm) {
-          const TmlTx x = S.txm[e];
-          const uint32_t i = s_tm[e].a;
+          const TmlTx x = LD_S(&S.txm[e]);
+          const TmlSEnt dtm = LD_S(&s_tm[e]);
+          const uint32_t i = dtm.a;
           act = x.valid && ((M >> i) & 1u) != x.u;
-          if (act) { off = x.off + s_coloff[x.cofs + (int)(M ^ (1u << i))]; J = (R)s_tm[e].J; }
+          if (act) { off = x.off + LD_S(&s_coloff[x.cofs + (int)(M ^ (1u << i))]); J = (R)dtm.J; }
         }
         const unsigned bal = __ballot_sync(0xffffffffu, act);
-        if (act) { const int pos = nU + __popc(bal & ltmask); Ul[pos].off = off; Ul[pos].J = J; sumJ += J; }
+        if (act) { const int pos = nU + __popc(bal & ltmask); ST_S(&Ul[pos].off, off); ST_S(&Ul[pos].J, J); sumJ += J; }
         nU += __popc(bal);
       }
       for (int e0 = 0; e0 < p.n_mm; e0 += 32) {          // MM: column M ^ mask of this tile, same lr
@@ -378,44 +388,49 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         uint32_t off = 0;
         R J = 0;
         if (e < p.n_mm) {
-          const TmlSEnt d = s_mm[e];
+          const TmlSEnt d = LD_S(&s_mm[e]);
           act = __popc(M & d.a) == 1;
-          if (act) { off = (uint32_t)co[M ^ d.a] * RB; J = (R)d.J; }
+          if (act) { off = (uint32_t)LD_S(&co[M ^ d.a]) * RB; J = (R)d.J; }
         }
         const unsigned bal = __ballot_sync(0xffffffffu, act);
-        if (act) { const int pos = nS + __popc(bal & ltmask); Sl[pos].off = off; Sl[pos].J = J; sumJ += J; }
+        if (act) { const int pos = nS + __popc(bal & ltmask); ST_S(&Sl[pos].off, off); ST_S(&Sl[pos].J, J); sumJ += J; }
         nS += __popc(bal);
       }
       for (int e = lane; e < nFS; e += 32) {             // ML: column M ^ bit_j, row flipped at L_i
-        const TmlSEnt d = s_ml[e];
+        const TmlSEnt d = LD_S(&s_ml[e]);
         const uint32_t u = (M >> d.b) & 1u;
-        FSl[e].off = (uint32_t)co[M ^ (1u << d.b)] - ((u ^ 1u) << 15);
-        FSl[e].J = (R)d.J;
-        FSl[e].fl = d.a * (uint32_t)nL * 2u;
-        FSl[e].uw = u << 15;
+        FEnt<R> fe{};
+        fe.off = (uint32_t)LD_S(&co[M ^ (1u << d.b)]) - ((u ^ 1u) << 15);
+        fe.J = (R)d.J;
+        fe.fl = d.a * (uint32_t)nL * 2u;
+        fe.uw = u << 15;
+        ST_S(&FSl[e], fe);
       }
       for (int e0 = 0; e0 < p.n_tl; e0 += 32) {          // TL: tile T ^ bit_s, column M, row flipped at L_i
         const int e = e0 + lane;
         bool act = false;
         TmlTx x;
-        if (e < p.n_tl) { x = S.txl[e]; act = x.valid != 0; }
+        if (e < p.n_tl) { x = LD_S(&S.txl[e]); act = x.valid != 0; }
         const unsigned bal = __ballot_sync(0xffffffffu, act);
         if (act) {
           const int pos = nFG + __popc(bal & ltmask);
-          FGl[pos].off = x.off + s_coloff[x.cofs + (int)M] - ((x.u ^ 1u) << 15);
-          FGl[pos].J = (R)s_tl[e].J;
-          FGl[pos].fl = s_tl[e].a * (uint32_t)nL * 2u;
-          FGl[pos].uw = x.u << 15;
+          const TmlSEnt dtl = LD_S(&s_tl[e]);
+          FEnt<R> fe{};
+          fe.off = x.off + LD_S(&s_coloff[x.cofs + (int)M]) - ((x.u ^ 1u) << 15);
+          fe.J = (R)dtl.J;
+          fe.fl = dtl.a * (uint32_t)nL * 2u;
+          fe.uw = x.u << 15;
+          ST_S(&FGl[pos], fe);
         }
         nFG += __popc(bal);
       }
       // pad the flip lists to a multiple of 4 with entries that are never active: row w of FLtab is
       // all zero, so (entry ^ 0) & 0x8000 == 0 for every lane
       if (lane < 4) {
-        FEnt<R> z; z.off = cb; z.J = 0; z.fl = (uint32_t)p.w * (uint32_t)nL * 2u; z.uw = 0;
-        { const uint32_t q = (nFS + lane); if (q < (uint32_t)((nFS + 3) & ~3)) FSl[q] = z; }
+        FEnt<R> z{}; z.off = cb; z.J = 0; z.fl = (uint32_t)p.w * (uint32_t)nL * 2u; z.uw = 0;
+        { const uint32_t q = (nFS + lane); if (q < (uint32_t)((nFS + 3) & ~3)) ST_S(&FSl[q], z); }
         z.off = base + cb;
-        { const uint32_t q = (nFG + lane); if (q < (uint32_t)((nFG + 3) & ~3)) FGl[q] = z; }
+        { const uint32_t q = (nFG + lane); if (q < (uint32_t)((nFG + 3) & ~3)) ST_S(&FGl[q], z); }
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) sumJ += __shfl_xor_sync(0xffffffffu, sumJ, o);
@@ -431,7 +446,7 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         const int Lidx = k0 + lrc;
         const unsigned char* pl = vsb0 + (size_t)lrc * RB;               // lane pointer: row lrc of column 0
         const unsigned char* flp = s_fl + Lidx * 2;
-        const V own = *(const V*)(vsb + (size_t)lrc * RB);
+        const V own = LD_S((const V*)(vsb + (size_t)lrc * RB));
         V qp;                                             // q_prev: issued now, consumed in the epilogue
         if (FUSED) qp = vec_ldcs(qprev + ((size_t)base + cb + lrc));
         V acc;
@@ -442,7 +457,7 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
           const V* vl = v + lrc;
           int e = 0;
           for (; e + 4 <= nU; e += 4) {
-            const UEnt<R> d0 = Ul[e], d1 = Ul[e + 1], d2 = Ul[e + 2], d3 = Ul[e + 3];
+            const UEnt<R> d0 = LD_S(&Ul[e]), d1 = LD_S(&Ul[e + 1]), d2 = LD_S(&Ul[e + 2]), d3 = LD_S(&Ul[e + 3]);
             const V a0 = vec_ldg((const V*)addr_u32(vl, d0.off, RB));
             const V a1 = vec_ldg((const V*)addr_u32(vl, d1.off, RB));
             const V a2 = vec_ldg((const V*)addr_u32(vl, d2.off, RB));
@@ -451,7 +466,7 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
             for (int b = 0; b < B; ++b) acc.x[b] += d0.J * a0.x[b] + d1.J * a1.x[b] + d2.J * a2.x[b] + d3.J * a3.x[b];
           }
           for (; e < nU; ++e) {
-            const UEnt<R> d = Ul[e];
+            const UEnt<R> d = LD_S(&Ul[e]);
             const V a = vec_ldg((const V*)addr_u32(vl, d.off, RB));
 #pragma unroll
             for (int b = 0; b < B; ++b) acc.x[b] += d.J * a.x[b];
@@ -463,8 +478,8 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
           R j0, j1, j2, j3;
           load_fent(FGl + e, o0, j0, f0, u0); load_fent(FGl + e + 1, o1, j1, f1, u1);
           load_fent(FGl + e + 2, o2, j2, f2, u2); load_fent(FGl + e + 3, o3, j3, f3, u3);
-          const uint32_t x0 = *(const uint16_t*)(flp + f0), x1 = *(const uint16_t*)(flp + f1);
-          const uint32_t x2 = *(const uint16_t*)(flp + f2), x3 = *(const uint16_t*)(flp + f3);
+          const uint32_t x0 = LD_S((const uint16_t*)(flp + f0)), x1 = LD_S((const uint16_t*)(flp + f1));
+          const uint32_t x2 = LD_S((const uint16_t*)(flp + f2)), x3 = LD_S((const uint16_t*)(flp + f3));
           V a0 = own, a1 = own, a2 = own, a3 = own;
           if ((x0 ^ u0) & 0x8000u) a0 = vec_ldg((const V*)addr_u32(v, o0 + x0, RB));
           if ((x1 ^ u1) & 0x8000u) a1 = vec_ldg((const V*)addr_u32(v, o1 + x1, RB));
@@ -476,11 +491,11 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         }
         // LL: swap form, 4 bonds per 8-byte table entry
         for (int g = 0; g < (p.n_ll4 >> 2); ++g) {
-          const uint2 q = s_ll[g * nL + Lidx];
-          const V a0 = *(const V*)(vsb + (q.x & 0xffffu) * RB);
-          const V a1 = *(const V*)(vsb + (q.x >> 16) * RB);
-          const V a2 = *(const V*)(vsb + (q.y & 0xffffu) * RB);
-          const V a3 = *(const V*)(vsb + (q.y >> 16) * RB);
+          const uint2 q = LD_S(&s_ll[g * nL + Lidx]);
+          const V a0 = LD_S((const V*)(vsb + (q.x & 0xffffu) * RB));
+          const V a1 = LD_S((const V*)(vsb + (q.x >> 16) * RB));
+          const V a2 = LD_S((const V*)(vsb + (q.y & 0xffffu) * RB));
+          const V a3 = LD_S((const V*)(vsb + (q.y >> 16) * RB));
           const R j0 = p.ll_J[4 * g + 0], j1 = p.ll_J[4 * g + 1], j2 = p.ll_J[4 * g + 2], j3 = p.ll_J[4 * g + 3];
 #pragma unroll
           for (int b = 0; b < B; ++b) acc.x[b] += j0 * a0.x[b] + j1 * a1.x[b] + j2 * a2.x[b] + j3 * a3.x[b];
@@ -488,8 +503,8 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         // S: other column of this tile, same lr
 #pragma unroll 4
         for (int e = 0; e < nS; ++e) {
-          const UEnt<R> d = Sl[e];
-          const V a = *(const V*)(pl + d.off);
+          const UEnt<R> d = LD_S(&Sl[e]);
+          const V a = LD_S((const V*)(pl + d.off));
 #pragma unroll
           for (int b = 0; b < B; ++b) acc.x[b] += d.J * a.x[b];
         }
@@ -499,13 +514,13 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
           R j0, j1, j2, j3;
           load_fent(FSl + e, o0, j0, f0, u0); load_fent(FSl + e + 1, o1, j1, f1, u1);
           load_fent(FSl + e + 2, o2, j2, f2, u2); load_fent(FSl + e + 3, o3, j3, f3, u3);
-          const uint32_t x0 = *(const uint16_t*)(flp + f0), x1 = *(const uint16_t*)(flp + f1);
-          const uint32_t x2 = *(const uint16_t*)(flp + f2), x3 = *(const uint16_t*)(flp + f3);
+          const uint32_t x0 = LD_S((const uint16_t*)(flp + f0)), x1 = LD_S((const uint16_t*)(flp + f1));
+          const uint32_t x2 = LD_S((const uint16_t*)(flp + f2)), x3 = LD_S((const uint16_t*)(flp + f3));
           V a0 = own, a1 = own, a2 = own, a3 = own;
-          if ((x0 ^ u0) & 0x8000u) a0 = *(const V*)(vsb0 + (size_t)(o0 + x0) * RB);
-          if ((x1 ^ u1) & 0x8000u) a1 = *(const V*)(vsb0 + (size_t)(o1 + x1) * RB);
-          if ((x2 ^ u2) & 0x8000u) a2 = *(const V*)(vsb0 + (size_t)(o2 + x2) * RB);
-          if ((x3 ^ u3) & 0x8000u) a3 = *(const V*)(vsb0 + (size_t)(o3 + x3) * RB);
+          if ((x0 ^ u0) & 0x8000u) a0 = LD_S((const V*)(vsb0 + (size_t)(o0 + x0) * RB));
+          if ((x1 ^ u1) & 0x8000u) a1 = LD_S((const V*)(vsb0 + (size_t)(o1 + x1) * RB));
+          if ((x2 ^ u2) & 0x8000u) a2 = LD_S((const V*)(vsb0 + (size_t)(o2 + x2) * RB));
+          if ((x3 ^ u3) & 0x8000u) a3 = LD_S((const V*)(vsb0 + (size_t)(o3 + x3) * RB));
 #pragma unroll
           for (int b = 0; b < B; ++b)
             acc.x[b] += j0 * (a0.x[b] - own.x[b]) + j1 * (a1.x[b] - own.x[b]) + j2 * (a2.x[b] - own.x[b]) + j3 * (a3.x[b] - own.x[b]);
@@ -532,13 +547,13 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
 #pragma unroll
       for (int b = 0; b < B; ++b) {
         const double a = warp_sum(s_qy[b]), bb = warp_sum(s_yy[b]), c = warp_sum(s_qq[b]);
-        if (lane == 0) { S.red[warp * 3 * B + 3 * b] = a; S.red[warp * 3 * B + 3 * b + 1] = bb; S.red[warp * 3 * B + 3 * b + 2] = c; }
+        if (lane == 0) { ST_S(&S.red[warp * 3 * B + 3 * b], a); ST_S(&S.red[warp * 3 * B + 3 * b + 1], bb); ST_S(&S.red[warp * 3 * B + 3 * b + 2], c); }
       }
       __syncthreads();
       if (tid < 3 * B) {
         double s = 0.0;
-        for (int wv = 0; wv < NW; ++wv) s += S.red[wv * 3 * B + tid];
-        p.partials[(size_t)tid * p.nT + T] = s;
+        for (int wv = 0; wv < NW; ++wv) s += LD_S(&S.red[wv * 3 * B + tid]);
+        ST_G(&p.partials[(size_t)tid * p.nT + T], s);
       }
     }
   }
@@ -555,22 +570,22 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
   if (FUSED != 1) return;
   for (int q = 0; q < 3 * B; ++q) {                       // fixed assignment and order
     double a = 0.0;
-    for (uint32_t k = tid; k < p.nT; k += NT) a += p.partials[(size_t)q * p.nT + k];
+    for (uint32_t k = tid; k < p.nT; k += NT) a += LD_G(&p.partials[(size_t)q * p.nT + k]);
     a = warp_sum(a);
     __syncthreads();
-    if (lane == 0) S.red[warp] = a;
+    if (lane == 0) ST_S(&S.red[warp], a);
     __syncthreads();
     if (tid == 0) {
       double s = 0.0;
-      for (int wv = 0; wv < NW; ++wv) s += S.red[wv];
-      S.red[64 + q] = s;
+      for (int wv = 0; wv < NW; ++wv) s += LD_S(&S.red[wv]);
+      ST_S(&S.red[64 + q], s);
     }
   }
   __syncthreads();
   if (tid < B) {
     ChainState* st = p.st + tid;
     if (!st->done) {
-      const double a = S.red[64 + 3 * tid], b = S.red[64 + 3 * tid + 1], c = S.red[64 + 3 * tid + 2];
+      const double a = LD_S(&S.red[64 + 3 * tid]), b = LD_S(&S.red[64 + 3 * tid + 1]), c = LD_S(&S.red[64 + 3 * tid + 2]);
       const int j = st->step;
       const double alpha = c > 0.0 ? a / c : 0.0;
       double b2 = c > 0.0 ? b - a * a / c : 0.0;
@@ -613,35 +628,35 @@ neighbors_tml_kernel(const __grid_constant__ TmlParams<R> p, const BondDev* __re
     uint64_t n = 0, rem = tr;
     int A = p.K;
     for (int q = p.N - 1; q >= 0 && A > 0; --q) {
-      const uint64_t c = p.binom[q * K1 + A];
+      const uint64_t c = LD_G(&p.binom[q * K1 + A]);
       if (rem >= c) { n |= 1ull << q; rem -= c; --A; }
     }
     const uint32_t T = (uint32_t)(n >> p.mw), M = (uint32_t)(n >> p.w) & (uint32_t)(nM - 1), L = (uint32_t)n & (uint32_t)(nL - 1);
     const int kT = p.K - __popc(T), kL = kT - __popc(M);
     const uint64_t base = tml_base<MODE>(T, p.mw, p.K, p.binom, p.clt);
-    const int cb = coloff[kT * nM + M];
+    const int cb = (kT >= 0 && kT <= p.mw) ? (int)LD_G(&coloff[kT * nM + M]) : 0;
     const int lr = (int)(tr - base) - cb;
-    bool ok = lr >= 0 && lr < koff[kL + 1] - koff[kL];
-    const int Lidx = ok ? koff[kL] + lr : 0;
-    for (int i = 0; ok && i < p.w; ++i) ok = ((fl[i * nL + Lidx] >> 15) == ((L >> i) & 1u));   // FLtab knows L
+    bool ok = kL >= 0 && kL <= p.w && lr >= 0 && lr < LD_G(&koff[kL + 1]) - LD_G(&koff[kL]);
+    const int Lidx = ok ? LD_G(&koff[kL]) + lr : 0;
+    for (int i = 0; ok && i < p.w; ++i) ok = ((LD_G(&fl[i * nL + Lidx]) >> 15) == ((L >> i) & 1u));   // FLtab knows L
     for (int b = 0; b < nb; ++b) {
-      const uint64_t mk = bonds[b].mask, x = n & mk;
+      const uint64_t mk = LD_G(&bonds[b].mask), x = n & mk;
       int64_t idx = -1;
-      const int e = bentry[b];
+      const int e = LD_G(&bentry[b]), bcls = LD_G(&bclass[b]);
       if (x != 0 && x != mk) {
-        switch (bclass[b]) {
+        switch (bcls) {
           case 0: {                                      // LL
-            const uint2 q = ll[(e >> 2) * nL + Lidx];
+            const uint2 q = LD_G(&ll[(e >> 2) * nL + Lidx]);
             const uint32_t h = (e & 2) ? q.y : q.x;
             idx = (int64_t)base + cb + (int)((e & 1) ? (h >> 16) : (h & 0xffffu));
             break;
           }
-          case 1: idx = (int64_t)base + coloff[kT * nM + (M ^ mm[e].a)] + lr; break;                 // MM
-          case 2: idx = (int64_t)base + coloff[kT * nM + (M ^ (1u << ml[e].b))] +                    // ML
-                        (int)(fl[ml[e].a * nL + Lidx] & 0x7fffu); break;
-          case 3: idx = (int64_t)tml_base<MODE>(T ^ p.tt_mask[e], p.mw, p.K, p.binom, p.clt) + cb + lr; break;  // TT
+          case 1: idx = (int64_t)base + LD_G(&coloff[kT * nM + (M ^ LD_G(&mm[e].a))]) + lr; break;                 // MM
+          case 2: idx = (int64_t)base + LD_G(&coloff[kT * nM + (M ^ (1u << LD_G(&ml[e].b)))]) +        // ML
+                        (int)(LD_G(&fl[LD_G(&ml[e].a) * nL + Lidx]) & 0x7fffu); break;
+          case 3: idx = (int64_t)tml_base<MODE>(T ^ p.tt_mask[e & (TML_MAX_TT - 1)], p.mw, p.K, p.binom, p.clt) + cb + lr; break;  // TT
           case 6: {                                      // PASS-B window e: run start of the swapped window word + offset in the run
-            const int lo = p.pb_lo[e];
+            const int lo = p.pb_lo[e & 7];
             const uint64_t hi = n >> lo, low = n & ((1ull << lo) - 1ull);
             const int kP = p.K - __popcll((unsigned long long)hi);
             const uint64_t x = passb_low_rank(low, p.K, p.binom);
@@ -651,21 +666,22 @@ neighbors_tml_kernel(const __grid_constant__ TmlParams<R> p, const BondDev* __re
             break;
           }
           default: {                                     // TM / TL
-            const TmlSEnt d = bclass[b] == 4 ? tm[e] : tl[e];
-            const uint32_t bit = 1u << p.ts_site[d.b];
+            const TmlSEnt d = bcls == 4 ? LD_G(&tm[e]) : LD_G(&tl[e]);
+            const uint32_t bit = 1u << p.ts_site[d.b & (TML_MAX_TS - 1)];
             const int kTp = (T & bit) ? kT + 1 : kT - 1;
             const uint64_t tb = tml_base<MODE>(T ^ bit, p.mw, p.K, p.binom, p.clt);
-            if (bclass[b] == 4) idx = (int64_t)tb + coloff[kTp * nM + (M ^ (1u << d.a))] + lr;
-            else idx = (int64_t)tb + coloff[kTp * nM + M] + (int)(fl[d.a * nL + Lidx] & 0x7fffu);
+            if (kTp < 0 || kTp > p.mw) idx = -5;         // cannot happen for an antiparallel bond
+            else if (bcls == 4) idx = (int64_t)tb + LD_G(&coloff[kTp * nM + (M ^ (1u << d.a))]) + lr;
+            else idx = (int64_t)tb + LD_G(&coloff[kTp * nM + M]) + (int)(LD_G(&fl[d.a * nL + Lidx]) & 0x7fffu);
           }
         }
         if (!ok) idx = -2;
-      } else if (bclass[b] == 0 && ok) {                 // parallel LL bond: the table must say "self"
-        const uint2 q = ll[(e >> 2) * nL + Lidx];
+      } else if (bcls == 0 && ok) {                 // parallel LL bond: the table must say "self"
+        const uint2 q = LD_G(&ll[(e >> 2) * nL + Lidx]);
         const uint32_t h = (e & 2) ? q.y : q.x;
         if ((int)((e & 1) ? (h >> 16) : (h & 0xffffu)) != lr) idx = -3;
       }
-      out[r * nb + b] = idx;
+      ST_G(&out[r * nb + b], idx);
     }
   }
 }
@@ -766,8 +782,8 @@ void ftlm_tml_plan_destroy(ftlm_ctx* c) {
   ftlm_tmlr_plan_destroy(c);
   TmlPlan* t = c->tml;
   if (!t) return;
-  cudaFree(t->d_blob); cudaFree(t->d_items); cudaFree(t->d_item_off); cudaFree(t->d_partials);
-  cudaFree(t->d_counter); cudaFree(t->d_bond_class); cudaFree(t->d_bond_entry);
+  ftlm_dfree(t->d_blob); ftlm_dfree(t->d_items); ftlm_dfree(t->d_item_off); ftlm_dfree(t->d_partials);
+  ftlm_dfree(t->d_counter); ftlm_dfree(t->d_bond_class); ftlm_dfree(t->d_bond_entry);
   delete t;
   c->tml = nullptr;
 }
@@ -922,7 +938,7 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
   // ---- upload ----------------------------------------------------------------------------------
   P->partials_batch = 4;
   auto up = [&](void** d, const void* h, size_t bytes) -> bool {
-    if (cudaMalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
+    if (ftlm_dmalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
     if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
     return true;
   };

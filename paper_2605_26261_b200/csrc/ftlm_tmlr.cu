@@ -19,6 +19,7 @@
 #include <cstring>
 #include <vector>
 
+#define FTLM_TU 4
 #include "ftlm_passb.cuh"
 
 #define TMLR_MAX_LL 16
@@ -139,11 +140,11 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
   const int nL = 1 << p.w, nM = 1 << p.m;
   TmlrSmem<R> S;
   tmlr_layout<R>(S, smem, p.N, p.K, p.blob_bytes, p.max_tile, nM, p.n_mm, p.n_ml, p.n_g, NW);
-  for (int k = tid; k < (p.N + 1) * (p.K + 1); k += NT) S.binom[k] = p.binom[k];
+  for (int k = tid; k < (p.N + 1) * (p.K + 1); k += NT) ST_S(&S.binom[k], LD_G(&p.binom[k]));
   {
     const uint4* src = (const uint4*)p.blob;
     uint4* dst = (uint4*)S.blob;
-    for (int k = tid; k < (p.blob_bytes >> 4); k += NT) dst[k] = __ldg(&src[k]);
+    for (int k = tid; k < (p.blob_bytes >> 4); k += NT) ST_S(&dst[k], LDG(&src[k]));
   }
   const int* s_koff = (const int*)(S.blob + p.off_koff);
   const int* s_tlen = (const int*)(S.blob + p.off_tlen);
@@ -168,7 +169,7 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
     if (kT < 0 || kT > p.mw) continue;                  // no rows with this top part
     const uint64_t base = p.mode == FTLM_INDEX_CLT ? passb_run_start<FTLM_INDEX_CLT>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt)
                                                    : passb_run_start<FTLM_INDEX_CR>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt);
-    const int tlen = s_tlen[kT];
+    const int tlen = LD_S(&s_tlen[kT]);
     if (p.lazy) {                                       // lazy normalisation: q_{j+1} formed while staging, written over y_j
       const R a = (R)p.st->a, ib = (R)p.st->inv_b;
       R* yq = p.vio + base;
@@ -178,16 +179,16 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           const int x = x0 + k * NT;
-          yv[k] = x < tlen ? __ldcs(&yq[x]) : (R)0;
-          qv[k] = x < tlen ? qs[x] : (R)0;
+          yv[k] = x < tlen ? LDCS(&yq[x]) : (R)0;
+          qv[k] = x < tlen ? LD_G(&qs[x]) : (R)0;
         }
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           const int x = x0 + k * NT;
           if (x < tlen) {
             const R qn = (yv[k] - a * qv[k]) * ib;
-            S.vs[x] = qn;
-            yq[x] = qn;
+            ST_S(&S.vs[x], qn);
+            ST_G(&yq[x], qn);
           }
         }
       }
@@ -202,13 +203,13 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
       for (int e = 0; e < n_mm; ++e) {
         const uint32_t mk = p.mm_mask[e];
         if (__popc((uint32_t)M & mk) == 1) {
-          S.dmm[M * n_mm + n] = (uint32_t)co[(uint32_t)M ^ mk];
-          S.dmmJ[M * n_mm + n] = p.mm_J[e];
+          ST_S(&S.dmm[M * n_mm + n], (uint32_t)LD_S(&co[(uint32_t)M ^ mk]));
+          ST_S(&S.dmmJ[M * n_mm + n], p.mm_J[e]);
           coef -= p.mm_J[e];
           ++n;
         }
       }
-      S.dnmm[M] = n;
+      ST_S(&S.dnmm[M], n);
       if (p.n_g) {                                       // left-over TT / TM bonds: rows of another tile, same lr
         int ng = 0;
         for (int g = 0; g < p.n_g; ++g) {
@@ -228,78 +229,78 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
             const uint32_t Tn = T ^ tm;
             const uint64_t bn = p.mode == FTLM_INDEX_CLT ? passb_run_start<FTLM_INDEX_CLT>((uint64_t)Tn, p.mw, kTn, p.K, S.binom, p.clt)
                                                          : passb_run_start<FTLM_INDEX_CR>((uint64_t)Tn, p.mw, kTn, p.K, S.binom, p.clt);
-            S.dg[M * p.n_g + ng] = (uint32_t)(bn + s_coloff[kTn * nM + (int)Mn]);
-            S.dgJ[M * p.n_g + ng] = p.g_J[g];
+            ST_S(&S.dg[M * p.n_g + ng], (uint32_t)(bn + LD_S(&s_coloff[kTn * nM + (int)Mn])));
+            ST_S(&S.dgJ[M * p.n_g + ng], p.g_J[g]);
             coef -= p.g_J[g];
             ++ng;
           }
         }
-        S.dng[M] = ng;
+        ST_S(&S.dng[M], ng);
       }
-      S.dcoef[M] = coef;
+      ST_S(&S.dcoef[M], coef);
       for (int e = 0; e < n_ml; ++e) {
         const int j = p.ml_j[e];                         // padding entries: j = -1, never active (flo = 0, bit 31 = 0)
-        S.dml[M * n_ml + e] = j < 0 ? 0u : ((uint32_t)co[(uint32_t)M ^ (1u << j)] * (uint32_t)sizeof(R) | (((uint32_t)M >> j) & 1u));
+        ST_S(&S.dml[M * n_ml + e], j < 0 ? 0u : ((uint32_t)LD_S(&co[(uint32_t)M ^ (1u << j)]) * (uint32_t)sizeof(R) | (((uint32_t)M >> j) & 1u)));
       }
     }
     cp_async_wait_all();
     __syncthreads();
     // ---- units: one chunk of 32 low parts x a block of columns per warp ----------------------------
-    const int u0 = __ldg(&p.unit_off[kT]), u1 = __ldg(&p.unit_off[kT + 1]);
+    const int u0 = LDG(&p.unit_off[kT]), u1 = LDG(&p.unit_off[kT + 1]);
     double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
     (void)s_qy; (void)s_yy; (void)s_qq;
     for (int it = u0 + warp; it < u1; it += NW) {
-      const uint32_t un = __ldg(&p.units[it]);
+      const uint32_t un = LDG(&p.units[it]);
       const int kL = (int)(un & 15u), chunk = (int)((un >> 4) & 15u), col0 = (int)((un >> 8) & 0xfffu), ncols = (int)(un >> 20);
-      const int k0 = s_koff[kL];
-      const int len = s_koff[kL + 1] - k0;
+      const int k0 = LD_S(&s_koff[kL]);
+      const int len = LD_S(&s_koff[kL + 1]) - k0;
       const int lr = chunk * 32 + lane;
       const bool valid = lr < len;
       const int lrc = valid ? lr : 0;
       const int Lidx = k0 + lrc;
       uint32_t llo[NLL], flo[NML];                      // lane tables (registers)
 #pragma unroll
-      for (int e = 0; e < NLL; ++e) llo[e] = (uint32_t)s_ll[e * nL + Lidx] * (uint32_t)sizeof(R);
+      for (int e = 0; e < NLL; ++e) llo[e] = (uint32_t)LD_S(&s_ll[e * nL + Lidx]) * (uint32_t)sizeof(R);
 #pragma unroll
       for (int e = 0; e < NML; ++e) {                    // byte offset of the flipped row | L_i
-        const uint32_t f = (uint32_t)s_fl[e * nL + Lidx];
+        const uint32_t f = (uint32_t)LD_S(&s_fl[e * nL + Lidx]);
         flo[e] = (f & 0x7fffu) * (uint32_t)sizeof(R) | (f >> 15);
       }
-      const uint16_t* ml = s_mlist + s_moff[kT - kL] + col0;
-      uint32_t Mn = ml[0];
-      uint32_t cbn = co[Mn];
+      const uint16_t* ml = s_mlist + LD_S(&s_moff[kT - kL]) + col0;
+      uint32_t Mn = LD_S(&ml[0]);
+      uint32_t cbn = LD_S(&co[Mn]);
       R qpn = (R)0;
-      if (FUSED) qpn = __ldcs(qprev + (base + cbn + (uint32_t)lrc));
+      if (FUSED) qpn = LDCS(qprev + (base + cbn + (uint32_t)lrc));
       for (int c = 0; c < ncols; ++c) {
         const uint32_t M = Mn, cb = cbn;
         const R qp = qpn;
         if (c + 1 < ncols) {                              // q_prev of the next column is requested now
-          Mn = ml[c + 1];
-          cbn = co[Mn];
-          if (FUSED) qpn = __ldcs(qprev + (base + cbn + (uint32_t)lrc));
+          Mn = LD_S(&ml[c + 1]);
+          cbn = LD_S(&co[Mn]);
+          if (FUSED) qpn = LDCS(qprev + (base + cbn + (uint32_t)lrc));
         }
         const unsigned char* colb = (const unsigned char*)(S.vs + cb);
-        const R own = S.vs[cb + (uint32_t)lrc];
+        const R own = LD_S(&S.vs[cb + (uint32_t)lrc]);
         // four independent partial sums (LL even/odd, ML even/odd) keep the FMA dependency chains short
-        R acc = S.dcoef[M] * own;
+        R acc = LD_S(&S.dcoef[M]) * own;
         R l0 = (R)0, l1 = (R)0, m0 = (R)0, m1 = (R)0;
 #pragma unroll
         for (int e = 0; e < NLL; e += 2) {
-          const R a0 = *(const R*)(colb + llo[e]), a1 = *(const R*)(colb + llo[e + 1]);
+          const R a0 = LD_S((const R*)(colb + llo[e])), a1 = LD_S((const R*)(colb + llo[e + 1]));
           if (UNIJ) { l0 += a0; l1 += a1; } else { l0 += p.ll_J[e] * a0; l1 += p.ll_J[e + 1] * a1; }
         }
-        const int nmm = S.dnmm[M];
-        for (int a = 0; a < nmm; ++a) acc += S.dmmJ[M * n_mm + a] * S.vs[S.dmm[M * n_mm + a] + (uint32_t)lrc];
+        const int nmm = LD_S(&S.dnmm[M]);
+        for (int a = 0; a < nmm; ++a) acc += LD_S(&S.dmmJ[M * n_mm + a]) * LD_S(&S.vs[LD_S(&S.dmm[M * n_mm + a]) + (uint32_t)lrc]);
         if (p.n_g) {
-          const int ng = S.dng[M];
-          for (int a = 0; a < ng; ++a) acc += S.dgJ[M * p.n_g + a] * __ldg(v + ((size_t)S.dg[M * p.n_g + a] + (uint32_t)lrc));
+          const int ng = LD_S(&S.dng[M]);
+          for (int a = 0; a < ng; ++a) acc += LD_S(&S.dgJ[M * p.n_g + a]) * LDG(v + ((size_t)LD_S(&S.dg[M * p.n_g + a]) + (uint32_t)lrc));
         }
 #pragma unroll
         for (int e = 0; e < NML; e += 2) {
-          const uint32_t d0 = S.dml[M * n_ml + e], f0 = flo[e], d1 = S.dml[M * n_ml + e + 1], f1 = flo[e + 1];
+          const uint32_t d0 = LD_S(&S.dml[M * n_ml + e]), f0 = flo[e], d1 = LD_S(&S.dml[M * n_ml + e + 1]), f1 = flo[e + 1];
           R a0 = own, a1 = own;
-          if ((d0 ^ f0) & 1u) a0 = *(const R*)(vsm1 + d0 + f0);   // active: exactly one of the two low bits is set
-          if ((d1 ^ f1) & 1u) a1 = *(const R*)(vsm1 + d1 + f1);
+          if ((d0 ^ f0) & 1u) a0 = LD_S((const R*)(vsm1 + d0 + f0));   // active: exactly one of the two low bits is set
+          if ((d1 ^ f1) & 1u) a1 = LD_S((const R*)(vsm1 + d1 + f1));
           if (UNIJ) { m0 += a0; m1 += a1; } else { m0 += p.ml_J[e] * a0; m1 += p.ml_J[e + 1] * a1; }
         }
         if (UNIJ) acc += p.ll_J[0] * (l0 + l1) + p.ml_J[0] * (m0 + m1);
@@ -314,18 +315,18 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
               s_qq += (double)own * (double)own;
             }
           }
-          __stcs(y + g, acc);
+          STCS(y + g, acc);
         }
       }
     }
     if (FUSED == 1) {                                   // deterministic per-tile partial sums
       const double a = warp_sum(s_qy), b = warp_sum(s_yy), c = warp_sum(s_qq);
-      if (lane == 0) { S.red[warp * 3] = a; S.red[warp * 3 + 1] = b; S.red[warp * 3 + 2] = c; }
+      if (lane == 0) { ST_S(&S.red[warp * 3], a); ST_S(&S.red[warp * 3 + 1], b); ST_S(&S.red[warp * 3 + 2], c); }
       __syncthreads();
       if (tid < 3) {
         double s = 0.0;
-        for (int wv = 0; wv < NW; ++wv) s += S.red[wv * 3 + tid];
-        p.partials[(size_t)tid * p.nT + T] = s;
+        for (int wv = 0; wv < NW; ++wv) s += LD_S(&S.red[wv * 3 + tid]);
+        ST_G(&p.partials[(size_t)tid * p.nT + T], s);
       }
     }
   }
@@ -343,13 +344,13 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
   double tot[3];
   for (int q = 0; q < 3; ++q) {                         // fixed assignment and order
     double a = 0.0;
-    for (uint32_t k = tid; k < p.nT; k += NT) a += p.partials[(size_t)q * p.nT + k];
+    for (uint32_t k = tid; k < p.nT; k += NT) a += LD_G(&p.partials[(size_t)q * p.nT + k]);
     a = warp_sum(a);
     __syncthreads();
-    if (lane == 0) S.red[warp] = a;
+    if (lane == 0) ST_S(&S.red[warp], a);
     __syncthreads();
     double s = 0.0;
-    if (tid == 0) for (int wv = 0; wv < NW; ++wv) s += S.red[wv];
+    if (tid == 0) for (int wv = 0; wv < NW; ++wv) s += LD_S(&S.red[wv]);
     tot[q] = s;
   }
   if (tid == 0) {
@@ -457,7 +458,7 @@ int launch_tmlr(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, 
 void ftlm_tmlr_plan_destroy(ftlm_ctx* c) {
   TmlrPlan* t = c->tmlr;
   if (!t) return;
-  cudaFree(t->d_blob); cudaFree(t->d_units); cudaFree(t->d_unit_off); cudaFree(t->d_partials); cudaFree(t->d_counter);
+  ftlm_dfree(t->d_blob); ftlm_dfree(t->d_units); ftlm_dfree(t->d_unit_off); ftlm_dfree(t->d_partials); ftlm_dfree(t->d_counter);
   delete t;
   c->tmlr = nullptr;
 }
@@ -589,7 +590,7 @@ int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_
   P->smem = c->prec == FTLM_FP32 ? tmlr_smem_bytes<float>(c, P) : tmlr_smem_bytes<double>(c, P);
   if (P->smem > (size_t)227 * 1024 - 1024) { c->tmlr = nullptr; delete P; return FTLM_OK; }
   auto up = [&](void** d, const void* h, size_t bytes) -> bool {
-    if (cudaMalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
+    if (ftlm_dmalloc(d, bytes ? bytes : 16) != cudaSuccess) return false;
     if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
     return true;
   };

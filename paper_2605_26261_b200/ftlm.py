@@ -12,12 +12,15 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libftlm.so")
+# FTLM_CHECKED=1 selects the range-checked build of the same kernels (csrc/ftlm_access.cuh); it is a test aid,
+# several times slower, and reports through ftlm_get_option(ctx, "check_violations").
+CHECKED = os.environ.get("FTLM_CHECKED", "0") not in ("", "0")
+LIB_PATH = os.path.join(_HERE, "libftlm_checked.so" if CHECKED else "libftlm.so")
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
 INDEX_CLT, INDEX_CR = 0, 1
 FP32, FP64 = 0, 1
-KERNEL_AUTO, KERNEL_ROW, KERNEL_TILE, KERNEL_TML = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_ROW, KERNEL_TML = 0, 1, 3
 MAX_STEPS = 1024
 
 EXPORTS = [
@@ -108,6 +111,19 @@ def ftlm_set_option(ctx, key: str, value: int):
 
 def ftlm_get_option(ctx, key: str) -> int:
     return int(lib().ftlm_get_option(ctx, key.encode()))
+
+
+def ftlm_check_info() -> dict:
+    """Checked build (FTLM_CHECKED=1): device-side address violations so far in this process and the first one
+    (translation unit, source line, kind 0/1 = global range/alignment, 2/3 = shared range/alignment)."""
+    keys = ["check_build", "check_violations", "check_first_tu", "check_first_line", "check_first_kind",
+            "check_first_block", "check_first_thread", "check_first_addr"]
+    return {k: int(lib().ftlm_get_option(C.c_void_p(0), k.encode())) for k in keys}
+
+
+def ftlm_check_selftest() -> int:
+    """Checked build: launch five deliberately bad accesses; returns how many the checker suppressed and counted (5)."""
+    return int(lib().ftlm_get_option(C.c_void_p(0), b"check_selftest"))
 
 
 def ftlm_table_bytes(ctx) -> int:

@@ -1,5 +1,8 @@
+import json
 import os
+import subprocess
 import sys
+import time
 
 import pytest
 
@@ -7,10 +10,65 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+PREFLIGHT_REPORT = os.path.join(ROOT, "gpurun_out", "checked_preflight.json")
+
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
     config.addinivalue_line("markers", "slow: heavier GPU parity case (full BASELINE sizes)")
+
+
+def _wants_gpu(config):
+    expr = config.getoption("-m") or ""
+    return "gpu" in expr and "not gpu" not in expr
+
+
+def pytest_sessionstart(session):
+    """Checked pre-flight.  A `-m gpu` session first runs the same selection of tests
+    in a child pytest with FTLM_CHECKED=1: the binding then loads libftlm_checked.so, the build of the same
+    kernel sources in which every computed address is range- and alignment-checked on the device and a
+    violation suppresses the access instead of faulting (csrc/ftlm_access.cuh).  The release library is
+    used only if that run passes with zero violations; otherwise the session ends here."""
+    config = session.config
+    if not _wants_gpu(config) or os.environ.get("FTLM_CHECKED", "0") not in ("", "0"):
+        return
+    if os.environ.get("FTLM_PREFLIGHT", "1") == "0":
+        return
+    try:
+        import torch
+        if not torch.cuda.is_available():
+            return
+    except Exception:
+        return
+    from paper_2605_26261_b200 import build
+    build.build(checked=True)
+    build.build()
+    env = dict(os.environ, FTLM_CHECKED="1", FTLM_PREFLIGHT="0")
+    args = [a for a in config.invocation_params.args]
+    t0 = time.time()
+    p = subprocess.run([sys.executable, "-m", "pytest", *args, "-p", "no:cacheprovider"], cwd=ROOT, env=env,
+                       capture_output=True, text=True, timeout=int(os.environ.get("FTLM_PREFLIGHT_TIMEOUT", "5400")))
+    rep = {"rc": p.returncode, "seconds": round(time.time() - t0, 1), "args": args,
+           "tail": p.stdout.strip().splitlines()[-12:]}
+    os.makedirs(os.path.dirname(PREFLIGHT_REPORT), exist_ok=True)
+    with open(PREFLIGHT_REPORT, "w") as f:
+        json.dump(rep, f, indent=1)
+    sys.stderr.write("[ftlm] checked pre-flight: rc=%d in %.0f s: %s\n" % (p.returncode, rep["seconds"], rep["tail"][-1] if rep["tail"] else ""))
+    if p.returncode != 0:
+        sys.stderr.write(p.stdout[-6000:] + "\n" + p.stderr[-2000:] + "\n")
+        pytest.exit("checked pre-flight failed (libftlm_checked.so): the release library is not run", returncode=3)
+
+
+@pytest.fixture(autouse=True)
+def _no_check_violations(request):
+    """In the checked build every GPU test ends with the device-side violation counter at zero."""
+    yield
+    if request.node.get_closest_marker("gpu") is None or os.environ.get("FTLM_CHECKED", "0") in ("", "0"):
+        return
+    from paper_2605_26261_b200 import ftlm
+    info = ftlm.ftlm_check_info()
+    assert info["check_build"] == 1, "FTLM_CHECKED=1 but the loaded library is not the checked build"
+    assert info["check_violations"] == 0, f"checked build: address violations on the device: {info}"
 
 
 def golden(name):

@@ -34,8 +34,9 @@ void* guarded_alloc(size_t bytes) {
   if (m == MAP_FAILED) return nullptr;
   mprotect(m, PAGE, PROT_NONE);
   mprotect(m + PAGE + body, PAGE, PROT_NONE);
-  char* p = m + PAGE + body - data;        // the data ends exactly at the trailing guard page
-  memset(m + PAGE, 0xCD, body - data);      // slack in front: poison
+  static const bool front = getenv("FTLM_EMU_ALIGN") && !strcmp(getenv("FTLM_EMU_ALIGN"), "front");
+  char* p = front ? m + PAGE : m + PAGE + body - data;   // data flush against the trailing (default) or the leading guard page
+  memset(m + PAGE, 0xCD, body);             // slack: poison
   memset(p, 0xA5, data);                    // uninitialised device memory is not zero
   g_allocs[p] = Alloc{m, total};
   return p;
@@ -48,7 +49,8 @@ void guarded_free(void* p) {
 }
 
 // ---- fibers ------------------------------------------------------------------------------------
-struct Fiber { ucontext_t ctx; char* stack = nullptr; bool done = false; bool started = false; };
+struct PendingCopy { void* dst; size_t bytes; unsigned char data[16]; };
+struct Fiber { ucontext_t ctx; char* stack = nullptr; bool done = false; bool started = false; std::vector<PendingCopy> pending; };
 const size_t STACK = 64 * 1024;
 std::vector<Fiber> g_fib;
 std::vector<char*> g_stack_pool;
@@ -105,6 +107,7 @@ void complete_collective(Warp& w) {
 void fiber_entry() {
   (*g_body)();
   Fiber& f = g_fib[(size_t)g_cur];
+  if (!f.pending.empty()) die("thread exits with cp.async copies it never waited for");
   f.done = true;
   g_progress++;
   g_alive--;
@@ -124,7 +127,7 @@ void run_block() {
   g_warps.assign((nt + 31) / 32, Warp());
   for (unsigned i = 0; i < nt; ++i) {
     Fiber& f = g_fib[i];
-    f.done = false; f.started = false; f.stack = g_stack_pool[i];
+    f.done = false; f.started = false; f.stack = g_stack_pool[i]; f.pending.clear();
     getcontext(&f.ctx);
     f.ctx.uc_stack.ss_sp = f.stack;
     f.ctx.uc_stack.ss_size = STACK;
@@ -171,6 +174,24 @@ cudaError_t g_last = cudaSuccess;
 namespace cuda_emu {
 
 unsigned char* dyn_smem() { return g_dyn; }
+
+void cp_async_issue(void* smem_dst, const void* gsrc, size_t bytes) {
+  if (g_cur < 0) die("cp.async outside a kernel");
+  if (bytes != 4 && bytes != 8 && bytes != 16) die("cp.async copies 4, 8 or 16 bytes");
+  if (((uintptr_t)smem_dst % bytes) || ((uintptr_t)gsrc % bytes)) die("cp.async: misaligned source or destination");
+  PendingCopy c;
+  c.dst = smem_dst; c.bytes = bytes;
+  memcpy(c.data, gsrc, bytes);              // faults here if the source is out of range (guard page)
+  memset(smem_dst, 0xFF, bytes);            // not visible yet: NaN until the issuing thread waits
+  g_fib[(size_t)g_cur].pending.push_back(c);
+}
+
+void cp_async_wait_all() {
+  if (g_cur < 0) die("cp.async.wait_all outside a kernel");
+  Fiber& f = g_fib[(size_t)g_cur];
+  for (const PendingCopy& c : f.pending) memcpy(c.dst, c.data, c.bytes);
+  f.pending.clear();
+}
 
 void sync_threads() {
   if (g_cur < 0) die("__syncthreads outside a kernel");

@@ -4,8 +4,11 @@
 // a fiber (ucontext), __syncthreads / __syncwarp / __ballot_sync / __shfl_*_sync are real rendezvous
 // points, "device" memory is guarded host memory (a PROT_NONE page directly behind every allocation
 // and behind the dynamic shared memory, so reads or writes past the end fault instead of passing).
-// CTAs of a grid run one after another.  This is a checker for index arithmetic, table construction,
-// barrier placement and bounds - it is never loaded by the product binding and has no performance
+// CTAs of a grid run one after another (nothing inter-CTA - the atomic tile / item hand-out with several CTAs in
+// flight, the last-CTA ticket - is exercised concurrently: that is left to the checked build on the device).
+// FTLM_EMU_ALIGN=front places every allocation flush against its FRONT guard page instead of the back one, so
+// that underruns fault too (the suite is run both ways).  This is a checker for index arithmetic, table construction,
+// barrier placement, cp.async waits, alignment and bounds - it is never loaded by the product binding and has no performance
 // meaning.
 #pragma once
 #include <algorithm>
@@ -89,6 +92,11 @@ void launch(unsigned grid, unsigned block, size_t dyn_smem, const std::function<
 unsigned char* dyn_smem();
 void sync_threads();
 uint64_t collective(int op, unsigned mask, uint64_t v, int arg);
+// cp.async model: the destination is poisoned (0xFF bytes = NaN) when the copy is issued and the bytes land
+// only when the ISSUING thread executes cp_async_wait_all(); a thread that exits with copies pending aborts.
+// A consumer that reads before the producer's wait + barrier therefore sees NaN instead of passing by luck.
+void cp_async_issue(void* smem_dst, const void* gsrc, size_t bytes);
+void cp_async_wait_all();
 enum { OP_SYNCWARP = 0, OP_BALLOT = 1, OP_SHFL_DOWN = 2, OP_SHFL_XOR = 3, OP_SHFL_IDX = 4, OP_SHFL_UP = 5 };
 template <typename T> static inline uint64_t pack(T v) { uint64_t u = 0; static_assert(sizeof(T) <= 8, "shfl payload"); memcpy(&u, &v, sizeof(T)); return u; }
 template <typename T> static inline T unpack(uint64_t u) { T v; memcpy(&v, &u, sizeof(T)); return v; }

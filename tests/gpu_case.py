@@ -119,6 +119,10 @@ def main():
         res["m_eff"] = int(out["m_eff"][0])
         res["ok"] = res["ok"] and da <= (1e-9 if prec == "fp64" else 2e-4) and res["m_eff"] == m
     ftlm.ftlm_destroy(ctx)
+    chk = ftlm.ftlm_check_info()                             # checked build (FTLM_CHECKED=1): no suppressed access
+    res["check"] = chk
+    if ftlm.CHECKED:
+        res["ok"] = res["ok"] and chk["check_build"] == 1 and chk["check_violations"] == 0
     print(json.dumps(res))
 
 

@@ -12,13 +12,11 @@ HV_TOL = {"fp32": 1e-5, "fp64": 1e-12}      # BASELINE.json north_star
 
 
 class Ctx:
-    def __init__(self, w, n_up, mode, prec, h=None, J=None, kernel=None, low_bits=None):
+    def __init__(self, w, n_up, mode, prec, h=None, J=None, kernel=None):
         self.w, self.n_up, self.mode, self.prec = w, n_up, mode, prec
         self.h = w.h if h is None else h
         self.J = w.J if J is None else J
         self.ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, self.J, n_up, MODES[mode], PRECS[prec], self.h)
-        if low_bits is not None:
-            ftlm.ftlm_set_option(self.ctx, "low_bits", low_bits)
         if kernel is not None:
             ftlm.ftlm_set_option(self.ctx, "kernel", kernel)
         self.dim = ftlm.ftlm_dim(self.ctx)

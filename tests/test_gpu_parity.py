@@ -15,7 +15,7 @@ from paper_2605_26261_b200 import ftlm         # noqa: E402
 from paper_2605_26261_b200 import workloads as W   # noqa: E402
 from gpu_util import Ctx, HV_TOL, NDT, relerr  # noqa: E402
 
-KERNELS = [ftlm.KERNEL_ROW, ftlm.KERNEL_TILE, ftlm.KERNEL_TML]
+KERNELS = [ftlm.KERNEL_ROW, ftlm.KERNEL_TML]
 
 
 def _kernel_ok(c, kernel):
@@ -26,6 +26,27 @@ def _kernel_ok(c, kernel):
             return False
         raise
     return True
+
+
+# ---------------------------------------------------------------- checked build (csrc/ftlm_access.cuh)
+
+def test_checked_build_suppresses_and_counts_bad_accesses():
+    """The range-checked build must catch (and suppress, without a device fault) five deliberately bad accesses:
+    global load / store out of range, misaligned global load, shared load out of the window, cp.async from a bad
+    source - and leave the violation counter as it found it.  Runs in a child process with FTLM_CHECKED=1."""
+    import os
+    import subprocess
+    import sys
+    from paper_2605_26261_b200 import build
+    build.build(checked=True)
+    code = ("import torch; torch.cuda.init(); from paper_2605_26261_b200 import ftlm; "
+            "print(ftlm.ftlm_check_selftest(), ftlm.ftlm_check_info()['check_violations'], ftlm.ftlm_version())")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    p = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, FTLM_CHECKED="1"),
+                       capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0, p.stderr[-2000:]
+    caught, left, version = p.stdout.strip().splitlines()[-1].split(None, 2)
+    assert int(caught) == 5 and int(left) == 0 and "CHECKED" in version, p.stdout
 
 
 # ---------------------------------------------------------------- index maps (bit-exact)
@@ -313,33 +334,7 @@ def test_thermodynamics_ring12_all_sectors_vs_oracle(mode, prec):
     assert _max_rel(got["E"], ref["E"]) <= tol
 
 
-# ---------------------------------------------------------------- TILE kernel: low-bit splits
-
-@pytest.mark.parametrize("prec", ["fp32", "fp64"])
-@pytest.mark.parametrize("mode", ["clt", "cr"])
-@pytest.mark.parametrize("w_bits", [6, 9, 12, 14, 15])
-def test_tile_kernel_low_bit_splits(prec, mode, w_bits):
-    # every ll / hh / mixed classification of the same bonds must give the same H.v and indices
-    rng = np.random.default_rng(w_bits)
-    w = W.triangular(4, 5)                       # N = 20, 60 bonds
-    J = rng.uniform(0.5, 1.5, w.n_bonds)
-    n_up = 9
-    basis = co.enumerate_basis(w.N, n_up)
-    v = rng.standard_normal(basis.shape[0]).astype(NDT[prec])
-    ref = co.apply_rows(w.N, w.bond_i, w.bond_j, J, 0.21, n_up, basis, v.astype(np.float64))
-    with Ctx(w, n_up, mode, prec, h=0.21, J=J) as c:
-        try:
-            ftlm.ftlm_set_option(c.ctx, "low_bits", w_bits)
-        except ftlm.FtlmError as e:
-            if e.code == ftlm.EUNSUPPORTED:
-                pytest.skip("split does not fit shared memory")
-            raise
-        ftlm.ftlm_set_option(c.ctx, "kernel", ftlm.KERNEL_TILE)
-        assert relerr(c.apply(v), ref) <= HV_TOL[prec]
-        got = c.neighbors(1000, 3000)
-        exp = co.neighbors_rows(w.N, w.bond_i, w.bond_j, basis, np.arange(1000, 4000))
-        assert (got == exp).all()
-
+# ---------------------------------------------------------------- TML kernel: label splits
 
 @pytest.mark.parametrize("prec", ["fp32", "fp64"])
 @pytest.mark.parametrize("mode", ["clt", "cr"])
@@ -388,8 +383,8 @@ def test_tml_lanczos_is_bit_reproducible_and_matches_row():
     assert abs(outs[0]["theta"][0, 0] - outs[2]["theta"][0, 0]) < 1e-9
 
 
-def test_tile_and_row_kernels_agree_on_config3_slice_fp32():
-    # 4x7 triangular lattice (N = 28, D = 40 116 600): ROW vs TILE on the whole vector, and both
+def test_tml_and_row_kernels_agree_on_config3_slice_fp32():
+    # 4x7 triangular lattice (N = 28, D = 40 116 600): ROW vs TML on the whole vector, and both
     # against the oracle on a slice of rows
     w = W.baseline_config(3)
     n_up = 14
@@ -398,7 +393,7 @@ def test_tile_and_row_kernels_agree_on_config3_slice_fp32():
     for mode in ("clt", "cr"):
         with Ctx(w, n_up, mode, "fp32") as c:
             v = c.fill_random(W.SEED_VECTORS, 0)
-            for kern in (ftlm.KERNEL_ROW, ftlm.KERNEL_TILE, ftlm.KERNEL_TML):
+            for kern in (ftlm.KERNEL_ROW, ftlm.KERNEL_TML):
                 ftlm.ftlm_set_option(c.ctx, "kernel", kern)
                 y = torch.empty_like(v)
                 ftlm.ftlm_apply_H(c.ctx, v, y)
