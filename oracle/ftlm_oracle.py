@@ -247,6 +247,24 @@ def apply_H(basis, N, bond_i, bond_j, J, h, N_up, v) -> np.ndarray:
     return y
 
 
+def apply_H_sampled_rows(N, bond_i, bond_j, J, h, N_up, rows, v_of) -> np.ndarray:
+    """Rows `rows` of y = H v (the same Eq. 12) for a sector too large to enumerate (config 5:
+    D = 2.33e9): the label of row t comes from the inverse map (L136), the index of every flipped label from
+    Algorithm 1 (L138-L144), and the input vector is a callable `v_of(indices) -> values` (e.g. the counter-based
+    start vector of DESIGN.md section 4, which has random access).  No basis array, no search.
+    Pinned in tests/test_oracle_hamiltonian.py against `apply_H` on every row of small sectors."""
+    rows = np.asarray(rows, dtype=np.int64)
+    _, Dc = cr_tables(N)
+    lab = alg1_unrank_vec(rows.astype(np.uint64), N, N_up, Dc)
+    y = diagonal(lab, N, bond_i, bond_j, J, h, N_up) * np.asarray(v_of(rows), dtype=np.float64)
+    for b in range(len(J)):
+        i, j = int(bond_i[b]), int(bond_j[b])
+        anti = ((lab >> np.uint64(i)) & np.uint64(1)) != ((lab >> np.uint64(j)) & np.uint64(1))
+        src = alg1_rank_vec(lab[anti] ^ np.uint64((1 << i) | (1 << j)), N, N_up, Dc)
+        y[anti] += 0.5 * J[b] * np.asarray(v_of(src), dtype=np.float64)
+    return y
+
+
 def neighbor_indices(basis, bond_i, bond_j, rows) -> np.ndarray:
     """Source index per (row, bond): index of the flipped label, -1 where the bond's spins
     are parallel (no off-diagonal element).  Used for the bit-exact neighbour check."""

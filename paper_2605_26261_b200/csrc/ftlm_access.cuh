@@ -91,14 +91,21 @@ static inline bool ftlm_emu_aligned(const void* p, size_t align, int line, const
   }
   return true;
 }
+// shared-memory accesses also feed the emulation's race detector (cuda_emu::smem_access: per-word last writer /
+// reader and the barrier epochs they were made in; two accesses of different threads to one word, one of them a
+// write, with no __syncthreads / __syncwarp between them abort the run)
 #define FTLM_G_OK(p, T, line) ftlm_emu_aligned((const void*)(p), alignof(T), (line), "global access")
-#define FTLM_S_OK(p, T, line) ftlm_emu_aligned((const void*)(p), alignof(T), (line), "shared access")
-#define FTLM_A_OK(p, T, line) ftlm_emu_aligned((const void*)(p), alignof(T), (line), "access")
+#define FTLM_S_OK(p, T, line) (ftlm_emu_aligned((const void*)(p), alignof(T), (line), "shared access") && cuda_emu::smem_access((const void*)(p), sizeof(T), false, FTLM_TU, (line)))
+#define FTLM_SW_OK(p, T, line) (ftlm_emu_aligned((const void*)(p), alignof(T), (line), "shared access") && cuda_emu::smem_access((const void*)(p), sizeof(T), true, FTLM_TU, (line)))
+#define FTLM_A_OK(p, T, line) (ftlm_emu_aligned((const void*)(p), alignof(T), (line), "access") && cuda_emu::smem_access((const void*)(p), sizeof(T), false, FTLM_TU, (line)))
 
 #else
 #define FTLM_G_OK(p, T, line) true
 #define FTLM_S_OK(p, T, line) true
 #define FTLM_A_OK(p, T, line) true
+#endif
+#ifndef FTLM_SW_OK
+#define FTLM_SW_OK(p, T, line) FTLM_S_OK(p, T, line)      /* shared-memory WRITE (the emulation's race detector tells them apart) */
 #endif
 
 #ifdef __CUDACC__
@@ -109,7 +116,7 @@ template <typename T> __device__ __forceinline__ T ldcs(const T* p, int line) { 
 template <typename T, typename U> __device__ __forceinline__ void st_g(T* p, const U& v, int line) { if (FTLM_G_OK(p, T, line)) *p = (T)v; }
 template <typename T, typename U> __device__ __forceinline__ void stcs(T* p, const U& v, int line) { if (FTLM_G_OK(p, T, line)) __stcs(p, (T)v); }
 template <typename T> __device__ __forceinline__ T ld_s(const T* p, int line) { if (!FTLM_S_OK(p, T, line)) return T{}; return *p; }
-template <typename T, typename U> __device__ __forceinline__ void st_s(T* p, const U& v, int line) { if (FTLM_S_OK(p, T, line)) *p = (T)v; }
+template <typename T, typename U> __device__ __forceinline__ void st_s(T* p, const U& v, int line) { if (FTLM_SW_OK(p, T, line)) *p = (T)v; }
 template <typename T> __device__ __forceinline__ T ld_a(const T* p, int line) { if (!FTLM_A_OK(p, T, line)) return T{}; return *p; }
 template <typename T> __device__ __forceinline__ T atom_add_g(T* p, T v, int line) { if (!FTLM_G_OK(p, T, line)) return T{}; return atomicAdd(p, v); }
 }  // namespace fa

@@ -183,7 +183,7 @@ __device__ __forceinline__ int ffs_(uint64_t x) { return __ffsll((long long)x); 
 // asynchronous global -> shared copy of one element (LDGSTS); the emulation copies at once
 template <typename T>
 __device__ __forceinline__ void cp_async_elem_(T* smem_dst, const T* gsrc, int line) {
-  if (!FTLM_S_OK(smem_dst, T, line) || !FTLM_G_OK(gsrc, T, line)) return;
+  if (!FTLM_SW_OK(smem_dst, T, line) || !FTLM_G_OK(gsrc, T, line)) return;
 #ifdef FTLM_EMU
   cuda_emu::cp_async_issue(smem_dst, gsrc, sizeof(T));
 #else

@@ -248,7 +248,9 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
         if (k < XK && x < nx) cp_async_elem(&dst[x], &src[x]);
       }
     }
+#if !defined(FTLM_NEG_TEST) || FTLM_NEG_TEST != 1     // (negative test of the host emulation: tests/emu/build_emu.py)
     cp_async_wait_all();
+#endif
     __syncthreads();
     // ---- phase 2: one warp per window word; y of PASSB_PF words is requested before the first is used ---
     double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;

@@ -435,7 +435,9 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) sumJ += __shfl_xor_sync(0xffffffffu, sumJ, o);
       const R dcoef = p.diag_coef - sumJ;
+#if !defined(FTLM_NEG_TEST) || FTLM_NEG_TEST != 2     // (negative test of the host emulation: tests/emu/build_emu.py)
       __syncwarp();
+#endif
       const int nFS4 = (nFS + 3) & ~3, nFG4 = (nFG + 3) & ~3;
       // ---- rows ------------------------------------------------------------------------------------
       const unsigned char* vsb = vsb0 + (size_t)cb * RB;                  // column base (bytes)

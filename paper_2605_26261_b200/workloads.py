@@ -184,7 +184,8 @@ def fold_order(n: int):
 
 
 def baseline_config(k: int) -> Workload:
-    """The five BASELINE.json configs, k = 1..5 (k = 40 is config 4's random-bond variant)."""
+    """The five BASELINE.json configs, k = 1..5 (k = 40 is config 4's random-bond variant, k = 41 config 4 in the
+    lexicographic site numbering of `icosidodecahedron()` instead of CONFIG4_SITE_ORDER)."""
     if k == 1:
         return ring(16, R=20, n_steps=60, note="N=16 ring, all S^z sectors, FP64+FP32")
     if k == 2:
@@ -200,6 +201,10 @@ def baseline_config(k: int) -> Workload:
         w = relabel(icosidodecahedron(True, R=10, n_steps=100, note="icosidodecahedron random J_b"),
                     CONFIG4_SITE_ORDER)
         w.name = "icosidodecahedron_randJ"
+        return w
+    if k == 41:
+        w = icosidodecahedron(False, R=10, n_steps=100, note="icosidodecahedron S^z=0, lexicographic site numbering")
+        w.name = "icosidodecahedron_lex"
         return w
     if k == 5:
         w = relabel(ring(34, 1.0, 0.5, sectors=[17], R=2, n_steps=80, note="N=34 J1-J2 ring S^z=0, CR only"),

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2605_26261_b200", "csrc")
 SO = os.path.join(HERE, "libftlm_emu.so")
 CXX = os.environ.get("CXX", "g++")
-FLAGS = ["-std=c++17", "-O1", "-g", "-fPIC", "-DFTLM_EMU", "-I", HERE, "-Wno-attributes", "-Wno-unknown-pragmas"]
+FLAGS = ["-std=c++17", "-O1", "-g", "-fPIC", "-pthread", "-DFTLM_EMU", "-I", HERE, "-Wno-attributes", "-Wno-unknown-pragmas"]
 
 
 def deps():
@@ -36,8 +36,29 @@ def build(force: bool = False) -> str:
     for p, cmd in procs:
         if p.wait() != 0:
             raise RuntimeError("emu compile failed: " + " ".join(cmd))
-    subprocess.check_call([CXX, "-shared", *objs, "-o", SO])
+    subprocess.check_call([CXX, "-shared", "-pthread", *objs, "-o", SO])
     return SO
+
+
+def build_negative(k: int) -> str:
+    """A deliberately broken copy of the library for the negative tests of the emulation itself: -DFTLM_NEG_TEST=k
+    removes one synchronisation from one kernel (1: the cp.async wait of PASS-B's staging phase, ftlm_passb.cu;
+    2: the __syncwarp between building and reading the per-column descriptor lists, ftlm_tml.cu).  A run through it
+    must be killed by the emulation (tests/test_emu_kernels.py::test_emu_detects_removed_synchronisation)."""
+    build()
+    so = os.path.join(HERE, f"libftlm_emu_neg{k}.so")
+    victim = {1: "ftlm_passb.cu", 2: "ftlm_tml.cu"}[k]
+    if os.path.exists(so) and all(os.path.getmtime(d) <= os.path.getmtime(so) for d in deps()):
+        return so
+    objs = []
+    for src in sorted(glob.glob(os.path.join(CSRC, "*.cu"))) + [os.path.join(HERE, "cuda_emu.cpp")]:
+        obj = os.path.join(HERE, os.path.basename(src) + ".emu.o")
+        if os.path.basename(src) == victim:
+            obj = os.path.join(HERE, os.path.basename(src) + f".neg{k}.emu.o")
+            subprocess.check_call([CXX, *FLAGS, f"-DFTLM_NEG_TEST={k}", "-x", "c++", "-c", src, "-o", obj])
+        objs.append(obj)
+    subprocess.check_call([CXX, "-shared", "-pthread", *objs, "-o", so])
+    return so
 
 
 if __name__ == "__main__":

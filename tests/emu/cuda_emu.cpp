@@ -7,11 +7,14 @@
 #include <ucontext.h>
 #include <unistd.h>
 
+#include <atomic>
 #include <map>
+#include <mutex>
+#include <thread>
 #include <vector>
 
-uint3 threadIdx, blockIdx;
-dim3 blockDim, gridDim;
+thread_local uint3 threadIdx, blockIdx;
+thread_local dim3 blockDim, gridDim;
 
 namespace {
 
@@ -24,6 +27,7 @@ namespace {
 // ---- guarded allocations: [PROT_NONE page][slack ... data (16-byte aligned, ends at page end)][PROT_NONE page]
 struct Alloc { void* map; size_t map_bytes; };
 std::map<void*, Alloc> g_allocs;
+std::mutex g_alloc_mu;
 const size_t PAGE = 4096;
 
 void* guarded_alloc(size_t bytes) {
@@ -38,10 +42,12 @@ void* guarded_alloc(size_t bytes) {
   char* p = front ? m + PAGE : m + PAGE + body - data;   // data flush against the trailing (default) or the leading guard page
   memset(m + PAGE, 0xCD, body);             // slack: poison
   memset(p, 0xA5, data);                    // uninitialised device memory is not zero
+  std::lock_guard<std::mutex> lk(g_alloc_mu);
   g_allocs[p] = Alloc{m, total};
   return p;
 }
 void guarded_free(void* p) {
+  std::lock_guard<std::mutex> lk(g_alloc_mu);
   auto it = g_allocs.find(p);
   if (it == g_allocs.end()) die("cudaFree of an unknown pointer");
   munmap(it->second.map, it->second.map_bytes);
@@ -52,32 +58,43 @@ void guarded_free(void* p) {
 struct PendingCopy { void* dst; size_t bytes; unsigned char data[16]; };
 struct Fiber { ucontext_t ctx; char* stack = nullptr; bool done = false; bool started = false; std::vector<PendingCopy> pending; };
 const size_t STACK = 64 * 1024;
-std::vector<Fiber> g_fib;
-std::vector<char*> g_stack_pool;
-ucontext_t g_main;
-int g_cur = -1;
-unsigned g_nthreads = 0;
-unsigned long long g_progress = 0;
-const std::function<void()>* g_body = nullptr;
-unsigned char* g_dyn = nullptr;
+// scheduler state of the CTA in flight on this host thread
+thread_local std::vector<Fiber> g_fib;
+thread_local std::vector<char*> g_stack_pool;
+std::vector<std::vector<char*>> g_free_stack_sets;       // fiber stacks outlive the short-lived host threads of a launch
+std::mutex g_stack_mu;
+thread_local ucontext_t g_main;
+thread_local int g_cur = -1;
+thread_local unsigned g_nthreads = 0;
+thread_local unsigned long long g_progress = 0;
+thread_local const std::function<void()>* g_body = nullptr;
+thread_local unsigned char* g_dyn = nullptr;
+thread_local size_t g_dyn_bytes = 0;
 
 // CTA barrier
-unsigned g_bar_arrived = 0, g_bar_gen = 0, g_alive = 0;
+thread_local unsigned g_bar_arrived = 0, g_bar_gen = 0, g_alive = 0;
+
+// race detector: per 4-byte word of the dynamic shared memory, the last write and the last read
+struct Access { int tid; unsigned bar, wgen; int tu, line; };
+struct Shadow { Access w, r; };
+thread_local std::vector<Shadow> g_shadow;
+bool race_on() { static const bool on = !(getenv("FTLM_EMU_RACE") && !strcmp(getenv("FTLM_EMU_RACE"), "0")); return on; }
 
 struct Warp {
   uint64_t val[32], out[32];
   int arg[32];
   unsigned arrived_mask = 0, gen = 0, alive_mask = 0, want_mask = 0;
+  unsigned sync_gen = 0;       // completed __syncwarp()s of every live lane (memory ordering inside the warp)
   int op = -1;
 };
-std::vector<Warp> g_warps;
+thread_local std::vector<Warp> g_warps;
 
 void yield_to_scheduler() { swapcontext(&g_fib[(size_t)g_cur].ctx, &g_main); }
 
 void complete_collective(Warp& w) {
   const unsigned part = w.arrived_mask;
   switch (w.op) {
-    case cuda_emu::OP_SYNCWARP: break;
+    case cuda_emu::OP_SYNCWARP: if (part == w.alive_mask) w.sync_gen++; break;   // shuffles and ballots order nothing
     case cuda_emu::OP_BALLOT: {
       unsigned b = 0;
       for (int l = 0; l < 32; ++l) if ((part >> l) & 1u) b |= (w.val[l] ? 1u : 0u) << l;
@@ -136,11 +153,13 @@ void run_block() {
     g_warps[i >> 5].alive_mask |= 1u << (i & 31);
   }
   g_alive = nt; g_bar_arrived = 0; g_bar_gen = 0;
+  if (race_on()) g_shadow.assign((g_dyn_bytes + 3) / 4, Shadow{Access{-1, 0, 0, 0, 0}, Access{-1, 0, 0, 0, 0}});
+  else g_shadow.clear();
   // FTLM_EMU_ORDER: order in which runnable threads are resumed in every scheduling round - 0 ascending
   // (default), 1 descending, n >= 2 a fresh pseudo-random permutation per round (seed n).  A kernel whose
   // result depends on this order has a race (missing __syncthreads / __syncwarp); the tests run all three.
   static const int order_mode = getenv("FTLM_EMU_ORDER") ? atoi(getenv("FTLM_EMU_ORDER")) : 0;
-  static unsigned long long rng = 0x9E3779B97F4A7C15ull * (unsigned long long)(order_mode + 1);
+  thread_local unsigned long long rng = 0x9E3779B97F4A7C15ull * (unsigned long long)(order_mode + 1);
   std::vector<unsigned> order(nt);
   for (unsigned i = 0; i < nt; ++i) order[i] = order_mode == 1 ? nt - 1 - i : i;
   for (;;) {
@@ -189,8 +208,39 @@ void cp_async_issue(void* smem_dst, const void* gsrc, size_t bytes) {
 void cp_async_wait_all() {
   if (g_cur < 0) die("cp.async.wait_all outside a kernel");
   Fiber& f = g_fib[(size_t)g_cur];
-  for (const PendingCopy& c : f.pending) memcpy(c.dst, c.data, c.bytes);
+  for (const PendingCopy& c : f.pending) { smem_access(c.dst, c.bytes, true, 0, 0); memcpy(c.dst, c.data, c.bytes); }
   f.pending.clear();
+}
+
+bool smem_access(const void* p, size_t bytes, bool write, int tu, int line) {
+  if (g_cur < 0 || g_shadow.empty()) return true;
+  const unsigned char* a = (const unsigned char*)p;
+  if (a < g_dyn || a >= g_dyn + g_dyn_bytes) return true;            // static __shared__ variables, global memory
+  const int t = g_cur;
+  const unsigned bar = g_bar_gen, wgen = g_warps[(size_t)t >> 5].sync_gen;
+  auto ordered = [&](const Access& x) {
+    if (x.tid < 0 || x.tid == t) return true;
+    if (x.bar != bar) return true;                                    // a __syncthreads completed in between
+    return (x.tid >> 5) == (t >> 5) && x.wgen != wgen;                // same warp and a __syncwarp in between
+  };
+  const size_t w0 = (size_t)(a - g_dyn) / 4, w1 = ((size_t)(a - g_dyn) + bytes - 1) / 4;
+  for (size_t k = w0; k <= w1 && k < g_shadow.size(); ++k) {
+    Shadow& sh = g_shadow[k];
+    const Access* bad = nullptr;
+    const char* kind = "";
+    if (!ordered(sh.w)) { bad = &sh.w; kind = write ? "write after write" : "read after write"; }
+    else if (write && !ordered(sh.r)) { bad = &sh.r; kind = "write after read"; }
+    if (bad) {
+      fprintf(stderr, "cuda_emu: shared-memory race (%s) on dynamic smem byte %zu: thread %d (tu %d line %d) and thread %d (tu %d line %d) "
+              "with no __syncthreads%s between them (block %u)\n", kind, k * 4, bad->tid, bad->tu, bad->line, t, tu, line,
+              (bad->tid >> 5) == (t >> 5) ? " / __syncwarp" : "", blockIdx.x);
+      fflush(stderr);
+      abort();
+    }
+    if (write) { sh.w = Access{t, bar, wgen, tu, line}; sh.r.tid = -1; }
+    else sh.r = Access{t, bar, wgen, tu, line};
+  }
+  return true;
 }
 
 void sync_threads() {
@@ -222,17 +272,39 @@ void launch(unsigned grid, unsigned block, size_t dyn_bytes, const std::function
   if (g_cur >= 0) die("nested launch");
   if (grid == 0 || block == 0 || block > 1024) { g_last = cudaErrorInvalidValue; return; }
   if (dyn_bytes > 227 * 1024) { g_last = cudaErrorInvalidValue; return; }
-  g_body = &body;
-  g_nthreads = block;
-  gridDim = dim3(grid); blockDim = dim3(block);
-  for (unsigned b = 0; b < grid; ++b) {
-    blockIdx.x = b; blockIdx.y = 0; blockIdx.z = 0;
-    g_dyn = dyn_bytes ? (unsigned char*)guarded_alloc(dyn_bytes) : nullptr;
-    run_block();
-    if (g_dyn) guarded_free(g_dyn);
-    g_dyn = nullptr;
-  }
-  g_body = nullptr;
+  // CTAs are taken from a shared counter by a few host threads and run concurrently (one CTA in flight per host
+  // thread, its CUDA threads as fibers on that thread)
+  static const unsigned max_workers = getenv("FTLM_EMU_CTAS") ? (unsigned)std::max(1, atoi(getenv("FTLM_EMU_CTAS"))) : 4u;
+  std::atomic<unsigned> next{0};
+  auto worker = [&]() {
+    {
+      std::lock_guard<std::mutex> lk(g_stack_mu);
+      if (g_stack_pool.empty() && !g_free_stack_sets.empty()) { g_stack_pool.swap(g_free_stack_sets.back()); g_free_stack_sets.pop_back(); }
+    }
+    g_body = &body;
+    g_nthreads = block;
+    gridDim = dim3(grid); blockDim = dim3(block);
+    for (;;) {
+      const unsigned b = next.fetch_add(1);
+      if (b >= grid) break;
+      blockIdx.x = b; blockIdx.y = 0; blockIdx.z = 0;
+      g_dyn = dyn_bytes ? (unsigned char*)guarded_alloc(dyn_bytes) : nullptr;
+      g_dyn_bytes = dyn_bytes;
+      run_block();
+      if (g_dyn) guarded_free(g_dyn);
+      g_dyn = nullptr; g_dyn_bytes = 0;
+    }
+    g_body = nullptr;
+    g_fib.clear(); g_warps.clear(); g_shadow.clear();
+    std::lock_guard<std::mutex> lk(g_stack_mu);
+    g_free_stack_sets.emplace_back();
+    g_free_stack_sets.back().swap(g_stack_pool);
+  };
+  const unsigned nw = std::min(grid, max_workers);
+  if (nw <= 1) { worker(); return; }
+  std::vector<std::thread> pool;
+  for (unsigned k = 0; k < nw; ++k) pool.emplace_back(worker);
+  for (std::thread& th : pool) th.join();
 }
 
 }  // namespace cuda_emu

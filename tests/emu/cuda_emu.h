@@ -4,8 +4,13 @@
 // a fiber (ucontext), __syncthreads / __syncwarp / __ballot_sync / __shfl_*_sync are real rendezvous
 // points, "device" memory is guarded host memory (a PROT_NONE page directly behind every allocation
 // and behind the dynamic shared memory, so reads or writes past the end fault instead of passing).
-// CTAs of a grid run one after another (nothing inter-CTA - the atomic tile / item hand-out with several CTAs in
-// flight, the last-CTA ticket - is exercised concurrently: that is left to the checked build on the device).
+// The CTAs of a grid run CONCURRENTLY on a few host threads (FTLM_EMU_CTAS, default 4; each CTA's fibers stay on one
+// host thread), taken from a shared counter like a hardware scheduler would: the atomic tile / item hand-out, the
+// last-CTA ticket and the counter reset of the persistent kernels really race; atomics are real atomics.
+// Shared-memory race detector: every access made through the LD_S / ST_S / cp_async macros of csrc/ftlm_access.cuh
+// is recorded per 4-byte word (last writer, last reader, the __syncthreads / __syncwarp epochs they were made in);
+// two accesses to one word by different threads, at least one a write, with no barrier between them abort the run
+// (FTLM_EMU_RACE=0 turns the detector off).
 // FTLM_EMU_ALIGN=front places every allocation flush against its FRONT guard page instead of the back one, so
 // that underruns fault too (the suite is run both ways).  This is a checker for index arithmetic, table construction,
 // barrier placement, cp.async waits, alignment and bounds - it is never loaded by the product binding and has no performance
@@ -26,7 +31,7 @@
 #define __launch_bounds__(...)
 #define __grid_constant__
 #define __align__(n) __attribute__((aligned(n)))
-#define __shared__ static
+#define __shared__ static thread_local      // one copy per host thread = per CTA in flight
 #ifndef __CUDACC__
 #define __CUDACC__ 1          // ftlm_common.cuh guards its device helpers with this
 #endif
@@ -46,8 +51,8 @@ static inline float4 make_float4(float a, float b, float c, float d) { return fl
 static inline double2 make_double2(double a, double b) { return double2{a, b}; }
 static inline int2 make_int2(int a, int b) { return int2{a, b}; }
 
-extern uint3 threadIdx, blockIdx;
-extern dim3 blockDim, gridDim;
+extern thread_local uint3 threadIdx, blockIdx;
+extern thread_local dim3 blockDim, gridDim;
 
 // ---- runtime API subset ------------------------------------------------------------------------
 typedef int cudaError_t;
@@ -97,6 +102,8 @@ uint64_t collective(int op, unsigned mask, uint64_t v, int arg);
 // A consumer that reads before the producer's wait + barrier therefore sees NaN instead of passing by luck.
 void cp_async_issue(void* smem_dst, const void* gsrc, size_t bytes);
 void cp_async_wait_all();
+// race detector hook (always returns true); a pointer outside the CTA's dynamic shared memory is ignored
+bool smem_access(const void* p, size_t bytes, bool write, int tu, int line);
 enum { OP_SYNCWARP = 0, OP_BALLOT = 1, OP_SHFL_DOWN = 2, OP_SHFL_XOR = 3, OP_SHFL_IDX = 4, OP_SHFL_UP = 5 };
 template <typename T> static inline uint64_t pack(T v) { uint64_t u = 0; static_assert(sizeof(T) <= 8, "shfl payload"); memcpy(&u, &v, sizeof(T)); return u; }
 template <typename T> static inline T unpack(uint64_t u) { T v; memcpy(&v, &u, sizeof(T)); return v; }
@@ -114,8 +121,8 @@ template <typename T> static inline T __shfl_down_sync(unsigned mask, T v, int d
 template <typename T> static inline T __shfl_up_sync(unsigned mask, T v, int d) { return cuda_emu::unpack<T>(cuda_emu::collective(cuda_emu::OP_SHFL_UP, mask, cuda_emu::pack(v), d)); }
 template <typename T> static inline T __shfl_xor_sync(unsigned mask, T v, int d) { return cuda_emu::unpack<T>(cuda_emu::collective(cuda_emu::OP_SHFL_XOR, mask, cuda_emu::pack(v), d)); }
 template <typename T> static inline T __shfl_sync(unsigned mask, T v, int src) { return cuda_emu::unpack<T>(cuda_emu::collective(cuda_emu::OP_SHFL_IDX, mask, cuda_emu::pack(v), src)); }
-static inline void __threadfence() {}
-static inline void __threadfence_block() {}
+static inline void __threadfence() { __atomic_thread_fence(__ATOMIC_SEQ_CST); }
+static inline void __threadfence_block() { __atomic_thread_fence(__ATOMIC_SEQ_CST); }
 static inline int __popc(unsigned x) { return __builtin_popcount(x); }
 static inline int __popcll(unsigned long long x) { return __builtin_popcountll(x); }
 static inline int __ffs(int x) { return __builtin_ffs(x); }
@@ -128,8 +135,16 @@ template <typename T> static inline T __ldcs(const T* p) { return *p; }
 template <typename T> static inline T __ldcg(const T* p) { return *p; }
 template <typename T> static inline void __stcs(T* p, const T& v) { *p = v; }
 template <typename T> static inline void __stcg(T* p, const T& v) { *p = v; }
-static inline unsigned atomicAdd(unsigned* p, unsigned v) { unsigned o = *p; *p = o + v; return o; }
-static inline int atomicAdd(int* p, int v) { int o = *p; *p = o + v; return o; }
-static inline unsigned long long atomicAdd(unsigned long long* p, unsigned long long v) { unsigned long long o = *p; *p = o + v; return o; }
-static inline double atomicAdd(double* p, double v) { double o = *p; *p = o + v; return o; }
-static inline float atomicAdd(float* p, float v) { float o = *p; *p = o + v; return o; }
+static inline unsigned atomicAdd(unsigned* p, unsigned v) { return __atomic_fetch_add(p, v, __ATOMIC_SEQ_CST); }
+static inline int atomicAdd(int* p, int v) { return __atomic_fetch_add(p, v, __ATOMIC_SEQ_CST); }
+static inline unsigned long long atomicAdd(unsigned long long* p, unsigned long long v) { return __atomic_fetch_add(p, v, __ATOMIC_SEQ_CST); }
+static inline double atomicAdd(double* p, double v) {
+  uint64_t o, n;
+  __atomic_load((uint64_t*)p, &o, __ATOMIC_SEQ_CST);
+  for (;;) { double d; memcpy(&d, &o, 8); d += v; memcpy(&n, &d, 8); if (__atomic_compare_exchange((uint64_t*)p, &o, &n, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST)) { memcpy(&d, &o, 8); return d; } }
+}
+static inline float atomicAdd(float* p, float v) {
+  uint32_t o, n;
+  __atomic_load((uint32_t*)p, &o, __ATOMIC_SEQ_CST);
+  for (;;) { float d; memcpy(&d, &o, 4); d += v; memcpy(&n, &d, 4); if (__atomic_compare_exchange((uint32_t*)p, &o, &n, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST)) { memcpy(&d, &o, 4); return d; } }
+}

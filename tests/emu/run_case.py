@@ -24,6 +24,8 @@ sys.path.insert(0, HERE)
 from oracle import ftlm_oracle as fo  # noqa: E402
 from paper_2605_26261_b200 import workloads as W  # noqa: E402
 import emu_harness as E  # noqa: E402
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+from hv_bound import elem_bound  # noqa: E402
 
 
 def workload(name):
@@ -91,7 +93,10 @@ def main():
             den = np.linalg.norm(ref)
             err = float(np.linalg.norm(y.astype(np.float64) - ref) / (den if den > 0 else 1.0))
             res["hv_relerr"] = err
-            res["ok"] = res["ok"] and bool(np.isfinite(y).all()) and err <= (1e-5 if prec == "fp32" else 1e-12)
+            res["hv_maxabs"] = float(np.max(np.abs(y.astype(np.float64) - ref))) if D else 0.0
+            res["hv_elem_bound"] = elem_bound(v, w.J, h, w.N, prec)       # element-wise criterion beside the norm
+            res["ok"] = (res["ok"] and bool(np.isfinite(y).all()) and err <= (1e-5 if prec == "fp32" else 1e-12)
+                         and res["hv_maxabs"] <= res["hv_elem_bound"])
         if "lanczos" in what:
             m = min(spec.get("steps", 12), D)
             out = c.lanczos(W.SEED_VECTORS, 1, m)
@@ -100,9 +105,12 @@ def main():
             k = min(int(out["m_eff"][0]), len(a), 8)
             tol = 1e-9 if prec == "fp64" else 2e-4
             da = float(np.max(np.abs(out["alpha"][0][:k] - np.asarray(a)[:k]))) if k else 0.0
-            res["lanczos_dalpha"] = da
+            kb = max(k - 1, 0)
+            db = float(np.max(np.abs(out["beta"][0][:kb] - np.asarray(b)[:kb]))) if kb else 0.0
+            res["lanczos_dalpha"], res["lanczos_dbeta"] = da, db
             res["m_eff"] = int(out["m_eff"][0])
-            res["ok"] = res["ok"] and da <= tol
+            res["ok"] = res["ok"] and da <= tol and db <= tol
+    res["ok"] = bool(res["ok"])
     print(json.dumps(res))
 
 

@@ -22,7 +22,7 @@ from oracle import c_oracle as co  # noqa: E402
 from oracle import ftlm_oracle as fo  # noqa: E402
 from paper_2605_26261_b200 import ftlm  # noqa: E402
 from paper_2605_26261_b200 import workloads as W  # noqa: E402
-from gpu_util import MODES, NDT, PRECS, TDT  # noqa: E402
+from gpu_util import MODES, NDT, PRECS, TDT, elem_bound  # noqa: E402
 
 
 def workload(spec):
@@ -101,28 +101,41 @@ def main():
             n = 1 << 16
             starts = [0, D - n] + [int(x) for x in rng.integers(0, D - n, spec.get("blocks", 6))]
             ranges = [(s, n) for s in starts]
-        err2 = ref2 = 0.0
+        err2 = ref2 = worst = 0.0
         for r0, n in ranges:
             ref = co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, v64, r0, n)
             err2 += float(np.sum((y[r0:r0 + n] - ref) ** 2))
             ref2 += float(np.sum(ref ** 2))
+            worst = max(worst, float(np.max(np.abs(y[r0:r0 + n] - ref))) if n else 0.0)
         res["hv_relerr"] = (err2 / ref2) ** 0.5 if ref2 > 0 else 0.0
-        res["ok"] = res["ok"] and res["finite"] and res["hv_relerr"] <= tol
+        res["hv_maxabs"], res["hv_elem_bound"] = worst, elem_bound(v, w.J, 0.0, w.N, prec)   # element-wise criterion beside the norm
+        res["ok"] = res["ok"] and res["finite"] and res["hv_relerr"] <= tol and worst <= res["hv_elem_bound"]
     if "lanczos" in what:
         m = min(spec.get("steps", 8), D)
         out = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, 1, m)
         q1 = fo.start_vector(W.SEED_VECTORS, n_up, 0, D)
         a, b = co.lanczos(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, q1, m)[:2]
         k = min(int(out["m_eff"][0]), len(a), 6)
+        ltol = 1e-9 if prec == "fp64" else 2e-4
         da = float(np.max(np.abs(out["alpha"][0][:k] - np.asarray(a)[:k]))) if k else 0.0
-        res["lanczos_dalpha"] = da
+        kb = max(k - 1, 0)
+        db = float(np.max(np.abs(out["beta"][0][:kb] - np.asarray(b)[:kb]))) if kb else 0.0
+        res["lanczos_dalpha"], res["lanczos_dbeta"] = da, db
         res["m_eff"] = int(out["m_eff"][0])
-        res["ok"] = res["ok"] and da <= (1e-9 if prec == "fp64" else 2e-4) and res["m_eff"] == m
+        # extremal Ritz values of the whole run (converge first, L246) and the weight sum rule
+        th_ref, _ = fo.ritz(np.asarray(a), np.asarray(b))
+        th = out["theta"][0][: res["m_eff"]]
+        res["ritz_dmin"], res["ritz_dmax"] = float(abs(th.min() - th_ref.min())), float(abs(th.max() - th_ref.max()))
+        res["wsum"] = float(out["weight"][0][: res["m_eff"]].sum())
+        rtol = (1e-9 if prec == "fp64" else 5e-4) * max(1.0, float(np.abs(th_ref).max()))
+        res["ok"] = (res["ok"] and da <= ltol and db <= ltol and res["m_eff"] == m and res["ritz_dmin"] <= rtol
+                     and res["ritz_dmax"] <= rtol and abs(res["wsum"] - 1.0) <= 1e-6)
     ftlm.ftlm_destroy(ctx)
     chk = ftlm.ftlm_check_info()                             # checked build (FTLM_CHECKED=1): no suppressed access
     res["check"] = chk
     if ftlm.CHECKED:
         res["ok"] = res["ok"] and chk["check_build"] == 1 and chk["check_violations"] == 0
+    res["ok"] = bool(res["ok"])
     print(json.dumps(res))
 
 

@@ -3,6 +3,7 @@ import numpy as np
 import torch
 
 from paper_2605_26261_b200 import ftlm
+from hv_bound import elem_bound  # noqa: F401
 
 MODES = {"clt": ftlm.INDEX_CLT, "cr": ftlm.INDEX_CR}
 PRECS = {"fp32": ftlm.FP32, "fp64": ftlm.FP64}
@@ -65,3 +66,13 @@ def relerr(y, ref):
     y = np.asarray(y, dtype=np.float64)
     den = np.linalg.norm(ref)
     return np.linalg.norm(y - ref) / (den if den > 0 else 1.0)
+
+
+def hv_err(y, ref, v, J, h, N, prec):
+    """Norm-relative error of y against the oracle's ref (north_star's criterion, returned) after asserting the
+    element-wise bound on every row."""
+    y = np.asarray(y, dtype=np.float64)
+    worst = float(np.max(np.abs(y - ref))) if y.size else 0.0
+    bound = elem_bound(v, J, h, N, prec)
+    assert worst <= bound, f"element-wise: max|y - ref| = {worst:.3e} > {bound:.3e} at row {int(np.argmax(np.abs(y - ref)))}"
+    return relerr(y, ref)

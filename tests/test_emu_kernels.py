@@ -196,6 +196,27 @@ def test_emu_lazy_normalisation_matches_separate_pass():
         assert d[prec][0] <= 1e-12 and d[prec][1] <= 1e-12 and d[prec][2] == 6, d
 
 
+@pytest.mark.parametrize("neg,spec,expect", [
+    (1, {"wl": "ring16j", "n_up": 8, "mode": "clt", "prec": "fp32",
+         "options": [["passb", 1], ["tml_split", 5 | (3 << 8)], ["kernel", 3]], "what": ["apply"]}, "cp.async"),
+    (2, {"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp32",
+         "options": [["tml_low_bits", 6], ["tml_mid_bits", 4], ["kernel", 3]], "what": ["apply"]}, "shared-memory race"),
+])
+def test_emu_detects_removed_synchronisation(neg, spec, expect):
+    """Negative test of the checker: a copy of the library with ONE synchronisation removed (1: the cp.async wait of
+    PASS-B's staging, 2: the __syncwarp between building and reading TML's descriptor lists) must be killed by the
+    emulation - by the deferred cp.async model / the shared-memory race detector - while the intact library passes
+    the same case."""
+    import build_emu
+    assert run_case(spec)["ok"]
+    so = build_emu.build_negative(neg)
+    p = subprocess.run([sys.executable, RUN, json.dumps(spec)], capture_output=True, text=True, timeout=900,
+                       env=dict(os.environ, FTLM_EMU_LIB=so))
+    ok = p.returncode == 0 and json.loads(p.stdout.strip().splitlines()[-1])["ok"]
+    assert not ok, "the emulation did not notice the removed synchronisation"
+    assert expect in p.stderr or p.returncode == 0, p.stderr[-1500:]      # died for the expected reason (or produced wrong values)
+
+
 @pytest.mark.parametrize("order", [5])
 def test_emu_result_does_not_depend_on_thread_schedule(order):
     """The emulation resumes runnable threads in ascending order by default; descending (1) and pseudo-random (>= 2)

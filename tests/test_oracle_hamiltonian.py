@@ -95,6 +95,40 @@ def test_table1_nnz_icosahedron(golden_paper):
     assert np.count_nonzero(H - np.diag(np.diag(H))) == int(golden_paper["table1_Nnz"]) - 924
 
 
+@pytest.mark.parametrize("wl,n_up", [(W.ring(8, 1.0, 0.5), 4), (W.ring(10, 1.0, 0.5), 3), (W.icosahedron(), 6),
+                                     (W.icosahedron(), 7), (W.square(3, 4), 5), (W.triangular(3, 4), 0),
+                                     (W.triangular(3, 4), 12)])
+def test_neighbor_lists_entry_by_entry_against_brute_force_counting(wl, n_up):
+    """Pins the expected values of every bit-exact neighbour test of the CUDA path (both the numpy and the C/OpenMP
+    helper): for EVERY (row, bond), the source index is the number of sector labels below the bond-flipped label
+    (counted by brute force over all 2^N words, no search structure, no ranking formula), or -1 on a parallel bond
+    (Eq. 12-14: only antiparallel pairs have an off-diagonal element; reading 2: ascending 0-based order)."""
+    N = wl.N
+    labels = [n for n in range(1 << N) if bin(n).count("1") == n_up]
+    below = {}
+    count = 0
+    for n in range(1 << N):                         # number of sector labels strictly below n
+        below[n] = count
+        if bin(n).count("1") == n_up:
+            count += 1
+    exp = np.full((len(labels), wl.n_bonds), -1, dtype=np.int64)
+    for t, n in enumerate(labels):
+        for b in range(wl.n_bonds):
+            i, j = int(wl.bond_i[b]), int(wl.bond_j[b])
+            if ((n >> i) & 1) != ((n >> j) & 1):
+                exp[t, b] = below[n ^ (1 << i) ^ (1 << j)]
+    basis = fo.sector_basis(N, n_up)
+    assert [int(x) for x in basis] == labels
+    rows = np.arange(len(labels), dtype=np.int64)
+    got_np = fo.neighbor_indices(basis, wl.bond_i, wl.bond_j, rows)
+    got_c = co.neighbors_rows(N, wl.bond_i, wl.bond_j, co.enumerate_basis(N, n_up), rows)
+    assert (got_np == exp).all() and (got_c == exp).all()
+    # a subset of rows in scrambled order (the form the sampled N = 34 test uses)
+    pick = np.random.default_rng(5).permutation(len(labels))[: max(1, len(labels) // 3)].astype(np.int64)
+    assert (co.neighbors_rows(N, wl.bond_i, wl.bond_j, co.enumerate_basis(N, n_up), pick) == exp[pick]).all()
+    assert (fo.neighbor_indices(basis, wl.bond_i, wl.bond_j, pick) == exp[pick]).all()
+
+
 def test_sector_trace_closed_form():
     # Tr_sector H = (sum_b J_b / 4) [C(N-2,N_up-2) + C(N-2,N_up) - 2 C(N-2,N_up-1)]
     def c(n, k):
@@ -166,3 +200,35 @@ def test_config1_ground_state_energy_by_lanczos_agrees_with_dense():
     ev = np.linalg.eigvalsh(_dense(w, 6))
     assert th[0] == pytest.approx(ev[0], abs=1e-9)
     assert th[-1] <= w.J.sum() / 4 + 1e-9
+
+
+def test_config1_lowest_levels_match_survey_values(golden_paper):
+    """BASELINE config 1 at its own size: lowest two distinct Ritz values of the C oracle's Lanczos on the S^z = 0
+    sector of the N = 16 ring against the values SURVEY.md 8(c) obtained with a sparse eigensolver (not the paper's,
+    not this repository's code): pins apply_rows + lanczos + ritz at D = 12 870."""
+    w = W.ring(16)
+    basis = co.enumerate_basis(16, 8)
+    q1 = fo.start_vector(1, 8, 0, basis.shape[0])
+    a, b = co.lanczos(16, w.bond_i, w.bond_j, w.J, 0.0, 8, basis, q1, 200)
+    th, _ = fo.ritz(a, b)
+    levels = [th[0]]
+    for x in th[1:]:                                   # ghosts are (converging) copies of converged levels (L254): skip them
+        if x - levels[-1] > 1e-2:                      # the gap of this sector is 0.27
+            levels.append(x)
+    assert levels[0] == pytest.approx(float(golden_paper["survey_config1_E0"]), abs=2e-8)
+    assert levels[1] == pytest.approx(float(golden_paper["survey_config1_E1"]), abs=2e-8)
+
+
+def test_sampled_row_form_equals_full_apply_H():
+    """`apply_H_sampled_rows` (labels by unranking, sources by Algorithm 1, v through a callable; used for config 5
+    where the basis cannot be enumerated) against `apply_H` with the enumerated basis: every row of two small sectors,
+    scrambled order, random couplings and a field."""
+    rng = np.random.default_rng(11)
+    for w, n_up in ((W.ring(12, 1.0, 0.5), 6), (W.triangular(3, 4), 4), (W.icosahedron(), 7)):
+        J = rng.uniform(0.5, 1.5, w.n_bonds)
+        basis = fo.sector_basis(w.N, n_up)
+        v = rng.standard_normal(basis.shape[0])
+        ref = fo.apply_H(basis, w.N, w.bond_i, w.bond_j, J, 0.3, n_up, v)
+        rows = rng.permutation(basis.shape[0])
+        got = fo.apply_H_sampled_rows(w.N, w.bond_i, w.bond_j, J, 0.3, n_up, rows, lambda idx: v[np.asarray(idx, dtype=np.int64)])
+        assert np.abs(got - ref[rows]).max() <= 1e-13 * max(1.0, np.abs(ref).max())

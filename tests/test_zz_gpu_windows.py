@@ -56,7 +56,8 @@ def test_tmlr_in_tile_pass_matches_oracle(wl, n_up, mode, prec, opts, lazy):
 
 @pytest.mark.parametrize("cfg,mode", [(3, "clt"), (3, "cr")])
 def test_autotune_config3(cfg, mode):
-    d = run({"config": cfg, "mode": mode, "autotune": True, "what": ["sampled"], "blocks": 4})
+    d = run({"config": cfg, "mode": mode, "autotune": True, "options": [["allow_unverified", 1]],
+             "what": ["sampled"], "blocks": 4})
     assert any(r["name"].startswith("tml+passb") for r in d["autotune"]), d
 
 
@@ -65,5 +66,6 @@ def test_autotune_config3(cfg, mode):
 def test_autotune_config4_full_size_sampled_rows(mode):
     """BASELINE config 4 in the configuration bench.py times (ftlm_autotune's choice): every candidate must
     agree with the ROW kernel on the whole vector, and the chosen one with the oracle on sampled row blocks."""
-    d = run({"config": 4, "mode": mode, "autotune": True, "what": ["sampled"], "blocks": 6}, timeout=3000)
+    d = run({"config": 4, "mode": mode, "autotune": True, "options": [["allow_unverified", 1]],
+             "what": ["sampled"], "blocks": 6}, timeout=3000)
     assert d["dim"] == 155117520 and d["hv_relerr"] <= 1e-5
