@@ -154,12 +154,16 @@ CANDIDATES = {
     "tml_w9m7": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 9 | (7 << 8)), ("passb", 0), ("kernel", 3)],
     "tml_w9m7+passb": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 9 | (7 << 8)), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
 }
-SAFE_CHOICE = "tml_w9m7"     # the kernel and launch shape measured on B200 in round 1 (profiles/): fallback if the probe dies
+SAFE_CHOICE = "row"          # thread-per-row kernel: parity-green on B200 in round 1 and the on-device reference of every candidate
 
 
 def run_probe(args):
-    """Child process: ftlm_autotune on the bench sector; prints {"choice", "report"} as one JSON line.
-    Runs in its own process so that a faulting candidate cannot take the bench's CUDA context down."""
+    """Child process: ftlm_autotune on the bench sector; prints one JSON line.
+    stage "checked" (FTLM_CHECKED=1 in the environment: the binding loads libftlm_checked.so, in which every computed
+    address is range- and alignment-checked on the device and a violation is suppressed and counted, never a fault):
+    every candidate computes H.v and three fused steps and is compared on the device with the thread-per-row kernel;
+    stage "release": the candidates named by --mask (those that passed the checked stage with zero violations) are
+    timed in the release library and the fastest is chosen."""
     import torch
     from paper_2605_26261_b200 import ftlm, workloads as W
     w = W.baseline_config(args.config)
@@ -167,23 +171,57 @@ def run_probe(args):
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
     mode = ftlm.INDEX_CR if (args.mode == "cr" or w.N > 32) else ftlm.INDEX_CLT
     ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, torch.cuda.current_device())
+    ftlm.ftlm_set_option(ctx, "allow_unverified", 1)
+    if args.probe_stage == "checked":
+        assert ftlm.CHECKED, "checked probe stage needs FTLM_CHECKED=1"
+        rep = ftlm.ftlm_autotune(ctx, 1)
+        info = ftlm.ftlm_check_info()
+        ftlm.ftlm_destroy(ctx)
+        print(json.dumps({"stage": "checked", "report": rep, "check": info}), flush=True)
+        return
+    assert not ftlm.CHECKED
+    ftlm.ftlm_set_option(ctx, "autotune_mask", args.mask)
     rep = ftlm.ftlm_autotune(ctx, 3)
     valid = [r for r in rep if r["valid"]]
     best = min(valid, key=lambda r: r["ms"])["name"] if valid else None
     ftlm.ftlm_destroy(ctx)
-    print(json.dumps({"choice": best, "report": rep}), flush=True)
+    print(json.dumps({"stage": "release", "choice": best, "report": rep}), flush=True)
+
+
+def _child_json(cmd, env, timeout):
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, env=env)
+    for ln in reversed(out.stdout.strip().splitlines()):
+        if ln.startswith("{"):
+            return json.loads(ln), None
+    return None, f"rc={out.returncode}: {out.stderr.strip()[-300:]}"
 
 
 def probe_choice(args):
+    """Kernel configuration of the default run.  No candidate is timed in the release library before the SAME candidate
+    has run on THIS device in the checked library with zero address violations and agreed with the thread-per-row
+    kernel; if any stage fails the bench times the thread-per-row kernel."""
     cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--config", str(args.config), "--mode", args.mode]
     try:
-        out = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
-        for ln in reversed(out.stdout.strip().splitlines()):
-            if ln.startswith("{"):
-                d = json.loads(ln)
-                if d.get("choice") in CANDIDATES:
-                    return d["choice"], d["report"], None
-        return SAFE_CHOICE, None, f"probe rc={out.returncode}: {out.stderr.strip()[-300:]}"
+        from paper_2605_26261_b200 import build
+        build.build(checked=True)                      # no-op when libftlm_checked.so is up to date
+        d, err = _child_json(cmd + ["--probe-stage", "checked"], dict(os.environ, FTLM_CHECKED="1"), 1800)
+        if d is None:
+            return SAFE_CHOICE, None, "checked probe " + err
+        chk, rep = d["check"], d["report"]
+        if chk.get("check_build") != 1 or chk.get("check_violations") != 0:
+            return SAFE_CHOICE, rep, f"checked probe: address violations on the device: {chk}"
+        mask = 0
+        for r in rep:
+            if r["valid"] and r["name"] in CANDIDATES:
+                mask |= 1 << int(r["index"])
+        if mask == 0:
+            return SAFE_CHOICE, rep, "checked probe: no valid candidate"
+        env = dict(os.environ)
+        env.pop("FTLM_CHECKED", None)
+        d2, err = _child_json(cmd + ["--probe-stage", "release", "--mask", str(mask)], env, 900)
+        if d2 is None or d2.get("choice") not in CANDIDATES:
+            return SAFE_CHOICE, rep, "release probe " + (err or "no choice")
+        return d2["choice"], {"checked": rep, "release": d2["report"]}, None
     except Exception as e:  # timeout, crash
         return SAFE_CHOICE, None, f"probe failed: {e!r}"
 
@@ -191,6 +229,8 @@ def probe_choice(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--probe", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--probe-stage", default="checked", choices=["checked", "release"], help=argparse.SUPPRESS)
+    ap.add_argument("--mask", type=int, default=0, help=argparse.SUPPRESS)
     ap.add_argument("--candidate", default="", help="one of " + ", ".join(CANDIDATES))
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)

@@ -99,6 +99,7 @@ struct ftlm_ctx {
   int tml_low_bits = 0, tml_mid_bits = 0;
   int use_graph = 0;
   int allow_unverified = 0;        // option "allow_unverified": ftlm_autotune may run candidates without a device record
+  uint64_t autotune_mask = 0;      // option "autotune_mask": bit k set = candidate k may run (0 = all); the ROW reference always runs
   int autotuned = 0;               // 1 + index of the candidate ftlm_autotune selected (0 = not tuned)
   double autotune_ms = 0.0;
 
@@ -123,7 +124,6 @@ struct ftlm_ctx {
 
   // chain workspace
   void* q[3] = {nullptr, nullptr, nullptr};
-  int cur = 0;                     // (unused by the chain driver; roles are ia / ib / ic below)
   int ia = 0, ib = 1, ic = 2;      // q[ia] = q_j, q[ib] = q_{j-1}, q[ic] = y
   bool pending_norm = false;       // lazy normalisation: q_{j+1} = (q[ic] - alpha_j q[ia]) / beta_j is not materialised yet
   int lazy_norm = 0;               // option "lazy_norm": 1 = the TMLR pass forms q_{j+1} while staging (no normalisation pass)

@@ -441,9 +441,14 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     ftlm_tml_plan_destroy(c);
     return ftlm_tml_plan_create(c);
   }
+#if defined(FTLM_EMU) || defined(FTLM_CHECKED)
+  // test hooks of the host-emulation and checked builds only (sampled tiles / items of full-size sectors);
+  // the release library answers FTLM_EINVAL "unknown key"
   if (!strcmp(key, "debug_pass_mask")) { c->debug_pass_mask = (int)value; return FTLM_OK; }
   if (!strcmp(key, "debug_item_first")) { c->debug_item_first = value; return FTLM_OK; }
   if (!strcmp(key, "debug_item_count")) { c->debug_item_count = value; return FTLM_OK; }
+#endif
+  if (!strcmp(key, "autotune_mask")) { c->autotune_mask = (uint64_t)value; return FTLM_OK; }
   if (!strcmp(key, "passb") || !strcmp(key, "tml_split")) {
     // "passb": 0/1;  "tml_split": w | m << 8 (both at once; 0 = auto).  Rebuilds the TML / PASS-B plans.
     const int old_pb = c->use_passb, old_w = c->tml_low_bits, old_m = c->tml_mid_bits;
@@ -495,6 +500,7 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "sm_count")) return c->sm_count;
   if (!strcmp(key, "autotuned")) return c->autotuned;
   if (!strcmp(key, "allow_unverified")) return c->allow_unverified;
+  if (!strcmp(key, "autotune_mask")) return (int64_t)c->autotune_mask;
   if (!strcmp(key, "tmlr")) return c->use_tmlr;
   if (!strcmp(key, "lazy_norm")) return c->lazy_norm;
   if (!strcmp(key, "lazy_norm_ok")) return ftlm_tmlr_lazy_ok(c) ? 1 : 0;
@@ -614,7 +620,6 @@ static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64
   int rc = ensure_workspace(c);
   if (rc != FTLM_OK) return rc;
   const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
-  c->cur = 0;
   c->ia = 0; c->ib = 1; c->ic = 2;
   c->pending_norm = false;
   c->steps_enqueued = 0;

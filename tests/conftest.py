@@ -44,7 +44,19 @@ def pytest_sessionstart(session):
     build.build(checked=True)
     build.build()
     env = dict(os.environ, FTLM_CHECKED="1", FTLM_PREFLIGHT="0")
-    args = [a for a in config.invocation_params.args]
+    # the checked child runs the same selection minus the `slow` cases (whole vectors at BASELINE's full sizes: the
+    # checked kernels are one to two orders of magnitude slower); full sizes are covered in the checked build by
+    # tests/test_gpu_parity.py::test_checked_full_size_sampled_items (first, last, middle and random tiles / items of
+    # configs 3, 4 and 5 with their real run starts and offsets), which only runs there
+    args = []
+    it = iter(config.invocation_params.args)
+    for a in it:
+        if a == "-m":
+            args += ["-m", f"({next(it)}) and not slow"]
+        elif a.startswith("-m") and len(a) > 2 and not a.startswith("--"):
+            args += ["-m", f"({a[2:].strip()}) and not slow"]
+        else:
+            args.append(a)
     t0 = time.time()
     p = subprocess.run([sys.executable, "-m", "pytest", *args, "-p", "no:cacheprovider"], cwd=ROOT, env=env,
                        capture_output=True, text=True, timeout=int(os.environ.get("FTLM_PREFLIGHT_TIMEOUT", "5400")))

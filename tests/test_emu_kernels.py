@@ -142,7 +142,9 @@ def test_emu_autotune_checks_every_candidate_against_row():
             "    rep0 = c.autotune(1)\n"
             "    c.set('allow_unverified', 1)\n"
             "    rep = c.autotune(1)\n"
-            "    print(json.dumps({'rep0': rep0, 'rep': rep, 'tuned': c.get('autotuned')}))\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
+            "    c.set('autotune_mask', 1 << [r['index'] for r in rep if r['name'] == 'tmlr+passb'][0])\n"
+            "    rep2 = c.autotune(1)\n"
+            "    print(json.dumps({'rep0': rep0, 'rep': rep, 'rep2': rep2, 'tuned': c.get('autotuned')}))\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
     p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=900)
     assert p.returncode == 0, p.stderr[-2000:]
     d = json.loads(p.stdout.strip().splitlines()[-1])
@@ -153,7 +155,9 @@ def test_emu_autotune_checks_every_candidate_against_row():
     assert {r["name"] for r in d["rep0"]} == verified and "row" in verified
     names = [r["name"] for r in d["rep"]]
     assert names[0] == "row" and "tml" in names and "tml+passb" in names and "tmlr+passb" in names
-    assert all(r["valid"] and r["relerr"] <= 1e-5 for r in d["rep"]) and d["tuned"] >= 1
+    assert all(r["valid"] and r["relerr"] <= 1e-5 and r["maxabs"] <= r["elem_bound"] for r in d["rep"]) and d["tuned"] >= 1
+    # "autotune_mask" (bench.py: the candidates its checked pre-flight passed): the reference and the named candidate only
+    assert [r["name"] for r in d["rep2"]] == ["row", "tmlr+passb"]
     import bench
     assert set(names) <= set(bench.CANDIDATES), set(names) - set(bench.CANDIDATES)   # bench.py can apply whatever is chosen
 

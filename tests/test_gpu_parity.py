@@ -408,3 +408,29 @@ def test_tml_and_row_kernels_agree_on_config3_slice_fp32():
     base = outs[("clt", ftlm.KERNEL_ROW)].astype(np.float64)
     for key, y in outs.items():
         assert relerr(y, base) <= 1e-6, key
+
+
+# ---------------------------------------------------------------- full sizes in the checked build (sampled items)
+
+@pytest.mark.parametrize("cfg,mode,tmlr", [(3, "clt", 1), (3, "cr", 0), (4, "clt", 1), (4, "cr", 0), (4, "clt", 0),
+                                           (40, "cr", 1), (41, "clt", 0), (5, "cr", 1), (5, "cr", 0)])
+def test_checked_full_size_sampled_items(cfg, mode, tmlr):
+    """Only in the checked build (FTLM_CHECKED=1; tests/conftest.py runs the -m gpu selection there first): the first,
+    last, middle and random tiles / window items of BASELINE configs 3, 4, 4b (40), 4 in lexicographic numbering (41)
+    and 5 - real run starts, offsets and vector sizes, rows beyond 2^31 - one at a time through the in-tile pass (TML or
+    TMLR) and every PASS-B window, against the oracle's sampled-row form, with zero suppressed accesses
+    (tests/gpu_sampled.py).  This is what stands in for the `slow` whole-vector cases in the checked pre-flight."""
+    import json
+    import os
+    import subprocess
+    import sys
+    if not ftlm.CHECKED:
+        pytest.skip("checked build only (debug item hooks are not in the release ABI)")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    p = subprocess.run([sys.executable, os.path.join(root, "tests", "gpu_sampled.py"),
+                        json.dumps({"config": cfg, "mode": mode, "tmlr": tmlr, "samples": 2})],
+                       capture_output=True, text=True, timeout=1800)
+    assert p.returncode == 0, (p.stdout[-1500:], p.stderr[-3000:])
+    d = json.loads(p.stdout.strip().splitlines()[-1])
+    assert d["ok"], d
+    assert d["windows"] >= (1 if cfg != 41 else 0)
