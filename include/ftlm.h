@@ -63,16 +63,18 @@ int ftlm_destroy(ftlm_ctx* ctx);
 /* Sector dimension C(N, N_up). */
 int64_t ftlm_dim(const ftlm_ctx* ctx);
 
-/* Options: "kernel" (FTLM_KERNEL_*),
+/* Options: "kernel" (FTLM_KERNEL_*), "batch" (1, 2, 4: chains ftlm_lanczos / ftlm_lanczos_host advance together on
+ * interleaved vectors, L207; default 1),
  * "tml_low_bits" / "tml_mid_bits" / "tml_split" = w | m << 8 (split of the TML kernels, 0 = auto),
  * "graph" (1 = replay Lanczos steps from a CUDA graph); multi-pass H.v of kernel TML (DESIGN.md
  * 6.4-6.5): "passb" (1 = bonds that leave the tile go to PASS-B window passes; default 0),
  * "passb_lo_min" / "passb_smax" / "passb_ctas" (window planner: lowest label position, largest
  * window, CTAs per SM tried first; 0 = auto), "tmlr" (1 = in-tile pass by the TMLR kernel when its
  * plan exists), "tmlr_unij" (0 = never use the uniform-J form), "lazy_norm" (1 = no separate
- * normalisation pass in a chain: the TMLR pass forms q_{j+1} while staging; needs "tmlr").  Test hooks: "debug_pass_mask",
- * "debug_item_first", "debug_item_count" (run only some passes / tiles / items of a non-fused
- * H.v; used by the host emulation tests).  FTLM_EINVAL on unknown key/value, FTLM_EUNSUPPORTED
+ * normalisation pass in a chain: the TMLR pass forms q_{j+1} while staging; needs "tmlr"), "allow_unverified" / "autotune_mask" (ftlm_autotune: run candidates without a device record / only
+ * the candidates whose bit is set).  The checked and emulation builds (not the release library) also accept the test
+ * hooks "debug_pass_mask", "debug_item_first", "debug_item_count" (run only some passes / tiles / items of a non-fused
+ * H.v).  FTLM_EINVAL on unknown key/value, FTLM_EUNSUPPORTED
  * when the requested kernel / split cannot be built for this sector.  ftlm_get_option also answers
  * read-only keys: "sm_count", "autotuned", "tml_w", "tml_m", "tml_smem", "tml_ctas_per_sm",
  * "tml_threads", "tml_tiles", "tml_n_ll|mm|ml|tt|tm|tl", "tml_bclass:<b>", "tmlr_available",
@@ -137,6 +139,17 @@ int ftlm_chain_steps(ftlm_ctx* ctx, int nsteps, void* stream);
 /* Synchronise `stream` and copy out the coefficients: alpha[0..m_eff), beta[0..m_eff-1).
  * `cap` = capacity of h_alpha (and of h_beta).  h_m_eff receives the number of steps done. */
 int ftlm_chain_end(ftlm_ctx* ctx, double* h_alpha, double* h_beta, int cap, int* h_m_eff, void* stream);
+
+/* Batched chains (the paper's batched Lanczos, L207, L309, Table 3 footnote L325): begin `batch` (1, 2 or 4) chains
+ * r0 .. r0 + batch - 1 from their seeded start vectors on interleaved work vectors q[t][batch]; every fused pass
+ * then computes the row state and every neighbour index once for all of them.  ftlm_chain_steps advances the whole
+ * batch; each chain has its own alpha, beta and breakdown state, and its coefficients are bit-identical to those of
+ * the same chain run alone with the same kernel and tile split.  batch > 1 runs the ROW kernel or the TML kernel
+ * without PASS-B windows (FTLM_EUNSUPPORTED while option "passb" is 1).  Asynchronous. */
+int ftlm_chain_begin_batch(ftlm_ctx* ctx, uint64_t seed, int r0, int batch, void* stream);
+
+/* ftlm_chain_end for the batch in progress: chain b -> h_alpha[b*cap ...], h_beta[b*cap ...], h_m_eff[b]. */
+int ftlm_chain_end_batch(ftlm_ctx* ctx, double* h_alpha, double* h_beta, int cap, int* h_m_eff, void* stream);
 
 /* Run `nsteps` steps with CUDA events around every kernel and return the average device time
  * (ms) of the fused H.v kernel and of the normalisation kernel.  Synchronous; for bench.py. */

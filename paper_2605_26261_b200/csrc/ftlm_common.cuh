@@ -37,6 +37,7 @@ cudaError_t ftlm_dfree(void* p);
 void ftlm_chk_caller(cudaStream_t s, const void* p, size_t bytes);
 
 #define FTLM_MAX_BONDS 4096
+#define FTLM_MAX_BATCH 4
 
 void ftlm_set_error(const char* fmt, ...);
 int ftlm_cuda_fail(cudaError_t e, const char* what);
@@ -127,9 +128,12 @@ struct ftlm_ctx {
   int ia = 0, ib = 1, ic = 2;      // q[ia] = q_j, q[ib] = q_{j-1}, q[ic] = y
   bool pending_norm = false;       // lazy normalisation: q_{j+1} = (q[ic] - alpha_j q[ia]) / beta_j is not materialised yet
   int lazy_norm = 0;               // option "lazy_norm": 1 = the TMLR pass forms q_{j+1} while staging (no normalisation pass)
-  ChainState* d_state = nullptr;
-  double* d_partials = nullptr;    // [3][max_blocks]
-  unsigned int* d_ticket = nullptr;
+  ChainState* d_state = nullptr;   // [FTLM_MAX_BATCH]
+  double* d_partials = nullptr;    // [3 * FTLM_MAX_BATCH][max_blocks]
+  unsigned int* d_ticket = nullptr;  // [FTLM_MAX_BATCH]
+  int batch = 1;                   // option "batch": chains ftlm_lanczos advances together on interleaved vectors (1, 2, 4)
+  int cur_batch = 1;               // batch of the chain(s) in progress
+  int q_batch = 0;                 // batch the work vectors were allocated for
   int max_blocks = 0;
   int steps_enqueued = 0;
   int chain_limit = 0;
@@ -142,7 +146,7 @@ int ftlm_effective_kernel(const ftlm_ctx* c);
 // ---- launches implemented in the kernel translation units -------------------------------
 // fused == 0: y = H v.   fused == 1: y = H q - beta_prev q_prev with the three FP64 sums and
 // the in-kernel finalisation of alpha_j, beta_j into ctx->d_state.
-int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
+int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, int batch, cudaStream_t s);
 int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
 
 int ftlm_tml_plan_create(ftlm_ctx* c);
@@ -251,6 +255,7 @@ __device__ __forceinline__ void lanczos_finish(double s_qy, double s_yy, double 
   block_sum3(a, b, c, sh);
   if (threadIdx.x == 0) {
     *ticket = 0;
+    if (st->done) return;                 // a chain of a batch that broke down earlier keeps its coefficients
     const int j = st->step;
     const double alpha = c > 0.0 ? a / c : 0.0;
     double b2 = c > 0.0 ? b - a * a / c : 0.0;
@@ -265,7 +270,7 @@ __device__ __forceinline__ void lanczos_finish(double s_qy, double s_yy, double 
     st->a = alpha;
     st->inv_b = beta > 0.0 ? 1.0 / beta : 0.0;
     st->beta_prev = beta;
-    if (j + 1 >= st->limit || beta <= st->tol * sc) st->done = 1;
+    if (j + 1 >= st->limit || beta <= st->tol * sc) { st->done = 1; st->inv_b = 0.0; }
   }
 }
 

@@ -239,29 +239,34 @@ __global__ void reduce_partials_kernel(const double* __restrict__ partials, int 
 
 template <typename R>
 __global__ void __launch_bounds__(256)
-gauss_write_kernel(uint64_t key, int64_t dim, const double* __restrict__ norm2, R* __restrict__ v) {
-  const double nrm = sqrt(*norm2);
+gauss_write_kernel(uint64_t key, int64_t dim, const double* __restrict__ norm2, R* __restrict__ v, int vstride, int voff) {
+  const double nrm = sqrt(*norm2);                       // element t of the chain goes to v[t * vstride + voff] (interleaved batch)
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
        t += (int64_t)gridDim.x * blockDim.x)
-    ST_G(&v[t], (R)(gauss_elem(key, (uint64_t)t) / nrm));
+    ST_G(&v[t * vstride + voff], (R)(gauss_elem(key, (uint64_t)t) / nrm));
 }
 
 template <typename R>
 __global__ void __launch_bounds__(256)
-scale_copy_kernel(const R* __restrict__ src, int64_t dim, const double* __restrict__ norm2, R* __restrict__ dst) {
+scale_copy_kernel(const R* __restrict__ src, int64_t dim, const double* __restrict__ norm2, R* __restrict__ dst, int dstride, int doff) {
   const double nrm = sqrt(*norm2);
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim;
        t += (int64_t)gridDim.x * blockDim.x)
-    ST_G(&dst[t], (R)((double)LD_G(&src[t]) / nrm));
+    ST_G(&dst[t * dstride + doff], (R)((double)LD_G(&src[t]) / nrm));
 }
 
 // ---- Lanczos normalisation pass (A7): q_{j+1} = (y - alpha_j q_j) / beta_j ----------------------
-template <typename R, typename V4>
+// B interleaved chains: element i of the arrays belongs to chain i % B and uses that chain's alpha_j, 1 / beta_j
+// (a chain that has broken down has 1 / beta = 0: its column becomes zero and stays out of the way).
+template <typename R, typename V4, int B>
 __global__ void __launch_bounds__(256)
 lanczos_next_kernel(const R* __restrict__ y, const R* __restrict__ q, R* __restrict__ qnext,
                     int64_t dim, const ChainState* __restrict__ st) {
-  if (st->done) return;
-  const R a = (R)st->a, ib = (R)st->inv_b;
+  bool all_done = true;
+  R av[B], ibv[B];
+#pragma unroll
+  for (int c = 0; c < B; ++c) { all_done = all_done && st[c].done; av[c] = (R)st[c].a; ibv[c] = (R)st[c].inv_b; }
+  if (all_done) return;
   constexpr int W = sizeof(V4) / sizeof(R);
   const int64_t nvec = dim / W;
   const V4* y4 = (const V4*)y;
@@ -274,15 +279,27 @@ lanczos_next_kernel(const R* __restrict__ y, const R* __restrict__ q, R* __restr
     R* yp = (R*)&yy;
     const R* qp = (const R*)&qq;
 #pragma unroll
-    for (int e = 0; e < W; ++e) yp[e] = (yp[e] - a * qp[e]) * ib;
+    for (int e = 0; e < W; ++e) {
+      const int c = B == 1 ? 0 : (int)((k * W + e) % B);
+      R a = av[0], ib = ibv[0];
+#pragma unroll
+      for (int cc = 1; cc < B; ++cc) if (c == cc) { a = av[cc]; ib = ibv[cc]; }
+      yp[e] = (yp[e] - a * qp[e]) * ib;
+    }
     ST_G(&o4[k], yy);
   }
-  for (int64_t t = nvec * W + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim; t += stride)
+  for (int64_t t = nvec * W + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < dim; t += stride) {
+    const int c = B == 1 ? 0 : (int)(t % B);
+    R a = av[0], ib = ibv[0];
+#pragma unroll
+    for (int cc = 1; cc < B; ++cc) if (c == cc) { a = av[cc]; ib = ibv[cc]; }
     ST_G(&qnext[t], (LD_G(&y[t]) - a * LD_G(&q[t])) * ib);
+  }
 }
 
-__global__ void chain_reset_kernel(ChainState* st, int limit, double tol) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) {
+__global__ void chain_reset_kernel(ChainState* st0, int limit, double tol, int nb) {
+  if (blockIdx.x == 0 && (int)threadIdx.x < nb) {
+    ChainState* st = st0 + threadIdx.x;
     st->scale = 0.0; st->beta_prev = 0.0; st->a = 0.0; st->inv_b = 0.0; st->tol = tol;
     st->step = 0; st->limit = limit; st->done = (limit <= 0);
   }
@@ -363,11 +380,11 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
   CKF(ftlm_dmalloc(&c->d_bonds, sizeof(BondDev) * (size_t)(n_bonds > 0 ? n_bonds : 1)));
   if (n_bonds > 0) CKF(cudaMemcpy(c->d_bonds, c->bonds.data(), sizeof(BondDev) * n_bonds, cudaMemcpyHostToDevice));
   c->max_blocks = c->sm_count * 32;
-  CKF(ftlm_dmalloc(&c->d_state, sizeof(ChainState)));
-  CKF(cudaMemset(c->d_state, 0, sizeof(ChainState)));
-  CKF(ftlm_dmalloc(&c->d_partials, sizeof(double) * 3 * (size_t)c->max_blocks));
-  CKF(ftlm_dmalloc(&c->d_ticket, sizeof(unsigned int)));
-  CKF(cudaMemset(c->d_ticket, 0, sizeof(unsigned int)));
+  CKF(ftlm_dmalloc(&c->d_state, sizeof(ChainState) * FTLM_MAX_BATCH));
+  CKF(cudaMemset(c->d_state, 0, sizeof(ChainState) * FTLM_MAX_BATCH));
+  CKF(ftlm_dmalloc(&c->d_partials, sizeof(double) * 3 * FTLM_MAX_BATCH * (size_t)c->max_blocks));
+  CKF(ftlm_dmalloc(&c->d_ticket, sizeof(unsigned int) * FTLM_MAX_BATCH));
+  CKF(cudaMemset(c->d_ticket, 0, sizeof(unsigned int) * FTLM_MAX_BATCH));
   if (index_mode == FTLM_INDEX_CLT) {
     c->n_clt = (int64_t)(((1ull << N) + 31ull) / 32ull);
     CKF(ftlm_dmalloc(&c->d_clt, sizeof(uint2) * (size_t)c->n_clt));
@@ -449,6 +466,18 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   if (!strcmp(key, "debug_item_count")) { c->debug_item_count = value; return FTLM_OK; }
 #endif
   if (!strcmp(key, "autotune_mask")) { c->autotune_mask = (uint64_t)value; return FTLM_OK; }
+  if (!strcmp(key, "batch")) {
+    // chains per row pass of ftlm_lanczos / ftlm_lanczos_host (L207, L309); the TML split is re-chosen so that a
+    // tile of `batch` interleaved vectors fits shared memory
+    if (value != 1 && value != 2 && value != 4) { ftlm_set_error("batch must be 1, 2 or 4"); return FTLM_EINVAL; }
+    const int old = c->batch;
+    c->batch = (int)value;
+    CK(cudaSetDevice(c->device));
+    ftlm_tml_plan_destroy(c);
+    int rc = ftlm_tml_plan_create(c);
+    if (rc != FTLM_OK) { c->batch = old; ftlm_tml_plan_destroy(c); ftlm_tml_plan_create(c); }
+    return rc;
+  }
   if (!strcmp(key, "passb") || !strcmp(key, "tml_split")) {
     // "passb": 0/1;  "tml_split": w | m << 8 (both at once; 0 = auto).  Rebuilds the TML / PASS-B plans.
     const int old_pb = c->use_passb, old_w = c->tml_low_bits, old_m = c->tml_mid_bits;
@@ -501,6 +530,7 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "autotuned")) return c->autotuned;
   if (!strcmp(key, "allow_unverified")) return c->allow_unverified;
   if (!strcmp(key, "autotune_mask")) return (int64_t)c->autotune_mask;
+  if (!strcmp(key, "batch")) return c->batch;
   if (!strcmp(key, "tmlr")) return c->use_tmlr;
   if (!strcmp(key, "lazy_norm")) return c->lazy_norm;
   if (!strcmp(key, "lazy_norm_ok")) return ftlm_tmlr_lazy_ok(c) ? 1 : 0;
@@ -521,8 +551,17 @@ extern "C" int ftlm_clt_read(ftlm_ctx* c, int64_t b0, int64_t nb, uint32_t* h_ma
 }
 
 // ---- H.v ---------------------------------------------------------------------------------------
-static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
+static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s, int batch = 1) {
   const int k = ftlm_effective_kernel(c);
+  if (batch > 1) {
+    // batched chains (L207, L309): the TML kernel with every bond that leaves the tile as a global read, or ROW;
+    // the window passes and the register-table in-tile pass are single-vector kernels
+    if (k == FTLM_KERNEL_TML) {
+      if (c->passb) { ftlm_set_error("batch > 1: set option \"passb\" to 0 (the PASS-B window passes take one vector)"); return FTLM_EUNSUPPORTED; }
+      return ftlm_launch_hv_tml(c, v, qp, y, fused, batch, s);
+    }
+    return ftlm_launch_hv_row(c, v, qp, y, fused, batch, s);
+  }
   if (k == FTLM_KERNEL_TML) {
     // two-pass step when PASS-B windows exist: the TML pass leaves the sums and the finish to PASS-B
     const bool pb = c->passb != nullptr;
@@ -534,7 +573,7 @@ static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fu
     if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, s);
     return rc;
   }
-  return ftlm_launch_hv_row(c, v, qp, y, fused, s);
+  return ftlm_launch_hv_row(c, v, qp, y, fused, 1, s);
 }
 
 extern "C" int ftlm_apply_H(ftlm_ctx* c, const void* d_v, void* d_y, void* stream) {
@@ -598,47 +637,62 @@ extern "C" int ftlm_fill_random(ftlm_ctx* c, uint64_t seed, int r, void* d_v, vo
   const int grid = stream_grid(c, c->dim, 8);
   FTLM_LAUNCH(gauss_norm_kernel, grid, 256, 0, s, key, c->dim, c->d_partials);
   FTLM_LAUNCH(reduce_partials_kernel, 1, 256, 0, s, c->d_partials, grid, &c->d_state->norm2);
-  if (c->prec == FTLM_FP32) { auto k__ = gauss_write_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, &c->d_state->norm2, (float*)d_v); }
-  else { auto k__ = gauss_write_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, &c->d_state->norm2, (double*)d_v); }
+  if (c->prec == FTLM_FP32) { auto k__ = gauss_write_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, &c->d_state->norm2, (float*)d_v, 1, 0); }
+  else { auto k__ = gauss_write_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, &c->d_state->norm2, (double*)d_v, 1, 0); }
   CK(cudaGetLastError());
   return FTLM_OK;
 }
 
 // ---- chain -------------------------------------------------------------------------------------
-static int ensure_workspace(ftlm_ctx* c) {
-  const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
+static int ensure_workspace(ftlm_ctx* c, int batch) {
+  const size_t bytes = (size_t)c->dim * ftlm_elem_size(c) * (size_t)batch;
+  if (c->q_batch < batch) {                            // (re)allocate for the widest batch seen so far
+    for (int k = 0; k < 3; ++k) { ftlm_dfree(c->q[k]); c->q[k] = nullptr; }
+    c->q_batch = 0;
+  }
   for (int k = 0; k < 3; ++k)
     if (!c->q[k]) {
       cudaError_t e = ftlm_dmalloc(&c->q[k], bytes);
       if (e != cudaSuccess) { ftlm_set_error("chain workspace: cannot allocate 3 x %zu bytes (%s)", bytes, cudaGetErrorString(e)); cudaGetLastError(); return FTLM_ENOMEM; }
     }
+  if (c->q_batch < batch) c->q_batch = batch;
   return FTLM_OK;
 }
 
-static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64_t seed, int r, cudaStream_t s) {
+// Begin `batch` chains r0 .. r0 + batch - 1 on interleaved work vectors q[t][batch] (batch = 1: plain vectors).
+// q1 == nullptr: seeded start vectors; else `batch` vectors of dim elements each, one after the other.
+static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64_t seed, int r0, int batch, cudaStream_t s) {
   CK(cudaSetDevice(c->device));
-  int rc = ensure_workspace(c);
+  if (batch != 1 && batch != 2 && batch != 4) { ftlm_set_error("batch must be 1, 2 or 4 (got %d)", batch); return FTLM_EINVAL; }
+  int rc = ensure_workspace(c, batch);
   if (rc != FTLM_OK) return rc;
-  const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
+  const size_t vbytes = (size_t)c->dim * ftlm_elem_size(c), bytes = vbytes * (size_t)batch;
   c->ia = 0; c->ib = 1; c->ic = 2;
   c->pending_norm = false;
   c->steps_enqueued = 0;
+  c->cur_batch = batch;
   c->chain_limit = (int)(c->dim < FTLM_MAX_STEPS ? c->dim : FTLM_MAX_STEPS);
-  if (!q1) {
-    rc = ftlm_fill_random(c, seed, r, c->q[0], s);
-    if (rc != FTLM_OK) return rc;
-  } else {
-    // copy into q[2] (scratch), then normalise in FP64 into q[0]
-    CK(cudaMemcpyAsync(c->q[2], q1, bytes, q1_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
-    const int grid = stream_grid(c, c->dim, 8);
-    if (c->prec == FTLM_FP32) { auto k__ = sumsq_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)c->q[2], c->dim, c->d_partials); }
-    else { auto k__ = sumsq_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)c->q[2], c->dim, c->d_partials); }
-    FTLM_LAUNCH(reduce_partials_kernel, 1, 256, 0, s, c->d_partials, grid, &c->d_state->norm2);
-    if (c->prec == FTLM_FP32) { auto k__ = scale_copy_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)c->q[2], c->dim, &c->d_state->norm2, (float*)c->q[0]); }
-    else { auto k__ = scale_copy_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)c->q[2], c->dim, &c->d_state->norm2, (double*)c->q[0]); }
+  const int grid = stream_grid(c, c->dim, 8);
+  for (int b = 0; b < batch; ++b) {
+    double* norm2 = &c->d_state[b].norm2;
+    if (!q1) {
+      const uint64_t key = chain_key(seed, c->N_up, r0 + b);
+      FTLM_LAUNCH(gauss_norm_kernel, grid, 256, 0, s, key, c->dim, c->d_partials);
+      FTLM_LAUNCH(reduce_partials_kernel, 1, 256, 0, s, c->d_partials, grid, norm2);
+      if (c->prec == FTLM_FP32) { auto k__ = gauss_write_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, norm2, (float*)c->q[0], batch, b); }
+      else { auto k__ = gauss_write_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, key, c->dim, norm2, (double*)c->q[0], batch, b); }
+    } else {
+      // copy into q[2] (scratch), then normalise in FP64 into column b of q[0]
+      CK(cudaMemcpyAsync(c->q[2], (const char*)q1 + (size_t)b * vbytes, vbytes, q1_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, s));
+      if (c->prec == FTLM_FP32) { auto k__ = sumsq_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)c->q[2], c->dim, c->d_partials); }
+      else { auto k__ = sumsq_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)c->q[2], c->dim, c->d_partials); }
+      FTLM_LAUNCH(reduce_partials_kernel, 1, 256, 0, s, c->d_partials, grid, norm2);
+      if (c->prec == FTLM_FP32) { auto k__ = scale_copy_kernel<float>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)c->q[2], c->dim, norm2, (float*)c->q[0], batch, b); }
+      else { auto k__ = scale_copy_kernel<double>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)c->q[2], c->dim, norm2, (double*)c->q[0], batch, b); }
+    }
   }
   CK(cudaMemsetAsync(c->q[1], 0, bytes, s));          // q_0 = 0
-  FTLM_LAUNCH(chain_reset_kernel, 1, 32, 0, s, c->d_state, c->chain_limit, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
+  FTLM_LAUNCH(chain_reset_kernel, 1, 32, 0, s, c->d_state, c->chain_limit, c->prec == FTLM_FP32 ? 1e-5 : 1e-12, batch);
   CK(cudaGetLastError());
   return FTLM_OK;
 }
@@ -646,16 +700,22 @@ static int chain_begin_impl(ftlm_ctx* c, const void* q1, bool q1_on_host, uint64
 extern "C" int ftlm_chain_begin(ftlm_ctx* c, const void* d_q1, uint64_t seed, int r, void* stream) {
   if (!c || r < 0) { ftlm_set_error("ftlm_chain_begin: bad argument"); return FTLM_EINVAL; }
   if (d_q1) ftlm_chk_caller((cudaStream_t)stream, d_q1, (size_t)c->dim * ftlm_elem_size(c));
-  return chain_begin_impl(c, d_q1, false, seed, r, (cudaStream_t)stream);
+  return chain_begin_impl(c, d_q1, false, seed, r, 1, (cudaStream_t)stream);
 }
 
 static int launch_next(ftlm_ctx* c, cudaStream_t s) {
   const void* y = c->q[c->ic];
   const void* q = c->q[c->ia];
   void* qn = c->q[c->ib];
-  const int grid = stream_grid(c, c->dim / 4 + 1, 8);
-  if (c->prec == FTLM_FP32) { auto k__ = lanczos_next_kernel<float, float4>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)y, (const float*)q, (float*)qn, c->dim, c->d_state); }
-  else { auto k__ = lanczos_next_kernel<double, double2>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)y, (const double*)q, (double*)qn, c->dim, c->d_state); }
+  const int64_t n = c->dim * c->cur_batch;             // interleaved batch: element i belongs to chain i % batch
+  const int grid = stream_grid(c, n / 4 + 1, 8);
+#define NEXT(BB)                                                                                                     \
+  do {                                                                                                               \
+    if (c->prec == FTLM_FP32) { auto k__ = lanczos_next_kernel<float, float4, BB>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const float*)y, (const float*)q, (float*)qn, n, c->d_state); } \
+    else { auto k__ = lanczos_next_kernel<double, double2, BB>; FTLM_LAUNCH(k__, grid, 256, 0, s, (const double*)y, (const double*)q, (double*)qn, n, c->d_state); } \
+  } while (0)
+  if (c->cur_batch == 1) NEXT(1); else if (c->cur_batch == 2) NEXT(2); else NEXT(4);
+#undef NEXT
   CK(cudaGetLastError());
   return FTLM_OK;
 }
@@ -663,7 +723,7 @@ static int launch_next(ftlm_ctx* c, cudaStream_t s) {
 static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv, float* ms_norm) {
   // lazy normalisation (option "lazy_norm", TMLR in-tile pass only): no normalisation pass; the next step's
   // in-tile pass forms q_{j+1} = (y_j - alpha_j q_j)/beta_j while it stages its tile and writes it over y_j
-  const bool lazy = c->lazy_norm && ftlm_effective_kernel(c) == FTLM_KERNEL_TML && ftlm_tmlr_lazy_ok(c);
+  const bool lazy = c->cur_batch == 1 && c->lazy_norm && ftlm_effective_kernel(c) == FTLM_KERNEL_TML && ftlm_tmlr_lazy_ok(c);
   // y = H q_j - beta_{j-1} q_{j-1}   (+ reductions, alpha_j, beta_j on the device)
   if (timed) CK(cudaEventRecord(c->ev[0], s));
   int rc;
@@ -680,7 +740,7 @@ static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv,
       const int a = c->ia; c->ia = c->ib; c->ib = a;
       c->pending_norm = false;
     }
-    rc = launch_hv(c, c->q[c->ia], c->q[c->ib], c->q[c->ic], 1, s);
+    rc = launch_hv(c, c->q[c->ia], c->q[c->ib], c->q[c->ic], 1, s, c->cur_batch);
   }
   if (rc != FTLM_OK) return rc;
   if (timed) CK(cudaEventRecord(c->ev[1], s));
@@ -729,18 +789,36 @@ extern "C" int ftlm_chain_profile(ftlm_ctx* c, int nsteps, void* stream, double*
   return FTLM_OK;
 }
 
+// coefficients of chain b of the batch in progress: alpha -> h_alpha + b * cap, beta -> h_beta + b * cap
+static int chain_end_impl(ftlm_ctx* c, double* h_alpha, double* h_beta, int cap, int* h_m_eff, int batch, cudaStream_t s) {
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(s));
+  static thread_local ChainState hs[FTLM_MAX_BATCH];
+  CK(cudaMemcpy(hs, c->d_state, sizeof(ChainState) * (size_t)batch, cudaMemcpyDeviceToHost));
+  for (int b = 0; b < batch; ++b) {
+    int m = hs[b].step;
+    h_m_eff[b] = m;
+    if (m > cap) m = cap;
+    if (h_alpha) for (int k = 0; k < m; ++k) h_alpha[(size_t)b * cap + k] = hs[b].alpha[k];
+    if (h_beta) for (int k = 0; k + 1 < m; ++k) h_beta[(size_t)b * cap + k] = hs[b].beta[k];
+  }
+  return FTLM_OK;
+}
+
 extern "C" int ftlm_chain_end(ftlm_ctx* c, double* h_alpha, double* h_beta, int cap, int* h_m_eff, void* stream) {
   if (!c || !h_m_eff || cap < 0) { ftlm_set_error("ftlm_chain_end: bad argument"); return FTLM_EINVAL; }
-  CK(cudaSetDevice(c->device));
-  CK(cudaStreamSynchronize((cudaStream_t)stream));
-  static thread_local ChainState hs;
-  CK(cudaMemcpy(&hs, c->d_state, sizeof(ChainState), cudaMemcpyDeviceToHost));
-  int m = hs.step;
-  *h_m_eff = m;
-  if (m > cap) m = cap;
-  if (h_alpha) for (int k = 0; k < m; ++k) h_alpha[k] = hs.alpha[k];
-  if (h_beta) for (int k = 0; k + 1 < m; ++k) h_beta[k] = hs.beta[k];
-  return FTLM_OK;
+  if (c->cur_batch != 1) { ftlm_set_error("ftlm_chain_end: a batch of %d chains is in progress; use ftlm_chain_end_batch", c->cur_batch); return FTLM_EINVAL; }
+  return chain_end_impl(c, h_alpha, h_beta, cap, h_m_eff, 1, (cudaStream_t)stream);
+}
+
+extern "C" int ftlm_chain_begin_batch(ftlm_ctx* c, uint64_t seed, int r0, int batch, void* stream) {
+  if (!c || r0 < 0) { ftlm_set_error("ftlm_chain_begin_batch: bad argument"); return FTLM_EINVAL; }
+  return chain_begin_impl(c, nullptr, false, seed, r0, batch, (cudaStream_t)stream);
+}
+
+extern "C" int ftlm_chain_end_batch(ftlm_ctx* c, double* h_alpha, double* h_beta, int cap, int* h_m_eff, void* stream) {
+  if (!c || !h_m_eff || cap < 0) { ftlm_set_error("ftlm_chain_end_batch: bad argument"); return FTLM_EINVAL; }
+  return chain_end_impl(c, h_alpha, h_beta, cap, h_m_eff, c->cur_batch, (cudaStream_t)stream);
 }
 
 static int lanczos_impl(ftlm_ctx* c, const void* h_q1, uint64_t seed, int R, int n_steps, double* h_alpha,
@@ -749,28 +827,35 @@ static int lanczos_impl(ftlm_ctx* c, const void* h_q1, uint64_t seed, int R, int
     ftlm_set_error("ftlm_lanczos: bad argument (n_steps must be in [1,%d])", FTLM_MAX_STEPS); return FTLM_EINVAL;
   }
   const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
-  for (int r = 0; r < R; ++r) {
+  for (size_t k = 0; k < (size_t)R * n_steps; ++k) { h_alpha[k] = 0.0; h_beta[k] = 0.0; }
+  // chains advance in groups of option "batch" (4, 2 or 1) on interleaved vectors; a remainder runs in smaller groups
+  for (int r = 0; r < R;) {
+    int nb = c->batch;
+    while (nb > R - r) nb >>= 1;
     double* a = h_alpha + (size_t)r * n_steps;
     double* b = h_beta + (size_t)r * n_steps;
-    for (int k = 0; k < n_steps; ++k) { a[k] = 0.0; b[k] = 0.0; }
-    int rc = chain_begin_impl(c, h_q1 ? (const char*)h_q1 + (size_t)r * bytes : nullptr, h_q1 != nullptr, seed, r, s);
+    int rc = chain_begin_impl(c, h_q1 ? (const char*)h_q1 + (size_t)r * bytes : nullptr, h_q1 != nullptr, seed, r, nb, s);
     if (rc != FTLM_OK) return rc;
     if (c->chain_limit > n_steps) {           // m = min(n_steps, dim)
       c->chain_limit = n_steps;
-      FTLM_LAUNCH(chain_reset_kernel, 1, 32, 0, s, c->d_state, n_steps, c->prec == FTLM_FP32 ? 1e-5 : 1e-12);
+      FTLM_LAUNCH(chain_reset_kernel, 1, 32, 0, s, c->d_state, n_steps, c->prec == FTLM_FP32 ? 1e-5 : 1e-12, nb);
     }
     rc = ftlm_chain_steps(c, n_steps, s);
     if (rc != FTLM_OK) return rc;
-    rc = ftlm_chain_end(c, a, b, n_steps, &h_m_eff[r], s);
+    rc = chain_end_impl(c, a, b, n_steps, &h_m_eff[r], nb, s);
     if (rc != FTLM_OK) return rc;
     if (h_theta && h_weight) {
-      double* th = h_theta + (size_t)r * n_steps;
-      double* w = h_weight + (size_t)r * n_steps;
-      for (int k = 0; k < n_steps; ++k) { th[k] = 0.0; w[k] = 0.0; }
-      rc = ftlm_tridiag_eig(h_m_eff[r], a, b, th, w);
-      if (rc != FTLM_OK) return rc;
+      for (int q = 0; q < nb; ++q) {
+        double* th = h_theta + (size_t)(r + q) * n_steps;
+        double* w = h_weight + (size_t)(r + q) * n_steps;
+        for (int k = 0; k < n_steps; ++k) { th[k] = 0.0; w[k] = 0.0; }
+        rc = ftlm_tridiag_eig(h_m_eff[r + q], a + (size_t)q * n_steps, b + (size_t)q * n_steps, th, w);
+        if (rc != FTLM_OK) return rc;
+      }
     }
+    r += nb;
   }
+  c->cur_batch = 1;
   return FTLM_OK;
 }
 

@@ -103,23 +103,36 @@ __device__ __forceinline__ void load_tables(const RowParams& p, I* s_binom, Bond
   __syncthreads();
 }
 
-template <typename R, typename L, typename I, int MODE, bool FUSED>
+// B > 1: the paper's batched Lanczos (L207, L309): B chains on interleaved vectors v[t][B] share the row state and
+// every index computation; each chain's arithmetic is the B = 1 arithmetic in the same order (bit-identical results).
+template <typename R, typename L, typename I, int MODE, bool FUSED, int B>
 __global__ void __launch_bounds__(256)
 hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev, R* __restrict__ y) {
   FTLM_DYN_SMEM(smem);
   __shared__ double sh_red[96];
-  if (FUSED) { if (p.st->done) return; }
+  if (FUSED) {
+    bool all_done = true;
+#pragma unroll
+    for (int c = 0; c < B; ++c) all_done = all_done && p.st[c].done;
+    if (all_done) return;
+  }
   I* s_binom = (I*)smem;
   const int nbin = (p.N + 1) * (p.K + 1);
   BondS<R>* s_bonds = (BondS<R>*)(smem + (((size_t)nbin * sizeof(I) + 15) & ~(size_t)15));
   load_tables<R, L, I>(p, s_binom, s_bonds);
   const int K1 = p.K + 1;
-  const R bprev = FUSED ? (R)p.st->beta_prev : (R)0;
-  double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
+  R bprev[B];
+#pragma unroll
+  for (int c = 0; c < B; ++c) bprev[c] = FUSED ? (R)p.st[c].beta_prev : (R)0;
+  double s_qy[B], s_yy[B], s_qq[B];
+#pragma unroll
+  for (int c = 0; c < B; ++c) { s_qy[c] = 0.0; s_yy[c] = 0.0; s_qq[c] = 0.0; }
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < p.dim; t += stride) {
     const L n = unrank<L, I>((I)t, p.N, K1, p.K, s_binom);
-    R acc = 0, danti = 0;
+    R acc[B], danti = 0;
+#pragma unroll
+    for (int c = 0; c < B; ++c) acc[c] = 0;
     for (int b = 0; b < p.nb; ++b) {
       const L m = (L)s_bonds[b].mask;
       const L x = n & m;
@@ -127,21 +140,29 @@ hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev,
         I idx;
         if (MODE == FTLM_INDEX_CLT) idx = (I)clt_lookup((uint32_t)(n ^ m), p.clt);
         else idx = (I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom);
-        acc += s_bonds[b].Jh * LDG(&v[idx]);
+#pragma unroll
+        for (int c = 0; c < B; ++c) acc[c] += s_bonds[b].Jh * LDG(&v[(size_t)idx * B + c]);
         danti += s_bonds[b].Jq;
       }
     }
-    const R vt = LD_G(&v[t]);
-    R out = ((R)p.diag0 - 2 * danti) * vt + acc;
-    if (FUSED) {
-      out -= bprev * LD_G(&qprev[t]);
-      s_qy += (double)vt * (double)out;
-      s_yy += (double)out * (double)out;
-      s_qq += (double)vt * (double)vt;
+#pragma unroll
+    for (int c = 0; c < B; ++c) {
+      const R vt = LD_G(&v[(size_t)t * B + c]);
+      R out = ((R)p.diag0 - 2 * danti) * vt + acc[c];
+      if (FUSED) {
+        out -= bprev[c] * LD_G(&qprev[(size_t)t * B + c]);
+        s_qy[c] += (double)vt * (double)out;
+        s_yy[c] += (double)out * (double)out;
+        s_qq[c] += (double)vt * (double)vt;
+      }
+      ST_G(&y[(size_t)t * B + c], out);
     }
-    ST_G(&y[t], out);
   }
-  if (FUSED) lanczos_finish(s_qy, s_yy, s_qq, p.partials, p.stride, p.ticket, p.st, sh_red);
+  if (FUSED) {
+#pragma unroll
+    for (int c = 0; c < B; ++c)        // chain c: partials [3c .. 3c+3) x stride, ticket c, state c
+      lanczos_finish(s_qy[c], s_yy[c], s_qq[c], p.partials + (size_t)3 * c * p.stride, p.stride, p.ticket + c, p.st + c, sh_red);
+  }
 }
 
 template <typename L, typename I, int MODE>
@@ -231,19 +252,28 @@ int grid_for(const ftlm_ctx* c, int64_t work, int per_sm) {
 }
 
 template <typename R, typename L, typename I>
-int launch_hv(ftlm_ctx* c, const RowParams& p, const void* v, const void* qp, void* y, int fused,
+int launch_hv(ftlm_ctx* c, const RowParams& p, const void* v, const void* qp, void* y, int fused, int batch,
               cudaStream_t s) {
   const size_t sm = table_smem(c, sizeof(BondS<R>));
   const int grid = grid_for(c, c->dim, 8);
   if (fused && grid > c->max_blocks) { ftlm_set_error("internal: grid > max_blocks"); return FTLM_EINVAL; }
-#define LAUNCH(MODE, FUSED)                                                                      \
+  if (batch != 1 && !fused) { ftlm_set_error("ROW: batched vectors exist in the fused Lanczos step only"); return FTLM_EINVAL; }
+#define LAUNCH(MODE, FUSED, BB)                                                                  \
   do {                                                                                           \
-    auto k = hv_row_kernel<R, L, I, MODE, FUSED>;                                                \
+    auto k = hv_row_kernel<R, L, I, MODE, FUSED, BB>;                                            \
     if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
     FTLM_LAUNCH(k, grid, 256, sm, s, p, (const R*)v, (const R*)qp, (R*)y);                                \
   } while (0)
-  if (c->mode == FTLM_INDEX_CLT) { if (fused) LAUNCH(FTLM_INDEX_CLT, true); else LAUNCH(FTLM_INDEX_CLT, false); }
-  else { if (fused) LAUNCH(FTLM_INDEX_CR, true); else LAUNCH(FTLM_INDEX_CR, false); }
+#define LAUNCHB(MODE)                                                                            \
+  do {                                                                                           \
+    if (!fused) LAUNCH(MODE, false, 1);                                                          \
+    else if (batch == 1) LAUNCH(MODE, true, 1);                                                  \
+    else if (batch == 2) LAUNCH(MODE, true, 2);                                                  \
+    else if (batch == 4) LAUNCH(MODE, true, 4);                                                  \
+    else { ftlm_set_error("ROW: batch must be 1, 2 or 4 (got %d)", batch); return FTLM_EINVAL; } \
+  } while (0)
+  if (c->mode == FTLM_INDEX_CLT) LAUNCHB(FTLM_INDEX_CLT); else LAUNCHB(FTLM_INDEX_CR);
+#undef LAUNCHB
 #undef LAUNCH
   CK(cudaGetLastError());
   return FTLM_OK;
@@ -251,16 +281,16 @@ int launch_hv(ftlm_ctx* c, const RowParams& p, const void* v, const void* qp, vo
 
 }  // namespace
 
-int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s) {
+int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, int batch, cudaStream_t s) {
   RowParams p = make_params(c);
   if (c->prec == FTLM_FP32) {
-    if (!c->lab64) return launch_hv<float, uint32_t, uint32_t>(c, p, v, qprev, y, fused, s);
-    if (!c->idx64) return launch_hv<float, uint64_t, uint32_t>(c, p, v, qprev, y, fused, s);
-    return launch_hv<float, uint64_t, uint64_t>(c, p, v, qprev, y, fused, s);
+    if (!c->lab64) return launch_hv<float, uint32_t, uint32_t>(c, p, v, qprev, y, fused, batch, s);
+    if (!c->idx64) return launch_hv<float, uint64_t, uint32_t>(c, p, v, qprev, y, fused, batch, s);
+    return launch_hv<float, uint64_t, uint64_t>(c, p, v, qprev, y, fused, batch, s);
   } else {
-    if (!c->lab64) return launch_hv<double, uint32_t, uint32_t>(c, p, v, qprev, y, fused, s);
-    if (!c->idx64) return launch_hv<double, uint64_t, uint32_t>(c, p, v, qprev, y, fused, s);
-    return launch_hv<double, uint64_t, uint64_t>(c, p, v, qprev, y, fused, s);
+    if (!c->lab64) return launch_hv<double, uint32_t, uint32_t>(c, p, v, qprev, y, fused, batch, s);
+    if (!c->idx64) return launch_hv<double, uint64_t, uint32_t>(c, p, v, qprev, y, fused, batch, s);
+    return launch_hv<double, uint64_t, uint64_t>(c, p, v, qprev, y, fused, batch, s);
   }
 }
 

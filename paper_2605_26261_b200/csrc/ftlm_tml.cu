@@ -936,7 +936,7 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
   P->blob_bytes = (int)blob.size();
   P->h_bond_class = bclass; P->h_bond_entry = bentry;
   c->tml = P;
-  if (tml_config(c, P, 1).smem == 0) { c->tml = nullptr; ftlm_passb_plan_destroy(c); delete P; return unusable("tables + tile exceed shared memory"); }
+  if (tml_config(c, P, c->batch).smem == 0) { c->tml = nullptr; ftlm_passb_plan_destroy(c); delete P; return unusable("tables + tile exceed shared memory"); }
   // ---- upload ----------------------------------------------------------------------------------
   P->partials_batch = 4;
   auto up = [&](void** d, const void* h, size_t bytes) -> bool {
@@ -972,9 +972,9 @@ int64_t ftlm_tml_info(const ftlm_ctx* c, const char* key) {
     return (int64_t)t->h_bond_class[(size_t)b] | ((int64_t)t->h_bond_entry[(size_t)b] << 8);
   }
   if (!strcmp(key, "tml_m")) return t->m;
-  if (!strcmp(key, "tml_smem")) return (int64_t)tml_config(c, t, 1).smem;
-  if (!strcmp(key, "tml_ctas_per_sm")) return tml_config(c, t, 1).ctas;
-  if (!strcmp(key, "tml_threads")) return tml_config(c, t, 1).threads;
+  if (!strcmp(key, "tml_smem")) return (int64_t)tml_config(c, t, c->batch).smem;
+  if (!strcmp(key, "tml_ctas_per_sm")) return tml_config(c, t, c->batch).ctas;
+  if (!strcmp(key, "tml_threads")) return tml_config(c, t, c->batch).threads;
   if (!strcmp(key, "tml_max_batch")) { int b = 4; while (b > 1 && tml_config(c, t, b).smem == 0) b >>= 1; return b; }
   if (!strcmp(key, "tml_n_ll")) return t->n_ll;
   if (!strcmp(key, "tml_n_mm")) return t->n_mm;

@@ -27,7 +27,7 @@ EXPORTS = [
     "ftlm_create", "ftlm_destroy", "ftlm_dim", "ftlm_set_option", "ftlm_get_option", "ftlm_table_bytes",
     "ftlm_clt_read", "ftlm_index_of", "ftlm_state_of", "ftlm_neighbors", "ftlm_apply_H",
     "ftlm_apply_H_host", "ftlm_fill_random", "ftlm_chain_begin", "ftlm_chain_steps", "ftlm_chain_end",
-    "ftlm_chain_profile", "ftlm_autotune", "ftlm_lanczos", "ftlm_lanczos_host", "ftlm_tridiag_eig", "ftlm_thermo",
+    "ftlm_chain_begin_batch", "ftlm_chain_end_batch", "ftlm_chain_profile", "ftlm_autotune", "ftlm_lanczos", "ftlm_lanczos_host", "ftlm_tridiag_eig", "ftlm_thermo",
     "ftlm_last_error", "ftlm_version",
 ]
 
@@ -178,6 +178,19 @@ def ftlm_chain_end(ctx, cap: int = MAX_STEPS, stream=None):
     _check(lib().ftlm_chain_end(ctx, _hp(a, C.c_double), _hp(b, C.c_double), C.c_int(cap), C.byref(m), _stream(stream)))
     k = min(m.value, cap)
     return a[:k].copy(), b[: max(k - 1, 0)].copy(), m.value
+
+
+def ftlm_chain_begin_batch(ctx, seed: int, r0: int, batch: int, stream=None):
+    _check(lib().ftlm_chain_begin_batch(ctx, C.c_uint64(seed), C.c_int(r0), C.c_int(batch), _stream(stream)))
+
+
+def ftlm_chain_end_batch(ctx, batch: int, cap: int = MAX_STEPS, stream=None):
+    """Returns (alpha[batch, cap], beta[batch, cap], m_eff[batch]) of the batch in progress."""
+    a = np.zeros((batch, cap), dtype=np.float64)
+    b = np.zeros((batch, cap), dtype=np.float64)
+    m = np.zeros(batch, dtype=np.int32)
+    _check(lib().ftlm_chain_end_batch(ctx, _hp(a, C.c_double), _hp(b, C.c_double), C.c_int(cap), _hp(m, C.c_int), _stream(stream)))
+    return a, b, m
 
 
 def ftlm_chain_profile(ctx, nsteps: int, stream=None):

@@ -110,6 +110,32 @@ def main():
             res["lanczos_dalpha"], res["lanczos_dbeta"] = da, db
             res["m_eff"] = int(out["m_eff"][0])
             res["ok"] = res["ok"] and da <= tol and db <= tol
+        if "batch" in spec:
+            # batched chains (L207, L309): R chains in groups of B on interleaved vectors; every chain must be
+            # bit-identical to the same chain run alone (same kernel, same tile split) and agree with the oracle
+            R, B = spec["batch"]
+            m = min(spec.get("steps", 10), D)
+            c.set("batch", 1)
+            one = c.lanczos(W.SEED_VECTORS, R, m)
+            c.set("batch", B)
+            res["batch_split"] = [c.get("tml_w"), c.get("tml_m"), c.get("kernel")]
+            many = c.lanczos(W.SEED_VECTORS, R, m)
+            same = all(np.array_equal(one[k], many[k]) for k in ("alpha", "beta", "m_eff", "theta", "weight"))
+            res["batch_identical"] = bool(same)
+            res["batch_m_eff"] = [int(x) for x in many["m_eff"]]
+            worst = 0.0
+            tol = 1e-9 if prec == "fp64" else 2e-4
+            for r in range(R):
+                q1 = fo.start_vector(W.SEED_VECTORS, n_up, r, D)
+                a, b = fo.lanczos(lambda x: fo.apply_H(basis, w.N, w.bond_i, w.bond_j, w.J, h, n_up, x), q1, m)[:2]
+                k = min(int(many["m_eff"][r]), len(a), 6)
+                if k:
+                    worst = max(worst, float(np.max(np.abs(many["alpha"][r][:k] - np.asarray(a)[:k]))))
+                if k > 1:
+                    worst = max(worst, float(np.max(np.abs(many["beta"][r][:k - 1] - np.asarray(b)[:k - 1]))))
+            res["batch_vs_oracle"] = worst
+            res["ok"] = res["ok"] and same and worst <= tol
+            c.set("batch", 1)
     res["ok"] = bool(res["ok"])
     print(json.dumps(res))
 

@@ -233,6 +233,22 @@ def test_emu_result_does_not_depend_on_thread_schedule(order):
     assert res["hv_relerr"] == ref["hv_relerr"] and res["lanczos_dalpha"] == ref["lanczos_dalpha"]
 
 
+@pytest.mark.parametrize("spec", [
+    {"wl": "ring12j", "n_up": 6, "mode": "cr", "prec": "fp64", "options": [["kernel", 1]], "batch": [5, 4]},
+    {"wl": "ring16", "n_up": 15, "mode": "clt", "prec": "fp32", "options": [["kernel", 1]], "batch": [4, 4], "steps": 16},   # D = 16: breakdown at step 9
+    {"wl": "ring16j", "n_up": 8, "mode": "clt", "prec": "fp32", "options": [["tml_split", 6 | (4 << 8)], ["kernel", 3]], "batch": [6, 4]},
+    {"wl": "rand14_30_3", "n_up": 7, "mode": "cr", "prec": "fp64", "options": [["tml_split", 5 | (5 << 8)], ["kernel", 3]], "batch": [3, 2]},
+])
+def test_emu_batched_chains_are_bit_identical_to_single_chains(spec):
+    """SURVEY 8(f)-1, PAPER.md L207 / L309: R chains advanced in groups of B on interleaved vectors through
+    ftlm_lanczos (ROW and TML kernels): alpha, beta, m_eff, theta, weight of every chain bit-identical to the same
+    chain run alone with the same kernel and split, and the first coefficients equal to the oracle's."""
+    res = run_case(dict(spec, what=[]))
+    assert res["batch_identical"] and len(res["batch_m_eff"]) == spec["batch"][0]
+    if spec["wl"] == "ring16":
+        assert max(res["batch_m_eff"]) < 16              # the Krylov space of this sector is exhausted early (reading 10)
+
+
 def test_bench_candidates_are_valid_option_lists():
     """Every configuration bench.py can select (its CANDIDATES table = the names ftlm_autotune reports) must be a list of
     options the library accepts, on the bench sector itself (plans only; nothing is launched)."""
