@@ -197,6 +197,25 @@ int ftlm_thermo(int n_sec, const int64_t* dim, const double* Mz, const double* m
                 const double* T, double g, double* E_ref, double* Zs, double* E, double* C,
                 double* chi);
 
+/* ---- host diagnostics ------------------------------------------------------ */
+
+/* Ghost diagnostic of one chain (section 3.2): theta/weight as ftlm_tridiag_eig; ell[k] = min_j |theta_k -
+ * theta^(1)_j| with T^(1) = T without its first row and column (Cullum-Willoughby, Eq. 25); ghost[k] = 1
+ * iff ell[k] < tau, tau = C_tau * 2^-24 * (theta_max - theta_min) (FP32 unit roundoff for both precisions, L262);
+ * cluster[k] = id (ascending from 0) of the cluster of Ritz values chained by gaps <= tau and cluster_weight[k] the
+ * summed weight of that cluster (L270); F[k] = sum_{k' <= k} weight[k'] (Eq. 23).  All arrays host, length m,
+ * caller-owned; ell, ghost, cluster, cluster_weight, F, tau may be NULL.  m = 1: ell = +inf. */
+int ftlm_ghost_diagnostic(int m, const double* alpha, const double* beta, double C_tau, double* theta,
+                          double* weight, double* ell, int* ghost, int* cluster, double* cluster_weight,
+                          double* F, double* tau);
+
+/* Eq. 22 (L225-L228): samples[s*nT + i] = estimate of an observable from seed set s at temperature i;
+ * mean[i] and sigma[i] = sqrt((1/N_s) sum_s (O_s - mean)^2). */
+int ftlm_sigma_emp(int n_seeds, int nT, const double* samples, double* mean, double* sigma);
+
+/* L230: sigma_theo[i] = |O[i]| / sqrt(Z_eff[i]), Z_eff = Tr exp(-(H - E_0)/T) (= Zs of ftlm_thermo). */
+int ftlm_sigma_theo(int nT, const double* O, const double* Z_eff, double* sigma);
+
 const char* ftlm_last_error(void);
 const char* ftlm_version(void);
 

@@ -485,3 +485,48 @@ def ftlm_run(N, bond_i, bond_j, J, h, N_up_list, R, n_steps, seed, T_grid, tol=1
         Mz = N_up - N / 2.0
         secs.append(dict(dim=D, Mz=Mz, mult=(1 if Mz == 0 else 2), chains=chains))
     return thermo(secs, T_grid), secs, coeffs
+
+
+# --------------------------------------------------------------------------------------
+# Diagnostics: ghost flags, cluster weights, stochastic error estimates
+# --------------------------------------------------------------------------------------
+
+U_FP32 = 2.0 ** -24
+
+
+def ghost_diagnostic(alpha, beta, C_tau: float = 1.0):
+    """Cullum-Willoughby test as the paper states it (L258-L262, Eq. 25): T^(1) = T without its first row and
+    column, l_k = min_j |theta_k - theta^(1)_j|, ghost iff l_k < tau, tau = C_tau u_FP32 W_T with
+    W_T = theta_max - theta_min (one tolerance for both precisions).  Clusters (L270): theta_k and theta_l belong
+    together whenever |theta_k - theta_l| <= tau (chains of such neighbours join); the meaningful weight of a
+    cluster is the sum of its members' weights.  Also the cumulative spectral weight F(theta_k) of Eq. 23 (L248).
+    Returns dict(theta, weight, ell, tau, ghost (bool), cluster (id per k, ascending), cluster_weight (per k:
+    the total weight of k's cluster), F)."""
+    theta, w = ritz(alpha, beta)
+    m = len(theta)
+    if m > 1:
+        theta1, _ = ritz(np.asarray(alpha)[1:], np.asarray(beta)[1:m - 1] if m > 2 else [])
+        ell = np.min(np.abs(theta[:, None] - theta1[None, :]), axis=1)
+    else:
+        ell = np.full(m, np.inf)
+    tau = C_tau * U_FP32 * (theta[-1] - theta[0]) if m else 0.0
+    ghost = ell < tau
+    cluster = np.zeros(m, dtype=np.int64)
+    for k in range(1, m):
+        cluster[k] = cluster[k - 1] + (0 if theta[k] - theta[k - 1] <= tau else 1)
+    cw = np.array([w[cluster == cluster[k]].sum() for k in range(m)])
+    return dict(theta=theta, weight=w, ell=ell, tau=tau, ghost=ghost, cluster=cluster, cluster_weight=cw, F=np.cumsum(w))
+
+
+def sigma_emp(samples):
+    """Eq. 22 (L225-L228): samples[s][i] = FTLM estimate of the observable at seed set s and temperature i;
+    sigma_emp = sqrt((1/N_s) sum_s (O_s - mean)^2) (population form, as printed).  Returns (mean, sigma)."""
+    a = np.asarray(samples, dtype=np.float64)
+    mean = a.mean(axis=0)
+    return mean, np.sqrt(((a - mean[None, :]) ** 2).mean(axis=0))
+
+
+def sigma_theo(O, Z_eff):
+    """L230: sigma_theo = O / sqrt(Z_eff), Z_eff = Tr exp(-(H - E_0)/T) (here: the FTLM estimate Zs of `thermo`,
+    whose reference energy is the lowest Ritz value)."""
+    return np.abs(np.asarray(O, dtype=np.float64)) / np.sqrt(np.asarray(Z_eff, dtype=np.float64))

@@ -108,3 +108,71 @@ extern "C" int ftlm_thermo(int n_sec, const int64_t* dim, const double* Mz, cons
   }
   return FTLM_OK;
 }
+
+// ---- host diagnostics ------------------------------------------------------------
+// Cullum-Willoughby ghost test (Eq. 25) and cluster weights (L270), cumulative spectral weight
+// (Eq. 23).  T^(1) is T without its first row and column; l_k = min_j |theta_k - theta^(1)_j|; a Ritz value is
+// flagged when l_k < tau = C_tau u_FP32 (theta_max - theta_min).  Ritz values closer than tau (chains of them) form
+// one cluster, whose weight is the sum of its members' weights.
+extern "C" int ftlm_ghost_diagnostic(int m, const double* alpha, const double* beta, double C_tau, double* theta,
+                                     double* weight, double* ell, int* ghost, int* cluster, double* cluster_weight,
+                                     double* F, double* tau_out) {
+  if (m < 1 || !alpha || (m > 1 && !beta) || !theta || !weight || !(C_tau > 0.0)) {
+    ftlm_set_error("ftlm_ghost_diagnostic: bad argument"); return FTLM_EINVAL;
+  }
+  int rc = ftlm_tridiag_eig(m, alpha, beta, theta, weight);
+  if (rc != FTLM_OK) return rc;
+  std::vector<double> th1((size_t)(m > 1 ? m - 1 : 0)), w1(th1.size());
+  if (m > 1) {
+    rc = ftlm_tridiag_eig(m - 1, alpha + 1, beta + 1, th1.data(), w1.data());
+    if (rc != FTLM_OK) return rc;
+  }
+  const double tau = C_tau * 5.9604644775390625e-8 * (theta[m - 1] - theta[0]);
+  if (tau_out) *tau_out = tau;
+  size_t j = 0;                                          // both lists ascend: the nearest theta^(1) moves forward only
+  for (int k = 0; k < m; ++k) {
+    double l = INFINITY;
+    if (m > 1) {
+      while (j + 1 < th1.size() && th1[j + 1] <= theta[k]) ++j;
+      l = std::fabs(theta[k] - th1[j]);
+      if (j + 1 < th1.size()) l = std::min(l, std::fabs(theta[k] - th1[j + 1]));
+    }
+    if (ell) ell[k] = l;
+    if (ghost) ghost[k] = l < tau ? 1 : 0;
+  }
+  int id = 0, first = 0;
+  double acc = 0.0, run = 0.0;
+  for (int k = 0; k <= m; ++k) {
+    if (k == m || (k > 0 && theta[k] - theta[k - 1] > tau)) {      // cluster [first, k) ends
+      for (int q = first; q < k; ++q) { if (cluster) cluster[q] = id; if (cluster_weight) cluster_weight[q] = acc; }
+      ++id; first = k; acc = 0.0;
+    }
+    if (k < m) { acc += weight[k]; run += weight[k]; if (F) F[k] = run; }
+  }
+  return FTLM_OK;
+}
+
+// Eq. 22 (L225-L228): mean and population standard deviation over N_s seed sets, per temperature.
+extern "C" int ftlm_sigma_emp(int n_seeds, int nT, const double* samples, double* mean, double* sigma) {
+  if (n_seeds < 1 || nT < 0 || (nT > 0 && (!samples || !mean || !sigma))) { ftlm_set_error("ftlm_sigma_emp: bad argument"); return FTLM_EINVAL; }
+  for (int i = 0; i < nT; ++i) {
+    double s = 0.0;
+    for (int q = 0; q < n_seeds; ++q) s += samples[(size_t)q * nT + i];
+    const double mu = s / n_seeds;
+    double v = 0.0;
+    for (int q = 0; q < n_seeds; ++q) { const double d = samples[(size_t)q * nT + i] - mu; v += d * d; }
+    mean[i] = mu;
+    sigma[i] = std::sqrt(v / n_seeds);
+  }
+  return FTLM_OK;
+}
+
+// L230: sigma_theo = |O| / sqrt(Z_eff), Z_eff = Tr exp(-(H - E_0)/T)  (ftlm_thermo's Zs).
+extern "C" int ftlm_sigma_theo(int nT, const double* O, const double* Z_eff, double* sigma) {
+  if (nT < 0 || (nT > 0 && (!O || !Z_eff || !sigma))) { ftlm_set_error("ftlm_sigma_theo: bad argument"); return FTLM_EINVAL; }
+  for (int i = 0; i < nT; ++i) {
+    if (!(Z_eff[i] > 0.0)) { ftlm_set_error("ftlm_sigma_theo: Z_eff[%d] <= 0", i); return FTLM_EINVAL; }
+    sigma[i] = std::fabs(O[i]) / std::sqrt(Z_eff[i]);
+  }
+  return FTLM_OK;
+}

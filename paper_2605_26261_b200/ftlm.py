@@ -28,6 +28,7 @@ EXPORTS = [
     "ftlm_clt_read", "ftlm_index_of", "ftlm_state_of", "ftlm_neighbors", "ftlm_apply_H",
     "ftlm_apply_H_host", "ftlm_fill_random", "ftlm_chain_begin", "ftlm_chain_steps", "ftlm_chain_end",
     "ftlm_chain_begin_batch", "ftlm_chain_end_batch", "ftlm_chain_profile", "ftlm_autotune", "ftlm_lanczos", "ftlm_lanczos_host", "ftlm_tridiag_eig", "ftlm_thermo",
+    "ftlm_ghost_diagnostic", "ftlm_sigma_emp", "ftlm_sigma_theo",
     "ftlm_last_error", "ftlm_version",
 ]
 
@@ -264,3 +265,33 @@ def ftlm_thermo(dim, Mz, mult, R, m_eff, theta, weight, T, g=2.0):
                              _hp(weight, C.c_double), C.c_int(nT), _hp(T, C.c_double), C.c_double(g), C.byref(eref),
                              _hp(Zs, C.c_double), _hp(E, C.c_double), _hp(Cv, C.c_double), _hp(chi, C.c_double)))
     return dict(E_ref=eref.value, Zs=Zs, E=E, C=Cv, chi=chi)
+
+
+def ftlm_ghost_diagnostic(alpha, beta, C_tau: float = 1.0) -> dict:
+    """Host: Cullum-Willoughby ghost flags, clusters and cluster weights of one chain (include/ftlm.h)."""
+    a = np.ascontiguousarray(alpha, dtype=np.float64)
+    m = a.shape[0]
+    b = np.zeros(max(m, 1), dtype=np.float64)
+    b[: max(m - 1, 0)] = np.asarray(beta, dtype=np.float64)[: max(m - 1, 0)]
+    th, w, ell, cw, F = (np.zeros(m) for _ in range(5))
+    gh, cl = np.zeros(m, dtype=np.int32), np.zeros(m, dtype=np.int32)
+    tau = C.c_double(0)
+    _check(lib().ftlm_ghost_diagnostic(C.c_int(m), _hp(a, C.c_double), _hp(b, C.c_double), C.c_double(C_tau),
+                                       _hp(th, C.c_double), _hp(w, C.c_double), _hp(ell, C.c_double), _hp(gh, C.c_int),
+                                       _hp(cl, C.c_int), _hp(cw, C.c_double), _hp(F, C.c_double), C.byref(tau)))
+    return dict(theta=th, weight=w, ell=ell, ghost=gh.astype(bool), cluster=cl, cluster_weight=cw, F=F, tau=tau.value)
+
+
+def ftlm_sigma_emp(samples):
+    a = np.ascontiguousarray(samples, dtype=np.float64)
+    mean, sig = np.zeros(a.shape[1]), np.zeros(a.shape[1])
+    _check(lib().ftlm_sigma_emp(C.c_int(a.shape[0]), C.c_int(a.shape[1]), _hp(a, C.c_double), _hp(mean, C.c_double), _hp(sig, C.c_double)))
+    return mean, sig
+
+
+def ftlm_sigma_theo(O, Z_eff):
+    o = np.ascontiguousarray(O, dtype=np.float64)
+    z = np.ascontiguousarray(Z_eff, dtype=np.float64)
+    sig = np.zeros_like(o)
+    _check(lib().ftlm_sigma_theo(C.c_int(o.shape[0]), _hp(o, C.c_double), _hp(z, C.c_double), _hp(sig, C.c_double)))
+    return sig
