@@ -158,6 +158,40 @@ def icosidodecahedron(random_bonds: bool = False, seed_J: int = SEED_J, **kw) ->
     return _mk("icosidodecahedron" + ("_randJ" if random_bonds else ""), 30, pairs, J, **kw)
 
 
+def dodecahedron(**kw) -> Workload:
+    """N=20 dodecahedron (Fig. 3 e-f): vertices (+-1, +-1, +-1) and the cyclic permutations of
+    (0, +-1/phi, +-phi), numbered in that order; bonds = the 30 pairs at the edge length 2/phi; every site has
+    degree 3, the faces are pentagons.  The paper runs all M sectors with R = 100, N_L = 100."""
+    phi = (1.0 + math.sqrt(5.0)) / 2.0
+    V = [(a, b, c) for a in (1.0, -1.0) for b in (1.0, -1.0) for c in (1.0, -1.0)]
+    for perm in range(3):
+        for s1 in (1.0, -1.0):
+            for s2 in (1.0, -1.0):
+                base = (0.0, s1 / phi, s2 * phi)
+                V.append(tuple(base[(k - perm) % 3] for k in range(3)))
+    pairs = []
+    for a in range(20):
+        for b in range(a + 1, 20):
+            d2 = sum((V[a][k] - V[b][k]) ** 2 for k in range(3))
+            if abs(d2 - (2.0 / phi) ** 2) < 1e-9:
+                pairs.append((a, b))
+    assert len(pairs) == 30
+    kw.setdefault("sectors", list(range(10, 21)))
+    kw.setdefault("R", 100)
+    kw.setdefault("n_steps", 100)
+    return _mk("dodecahedron", 20, pairs, **kw)
+
+
+def paper_workload(name: str) -> Workload:
+    """The paper's second spin-1/2 systems (Fig. 3 c-f): "ring20" and "dodecahedron",
+    all M >= 0 sectors, R = 100 random vectors per sector, N_L = 100."""
+    if name == "ring20":
+        return ring(20, R=100, n_steps=100, note="N=20 ring, all sectors (Fig. 3 c-d)")
+    if name == "dodecahedron":
+        return dodecahedron(note="N=20 dodecahedron, all sectors (Fig. 3 e-f)")
+    raise ValueError(name)
+
+
 def relabel(w: Workload, perm) -> Workload:
     """Renumber sites: old site s becomes perm[s].  Same physics (reading 30)."""
     perm = np.asarray(perm, dtype=np.int64)

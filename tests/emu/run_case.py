@@ -45,6 +45,8 @@ def workload(name):
         return W.triangular(int(a), int(b))
     if name == "icosahedron":
         return W.icosahedron()
+    if name in ("dodecahedron", "ring20"):
+        return W.paper_workload(name)
     if name.startswith("rand"):                      # randN_E_seed : random graph, random J
         n, e, s = (int(x) for x in name[4:].split("_"))
         rng = np.random.default_rng(s)

@@ -42,6 +42,8 @@ def workload(spec):
     if name.startswith("tri"):
         a, b = name[3:].split("x")
         return W.triangular(int(a), int(b))
+    if name in ("dodecahedron", "ring20"):
+        return W.paper_workload(name)
     if name.startswith("rand"):                          # randN_E_seed: random graph, random J
         n, e, s = (int(x) for x in name[4:].split("_"))
         rng = np.random.default_rng(s)

@@ -249,6 +249,18 @@ def test_emu_batched_chains_are_bit_identical_to_single_chains(spec):
         assert max(res["batch_m_eff"]) < 16              # the Krylov space of this sector is exhausted early (reading 10)
 
 
+@pytest.mark.parametrize("n_up,mode,prec,opts", [
+    (4, "clt", "fp32", [["kernel", 1]]),
+    (5, "cr", "fp32", [["tml_split", 6 | (5 << 8)], ["kernel", 3]]),
+    (6, "clt", "fp64", [["tml_split", 7 | (6 << 8)], ["passb", 1], ["passb_lo_min", 6], ["kernel", 3]]),
+])
+def test_emu_dodecahedron(n_up, mode, prec, opts):
+    """SURVEY 8(f)-2 (Fig. 3 e-f): sectors of the N = 20 dodecahedron through the ROW kernel, the TML
+    kernel and TML + windows: neighbour indices bit-exact, H.v and the first Lanczos coefficients against the oracle."""
+    run_case({"wl": "dodecahedron", "n_up": n_up, "mode": mode, "prec": prec, "options": opts,
+              "what": ["neighbors", "apply", "lanczos"], "steps": 6}, timeout=1200)
+
+
 def test_bench_candidates_are_valid_option_lists():
     """Every configuration bench.py can select (its CANDIDATES table = the names ftlm_autotune reports) must be a list of
     options the library accepts, on the bench sector itself (plans only; nothing is launched)."""
