@@ -35,7 +35,11 @@ extern "C" {
 typedef struct ftlm_ctx ftlm_ctx;
 
 enum { FTLM_OK = 0, FTLM_EINVAL = 1, FTLM_ENOMEM = 2, FTLM_ECUDA = 3, FTLM_EUNSUPPORTED = 4 };
-enum { FTLM_INDEX_CLT = 0, FTLM_INDEX_CR = 1 };
+/* State-to-index strategies: the paper's compressed lookup table (Alg. 2), combinatorial ranking (Alg. 1,
+ * L121-L146), and Lin's two half-system tables (L119: index = Ja[n >> h] + Jb[n & (2^h - 1)], h = N / 2, in the same
+ * ascending-label order; N <= 48; served by the thread-per-row kernel only - the paper's own Lin kernel is its
+ * comparison row kernel, "roughly half the throughput of the CLT-based variant"). */
+enum { FTLM_INDEX_CLT = 0, FTLM_INDEX_CR = 1, FTLM_INDEX_LIN = 2 };
 enum { FTLM_FP32 = 0, FTLM_FP64 = 1 };
 
 /* Kernel variants selectable with ftlm_set_option("kernel", ...).
@@ -51,8 +55,8 @@ enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_TML = 3 };
  * Eq. 16 at d = 2), bond masks and couplings, and in CLT mode the table of (M_b, C_b) pairs of
  * L150-L154 / Eq. 18.  All array arguments are host pointers and are copied.
  *   N in [1, 62]; 0 <= bond_i[b] != bond_j[b] < N (duplicates are legal and add); N_up in
- *   [0, N]; n_bonds in [0, 4096].  CLT needs N <= 32.
- * Errors: FTLM_EINVAL (bad argument), FTLM_EUNSUPPORTED (CLT with N > 32),
+ *   [0, N]; n_bonds in [0, 4096].  CLT needs N <= 32, LIN needs N <= 48.
+ * Errors: FTLM_EINVAL (bad argument), FTLM_EUNSUPPORTED (CLT with N > 32, LIN with N > 48),
  *         FTLM_ENOMEM (table does not fit), FTLM_ECUDA (no device / CUDA failure). */
 int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bond_i, const int32_t* bond_j,
                 const double* J, double h, int N_up, int index_mode, int precision, int device);

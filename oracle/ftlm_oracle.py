@@ -189,6 +189,34 @@ def clt_lookup_vec(n, M: np.ndarray, C: np.ndarray) -> np.ndarray:
     return np.where(inside, C[b] + np.bitwise_count(low).astype(np.int64), -1).astype(np.int64)
 
 
+def lin_tables(basis: np.ndarray, N: int):
+    """Lin's two-table index (L119: "partitioning the system into two halves, with rank tables of size approximately
+    d^(N/2) for each half"), from the explicit basis in ascending order (L154): label n = (a << h) | b with
+    h = N // 2 low positions; index(n) = Ja[a] + Jb[b].  Ja[a] = number of sector labels whose high half is smaller
+    than a (labels with equal high half are contiguous); Jb[b] = position of b among the h-bit words of the same
+    popcount in ascending order (the labels sharing a high half differ only in b and all have that popcount).
+    Built by counting, not by a formula."""
+    h = N // 2
+    hi = (basis >> np.uint64(h)).astype(np.int64)
+    Ja = np.concatenate(([0], np.cumsum(np.bincount(hi, minlength=1 << (N - h)))))[: 1 << (N - h)].astype(np.int64)
+    words = np.arange(1 << h, dtype=np.uint64)
+    pc = popcount(words)
+    Jb = np.zeros(1 << h, dtype=np.int64)
+    for k in range(h + 1):
+        sel = np.flatnonzero(pc == k)                   # ascending
+        Jb[sel] = np.arange(sel.shape[0])
+    return h, Ja, Jb
+
+
+def lin_lookup_vec(n, N: int, N_up: int, h: int, Ja: np.ndarray, Jb: np.ndarray) -> np.ndarray:
+    """index = Ja[n >> h] + Jb[n & (2^h - 1)], -1 for labels outside the sector (two table reads and a popcount)."""
+    n = np.asarray(n, dtype=np.uint64)
+    ok = (popcount(n) == N_up) & ((n >> np.uint64(N)) == 0) if N < 64 else (popcount(n) == N_up)
+    a = (n >> np.uint64(h)).astype(np.int64) & ((1 << (N - h)) - 1)
+    b = (n & np.uint64((1 << h) - 1)).astype(np.int64)
+    return np.where(ok, Ja[a] + Jb[b], -1).astype(np.int64)
+
+
 def clt_bytes(N: int) -> int:
     """Eq. 21 (L177-L181): 8 bytes per block of 32 labels."""
     return 8 * (((1 << N) + 31) // 32)

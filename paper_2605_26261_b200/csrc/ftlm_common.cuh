@@ -92,6 +92,9 @@ struct ftlm_ctx {
   BondDev* d_bonds = nullptr;
   uint2* d_clt = nullptr;          // {M_b, C_b}
   int64_t n_clt = 0;
+  uint64_t* d_lin_hi = nullptr;    // LIN mode: Ja[2^(N-h)] = number of sector labels with a smaller high half
+  uint32_t* d_lin_lo = nullptr;    // LIN mode: Jb[2^h] = rank of the low half among the h-bit words of equal popcount
+  int lin_h = 0;                   // low-half width N / 2
   std::vector<BondDev> bonds;
   std::vector<uint64_t> binom64;   // host copy
 

@@ -323,7 +323,7 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
   if (n_bonds < 0 || n_bonds > FTLM_MAX_BONDS || (n_bonds > 0 && (!bond_i || !bond_j || !J))) {
     ftlm_set_error("ftlm_create: bad bond list (n_bonds=%d)", n_bonds); return FTLM_EINVAL;
   }
-  if (index_mode != FTLM_INDEX_CLT && index_mode != FTLM_INDEX_CR) { ftlm_set_error("ftlm_create: bad index_mode %d", index_mode); return FTLM_EINVAL; }
+  if (index_mode != FTLM_INDEX_CLT && index_mode != FTLM_INDEX_CR && index_mode != FTLM_INDEX_LIN) { ftlm_set_error("ftlm_create: bad index_mode %d", index_mode); return FTLM_EINVAL; }
   if (precision != FTLM_FP32 && precision != FTLM_FP64) { ftlm_set_error("ftlm_create: bad precision %d", precision); return FTLM_EINVAL; }
   for (int b = 0; b < n_bonds; ++b) {
     if (bond_i[b] < 0 || bond_i[b] >= N || bond_j[b] < 0 || bond_j[b] >= N || bond_i[b] == bond_j[b]) {
@@ -332,6 +332,7 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
     }
   }
   if (index_mode == FTLM_INDEX_CLT && N > 32) { ftlm_set_error("ftlm_create: CLT needs N <= 32 (got %d); use CR", N); return FTLM_EUNSUPPORTED; }
+  if (index_mode == FTLM_INDEX_LIN && N > 48) { ftlm_set_error("ftlm_create: LIN needs N <= 48 (got %d); use CR", N); return FTLM_EUNSUPPORTED; }
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
   if (e != cudaSuccess || ndev <= 0) {
@@ -393,6 +394,25 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
     FTLM_LAUNCH(clt_build_kernel, grid, 256, 0, 0, c->d_clt, c->n_clt, N, N_up, c->d_binom64);
     CKF(cudaGetLastError());
   }
+  if (index_mode == FTLM_INDEX_LIN) {
+    // Lin's two tables (L119) in the ascending-label order: Ja by a running count over the high halves
+    // (C(h, N_up - popc(a)) labels share the high half a), Jb by counting, per popcount, the low halves seen so far
+    const int h = N / 2, g = N - h;
+    c->lin_h = h;
+    std::vector<uint64_t> Ja((size_t)1 << g);
+    std::vector<uint32_t> Jb((size_t)1 << h);
+    uint64_t run = 0;
+    for (uint64_t a = 0; a < (1ull << g); ++a) {
+      Ja[(size_t)a] = run;
+      run += binom_u64(h, N_up - __builtin_popcountll(a));
+    }
+    std::vector<uint32_t> seen((size_t)h + 1, 0);
+    for (uint64_t b = 0; b < (1ull << h); ++b) Jb[(size_t)b] = seen[(size_t)__builtin_popcountll(b)]++;
+    CKF(ftlm_dmalloc(&c->d_lin_hi, Ja.size() * 8));
+    CKF(ftlm_dmalloc(&c->d_lin_lo, Jb.size() * 4));
+    CKF(cudaMemcpy(c->d_lin_hi, Ja.data(), Ja.size() * 8, cudaMemcpyHostToDevice));
+    CKF(cudaMemcpy(c->d_lin_lo, Jb.data(), Jb.size() * 4, cudaMemcpyHostToDevice));
+  }
   for (int k = 0; k < 4; ++k) CKF(cudaEventCreate(&c->ev[k]));
   rc = ftlm_tml_plan_create(c);
   if (rc != FTLM_OK) return fail(rc);
@@ -407,7 +427,7 @@ extern "C" int ftlm_destroy(ftlm_ctx* c) {
   cudaSetDevice(c->device);
   ftlm_tml_plan_destroy(c);
   ftlm_dfree(c->d_binom64); ftlm_dfree(c->d_binom32); ftlm_dfree(c->d_bonds); ftlm_dfree(c->d_clt);
-  ftlm_dfree(c->d_state); ftlm_dfree(c->d_partials); ftlm_dfree(c->d_ticket);
+  ftlm_dfree(c->d_state); ftlm_dfree(c->d_partials); ftlm_dfree(c->d_ticket); ftlm_dfree(c->d_lin_hi); ftlm_dfree(c->d_lin_lo);
   for (int k = 0; k < 3; ++k) ftlm_dfree(c->q[k]);
   for (int k = 0; k < 4; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
   delete c;
@@ -420,11 +440,12 @@ extern "C" int64_t ftlm_table_bytes(const ftlm_ctx* c) {
   if (!c) return -1;
   int64_t b = (int64_t)c->binom64.size() * 12 + (int64_t)c->nb * (int64_t)sizeof(BondDev);
   if (c->mode == FTLM_INDEX_CLT) b += c->n_clt * 8;
+  if (c->mode == FTLM_INDEX_LIN) b += ((int64_t)8 << (c->N - c->lin_h)) + ((int64_t)4 << c->lin_h);
   return b;
 }
 
 int ftlm_effective_kernel(const ftlm_ctx* c) {
-  if (c->kernel == FTLM_KERNEL_ROW) return FTLM_KERNEL_ROW;
+  if (c->kernel == FTLM_KERNEL_ROW || c->mode == FTLM_INDEX_LIN) return FTLM_KERNEL_ROW;   // LIN: thread-per-row kernel only
   if (c->kernel == FTLM_KERNEL_TML && c->tml) return FTLM_KERNEL_TML;
   if (c->kernel == FTLM_KERNEL_AUTO && c->tml && c->dim >= (1 << 20)) return FTLM_KERNEL_TML;
   return FTLM_KERNEL_ROW;                    // AUTO: small sectors are launch-bound, ROW is simpler
@@ -434,7 +455,7 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   if (!c || !key) { ftlm_set_error("ftlm_set_option: NULL"); return FTLM_EINVAL; }
   if (!strcmp(key, "kernel")) {
     if (value != FTLM_KERNEL_AUTO && value != FTLM_KERNEL_ROW && value != FTLM_KERNEL_TML) { ftlm_set_error("kernel must be FTLM_KERNEL_AUTO, _ROW or _TML"); return FTLM_EINVAL; }
-    if (value == FTLM_KERNEL_TML && !c->tml) { ftlm_set_error("TML kernel unavailable for this sector"); return FTLM_EUNSUPPORTED; }
+    if (value == FTLM_KERNEL_TML && (!c->tml || c->mode == FTLM_INDEX_LIN)) { ftlm_set_error("TML kernel unavailable for this sector / index mode"); return FTLM_EUNSUPPORTED; }
     c->kernel = (int)value; return FTLM_OK;
   }
   if (!strcmp(key, "tml_low_bits") || !strcmp(key, "tml_mid_bits")) {

@@ -73,8 +73,16 @@ __device__ __forceinline__ uint32_t clt_lookup(uint32_t n, const uint2* __restri
   return e.y + __popc(e.x & ((1u << (n & 31u)) - 1u));
 }
 
+// Lin's two-table lookup (L119): index = Ja[n >> h] + Jb[n & (2^h - 1)] for an in-sector label n.
+__device__ __forceinline__ uint64_t lin_lookup(uint64_t n, int h, const uint64_t* __restrict__ Ja, const uint32_t* __restrict__ Jb) {
+  return LDG(&Ja[n >> h]) + (uint64_t)LDG(&Jb[n & ((1ull << h) - 1ull)]);
+}
+
 struct RowParams {
   int N, K, nb, mode;
+  int lin_h;
+  const uint64_t* lin_hi;
+  const uint32_t* lin_lo;
   int64_t dim;
   const void* binom;       // I[(N+1)*(K+1)]
   const BondDev* bonds;
@@ -139,6 +147,7 @@ hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev,
       if (x != 0 && x != m) {                                   // antiparallel spins
         I idx;
         if (MODE == FTLM_INDEX_CLT) idx = (I)clt_lookup((uint32_t)(n ^ m), p.clt);
+        else if (MODE == FTLM_INDEX_LIN) idx = (I)lin_lookup((uint64_t)(n ^ m), p.lin_h, p.lin_hi, p.lin_lo);
         else idx = (I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom);
 #pragma unroll
         for (int c = 0; c < B; ++c) acc[c] += s_bonds[b].Jh * LDG(&v[(size_t)idx * B + c]);
@@ -184,6 +193,7 @@ neighbors_row_kernel(RowParams p, int64_t row0, int64_t nrows, int64_t* __restri
       int64_t idx = -1;
       if (x != 0 && x != m) {
         if (MODE == FTLM_INDEX_CLT) idx = (int64_t)clt_lookup((uint32_t)(n ^ m), p.clt);
+        else if (MODE == FTLM_INDEX_LIN) idx = (int64_t)lin_lookup((uint64_t)(n ^ m), p.lin_h, p.lin_hi, p.lin_lo);
         else idx = (int64_t)(I)((I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom));
       }
       ST_G(&out[r * p.nb + b], idx);
@@ -205,6 +215,9 @@ __global__ void index_of_kernel(RowParams p, const uint64_t* __restrict__ labels
     int64_t idx;
     if (p.mode == FTLM_INDEX_CLT) {
       idx = clt_lookup_checked(lab, p.N, p.clt);
+    } else if (p.mode == FTLM_INDEX_LIN) {
+      const bool in = (lab >> p.N) == 0 && __popcll(lab) == p.K;          // N <= 48 in this mode
+      idx = in ? (int64_t)lin_lookup(lab, p.lin_h, p.lin_hi, p.lin_lo) : -1;
     } else {
       const bool in = (p.N >= 64 || (lab >> p.N) == 0) && __popcll(lab) == p.K;
       idx = in ? (int64_t)rank_alg1<L, I>((L)lab, p.N, p.K + 1, p.K, s_binom) : -1;
@@ -233,6 +246,7 @@ RowParams make_params(ftlm_ctx* c) {
   p.N = c->N; p.K = c->N_up; p.nb = c->nb; p.mode = c->mode; p.dim = c->dim;
   p.binom = c->idx64 ? (const void*)c->d_binom64 : (const void*)c->d_binom32;
   p.bonds = c->d_bonds; p.clt = c->d_clt; p.diag0 = c->diag0;
+  p.lin_h = c->lin_h; p.lin_hi = c->d_lin_hi; p.lin_lo = c->d_lin_lo;
   p.st = c->d_state; p.partials = c->d_partials; p.ticket = c->d_ticket; p.stride = c->max_blocks;
   return p;
 }
@@ -272,7 +286,7 @@ int launch_hv(ftlm_ctx* c, const RowParams& p, const void* v, const void* qp, vo
     else if (batch == 4) LAUNCH(MODE, true, 4);                                                  \
     else { ftlm_set_error("ROW: batch must be 1, 2 or 4 (got %d)", batch); return FTLM_EINVAL; } \
   } while (0)
-  if (c->mode == FTLM_INDEX_CLT) LAUNCHB(FTLM_INDEX_CLT); else LAUNCHB(FTLM_INDEX_CR);
+  if (c->mode == FTLM_INDEX_CLT) LAUNCHB(FTLM_INDEX_CLT); else if (c->mode == FTLM_INDEX_LIN) LAUNCHB(FTLM_INDEX_LIN); else LAUNCHB(FTLM_INDEX_CR);
 #undef LAUNCHB
 #undef LAUNCH
   CK(cudaGetLastError());
@@ -302,6 +316,10 @@ int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
   do {                                                                                                \
     if (c->mode == FTLM_INDEX_CLT) {                                                                  \
       auto k = neighbors_row_kernel<L, I, FTLM_INDEX_CLT>;                                            \
+      if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
+      FTLM_LAUNCH(k, grid, 256, sm, s, p, row0, nrows, d_idx);                                                 \
+    } else if (c->mode == FTLM_INDEX_LIN) {                                                           \
+      auto k = neighbors_row_kernel<L, I, FTLM_INDEX_LIN>;                                            \
       if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
       FTLM_LAUNCH(k, grid, 256, sm, s, p, row0, nrows, d_idx);                                                 \
     } else {                                                                                          \

@@ -796,6 +796,7 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced);
 
 int ftlm_tml_plan_create(ftlm_ctx* c) {
   c->tml = nullptr;
+  if (c->mode == FTLM_INDEX_LIN) return FTLM_OK;       // Lin tables serve the thread-per-row kernel only
   const int N = c->N;
   const bool forced = c->tml_low_bits != 0 || c->tml_mid_bits != 0;
   if (forced) return tml_plan_try(c, c->tml_low_bits ? c->tml_low_bits : 9, c->tml_mid_bits ? c->tml_mid_bits : 7, true);

@@ -18,7 +18,7 @@ CHECKED = os.environ.get("FTLM_CHECKED", "0") not in ("", "0")
 LIB_PATH = os.path.join(_HERE, "libftlm_checked.so" if CHECKED else "libftlm.so")
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
-INDEX_CLT, INDEX_CR = 0, 1
+INDEX_CLT, INDEX_CR, INDEX_LIN = 0, 1, 2
 FP32, FP64 = 0, 1
 KERNEL_AUTO, KERNEL_ROW, KERNEL_TML = 0, 1, 3
 MAX_STEPS = 1024

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(os.path.dirname(HERE))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-INDEX = {"clt": 0, "cr": 1}
+INDEX = {"clt": 0, "cr": 1, "lin": 2}
 PREC = {"fp32": 0, "fp64": 1}
 NDT = {"fp32": np.float32, "fp64": np.float64}
 KERNEL = {"auto": 0, "row": 1, "tml": 3}

@@ -5,7 +5,7 @@ import torch
 from paper_2605_26261_b200 import ftlm
 from hv_bound import elem_bound  # noqa: F401
 
-MODES = {"clt": ftlm.INDEX_CLT, "cr": ftlm.INDEX_CR}
+MODES = {"clt": ftlm.INDEX_CLT, "cr": ftlm.INDEX_CR, "lin": ftlm.INDEX_LIN}
 PRECS = {"fp32": ftlm.FP32, "fp64": ftlm.FP64}
 TDT = {"fp32": torch.float32, "fp64": torch.float64}
 NDT = {"fp32": np.float32, "fp64": np.float64}

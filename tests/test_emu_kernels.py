@@ -261,6 +261,44 @@ def test_emu_dodecahedron(n_up, mode, prec, opts):
               "what": ["neighbors", "apply", "lanczos"], "steps": 6}, timeout=1200)
 
 
+def test_emu_lin_two_table_index_mode():
+    """index_mode LIN through the emulated kernels: ftlm_index_of on EVERY label of the
+    full space (in-sector: the oracle's sorted-search index, else -1), ftlm_state_of round trip, neighbour lists, H.v,
+    Lanczos and batched chains on small sectors; N = 34 (64-bit labels, dim > 2^31) on sampled labels against Alg. 1."""
+    for spec in ({"wl": "ring12j", "n_up": 6, "mode": "lin", "prec": "fp64", "what": ["neighbors", "apply", "lanczos"]},
+                 {"wl": "rand15_40_5", "n_up": 7, "mode": "lin", "prec": "fp32", "what": ["neighbors", "apply", "lanczos"], "batch": [3, 2]}):
+        res = run_case(spec)
+        assert res["kernel"] == K["row"]
+    code = ("import sys, json; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+            "import numpy as np, emu_harness as E\n"
+            "from oracle import ftlm_oracle as fo\n"
+            "from paper_2605_26261_b200 import workloads as W\n"
+            "bad = 0\n"
+            "for N, n_up in ((11, 4), (12, 6), (9, 0), (9, 9)):\n"
+            "    w = W.ring(N)\n"
+            "    basis = fo.sector_basis(N, n_up)\n"
+            "    lab = np.arange(1 << N, dtype=np.uint64)\n"
+            "    with E.EmuCtx(w, n_up, 'lin', 'fp64') as c:\n"
+            "        bad += int(np.count_nonzero(c.index_of(lab) != fo.index_of_sorted(basis, lab)))\n"
+            "        bad += int(np.count_nonzero(c.state_of(np.arange(c.dim)) != basis))\n"
+            "w = W.ring(34, 1.0, 0.5)\n"
+            "rng = np.random.default_rng(3)\n"
+            "_, Dc = fo.cr_tables(34)\n"
+            "with E.EmuCtx(w, 17, 'lin', 'fp32') as c:\n"
+            "    idx = np.concatenate([[0, c.dim - 1, 2**31 - 1, 2**31, 2**32 - 1 if c.dim > 2**32 else c.dim - 2], rng.integers(0, c.dim, 500)]).astype(np.int64)\n"
+            "    lab = fo.alg1_unrank_vec(idx.astype(np.uint64), 34, 17, Dc)\n"
+            "    bad += int(np.count_nonzero(c.index_of(lab) != idx))\n"
+            "    out = rng.integers(0, 2**34, 200).astype(np.uint64)\n"
+            "    exp = np.where(fo.popcount(out) == 17, fo.alg1_rank_vec(out, 34, 17, Dc).astype(np.int64), -1)\n"
+            "    bad += int(np.count_nonzero(c.index_of(out) != exp))\n"
+            "    nb = c.neighbors(int(idx[3]), 4)\n"
+            "    bad += int((nb >= c.dim).sum())\n"
+            "print(json.dumps({'bad': bad}))\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    assert json.loads(p.stdout.strip().splitlines()[-1])["bad"] == 0
+
+
 def test_bench_candidates_are_valid_option_lists():
     """Every configuration bench.py can select (its CANDIDATES table = the names ftlm_autotune reports) must be a list of
     options the library accepts, on the bench sector itself (plans only; nothing is launched)."""

@@ -137,3 +137,22 @@ def test_counting_rank_matches_enumeration_at_N30_samples():
         n = int(basis[int(t)])
         assert fo.rank_by_counting(n, N, N_up) == int(t)
         assert fo.unrank_by_counting(int(t), N, N_up) == n
+
+
+def test_lin_two_table_map_equals_sorted_search_on_every_label():
+    """SURVEY 8(f)-3 / PAPER.md L119: Lin's two half-system tables (built by counting over the explicit basis) give the
+    ascending-order index of every in-sector label and -1 outside, for every sector of N = 9 (odd: halves 4 + 5), 12
+    and 13; table sizes are 2^(N - N//2) and 2^(N//2)."""
+    for N in (9, 12, 13):
+        all_labels = np.arange(1 << N, dtype=np.uint64)
+        for n_up in range(N + 1):
+            basis = fo.sector_basis(N, n_up)
+            h, Ja, Jb = fo.lin_tables(basis, N)
+            assert (h, Ja.shape[0], Jb.shape[0]) == (N // 2, 1 << (N - N // 2), 1 << (N // 2))
+            got = fo.lin_lookup_vec(all_labels, N, n_up, h, Ja, Jb)
+            assert (got == fo.index_of_sorted(basis, all_labels)).all()
+    # brute force on one sector: the index is the number of smaller sector labels
+    basis = fo.sector_basis(10, 4)
+    h, Ja, Jb = fo.lin_tables(basis, 10)
+    for n in basis[::7]:
+        assert fo.lin_lookup_vec([n], 10, 4, h, Ja, Jb)[0] == fo.rank_by_counting(int(n), 10, 4)
