@@ -172,6 +172,26 @@ def run_probe(args):
     mode = ftlm.INDEX_CR if (args.mode == "cr" or w.N > 32) else ftlm.INDEX_CLT
     ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, torch.cuda.current_device())
     ftlm.ftlm_set_option(ctx, "allow_unverified", 1)
+    if args.probe_stage == "batchcheck":
+        # checked library: three fused steps of `batch` interleaved chains through the TML kernel (no windows) against
+        # the same chains through the thread-per-row kernel one at a time; zero suppressed accesses
+        assert ftlm.CHECKED, "checked probe stage needs FTLM_CHECKED=1"
+        B = args.batch
+        ftlm.ftlm_set_option(ctx, "kernel", 1)
+        ref = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, B, 3)
+        ftlm.ftlm_set_option(ctx, "batch", B)
+        ftlm.ftlm_set_option(ctx, "passb", 0)
+        ok = False
+        try:
+            ftlm.ftlm_set_option(ctx, "kernel", 3)
+            got = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, B, 3)
+            ok = bool(np.abs(got["alpha"] - ref["alpha"]).max() <= 1e-4 and np.abs(got["beta"] - ref["beta"]).max() <= 1e-4)
+        except ftlm.FtlmError:
+            ok = False
+        info = ftlm.ftlm_check_info()
+        ftlm.ftlm_destroy(ctx)
+        print(json.dumps({"stage": "batchcheck", "ok": ok, "check": info}), flush=True)
+        return
     if args.probe_stage == "checked":
         assert ftlm.CHECKED, "checked probe stage needs FTLM_CHECKED=1"
         rep = ftlm.ftlm_autotune(ctx, 1)
@@ -194,6 +214,22 @@ def _child_json(cmd, env, timeout):
         if ln.startswith("{"):
             return json.loads(ln), None
     return None, f"rc={out.returncode}: {out.stderr.strip()[-300:]}"
+
+
+def probe_batch(args):
+    """batch > 1: the batched TML kernel is timed only after the checked library ran it on this device without a
+    suppressed access and in agreement with the thread-per-row kernel; else the batched thread-per-row kernel."""
+    cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--probe-stage", "batchcheck", "--config", str(args.config),
+           "--mode", args.mode, "--batch", str(args.batch)]
+    try:
+        from paper_2605_26261_b200 import build
+        build.build(checked=True)
+        d, err = _child_json(cmd, dict(os.environ, FTLM_CHECKED="1"), 1800)
+        if d and d.get("ok") and d["check"].get("check_violations") == 0:
+            return "tml", None, None
+        return "row", None, f"batch check: {err or d}"
+    except Exception as e:
+        return "row", None, f"batch check failed: {e!r}"
 
 
 def probe_choice(args):
@@ -226,10 +262,65 @@ def probe_choice(args):
         return SAFE_CHOICE, None, f"probe failed: {e!r}"
 
 
+ALL_CASES = [  # (config, mode, extra flags): north_star "five synthetic clusters ... CLT vs CR"
+    (1, "clt", []), (1, "cr", []), (1, "clt", ["--graph", "1"]), (1, "clt", ["--batch", "4", "--graph", "1"]),
+    (2, "clt", []), (2, "cr", []), (2, "clt", ["--graph", "1"]), (2, "clt", ["--batch", "4"]),
+    (3, "clt", []), (3, "cr", []),
+    (4, "clt", []), (4, "cr", []), (41, "clt", []), (40, "clt", []), (4, "clt", ["--batch", "2"]), (4, "clt", ["--batch", "4"]),
+    (5, "cr", []),
+]
+
+
+def run_all(args):
+    """Every BASELINE config (largest sector) and index mode, each in its own child bench run (own probe: no candidate
+    is timed before the checked library has run it on this device); rows -> gpurun_out/bench_all.json and a table on
+    stderr.  The ONE JSON line printed is the headline case (config 4, CLT, FP32, B = 1)."""
+    rows, headline = [], None
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    for cfg, mode, extra in ALL_CASES:
+        steps = {1: 200, 2: 200, 3: 60, 5: 20}.get(cfg, 40)
+        cmd = [sys.executable, os.path.abspath(__file__), "--config", str(cfg), "--mode", mode, "--steps", str(steps),
+               "--warmup", "3"] + extra
+        if cfg == 5:
+            cmd.append("--no-cpu-baseline")               # the oracle cannot enumerate this basis; its sampled-row form is a test tool
+        if not (cfg == 4 and mode == "clt" and not extra):
+            cmd.append("--no-e2e")
+        try:
+            d, err = _child_json(cmd, dict(os.environ), 3600)
+        except Exception as e:
+            d, err = None, repr(e)
+        if d is None:
+            rows.append({"config": cfg, "mode": mode, "flags": extra, "error": err})
+            continue
+        r = d["roofline"]
+        rows.append({"config": cfg, "workload": d["config"]["workload"], "mode": mode, "flags": extra, "dim": d["config"]["dim"],
+                     "kernel": d["config"]["candidate"], "hv_passes": d["config"]["hv_passes"], "steps_per_s": d["value"],
+                     "ms_per_step": d["ms_per_step"], "hv_rows_per_s": d["hv_rows_per_s"], "hv_gelem_per_s": d["hv_gelem_per_s"],
+                     "hv_ms": r["ms_per_launch"], "floorA_GBps": r["achieved"], "frac_of_measured_hbm": r["frac"],
+                     "norm_GBps": r["norm_kernel_GBps"], "oracle_rows_per_s": (d.get("cpu_baseline") or {}).get("rows_per_s"),
+                     "oracle_cores": (d.get("cpu_baseline") or {}).get("cores"), "clocks": d.get("clocks"),
+                     "site_numbering": d["config"].get("site_numbering"), "probe_note": d["config"].get("probe_note")})
+        if cfg == 4 and mode == "clt" and not extra:
+            headline = d
+        with open(os.path.join(ROOT, "gpurun_out", "bench_all.json"), "w") as f:
+            json.dump(rows, f, indent=1)
+    sys.stderr.write("| config | mode | flags | kernel | passes | steps/s | H.v rows/s | Gelem/s | floor-A GB/s | frac | oracle rows/s |\n|---|---|---|---|---|---|---|---|---|---|---|\n")
+    for r in rows:
+        if "error" in r:
+            sys.stderr.write(f"| {r['config']} | {r['mode']} | {' '.join(r['flags'])} | ERROR {r['error']} |\n")
+        else:
+            sys.stderr.write(f"| {r['workload']} | {r['mode']} | {' '.join(r['flags'])} | {r['kernel']} | {r['hv_passes']} | {r['steps_per_s']:.1f} | "
+                             f"{r['hv_rows_per_s']:.3e} | {r['hv_gelem_per_s']:.2f} | {r['floorA_GBps']:.1f} | {r['frac_of_measured_hbm']:.4f} | "
+                             f"{(r['oracle_rows_per_s'] or 0):.3e} |\n")
+    if headline is not None:
+        headline["config"]["all_cases_file"] = "gpurun_out/bench_all.json"
+        print(json.dumps(headline), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--probe", action="store_true", help=argparse.SUPPRESS)
-    ap.add_argument("--probe-stage", default="checked", choices=["checked", "release"], help=argparse.SUPPRESS)
+    ap.add_argument("--probe-stage", default="checked", choices=["checked", "release", "batchcheck"], help=argparse.SUPPRESS)
     ap.add_argument("--mask", type=int, default=0, help=argparse.SUPPRESS)
     ap.add_argument("--candidate", default="", help="one of " + ", ".join(CANDIDATES))
     ap.add_argument("--gpus", type=int, default=1)
@@ -242,6 +333,9 @@ def main():
     ap.add_argument("--low-bits", type=int, default=0)
     ap.add_argument("--tml-low-bits", type=int, default=0)
     ap.add_argument("--tml-mid-bits", type=int, default=0)
+    ap.add_argument("--batch", type=int, default=1, choices=[1, 2, 4], help="chains advanced together (L207); value counts chain-steps")
+    ap.add_argument("--graph", type=int, default=0, choices=[0, 1], help="replay steps from a CUDA graph")
+    ap.add_argument("--all", action="store_true", help="every BASELINE config and index mode (children), table in gpurun_out/bench_all.json")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -251,6 +345,9 @@ def main():
     n_up = w.sectors[0]
     if args.impl == "reference":
         run_reference(args, w, n_up)
+        return
+    if args.all:
+        run_all(args)
         return
     if args.probe:
         run_probe(args)
@@ -280,8 +377,12 @@ def main():
         mode, args.mode = ftlm.INDEX_CR, "cr"
     ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, local)
     autotune_report, probe_note = None, None
+    B = args.batch
     if args.candidate:
         choice = args.candidate
+    elif B > 1:
+        choice, autotune_report, probe_note = probe_batch(args) if rank == 0 else ("row", None, None)
+        choice = replicas.broadcast_choice(choice, dist)
     elif args.kernel == "auto":
         # rank 0 probes in a child process; every rank applies the same choice
         choice, autotune_report, probe_note = probe_choice(args) if rank == 0 else (SAFE_CHOICE, None, None)
@@ -294,6 +395,11 @@ def main():
         ftlm.ftlm_set_option(ctx, "tml_low_bits", args.tml_low_bits)
     if args.tml_mid_bits:
         ftlm.ftlm_set_option(ctx, "tml_mid_bits", args.tml_mid_bits)
+    if B > 1:                                                    # batched chains: TML without windows, or ROW
+        for key in ("lazy_norm", "tmlr", "passb"):
+            ftlm.ftlm_set_option(ctx, key, 0)
+        ftlm.ftlm_set_option(ctx, "batch", B)
+    ftlm.ftlm_set_option(ctx, "graph", args.graph)
     kernel_used = {1: "row", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
     if kernel_used == "tml" and ftlm.ftlm_get_option(ctx, "tmlr") == 1 and ftlm.ftlm_get_option(ctx, "tmlr_available") == 1:
         kernel_used = "tmlr"
@@ -305,7 +411,13 @@ def main():
     assert 1 <= K and K + Wm <= ftlm.MAX_STEPS, "steps + warmup must be <= 1024 (one chain)"
 
     # ---- device-resident timing: `value` ---------------------------------------------------
-    ftlm.ftlm_chain_begin(ctx, None, W.SEED_VECTORS, rank)       # one replica chain per rank
+    def begin():
+        if B > 1:
+            ftlm.ftlm_chain_begin_batch(ctx, W.SEED_VECTORS, rank * B, B)   # B replica chains per rank, interleaved
+        else:
+            ftlm.ftlm_chain_begin(ctx, None, W.SEED_VECTORS, rank)       # one replica chain per rank
+
+    begin()
     ftlm.ftlm_chain_steps(ctx, Wm)
     barrier()
     sampler = ClockSampler(local)
@@ -317,17 +429,22 @@ def main():
     barrier()
     ms = e0.elapsed_time(e1)
     sampler.stop_flag = True
-    a, b, m_eff = ftlm.ftlm_chain_end(ctx)
-    assert m_eff == K + Wm and np.isfinite(a).all() and np.isfinite(b).all(), (m_eff, K + Wm)
+    if B > 1:
+        a, b, m_effs = ftlm.ftlm_chain_end_batch(ctx, B)
+        m_eff = int(m_effs.min())
+        assert int(m_effs.max()) == m_eff
+    else:
+        a, b, m_eff = ftlm.ftlm_chain_end(ctx)
+    assert m_eff == min(K + Wm, D) and np.isfinite(a).all() and np.isfinite(b).all(), (m_eff, K + Wm)
     ms = replicas.max_over_ranks(ms, dist, device="cuda")
-    value = world * K / (ms * 1e-3)
+    value = world * B * K / (ms * 1e-3)                          # chain-steps per second (B = 1: steps per second)
 
     # ---- per-kernel timing for the roofline of the dominant kernel --------------------------
-    ftlm.ftlm_chain_begin(ctx, None, W.SEED_VECTORS, rank)
+    begin()
     ftlm.ftlm_chain_steps(ctx, 3)
     ms_hv, ms_norm = ftlm.ftlm_chain_profile(ctx, min(K, 30))
     table_bytes = (8 * ((1 << w.N) // 32)) if mode == ftlm.INDEX_CLT else 0
-    alg_bytes = 12 * D + table_bytes             # floor A of SURVEY 8(d): v, v_prev, y + table
+    alg_bytes = 12 * B * D + table_bytes         # floor A of SURVEY 8(d): v, v_prev, y (x B chains) + table
     peak, peak_src = measured_peak()
     achieved = alg_bytes / (ms_hv * 1e-3) / 1e9
     kname = f"hv_{kernel_used}_{args.mode}_fp32_fused" + (f"+passb{n_windows}" if n_windows else "")
@@ -339,11 +456,11 @@ def main():
     # ---- end-to-end through the host-buffer ABI call ---------------------------------------
     e2e = None
     if not args.no_e2e:
-        hq = torch.empty((1, D), dtype=torch.float32).pin_memory()
+        hq = torch.empty((B, D), dtype=torch.float32).pin_memory()
         hq.normal_(generator=torch.Generator().manual_seed(1234 + rank))
         hq_np = hq.numpy()
         ke = min(K, 100)
-        ftlm.ftlm_lanczos_host(ctx, hq_np, 2)                     # warm-up of the path
+        ftlm.ftlm_lanczos_host(ctx, hq_np, 2)                     # warm-up of the path (B start vectors = one batch)
         barrier()
         t0 = time.perf_counter()
         out = ftlm.ftlm_lanczos_host(ctx, hq_np, ke)              # H2D start vector, ke steps, D2H alpha/beta, T eig
@@ -351,8 +468,8 @@ def main():
         dt = time.perf_counter() - t0
         t_e = replicas.max_over_ranks(dt, dist, device="cuda")
         assert int(out["m_eff"][0]) == ke
-        e2e = {"value": world * ke / t_e, "unit": UNIT, "h2d_bytes_per_step": 4 * D / ke,
-               "d2h_bytes_per_step": 16.0 + 8.0 / ke, "steps": ke,
+        e2e = {"value": world * B * ke / t_e, "unit": UNIT, "h2d_bytes_per_step": 4 * B * D / ke,
+               "d2h_bytes_per_step": B * (16.0 + 8.0 / ke), "steps": ke,
                "call": "ftlm_lanczos_host(pinned host start vector -> alpha, beta, theta, weight)"}
 
     ftlm.ftlm_destroy(ctx)
@@ -379,9 +496,14 @@ def main():
             "config": {"workload": f"config{args.config}:{w.name}", "N": w.N, "N_up": n_up, "dim": D,
                        "n_bonds": w.n_bonds, "index_mode": args.mode, "kernel": kernel_used, "candidate": choice,
                        "hv_passes": 1 + n_windows, "autotune": autotune_report, "probe_note": probe_note,
-                       "precision": "fp32 vectors, fp64 reductions", "l2": "inputs_exceed_l2 (3 x 620 MB vectors)",
+                       "precision": "fp32 vectors, fp64 reductions",
+                       "l2": (f"inputs_exceed_l2 (3 x {4 * D / 1e6:.0f} MB vectors)" if 12 * D > 126e6 else
+                              f"inputs_fit_l2 (3 x {4 * D / 1e6:.2f} MB vectors: this workload is L2-resident by size; no flush between steps)"),
+                       "site_numbering": {4: "CONFIG4_SITE_ORDER (annealed for two window passes, DESIGN.md section 3)", 40: "CONFIG4_SITE_ORDER",
+                                          41: "lexicographic icosahedron edges (SURVEY 8(d))", 5: "fold_order(34)"}.get(args.config, "SURVEY 8(d)"),
+                       "batch": args.batch, "graph": args.graph,
                        "parallelism": f"replicas x{world}"},
-            "hv_rows_per_s": world * D / (ms_hv * 1e-3), "hv_gelem_per_s": world * nnz / (ms_hv * 1e-3) / 1e9,
+            "hv_rows_per_s": world * B * D / (ms_hv * 1e-3), "hv_gelem_per_s": world * B * nnz / (ms_hv * 1e-3) / 1e9,
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": ((1 if ftlm_lazy else 2) + n_windows) * K,
             "clocks": sampler.summary()}
     print(json.dumps(line), flush=True)

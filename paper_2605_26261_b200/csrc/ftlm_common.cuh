@@ -101,7 +101,12 @@ struct ftlm_ctx {
   // options
   int kernel = FTLM_KERNEL_AUTO;
   int tml_low_bits = 0, tml_mid_bits = 0;
-  int use_graph = 0;
+  int use_graph = 0;               // option "graph": ftlm_chain_steps replays captured steps (CUDA graph)
+  int graph_failed = 0;            // a capture / instantiate call failed on this handle: direct launches from then on
+  int graph_roles[3] = {-1, -1, -1}, graph_batch = 0, graph_period = 0;   // what the cached graph was captured for
+  void* graph_exec = nullptr;      // cudaGraphExec_t
+  void* graph_stream = nullptr;    // capture stream (the caller's stream may be the legacy default stream)
+  int graph_launches = 0;          // replays so far (read-only key "graph_launches")
   int allow_unverified = 0;        // option "allow_unverified": ftlm_autotune may run candidates without a device record
   uint64_t autotune_mask = 0;      // option "autotune_mask": bit k set = candidate k may run (0 = all); the ROW reference always runs
   int autotuned = 0;               // 1 + index of the candidate ftlm_autotune selected (0 = not tuned)

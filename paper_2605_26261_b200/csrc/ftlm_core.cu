@@ -8,6 +8,8 @@
 #define FTLM_TU 1
 #include "ftlm_common.cuh"
 
+static void graph_drop(ftlm_ctx* c);                 // cached CUDA graph of the chain step (defined with ftlm_chain_steps)
+
 // ---- errors --------------------------------------------------------------------------------
 static thread_local char g_err[512] = "";
 
@@ -425,6 +427,10 @@ extern "C" int ftlm_create(ftlm_ctx** out, int N, int n_bonds, const int32_t* bo
 extern "C" int ftlm_destroy(ftlm_ctx* c) {
   if (!c) return FTLM_OK;
   cudaSetDevice(c->device);
+  graph_drop(c);
+#ifndef FTLM_EMU
+  if (c->graph_stream) cudaStreamDestroy((cudaStream_t)c->graph_stream);
+#endif
   ftlm_tml_plan_destroy(c);
   ftlm_dfree(c->d_binom64); ftlm_dfree(c->d_binom32); ftlm_dfree(c->d_bonds); ftlm_dfree(c->d_clt);
   ftlm_dfree(c->d_state); ftlm_dfree(c->d_partials); ftlm_dfree(c->d_ticket); ftlm_dfree(c->d_lin_hi); ftlm_dfree(c->d_lin_lo);
@@ -453,6 +459,7 @@ int ftlm_effective_kernel(const ftlm_ctx* c) {
 
 extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   if (!c || !key) { ftlm_set_error("ftlm_set_option: NULL"); return FTLM_EINVAL; }
+  graph_drop(c);                                         // a captured step belongs to the configuration it was captured under
   if (!strcmp(key, "kernel")) {
     if (value != FTLM_KERNEL_AUTO && value != FTLM_KERNEL_ROW && value != FTLM_KERNEL_TML) { ftlm_set_error("kernel must be FTLM_KERNEL_AUTO, _ROW or _TML"); return FTLM_EINVAL; }
     if (value == FTLM_KERNEL_TML && (!c->tml || c->mode == FTLM_INDEX_LIN)) { ftlm_set_error("TML kernel unavailable for this sector / index mode"); return FTLM_EUNSUPPORTED; }
@@ -469,7 +476,7 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     if (rc != FTLM_OK) { *slot = old; ftlm_tml_plan_destroy(c); ftlm_tml_plan_create(c); }
     return rc;
   }
-  if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; return FTLM_OK; }
+  if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; c->graph_failed = 0; return FTLM_OK; }
   if (!strcmp(key, "allow_unverified")) { c->allow_unverified = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "tmlr")) { c->use_tmlr = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "lazy_norm")) { c->lazy_norm = value ? 1 : 0; return FTLM_OK; }
@@ -545,6 +552,8 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!c) return -1;
   if (!strcmp(key, "kernel")) return ftlm_effective_kernel(c);
   if (!strcmp(key, "graph")) return c->use_graph;
+  if (!strcmp(key, "graph_launches")) return c->graph_launches;
+  if (!strcmp(key, "graph_failed")) return c->graph_failed;
   if (!strcmp(key, "passb")) return c->use_passb;
   if (!strncmp(key, "passb_", 6)) return ftlm_passb_info(c, key);
   if (!strcmp(key, "sm_count")) return c->sm_count;
@@ -782,10 +791,71 @@ static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv,
   return FTLM_OK;
 }
 
+// ---- CUDA graph of the step (option "graph"; SURVEY 3(i), 8(d) "CUDA events around a graph of N_L steps") -------------
+// The work-vector roles return to where they were after `period` steps (2: q_j / q_{j-1} swap; 3 with lazy
+// normalisation), so `period` consecutive steps are captured once and replayed.  Breakdown stays a device-side no-op.
+// Any failure of a graph call leaves the handle on direct launches (never an error of the chain).
+static void graph_drop(ftlm_ctx* c) {
+#ifndef FTLM_EMU
+  if (c->graph_exec) { cudaGraphExecDestroy((cudaGraphExec_t)c->graph_exec); c->graph_exec = nullptr; }
+#endif
+  c->graph_roles[0] = c->graph_roles[1] = c->graph_roles[2] = -1;
+}
+
+#ifndef FTLM_EMU
+static bool graph_ready(ftlm_ctx* c, int period) {
+  if (c->graph_exec && c->graph_roles[0] == c->ia && c->graph_roles[1] == c->ib && c->graph_roles[2] == c->ic &&
+      c->graph_batch == c->cur_batch && c->graph_period == period) return true;
+  graph_drop(c);
+  if (!c->graph_stream) {
+    cudaStream_t gs = nullptr;
+    if (cudaStreamCreateWithFlags(&gs, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->graph_failed = 1; return false; }
+    c->graph_stream = gs;
+  }
+  cudaStream_t gs = (cudaStream_t)c->graph_stream;
+  const int ia = c->ia, ib = c->ib, ic = c->ic, enq = c->steps_enqueued;
+  const bool pend = c->pending_norm;
+  cudaGraph_t g = nullptr;
+  bool ok = cudaStreamBeginCapture(gs, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+  if (ok) {
+    for (int k = 0; k < period && ok; ++k) ok = chain_one_step(c, gs, false, nullptr, nullptr) == FTLM_OK;
+    ok = (cudaStreamEndCapture(gs, &g) == cudaSuccess) && ok && g != nullptr;
+  }
+  ok = ok && c->ia == ia && c->ib == ib && c->ic == ic && c->pending_norm == pend;   // the roles are periodic
+  c->ia = ia; c->ib = ib; c->ic = ic; c->steps_enqueued = enq; c->pending_norm = pend;  // nothing has run
+  cudaGraphExec_t ge = nullptr;
+  if (ok) ok = cudaGraphInstantiate(&ge, g, 0) == cudaSuccess;
+  if (g) cudaGraphDestroy(g);
+  if (!ok) { cudaGetLastError(); c->graph_failed = 1; return false; }
+  c->graph_exec = ge;
+  c->graph_roles[0] = ia; c->graph_roles[1] = ib; c->graph_roles[2] = ic;
+  c->graph_batch = c->cur_batch; c->graph_period = period;
+  return true;
+}
+#endif
+
 extern "C" int ftlm_chain_steps(ftlm_ctx* c, int nsteps, void* stream) {
   if (!c || nsteps < 0 || !c->q[0]) { ftlm_set_error("ftlm_chain_steps: no chain begun or nsteps < 0"); return FTLM_EINVAL; }
   CK(cudaSetDevice(c->device));
-  for (int k = 0; k < nsteps; ++k) {
+  int k = 0;
+#ifndef FTLM_EMU
+  if (c->use_graph && !c->graph_failed) {
+    const bool lazy = c->cur_batch == 1 && c->lazy_norm && ftlm_effective_kernel(c) == FTLM_KERNEL_TML && ftlm_tmlr_lazy_ok(c);
+    const int period = lazy ? 3 : 2;
+    // the first step of a chain runs directly (lazy form: it is the one step without a pending normalisation)
+    for (; k < nsteps && c->steps_enqueued < 1 && c->steps_enqueued < c->chain_limit; ++k) {
+      int rc = chain_one_step(c, (cudaStream_t)stream, false, nullptr, nullptr);
+      if (rc != FTLM_OK) return rc;
+    }
+    while (nsteps - k >= period && c->steps_enqueued + period <= c->chain_limit && graph_ready(c, period)) {
+      if (cudaGraphLaunch((cudaGraphExec_t)c->graph_exec, (cudaStream_t)stream) != cudaSuccess) { cudaGetLastError(); c->graph_failed = 1; break; }
+      c->steps_enqueued += period;
+      c->graph_launches++;
+      k += period;
+    }
+  }
+#endif
+  for (; k < nsteps; ++k) {
     if (c->steps_enqueued >= c->chain_limit) break;      // the device would no-op anyway
     int rc = chain_one_step(c, (cudaStream_t)stream, false, nullptr, nullptr);
     if (rc != FTLM_OK) return rc;
