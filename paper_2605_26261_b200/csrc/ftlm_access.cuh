@@ -78,6 +78,8 @@ __device__ __noinline__ static bool ftlm_chk_s(const void* p, int bytes, int ali
 }
 #define FTLM_G_OK(p, T, line) ftlm_chk_g((const void*)(p), (int)sizeof(T), (int)alignof(T), (line))
 #define FTLM_S_OK(p, T, line) ftlm_chk_s((const void*)(p), (int)sizeof(T), (int)alignof(T), (line))
+#define FTLM_G_OKN(p, bytes, align, line) ftlm_chk_g((const void*)(p), (int)(bytes), (int)(align), (line))   /* a whole range (bulk copy) */
+#define FTLM_S_OKN(p, bytes, align, line) ftlm_chk_s((const void*)(p), (int)(bytes), (int)(align), (line))
 #define FTLM_A_OK(p, T, line) (__isShared((const void*)(p)) ? FTLM_S_OK(p, T, line) : FTLM_G_OK(p, T, line))
 
 #elif defined(FTLM_EMU)
@@ -98,11 +100,15 @@ static inline bool ftlm_emu_aligned(const void* p, size_t align, int line, const
 #define FTLM_S_OK(p, T, line) (ftlm_emu_aligned((const void*)(p), alignof(T), (line), "shared access") && cuda_emu::smem_access((const void*)(p), sizeof(T), false, FTLM_TU, (line)))
 #define FTLM_SW_OK(p, T, line) (ftlm_emu_aligned((const void*)(p), alignof(T), (line), "shared access") && cuda_emu::smem_access((const void*)(p), sizeof(T), true, FTLM_TU, (line)))
 #define FTLM_A_OK(p, T, line) (ftlm_emu_aligned((const void*)(p), alignof(T), (line), "access") && cuda_emu::smem_access((const void*)(p), sizeof(T), false, FTLM_TU, (line)))
+#define FTLM_G_OKN(p, bytes, align, line) ftlm_emu_aligned((const void*)(p), (align), (line), "bulk-copy source")
+#define FTLM_S_OKN(p, bytes, align, line) ftlm_emu_aligned((const void*)(p), (align), (line), "bulk-copy destination")
 
 #else
 #define FTLM_G_OK(p, T, line) true
 #define FTLM_S_OK(p, T, line) true
 #define FTLM_A_OK(p, T, line) true
+#define FTLM_G_OKN(p, bytes, align, line) true
+#define FTLM_S_OKN(p, bytes, align, line) true
 #endif
 #ifndef FTLM_SW_OK
 #define FTLM_SW_OK(p, T, line) FTLM_S_OK(p, T, line)      /* shared-memory WRITE (the emulation's race detector tells them apart) */

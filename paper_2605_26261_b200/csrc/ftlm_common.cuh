@@ -215,6 +215,58 @@ __device__ __forceinline__ void cp_async_wait_all() {
 #endif
 }
 
+// ---- bulk copy global -> shared with mbarrier completion (Blackwell/Hopper async proxy; SASS UBLKCP + SYNCS) -----
+// One thread announces the bytes (arrive.expect_tx) and issues the copy; every thread of the CTA waits on the phase
+// parity.  Source, destination and size are multiples of 16 bytes.  The emulation lands the bytes at the first wait
+// that finds the phase complete (destination poisoned until then).
+__device__ __forceinline__ void mbar_init(uint64_t* mbar, int count) {
+#ifdef FTLM_EMU
+  cuda_emu::mbar_init(mbar, count);
+#else
+  const unsigned a = (unsigned)__cvta_generic_to_shared(mbar);
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+#endif
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* mbar, uint32_t bytes) {
+#ifdef FTLM_EMU
+  cuda_emu::mbar_arrive_expect_tx(mbar, bytes);
+#else
+  const unsigned a = (unsigned)__cvta_generic_to_shared(mbar);
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+#endif
+}
+__device__ __forceinline__ void bulk_copy_g2s_(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* mbar, int line) {
+  if (!FTLM_S_OKN(smem_dst, bytes, 16, line) || !FTLM_G_OKN(gsrc, bytes, 16, line)) {
+    // checked build: the copy is suppressed; its bytes are taken back from the barrier so that nobody waits for them
+#if defined(FTLM_CHECKED) && !defined(FTLM_EMU)
+    const unsigned a = (unsigned)__cvta_generic_to_shared(mbar);
+    asm volatile("mbarrier.complete_tx.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+#endif
+    return;
+  }
+#ifdef FTLM_EMU
+  cuda_emu::bulk_issue(smem_dst, gsrc, bytes, mbar, FTLM_TU, line);
+#else
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), a = (unsigned)__cvta_generic_to_shared(mbar);
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(d), "l"(gsrc), "r"(bytes), "r"(a) : "memory");
+#endif
+}
+#define bulk_copy_g2s(dst, src, bytes, mbar) bulk_copy_g2s_((dst), (src), (bytes), (mbar), __LINE__)
+__device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
+#ifdef FTLM_EMU
+  cuda_emu::mbar_wait(mbar, parity);
+#else
+  const unsigned a = (unsigned)__cvta_generic_to_shared(mbar);
+  unsigned done = 0;
+  while (!done) {
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(a), "r"(parity) : "memory");
+  }
+#endif
+}
+
 __device__ __forceinline__ double warp_sum(double x) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);

@@ -104,7 +104,7 @@ __host__ __device__ inline size_t tmlr_layout(TmlrSmem<R>& s, unsigned char* p0,
   auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return p0 + at; };
   s.binom = (uint64_t*)take((size_t)(N + 1) * (K + 1) * 8);
   s.blob = take((size_t)blob_bytes);
-  s.vs = (R*)take((size_t)max_tile * sizeof(R));
+  s.vs = (R*)take((size_t)max_tile * sizeof(R) + 16);    // + 16: the tile keeps the global address's residue mod 16 bytes
   s.dcoef = (R*)take((size_t)nM * sizeof(R));
   s.dmmJ = (R*)take((size_t)nM * (n_mm ? n_mm : 1) * sizeof(R));
   s.dmm = (uint32_t*)take((size_t)nM * (n_mm ? n_mm : 1) * 4);
@@ -154,9 +154,12 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
   const uint16_t* s_ll = (const uint16_t*)(S.blob + p.off_ll);               // [bond][Lidx]: target row in the column
   const uint16_t* s_fl = (const uint16_t*)(S.blob + p.off_fl);               // [bond][Lidx]: flipped row | L_i << 15
   const R bprev = FUSED ? (R)p.st->beta_prev : (R)0;
-  const unsigned char* vsm1 = (const unsigned char*)S.vs - 1;
   const int n_mm = p.n_mm;
   constexpr int n_ml = NML;
+  constexpr int RPV = 16 / (int)sizeof(R);              // rows per 16 bytes
+  __shared__ __align__(8) uint64_t s_mbar;              // completion barrier of the tile's bulk copy
+  uint32_t mbar_parity = 0;
+  if (tid == 0) mbar_init(&s_mbar, 1);
 
   if (tid == 0) S.misc[0] = (int)atomicAdd(&p.counter[0], 1u);
   for (;;) {
@@ -170,6 +173,14 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
     const uint64_t base = p.mode == FTLM_INDEX_CLT ? passb_run_start<FTLM_INDEX_CLT>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt)
                                                    : passb_run_start<FTLM_INDEX_CR>((uint64_t)T, p.mw, kT, p.K, S.binom, p.clt);
     const int tlen = LD_S(&s_tlen[kT]);
+    // the tile sits in shared memory at the same residue mod 16 bytes as in global memory, so that its 16-byte
+    // aligned interior is one bulk copy (cp.async.bulk, SASS UBLKCP: no per-element issue slots); the < 16-byte
+    // head and tail are plain loads
+    const int mis = (int)(((uintptr_t)((p.lazy ? (const R*)p.vio : v) + base) & 15u) / sizeof(R));   // (a caller's vector need not be 16-byte aligned)
+    R* const vs0 = S.vs + mis;                           // row 0 of the tile
+    const unsigned char* vsm1 = (const unsigned char*)vs0 - 1;
+    const int head = mis ? (RPV - mis < tlen ? RPV - mis : tlen) : 0;
+    const int body = p.lazy ? 0 : ((tlen - head) / RPV) * RPV;
     if (p.lazy) {                                       // lazy normalisation: q_{j+1} formed while staging, written over y_j
       const R a = (R)p.st->a, ib = (R)p.st->inv_b;
       R* yq = p.vio + base;
@@ -187,14 +198,22 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
           const int x = x0 + k * NT;
           if (x < tlen) {
             const R qn = (yv[k] - a * qv[k]) * ib;
-            ST_S(&S.vs[x], qn);
+            ST_S(&vs0[x], qn);
             ST_G(&yq[x], qn);
           }
         }
       }
-    } else {                                            // stage the tile: every copy in flight at once
+    } else {                                            // stage the tile
       const R* src = v + base;
-      for (int x = tid; x < tlen; x += NT) cp_async_elem(&S.vs[x], &src[x]);
+      if (body > 0 && tid == 0) {
+        const uint32_t bytes = (uint32_t)body * (uint32_t)sizeof(R);
+        mbar_arrive_expect_tx(&s_mbar, bytes);
+        for (uint32_t o = 0; o < bytes; o += 32768u)      // 32 KB pieces
+          bulk_copy_g2s((unsigned char*)(vs0 + head) + o, (const unsigned char*)(src + head) + o, bytes - o < 32768u ? bytes - o : 32768u, &s_mbar);
+      }
+      if (tid < head) ST_S(&vs0[tid], LD_G(&src[tid]));
+      const int done = head + body;
+      if (tid < tlen - done) ST_S(&vs0[done + tid], LD_G(&src[done + tid]));
     }
     const uint16_t* co = s_coloff + kT * nM;
     for (int M = tid; M < nM; M += NT) {                // column descriptors of this kT
@@ -243,8 +262,10 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         ST_S(&S.dml[M * n_ml + e], j < 0 ? 0u : ((uint32_t)LD_S(&co[(uint32_t)M ^ (1u << j)]) * (uint32_t)sizeof(R) | (((uint32_t)M >> j) & 1u)));
       }
     }
-    cp_async_wait_all();
-    __syncthreads();
+#if !defined(FTLM_NEG_TEST) || FTLM_NEG_TEST != 3     // (negative test of the host emulation: tests/emu/build_emu.py)
+    if (body > 0) { mbar_wait(&s_mbar, mbar_parity); mbar_parity ^= 1u; }   // the bulk copy has landed (every thread observes it)
+#endif
+    __syncthreads();                                    // descriptors, head and tail written by other threads
     // ---- units: one chunk of 32 low parts x a block of columns per warp ----------------------------
     const int u0 = LDG(&p.unit_off[kT]), u1 = LDG(&p.unit_off[kT + 1]);
     double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
@@ -279,8 +300,8 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
           cbn = LD_S(&co[Mn]);
           if (FUSED) qpn = LDCS(qprev + (base + cbn + (uint32_t)lrc));
         }
-        const unsigned char* colb = (const unsigned char*)(S.vs + cb);
-        const R own = LD_S(&S.vs[cb + (uint32_t)lrc]);
+        const unsigned char* colb = (const unsigned char*)(vs0 + cb);
+        const R own = LD_S(&vs0[cb + (uint32_t)lrc]);
         // four independent partial sums (LL even/odd, ML even/odd) keep the FMA dependency chains short
         R acc = LD_S(&S.dcoef[M]) * own;
         R l0 = (R)0, l1 = (R)0, m0 = (R)0, m1 = (R)0;
@@ -290,7 +311,7 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
           if (UNIJ) { l0 += a0; l1 += a1; } else { l0 += p.ll_J[e] * a0; l1 += p.ll_J[e + 1] * a1; }
         }
         const int nmm = LD_S(&S.dnmm[M]);
-        for (int a = 0; a < nmm; ++a) acc += LD_S(&S.dmmJ[M * n_mm + a]) * LD_S(&S.vs[LD_S(&S.dmm[M * n_mm + a]) + (uint32_t)lrc]);
+        for (int a = 0; a < nmm; ++a) acc += LD_S(&S.dmmJ[M * n_mm + a]) * LD_S(&vs0[LD_S(&S.dmm[M * n_mm + a]) + (uint32_t)lrc]);
         if (p.n_g) {
           const int ng = LD_S(&S.dng[M]);
           for (int a = 0; a < ng; ++a) acc += LD_S(&S.dgJ[M * p.n_g + a]) * LDG(v + ((size_t)LD_S(&S.dg[M * p.n_g + a]) + (uint32_t)lrc));

@@ -43,11 +43,12 @@ def build(force: bool = False) -> str:
 def build_negative(k: int) -> str:
     """A deliberately broken copy of the library for the negative tests of the emulation itself: -DFTLM_NEG_TEST=k
     removes one synchronisation from one kernel (1: the cp.async wait of PASS-B's staging phase, ftlm_passb.cu;
-    2: the __syncwarp between building and reading the per-column descriptor lists, ftlm_tml.cu).  A run through it
+    2: the __syncwarp between building and reading the per-column descriptor lists, ftlm_tml.cu;
+    3: the mbarrier wait after the bulk copy of TMLR's tile, ftlm_tmlr.cu).  A run through it
     must be killed by the emulation (tests/test_emu_kernels.py::test_emu_detects_removed_synchronisation)."""
     build()
     so = os.path.join(HERE, f"libftlm_emu_neg{k}.so")
-    victim = {1: "ftlm_passb.cu", 2: "ftlm_tml.cu"}[k]
+    victim = {1: "ftlm_passb.cu", 2: "ftlm_tml.cu", 3: "ftlm_tmlr.cu"}[k]
     if os.path.exists(so) and all(os.path.getmtime(d) <= os.path.getmtime(so) for d in deps()):
         return so
     objs = []

@@ -57,6 +57,10 @@ void guarded_free(void* p) {
 // ---- fibers ------------------------------------------------------------------------------------
 struct PendingCopy { void* dst; size_t bytes; unsigned char data[16]; };
 struct Fiber { ucontext_t ctx; char* stack = nullptr; bool done = false; bool started = false; std::vector<PendingCopy> pending; };
+struct PendingBulk { void* dst; std::vector<unsigned char> data; void* mbar; };
+struct MBar { int count = 0, pending = 0; long tx = 0; unsigned completed = 0; };
+thread_local std::vector<PendingBulk> g_bulk;           // bulk copies in flight of the CTA on this host thread
+thread_local std::map<void*, MBar> g_mbar;
 const size_t STACK = 64 * 1024;
 // scheduler state of the CTA in flight on this host thread
 thread_local std::vector<Fiber> g_fib;
@@ -125,6 +129,7 @@ void fiber_entry() {
   (*g_body)();
   Fiber& f = g_fib[(size_t)g_cur];
   if (!f.pending.empty()) die("thread exits with cp.async copies it never waited for");
+  if (g_alive == 1 && !g_bulk.empty()) die("CTA exits with bulk copies nobody waited for");
   f.done = true;
   g_progress++;
   g_alive--;
@@ -153,6 +158,7 @@ void run_block() {
     g_warps[i >> 5].alive_mask |= 1u << (i & 31);
   }
   g_alive = nt; g_bar_arrived = 0; g_bar_gen = 0;
+  g_bulk.clear(); g_mbar.clear();
   if (race_on()) g_shadow.assign((g_dyn_bytes + 3) / 4, Shadow{Access{-1, 0, 0, 0, 0}, Access{-1, 0, 0, 0, 0}});
   else g_shadow.clear();
   // FTLM_EMU_ORDER: order in which runnable threads are resumed in every scheduling round - 0 ascending
@@ -210,6 +216,61 @@ void cp_async_wait_all() {
   Fiber& f = g_fib[(size_t)g_cur];
   for (const PendingCopy& c : f.pending) { smem_access(c.dst, c.bytes, true, 0, 0); memcpy(c.dst, c.data, c.bytes); }
   f.pending.clear();
+}
+
+// ---- bulk copies + mbarriers (per CTA = per host thread) ------------------------------------------------------------
+void mbar_init(void* mbar, int count) {
+  if (g_cur < 0) die("mbarrier.init outside a kernel");
+  MBar b; b.count = count; b.pending = count;
+  g_mbar[mbar] = b;
+}
+
+void mbar_arrive_expect_tx(void* mbar, unsigned bytes) {
+  auto it = g_mbar.find(mbar);
+  if (it == g_mbar.end()) die("mbarrier.arrive on an uninitialised barrier");
+  it->second.tx += (long)bytes;
+  if (--it->second.pending < 0) die("mbarrier: more arrivals than its count");
+  g_progress++;
+}
+
+void bulk_issue(void* smem_dst, const void* gsrc, unsigned bytes, void* mbar, int tu, int line) {
+  if (g_cur < 0) die("cp.async.bulk outside a kernel");
+  if (bytes == 0 || (bytes & 15u) || ((uintptr_t)smem_dst & 15u) || ((uintptr_t)gsrc & 15u)) die("cp.async.bulk: size, source and destination must be multiples of 16 bytes");
+  if ((unsigned char*)smem_dst < g_dyn || (unsigned char*)smem_dst + bytes > g_dyn + g_dyn_bytes) die("cp.async.bulk: destination outside the dynamic shared memory");
+  if (g_mbar.find(mbar) == g_mbar.end()) die("cp.async.bulk on an uninitialised barrier");
+  PendingBulk c;
+  c.dst = smem_dst; c.mbar = mbar;
+  c.data.assign((const unsigned char*)gsrc, (const unsigned char*)gsrc + bytes);    // faults here if the source is out of range
+  smem_access(smem_dst, bytes, true, tu, line);                                      // overwriting what others may still read?
+  memset(smem_dst, 0xFF, bytes);
+  g_bulk.push_back(std::move(c));
+}
+
+void mbar_wait(void* mbar, unsigned parity) {
+  if (g_cur < 0) die("mbarrier.try_wait outside a kernel");
+  for (;;) {
+    auto it = g_mbar.find(mbar);
+    if (it == g_mbar.end()) die("mbarrier.try_wait on an uninitialised barrier");
+    MBar& b = it->second;
+    if ((b.completed & 1u) != (parity & 1u)) return;           // the phase of this parity has completed
+    if (b.pending == 0) {                                      // all arrivals made: the outstanding copies complete now
+      for (size_t k = 0; k < g_bulk.size();) {
+        if (g_bulk[k].mbar != mbar) { ++k; continue; }
+        PendingBulk& c = g_bulk[k];
+        memcpy(c.dst, c.data.data(), c.data.size());
+        b.tx -= (long)c.data.size();
+        const size_t w0 = (size_t)((unsigned char*)c.dst - g_dyn) / 4, w1 = w0 + c.data.size() / 4;
+        for (size_t w = w0; w < w1 && w < g_shadow.size(); ++w) { g_shadow[w].w.tid = -1; g_shadow[w].r.tid = -1; }   // written by the async proxy
+        g_bulk.erase(g_bulk.begin() + (long)k);
+      }
+      if (b.tx != 0) die("mbarrier: expected and completed transaction bytes differ");
+      b.completed++; b.pending = b.count;
+      g_progress++;
+      continue;
+    }
+    yield_to_scheduler();
+    threadIdx.x = (unsigned)g_cur;
+  }
 }
 
 bool smem_access(const void* p, size_t bytes, bool write, int tu, int line) {

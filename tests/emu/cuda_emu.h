@@ -102,6 +102,14 @@ uint64_t collective(int op, unsigned mask, uint64_t v, int arg);
 // A consumer that reads before the producer's wait + barrier therefore sees NaN instead of passing by luck.
 void cp_async_issue(void* smem_dst, const void* gsrc, size_t bytes);
 void cp_async_wait_all();
+// Bulk copy + mbarrier model (cp.async.bulk ... mbarrier::complete_tx::bytes): the destination is poisoned when the
+// copy is issued (and the issue counts as a write of the issuing thread for the race detector: readers of the old
+// content must have passed a barrier); the bytes land when some thread's mbar_wait finds all arrivals made and then
+// completes the phase.  Size, source and destination must be multiples of 16 bytes.
+void mbar_init(void* mbar, int count);
+void mbar_arrive_expect_tx(void* mbar, unsigned bytes);
+void bulk_issue(void* smem_dst, const void* gsrc, unsigned bytes, void* mbar, int tu, int line);
+void mbar_wait(void* mbar, unsigned parity);
 // race detector hook (always returns true); a pointer outside the CTA's dynamic shared memory is ignored
 bool smem_access(const void* p, size_t bytes, bool write, int tu, int line);
 enum { OP_SYNCWARP = 0, OP_BALLOT = 1, OP_SHFL_DOWN = 2, OP_SHFL_XOR = 3, OP_SHFL_IDX = 4, OP_SHFL_UP = 5 };

@@ -74,11 +74,17 @@ class EmuCtx:
     def __exit__(self, *a):
         self.close()
 
-    def apply(self, v):
-        v = np.ascontiguousarray(v, dtype=NDT[self.prec])
-        y = np.full(self.dim, np.nan, dtype=NDT[self.prec])
-        _check(lib().ftlm_apply_H(self.ctx, _p(v), _p(y), C.c_void_p(0)))
-        return y
+    def apply(self, v, shift=0):
+        """shift: the caller's vectors start `shift` elements after a 64-byte boundary (a slice of a larger buffer:
+        only element alignment is guaranteed to the library)."""
+        buf_v = np.zeros(self.dim + 32, dtype=NDT[self.prec])
+        buf_y = np.full(self.dim + 32, np.nan, dtype=NDT[self.prec])
+        off = (-buf_v.ctypes.data // buf_v.itemsize) % (64 // buf_v.itemsize) + shift
+        offy = (-buf_y.ctypes.data // buf_y.itemsize) % (64 // buf_y.itemsize) + shift
+        vv, y = buf_v[off:off + self.dim], buf_y[offy:offy + self.dim]
+        vv[:] = v
+        _check(lib().ftlm_apply_H(self.ctx, _p(vv), _p(y), C.c_void_p(0)))
+        return y.copy()
 
     def apply_into(self, v, y):
         """y is read-modify-written when only PASS-B windows run (option debug_pass_mask)."""

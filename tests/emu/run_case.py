@@ -90,7 +90,7 @@ def main():
         if "apply" in what:
             rng = np.random.default_rng(spec.get("seed", 1))
             v = rng.standard_normal(D).astype(E.NDT[prec])
-            y = c.apply(v)
+            y = c.apply(v, spec.get("shift", 0))
             ref = fo.apply_H(basis, w.N, w.bond_i, w.bond_j, w.J, h, n_up, v.astype(np.float64))
             den = np.linalg.norm(ref)
             err = float(np.linalg.norm(y.astype(np.float64) - ref) / (den if den > 0 else 1.0))

@@ -125,6 +125,16 @@ def test_emu_tmlr_in_tile_pass(wl, n_up, split, mode, prec, opts):
     assert res["tmlr"] == [1, 1] and res["passb"][0] >= 1
 
 
+@pytest.mark.parametrize("shift,prec", [(1, "fp32"), (2, "fp32"), (3, "fp32"), (1, "fp64")])
+def test_emu_tmlr_bulk_copy_with_unaligned_caller_vectors(shift, prec):
+    """The tile's bulk copy (cp.async.bulk: 16-byte aligned source, destination, size) takes its alignment from the
+    actual address of the caller's vector, which is only element-aligned (a slice of a larger buffer)."""
+    res = run_case({"wl": "fring16j", "n_up": 8, "mode": "clt", "prec": prec, "shift": shift,
+                    "options": [["passb", 1], ["passb_lo_min", 4], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]], ["tmlr", 1]],
+                    "what": ["apply"]})
+    assert res["tmlr"] == [1, 1]
+
+
 def test_emu_passb_off_keeps_top_bonds_in_tml():
     res = run_case({"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp64",
                     "options": [["passb", 0], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]],
@@ -205,10 +215,13 @@ def test_emu_lazy_normalisation_matches_separate_pass():
          "options": [["passb", 1], ["tml_split", 5 | (3 << 8)], ["kernel", 3]], "what": ["apply"]}, "cp.async"),
     (2, {"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp32",
          "options": [["tml_low_bits", 6], ["tml_mid_bits", 4], ["kernel", 3]], "what": ["apply"]}, "shared-memory race"),
+    (3, {"wl": "fring16j", "n_up": 8, "mode": "cr", "prec": "fp32",
+         "options": [["passb", 1], ["passb_lo_min", 4], ["tml_split", 5 | (3 << 8)], ["kernel", 3], ["tmlr", 1]], "what": ["apply"]}, "mbarrier"),
 ])
 def test_emu_detects_removed_synchronisation(neg, spec, expect):
     """Negative test of the checker: a copy of the library with ONE synchronisation removed (1: the cp.async wait of
-    PASS-B's staging, 2: the __syncwarp between building and reading TML's descriptor lists) must be killed by the
+    PASS-B's staging, 2: the __syncwarp between building and reading TML's descriptor lists, 3: the mbarrier wait after the bulk copy of
+    TMLR's tile) must be killed by the
     emulation - by the deferred cp.async model / the shared-memory race detector - while the intact library passes
     the same case."""
     import build_emu
