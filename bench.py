@@ -172,25 +172,42 @@ def run_probe(args):
     mode = ftlm.INDEX_CR if (args.mode == "cr" or w.N > 32) else ftlm.INDEX_CLT
     ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, mode, ftlm.FP32, 0.0, torch.cuda.current_device())
     ftlm.ftlm_set_option(ctx, "allow_unverified", 1)
-    if args.probe_stage == "batchcheck":
-        # checked library: three fused steps of `batch` interleaved chains through the TML kernel (no windows) against
-        # the same chains through the thread-per-row kernel one at a time; zero suppressed accesses
-        assert ftlm.CHECKED, "checked probe stage needs FTLM_CHECKED=1"
+    if args.probe_stage in ("batchcheck", "batchtime"):
+        # batch > 1.  "batchcheck" (checked library): three fused steps of `batch` interleaved chains through each batched
+        # configuration (TML in-tile pass + PASS-B windows; TML with global reads) against the same chains through
+        # the thread-per-row kernel one at a time; zero suppressed accesses.  "batchtime" (release library): times the
+        # configurations named by --names over whole fused steps.
         B = args.batch
-        ftlm.ftlm_set_option(ctx, "kernel", 1)
-        ref = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, B, 3)
+        names = [n for n in (args.names.split(",") if args.names else ["tml+passb", "tml"])]
+        out = {}
+        if args.probe_stage == "batchcheck":
+            assert ftlm.CHECKED, "checked probe stage needs FTLM_CHECKED=1"
+            ftlm.ftlm_set_option(ctx, "kernel", 1)
+            ref = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, B, 3)
+        else:
+            assert not ftlm.CHECKED
         ftlm.ftlm_set_option(ctx, "batch", B)
-        ftlm.ftlm_set_option(ctx, "passb", 0)
-        ok = False
-        try:
-            ftlm.ftlm_set_option(ctx, "kernel", 3)
-            got = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, B, 3)
-            ok = bool(np.abs(got["alpha"] - ref["alpha"]).max() <= 1e-4 and np.abs(got["beta"] - ref["beta"]).max() <= 1e-4)
-        except ftlm.FtlmError:
-            ok = False
+        for name in names:
+            try:
+                for key, val in CANDIDATES[name]:
+                    ftlm.ftlm_set_option(ctx, key, val)
+                if args.probe_stage == "batchcheck":
+                    got = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, B, 3)
+                    out[name] = bool(np.abs(got["alpha"] - ref["alpha"]).max() <= 1e-4 and np.abs(got["beta"] - ref["beta"]).max() <= 1e-4)
+                else:
+                    ftlm.ftlm_chain_begin_batch(ctx, W.SEED_VECTORS, 0, B)
+                    ftlm.ftlm_chain_steps(ctx, 2)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    ftlm.ftlm_chain_steps(ctx, 5)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    out[name] = e0.elapsed_time(e1) / 5
+            except ftlm.FtlmError:
+                out[name] = False
         info = ftlm.ftlm_check_info()
         ftlm.ftlm_destroy(ctx)
-        print(json.dumps({"stage": "batchcheck", "ok": ok, "check": info}), flush=True)
+        print(json.dumps({"stage": args.probe_stage, "result": out, "check": info}), flush=True)
         return
     if args.probe_stage == "checked":
         assert ftlm.CHECKED, "checked probe stage needs FTLM_CHECKED=1"
@@ -217,17 +234,27 @@ def _child_json(cmd, env, timeout):
 
 
 def probe_batch(args):
-    """batch > 1: the batched TML kernel is timed only after the checked library ran it on this device without a
+    """batch > 1: a batched configuration is timed only after the checked library ran it on this device without a
     suppressed access and in agreement with the thread-per-row kernel; else the batched thread-per-row kernel."""
-    cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--probe-stage", "batchcheck", "--config", str(args.config),
-           "--mode", args.mode, "--batch", str(args.batch)]
+    cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--config", str(args.config), "--mode", args.mode, "--batch", str(args.batch)]
     try:
         from paper_2605_26261_b200 import build
         build.build(checked=True)
-        d, err = _child_json(cmd, dict(os.environ, FTLM_CHECKED="1"), 1800)
-        if d and d.get("ok") and d["check"].get("check_violations") == 0:
-            return "tml", None, None
-        return "row", None, f"batch check: {err or d}"
+        d, err = _child_json(cmd + ["--probe-stage", "batchcheck"], dict(os.environ, FTLM_CHECKED="1"), 1800)
+        if not d or d["check"].get("check_violations") != 0:
+            return "row", None, f"batch check: {err or d}"
+        ok = [n for n, v in d["result"].items() if v is True]
+        if not ok:
+            return "row", d, "batch check: no valid batched configuration"
+        env = dict(os.environ)
+        env.pop("FTLM_CHECKED", None)
+        d2, err = _child_json(cmd + ["--probe-stage", "batchtime", "--names", ",".join(ok)], env, 900)
+        if not d2:
+            return "row", d, "batch timing " + str(err)
+        timed = {n: v for n, v in d2["result"].items() if v is not False}
+        if not timed:
+            return "row", d2, "batch timing: nothing ran"
+        return min(timed, key=timed.get), {"checked": d["result"], "release_ms": d2["result"]}, None
     except Exception as e:
         return "row", None, f"batch check failed: {e!r}"
 
@@ -320,7 +347,8 @@ def run_all(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--probe", action="store_true", help=argparse.SUPPRESS)
-    ap.add_argument("--probe-stage", default="checked", choices=["checked", "release", "batchcheck"], help=argparse.SUPPRESS)
+    ap.add_argument("--probe-stage", default="checked", choices=["checked", "release", "batchcheck", "batchtime"], help=argparse.SUPPRESS)
+    ap.add_argument("--names", default="", help=argparse.SUPPRESS)
     ap.add_argument("--mask", type=int, default=0, help=argparse.SUPPRESS)
     ap.add_argument("--candidate", default="", help="one of " + ", ".join(CANDIDATES))
     ap.add_argument("--gpus", type=int, default=1)
@@ -395,8 +423,8 @@ def main():
         ftlm.ftlm_set_option(ctx, "tml_low_bits", args.tml_low_bits)
     if args.tml_mid_bits:
         ftlm.ftlm_set_option(ctx, "tml_mid_bits", args.tml_mid_bits)
-    if B > 1:                                                    # batched chains: TML without windows, or ROW
-        for key in ("lazy_norm", "tmlr", "passb"):
+    if B > 1:                                                    # batched chains: TML in-tile pass (+ windows), or ROW
+        for key in ("lazy_norm", "tmlr"):
             ftlm.ftlm_set_option(ctx, key, 0)
         ftlm.ftlm_set_option(ctx, "batch", B)
     ftlm.ftlm_set_option(ctx, "graph", args.graph)

@@ -68,7 +68,8 @@ int ftlm_destroy(ftlm_ctx* ctx);
 int64_t ftlm_dim(const ftlm_ctx* ctx);
 
 /* Options: "kernel" (FTLM_KERNEL_*), "batch" (1, 2, 4: chains ftlm_lanczos / ftlm_lanczos_host advance together on
- * interleaved vectors, L207; default 1),
+ * interleaved vectors, L207; default 1; rebuilds the tile split and the windows for rows of that many values),
+ * "plan_batch" (0 = follow "batch"; else build the plans for that many chains even when fewer run),
  * "tml_low_bits" / "tml_mid_bits" / "tml_split" = w | m << 8 (split of the TML kernels, 0 = auto),
  * "graph" (1 = ftlm_chain_steps captures two consecutive fused steps - three with "lazy_norm" - into a CUDA graph
  * once and replays it; same kernels, same arithmetic, fewer launches: for the launch-bound small sectors; falls back
@@ -150,8 +151,10 @@ int ftlm_chain_end(ftlm_ctx* ctx, double* h_alpha, double* h_beta, int cap, int*
  * r0 .. r0 + batch - 1 from their seeded start vectors on interleaved work vectors q[t][batch]; every fused pass
  * then computes the row state and every neighbour index once for all of them.  ftlm_chain_steps advances the whole
  * batch; each chain has its own alpha, beta and breakdown state, and its coefficients are bit-identical to those of
- * the same chain run alone with the same kernel and tile split.  batch > 1 runs the ROW kernel or the TML kernel
- * without PASS-B windows (FTLM_EUNSUPPORTED while option "passb" is 1).  Asynchronous. */
+ * the same chain run alone with the same kernel, tile split and windows (option "plan_batch" builds a single chain's
+ * plans for a batch's geometry).  batch > 1 runs the ROW kernel, or the TML in-tile pass with or without PASS-B
+ * windows (the register-table TMLR pass and lazy normalisation are single-vector); batch must not exceed the batch
+ * the handle's plans were built for (options "batch" / "plan_batch"; FTLM_EINVAL).  Asynchronous. */
 int ftlm_chain_begin_batch(ftlm_ctx* ctx, uint64_t seed, int r0, int batch, void* stream);
 
 /* ftlm_chain_end for the batch in progress: chain b -> h_alpha[b*cap ...], h_beta[b*cap ...], h_m_eff[b]. */

@@ -140,6 +140,7 @@ struct ftlm_ctx {
   double* d_partials = nullptr;    // [3 * FTLM_MAX_BATCH][max_blocks]
   unsigned int* d_ticket = nullptr;  // [FTLM_MAX_BATCH]
   int batch = 1;                   // option "batch": chains ftlm_lanczos advances together on interleaved vectors (1, 2, 4)
+  int plan_batch = 0;              // option "plan_batch": build the tile / window plans for this many chains even when fewer run (0 = follow "batch")
   int cur_batch = 1;               // batch of the chain(s) in progress
   int q_batch = 0;                 // batch the work vectors were allocated for
   int max_blocks = 0;
@@ -182,7 +183,9 @@ void ftlm_passb_window_geometry(const ftlm_ctx* c, int window, int* lo, int* s);
 int64_t ftlm_passb_info(const ftlm_ctx* c, const char* key);
 // y += sum over the windows' bonds of (J_b/2)(P_b - 1) v.  fused: the last window also accumulates the
 // three FP64 sums over the final y and advances the chain state.
-int ftlm_launch_passb(ftlm_ctx* c, const void* v, void* y, int fused, cudaStream_t s);
+int ftlm_launch_passb(ftlm_ctx* c, const void* v, void* y, int fused, int batch, cudaStream_t s);
+// chains the plans (tile split, window sizes) are built for
+static inline int ftlm_plan_batch(const ftlm_ctx* c) { return c->plan_batch > c->batch ? c->plan_batch : c->batch; }
 
 // ---- device helpers ---------------------------------------------------------------------
 #ifdef __CUDACC__

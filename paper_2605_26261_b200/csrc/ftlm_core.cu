@@ -494,16 +494,20 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   if (!strcmp(key, "debug_item_count")) { c->debug_item_count = value; return FTLM_OK; }
 #endif
   if (!strcmp(key, "autotune_mask")) { c->autotune_mask = (uint64_t)value; return FTLM_OK; }
-  if (!strcmp(key, "batch")) {
-    // chains per row pass of ftlm_lanczos / ftlm_lanczos_host (L207, L309); the TML split is re-chosen so that a
-    // tile of `batch` interleaved vectors fits shared memory
-    if (value != 1 && value != 2 && value != 4) { ftlm_set_error("batch must be 1, 2 or 4"); return FTLM_EINVAL; }
-    const int old = c->batch;
-    c->batch = (int)value;
+  if (!strcmp(key, "batch") || !strcmp(key, "plan_batch")) {
+    // "batch": chains per row pass of ftlm_lanczos / ftlm_lanczos_host (L207, L309); the TML split and the window
+    // sizes are re-chosen so that tiles of `batch` interleaved vectors fit shared memory.  "plan_batch" (0 = follow
+    // "batch"): build the plans for this many chains even when fewer run (same tiles and windows, hence the same
+    // order of every sum: a chain then has bit-identical coefficients alone and inside a batch).
+    const bool is_plan = key[0] == 'p';
+    if (!(value == 1 || value == 2 || value == 4 || (is_plan && value == 0))) { ftlm_set_error("%s must be 1, 2 or 4", key); return FTLM_EINVAL; }
+    int* slot = is_plan ? &c->plan_batch : &c->batch;
+    const int old = *slot;
+    *slot = (int)value;
     CK(cudaSetDevice(c->device));
     ftlm_tml_plan_destroy(c);
     int rc = ftlm_tml_plan_create(c);
-    if (rc != FTLM_OK) { c->batch = old; ftlm_tml_plan_destroy(c); ftlm_tml_plan_create(c); }
+    if (rc != FTLM_OK) { *slot = old; ftlm_tml_plan_destroy(c); ftlm_tml_plan_create(c); }
     return rc;
   }
   if (!strcmp(key, "passb") || !strcmp(key, "tml_split")) {
@@ -561,6 +565,7 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!strcmp(key, "allow_unverified")) return c->allow_unverified;
   if (!strcmp(key, "autotune_mask")) return (int64_t)c->autotune_mask;
   if (!strcmp(key, "batch")) return c->batch;
+  if (!strcmp(key, "plan_batch")) return c->plan_batch;
   if (!strcmp(key, "tmlr")) return c->use_tmlr;
   if (!strcmp(key, "lazy_norm")) return c->lazy_norm;
   if (!strcmp(key, "lazy_norm_ok")) return ftlm_tmlr_lazy_ok(c) ? 1 : 0;
@@ -583,27 +588,21 @@ extern "C" int ftlm_clt_read(ftlm_ctx* c, int64_t b0, int64_t nb, uint32_t* h_ma
 // ---- H.v ---------------------------------------------------------------------------------------
 static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s, int batch = 1) {
   const int k = ftlm_effective_kernel(c);
-  if (batch > 1) {
-    // batched chains (L207, L309): the TML kernel with every bond that leaves the tile as a global read, or ROW;
-    // the window passes and the register-table in-tile pass are single-vector kernels
-    if (k == FTLM_KERNEL_TML) {
-      if (c->passb) { ftlm_set_error("batch > 1: set option \"passb\" to 0 (the PASS-B window passes take one vector)"); return FTLM_EUNSUPPORTED; }
-      return ftlm_launch_hv_tml(c, v, qp, y, fused, batch, s);
-    }
-    return ftlm_launch_hv_row(c, v, qp, y, fused, batch, s);
-  }
   if (k == FTLM_KERNEL_TML) {
-    // two-pass step when PASS-B windows exist: the TML pass leaves the sums and the finish to PASS-B
+    // multi-pass step when PASS-B windows exist: the in-tile pass leaves the sums and the finish to the last window.
+    // batch > 1 (L207): rows of `batch` interleaved chains through the same passes (TML in-tile pass; the
+    // register-table TMLR pass is a single-vector kernel)
     const bool pb = c->passb != nullptr;
     int rc = FTLM_OK;
+    if (batch > ftlm_plan_batch(c)) { ftlm_set_error("batch %d: the plans of this handle were built for %d chains (option \"batch\")", batch, ftlm_plan_batch(c)); return FTLM_EINVAL; }
     if (fused || !c->debug_pass_mask || (c->debug_pass_mask & 1)) {
-      if (c->use_tmlr && c->tmlr) rc = ftlm_launch_hv_tmlr(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, s);
-      else rc = ftlm_launch_hv_tml(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, 1, s);
+      if (c->use_tmlr && c->tmlr && batch == 1) rc = ftlm_launch_hv_tmlr(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, s);
+      else rc = ftlm_launch_hv_tml(c, v, qp, y, fused ? (pb ? 2 : 1) : 0, batch, s);
     }
-    if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, s);
+    if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, batch, s);
     return rc;
   }
-  return ftlm_launch_hv_row(c, v, qp, y, fused, 1, s);
+  return ftlm_launch_hv_row(c, v, qp, y, fused, batch, s);
 }
 
 extern "C" int ftlm_apply_H(ftlm_ctx* c, const void* d_v, void* d_y, void* stream) {
@@ -760,7 +759,7 @@ static int chain_one_step(ftlm_ctx* c, cudaStream_t s, bool timed, float* ms_hv,
   if (lazy && c->pending_norm) {
     const bool pb = c->passb != nullptr;
     rc = ftlm_launch_hv_tmlr_lazy(c, c->q[c->ic], c->q[c->ia], c->q[c->ib], pb ? 2 : 1, s);
-    if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, c->q[c->ic], c->q[c->ib], 1, s);
+    if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, c->q[c->ic], c->q[c->ib], 1, 1, s);
     const int a = c->ia, b = c->ib, y = c->ic;             // q_{j+1} now lives in the old y, q_j becomes q_prev, y is the old q_{j-1}
     c->ia = y; c->ib = a; c->ic = b;
   } else {

@@ -20,13 +20,15 @@
 
 #define FTLM_TU 5
 #include "ftlm_passb.cuh"
+#include "ftlm_vec.cuh"
 
 #define PASSB_MAX_BONDS 31          // one neighbour entry per lane; entry 31 holds the count and the sum of J
 #define PASSB_MAX_S 12
 #define PASSB_THREADS 1024
 #define PASSB_END 0xFFFFFFFFu
 #define PASSB_XK 2                  // run offsets per lane and window word (X = 32 * xk, xk <= PASSB_XK)
-#define PASSB_PF 8                  // window words whose y is in flight per warp
+#define PASSB_RED_DOUBLES (32 * 3 * FTLM_MAX_BATCH + 64 + 3 * FTLM_MAX_BATCH + 4)   // per-warp sums + finish_chains scratch; even: the tile behind it stays 16-byte aligned
+#define PASSB_PF 8                  // window words whose y is in flight per warp (divided by the batch: registers)
 
 template <typename R>
 struct PassBParams {
@@ -39,13 +41,13 @@ struct PassBParams {
   const uint2* clt;
   const uint16_t* ustate;           // [2^s]: window words grouped by popcount, ascending inside a group
   const int* koff;                  // [s+2]: first slot of popcount class p in ustate
-  const uint32_t* nbr_off;          // [2^s][32], row = position of u in ustate: byte offset of row slot(u') in the tile; [31] = number of entries
+  const uint32_t* nbr_off;          // [2^s][32], row = position of u in ustate: index of row slot(u') * X in the tile; [31] = number of entries
   const R* nbr_J;                   // [2^s][32]: J_b/2 of the same entries; [31] = their sum
   const uint32_t* grp_first;        // [ngroups+1]: first item of group g = F*(s+1) + p_S
   const uint32_t* item_group;       // [nitems]: group of every item
-  double* partials;                 // [3][nitems]
+  double* partials;                 // [3 * B][nitems]
   unsigned int* counter;            // [0] item counter, [1] ticket
-  ChainState* st;
+  ChainState* st;                   // [B]
   int xk[PASSB_MAX_S + 1];          // X/32 per popcount class
   int max_conf;                     // largest C(s, p_S) among non-empty classes
   int unij;                         // every bond of the window has the same J_b/2 (= Juni)
@@ -63,7 +65,7 @@ struct PassBWindow {
   std::vector<double> Jh;
   uint16_t* d_ustate = nullptr;
   int* d_koff = nullptr;
-  uint32_t* d_nbr = nullptr;          // byte offsets
+  uint32_t* d_nbr = nullptr;          // row indices in the tile
   void* d_nbrJ = nullptr;             // J_b/2 in the handle's precision
   uint32_t* d_grp_first = nullptr;
   uint32_t* d_item_group = nullptr;
@@ -87,21 +89,24 @@ __host__ __device__ inline uint64_t bits_deposit(uint64_t x, uint64_t mask) {
   return r;
 }
 
+// esz = bytes of one row of the batch (element size x chains)
 __host__ __device__ inline size_t passb_smem_bytes(int N, int K, int max_conf, int max_rows, int esz) {
   size_t o = 0;
   o += ((size_t)(N + 1) * (K + 1) * 8 + 15) & ~(size_t)15;      // binom
   o += ((size_t)max_conf * 8 + 15) & ~(size_t)15;               // run starts
-  o += (size_t)32 * 3 * 8;                                      // reduction scratch
+  o += (size_t)PASSB_RED_DOUBLES * 8;                           // reduction scratch (per-warp sums; finish_chains)
   o += (size_t)max_rows * esz;                                  // tile: max over classes of C(s,p) * X
   return o;
 }
 
-// Phase 2 of one work item, specialised on the run offsets per lane (XKC) and on uniform couplings (UNIJ) so
-// that an item executes one straight variant of the word loop (small instruction working set).
-template <typename R, bool FUSED, int XKC, bool UNIJ>
-__device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* tile, R* __restrict__ y, const uint64_t* s_start,
+// Phase 2 of one work item, specialised on the run offsets per lane (XKC), on uniform couplings (UNIJ) and on the
+// batch B (rows of B interleaved chains, L207) so that an item executes one straight variant of the word loop.
+template <typename R, int B, bool FUSED, int XKC, bool UNIJ>
+__device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const Vec<R, B>* tile, Vec<R, B>* __restrict__ y, const uint64_t* s_start,
                                              int c0, int nconf, int X, uint64_t x0, int nx, int lane, int warp, int NW,
-                                             double& s_qy, double& s_yy, double& s_qq) {
+                                             double* s_qy, double* s_yy, double* s_qq) {
+  typedef Vec<R, B> V;
+  constexpr int PF = PASSB_PF / B;
   // neighbour rows are stored in window-word order (row c0 + sl); the row of the next word is requested
   // while the current word is processed
   uint32_t eo_n = 0;
@@ -110,67 +115,79 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* t
     eo_n = LDG(&p.nbr_off[(size_t)(c0 + warp) * 32 + lane]);
     eJ_n = LDG(&p.nbr_J[(size_t)(c0 + warp) * 32 + lane]);
   }
-  for (int sl0 = warp; sl0 < nconf; sl0 += NW * PASSB_PF) {
-    R yold[PASSB_PF][PASSB_XK];
+  for (int sl0 = warp; sl0 < nconf; sl0 += NW * PF) {
+    V yold[PF][PASSB_XK];
 #pragma unroll
-    for (int j = 0; j < PASSB_PF; ++j) {
+    for (int j = 0; j < PF; ++j) {
       const int sl = sl0 + j * NW;
 #pragma unroll
       for (int k = 0; k < PASSB_XK; ++k) {
         const int x = lane + 32 * k;
-        yold[j][k] = (sl < nconf && k < XKC && x < nx) ? LDCS(y + LD_S(&s_start[sl]) + x0 + x) : (R)0;
+        if (sl < nconf && k < XKC && x < nx) yold[j][k] = vec_ldcs(y + LD_S(&s_start[sl]) + x0 + x);
+        else yold[j][k] = V{};
       }
     }
 #pragma unroll
-    for (int j = 0; j < PASSB_PF; ++j) {
+    for (int j = 0; j < PF; ++j) {
       const int sl = sl0 + j * NW;
       if (sl >= nconf) break;
-      const uint32_t eo = eo_n;
+      const uint32_t eo_rows = eo_n;
       const R eJ = eJ_n;
       if (sl + NW < nconf) {
         eo_n = LDG(&p.nbr_off[(size_t)(c0 + sl + NW) * 32 + lane]);
         eJ_n = LDG(&p.nbr_J[(size_t)(c0 + sl + NW) * 32 + lane]);
       }
-      const int cnt = (int)__shfl_sync(0xffffffffu, eo, 31);
+      const int cnt = (int)__shfl_sync(0xffffffffu, eo_rows, 31);
+      const uint32_t eo = eo_rows * (uint32_t)sizeof(V);    // row index -> byte offset, once per word (entry 31 is not an offset)
       const R sumJ = __shfl_sync(0xffffffffu, eJ, 31);
       // lanes past the end of the run (x >= nx) read stale tile words and are discarded at the store
-      const unsigned char* tl = (const unsigned char*)tile + (size_t)lane * sizeof(R);
-      R* yrow = y + LD_S(&s_start[sl]) + x0;
-      R own[PASSB_XK], acc[PASSB_XK];
-      own[0] = LD_S((const R*)(tl + (size_t)sl * X * sizeof(R)));
-      acc[0] = (R)0;
+      const unsigned char* tl = (const unsigned char*)tile + (size_t)lane * sizeof(V);
+      V* yrow = y + LD_S(&s_start[sl]) + x0;
+      V own[PASSB_XK], acc[PASSB_XK];
+      own[0] = LD_S((const V*)(tl + (size_t)sl * X * sizeof(V)));
+      acc[0] = V{};
       if (XKC == 1) {
-        own[1] = (R)0; acc[1] = (R)0;
+        own[1] = V{}; acc[1] = V{};
         if (UNIJ) {                                  // one J_b for the whole window: add, multiply once
 #pragma unroll 4
-          for (int e = 0; e < cnt; ++e) acc[0] += LD_S((const R*)(tl + __shfl_sync(0xffffffffu, eo, e)));
-          acc[0] *= p.Juni;
+          for (int e = 0; e < cnt; ++e) {
+            const V g = LD_S((const V*)(tl + __shfl_sync(0xffffffffu, eo, e)));
+#pragma unroll
+            for (int c = 0; c < B; ++c) acc[0].x[c] += g.x[c];
+          }
+#pragma unroll
+          for (int c = 0; c < B; ++c) acc[0].x[c] *= p.Juni;
         } else {
 #pragma unroll 4
           for (int e = 0; e < cnt; ++e) {
             const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
             const R J = __shfl_sync(0xffffffffu, eJ, e);
-            acc[0] += J * LD_S((const R*)(tl + off));
+            const V g = LD_S((const V*)(tl + off));
+#pragma unroll
+            for (int c = 0; c < B; ++c) acc[0].x[c] += J * g.x[c];
           }
         }
       } else {
-        own[1] = LD_S((const R*)(tl + (size_t)sl * X * sizeof(R) + 32 * sizeof(R)));
-        acc[1] = (R)0;
+        own[1] = LD_S((const V*)(tl + (size_t)sl * X * sizeof(V) + 32 * sizeof(V)));
+        acc[1] = V{};
         if (UNIJ) {
 #pragma unroll 4
           for (int e = 0; e < cnt; ++e) {
             const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
-            acc[0] += LD_S((const R*)(tl + off));
-            acc[1] += LD_S((const R*)(tl + off + 32 * sizeof(R)));
+            const V g0 = LD_S((const V*)(tl + off)), g1 = LD_S((const V*)(tl + off + 32 * sizeof(V)));
+#pragma unroll
+            for (int c = 0; c < B; ++c) { acc[0].x[c] += g0.x[c]; acc[1].x[c] += g1.x[c]; }
           }
-          acc[0] *= p.Juni; acc[1] *= p.Juni;
+#pragma unroll
+          for (int c = 0; c < B; ++c) { acc[0].x[c] *= p.Juni; acc[1].x[c] *= p.Juni; }
         } else {
 #pragma unroll 4
           for (int e = 0; e < cnt; ++e) {
             const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
             const R J = __shfl_sync(0xffffffffu, eJ, e);
-            acc[0] += J * LD_S((const R*)(tl + off));
-            acc[1] += J * LD_S((const R*)(tl + off + 32 * sizeof(R)));
+            const V g0 = LD_S((const V*)(tl + off)), g1 = LD_S((const V*)(tl + off + 32 * sizeof(V)));
+#pragma unroll
+            for (int c = 0; c < B; ++c) { acc[0].x[c] += J * g0.x[c]; acc[1].x[c] += J * g1.x[c]; }
           }
         }
       }
@@ -178,26 +195,38 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const R* t
       for (int k = 0; k < PASSB_XK; ++k) {
         const int x = lane + 32 * k;
         if (k < XKC && x < nx) {
-          const R yn = yold[j][k] + (acc[k] - sumJ * own[k]);
-          STCS(&yrow[x], yn);
-          if (FUSED) {
-            s_qy += (double)own[k] * (double)yn;
-            s_yy += (double)yn * (double)yn;
-            s_qq += (double)own[k] * (double)own[k];
+          V yn;
+#pragma unroll
+          for (int c = 0; c < B; ++c) {
+            yn.x[c] = yold[j][k].x[c] + (acc[k].x[c] - sumJ * own[k].x[c]);
+            if (FUSED) {
+              s_qy[c] += (double)own[k].x[c] * (double)yn.x[c];
+              s_yy[c] += (double)yn.x[c] * (double)yn.x[c];
+              s_qq[c] += (double)own[k].x[c] * (double)own[k].x[c];
+            }
           }
+          vec_stcs(&yrow[x], yn);
         }
       }
     }
   }
 }
 
-template <typename R, int MODE, bool FUSED>
+template <typename R, int B, int MODE, bool FUSED>
 __global__ void __launch_bounds__(PASSB_THREADS, 1)
-passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, R* __restrict__ y) {
+passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v_, R* __restrict__ y_) {
+  typedef Vec<R, B> V;
   FTLM_DYN_SMEM(smem);
   __shared__ unsigned int s_item;
   __shared__ bool s_last;
-  if (FUSED && p.st->done) return;
+  if (FUSED) {
+    bool all_done = true;
+#pragma unroll
+    for (int c = 0; c < B; ++c) all_done = all_done && p.st[c].done;
+    if (all_done) return;
+  }
+  const V* __restrict__ v = (const V*)v_;
+  V* __restrict__ y = (V*)y_;
   const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
   const int K1 = p.K + 1;
   uint64_t* s_binom = (uint64_t*)smem;
@@ -205,8 +234,9 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
   uint64_t* s_start = (uint64_t*)(smem + o);
   o += ((size_t)p.max_conf * 8 + 15) & ~(size_t)15;
   double* s_red = (double*)(smem + o);
-  o += (size_t)32 * 3 * 8;
-  R* tile = (R*)(smem + o);
+  o += (size_t)PASSB_RED_DOUBLES * 8;
+  static_assert((PASSB_RED_DOUBLES * 8) % 16 == 0, "tile alignment");
+  V* tile = (V*)(smem + o);
   for (int k = tid; k < (p.N + 1) * K1; k += NT) ST_S(&s_binom[k], LD_G(&p.binom[k]));
   int cur_group = -1;
   const int s1 = p.s + 1;
@@ -240,39 +270,44 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
     const int nx = left < (uint64_t)X ? (int)left : X;  // valid offsets in this chunk
     // ---- phase 1: stage the run chunks (cp.async: every copy of the item is in flight at once) ------
     for (int sl = warp; sl < nconf; sl += NW) {
-      const R* src = v + LD_S(&s_start[sl]) + x0;
-      R* dst = tile + (size_t)sl * X;
+      const V* src = v + LD_S(&s_start[sl]) + x0;
+      V* dst = tile + (size_t)sl * X;
 #pragma unroll
       for (int k = 0; k < PASSB_XK; ++k) {
         const int x = lane + 32 * k;
-        if (k < XK && x < nx) cp_async_elem(&dst[x], &src[x]);
+        if (k < XK && x < nx) cp_async_vec(&dst[x], &src[x]);
       }
     }
 #if !defined(FTLM_NEG_TEST) || FTLM_NEG_TEST != 1     // (negative test of the host emulation: tests/emu/build_emu.py)
     cp_async_wait_all();
 #endif
     __syncthreads();
-    // ---- phase 2: one warp per window word; y of PASSB_PF words is requested before the first is used ---
-    double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
+    // ---- phase 2: one warp per window word; y of PASSB_PF / B words is requested before the first is used ---
+    double s_qy[B], s_yy[B], s_qq[B];
+#pragma unroll
+    for (int c = 0; c < B; ++c) { s_qy[c] = 0.0; s_yy[c] = 0.0; s_qq[c] = 0.0; }
     if (XK == 1) {
-      if (p.unij) passb_phase2<R, FUSED, 1, true>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
-      else passb_phase2<R, FUSED, 1, false>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
+      if (p.unij) passb_phase2<R, B, FUSED, 1, true>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
+      else passb_phase2<R, B, FUSED, 1, false>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
     } else {
-      if (p.unij) passb_phase2<R, FUSED, 2, true>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
-      else passb_phase2<R, FUSED, 2, false>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
+      if (p.unij) passb_phase2<R, B, FUSED, 2, true>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
+      else passb_phase2<R, B, FUSED, 2, false>(p, tile, y, s_start, c0, nconf, X, x0, nx, lane, warp, NW, s_qy, s_yy, s_qq);
     }
     if (FUSED) {                                        // deterministic per-item partial sums
-      const double a = warp_sum(s_qy), b = warp_sum(s_yy), c = warp_sum(s_qq);
-      if (lane == 0) { ST_S(&s_red[warp * 3], a); ST_S(&s_red[warp * 3 + 1], b); ST_S(&s_red[warp * 3 + 2], c); }
+#pragma unroll
+      for (int c = 0; c < B; ++c) {
+        const double a = warp_sum(s_qy[c]), b = warp_sum(s_yy[c]), cc = warp_sum(s_qq[c]);
+        if (lane == 0) { ST_S(&s_red[warp * 3 * B + 3 * c], a); ST_S(&s_red[warp * 3 * B + 3 * c + 1], b); ST_S(&s_red[warp * 3 * B + 3 * c + 2], cc); }
+      }
       __syncthreads();
-      if (tid < 3) {
+      if (tid < 3 * B) {
         double s = 0.0;
-        for (int wv = 0; wv < NW; ++wv) s += LD_S(&s_red[wv * 3 + tid]);
+        for (int wv = 0; wv < NW; ++wv) s += LD_S(&s_red[wv * 3 * B + tid]);
         ST_G(&p.partials[(size_t)tid * p.nitems + item], s);
       }
     }
   }
-  // ---- grid-wide finish: the last CTA resets the counters and (fused) advances the chain ----------
+  // ---- grid-wide finish: the last CTA resets the counters and (fused) advances the chains ---------
   __syncthreads();
   if (tid == 0) {
     __threadfence();
@@ -283,37 +318,7 @@ passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v, 
   __threadfence();
   if (tid == 0) { p.counter[0] = 0; p.counter[1] = 0; }
   if (!FUSED) return;
-  double tot[3];
-  for (int q = 0; q < 3; ++q) {                         // fixed assignment and order
-    double a = 0.0;
-    for (uint32_t k = tid; k < p.nitems; k += NT) a += LD_G(&p.partials[(size_t)q * p.nitems + k]);
-    a = warp_sum(a);
-    __syncthreads();
-    if (lane == 0) ST_S(&s_red[warp], a);
-    __syncthreads();
-    double s = 0.0;
-    if (tid == 0) for (int wv = 0; wv < NW; ++wv) s += LD_S(&s_red[wv]);
-    tot[q] = s;
-  }
-  if (tid == 0) {
-    ChainState* st = p.st;
-    const double a = tot[0], b = tot[1], c = tot[2];
-    const int j = st->step;
-    const double alpha = c > 0.0 ? a / c : 0.0;
-    double b2 = c > 0.0 ? b - a * a / c : 0.0;
-    if (!(b2 > 0.0)) b2 = 0.0;
-    const double beta = sqrt(b2);
-    st->alpha[j] = alpha;
-    st->beta[j] = beta;
-    double sc = st->scale;
-    sc = fmax(sc, fmax(fabs(alpha), beta));
-    st->scale = sc;
-    st->step = j + 1;
-    st->a = alpha;
-    st->inv_b = beta > 0.0 ? 1.0 / beta : 0.0;
-    st->beta_prev = beta;
-    if (j + 1 >= st->limit || beta <= st->tol * sc) { st->done = 1; st->inv_b = 0.0; }
-  }
+  finish_chains<B>(p.partials, p.nitems, p.st, s_red + 32 * 3 * FTLM_MAX_BATCH);
 }
 
 // bit k of x goes to the position of the k-th set bit of mask / back
@@ -378,7 +383,7 @@ int64_t ftlm_passb_info(const ftlm_ctx* c, const char* key) {
 // Two CTAs per SM when every class fits half of the shared memory at X >= 32: one CTA's staging
 // phase then overlaps the other's compute phase.
 static bool passb_geometry(const ftlm_ctx* c, PassBWindow& w, std::vector<uint32_t>& grp_first) {
-  const int N = c->N, K = c->N_up, esz = (int)ftlm_elem_size(c);
+  const int N = c->N, K = c->N_up, esz = (int)ftlm_elem_size(c) * ftlm_plan_batch(c);   // bytes of one row of the batch
   w.f = N - w.lo - w.s;
   if (w.f < 0 || w.f > 20 || w.s < 2 || w.s > PASSB_MAX_S || w.lo < 0) return false;
   const int s1 = w.s + 1;
@@ -441,7 +446,8 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
   c->passb = nullptr;
   if (!c->use_passb || cand.empty()) return FTLM_OK;
   const int N = c->N;
-  int smax = ftlm_elem_size(c) == 4 ? PASSB_MAX_S : PASSB_MAX_S - 1;
+  int smax = PASSB_MAX_S;                               // 12 for 4-byte rows; one position less per doubling of the row
+  for (size_t rb = ftlm_elem_size(c) * (size_t)ftlm_plan_batch(c); rb > 4; rb >>= 1) --smax;
   if (c->passb_smax >= 2 && c->passb_smax < smax) smax = c->passb_smax;
   int lo_min = c->passb_lo_min > 0 ? c->passb_lo_min : std::max(8, mw - 7);
   if (lo_min > mw) lo_min = mw;
@@ -550,7 +556,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
         const BondDev& d = c->bonds[(size_t)w.bonds[e]];
         const uint32_t mk = (uint32_t)bits_extract(d.mask, w.smask), x = (uint32_t)u & mk;
         if (x != 0 && x != mk) {
-          nbr[row * 32 + (size_t)n] = (uint32_t)slot[(size_t)((uint32_t)u ^ mk)] * (uint32_t)X * (uint32_t)esz;
+          nbr[row * 32 + (size_t)n] = (uint32_t)slot[(size_t)((uint32_t)u ^ mk)] * (uint32_t)X;   // row index in the tile (the kernel scales by its row size)
           nbrJ[row * 32 + (size_t)n] = d.Jh;
           sj += d.Jh;
           ++n;
@@ -566,7 +572,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
       if (bytes && h && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) return false;
       return true;
     };
-    const size_t pbytes = (size_t)w.nitems * 24;
+    const size_t pbytes = (size_t)w.nitems * 24 * FTLM_MAX_BATCH;
     bool ok = up((void**)&w.d_ustate, ustate.data(), ustate.size() * 2) && up((void**)&w.d_koff, koff.data(), koff.size() * 4) &&
               up((void**)&w.d_nbr, nbr.data(), nbr.size() * 4) &&
               up(&w.d_nbrJ, esz == 4 ? (const void*)nbrJf.data() : (const void*)nbrJ.data(), nbrJ.size() * esz) &&
@@ -579,7 +585,7 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
   return FTLM_OK;
 }
 
-template <typename R, int MODE>
+template <typename R, int B, int MODE>
 static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, int fused, cudaStream_t s) {
   PassBParams<R> p;
   memset(&p, 0, sizeof(p));
@@ -601,11 +607,11 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   int grid = c->sm_count * w.ctas;
   if ((uint32_t)grid > p.item_end - p.item_begin) grid = (int)std::max(1u, p.item_end - p.item_begin);
   if (fused) {
-    auto k = passb_kernel<R, MODE, true>;
+    auto k = passb_kernel<R, B, MODE, true>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
     FTLM_LAUNCH(k, grid, w.threads, w.smem, s, p, (const R*)v, (R*)y);
   } else {
-    auto k = passb_kernel<R, MODE, false>;
+    auto k = passb_kernel<R, B, MODE, false>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
     FTLM_LAUNCH(k, grid, w.threads, w.smem, s, p, (const R*)v, (R*)y);
   }
@@ -613,20 +619,23 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   return FTLM_OK;
 }
 
-int ftlm_launch_passb(ftlm_ctx* c, const void* v, void* y, int fused, cudaStream_t s) {
+template <typename R, int B>
+static int launch_window_m(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, int fused, cudaStream_t s) {
+  return c->mode == FTLM_INDEX_CLT ? launch_window<R, B, FTLM_INDEX_CLT>(c, w, v, y, fused, s)
+                                   : launch_window<R, B, FTLM_INDEX_CR>(c, w, v, y, fused, s);
+}
+
+int ftlm_launch_passb(ftlm_ctx* c, const void* v, void* y, int fused, int batch, cudaStream_t s) {
   PassBSet* S = c->passb;
   if (!S) return FTLM_OK;
+  if (batch > ftlm_plan_batch(c)) { ftlm_set_error("PASS-B: the window plan was built for %d chains, %d requested", ftlm_plan_batch(c), batch); return FTLM_EINVAL; }
   for (size_t wi = 0; wi < S->win.size(); ++wi) {
     PassBWindow& w = S->win[wi];
     if (!fused && c->debug_pass_mask && !((c->debug_pass_mask >> (wi + 1)) & 1)) continue;
     const int fz = (fused && wi + 1 == S->win.size()) ? 1 : 0;
     int rc;
-    if (c->prec == FTLM_FP32)
-      rc = c->mode == FTLM_INDEX_CLT ? launch_window<float, FTLM_INDEX_CLT>(c, w, v, y, fz, s)
-                                     : launch_window<float, FTLM_INDEX_CR>(c, w, v, y, fz, s);
-    else
-      rc = c->mode == FTLM_INDEX_CLT ? launch_window<double, FTLM_INDEX_CLT>(c, w, v, y, fz, s)
-                                     : launch_window<double, FTLM_INDEX_CR>(c, w, v, y, fz, s);
+    if (c->prec == FTLM_FP32) rc = batch == 1 ? launch_window_m<float, 1>(c, w, v, y, fz, s) : batch == 2 ? launch_window_m<float, 2>(c, w, v, y, fz, s) : launch_window_m<float, 4>(c, w, v, y, fz, s);
+    else rc = batch == 1 ? launch_window_m<double, 1>(c, w, v, y, fz, s) : batch == 2 ? launch_window_m<double, 2>(c, w, v, y, fz, s) : launch_window_m<double, 4>(c, w, v, y, fz, s);
     if (rc != FTLM_OK) return rc;
   }
   return FTLM_OK;

@@ -36,6 +36,7 @@
 
 #define FTLM_TU 3
 #include "ftlm_passb.cuh"
+#include "ftlm_vec.cuh"
 
 #define TML_MAX_LL 32
 #define TML_MAX_TT 64
@@ -93,46 +94,6 @@ struct TmlPlan {
 };
 
 namespace {
-
-// ---- B interleaved values of R --------------------------------------------------------------
-template <typename R, int B>
-struct __align__((sizeof(R) * B) > 16 ? 16 : (sizeof(R) * B)) Vec { R x[B]; };
-
-template <typename V> __device__ __forceinline__ V vec_ldg_(const V* p, int line) {
-  V r;
-  if (!FTLM_G_OK(p, V, line)) return V{};
-  if constexpr (sizeof(V) == 4) *(float*)&r = __ldg((const float*)p);
-  else if constexpr (sizeof(V) == 8) *(float2*)&r = __ldg((const float2*)p);
-  else {
-#pragma unroll
-    for (int k = 0; k < (int)(sizeof(V) / 16); ++k) ((float4*)&r)[k] = __ldg((const float4*)p + k);
-  }
-  return r;
-}
-template <typename V> __device__ __forceinline__ V vec_ldcs_(const V* p, int line) {
-  V r;
-  if (!FTLM_G_OK(p, V, line)) return V{};
-  if constexpr (sizeof(V) == 4) *(float*)&r = __ldcs((const float*)p);
-  else if constexpr (sizeof(V) == 8) *(float2*)&r = __ldcs((const float2*)p);
-  else {
-#pragma unroll
-    for (int k = 0; k < (int)(sizeof(V) / 16); ++k) ((float4*)&r)[k] = __ldcs((const float4*)p + k);
-  }
-  return r;
-}
-template <typename V> __device__ __forceinline__ void vec_stcs_(V* p, const V& r, int line) {
-  if (!FTLM_G_OK(p, V, line)) return;
-  if constexpr (sizeof(V) == 4) __stcs((float*)p, *(const float*)&r);
-  else if constexpr (sizeof(V) == 8) __stcs((float2*)p, *(const float2*)&r);
-  else {
-#pragma unroll
-    for (int k = 0; k < (int)(sizeof(V) / 16); ++k) __stcs((float4*)p + k, ((const float4*)&r)[k]);
-  }
-}
-
-#define vec_ldg(p) vec_ldg_((p), __LINE__)
-#define vec_ldcs(p) vec_ldcs_((p), __LINE__)
-#define vec_stcs(p, r) vec_stcs_((p), (r), __LINE__)
 
 // descriptor entries of the per-warp scratch lists
 template <typename R> struct UEnt;      // uniform gather: {offset, J}
@@ -818,7 +779,9 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
     if (forced) { ftlm_set_error("TML: low_bits=%d mid_bits=%d unusable for N=%d: %s", w, m, N, why); return (int)FTLM_EUNSUPPORTED; }
     return (int)FTLM_OK;
   };
-  if (w < 5 || w > 12 || m < 1 || m > 9 || w + m > 18 || t < 1 || t > 31) return unusable("need 5<=w<=12, 1<=m<=9, w+m<=18, 1<=t<=31");
+  // t <= 22: the per-tile partial sums (96 bytes per top part and chain) and the tile counter stay small; sparse
+  // sectors of very long labels (N = 46..48 with few up spins) fall back to the ROW kernel instead of asking for 10^11 bytes
+  if (w < 5 || w > 12 || m < 1 || m > 9 || w + m > 18 || t < 1 || t > 22) return unusable("need 5<=w<=12, 1<=m<=9, w+m<=18, 1<=t<=22");
   if (c->dim < 64) return unusable("sector too small");
   if ((uint64_t)c->dim >= (1ull << 32)) return unusable("dim >= 2^32 (row offsets are 32-bit)");
   const int mw = w + m;
@@ -937,7 +900,7 @@ static int tml_plan_try(ftlm_ctx* c, int w, int m, bool forced) {
   P->blob_bytes = (int)blob.size();
   P->h_bond_class = bclass; P->h_bond_entry = bentry;
   c->tml = P;
-  if (tml_config(c, P, c->batch).smem == 0) { c->tml = nullptr; ftlm_passb_plan_destroy(c); delete P; return unusable("tables + tile exceed shared memory"); }
+  if (tml_config(c, P, ftlm_plan_batch(c)).smem == 0) { c->tml = nullptr; ftlm_passb_plan_destroy(c); delete P; return unusable("tables + tile exceed shared memory"); }
   // ---- upload ----------------------------------------------------------------------------------
   P->partials_batch = 4;
   auto up = [&](void** d, const void* h, size_t bytes) -> bool {

@@ -490,7 +490,7 @@ void ftlm_tmlr_plan_destroy(ftlm_ctx* c) {
 int ftlm_tmlr_plan_create(ftlm_ctx* c, int w, int m, const std::vector<int>& in_window) {
   ftlm_tmlr_plan_destroy(c);
   const int N = c->N, mw = w + m, t = N - mw;
-  if (w < 5 || w > 11 || m < 1 || m > 12 || t < 1 || t > 31 || c->dim < 64 || (uint64_t)c->dim >= (1ull << 32)) return FTLM_OK;
+  if (w < 5 || w > 11 || m < 1 || m > 12 || t < 1 || t > 22 || c->dim < 64 || (uint64_t)c->dim >= (1ull << 32)) return FTLM_OK;
   TmlrPlan* P = new TmlrPlan();
   P->w = w; P->m = m; P->nT = 1u << t;
   struct LLb { uint32_t mask; };

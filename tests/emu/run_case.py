@@ -117,10 +117,11 @@ def main():
             # bit-identical to the same chain run alone (same kernel, same tile split) and agree with the oracle
             R, B = spec["batch"]
             m = min(spec.get("steps", 10), D)
+            c.set("plan_batch", B)                      # same tiles and windows for the single chains: bit-identical sums
             c.set("batch", 1)
             one = c.lanczos(W.SEED_VECTORS, R, m)
             c.set("batch", B)
-            res["batch_split"] = [c.get("tml_w"), c.get("tml_m"), c.get("kernel")]
+            res["batch_split"] = [c.get("tml_w"), c.get("tml_m"), c.get("kernel"), c.get("passb_windows")]
             many = c.lanczos(W.SEED_VECTORS, R, m)
             same = all(np.array_equal(one[k], many[k]) for k in ("alpha", "beta", "m_eff", "theta", "weight"))
             res["batch_identical"] = bool(same)
@@ -138,6 +139,7 @@ def main():
             res["batch_vs_oracle"] = worst
             res["ok"] = res["ok"] and same and worst <= tol
             c.set("batch", 1)
+            c.set("plan_batch", 0)
     res["ok"] = bool(res["ok"])
     print(json.dumps(res))
 

@@ -57,8 +57,76 @@ def workload(spec):
     raise ValueError(name)
 
 
+def run_variants(spec):
+    """Whole-vector parity of several kernel configurations of ONE workload in one process: the basis, the input
+    vector, the oracle's y = H v and the oracle's Lanczos coefficients are computed once (they do not depend on the
+    index mode or the kernel), then every variant {"mode", "options", "steps"} is run through the C ABI and compared."""
+    w = workload(spec)
+    n_up = spec.get("n_up", w.sectors[0])
+    prec = spec.get("prec", "fp32")
+    tol = 1e-5 if prec == "fp32" else 1e-12
+    torch.cuda.set_device(0)
+    basis = co.enumerate_basis(w.N, n_up)
+    D = basis.shape[0]
+    rng = np.random.default_rng(spec.get("seed", 1))
+    v = rng.standard_normal(D).astype(NDT[prec])
+    ref = co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, v.astype(np.float64), 0, D)
+    ref_norm = float(np.linalg.norm(ref))
+    bound = elem_bound(v, w.J, 0.0, w.N, prec)
+    max_steps = max([int(x.get("steps", 0)) for x in spec["variants"]] + [0])
+    a_ref = b_ref = None
+    if max_steps:
+        q1 = fo.start_vector(W.SEED_VECTORS, n_up, 0, D)
+        a_ref, b_ref = co.lanczos(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, q1, max_steps)[:2]
+        a_ref, b_ref = np.asarray(a_ref), np.asarray(b_ref)
+    dv = torch.from_numpy(v).cuda()
+    res = {"ok": True, "dim": D, "variants": []}
+    for var in spec["variants"]:
+        ctx = ftlm.ftlm_create(w.N, w.bond_i, w.bond_j, w.J, n_up, MODES[var["mode"]], PRECS[prec], 0.0)
+        for k, val in var.get("options", ()):
+            ftlm.ftlm_set_option(ctx, k, val)
+        r = {"mode": var["mode"], "options": var.get("options", []), "kernel": ftlm.ftlm_get_option(ctx, "kernel"),
+             "windows": ftlm.ftlm_get_option(ctx, "passb_windows"),
+             "tmlr": [ftlm.ftlm_get_option(ctx, "tmlr"), ftlm.ftlm_get_option(ctx, "tmlr_available")]}
+        dy = torch.full_like(dv, float("nan"))
+        ftlm.ftlm_apply_H(ctx, dv, dy)
+        torch.cuda.synchronize()
+        y = dy.cpu().numpy().astype(np.float64)
+        del dy
+        r["hv_relerr"] = float(np.linalg.norm(y - ref)) / ref_norm
+        r["hv_maxabs"], r["hv_elem_bound"] = float(np.max(np.abs(y - ref))), bound
+        ok = bool(np.isfinite(y).all()) and r["hv_relerr"] <= tol and r["hv_maxabs"] <= bound
+        m = int(var.get("steps", 0))
+        if m:
+            out = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, 1, m)
+            k = min(int(out["m_eff"][0]), m, 6)
+            ltol = 1e-9 if prec == "fp64" else 2e-4
+            r["lanczos_dalpha"] = float(np.max(np.abs(out["alpha"][0][:k] - a_ref[:k])))
+            r["lanczos_dbeta"] = float(np.max(np.abs(out["beta"][0][:k - 1] - b_ref[:k - 1]))) if k > 1 else 0.0
+            th_ref, _ = fo.ritz(a_ref[:m], b_ref[:m - 1])
+            th = out["theta"][0][:m]
+            rtol = (1e-9 if prec == "fp64" else 5e-4) * max(1.0, float(np.abs(th_ref).max()))
+            r["ritz_dmin"], r["ritz_dmax"] = float(abs(th.min() - th_ref.min())), float(abs(th.max() - th_ref.max()))
+            r["wsum"] = float(out["weight"][0][:m].sum())
+            ok = (ok and int(out["m_eff"][0]) == m and r["lanczos_dalpha"] <= ltol and r["lanczos_dbeta"] <= ltol
+                  and r["ritz_dmin"] <= rtol and r["ritz_dmax"] <= rtol and abs(r["wsum"] - 1.0) <= 1e-6)
+        ftlm.ftlm_destroy(ctx)
+        r["ok"] = bool(ok)
+        res["variants"].append(r)
+        res["ok"] = res["ok"] and bool(ok)
+    chk = ftlm.ftlm_check_info()
+    res["check"] = chk
+    if ftlm.CHECKED:
+        res["ok"] = res["ok"] and chk["check_build"] == 1 and chk["check_violations"] == 0
+    res["ok"] = bool(res["ok"])
+    print(json.dumps(res))
+
+
 def main():
     spec = json.loads(sys.argv[1])
+    if "variants" in spec:
+        run_variants(spec)
+        return
     w = workload(spec)
     n_up = spec.get("n_up", w.sectors[0])
     mode, prec = spec.get("mode", "cr"), spec.get("prec", "fp32")

@@ -247,10 +247,14 @@ def test_emu_result_does_not_depend_on_thread_schedule(order):
 
 
 @pytest.mark.parametrize("spec", [
-    {"wl": "ring12j", "n_up": 6, "mode": "cr", "prec": "fp64", "options": [["kernel", 1]], "batch": [5, 4]},
+    {"wl": "ring12j", "n_up": 6, "mode": "cr", "prec": "fp64", "options": [["kernel", 1]], "batch": [5, 4], "steps": 6},
     {"wl": "ring16", "n_up": 15, "mode": "clt", "prec": "fp32", "options": [["kernel", 1]], "batch": [4, 4], "steps": 16},   # D = 16: breakdown at step 9
-    {"wl": "ring16j", "n_up": 8, "mode": "clt", "prec": "fp32", "options": [["tml_split", 6 | (4 << 8)], ["kernel", 3]], "batch": [6, 4]},
-    {"wl": "rand14_30_3", "n_up": 7, "mode": "cr", "prec": "fp64", "options": [["tml_split", 5 | (5 << 8)], ["kernel", 3]], "batch": [3, 2]},
+    {"wl": "ring14j", "n_up": 7, "mode": "clt", "prec": "fp32", "options": [["tml_split", 5 | (4 << 8)], ["kernel", 3]], "batch": [5, 4], "steps": 5},
+    # multi-pass step: TML in-tile pass + PASS-B windows on rows of B interleaved chains (remainder groups run B = 1
+    # on the same window geometry: option "plan_batch")
+    {"wl": "ring14j", "n_up": 7, "mode": "cr", "prec": "fp32", "options": [["passb", 1], ["passb_lo_min", 4], ["tml_split", 5 | (3 << 8)], ["kernel", 3]], "batch": [5, 4], "steps": 5},
+    {"wl": "rand13_30_5", "n_up": 6, "mode": "cr", "prec": "fp64",
+     "options": [["passb", 1], ["passb_lo_min", 3], ["passb_smax", 6], ["tml_split", 5 | (2 << 8)], ["kernel", 3]], "batch": [3, 2], "steps": 4},
 ])
 def test_emu_batched_chains_are_bit_identical_to_single_chains(spec):
     """SURVEY 8(f)-1, PAPER.md L207 / L309: R chains advanced in groups of B on interleaved vectors through
@@ -263,9 +267,8 @@ def test_emu_batched_chains_are_bit_identical_to_single_chains(spec):
 
 
 @pytest.mark.parametrize("n_up,mode,prec,opts", [
-    (4, "clt", "fp32", [["kernel", 1]]),
-    (5, "cr", "fp32", [["tml_split", 6 | (5 << 8)], ["kernel", 3]]),
-    (6, "clt", "fp64", [["tml_split", 7 | (6 << 8)], ["passb", 1], ["passb_lo_min", 6], ["kernel", 3]]),
+    (3, "clt", "fp32", [["kernel", 1]]),
+    (5, "cr", "fp64", [["tml_split", 7 | (6 << 8)], ["passb", 1], ["passb_lo_min", 6], ["kernel", 3]]),
 ])
 def test_emu_dodecahedron(n_up, mode, prec, opts):
     """SURVEY 8(f)-2 (Fig. 3 e-f): sectors of the N = 20 dodecahedron through the ROW kernel, the TML

@@ -1,5 +1,5 @@
 """-m gpu parity of the batched Lanczos chains (Table 3 footnote L325: B = 4 on the
-paper's GPU): ftlm_lanczos with option "batch" = 2, 4 against the same chains run one at a time (bit-identical: the
+paper's GPU): ftlm_lanczos with option "batch" = 2, 4 against the same chains run one at a time on the same tiles and windows (bit-identical: the
 per-chain arithmetic and the reduction order do not depend on B) and against the FP64 oracle."""
 import numpy as np
 import pytest
@@ -21,6 +21,11 @@ from gpu_util import Ctx                       # noqa: E402
     ("square4x5", 10, "cr", "fp64", [["tml_split", 7 | (5 << 8)], ["kernel", 3]], 3, 2, 10),
     ("square4x6", 12, "clt", "fp32", [["kernel", 3]], 4, 4, 8),                 # BASELINE config 2's largest sector, auto split
     ("square4x6", 12, "cr", "fp32", [["kernel", 3]], 2, 2, 8),
+    # multi-pass step on rows of B chains: TML in-tile pass + PASS-B windows
+    ("ring16j", 8, "clt", "fp32", [["passb", 1], ["tml_split", 5 | (3 << 8)], ["kernel", 3]], 5, 4, 12),
+    ("rand15_40_5", 7, "cr", "fp64", [["passb", 1], ["passb_lo_min", 3], ["passb_smax", 6], ["tml_split", 5 | (2 << 8)], ["kernel", 3]], 3, 2, 10),
+    ("ring20j", 10, "clt", "fp32", [["passb", 1], ["passb_lo_min", 4], ["passb_smax", 7], ["tml_split", 5 | (1 << 8)], ["kernel", 3]], 4, 4, 6),
+    ("square4x6", 12, "clt", "fp32", [["passb", 1], ["kernel", 3]], 4, 4, 8),
 ])
 def test_batched_chains_match_single_chains_and_oracle(wl, n_up, mode, prec, opts, R, B, steps):
     from gpu_case import workload
@@ -34,6 +39,7 @@ def test_batched_chains_match_single_chains_and_oracle(wl, n_up, mode, prec, opt
         split = (ftlm.ftlm_get_option(c.ctx, "tml_w"), ftlm.ftlm_get_option(c.ctx, "tml_m"))
         if split[0] > 0:
             ftlm.ftlm_set_option(c.ctx, "tml_split", split[0] | (split[1] << 8))
+        ftlm.ftlm_set_option(c.ctx, "plan_batch", B)      # the single chains run on the batch's tiles and windows
         ftlm.ftlm_set_option(c.ctx, "batch", 1)
         assert (ftlm.ftlm_get_option(c.ctx, "tml_w"), ftlm.ftlm_get_option(c.ctx, "tml_m")) == split
         one = ftlm.ftlm_lanczos(c.ctx, W.SEED_VECTORS, R, steps)
@@ -50,15 +56,3 @@ def test_batched_chains_match_single_chains_and_oracle(wl, n_up, mode, prec, opt
         assert abs(many["weight"][r][: int(many["m_eff"][r])].sum() - 1.0) <= 1e-6
     if wl == "ring16":
         assert many["m_eff"].max() < 16
-
-
-def test_batch_refuses_window_passes():
-    w = W.baseline_config(2)
-    with Ctx(w, 12, "cr", "fp32") as c:
-        ftlm.ftlm_set_option(c.ctx, "kernel", 3)
-        ftlm.ftlm_set_option(c.ctx, "passb", 1)
-        ftlm.ftlm_set_option(c.ctx, "batch", 2)
-        if ftlm.ftlm_get_option(c.ctx, "passb_windows") > 0:
-            with pytest.raises(ftlm.FtlmError) as e:
-                ftlm.ftlm_lanczos(c.ctx, W.SEED_VECTORS, 2, 3)
-            assert e.value.code == ftlm.EUNSUPPORTED
