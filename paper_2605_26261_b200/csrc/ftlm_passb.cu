@@ -117,13 +117,15 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const Vec<
   }
   for (int sl0 = warp; sl0 < nconf; sl0 += NW * PF) {
     V yold[PF][PASSB_XK];
+    uint64_t rstart[PF];                               // run start of each word: read once from shared memory
 #pragma unroll
     for (int j = 0; j < PF; ++j) {
       const int sl = sl0 + j * NW;
+      rstart[j] = sl < nconf ? LD_S(&s_start[sl]) : 0ull;
 #pragma unroll
       for (int k = 0; k < PASSB_XK; ++k) {
         const int x = lane + 32 * k;
-        if (sl < nconf && k < XKC && x < nx) yold[j][k] = vec_ldcs(y + LD_S(&s_start[sl]) + x0 + x);
+        if (sl < nconf && k < XKC && x < nx) yold[j][k] = vec_ldcs(y + rstart[j] + x0 + x);
         else yold[j][k] = V{};
       }
     }
@@ -142,7 +144,7 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const Vec<
       const R sumJ = __shfl_sync(0xffffffffu, eJ, 31);
       // lanes past the end of the run (x >= nx) read stale tile words and are discarded at the store
       const unsigned char* tl = (const unsigned char*)tile + (size_t)lane * sizeof(V);
-      V* yrow = y + LD_S(&s_start[sl]) + x0;
+      V* yrow = y + rstart[j] + x0;
       V own[PASSB_XK], acc[PASSB_XK];
       own[0] = LD_S((const V*)(tl + (size_t)sl * X * sizeof(V)));
       acc[0] = V{};
@@ -212,8 +214,10 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const Vec<
   }
 }
 
+// rows wider than 4 bytes (FP64, batches) run with 512 threads per CTA: 128 registers per thread instead of 64
+// (ptxas: the y prefetch of 8 / B window words x 2 offsets spills at 64)
 template <typename R, int B, int MODE, bool FUSED>
-__global__ void __launch_bounds__(PASSB_THREADS, 1)
+__global__ void __launch_bounds__((sizeof(R) * B > 4) ? 512 : PASSB_THREADS, 1)
 passb_kernel(const __grid_constant__ PassBParams<R> p, const R* __restrict__ v_, R* __restrict__ y_) {
   typedef Vec<R, B> V;
   FTLM_DYN_SMEM(smem);
@@ -416,7 +420,7 @@ static bool passb_geometry(const ftlm_ctx* c, PassBWindow& w, std::vector<uint32
       w.xk[p] = xk;
       max_rows = std::max(max_rows, (int)binom_b(w.s, p) * 32 * xk);
     }
-    if (fits) { w.ctas = ctas; w.threads = ctas >= 2 ? 512 : PASSB_THREADS; }
+    if (fits) { w.ctas = ctas; w.threads = (ctas >= 2 || ftlm_elem_size(c) > 4) ? 512 : PASSB_THREADS; }
   }
   if (!fits) return false;
   w.smem = passb_smem_bytes(N, K, w.max_conf, max_rows, esz);
@@ -606,14 +610,15 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   }
   int grid = c->sm_count * w.ctas;
   if ((uint32_t)grid > p.item_end - p.item_begin) grid = (int)std::max(1u, p.item_end - p.item_begin);
+  const int threads = (sizeof(R) * B > 4) ? 512 : w.threads;     // the kernel's launch bound
   if (fused) {
     auto k = passb_kernel<R, B, MODE, true>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
-    FTLM_LAUNCH(k, grid, w.threads, w.smem, s, p, (const R*)v, (R*)y);
+    FTLM_LAUNCH(k, grid, threads, w.smem, s, p, (const R*)v, (R*)y);
   } else {
     auto k = passb_kernel<R, B, MODE, false>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));
-    FTLM_LAUNCH(k, grid, w.threads, w.smem, s, p, (const R*)v, (R*)y);
+    FTLM_LAUNCH(k, grid, threads, w.smem, s, p, (const R*)v, (R*)y);
   }
   CK(cudaGetLastError());
   return FTLM_OK;

@@ -79,6 +79,11 @@ struct TmlrPlan {
 
 namespace {
 
+// antiparallel MM bond of a column: row offset of the target column and J/2, read with one (broadcast) load
+template <typename R> struct MmEnt;
+template <> struct __align__(8) MmEnt<float> { uint32_t off; float J; };
+template <> struct __align__(16) MmEnt<double> { uint32_t off, pad; double J; };
+
 // per-column descriptor arrays in shared memory (rebuilt for every tile: they depend on kT)
 template <typename R>
 struct TmlrSmem {
@@ -86,8 +91,7 @@ struct TmlrSmem {
   unsigned char* blob;
   R* vs;                // tile
   R* dcoef;             // [nM] diagonal coefficient of column M
-  R* dmmJ;              // [nM][n_mm] J/2 of the antiparallel MM bonds (compacted)
-  uint32_t* dmm;        // [nM][n_mm] row offset of their target columns
+  MmEnt<R>* dmm;        // [nM][n_mm] antiparallel MM bonds (compacted): row offset of the target column, J/2
   uint32_t* dml;        // [nM][n_ml] byte offset of the target column | M_j (bit 0)
   int* dnmm;            // [nM]
   uint32_t* dg;         // [nM][n_g] global row (target tile base + target column offset) of the active left-over bonds
@@ -106,8 +110,7 @@ __host__ __device__ inline size_t tmlr_layout(TmlrSmem<R>& s, unsigned char* p0,
   s.blob = take((size_t)blob_bytes);
   s.vs = (R*)take((size_t)max_tile * sizeof(R) + 16);    // + 16: the tile keeps the global address's residue mod 16 bytes
   s.dcoef = (R*)take((size_t)nM * sizeof(R));
-  s.dmmJ = (R*)take((size_t)nM * (n_mm ? n_mm : 1) * sizeof(R));
-  s.dmm = (uint32_t*)take((size_t)nM * (n_mm ? n_mm : 1) * 4);
+  s.dmm = (MmEnt<R>*)take((size_t)nM * (n_mm ? n_mm : 1) * sizeof(MmEnt<R>));
   s.dml = (uint32_t*)take((size_t)nM * (n_ml ? n_ml : 1) * 4);
   s.dnmm = (int*)take((size_t)nM * 4);
   s.dg = (uint32_t*)take((size_t)nM * (n_g ? n_g : 1) * 4);
@@ -222,8 +225,9 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
       for (int e = 0; e < n_mm; ++e) {
         const uint32_t mk = p.mm_mask[e];
         if (__popc((uint32_t)M & mk) == 1) {
-          ST_S(&S.dmm[M * n_mm + n], (uint32_t)LD_S(&co[(uint32_t)M ^ mk]));
-          ST_S(&S.dmmJ[M * n_mm + n], p.mm_J[e]);
+          MmEnt<R> me{};
+          me.off = (uint32_t)LD_S(&co[(uint32_t)M ^ mk]); me.J = p.mm_J[e];
+          ST_S(&S.dmm[M * n_mm + n], me);
           coef -= p.mm_J[e];
           ++n;
         }
@@ -305,24 +309,36 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         // four independent partial sums (LL even/odd, ML even/odd) keep the FMA dependency chains short
         R acc = LD_S(&S.dcoef[M]) * own;
         R l0 = (R)0, l1 = (R)0, m0 = (R)0, m1 = (R)0;
+        const uint32_t ownoff = (uint32_t)lrc * (uint32_t)sizeof(R);
 #pragma unroll
         for (int e = 0; e < NLL; e += 2) {
-          const R a0 = LD_S((const R*)(colb + llo[e])), a1 = LD_S((const R*)(colb + llo[e + 1]));
+          // a parallel bond's table entry is the row itself: only the antiparallel lanes read (fewer lanes per
+          // shared-memory wavefront = fewer bank conflicts; emulated profile in profiles/r02_emu_smem_profile.md)
+          R a0 = own, a1 = own;
+          if (llo[e] != ownoff) a0 = LD_S((const R*)(colb + llo[e]));
+          if (llo[e + 1] != ownoff) a1 = LD_S((const R*)(colb + llo[e + 1]));
           if (UNIJ) { l0 += a0; l1 += a1; } else { l0 += p.ll_J[e] * a0; l1 += p.ll_J[e + 1] * a1; }
         }
         const int nmm = LD_S(&S.dnmm[M]);
-        for (int a = 0; a < nmm; ++a) acc += LD_S(&S.dmmJ[M * n_mm + a]) * LD_S(&vs0[LD_S(&S.dmm[M * n_mm + a]) + (uint32_t)lrc]);
+        for (int a = 0; a < nmm; ++a) {
+          const MmEnt<R> me = LD_S(&S.dmm[M * n_mm + a]);                  // one broadcast read: offset and J
+          acc += me.J * LD_S(&vs0[me.off + (uint32_t)lrc]);
+        }
         if (p.n_g) {
           const int ng = LD_S(&S.dng[M]);
           for (int a = 0; a < ng; ++a) acc += LD_S(&S.dgJ[M * p.n_g + a]) * LDG(v + ((size_t)LD_S(&S.dg[M * p.n_g + a]) + (uint32_t)lrc));
         }
 #pragma unroll
-        for (int e = 0; e < NML; e += 2) {
-          const uint32_t d0 = LD_S(&S.dml[M * n_ml + e]), f0 = flo[e], d1 = LD_S(&S.dml[M * n_ml + e + 1]), f1 = flo[e + 1];
-          R a0 = own, a1 = own;
+        for (int e = 0; e < NML; e += 4) {                 // four column descriptors per 16-byte broadcast read
+          const uint4 d4 = LD_S((const uint4*)&S.dml[M * n_ml + e]);
+          const uint32_t d0 = d4.x, d1 = d4.y, d2 = d4.z, d3 = d4.w, f0 = flo[e], f1 = flo[e + 1], f2 = flo[e + 2], f3 = flo[e + 3];
+          R a0 = own, a1 = own, a2 = own, a3 = own;
           if ((d0 ^ f0) & 1u) a0 = LD_S((const R*)(vsm1 + d0 + f0));   // active: exactly one of the two low bits is set
           if ((d1 ^ f1) & 1u) a1 = LD_S((const R*)(vsm1 + d1 + f1));
-          if (UNIJ) { m0 += a0; m1 += a1; } else { m0 += p.ml_J[e] * a0; m1 += p.ml_J[e + 1] * a1; }
+          if ((d2 ^ f2) & 1u) a2 = LD_S((const R*)(vsm1 + d2 + f2));
+          if ((d3 ^ f3) & 1u) a3 = LD_S((const R*)(vsm1 + d3 + f3));
+          if (UNIJ) { m0 += a0; m1 += a1; m0 += a2; m1 += a3; }
+          else { m0 += p.ml_J[e] * a0; m1 += p.ml_J[e + 1] * a1; m0 += p.ml_J[e + 2] * a2; m1 += p.ml_J[e + 3] * a3; }
         }
         if (UNIJ) acc += p.ll_J[0] * (l0 + l1) + p.ml_J[0] * (m0 + m1);
         else acc += (l0 + l1) + (m0 + m1);

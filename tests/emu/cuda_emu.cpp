@@ -7,6 +7,7 @@
 #include <ucontext.h>
 #include <unistd.h>
 
+#include <algorithm>
 #include <atomic>
 #include <map>
 #include <mutex>
@@ -61,6 +62,17 @@ struct PendingBulk { void* dst; std::vector<unsigned char> data; void* mbar; };
 struct MBar { int count = 0, pending = 0; long tx = 0; unsigned completed = 0; };
 thread_local std::vector<PendingBulk> g_bulk;           // bulk copies in flight of the CTA on this host thread
 thread_local std::map<void*, MBar> g_mbar;
+// Shared-memory profile (FTLM_EMU_PROFILE=<file>): every LD_S / ST_S / cp.async access is logged per CTA with its
+// warp, lane, source line and the per-thread occurrence number of that line; at the end of the CTA the lanes of one
+// warp instruction are put together and its shared-memory wavefronts are counted as on the hardware: 4-byte words
+// of one instruction that fall into the same bank (word mod 32) but differ need one wavefront each.
+struct ProfEv { uint32_t warp_lane; uint32_t tuline; uint32_t occ; uint32_t word; uint8_t nwords, write; };
+struct ProfAgg { unsigned long long instr = 0, wavefronts = 0, ideal = 0, lanes = 0; };
+thread_local std::vector<ProfEv> g_prof_ev;
+thread_local std::vector<std::map<uint32_t, uint32_t>> g_prof_occ;      // per thread: occurrences of each source line
+std::map<uint32_t, ProfAgg> g_prof;                                      // (tu << 20 | line) << 1 | write
+std::mutex g_prof_mu;
+const char* prof_path() { static const char* p = getenv("FTLM_EMU_PROFILE"); return (p && *p) ? p : nullptr; }
 const size_t STACK = 64 * 1024;
 // scheduler state of the CTA in flight on this host thread
 thread_local std::vector<Fiber> g_fib;
@@ -123,6 +135,58 @@ void complete_collective(Warp& w) {
   w.op = -1;
   w.gen++;
   g_progress++;
+}
+
+// one warp instruction = the events of one warp with the same source line and occurrence number
+void prof_reduce() {
+  std::sort(g_prof_ev.begin(), g_prof_ev.end(), [](const ProfEv& a, const ProfEv& b) {
+    const uint32_t wa = a.warp_lane >> 5, wb = b.warp_lane >> 5;
+    if (wa != wb) return wa < wb;
+    if (a.tuline != b.tuline) return a.tuline < b.tuline;
+    if (a.write != b.write) return a.write < b.write;
+    return a.occ < b.occ;
+  });
+  std::map<uint32_t, ProfAgg> local;
+  std::vector<uint32_t> words;
+  for (size_t i = 0; i < g_prof_ev.size();) {
+    size_t j = i;
+    words.clear();
+    unsigned long long bytes = 0;
+    while (j < g_prof_ev.size() && (g_prof_ev[j].warp_lane >> 5) == (g_prof_ev[i].warp_lane >> 5) && g_prof_ev[j].tuline == g_prof_ev[i].tuline &&
+           g_prof_ev[j].write == g_prof_ev[i].write && g_prof_ev[j].occ == g_prof_ev[i].occ) {
+      for (unsigned k = 0; k < g_prof_ev[j].nwords; ++k) words.push_back(g_prof_ev[j].word + k);
+      bytes += 4ull * g_prof_ev[j].nwords;
+      ++j;
+    }
+    std::sort(words.begin(), words.end());
+    words.erase(std::unique(words.begin(), words.end()), words.end());
+    unsigned per_bank[32] = {0}, wf = 0;
+    for (uint32_t w : words) wf = std::max(wf, ++per_bank[w & 31u]);
+    ProfAgg& a = local[(g_prof_ev[i].tuline << 1) | g_prof_ev[i].write];
+    a.instr++; a.wavefronts += wf; a.ideal += (bytes + 127) / 128; a.lanes += (unsigned long long)(j - i);
+    i = j;
+  }
+  g_prof_ev.clear();
+  for (auto& m : g_prof_occ) m.clear();
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  for (auto& kv : local) { ProfAgg& g = g_prof[kv.first]; g.instr += kv.second.instr; g.wavefronts += kv.second.wavefronts; g.ideal += kv.second.ideal; g.lanes += kv.second.lanes; }
+}
+
+void prof_dump() {
+  const char* path = prof_path();
+  if (!path) return;
+  FILE* f = fopen(path, "w");
+  if (!f) return;
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  fprintf(f, "[");
+  bool first = true;
+  for (auto& kv : g_prof) {
+    fprintf(f, "%s{\"tu\": %u, \"line\": %u, \"write\": %u, \"warp_instr\": %llu, \"wavefronts\": %llu, \"ideal\": %llu, \"lanes\": %llu}", first ? "" : ",\n ",
+            (kv.first >> 1) >> 20, (kv.first >> 1) & 0xFFFFFu, kv.first & 1u, kv.second.instr, kv.second.wavefronts, kv.second.ideal, kv.second.lanes);
+    first = false;
+  }
+  fprintf(f, "]\n");
+  fclose(f);
 }
 
 void fiber_entry() {
@@ -190,6 +254,7 @@ void run_block() {
     if (g_progress == before) die("deadlock: no thread of the CTA can make progress (mismatched barrier / collective)");
   }
   g_cur = -1;
+  if (prof_path()) prof_reduce();
 }
 
 cudaError_t g_last = cudaSuccess;
@@ -277,6 +342,12 @@ bool smem_access(const void* p, size_t bytes, bool write, int tu, int line) {
   if (g_cur < 0 || g_shadow.empty()) return true;
   const unsigned char* a = (const unsigned char*)p;
   if (a < g_dyn || a >= g_dyn + g_dyn_bytes) return true;            // static __shared__ variables, global memory
+  if (prof_path() && (tu || line)) {
+    const uint32_t key = ((uint32_t)tu << 20) | (uint32_t)line;
+    if (g_prof_occ.size() < g_nthreads) g_prof_occ.resize(g_nthreads);
+    const uint32_t occ = g_prof_occ[(size_t)g_cur][key]++;
+    g_prof_ev.push_back(ProfEv{(uint32_t)g_cur, key, occ, (uint32_t)((a - g_dyn) / 4), (uint8_t)((bytes + 3) / 4), (uint8_t)write});
+  }
   const int t = g_cur;
   const unsigned bar = g_bar_gen, wgen = g_warps[(size_t)t >> 5].sync_gen;
   auto ordered = [&](const Access& x) {
@@ -331,6 +402,8 @@ uint64_t collective(int op, unsigned mask, uint64_t v, int arg) {
 
 void launch(unsigned grid, unsigned block, size_t dyn_bytes, const std::function<void()>& body) {
   if (g_cur >= 0) die("nested launch");
+  static const bool prof_registered = (prof_path() ? atexit(prof_dump) : 0, true);
+  (void)prof_registered;
   if (grid == 0 || block == 0 || block > 1024) { g_last = cudaErrorInvalidValue; return; }
   if (dyn_bytes > 227 * 1024) { g_last = cudaErrorInvalidValue; return; }
   // CTAs are taken from a shared counter by a few host threads and run concurrently (one CTA in flight per host
