@@ -122,6 +122,17 @@ template <typename T> __device__ __forceinline__ T ldcs(const T* p, int line) { 
 template <typename T, typename U> __device__ __forceinline__ void st_g(T* p, const U& v, int line) { if (FTLM_G_OK(p, T, line)) *p = (T)v; }
 template <typename T, typename U> __device__ __forceinline__ void stcs(T* p, const U& v, int line) { if (FTLM_G_OK(p, T, line)) __stcs(p, (T)v); }
 template <typename T> __device__ __forceinline__ T ld_s(const T* p, int line) { if (!FTLM_S_OK(p, T, line)) return T{}; return *p; }
+// predicated shared-memory load: `other` for lanes whose condition is false.  (In the emulation every lane passes
+// here, which keeps the per-thread occurrence numbers of the shared-memory profile aligned across the lanes of a warp.)
+template <typename T> __device__ __forceinline__ T ld_s_if(bool c, const T* p, const T& other, int line) {
+#ifdef FTLM_EMU
+  if (!c) { cuda_emu::smem_skip(FTLM_TU, line); return other; }
+#else
+  if (!c) return other;
+#endif
+  if (!FTLM_S_OK(p, T, line)) return T{};
+  return *p;
+}
 template <typename T, typename U> __device__ __forceinline__ void st_s(T* p, const U& v, int line) { if (FTLM_SW_OK(p, T, line)) *p = (T)v; }
 template <typename T> __device__ __forceinline__ T ld_a(const T* p, int line) { if (!FTLM_A_OK(p, T, line)) return T{}; return *p; }
 template <typename T> __device__ __forceinline__ T atom_add_g(T* p, T v, int line) { if (!FTLM_G_OK(p, T, line)) return T{}; return atomicAdd(p, v); }
@@ -133,6 +144,7 @@ template <typename T> __device__ __forceinline__ T atom_add_g(T* p, T v, int lin
 #define ST_G(p, ...) fa::st_g((p), (__VA_ARGS__), __LINE__)  /* plain global store */
 #define STCS(p, ...) fa::stcs((p), (__VA_ARGS__), __LINE__)  /* streaming global store */
 #define LD_S(p) fa::ld_s((p), __LINE__)          /* shared-memory load */
+#define LD_S_IF(c, p, other) fa::ld_s_if((c), (p), (other), __LINE__)   /* predicated shared-memory load */
 #define ST_S(p, ...) fa::st_s((p), (__VA_ARGS__), __LINE__)  /* shared-memory store */
 #define LD_A(p) fa::ld_a((p), __LINE__)          /* load through a pointer that is shared in some callers, global in others */
 #define ATOM_ADD_G(p, ...) fa::atom_add_g((p), (__VA_ARGS__), __LINE__)

@@ -479,11 +479,10 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
           load_fent(FSl + e + 2, o2, j2, f2, u2); load_fent(FSl + e + 3, o3, j3, f3, u3);
           const uint32_t x0 = LD_S((const uint16_t*)(flp + f0)), x1 = LD_S((const uint16_t*)(flp + f1));
           const uint32_t x2 = LD_S((const uint16_t*)(flp + f2)), x3 = LD_S((const uint16_t*)(flp + f3));
-          V a0 = own, a1 = own, a2 = own, a3 = own;
-          if ((x0 ^ u0) & 0x8000u) a0 = LD_S((const V*)(vsb0 + (size_t)(o0 + x0) * RB));
-          if ((x1 ^ u1) & 0x8000u) a1 = LD_S((const V*)(vsb0 + (size_t)(o1 + x1) * RB));
-          if ((x2 ^ u2) & 0x8000u) a2 = LD_S((const V*)(vsb0 + (size_t)(o2 + x2) * RB));
-          if ((x3 ^ u3) & 0x8000u) a3 = LD_S((const V*)(vsb0 + (size_t)(o3 + x3) * RB));
+          const V a0 = LD_S_IF((x0 ^ u0) & 0x8000u, (const V*)(vsb0 + (size_t)(o0 + x0) * RB), own);
+          const V a1 = LD_S_IF((x1 ^ u1) & 0x8000u, (const V*)(vsb0 + (size_t)(o1 + x1) * RB), own);
+          const V a2 = LD_S_IF((x2 ^ u2) & 0x8000u, (const V*)(vsb0 + (size_t)(o2 + x2) * RB), own);
+          const V a3 = LD_S_IF((x3 ^ u3) & 0x8000u, (const V*)(vsb0 + (size_t)(o3 + x3) * RB), own);
 #pragma unroll
           for (int b = 0; b < B; ++b)
             acc.x[b] += j0 * (a0.x[b] - own.x[b]) + j1 * (a1.x[b] - own.x[b]) + j2 * (a2.x[b] - own.x[b]) + j3 * (a3.x[b] - own.x[b]);

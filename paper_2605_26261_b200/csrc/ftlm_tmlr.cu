@@ -314,9 +314,8 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         for (int e = 0; e < NLL; e += 2) {
           // a parallel bond's table entry is the row itself: only the antiparallel lanes read (fewer lanes per
           // shared-memory wavefront = fewer bank conflicts; emulated profile in profiles/r02_emu_smem_profile.md)
-          R a0 = own, a1 = own;
-          if (llo[e] != ownoff) a0 = LD_S((const R*)(colb + llo[e]));
-          if (llo[e + 1] != ownoff) a1 = LD_S((const R*)(colb + llo[e + 1]));
+          const R a0 = LD_S_IF(llo[e] != ownoff, (const R*)(colb + llo[e]), own);
+          const R a1 = LD_S_IF(llo[e + 1] != ownoff, (const R*)(colb + llo[e + 1]), own);
           if (UNIJ) { l0 += a0; l1 += a1; } else { l0 += p.ll_J[e] * a0; l1 += p.ll_J[e + 1] * a1; }
         }
         const int nmm = LD_S(&S.dnmm[M]);
@@ -332,11 +331,10 @@ hv_tmlr_kernel(const __grid_constant__ TmlrParams<R> p, const R* __restrict__ v,
         for (int e = 0; e < NML; e += 4) {                 // four column descriptors per 16-byte broadcast read
           const uint4 d4 = LD_S((const uint4*)&S.dml[M * n_ml + e]);
           const uint32_t d0 = d4.x, d1 = d4.y, d2 = d4.z, d3 = d4.w, f0 = flo[e], f1 = flo[e + 1], f2 = flo[e + 2], f3 = flo[e + 3];
-          R a0 = own, a1 = own, a2 = own, a3 = own;
-          if ((d0 ^ f0) & 1u) a0 = LD_S((const R*)(vsm1 + d0 + f0));   // active: exactly one of the two low bits is set
-          if ((d1 ^ f1) & 1u) a1 = LD_S((const R*)(vsm1 + d1 + f1));
-          if ((d2 ^ f2) & 1u) a2 = LD_S((const R*)(vsm1 + d2 + f2));
-          if ((d3 ^ f3) & 1u) a3 = LD_S((const R*)(vsm1 + d3 + f3));
+          const R a0 = LD_S_IF((d0 ^ f0) & 1u, (const R*)(vsm1 + d0 + f0), own);   // active: exactly one of the two low bits is set
+          const R a1 = LD_S_IF((d1 ^ f1) & 1u, (const R*)(vsm1 + d1 + f1), own);
+          const R a2 = LD_S_IF((d2 ^ f2) & 1u, (const R*)(vsm1 + d2 + f2), own);
+          const R a3 = LD_S_IF((d3 ^ f3) & 1u, (const R*)(vsm1 + d3 + f3), own);
           if (UNIJ) { m0 += a0; m1 += a1; m0 += a2; m1 += a3; }
           else { m0 += p.ml_J[e] * a0; m1 += p.ml_J[e + 1] * a1; m0 += p.ml_J[e + 2] * a2; m1 += p.ml_J[e + 3] * a3; }
         }

@@ -338,6 +338,12 @@ void mbar_wait(void* mbar, unsigned parity) {
   }
 }
 
+void smem_skip(int tu, int line) {
+  if (g_cur < 0 || !prof_path()) return;
+  if (g_prof_occ.size() < g_nthreads) g_prof_occ.resize(g_nthreads);
+  g_prof_occ[(size_t)g_cur][((uint32_t)tu << 20) | (uint32_t)line]++;
+}
+
 bool smem_access(const void* p, size_t bytes, bool write, int tu, int line) {
   if (g_cur < 0 || g_shadow.empty()) return true;
   const unsigned char* a = (const unsigned char*)p;

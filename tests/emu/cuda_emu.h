@@ -112,6 +112,8 @@ void bulk_issue(void* smem_dst, const void* gsrc, unsigned bytes, void* mbar, in
 void mbar_wait(void* mbar, unsigned parity);
 // race detector hook (always returns true); a pointer outside the CTA's dynamic shared memory is ignored
 bool smem_access(const void* p, size_t bytes, bool write, int tu, int line);
+// profile only: an inactive lane of a predicated shared-memory load passes the instruction (occurrence numbering)
+void smem_skip(int tu, int line);
 enum { OP_SYNCWARP = 0, OP_BALLOT = 1, OP_SHFL_DOWN = 2, OP_SHFL_XOR = 3, OP_SHFL_IDX = 4, OP_SHFL_UP = 5 };
 template <typename T> static inline uint64_t pack(T v) { uint64_t u = 0; static_assert(sizeof(T) <= 8, "shfl payload"); memcpy(&u, &v, sizeof(T)); return u; }
 template <typename T> static inline T unpack(uint64_t u) { T v; memcpy(&v, &u, sizeof(T)); return v; }
