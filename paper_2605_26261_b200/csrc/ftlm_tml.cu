@@ -455,10 +455,13 @@ hv_tml_kernel(const __grid_constant__ TmlParams<R> p, const R* __restrict__ v_, 
         // LL: swap form, 4 bonds per 8-byte table entry
         for (int g = 0; g < (p.n_ll4 >> 2); ++g) {
           const uint2 q = LD_S(&s_ll[g * nL + Lidx]);
-          const V a0 = LD_S((const V*)(vsb + (q.x & 0xffffu) * RB));
-          const V a1 = LD_S((const V*)(vsb + (q.x >> 16) * RB));
-          const V a2 = LD_S((const V*)(vsb + (q.y & 0xffffu) * RB));
-          const V a3 = LD_S((const V*)(vsb + (q.y >> 16) * RB));
+          // a parallel (or padding) bond's table entry is the row itself: only the antiparallel lanes read
+          // (fewer lanes per shared-memory wavefront, fewer bank conflicts: profiles/r02_emu_smem_profile.md)
+          const uint32_t t0 = q.x & 0xffffu, t1 = q.x >> 16, t2 = q.y & 0xffffu, t3 = q.y >> 16;
+          const V a0 = LD_S_IF(t0 != (uint32_t)lrc, (const V*)(vsb + t0 * RB), own);
+          const V a1 = LD_S_IF(t1 != (uint32_t)lrc, (const V*)(vsb + t1 * RB), own);
+          const V a2 = LD_S_IF(t2 != (uint32_t)lrc, (const V*)(vsb + t2 * RB), own);
+          const V a3 = LD_S_IF(t3 != (uint32_t)lrc, (const V*)(vsb + t3 * RB), own);
           const R j0 = p.ll_J[4 * g + 0], j1 = p.ll_J[4 * g + 1], j2 = p.ll_J[4 * g + 2], j3 = p.ll_J[4 * g + 3];
 #pragma unroll
           for (int b = 0; b < B; ++b) acc.x[b] += j0 * a0.x[b] + j1 * a1.x[b] + j2 * a2.x[b] + j3 * a3.x[b];
