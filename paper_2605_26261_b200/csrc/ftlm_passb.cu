@@ -22,7 +22,7 @@
 #include "ftlm_passb.cuh"
 #include "ftlm_vec.cuh"
 
-#define PASSB_MAX_BONDS 31          // one neighbour entry per lane; entry 31 holds the count and the sum of J
+#define PASSB_MAX_BONDS 28          // neighbour rows of 32 entries: up to 28 bonds (padded to multiples of 4), entry 31 holds the count and the sum of J
 #define PASSB_MAX_S 12
 #define PASSB_THREADS 1024
 #define PASSB_END 0xFFFFFFFFu
@@ -107,14 +107,6 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const Vec<
                                              double* s_qy, double* s_yy, double* s_qq) {
   typedef Vec<R, B> V;
   constexpr int PF = PASSB_PF / B;
-  // neighbour rows are stored in window-word order (row c0 + sl); the row of the next word is requested
-  // while the current word is processed
-  uint32_t eo_n = 0;
-  R eJ_n = (R)0;
-  if (warp < nconf) {
-    eo_n = LDG(&p.nbr_off[(size_t)(c0 + warp) * 32 + lane]);
-    eJ_n = LDG(&p.nbr_J[(size_t)(c0 + warp) * 32 + lane]);
-  }
   for (int sl0 = warp; sl0 < nconf; sl0 += NW * PF) {
     V yold[PF][PASSB_XK];
     uint64_t rstart[PF];                               // run start of each word: read once from shared memory
@@ -133,65 +125,46 @@ __device__ __forceinline__ void passb_phase2(const PassBParams<R>& p, const Vec<
     for (int j = 0; j < PF; ++j) {
       const int sl = sl0 + j * NW;
       if (sl >= nconf) break;
-      const uint32_t eo_rows = eo_n;
-      const R eJ = eJ_n;
-      if (sl + NW < nconf) {
-        eo_n = LDG(&p.nbr_off[(size_t)(c0 + sl + NW) * 32 + lane]);
-        eJ_n = LDG(&p.nbr_J[(size_t)(c0 + sl + NW) * 32 + lane]);
-      }
-      const int cnt = (int)__shfl_sync(0xffffffffu, eo_rows, 31);
-      const uint32_t eo = eo_rows * (uint32_t)sizeof(V);    // row index -> byte offset, once per word (entry 31 is not an offset)
-      const R sumJ = __shfl_sync(0xffffffffu, eJ, 31);
+      // the word's neighbour row: entries 0 .. cnt-1 (cnt a multiple of 4: padded with the word's own tile row and
+      // J = 0), entry 31 = cnt / sum of J.  Every lane reads the same addresses: 16-byte broadcast loads that stay in
+      // L1 (one load per four bonds instead of one shuffle per bond).
+      const uint32_t* nro = p.nbr_off + (size_t)(c0 + sl) * 32;
+      const R* nrJ = p.nbr_J + (size_t)(c0 + sl) * 32;
+      const int cnt = (int)LDG(&nro[31]);
+      const R sumJ = LDG(&nrJ[31]);
       // lanes past the end of the run (x >= nx) read stale tile words and are discarded at the store
       const unsigned char* tl = (const unsigned char*)tile + (size_t)lane * sizeof(V);
       V* yrow = y + rstart[j] + x0;
       V own[PASSB_XK], acc[PASSB_XK];
       own[0] = LD_S((const V*)(tl + (size_t)sl * X * sizeof(V)));
       acc[0] = V{};
-      if (XKC == 1) {
-        own[1] = V{}; acc[1] = V{};
-        if (UNIJ) {                                  // one J_b for the whole window: add, multiply once
-#pragma unroll 4
-          for (int e = 0; e < cnt; ++e) {
-            const V g = LD_S((const V*)(tl + __shfl_sync(0xffffffffu, eo, e)));
+      own[1] = V{}; acc[1] = V{};
+      if (XKC == 2) own[1] = LD_S((const V*)(tl + (size_t)sl * X * sizeof(V) + 32 * sizeof(V)));
+#pragma unroll 2
+      for (int e = 0; e < cnt; e += 4) {
+        const uint4 o4 = LDG((const uint4*)(nro + e));
+        const uint32_t oo[4] = {o4.x, o4.y, o4.z, o4.w};
+        R jj[4];
+        if (!UNIJ) {
+          if constexpr (sizeof(R) == 4) { const uint4 j4 = LDG((const uint4*)(nrJ + e)); jj[0] = __uint_as_float(j4.x); jj[1] = __uint_as_float(j4.y); jj[2] = __uint_as_float(j4.z); jj[3] = __uint_as_float(j4.w); }
+          else { const double2 ja = LDG((const double2*)(nrJ + e)), jb = LDG((const double2*)(nrJ + e + 2)); jj[0] = (R)ja.x; jj[1] = (R)ja.y; jj[2] = (R)jb.x; jj[3] = (R)jb.y; }
+        }
 #pragma unroll
-            for (int c = 0; c < B; ++c) acc[0].x[c] += g.x[c];
-          }
+        for (int q = 0; q < 4; ++q) {
+          const unsigned char* src = tl + (size_t)oo[q] * sizeof(V);       // row index -> byte offset
+          const V g0 = LD_S((const V*)src);
+          V g1 = V{};
+          if (XKC == 2) g1 = LD_S((const V*)(src + 32 * sizeof(V)));
 #pragma unroll
-          for (int c = 0; c < B; ++c) acc[0].x[c] *= p.Juni;
-        } else {
-#pragma unroll 4
-          for (int e = 0; e < cnt; ++e) {
-            const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
-            const R J = __shfl_sync(0xffffffffu, eJ, e);
-            const V g = LD_S((const V*)(tl + off));
-#pragma unroll
-            for (int c = 0; c < B; ++c) acc[0].x[c] += J * g.x[c];
+          for (int c = 0; c < B; ++c) {
+            if (UNIJ) { acc[0].x[c] += g0.x[c]; if (XKC == 2) acc[1].x[c] += g1.x[c]; }
+            else { acc[0].x[c] += jj[q] * g0.x[c]; if (XKC == 2) acc[1].x[c] += jj[q] * g1.x[c]; }
           }
         }
-      } else {
-        own[1] = LD_S((const V*)(tl + (size_t)sl * X * sizeof(V) + 32 * sizeof(V)));
-        acc[1] = V{};
-        if (UNIJ) {
-#pragma unroll 4
-          for (int e = 0; e < cnt; ++e) {
-            const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
-            const V g0 = LD_S((const V*)(tl + off)), g1 = LD_S((const V*)(tl + off + 32 * sizeof(V)));
+      }
+      if (UNIJ) {
 #pragma unroll
-            for (int c = 0; c < B; ++c) { acc[0].x[c] += g0.x[c]; acc[1].x[c] += g1.x[c]; }
-          }
-#pragma unroll
-          for (int c = 0; c < B; ++c) { acc[0].x[c] *= p.Juni; acc[1].x[c] *= p.Juni; }
-        } else {
-#pragma unroll 4
-          for (int e = 0; e < cnt; ++e) {
-            const uint32_t off = __shfl_sync(0xffffffffu, eo, e);
-            const R J = __shfl_sync(0xffffffffu, eJ, e);
-            const V g0 = LD_S((const V*)(tl + off)), g1 = LD_S((const V*)(tl + off + 32 * sizeof(V)));
-#pragma unroll
-            for (int c = 0; c < B; ++c) { acc[0].x[c] += J * g0.x[c]; acc[1].x[c] += J * g1.x[c]; }
-          }
-        }
+        for (int c = 0; c < B; ++c) { acc[0].x[c] *= p.Juni; acc[1].x[c] *= p.Juni; }
       }
 #pragma unroll
       for (int k = 0; k < PASSB_XK; ++k) {
@@ -565,6 +538,15 @@ int ftlm_passb_plan_create(ftlm_ctx* c, int mw, const std::vector<int>& cand, st
           sj += d.Jh;
           ++n;
         }
+      }
+      // pad to a multiple of 4 with the word's own tile row: J = 0, or - uniform couplings, where the kernel adds first
+      // and multiplies once - the common J with the added J * v[n] taken back through the sum of J
+      const bool uni_w = [&] { for (size_t e = 1; e < w.Jh.size(); ++e) if (w.Jh[e] != w.Jh[0]) return false; return c->unij_allowed != 0 && !w.Jh.empty(); }();
+      while (n & 3) {
+        nbr[row * 32 + (size_t)n] = (uint32_t)slot[(size_t)u] * (uint32_t)X;
+        nbrJ[row * 32 + (size_t)n] = 0.0;
+        if (uni_w) sj += w.Jh[0];
+        ++n;
       }
       nbr[row * 32 + 31] = (uint32_t)n;
       nbrJ[row * 32 + 31] = sj;
