@@ -592,7 +592,9 @@ static int launch_window(ftlm_ctx* c, PassBWindow& w, const void* v, void* y, in
   }
   int grid = c->sm_count * w.ctas;
   if ((uint32_t)grid > p.item_end - p.item_begin) grid = (int)std::max(1u, p.item_end - p.item_begin);
-  const int threads = (sizeof(R) * B > 4) ? 512 : w.threads;     // the kernel's launch bound
+  // 512 threads whenever the plan's rows are wider than 4 bytes (the launch bound of those kernels); a narrower run on
+  // the same plan (remainder group, plan_batch) keeps that shape, so that the order of every sum is the same
+  const int threads = (sizeof(R) * (size_t)ftlm_plan_batch(c) > 4) ? 512 : w.threads;
   if (fused) {
     auto k = passb_kernel<R, B, MODE, true>;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)w.smem));

@@ -706,7 +706,9 @@ TmlLaunchCfg tml_config(const ftlm_ctx* c, const TmlPlan* t, int batch) {
 template <typename R, int B, int MODE>
 int launch_tml(ftlm_ctx* c, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
   TmlPlan* t = c->tml;
-  const TmlLaunchCfg cfg = tml_config(c, t, B);
+  // launch shape of the batch the plan was built for: a narrower run on the same plan (remainder group, plan_batch)
+  // keeps the thread count and hence the order of every sum
+  const TmlLaunchCfg cfg = tml_config(c, t, std::max(B, ftlm_plan_batch(c)));
   if (cfg.smem == 0) { ftlm_set_error("TML: batch %d does not fit shared memory with this split", B); return FTLM_EUNSUPPORTED; }
   if (fused == 1 && B > t->partials_batch) { ftlm_set_error("TML: internal: partials sized for batch %d", t->partials_batch); return FTLM_EINVAL; }
   TmlParams<R> p;

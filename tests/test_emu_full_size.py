@@ -43,3 +43,19 @@ def test_emu_full_size_sampled(cfg, mode, opts, both):
 def test_emu_config5_full_size_sampled(opts):
     d = sampled({"config": 5, "mode": "cr", "samples": 1, "lowmem": True, "options": opts}, timeout=3 * 3600)
     assert d["dim"] == 2333606220 and d["windows"] >= 1
+
+
+def test_emu_smoke_configurations():
+    """The two multi-pass configurations __graft_entry__.smoke() runs on the device (folded N = 18 ring, D = 48 620):
+    TMLR + window + lazy normalisation, and a batch of 4 chains through TML + window (bit-identical to single chains)."""
+    run = os.path.join(ROOT, "tests", "emu", "run_case.py")
+    for spec in ({"wl": "fring18j", "n_up": 9, "mode": "clt", "prec": "fp32", "what": ["apply", "lanczos"], "steps": 6,
+                  "options": [["passb", 1], ["passb_lo_min", 5], ["tml_split", 6 | (4 << 8)], ["kernel", 3], ["tmlr", 1], ["lazy_norm", 1]]},
+                 {"wl": "fring18j", "n_up": 9, "mode": "cr", "prec": "fp32", "what": [], "steps": 8, "batch": [4, 4],
+                  "options": [["passb", 1], ["passb_lo_min", 5], ["tml_split", 6 | (4 << 8)], ["kernel", 3]]}):
+        p = subprocess.run([sys.executable, run, json.dumps(spec)], capture_output=True, text=True, timeout=3600)
+        assert p.returncode == 0, p.stderr[-2000:]
+        d = json.loads(p.stdout.strip().splitlines()[-1])
+        assert d["ok"] and d["passb"][0] >= 1, d
+        if "batch" in spec:
+            assert d["batch_identical"], d

@@ -338,7 +338,7 @@ def test_thermodynamics_ring12_all_sectors_vs_oracle(mode, prec):
 
 @pytest.mark.parametrize("prec", ["fp32", "fp64"])
 @pytest.mark.parametrize("mode", ["clt", "cr"])
-@pytest.mark.parametrize("w_bits,m_bits", [(5, 1), (6, 4), (8, 7), (9, 7), (10, 6), (12, 3), (7, 9), (5, 9)])
+@pytest.mark.parametrize("w_bits,m_bits", [(5, 1), (6, 4), (8, 7), (9, 7), (9, 8), (10, 6), (12, 3), (7, 9), (5, 9)])
 def test_tml_kernel_splits(prec, mode, w_bits, m_bits):
     # every LL/MM/ML/TT/TM/TL classification of the same bonds must give the same H.v and indices
     rng = np.random.default_rng(100 * w_bits + m_bits)
