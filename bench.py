@@ -142,6 +142,7 @@ def run_reference(args, w, n_up):
 # name -> option settings, in order (the candidates of ftlm_autotune, include/ftlm.h)
 CANDIDATES = {
     "row": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 1)],
+    "rowg": [("lazy_norm", 0), ("tmlr", 0), ("kernel", 2)],
     "tml": [("lazy_norm", 0), ("tmlr", 0), ("tml_split", 0), ("passb", 0), ("kernel", 3)],
     "tml+passb": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 0), ("passb", 1), ("kernel", 3)],
     "tml+passb_1cta": [("tmlr", 0), ("tml_split", 0), ("passb_smax", 0), ("passb_ctas", 1), ("passb", 1), ("kernel", 3)],
@@ -428,7 +429,7 @@ def main():
             ftlm.ftlm_set_option(ctx, key, 0)
         ftlm.ftlm_set_option(ctx, "batch", B)
     ftlm.ftlm_set_option(ctx, "graph", args.graph)
-    kernel_used = {1: "row", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
+    kernel_used = {1: "row", 2: "rowg", 3: "tml"}[ftlm.ftlm_get_option(ctx, "kernel")]
     if kernel_used == "tml" and ftlm.ftlm_get_option(ctx, "tmlr") == 1 and ftlm.ftlm_get_option(ctx, "tmlr_available") == 1:
         kernel_used = "tmlr"
     n_windows = max(ftlm.ftlm_get_option(ctx, "passb_windows"), 0) if kernel_used in ("tml", "tmlr") else 0

@@ -45,9 +45,12 @@ enum { FTLM_FP32 = 0, FTLM_FP64 = 1 };
 /* Kernel variants selectable with ftlm_set_option("kernel", ...).
  * ROW  = one thread per row, every row unranked, per-bond loop (the paper's launch shape, L105,
  *        L136, L203), kept as the plain in-library baseline.
+ * ROWG = the same per-bond loop with the row state the north_star describes: a thread owns 8 consecutive rows,
+ *        unranks the first (L136) and steps to the next seven with a Gosper-style same-popcount successor; a lane's
+ *        rows are 32 contiguous bytes, so the vector streams stay coalesced.  Single vector (no batch).
  * TML  = B200 design: label split into top/middle/low parts, one CTA per top part with the tile
  *        staged in shared memory and per-class neighbour tables. */
-enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_TML = 3 };
+enum { FTLM_KERNEL_AUTO = 0, FTLM_KERNEL_ROW = 1, FTLM_KERNEL_ROWG = 2, FTLM_KERNEL_TML = 3 };
 
 /* ---- handle ------------------------------------------------------------------------------ */
 

@@ -99,6 +99,7 @@ extern "C" int ftlm_autotune(ftlm_ctx* c, int reps, char* report, int report_cap
   const int home_split = saved_w | (saved_m << 8);
   const Cand cands[] = {
       {"row", FTLM_KERNEL_ROW, 0, 0, 0, 0, 0, 0, 1},
+      {"rowg", FTLM_KERNEL_ROWG, 0, 0, 0, 0, 0, 0, 0},
       {"tml", FTLM_KERNEL_TML, 0, 0, 0, 0, 0, 0, 0},
       {"tml+passb", FTLM_KERNEL_TML, 1, 0, 0, 0, 0, 0, 0},
       {"tml+passb_1cta", FTLM_KERNEL_TML, 1, 0, 1, 0, 0, 0, 0},

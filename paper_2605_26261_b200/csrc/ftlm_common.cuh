@@ -157,6 +157,9 @@ int ftlm_effective_kernel(const ftlm_ctx* c);
 // the in-kernel finalisation of alpha_j, beta_j into ctx->d_state.
 int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, int batch, cudaStream_t s);
 int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
+// ROWG: unrank once per 8 consecutive rows, Gosper-style successor in between (single vector)
+int ftlm_launch_hv_rowg(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s);
+int ftlm_launch_neighbors_rowg(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s);
 
 int ftlm_tml_plan_create(ftlm_ctx* c);
 void ftlm_tml_plan_destroy(ftlm_ctx* c);

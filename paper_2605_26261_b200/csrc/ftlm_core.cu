@@ -451,7 +451,8 @@ extern "C" int64_t ftlm_table_bytes(const ftlm_ctx* c) {
 }
 
 int ftlm_effective_kernel(const ftlm_ctx* c) {
-  if (c->kernel == FTLM_KERNEL_ROW || c->mode == FTLM_INDEX_LIN) return FTLM_KERNEL_ROW;   // LIN: thread-per-row kernel only
+  if (c->kernel == FTLM_KERNEL_ROWG) return FTLM_KERNEL_ROWG;
+  if (c->kernel == FTLM_KERNEL_ROW || c->mode == FTLM_INDEX_LIN) return FTLM_KERNEL_ROW;   // LIN: thread-per-row kernels only
   if (c->kernel == FTLM_KERNEL_TML && c->tml) return FTLM_KERNEL_TML;
   if (c->kernel == FTLM_KERNEL_AUTO && c->tml && c->dim >= (1 << 20)) return FTLM_KERNEL_TML;
   return FTLM_KERNEL_ROW;                    // AUTO: small sectors are launch-bound, ROW is simpler
@@ -461,7 +462,7 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
   if (!c || !key) { ftlm_set_error("ftlm_set_option: NULL"); return FTLM_EINVAL; }
   graph_drop(c);                                         // a captured step belongs to the configuration it was captured under
   if (!strcmp(key, "kernel")) {
-    if (value != FTLM_KERNEL_AUTO && value != FTLM_KERNEL_ROW && value != FTLM_KERNEL_TML) { ftlm_set_error("kernel must be FTLM_KERNEL_AUTO, _ROW or _TML"); return FTLM_EINVAL; }
+    if (value != FTLM_KERNEL_AUTO && value != FTLM_KERNEL_ROW && value != FTLM_KERNEL_ROWG && value != FTLM_KERNEL_TML) { ftlm_set_error("kernel must be FTLM_KERNEL_AUTO, _ROW, _ROWG or _TML"); return FTLM_EINVAL; }
     if (value == FTLM_KERNEL_TML && (!c->tml || c->mode == FTLM_INDEX_LIN)) { ftlm_set_error("TML kernel unavailable for this sector / index mode"); return FTLM_EUNSUPPORTED; }
     c->kernel = (int)value; return FTLM_OK;
   }
@@ -602,6 +603,7 @@ static int launch_hv(ftlm_ctx* c, const void* v, const void* qp, void* y, int fu
     if (rc == FTLM_OK && pb) rc = ftlm_launch_passb(c, v, y, fused, batch, s);
     return rc;
   }
+  if (k == FTLM_KERNEL_ROWG && batch == 1) return ftlm_launch_hv_rowg(c, v, qp, y, fused, s);   // (a batch runs the ROW kernel)
   return ftlm_launch_hv_row(c, v, qp, y, fused, batch, s);
 }
 
@@ -638,6 +640,7 @@ extern "C" int ftlm_neighbors(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
   CK(cudaSetDevice(c->device));
   ftlm_chk_caller((cudaStream_t)stream, d_idx, (size_t)nrows * (size_t)c->nb * 8);
   if (ftlm_effective_kernel(c) == FTLM_KERNEL_TML) return ftlm_launch_neighbors_tml(c, row0, nrows, d_idx, (cudaStream_t)stream);
+  if (ftlm_effective_kernel(c) == FTLM_KERNEL_ROWG) return ftlm_launch_neighbors_rowg(c, row0, nrows, d_idx, (cudaStream_t)stream);
   return ftlm_launch_neighbors_row(c, row0, nrows, d_idx, (cudaStream_t)stream);
 }
 

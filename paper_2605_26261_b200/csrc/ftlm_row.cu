@@ -174,6 +174,107 @@ hv_row_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev,
   }
 }
 
+// ---- ROWG: unrank once, then Gosper-style successor (north_star: "row bit-states by unranking plus Gosper-style
+// successor enumeration"; L136 for the unrank) ---------------------------------------------------------------------
+// A thread owns G = 8 consecutive rows: the label of the first comes from the inverse map, the next seven from the
+// same-popcount successor  c = n & -n, r = n + c, n' = r | (((n ^ r) >> 2) >> ctz(n))  (the next larger integer with
+// the same number of ones = the next basis state in ascending order, reading 2).  A lane's 8 rows are 32 (FP32) or
+// 64 (FP64) contiguous bytes, a warp's 256 rows one contiguous kilobyte: the streams of v, q_prev and y stay fully
+// coalesced while the N-step unrank is paid once per 8 rows.
+#define ROWG_G 8
+template <typename L>
+__device__ __forceinline__ L gosper_next(L n) {
+  const L c = n & (L)(0 - n);
+  const L r = n + c;
+  return r | (((n ^ r) >> 2) >> (ffs_(n) - 1));
+}
+
+template <typename R, typename L, typename I, int MODE, bool FUSED>
+__global__ void __launch_bounds__(256)
+hv_rowg_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev, R* __restrict__ y) {
+  FTLM_DYN_SMEM(smem);
+  __shared__ double sh_red[96];
+  if (FUSED) { if (p.st->done) return; }
+  I* s_binom = (I*)smem;
+  const int nbin = (p.N + 1) * (p.K + 1);
+  BondS<R>* s_bonds = (BondS<R>*)(smem + (((size_t)nbin * sizeof(I) + 15) & ~(size_t)15));
+  load_tables<R, L, I>(p, s_binom, s_bonds);
+  const int K1 = p.K + 1;
+  const R bprev = FUSED ? (R)p.st->beta_prev : (R)0;
+  double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x * ROWG_G;
+  for (int64_t t0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * ROWG_G; t0 < p.dim; t0 += stride) {
+    const int ng = (int)(p.dim - t0 < ROWG_G ? p.dim - t0 : ROWG_G);
+    R vt[ROWG_G], qp[ROWG_G], out[ROWG_G];
+#pragma unroll
+    for (int g = 0; g < ROWG_G; ++g) {
+      vt[g] = g < ng ? LD_G(&v[t0 + g]) : (R)0;
+      qp[g] = (FUSED && g < ng) ? LD_G(&qprev[t0 + g]) : (R)0;
+    }
+    L n = unrank<L, I>((I)t0, p.N, K1, p.K, s_binom);
+#pragma unroll 1
+    for (int g = 0; g < ng; ++g) {
+      const int64_t t = t0 + g;
+      R acc = 0, danti = 0;
+      for (int b = 0; b < p.nb; ++b) {
+        const L m = (L)s_bonds[b].mask;
+        const L x = n & m;
+        if (x != 0 && x != m) {                                   // antiparallel spins
+          I idx;
+          if (MODE == FTLM_INDEX_CLT) idx = (I)clt_lookup((uint32_t)(n ^ m), p.clt);
+          else if (MODE == FTLM_INDEX_LIN) idx = (I)lin_lookup((uint64_t)(n ^ m), p.lin_h, p.lin_hi, p.lin_lo);
+          else idx = (I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom);
+          acc += s_bonds[b].Jh * LDG(&v[idx]);
+          danti += s_bonds[b].Jq;
+        }
+      }
+      R o = ((R)p.diag0 - 2 * danti) * vt[g] + acc;
+      if (FUSED) {
+        o -= bprev * qp[g];
+        s_qy += (double)vt[g] * (double)o;
+        s_yy += (double)o * (double)o;
+        s_qq += (double)vt[g] * (double)vt[g];
+      }
+      out[g] = o;
+      if (n != 0) n = gosper_next<L>(n);                          // (n == 0: the one-state sector N_up = 0)
+    }
+#pragma unroll
+    for (int g = 0; g < ROWG_G; ++g) if (g < ng) ST_G(&y[t0 + g], out[g]);
+  }
+  if (FUSED) lanczos_finish(s_qy, s_yy, s_qq, p.partials, p.stride, p.ticket, p.st, sh_red);
+}
+
+// neighbour indices through the same enumeration (unrank at the first row of a group, successor afterwards)
+template <typename L, typename I, int MODE>
+__global__ void __launch_bounds__(256)
+neighbors_rowg_kernel(RowParams p, int64_t row0, int64_t nrows, int64_t* __restrict__ out) {
+  FTLM_DYN_SMEM(smem);
+  I* s_binom = (I*)smem;
+  const int nbin = (p.N + 1) * (p.K + 1);
+  BondS<float>* s_bonds = (BondS<float>*)(smem + (((size_t)nbin * sizeof(I) + 15) & ~(size_t)15));
+  load_tables<float, L, I>(p, s_binom, s_bonds);
+  const int K1 = p.K + 1;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x * ROWG_G;
+  for (int64_t r0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * ROWG_G; r0 < nrows; r0 += stride) {
+    L n = unrank<L, I>((I)(row0 + r0), p.N, K1, p.K, s_binom);
+    for (int g = 0; g < ROWG_G && r0 + g < nrows; ++g) {
+      const int64_t t = row0 + r0 + g;
+      for (int b = 0; b < p.nb; ++b) {
+        const L m = (L)s_bonds[b].mask;
+        const L x = n & m;
+        int64_t idx = -1;
+        if (x != 0 && x != m) {
+          if (MODE == FTLM_INDEX_CLT) idx = (int64_t)clt_lookup((uint32_t)(n ^ m), p.clt);
+          else if (MODE == FTLM_INDEX_LIN) idx = (int64_t)lin_lookup((uint64_t)(n ^ m), p.lin_h, p.lin_hi, p.lin_lo);
+          else idx = (int64_t)(I)((I)t + cr_delta<L, I>(n, s_bonds[b].i, s_bonds[b].j, K1, s_binom));
+        }
+        ST_G(&out[(r0 + g) * p.nb + b], idx);
+      }
+      if (n != 0) n = gosper_next<L>(n);
+    }
+  }
+}
+
 template <typename L, typename I, int MODE>
 __global__ void __launch_bounds__(256)
 neighbors_row_kernel(RowParams p, int64_t row0, int64_t nrows, int64_t* __restrict__ out) {
@@ -306,6 +407,58 @@ int ftlm_launch_hv_row(ftlm_ctx* c, const void* v, const void* qprev, void* y, i
     if (!c->idx64) return launch_hv<double, uint64_t, uint32_t>(c, p, v, qprev, y, fused, batch, s);
     return launch_hv<double, uint64_t, uint64_t>(c, p, v, qprev, y, fused, batch, s);
   }
+}
+
+namespace {
+template <typename R, typename L, typename I>
+int launch_hv_g(ftlm_ctx* c, const RowParams& p, const void* v, const void* qp, void* y, int fused, cudaStream_t s) {
+  const size_t sm = table_smem(c, sizeof(BondS<R>));
+  const int grid = grid_for(c, (c->dim + ROWG_G - 1) / ROWG_G, 8);
+  if (fused && grid > c->max_blocks) { ftlm_set_error("internal: grid > max_blocks"); return FTLM_EINVAL; }
+#define LAUNCHG(MODE, FUSED)                                                                     \
+  do {                                                                                           \
+    auto k = hv_rowg_kernel<R, L, I, MODE, FUSED>;                                               \
+    if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); \
+    FTLM_LAUNCH(k, grid, 256, sm, s, p, (const R*)v, (const R*)qp, (R*)y);                                \
+  } while (0)
+  if (c->mode == FTLM_INDEX_CLT) { if (fused) LAUNCHG(FTLM_INDEX_CLT, true); else LAUNCHG(FTLM_INDEX_CLT, false); }
+  else if (c->mode == FTLM_INDEX_LIN) { if (fused) LAUNCHG(FTLM_INDEX_LIN, true); else LAUNCHG(FTLM_INDEX_LIN, false); }
+  else { if (fused) LAUNCHG(FTLM_INDEX_CR, true); else LAUNCHG(FTLM_INDEX_CR, false); }
+#undef LAUNCHG
+  CK(cudaGetLastError());
+  return FTLM_OK;
+}
+}  // namespace
+
+int ftlm_launch_hv_rowg(ftlm_ctx* c, const void* v, const void* qprev, void* y, int fused, cudaStream_t s) {
+  RowParams p = make_params(c);
+  if (c->prec == FTLM_FP32) {
+    if (!c->lab64) return launch_hv_g<float, uint32_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    if (!c->idx64) return launch_hv_g<float, uint64_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    return launch_hv_g<float, uint64_t, uint64_t>(c, p, v, qprev, y, fused, s);
+  } else {
+    if (!c->lab64) return launch_hv_g<double, uint32_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    if (!c->idx64) return launch_hv_g<double, uint64_t, uint32_t>(c, p, v, qprev, y, fused, s);
+    return launch_hv_g<double, uint64_t, uint64_t>(c, p, v, qprev, y, fused, s);
+  }
+}
+
+int ftlm_launch_neighbors_rowg(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s) {
+  RowParams p = make_params(c);
+  const size_t sm = table_smem(c, sizeof(BondS<float>));
+  const int grid = grid_for(c, (nrows + ROWG_G - 1) / ROWG_G, 8);
+#define LAUNCHNG(L, I)                                                                                \
+  do {                                                                                                \
+    if (c->mode == FTLM_INDEX_CLT) { auto k = neighbors_rowg_kernel<L, I, FTLM_INDEX_CLT>; if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); FTLM_LAUNCH(k, grid, 256, sm, s, p, row0, nrows, d_idx); } \
+    else if (c->mode == FTLM_INDEX_LIN) { auto k = neighbors_rowg_kernel<L, I, FTLM_INDEX_LIN>; if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); FTLM_LAUNCH(k, grid, 256, sm, s, p, row0, nrows, d_idx); } \
+    else { auto k = neighbors_rowg_kernel<L, I, FTLM_INDEX_CR>; if (sm > 48 * 1024) CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); FTLM_LAUNCH(k, grid, 256, sm, s, p, row0, nrows, d_idx); } \
+  } while (0)
+  if (!c->lab64) LAUNCHNG(uint32_t, uint32_t);
+  else if (!c->idx64) LAUNCHNG(uint64_t, uint32_t);
+  else LAUNCHNG(uint64_t, uint64_t);
+#undef LAUNCHNG
+  CK(cudaGetLastError());
+  return FTLM_OK;
 }
 
 int ftlm_launch_neighbors_row(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t* d_idx, cudaStream_t s) {

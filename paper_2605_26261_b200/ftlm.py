@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libftlm_checked.so" if CHECKED else "libftlm.so"
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
 INDEX_CLT, INDEX_CR, INDEX_LIN = 0, 1, 2
 FP32, FP64 = 0, 1
-KERNEL_AUTO, KERNEL_ROW, KERNEL_TML = 0, 1, 3
+KERNEL_AUTO, KERNEL_ROW, KERNEL_ROWG, KERNEL_TML = 0, 1, 2, 3
 MAX_STEPS = 1024
 
 EXPORTS = [

@@ -18,7 +18,7 @@ if ROOT not in sys.path:
 INDEX = {"clt": 0, "cr": 1, "lin": 2}
 PREC = {"fp32": 0, "fp64": 1}
 NDT = {"fp32": np.float32, "fp64": np.float64}
-KERNEL = {"auto": 0, "row": 1, "tml": 3}
+KERNEL = {"auto": 0, "row": 1, "rowg": 2, "tml": 3}
 
 _lib = None
 

@@ -135,6 +135,45 @@ def test_emu_tmlr_bulk_copy_with_unaligned_caller_vectors(shift, prec):
     assert res["tmlr"] == [1, 1]
 
 
+@pytest.mark.parametrize("spec", [
+    {"wl": "ring12j", "n_up": 6, "mode": "cr", "prec": "fp64"},
+    {"wl": "rand15_40_5", "n_up": 7, "mode": "clt", "prec": "fp32"},
+    {"wl": "ring16", "n_up": 15, "mode": "lin", "prec": "fp32", "steps": 16},       # D = 16: two groups of 8, breakdown
+    {"wl": "ring12", "n_up": 0, "mode": "cr", "prec": "fp64", "what": ["neighbors", "apply"]},   # D = 1, label 0
+    {"wl": "ring12", "n_up": 12, "mode": "clt", "prec": "fp32", "what": ["neighbors", "apply"]},
+    {"wl": "ring13", "n_up": 5, "mode": "cr", "prec": "fp32"},                        # D = 1287: ragged last group
+])
+def test_emu_rowg_unrank_plus_gosper_successor(spec):
+    """Kernel ROWG (north_star: "row bit-states by unranking plus Gosper-style successor enumeration"): a thread unranks
+    the first of 8 consecutive rows (L136) and steps through the next seven with the same-popcount successor; neighbour
+    indices bit-exact, H.v and Lanczos against the oracle, in all three index modes and on the degenerate sectors."""
+    res = run_case(dict({"what": ["neighbors", "apply", "lanczos"], "options": [["kernel", 2]]}, **spec))
+    assert res["kernel"] == 2
+
+
+def test_emu_rowg_64_bit_labels_sampled():
+    code = ("import sys, json; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+            "import numpy as np, emu_harness as E\n"
+            "from oracle import ftlm_oracle as fo\n"
+            "from paper_2605_26261_b200 import workloads as W\n"
+            "w = W.baseline_config(5)\n"
+            "_, Dc = fo.cr_tables(34)\n"
+            "bad = 0\n"
+            "with E.EmuCtx(w, 17, 'cr', 'fp32', options=[('kernel', 2)]) as c:\n"
+            "    for r0 in (0, 2**31 - 5, c.dim // 2 + 3, c.dim - 19):\n"
+            "        nb = c.neighbors(int(r0), 19)\n"
+            "        lab = fo.alg1_unrank_vec(np.arange(r0, r0 + 19, dtype=np.uint64), 34, 17, Dc)\n"
+            "        for k in range(19):\n"
+            "            for b in range(w.n_bonds):\n"
+            "                m = (1 << int(w.bond_i[b])) | (1 << int(w.bond_j[b])); x = int(lab[k]) & m\n"
+            "                e = -1 if x in (0, m) else fo.rank_by_counting(int(lab[k]) ^ m, 34, 17)\n"
+            "                bad += int(nb[k, b] != e)\n"
+            "print(json.dumps({'bad': bad}))\n" % (ROOT, os.path.join(ROOT, "tests", "emu")))
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    assert json.loads(p.stdout.strip().splitlines()[-1])["bad"] == 0
+
+
 def test_emu_passb_off_keeps_top_bonds_in_tml():
     res = run_case({"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp64",
                     "options": [["passb", 0], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]],
