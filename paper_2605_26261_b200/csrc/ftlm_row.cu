@@ -212,8 +212,9 @@ hv_rowg_kernel(RowParams p, const R* __restrict__ v, const R* __restrict__ qprev
       qp[g] = (FUSED && g < ng) ? LD_G(&qprev[t0 + g]) : (R)0;
     }
     L n = unrank<L, I>((I)t0, p.N, K1, p.K, s_binom);
-#pragma unroll 1
-    for (int g = 0; g < ng; ++g) {
+#pragma unroll
+    for (int g = 0; g < ROWG_G; ++g) {                             // unrolled: the 8 rows' values stay in registers
+      if (g >= ng) break;
       const int64_t t = t0 + g;
       R acc = 0, danti = 0;
       for (int b = 0; b < p.nb; ++b) {
