@@ -291,7 +291,7 @@ def probe_choice(args):
 
 
 ALL_CASES = [  # (config, mode, extra flags): north_star "five synthetic clusters ... CLT vs CR"
-    (1, "clt", []), (1, "cr", []), (1, "clt", ["--graph", "1"]), (1, "clt", ["--batch", "4", "--graph", "1"]),
+    (1, "clt", []), (1, "cr", []), (1, "clt", ["--graph", "1"]), (1, "clt", ["--batch", "4", "--graph", "1"]), (1, "clt", ["--persistent", "1"]),
     (2, "clt", []), (2, "cr", []), (2, "clt", ["--graph", "1"]), (2, "clt", ["--batch", "4"]),
     (3, "clt", []), (3, "cr", []),
     (4, "clt", []), (4, "cr", []), (41, "clt", []), (40, "clt", []), (4, "clt", ["--batch", "2"]), (4, "clt", ["--batch", "4"]),
@@ -324,8 +324,8 @@ def run_all(args):
         rows.append({"config": cfg, "workload": d["config"]["workload"], "mode": mode, "flags": extra, "dim": d["config"]["dim"],
                      "kernel": d["config"]["candidate"], "hv_passes": d["config"]["hv_passes"], "steps_per_s": d["value"],
                      "ms_per_step": d["ms_per_step"], "hv_rows_per_s": d["hv_rows_per_s"], "hv_gelem_per_s": d["hv_gelem_per_s"],
-                     "hv_ms": r["ms_per_launch"], "floorA_GBps": r["achieved"], "frac_of_measured_hbm": r["frac"],
-                     "norm_GBps": r["norm_kernel_GBps"], "oracle_rows_per_s": (d.get("cpu_baseline") or {}).get("rows_per_s"),
+                     "hv_ms": r.get("ms_per_launch"), "floorA_GBps": r["achieved"], "frac_of_measured_hbm": r["frac"],
+                     "norm_GBps": r.get("norm_kernel_GBps"), "oracle_rows_per_s": (d.get("cpu_baseline") or {}).get("rows_per_s"),
                      "oracle_cores": (d.get("cpu_baseline") or {}).get("cores"), "clocks": d.get("clocks"),
                      "site_numbering": d["config"].get("site_numbering"), "probe_note": d["config"].get("probe_note")})
         if cfg == 4 and mode == "clt" and not extra:
@@ -338,7 +338,7 @@ def run_all(args):
             sys.stderr.write(f"| {r['config']} | {r['mode']} | {' '.join(r['flags'])} | ERROR {r['error']} |\n")
         else:
             sys.stderr.write(f"| {r['workload']} | {r['mode']} | {' '.join(r['flags'])} | {r['kernel']} | {r['hv_passes']} | {r['steps_per_s']:.1f} | "
-                             f"{r['hv_rows_per_s']:.3e} | {r['hv_gelem_per_s']:.2f} | {r['floorA_GBps']:.1f} | {r['frac_of_measured_hbm']:.4f} | "
+                             f"{r['hv_rows_per_s']:.3e} | {(r['hv_gelem_per_s'] or 0):.2f} | {r['floorA_GBps']:.1f} | {r['frac_of_measured_hbm']:.4f} | "
                              f"{(r['oracle_rows_per_s'] or 0):.3e} |\n")
     if headline is not None:
         headline["config"]["all_cases_file"] = "gpurun_out/bench_all.json"
@@ -364,6 +364,7 @@ def main():
     ap.add_argument("--tml-mid-bits", type=int, default=0)
     ap.add_argument("--batch", type=int, default=1, choices=[1, 2, 4], help="chains advanced together (L207); value counts chain-steps")
     ap.add_argument("--graph", type=int, default=0, choices=[0, 1], help="replay steps from a CUDA graph")
+    ap.add_argument("--persistent", type=int, default=0, choices=[0, 1], help="small sectors: all chains of the sector in one launch (csrc/ftlm_chain.cu); times ftlm_lanczos(R, steps)")
     ap.add_argument("--all", action="store_true", help="every BASELINE config and index mode (children), table in gpurun_out/bench_all.json")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -438,6 +439,47 @@ def main():
     D = ftlm.ftlm_dim(ctx)
     K, Wm = args.steps, args.warmup
     assert 1 <= K and K + Wm <= ftlm.MAX_STEPS, "steps + warmup must be <= 1024 (one chain)"
+
+    if args.persistent:
+        # small sectors: ONE launch runs all R chains of the sector, one CTA per chain, vectors in shared
+        # memory; the unit is still a fused chain-step, timed over whole ftlm_lanczos calls (device events)
+        ftlm.ftlm_set_option(ctx, "persistent", 1)
+        assert ftlm.ftlm_get_option(ctx, "persistent_fits") == 1, "--persistent: this sector does not fit shared memory"
+        Rp = max(w.R, 1)
+        for _ in range(max(Wm, 3)):
+            ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, Rp, K)
+        barrier()
+        sampler = ClockSampler(local)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 5
+        e0.record()
+        for _ in range(reps):
+            out = ftlm.ftlm_lanczos(ctx, W.SEED_VECTORS, Rp, K)
+        e1.record()
+        barrier()
+        ms = replicas.max_over_ranks(e0.elapsed_time(e1), dist, device="cuda")
+        sampler.stop_flag = True
+        steps_done = int(out["m_eff"].sum())
+        table_bytes = (8 * ((1 << w.N) // 32)) if mode == ftlm.INDEX_CLT else 0
+        line = {"metric": METRIC, "value": world * reps * steps_done / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": ms / (reps * max(steps_done, 1)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic",
+                "config": {"workload": f"config{args.config}:{w.name}", "N": w.N, "N_up": n_up, "dim": D, "n_bonds": w.n_bonds,
+                           "index_mode": args.mode, "kernel": "persistent_chain", "candidate": "persistent", "hv_passes": 1, "chains_per_launch": Rp,
+                           "l2": "vectors resident in shared memory for the whole chain", "parallelism": f"replicas x{world}",
+                           "note": "one launch = R chains x steps (start vectors, H.v, reductions, normalisation); includes the host tridiagonal solves of ftlm_lanczos"},
+                "roofline": {"bound": "hbm", "achieved": (12 * D + table_bytes) * reps * steps_done / (ms * 1e-3) / 1e9, "peak": measured_peak()[0], "unit": "GB/s",
+                             "frac": (12 * D + table_bytes) * reps * steps_done / (ms * 1e-3) / 1e9 / measured_peak()[0], "traffic": None,
+                             "kernel": "lanczos_chain_kernel", "note": "launch-bound sector: the byte floor is not what bounds it (SURVEY H7)"},
+                "cpu_baseline": None, "e2e": None, "gpu_launches": reps, "clocks": sampler.summary(),
+                "hv_rows_per_s": world * D * reps * steps_done / (ms * 1e-3), "hv_gelem_per_s": None}
+        ftlm.ftlm_destroy(ctx)
+        if rank == 0:
+            print(json.dumps(line), flush=True)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
 
     # ---- device-resident timing: `value` ---------------------------------------------------
     def begin():

@@ -76,7 +76,9 @@ int64_t ftlm_dim(const ftlm_ctx* ctx);
  * "tml_low_bits" / "tml_mid_bits" / "tml_split" = w | m << 8 (split of the TML kernels, 0 = auto),
  * "graph" (1 = ftlm_chain_steps captures two consecutive fused steps - three with "lazy_norm" - into a CUDA graph
  * once and replays it; same kernels, same arithmetic, fewer launches: for the launch-bound small sectors; falls back
- * to direct launches if a graph call fails; read-only "graph_launches", "graph_failed"); multi-pass H.v of kernel TML (DESIGN.md
+ * to direct launches if a graph call fails; read-only "graph_launches", "graph_failed"); "persistent" (1 =
+ * ftlm_lanczos runs a sector whose three work vectors fit shared memory - read-only "persistent_fits" - with ONE
+ * launch for all R chains: one CTA per chain, vectors resident in shared memory for the whole chain); multi-pass H.v of kernel TML (DESIGN.md
  * 6.4-6.5): "passb" (1 = bonds that leave the tile go to PASS-B window passes; default 0),
  * "passb_lo_min" / "passb_smax" / "passb_ctas" (window planner: lowest label position, largest
  * window, CTAs per SM tried first; 0 = auto), "tmlr" (1 = in-tile pass by the TMLR kernel when its

@@ -101,6 +101,7 @@ struct ftlm_ctx {
   // options
   int kernel = FTLM_KERNEL_AUTO;
   int tml_low_bits = 0, tml_mid_bits = 0;
+  int use_persistent = 0;          // option "persistent": ftlm_lanczos runs small sectors with the one-launch chain kernel
   int use_graph = 0;               // option "graph": ftlm_chain_steps replays captured steps (CUDA graph)
   int graph_failed = 0;            // a capture / instantiate call failed on this handle: direct launches from then on
   int graph_roles[3] = {-1, -1, -1}, graph_batch = 0, graph_period = 0;   // what the cached graph was captured for
@@ -176,6 +177,13 @@ int ftlm_launch_hv_tmlr(ftlm_ctx* c, const void* v, const void* qprev, void* y, 
 int ftlm_launch_hv_tmlr_lazy(ftlm_ctx* c, void* yq, const void* q, void* y, int fused, cudaStream_t s);
 bool ftlm_tmlr_lazy_ok(const ftlm_ctx* c);
 
+// Persistent chain kernel (ftlm_chain.cu): whole Lanczos chains of a small sector in one launch, one CTA per chain,
+// the three work vectors in shared memory.  ftlm_chain_persistent_fits: the sector fits; the launch runs chains
+// r0 .. r0 + nchains - 1 for `limit` steps and leaves alpha / beta / step counts in d_alpha, d_beta [nchains][limit], d_m_eff.
+bool ftlm_chain_persistent_fits(const ftlm_ctx* c);
+int ftlm_launch_chain_persistent(ftlm_ctx* c, uint64_t seed, int r0, int nchains, int limit, double* d_alpha, double* d_beta,
+                                 int* d_m_eff, cudaStream_t s);
+
 // PASS-B (ftlm_passb.cu).  `tt` lists the bonds whose two sites lie at positions >= mw (candidate
 // top-top bonds) as indices into c->bonds; on return window_of[k] is the PASS-B window that took
 // tt[k] or -1 if the bond stays in the TML kernel.  FTLM_OK with c->passb == nullptr if no window pays.
@@ -192,6 +200,21 @@ static inline int ftlm_plan_batch(const ftlm_ctx* c) { return c->plan_batch > c-
 
 // ---- device helpers ---------------------------------------------------------------------
 #ifdef __CUDACC__
+
+// counter-based start-vector generator: element t of the chain with key `key`
+#define FTLM_GOLD 0x9E3779B97F4A7C15ull
+__device__ __forceinline__ uint64_t mix64(uint64_t x) {
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+  return x ^ (x >> 31);
+}
+__device__ __forceinline__ double gauss_elem(uint64_t key, uint64_t t) {
+  const uint64_t a = mix64(key + FTLM_GOLD * (2ull * t + 1ull));
+  const uint64_t b = mix64(key + FTLM_GOLD * (2ull * t + 2ull));
+  const double u1 = ((double)(a >> 11) + 1.0) * 0x1.0p-53;
+  const double u2 = (double)(b >> 11) * 0x1.0p-53;
+  return sqrt(-2.0 * log(u1)) * cos(6.283185307179586 * u2);
+}
 
 __device__ __forceinline__ int popc_(uint32_t x) { return __popc(x); }
 __device__ __forceinline__ int popc_(uint64_t x) { return __popcll(x); }

@@ -1,5 +1,6 @@
 // libftlm core: handle, sector tables (A0/A1), start vectors, the fused Lanczos chain driver
 // and the C-ABI entry points that dispatch to the ROW / TML kernels.
+#include <algorithm>
 #include <cstdarg>
 #include <cstddef>
 #include <cstdio>
@@ -184,24 +185,10 @@ __global__ void clt_build_kernel(uint2* __restrict__ clt, int64_t nblk, int N, i
 }
 
 // ---- start vectors (readings 12-14) ---------------------------------------
-__device__ __forceinline__ uint64_t mix64(uint64_t x) {
-  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
-  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
-  return x ^ (x >> 31);
-}
 static uint64_t mix64_host(uint64_t x) {
   x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
   x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
   return x ^ (x >> 31);
-}
-#define FTLM_GOLD 0x9E3779B97F4A7C15ull
-
-__device__ __forceinline__ double gauss_elem(uint64_t key, uint64_t t) {
-  const uint64_t a = mix64(key + FTLM_GOLD * (2ull * t + 1ull));
-  const uint64_t b = mix64(key + FTLM_GOLD * (2ull * t + 2ull));
-  const double u1 = ((double)(a >> 11) + 1.0) * 0x1.0p-53;
-  const double u2 = (double)(b >> 11) * 0x1.0p-53;
-  return sqrt(-2.0 * log(u1)) * cos(6.283185307179586 * u2);
 }
 
 __global__ void __launch_bounds__(256)
@@ -478,6 +465,7 @@ extern "C" int ftlm_set_option(ftlm_ctx* c, const char* key, int64_t value) {
     return rc;
   }
   if (!strcmp(key, "graph")) { c->use_graph = value ? 1 : 0; c->graph_failed = 0; return FTLM_OK; }
+  if (!strcmp(key, "persistent")) { c->use_persistent = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "allow_unverified")) { c->allow_unverified = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "tmlr")) { c->use_tmlr = value ? 1 : 0; return FTLM_OK; }
   if (!strcmp(key, "lazy_norm")) { c->lazy_norm = value ? 1 : 0; return FTLM_OK; }
@@ -557,6 +545,8 @@ extern "C" int64_t ftlm_get_option(const ftlm_ctx* c, const char* key) {
   if (!c) return -1;
   if (!strcmp(key, "kernel")) return ftlm_effective_kernel(c);
   if (!strcmp(key, "graph")) return c->use_graph;
+  if (!strcmp(key, "persistent")) return c->use_persistent;
+  if (!strcmp(key, "persistent_fits")) return ftlm_chain_persistent_fits(c) ? 1 : 0;
   if (!strcmp(key, "graph_launches")) return c->graph_launches;
   if (!strcmp(key, "graph_failed")) return c->graph_failed;
   if (!strcmp(key, "passb")) return c->use_passb;
@@ -645,7 +635,9 @@ extern "C" int ftlm_neighbors(ftlm_ctx* c, int64_t row0, int64_t nrows, int64_t*
 }
 
 // ---- start vectors -----------------------------------------------------------------------------
-static uint64_t chain_key(uint64_t seed, int N_up, int r) {
+uint64_t ftlm_chain_key(uint64_t seed, int N_up, int r);
+static uint64_t chain_key(uint64_t seed, int N_up, int r) { return ftlm_chain_key(seed, N_up, r); }
+uint64_t ftlm_chain_key(uint64_t seed, int N_up, int r) {
   uint64_t k = mix64_host(seed);
   k = mix64_host(k + FTLM_GOLD * (uint64_t)(N_up + 1));
   k = mix64_host(k + FTLM_GOLD * (uint64_t)(r + 1));
@@ -921,6 +913,38 @@ static int lanczos_impl(ftlm_ctx* c, const void* h_q1, uint64_t seed, int R, int
   }
   const size_t bytes = (size_t)c->dim * ftlm_elem_size(c);
   for (size_t k = 0; k < (size_t)R * n_steps; ++k) { h_alpha[k] = 0.0; h_beta[k] = 0.0; }
+  if (c->use_persistent && !h_q1 && R > 0 && ftlm_chain_persistent_fits(c)) {
+    // small sector: all R chains in ONE launch, one CTA per chain, vectors in shared memory (ftlm_chain.cu)
+    CK(cudaSetDevice(c->device));
+    const int limit = (int)std::min<int64_t>(n_steps, c->dim);
+    double *d_a = nullptr, *d_b = nullptr;
+    int* d_m = nullptr;
+    const size_t nb = (size_t)R * limit * 8;
+    if (ftlm_dmalloc(&d_a, nb) != cudaSuccess || ftlm_dmalloc(&d_b, nb) != cudaSuccess || ftlm_dmalloc(&d_m, (size_t)R * 4) != cudaSuccess) {
+      cudaGetLastError(); ftlm_dfree(d_a); ftlm_dfree(d_b); ftlm_dfree(d_m);
+      ftlm_set_error("ftlm_lanczos: out of device memory"); return FTLM_ENOMEM;
+    }
+    int rc = ftlm_launch_chain_persistent(c, seed, 0, R, limit, d_a, d_b, d_m, s);
+    std::vector<double> ha((size_t)R * limit), hb((size_t)R * limit);
+    if (rc == FTLM_OK && (cudaMemcpy(ha.data(), d_a, nb, cudaMemcpyDeviceToHost) != cudaSuccess || cudaMemcpy(hb.data(), d_b, nb, cudaMemcpyDeviceToHost) != cudaSuccess ||
+                          cudaMemcpy(h_m_eff, d_m, (size_t)R * 4, cudaMemcpyDeviceToHost) != cudaSuccess))
+      rc = ftlm_cuda_fail(cudaGetLastError(), "ftlm_lanczos: copy of the coefficients");
+    ftlm_dfree(d_a); ftlm_dfree(d_b); ftlm_dfree(d_m);
+    if (rc != FTLM_OK) return rc;
+    for (int r = 0; r < R; ++r) {
+      const int m = h_m_eff[r];
+      for (int k = 0; k < m; ++k) h_alpha[(size_t)r * n_steps + k] = ha[(size_t)r * limit + k];
+      for (int k = 0; k + 1 < m; ++k) h_beta[(size_t)r * n_steps + k] = hb[(size_t)r * limit + k];
+      if (h_theta && h_weight) {
+        double* th = h_theta + (size_t)r * n_steps;
+        double* w = h_weight + (size_t)r * n_steps;
+        for (int k = 0; k < n_steps; ++k) { th[k] = 0.0; w[k] = 0.0; }
+        rc = ftlm_tridiag_eig(m, h_alpha + (size_t)r * n_steps, h_beta + (size_t)r * n_steps, th, w);
+        if (rc != FTLM_OK) return rc;
+      }
+    }
+    return FTLM_OK;
+  }
   // chains advance in groups of option "batch" (4, 2 or 1) on interleaved vectors; a remainder runs in smaller groups
   for (int r = 0; r < R;) {
     int nb = c->batch;

@@ -76,6 +76,7 @@ def main():
         res["passb"] = [c.get("passb_windows"), c.get("passb_bonds"), c.get("passb_lo"), c.get("passb_s")]
         res["tml"] = [c.get("tml_w"), c.get("tml_m")]
         res["tmlr"] = [c.get("tmlr"), c.get("tmlr_available")]
+        res["persistent"] = [c.get("persistent"), c.get("persistent_fits")]
         assert c.dim == D
         what = spec.get("what", ["neighbors", "apply"])
         if "neighbors" in what:
@@ -112,6 +113,22 @@ def main():
             res["lanczos_dalpha"], res["lanczos_dbeta"] = da, db
             res["m_eff"] = int(out["m_eff"][0])
             res["ok"] = res["ok"] and da <= tol and db <= tol
+            if spec.get("chains", 1) > 1:                  # several chains in one call (persistent kernel: one CTA each)
+                Rn = spec["chains"]
+                outR = c.lanczos(W.SEED_VECTORS, Rn, m)
+                worst = 0.0
+                for r in range(Rn):
+                    q1 = fo.start_vector(W.SEED_VECTORS, n_up, r, D)
+                    ar, br = fo.lanczos(lambda x: fo.apply_H(basis, w.N, w.bond_i, w.bond_j, w.J, h, n_up, x), q1, m)[:2]
+                    kk = min(int(outR["m_eff"][r]), len(ar), 8)
+                    if kk:
+                        worst = max(worst, float(np.max(np.abs(outR["alpha"][r][:kk] - np.asarray(ar)[:kk]))))
+                    if kk > 1:
+                        worst = max(worst, float(np.max(np.abs(outR["beta"][r][:kk - 1] - np.asarray(br)[:kk - 1]))))
+                    worst = max(worst, abs(float(outR["weight"][r][: int(outR["m_eff"][r])].sum()) - 1.0))
+                res["chains_worst"] = worst
+                res["chains_m_eff"] = [int(x) for x in outR["m_eff"]]
+                res["ok"] = res["ok"] and worst <= max(tol, 1e-6)
         if "batch" in spec:
             # batched chains (L207, L309): R chains in groups of B on interleaved vectors; every chain must be
             # bit-identical to the same chain run alone (same kernel, same tile split) and agree with the oracle

@@ -174,6 +174,20 @@ def test_emu_rowg_64_bit_labels_sampled():
     assert json.loads(p.stdout.strip().splitlines()[-1])["bad"] == 0
 
 
+@pytest.mark.parametrize("spec,fits", [
+    ({"wl": "ring12j", "n_up": 6, "mode": "cr", "prec": "fp64", "steps": 20, "chains": 3}, 1),
+    ({"wl": "ring14", "n_up": 7, "mode": "clt", "prec": "fp32", "steps": 8, "chains": 5}, 1),
+    ({"wl": "ring16", "n_up": 15, "mode": "lin", "prec": "fp32", "steps": 16, "chains": 2}, 1),       # breakdown at step 9
+    ({"wl": "ring16", "n_up": 16, "mode": "cr", "prec": "fp64", "steps": 5}, 1),                        # D = 1
+    ({"wl": "ring16", "n_up": 8, "mode": "cr", "prec": "fp64", "steps": 3}, 0),                         # 3 x 12 870 doubles do not fit: ordinary path
+])
+def test_emu_persistent_chain_kernel(spec, fits):
+    """Option "persistent": all chains of a small sector in one launch, one CTA per chain with the three
+    work vectors in shared memory; alpha, beta, weights against the oracle chain by chain."""
+    res = run_case(dict({"what": ["lanczos"], "options": [["persistent", 1]]}, **spec))
+    assert res["persistent"] == [1, fits]
+
+
 def test_emu_passb_off_keeps_top_bonds_in_tml():
     res = run_case({"wl": "ring16j", "n_up": 8, "mode": "cr", "prec": "fp64",
                     "options": [["passb", 0], ["tml_split", 5 | (3 << 8)], ["kernel", K["tml"]]],
