@@ -20,6 +20,7 @@ namespace {
 
 struct ChainParams {
   int N, K, nb, mode, limit;
+  int labels;                // 1: the row labels are unranked once per chain and kept in shared memory (when they fit)
   int lin_h;
   const uint64_t* lin_hi;
   const uint32_t* lin_lo;
@@ -35,11 +36,13 @@ struct ChainParams {
 
 template <typename R> struct CBond { uint64_t mask; R Jh, Jq; int i, j; };
 
-__host__ __device__ inline size_t chain_smem_bytes(int N, int K, int nb, int64_t dim, int esz, int isz, int bond_sz) {
+// lsz: bytes per stored row label (0 = labels are unranked on the fly every step)
+__host__ __device__ inline size_t chain_smem_bytes(int N, int K, int nb, int64_t dim, int esz, int isz, int bond_sz, int lsz) {
   size_t o = ((size_t)(N + 1) * (K + 1) * isz + 15) & ~(size_t)15;
   o += ((size_t)nb * bond_sz + 15) & ~(size_t)15;
   o += (size_t)96 * 8 + 64;                              // reduction scratch + scalars
   o += 3 * (((size_t)dim * esz + 15) & ~(size_t)15);
+  o += ((size_t)dim * lsz + 15) & ~(size_t)15;
   return o;
 }
 
@@ -58,6 +61,8 @@ lanczos_chain_kernel(ChainParams p, const uint64_t* __restrict__ keys) {
   o += (size_t)96 * 8 + 64;
   const size_t vstride = (((size_t)D * sizeof(R) + 15) & ~(size_t)15) / sizeof(R);
   R* vec = (R*)(smem + o);
+  o += 3 * (((size_t)D * sizeof(R) + 15) & ~(size_t)15);
+  L* lab = (L*)(smem + o);                                 // [D] row labels (only if p.labels)
   for (int k = tid; k < (p.N + 1) * K1; k += NT) ST_S(&s_binom[k], LD_G(&((const I*)p.binom)[k]));
   for (int k = tid; k < p.nb; k += NT) {
     const BondDev b = LD_G(&p.bonds[k]);
@@ -81,6 +86,9 @@ lanczos_chain_kernel(ChainParams p, const uint64_t* __restrict__ keys) {
       ST_S(&vec[(size_t)ip * vstride + t], (R)0);
     }
   }
+  if (p.labels) {                                          // (s_binom was written by other threads: the barrier inside block_sum3 above orders it)
+    for (int t = tid; t < D; t += NT) ST_S(&lab[t], unrank<L, I>((I)t, p.N, K1, p.K, s_binom));
+  }
   __syncthreads();
   int steps = 0;
   for (int j = 0; j < p.limit; ++j) {
@@ -90,7 +98,7 @@ lanczos_chain_kernel(ChainParams p, const uint64_t* __restrict__ keys) {
     const R bprev = (R)s_sc[0];
     double s_qy = 0.0, s_yy = 0.0, s_qq = 0.0;
     for (int t = tid; t < D; t += NT) {
-      const L n = unrank<L, I>((I)t, p.N, K1, p.K, s_binom);
+      const L n = p.labels ? LD_S(&lab[t]) : unrank<L, I>((I)t, p.N, K1, p.K, s_binom);
       R acc = 0, danti = 0;
       for (int b = 0; b < p.nb; ++b) {
         const CBond<R> bd = LD_S(&s_bonds[b]);
@@ -143,7 +151,7 @@ lanczos_chain_kernel(ChainParams p, const uint64_t* __restrict__ keys) {
 bool ftlm_chain_persistent_fits(const ftlm_ctx* c) {
   if (c->dim < 1 || c->dim > (1 << 20)) return false;
   const int isz = c->idx64 ? 8 : 4;
-  const size_t need = chain_smem_bytes(c->N, c->N_up, c->nb, c->dim, (int)ftlm_elem_size(c), isz, c->prec == FTLM_FP32 ? (int)sizeof(CBond<float>) : (int)sizeof(CBond<double>));
+  const size_t need = chain_smem_bytes(c->N, c->N_up, c->nb, c->dim, (int)ftlm_elem_size(c), isz, c->prec == FTLM_FP32 ? (int)sizeof(CBond<float>) : (int)sizeof(CBond<double>), 0);
   return need <= (size_t)227 * 1024 - 1024;
 }
 
@@ -179,14 +187,17 @@ int ftlm_launch_chain_persistent(ftlm_ctx* c, uint64_t seed, int r0, int nchains
   p.binom = c->idx64 ? (const void*)c->d_binom64 : (const void*)c->d_binom32;
   p.bonds = c->d_bonds; p.clt = c->d_clt; p.diag0 = c->diag0; p.tol = c->prec == FTLM_FP32 ? 1e-5 : 1e-12;
   p.alpha = d_alpha; p.beta = d_beta; p.m_eff = d_m_eff;
-  const int isz = c->idx64 ? 8 : 4;
+  const int isz = c->idx64 ? 8 : 4, lsz = c->lab64 ? 8 : 4;
+  const int esz0 = (int)ftlm_elem_size(c), bsz0 = c->prec == FTLM_FP32 ? (int)sizeof(CBond<float>) : (int)sizeof(CBond<double>);
+  p.labels = chain_smem_bytes(c->N, c->N_up, c->nb, c->dim, esz0, isz, bsz0, lsz) <= (size_t)227 * 1024 - 1024 ? 1 : 0;
+  const int lz = p.labels ? lsz : 0;
   if (rc == FTLM_OK) {
     if (c->prec == FTLM_FP32) {
-      const size_t smem = chain_smem_bytes(c->N, c->N_up, c->nb, c->dim, 4, isz, (int)sizeof(CBond<float>));
+      const size_t smem = chain_smem_bytes(c->N, c->N_up, c->nb, c->dim, 4, isz, (int)sizeof(CBond<float>), lz);
       rc = !c->lab64 ? launch_chain<float, uint32_t, uint32_t>(c, p, d_keys, nchains, smem, s)
                      : launch_chain<float, uint64_t, uint32_t>(c, p, d_keys, nchains, smem, s);
     } else {
-      const size_t smem = chain_smem_bytes(c->N, c->N_up, c->nb, c->dim, 8, isz, (int)sizeof(CBond<double>));
+      const size_t smem = chain_smem_bytes(c->N, c->N_up, c->nb, c->dim, 8, isz, (int)sizeof(CBond<double>), lz);
       rc = !c->lab64 ? launch_chain<double, uint32_t, uint32_t>(c, p, d_keys, nchains, smem, s)
                      : launch_chain<double, uint64_t, uint32_t>(c, p, d_keys, nchains, smem, s);
     }

@@ -179,6 +179,7 @@ def test_emu_rowg_64_bit_labels_sampled():
     ({"wl": "ring14", "n_up": 7, "mode": "clt", "prec": "fp32", "steps": 8, "chains": 5}, 1),
     ({"wl": "ring16", "n_up": 15, "mode": "lin", "prec": "fp32", "steps": 16, "chains": 2}, 1),       # breakdown at step 9
     ({"wl": "ring16", "n_up": 16, "mode": "cr", "prec": "fp64", "steps": 5}, 1),                        # D = 1
+    ({"wl": "ring20", "n_up": 5, "mode": "cr", "prec": "fp32", "steps": 4}, 1),                         # D = 15 504: vectors fit, stored labels do not
     ({"wl": "ring16", "n_up": 8, "mode": "cr", "prec": "fp64", "steps": 3}, 0),                         # 3 x 12 870 doubles do not fit: ordinary path
 ])
 def test_emu_persistent_chain_kernel(spec, fits):
