@@ -26,9 +26,9 @@ int ftlm_cuda_fail(cudaError_t e, const char* what) {
 }
 extern "C" const char* ftlm_last_error(void) { return g_err; }
 #ifdef FTLM_CHECKED
-extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.2 (sm_100a) CHECKED"; }
+extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.3 (sm_100a) CHECKED"; }
 #else
-extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.2 (sm_100a)"; }
+extern "C" const char* ftlm_version(void) { return "ftlm-b200 0.3 (sm_100a)"; }
 #endif
 
 // ---- device allocations; checked build: table of live ranges (ftlm_access.cuh) -------------------
