@@ -31,6 +31,22 @@ def test_library_exports_every_declared_symbol():
     assert "sm_100a" in ftlm.ftlm_version()
 
 
+def test_checked_library_exports_the_same_symbols():
+    """libftlm_checked.so (the range-checked build of the same sources: -m gpu pre-flight, bench.py probe, smoke()) exports
+    every declared symbol too and says what it is; it is only inspected here (the binding loads it with FTLM_CHECKED=1)."""
+    import ctypes
+    so = os.path.join(ROOT, "paper_2605_26261_b200", "libftlm_checked.so")
+    if not os.path.exists(so) or ftlm_build.stale(so):
+        pytest.skip("libftlm_checked.so not built (python -m paper_2605_26261_b200.build --checked; __graft_entry__.build() builds it)")
+    L = ctypes.CDLL(so)
+    for name in ftlm.EXPORTS:
+        assert hasattr(L, name), name
+    L.ftlm_version.restype = ctypes.c_char_p
+    assert b"CHECKED" in L.ftlm_version()
+    L.ftlm_get_option.restype = ctypes.c_int64
+    assert L.ftlm_get_option(None, b"check_build") == 1
+
+
 def test_create_validates_arguments_before_touching_the_device():
     for kw, code in [
         (dict(N=0, bond_i=[], bond_j=[], J=[], N_up=0), ftlm.EINVAL),
