@@ -24,7 +24,7 @@ def build(force: bool = False) -> str:
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
+        _lib = C.CDLL(os.environ.get("FTLM_ORACLE_LIB") or build())   # (a sanitizer build of the same file, for tests)
         _lib.orc_enumerate.restype = C.c_int64
         _lib.orc_index.restype = C.c_int64
         _lib.orc_lanczos.restype = C.c_int

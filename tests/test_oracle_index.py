@@ -156,3 +156,35 @@ def test_lin_two_table_map_equals_sorted_search_on_every_label():
     h, Ja, Jb = fo.lin_tables(basis, 10)
     for n in basis[::7]:
         assert fo.lin_lookup_vec([n], 10, 4, h, Ja, Jb)[0] == fo.rank_by_counting(int(n), 10, 4)
+
+
+def test_c_oracle_under_ubsan(tmp_path):
+    """SURVEY section 5 ("ASan/UBSan on oracle"): the C oracle compiled with -fsanitize=undefined,bounds (trap on error)
+    must run its whole interface - enumeration, search, H.v, neighbour lists, Lanczos - on small sectors (incl. the
+    one-state sectors and N = 34 labels) without tripping, and agree with the numpy oracle."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    so = str(tmp_path / "liborc_ubsan.so")
+    subprocess.check_call(["gcc", "-O1", "-g", "-fopenmp", "-shared", "-fPIC", "-fsanitize=undefined,bounds",
+                           "-fsanitize-undefined-trap-on-error", os.path.join(root, "oracle", "ftlm_oracle_c.c"), "-o", so, "-lm"])
+    code = ("import sys; sys.path.insert(0, %r)\n"
+            "import numpy as np\n"
+            "from oracle import c_oracle as co, ftlm_oracle as fo\n"
+            "from paper_2605_26261_b200 import workloads as W\n"
+            "for w, n_up in ((W.ring(12, 1.0, 0.5), 6), (W.ring(9), 0), (W.ring(9), 9), (W.icosahedron(), 7)):\n"
+            "    basis = co.enumerate_basis(w.N, n_up)\n"
+            "    assert (basis == fo.sector_basis(w.N, n_up)).all()\n"
+            "    v = np.random.default_rng(1).standard_normal(basis.shape[0])\n"
+            "    y = co.apply_rows(w.N, w.bond_i, w.bond_j, w.J, 0.2, n_up, basis, v)\n"
+            "    assert np.abs(y - fo.apply_H(basis, w.N, w.bond_i, w.bond_j, w.J, 0.2, n_up, v)).max() < 1e-12\n"
+            "    nb = co.neighbors_rows(w.N, w.bond_i, w.bond_j, basis, np.arange(basis.shape[0], dtype=np.int64))\n"
+            "    assert (nb == fo.neighbor_indices(basis, w.bond_i, w.bond_j, np.arange(basis.shape[0]))).all()\n"
+            "    a, b = co.lanczos(w.N, w.bond_i, w.bond_j, w.J, 0.0, n_up, basis, fo.start_vector(3, n_up, 0, basis.shape[0]), 10)[:2]\n"
+            "    assert np.isfinite(a).all() and np.isfinite(b).all()\n"
+            "lab = np.array([(1 << 34) - 1 - (1 << 20), (1 << 17) - 1, 5], dtype=np.uint64)\n"
+            "assert (co.index_many(co.enumerate_basis(20, 3), np.array([7, 11, 1 << 19], dtype=np.uint64)) == [0, 1, -1]).all()\n"
+            "print('ok')\n" % root)
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600, env=dict(os.environ, FTLM_ORACLE_LIB=so))
+    assert p.returncode == 0 and p.stdout.strip().endswith("ok"), (p.returncode, p.stderr[-1500:])
