@@ -59,3 +59,36 @@ def broadcast_choice(choice, dist=None):
     box = [choice]
     dist.broadcast_object_list(box, src=0)
     return box[0]
+
+
+def save_chain_results(path: str, results: Dict[int, dict], meta: dict | None = None) -> None:
+    """Checkpoint between chains (only alpha, beta survive a chain, L45): the coefficients of the
+    finished chains as JSON - {chain id: {"alpha": [...], "beta": [...], "m_eff": m}} plus free-form `meta` (workload,
+    seed, index mode) - written to a temporary file and renamed, so that an interrupted run leaves the previous file."""
+    import json
+    import os
+    doc = {"meta": meta or {}, "chains": {str(k): {"alpha": [float(x) for x in v["alpha"]], "beta": [float(x) for x in v["beta"]],
+                                                   "m_eff": int(v["m_eff"])} for k, v in sorted(results.items())}}
+    tmp = path + ".tmp"
+    with open(tmp, "w") as f:
+        json.dump(doc, f)
+    os.replace(tmp, path)
+
+
+def load_chain_results(path: str, meta: dict | None = None) -> Dict[int, dict]:
+    """The chains a previous run finished ({} if there is no file); with `meta`, a file written for another workload /
+    seed is refused.  float -> JSON -> float is exact for IEEE doubles (repr round trip)."""
+    import json
+    import os
+    if not os.path.exists(path):
+        return {}
+    with open(path) as f:
+        doc = json.load(f)
+    if meta is not None and doc.get("meta") != meta:
+        raise ValueError(f"{path} belongs to another run: {doc.get('meta')}")
+    return {int(k): v for k, v in doc["chains"].items()}
+
+
+def remaining_chains(n_chains: int, done: Dict[int, dict]) -> List[int]:
+    """Chain ids still to run after a resume."""
+    return [k for k in range(n_chains) if k not in done]

@@ -72,3 +72,24 @@ def test_two_gloo_ranks_gather_chain_results():
     assert d["ranks"] == [k % 2 for k in range(9)]              # round-robin
     assert np.allclose(d["wsum"], 1.0, atol=1e-12)              # sum_k w_k = 1 for every chain
     assert d["t"] == 2.0 and d["choice"] == "tmlr+passb"
+
+
+def test_chain_checkpoint_round_trip(tmp_path):
+    """Resume between chains: coefficients survive JSON exactly, a foreign file is refused, the rest list is right."""
+    import numpy as np
+    from paper_2605_26261_b200 import replicas
+    rng = np.random.default_rng(0)
+    res = {k: {"alpha": rng.standard_normal(7), "beta": np.abs(rng.standard_normal(6)), "m_eff": 7} for k in (0, 2, 5)}
+    path = str(tmp_path / "chains.json")
+    assert replicas.load_chain_results(path) == {}
+    meta = {"workload": "ring16", "seed": 20260526, "mode": "clt"}
+    replicas.save_chain_results(path, res, meta)
+    back = replicas.load_chain_results(path, meta)
+    assert sorted(back) == [0, 2, 5]
+    for k in res:
+        assert back[k]["alpha"] == [float(x) for x in res[k]["alpha"]] and back[k]["m_eff"] == 7
+        assert np.array_equal(np.array(back[k]["beta"]), res[k]["beta"])          # bit-exact round trip
+    assert replicas.remaining_chains(6, back) == [1, 3, 4]
+    import pytest
+    with pytest.raises(ValueError):
+        replicas.load_chain_results(path, dict(meta, seed=1))
