@@ -1,7 +1,7 @@
 // ROW kernels: one thread per sector row, every row unranked, per-bond loop.  This is the
 // paper's launch shape ("assigning one GPU thread to each
 // sector-basis state") written for sm_100a; it is the plain in-library baseline and the path
-// used for index-map queries.  The B200 design proper is in ftlm_tile.cu.
+// used for index-map queries.  The B200 design proper is in ftlm_tml.cu / ftlm_tmlr.cu / ftlm_passb.cu.
 #define FTLM_TU 2
 #include "ftlm_common.cuh"
 #include "ftlm_index.cuh"
